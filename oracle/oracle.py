@@ -1,0 +1,263 @@
+"""ctypes front-end of the CPU oracle (oracle/rga_oracle.cpp).  TEST INFRASTRUCTURE ONLY: imported by tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs; never by the product package.
+
+`avatar_load(inputs)` mirrors step L0 and `render_frame(av, inputs, ...)` runs H1..H10 in the paper's order
+(Fig.1 :84, test-time flow :197) and returns every intermediate as numpy arrays.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.orc_emit_sort.restype = C.c_int64
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def set_threads(n):
+    os.environ["OMP_NUM_THREADS"] = str(n)
+
+
+# ------------------------------------------------------------------------------------------------ steps
+def knn(q, v, K):
+    q, v = _f32(q), _f32(v)
+    idx = np.empty((len(q), K), np.int32); d2 = np.empty((len(q), K), np.float32)
+    lib().orc_knn(_p(q), C.c_int(len(q)), _p(v), C.c_int(len(v)), C.c_int(K), _p(idx), _p(d2))
+    return idx, d2
+
+
+def interp_weights(d2):
+    d2 = _f32(d2); out = np.empty_like(d2)
+    lib().orc_interp_weights(_p(d2), C.c_int(d2.shape[0]), C.c_int(d2.shape[1]), _p(out))
+    return out
+
+
+def interp_attr(idx, ubar, attr):
+    attr = _f32(attr)
+    a2 = attr.reshape(len(attr), -1)
+    out = np.empty((len(idx), a2.shape[1]), np.float32)
+    lib().orc_interp_attr(_p(idx), _p(ubar), C.c_int(len(idx)), C.c_int(idx.shape[1]), _p(a2), C.c_int(a2.shape[1]), _p(out))
+    return out.reshape((len(idx),) + attr.shape[1:])
+
+
+def normalize_rows3(v):
+    v = _f32(v).copy()
+    lib().orc_normalize_rows3(_p(v), C.c_int(len(v)))
+    return v
+
+
+def skin(x, dx, n, w, G):
+    x, n, w, G = _f32(x), _f32(n), _f32(w), _f32(G)
+    dx = None if dx is None else _f32(dx)
+    xo = np.empty_like(x); no = np.empty_like(x); M = np.empty((len(x), 12), np.float32)
+    lib().orc_skin(_p(x), _p(dx), _p(n), _p(w), C.c_int(len(x)), C.c_int(w.shape[1]), _p(G), _p(xo), _p(no), _p(M))
+    return xo, no, M
+
+
+def gauss_cov(M, q, s):
+    M, q, s = _f32(M), _f32(q), _f32(s)
+    out = np.empty((len(q), 6), np.float32)
+    lib().orc_gauss_cov(_p(M), _p(q), _p(s), C.c_int(len(q)), _p(out))
+    return out
+
+
+def window(x):
+    x = _f32(x); c = np.empty(3, np.float32); r = C.c_float(0)
+    lib().orc_window(_p(x), C.c_int(len(x)), _p(c), C.byref(r))
+    return c, np.float32(r.value)
+
+
+def light_frames(dirs):
+    dirs = _f32(dirs); out = np.empty((len(dirs), 9), np.float32)
+    lib().orc_light_frames(_p(dirs), C.c_int(len(dirs)), _p(out))
+    return out
+
+
+def vis_raster(xp, faces, dirs, R, c, r, want_ids=True):
+    xp, dirs, c = _f32(xp), _f32(dirs), _f32(c)
+    faces = np.ascontiguousarray(faces, np.int32)
+    K = len(dirs)
+    z = np.empty((K, R, R), np.uint32)
+    ids = np.empty((K, R, R), np.int32) if want_ids else None
+    lib().orc_vis_raster(_p(xp), C.c_int(len(xp)), _p(faces), C.c_int(len(faces)), _p(dirs), C.c_int(K), C.c_int(R),
+                         _p(c), C.c_float(r), _p(z), _p(ids))
+    return z, ids
+
+
+def vis_depth_test(xg, ng, dirs, R, c, r, zmap, bias_texels, bias_world, slope_max):
+    xg, ng, dirs, c = _f32(xg), _f32(ng), _f32(dirs), _f32(c)
+    K = len(dirs)
+    bits = np.empty((len(xg), (K + 31) // 32), np.uint32)
+    lib().orc_vis_depth_test(_p(xg), _p(ng), C.c_int(len(xg)), _p(dirs), C.c_int(K), C.c_int(R), _p(c), C.c_float(r),
+                             _p(zmap), C.c_float(bias_texels), C.c_float(bias_world), C.c_float(slope_max), _p(bits))
+    return bits
+
+
+def vis_paper(idmap, faces, nv, knn_v, want_stages=False):
+    K, R = idmap.shape[0], idmap.shape[1]
+    faces = np.ascontiguousarray(faces, np.int32)
+    vcount = np.empty((nv, K), np.uint8)
+    st = [np.empty((K, nv), np.uint8) for _ in range(3)] if want_stages else [None] * 3
+    lib().orc_vis_paper(_p(idmap), _p(faces), C.c_int(len(faces)), C.c_int(nv), C.c_int(K), C.c_int(R), _p(knn_v),
+                        C.c_int(knn_v.shape[1]), _p(vcount), _p(st[0]), _p(st[1]), _p(st[2]))
+    return (vcount, st) if want_stages else vcount
+
+
+def vis_gauss(vcount, knn_g, ubar, Kv):
+    ng, K = len(knn_g), vcount.shape[1]
+    out = np.empty((ng, K), np.float64)
+    lib().orc_vis_gauss(_p(vcount), _p(knn_g), _p(ubar), C.c_int(ng), C.c_int(knn_g.shape[1]), C.c_int(K), C.c_int(Kv), _p(out))
+    return out
+
+
+def env_table(rows, cols):
+    w = np.empty((rows * cols, 3), np.float64); A = np.empty(rows * cols, np.float64)
+    lib().orc_env_table(C.c_int(rows), C.c_int(cols), _p(w), _p(A))
+    return w, A
+
+
+def brdf(wi, wo, n, albedo, rough, spec):
+    a = [np.ascontiguousarray(v, np.float64) for v in (wi, wo, n, albedo)]
+    out = np.empty(3, np.float64)
+    lib().orc_brdf(_p(a[0]), _p(a[1]), _p(a[2]), _p(a[3]), C.c_double(rough), C.c_double(spec), _p(out))
+    return out
+
+
+def shade(xg, ng, alb, rough, spec, cam_pos, env, t2d, vis_mode, bits=None, vg=None, K=0, gamma=2.2):
+    xg, ng, alb, rough, spec, cam_pos, env = map(_f32, (xg, ng, alb, rough, spec, cam_pos, env))
+    rows, cols = env.shape[0], env.shape[1]
+    n = len(xg)
+    Lo = np.empty((n, 3), np.float64); cg = np.empty((n, 3), np.float64)
+    t2d = None if t2d is None else np.ascontiguousarray(t2d, np.int32)
+    lib().orc_shade(_p(xg), _p(ng), _p(alb), _p(rough), _p(spec), C.c_int(n), _p(cam_pos), _p(env), C.c_int(rows),
+                    C.c_int(cols), _p(t2d), C.c_int(vis_mode), _p(bits), _p(vg), C.c_int(K), C.c_double(gamma), _p(Lo), _p(cg))
+    return Lo, cg
+
+
+def camera_array(cam):
+    return np.concatenate([_f32(cam["R_wc"]).reshape(9), _f32(cam["t_wc"]).reshape(3),
+                           np.array([cam["fx"], cam["fy"], cam["cx"], cam["cy"], cam["width"], cam["height"],
+                                     cam["z_near"]], np.float32)]).astype(np.float32)
+
+
+def project(xg, ng, cov6, opac, cam):
+    xg, ng, cov6 = _f32(xg), _f32(ng), _f32(cov6)
+    opac = None if opac is None else _f32(opac)
+    n = len(xg); ca = camera_array(cam)
+    o = dict(mu=np.empty((n, 2), np.float32), depth=np.empty(n, np.float32), conic_o=np.empty((n, 4), np.float32),
+             rect=np.empty((n, 4), np.int32), touched=np.empty(n, np.uint32), radius=np.empty(n, np.int32))
+    lib().orc_project(_p(xg), _p(ng), _p(cov6), _p(opac), C.c_int(n), _p(ca), _p(o["mu"]), _p(o["depth"]),
+                      _p(o["conic_o"]), _p(o["rect"]), _p(o["touched"]), _p(o["radius"]))
+    return o
+
+
+def emit_sort(depth, rect, touched, TX):
+    D = int(touched.astype(np.int64).sum())
+    keys = np.empty(max(D, 1), np.uint64); vals = np.empty(max(D, 1), np.uint32)
+    d = lib().orc_emit_sort(_p(depth), _p(rect), _p(touched), C.c_int(len(depth)), C.c_int(TX), _p(keys), _p(vals))
+    assert d == D
+    return keys[:D], vals[:D]
+
+
+def tile_ranges(keys, ntiles):
+    r = np.zeros((ntiles, 2), np.uint32)
+    k = np.ascontiguousarray(keys, np.uint64)
+    lib().orc_tile_ranges(_p(k), C.c_int64(len(k)), C.c_int(ntiles), _p(r))
+    return r
+
+
+def composite(vals, ranges, mu, conic_o, col, bg, W, H):
+    col = np.ascontiguousarray(col, np.float64); bg = _f32(bg)
+    vals = np.ascontiguousarray(vals, np.uint32)
+    if len(vals) == 0:
+        vals = np.zeros(1, np.uint32)
+    img = np.empty((H, W, 3), np.float64); T = np.empty((H, W), np.float64)
+    nc = np.empty((H, W), np.uint32); fl = np.empty((H, W), np.uint8)
+    lib().orc_composite(_p(vals), _p(ranges), _p(mu), _p(conic_o), _p(col), _p(bg), C.c_int(W), C.c_int(H), _p(img),
+                        _p(T), _p(nc), _p(fl))
+    return img, T, nc, fl
+
+
+def composite_bruteforce(depth, rect, touched, mu, conic_o, col, bg, W, H):
+    col = np.ascontiguousarray(col, np.float64); bg = _f32(bg)
+    img = np.empty((H, W, 3), np.float64); T = np.empty((H, W), np.float64); nc = np.empty((H, W), np.uint32)
+    lib().orc_composite_bruteforce(_p(depth), _p(rect), _p(touched), C.c_int(len(depth)), _p(mu), _p(conic_o), _p(col),
+                                   _p(bg), C.c_int(W), C.c_int(H), _p(img), _p(T), _p(nc))
+    return img, T, nc
+
+
+# ------------------------------------------------------------------------------------------------ pipeline
+K_G, K_V = 3, 19
+
+
+def avatar_load(inp):
+    """L0: KNN sets S_g, S_v and Eq.1 interpolation of the pose-independent attributes."""
+    av = {}
+    av["knn_g"], d2g = knn(inp["gauss_pos"], inp["vert_pos"], K_G)
+    av["ubar_g"] = interp_weights(d2g)
+    kv = min(K_V, len(inp["vert_pos"]))
+    av["knn_v"], _ = knn(inp["vert_pos"], inp["vert_pos"], kv)
+    i, u = av["knn_g"], av["ubar_g"]
+    av["normal_g"] = normalize_rows3(interp_attr(i, u, inp["vert_normal"]))
+    av["albedo_g"] = interp_attr(i, u, inp["vert_albedo"])
+    av["rough_g"] = interp_attr(i, u, inp["vert_rough"])
+    av["spec_g"] = interp_attr(i, u, inp["vert_spec"])
+    av["skin_w_g"] = interp_attr(i, u, inp["vert_skin_w"])
+    av["disp_g"] = interp_attr(i, u, inp["vert_disp"])
+    return av
+
+
+def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None):
+    """H1..H10.  vis_mode 0 = depth test (north_star), 1 = paper (Eq.3-4), 2 = no visibility (v = 1)."""
+    o = {}
+    G = inp["bone_mats"][frame]
+    o["vert_posed"], o["vert_normal_posed"], _ = skin(inp["vert_pos"], inp["vert_disp"], inp["vert_normal"],
+                                                      inp["vert_skin_w"], G)
+    o["gauss_posed"], o["gauss_normal_posed"], M = skin(inp["gauss_pos"], av["disp_g"], av["normal_g"], av["skin_w_g"], G)
+    o["cov6"] = gauss_cov(M, inp["gauss_quat"], inp["gauss_scale"])
+    o["win_c"], o["win_r"] = window(o["vert_posed"])
+    if stop_after == "skin":
+        return o
+    dirs, R = inp["vis_dirs"], inp["vis_res"]
+    K = len(dirs)
+    bits = vg = None
+    if vis_mode in (0, 1):
+        o["zmap"], o["idmap"] = vis_raster(o["vert_posed"], inp["faces"], dirs, R, o["win_c"], o["win_r"], want_ids=True)
+    if vis_mode == 0:
+        bits = o["visbits"] = vis_depth_test(o["gauss_posed"], o["gauss_normal_posed"], dirs, R, o["win_c"], o["win_r"],
+                                             o["zmap"], inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
+    elif vis_mode == 1:
+        o["vcount"] = vis_paper(o["idmap"], inp["faces"], len(inp["vert_pos"]), av["knn_v"])
+        vg = o["vis_g"] = vis_gauss(o["vcount"], av["knn_g"], av["ubar_g"], av["knn_v"].shape[1])
+    if stop_after == "vis":
+        return o
+    env = inp["env"][inp["env_of_frame"][frame]]
+    o["L_o"], o["color"] = shade(o["gauss_posed"], o["gauss_normal_posed"], av["albedo_g"], av["rough_g"], av["spec_g"],
+                                 inp["cam_pos"], env, inp["texel_to_dir"], vis_mode, bits, vg, K, inp["gamma"])
+    if stop_after == "shade":
+        return o
+    cam = camera or inp["camera"]
+    W, H = cam["width"], cam["height"]
+    TX, TY = (W + 15) // 16, (H + 15) // 16
+    o.update(project(o["gauss_posed"], o["gauss_normal_posed"], o["cov6"], inp["gauss_opacity"], cam))
+    o["keys"], o["vals"] = emit_sort(o["depth"], o["rect"], o["touched"], TX)
+    o["ranges"] = tile_ranges(o["keys"], TX * TY)
+    o["image"], o["T_final"], o["n_contrib"], o["flags"] = composite(o["vals"], o["ranges"], o["mu"], o["conic_o"],
+                                                                     o["color"], inp["bg"], W, H)
+    return o

@@ -1,0 +1,402 @@
+"""Pins for the CPU oracle (oracle/): each check ties one oracle function to something OTHER than itself --
+a closed form, a library routine, an invariant, a brute force on tiny inputs -- so that a dropped term, wrong
+sign/index or transposed operand fails here.  No GPU.  Citations are PAPER.md lines / DESIGN.md readings."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from synth import mesh as smesh
+from synth import workloads
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _golden(name):
+    rows = []
+    for line in open(os.path.join(GOLD, name)):
+        line = line.split("#")[0].strip()
+        if line:
+            rows.append([float(t) for t in line.split()])
+    return np.array(rows)
+
+
+# ------------------------------------------------------------------ L0: KNN + Eq.1
+def test_knn_matches_kdtree_and_tie_rule():
+    from scipy.spatial import cKDTree
+    r = np.random.default_rng(1)
+    v = r.normal(size=(500, 3)).astype(np.float32)
+    q = r.normal(size=(200, 3)).astype(np.float32)
+    idx, d2 = orc.knn(q, v, 19)
+    _, ref = cKDTree(v.astype(np.float64)).query(q.astype(np.float64), k=19)
+    assert (np.sort(idx, 1) == np.sort(ref, 1)).mean() > 0.999          # library routine (fp64) agrees
+    assert np.all(np.diff(d2, axis=1) >= 0)
+    # ties: integer lattice, many equal distances -> lower index first (PAPER.md silent; L0)
+    g = np.stack(np.meshgrid(*[np.arange(4)] * 3, indexing="ij"), -1).reshape(-1, 3).astype(np.float32)
+    idx, d2 = orc.knn(g, g, 7)
+    D = ((g[:, None] - g[None]) ** 2).sum(-1)
+    ref = np.argsort(D, axis=1, kind="stable")[:, :7]
+    assert np.array_equal(idx, ref)
+    assert np.array_equal(idx[:, 0], np.arange(len(g)))                 # self is its own nearest (A15)
+
+
+def test_eq1_weights_hand_example_and_constant_field():
+    # u_j = 1/||x_g - x_j||.  Distances 1,2,4 -> u = 1, 1/2, 1/4 -> ubar = 4/7, 2/7, 1/7.
+    v = np.array([[1, 0, 0], [0, 2, 0], [0, 0, 4], [9, 9, 9]], np.float32)
+    q = np.zeros((1, 3), np.float32)
+    idx, d2 = orc.knn(q, v, 3)
+    ub = orc.interp_weights(d2)
+    assert idx.tolist() == [[0, 1, 2]]
+    np.testing.assert_allclose(ub[0], [4 / 7, 2 / 7, 1 / 7], rtol=1e-6)
+    attr = np.array([[7.0], [14.0], [28.0], [0.0]], np.float32)
+    np.testing.assert_allclose(orc.interp_attr(idx, ub, attr)[0, 0], 4 + 4 + 4, rtol=1e-6)
+    r = np.random.default_rng(2)
+    v = r.normal(size=(300, 3)).astype(np.float32); q = r.normal(size=(50, 3)).astype(np.float32)
+    idx, d2 = orc.knn(q, v, 3); ub = orc.interp_weights(d2)
+    np.testing.assert_allclose(ub.sum(1), 1.0, atol=2e-7)
+    const = np.full((300, 5), 3.25, np.float32)
+    np.testing.assert_allclose(orc.interp_attr(idx, ub, const), 3.25, rtol=3e-7)
+    # a Gaussian sitting exactly on a vertex takes that vertex's value (distance clamp, A1)
+    idx, d2 = orc.knn(v[:4], v, 3); ub = orc.interp_weights(d2)
+    lin = v @ np.array([1.0, 2.0, 3.0], np.float32)
+    np.testing.assert_allclose(orc.interp_attr(idx, ub, lin[:, None])[:, 0], lin[:4], rtol=1e-5)
+
+
+# ------------------------------------------------------------------ H1/H2: skinning
+def _rigid(r):
+    A = r.normal(size=(3, 3)); Q, _ = np.linalg.qr(A)
+    if np.linalg.det(Q) < 0:
+        Q[:, 0] *= -1
+    return np.concatenate([Q, r.normal(size=(3, 1))], 1)
+
+
+def test_skin_identity_rigid_and_blend():
+    r = np.random.default_rng(3)
+    n, B = 64, 5
+    x = r.normal(size=(n, 3)).astype(np.float32); dx = (0.01 * r.normal(size=(n, 3))).astype(np.float32)
+    nr = r.normal(size=(n, 3)); nr = (nr / np.linalg.norm(nr, axis=1, keepdims=True)).astype(np.float32)
+    w = r.uniform(size=(n, B)).astype(np.float32); w /= w.sum(1, keepdims=True)
+    I = np.tile(np.eye(3, 4).reshape(12), (B, 1)).astype(np.float32)
+    xo, no, _ = orc.skin(x, dx, nr, np.eye(B, dtype=np.float32)[r.integers(0, B, n)], I)
+    assert np.array_equal(xo, x + dx)                                   # identity pose: bit-exact x + dx
+    G = _rigid(r)
+    xo, no, M = orc.skin(x, dx, nr, w, np.tile(G.reshape(12), (B, 1)).astype(np.float32))
+    xb = (x + dx).astype(np.float64)
+    np.testing.assert_allclose(xo, xb @ G[:, :3].T + G[:, 3], atol=2e-6)   # partition of unity
+    np.testing.assert_allclose(no, nr.astype(np.float64) @ G[:, :3].T, atol=2e-6)
+    # covariance under a rigid bone: eigenvalues = s^2 (rotation invariance, A3)
+    q = r.normal(size=(n, 4)).astype(np.float32); s = np.exp(r.uniform(-5, -3, (n, 3))).astype(np.float32)
+    c6 = orc.gauss_cov(M, q, s).astype(np.float64)
+    S = np.zeros((n, 3, 3)); iu = [(0, 0), (0, 1), (0, 2), (1, 1), (1, 2), (2, 2)]
+    for k, (a, b) in enumerate(iu):
+        S[:, a, b] = c6[:, k]; S[:, b, a] = c6[:, k]
+    ev = np.linalg.eigvalsh(S)
+    np.testing.assert_allclose(ev, np.sort(s.astype(np.float64) ** 2, 1), rtol=2e-4)
+    # two translating bones, weights 1/4, 3/4 -> x + t1/4 + 3 t2/4 (hand example of linear blend)
+    G2 = np.tile(np.eye(3, 4), (2, 1, 1)); G2[0, :, 3] = [4, 0, 0]; G2[1, :, 3] = [0, 8, 0]
+    xo, _, _ = orc.skin(np.zeros((1, 3), np.float32), None, np.array([[0, 0, 1]], np.float32),
+                        np.array([[0.25, 0.75]], np.float32), G2.reshape(2, 12).astype(np.float32))
+    assert xo.tolist() == [[1.0, 6.0, 0.0]]
+
+
+def test_cov_axis_aligned_quaternion():
+    # q = (cos 45deg, 0, 0, sin 45deg): rotation by 90deg about z sends x->y: Sigma = diag(s_y^2, s_x^2, s_z^2)
+    M = np.eye(3, 4, dtype=np.float32).reshape(1, 12)
+    q = np.array([[np.sqrt(0.5), 0, 0, np.sqrt(0.5)]], np.float32)
+    c6 = orc.gauss_cov(M, q, np.array([[1.0, 2.0, 3.0]], np.float32))[0]
+    np.testing.assert_allclose(c6, [4, 0, 0, 1, 0, 9], atol=1e-5)
+
+
+# ------------------------------------------------------------------ env quadrature + BRDF + shading
+def test_env_quadrature_closed_forms():
+    for (R, C) in [(8, 16), (16, 32), (32, 64)]:
+        w, A = orc.env_table(R, C)
+        np.testing.assert_allclose(A.sum(), 4 * np.pi, rtol=1e-12)      # exact solid angles (A6)
+        np.testing.assert_allclose((A[:, None] * w).sum(0), 0, atol=1e-12)
+        np.testing.assert_allclose(np.linalg.norm(w, axis=1), 1, atol=1e-12)
+    w, A = orc.env_table(16, 32)
+    assert w[0, 2] > 0.99 and w[-1, 2] < -0.99                          # row 0 = +z pole (z-up)
+    # texel (8,0): theta just past the equator, phi = pi/32
+    np.testing.assert_allclose(w[8 * 32], [np.sin(8.5 * np.pi / 16) * np.cos(np.pi / 32),
+                                            np.sin(8.5 * np.pi / 16) * np.sin(np.pi / 32), np.cos(8.5 * np.pi / 16)], atol=1e-12)
+
+
+def test_brdf_normal_incidence_golden():
+    # Closed form of Eq.12-15 at w_i = w_o = n: D = 1/(pi a^2), G1 = 1, F = .04 + .96 2^-12.53789
+    n = np.array([0, 0, 1.0])
+    for rough, spec_gold in _golden("brdf_normal_incidence.txt"):
+        R = orc.brdf(n, n, n, np.zeros(3), rough, 1.0)
+        np.testing.assert_allclose(R, spec_gold, rtol=2e-4)
+    R = orc.brdf(n, n, n, np.array([0.2, 0.4, 0.6]), 0.5, 0.0)
+    np.testing.assert_allclose(R, np.array([0.2, 0.4, 0.6]) / np.pi, rtol=1e-12)    # Lambert term a/pi
+
+
+def test_brdf_reciprocity_ndf_normalisation_fresnel():
+    r = np.random.default_rng(5)
+    n = np.array([0, 0, 1.0])
+    for _ in range(50):
+        a = r.normal(size=3); a[2] = abs(a[2]) + 0.05; a /= np.linalg.norm(a)
+        b = r.normal(size=3); b[2] = abs(b[2]) + 0.05; b /= np.linalg.norm(b)
+        rough = r.uniform(0.1, 1)
+        np.testing.assert_allclose(orc.brdf(a, b, n, np.ones(3), rough, 0.7), orc.brdf(b, a, n, np.ones(3), rough, 0.7), rtol=1e-10)
+    # NDF normalisation: with w_i = w_o = h,  D(h) = R 4 ((n.h)(1-k)+k)^2 / F(1);  integral D (n.h) dh = 1 (GGX)
+    for rough in (0.3, 0.5, 1.0):
+        k = (rough + 1) ** 2 / 8
+        F1 = 0.04 + 0.96 * 2 ** (-5.55473 - 6.98316)
+        th = (np.arange(20000) + 0.5) * (np.pi / 2) / 20000
+        D = np.array([orc.brdf(h, h, n, np.zeros(3), rough, 1.0)[0] for h in
+                      np.stack([np.sin(th), 0 * th, np.cos(th)], 1)]) * 4 * (np.cos(th) * (1 - k) + k) ** 2 / F1
+        integral = (D * np.cos(th) * np.sin(th)).sum() * (np.pi / 2 / 20000) * 2 * np.pi
+        np.testing.assert_allclose(integral, 1.0, rtol=2e-4)
+    # gamma = 1 -> alpha = 1 -> D = 1/pi for every h
+    h = np.array([np.sin(0.7), 0, np.cos(0.7)])
+    k = 0.5
+    np.testing.assert_allclose(orc.brdf(h, h, n, np.zeros(3), 1.0, 1.0)[0] * 4 * (h[2] * (1 - k) + k) ** 2 / F1, 1 / np.pi, rtol=1e-10)
+    # spherical-Gaussian Fresnel stays within 0.004 of Schlick's (1-x)^5 (UE4 approximation, Eq.14)
+    x = np.linspace(0, 1, 1001)
+    assert np.abs((0.04 + 0.96 * 2 ** ((-5.55473 * x - 6.98316) * x)) - (0.04 + 0.96 * (1 - x) ** 5)).max() < 0.004
+
+
+def test_white_furnace_lambert():
+    # north_star pin: constant white env, full visibility, Lambertian (p = 0): L_o = a E(n) / pi,
+    # E(n) = sum_k A_k max(0, n.w_k) by an independent loop; E/pi -> 1 within the quadrature error of the grid.
+    r = np.random.default_rng(6)
+    n = r.normal(size=(300, 3)); n = (n / np.linalg.norm(n, axis=1, keepdims=True)).astype(np.float32)
+    x = (0.1 * r.normal(size=(300, 3))).astype(np.float32)
+    alb = r.uniform(size=(300, 3)).astype(np.float32)
+    for (R, C, lo, hi) in [(16, 32, 0.995, 1.005), (8, 16, 0.98, 1.02), (32, 64, 0.9985, 1.0015)]:
+        env = np.ones((R, C, 3), np.float32)
+        Lo, cg = orc.shade(x, n, alb, np.full(300, 0.5, np.float32), np.zeros(300, np.float32), np.array([0, -5, 0], np.float32),
+                           env, None, 2)
+        th = (np.arange(R) + 0.5) * np.pi / R; ph = (np.arange(C) + 0.5) * 2 * np.pi / C
+        E = np.zeros(300)
+        for i in range(R):
+            A = (np.cos(i * np.pi / R) - np.cos((i + 1) * np.pi / R)) * 2 * np.pi / C
+            for j in range(C):
+                wk = np.array([np.sin(th[i]) * np.cos(ph[j]), np.sin(th[i]) * np.sin(ph[j]), np.cos(th[i])])
+                E += A * np.maximum(0, n.astype(np.float64) @ wk)
+        np.testing.assert_allclose(Lo, alb.astype(np.float64) * E[:, None] / np.pi, rtol=1e-9)
+        assert lo <= (E / np.pi).min() and (E / np.pi).max() <= hi
+        np.testing.assert_allclose(cg, np.clip(Lo, 0, 1) ** (1 / 2.2), rtol=1e-12)       # gamma (A9, unpinned value)
+
+
+def test_shade_single_light_hand_example():
+    # One bright texel, everything else black: L_o = L A R cos (Eq.2 with a single term), visibility bit gates it.
+    R_, C_ = 8, 16
+    w, A = orc.env_table(R_, C_)
+    k = 2 * C_ + 3
+    env = np.zeros((R_, C_, 3), np.float32); env[2, 3] = [2.0, 3.0, 4.0]
+    n = np.array([[0, 0, 1.0]], np.float32); x = np.zeros((1, 3), np.float32)
+    cam = np.array([0, -3.0, 4.0], np.float32); wo = cam / np.linalg.norm(cam)
+    alb = np.array([[0.5, 0.6, 0.7]], np.float32)
+    Rr = orc.brdf(w[k], wo.astype(np.float64), n[0].astype(np.float64), alb[0].astype(np.float64), 0.4, 0.8)
+    bits = np.zeros((1, 4), np.uint32); bits[0, k >> 5] = 1 << (k & 31)
+    Lo, _ = orc.shade(x, n, alb, np.array([0.4], np.float32), np.array([0.8], np.float32), cam, env, None, 0, bits=bits, K=128)
+    np.testing.assert_allclose(Lo[0], np.array([2.0, 3.0, 4.0]) * A[k] * Rr * w[k, 2], rtol=1e-7)
+    Lo0, _ = orc.shade(x, n, alb, np.array([0.4], np.float32), np.array([0.8], np.float32), cam, env, None, 0,
+                       bits=np.zeros((1, 4), np.uint32), K=128)
+    assert np.all(Lo0 == 0)                                             # shadowed -> no light
+
+
+# ------------------------------------------------------------------ H3/H4: visibility
+def _ray_tri_depth(orig, w, v, f):
+    """Nearest hit parameter of rays orig - t*w ... brute-force double Moeller-Trumbore; returns max over w.(p-c)."""
+    best = np.full(len(orig), -np.inf)
+    hit = np.zeros(len(orig), bool)
+    for t in f:
+        a, b, c = v[t[0]], v[t[1]], v[t[2]]
+        e1, e2 = b - a, c - a
+        d = -w
+        pv = np.cross(d, e2); det = e1 @ pv
+        if abs(det) < 1e-14:
+            continue
+        tv = orig - a
+        uu = (tv @ pv) / det
+        qv = np.cross(tv, e1)
+        vv = (qv @ d) / det
+        tt = (qv @ e2) / det
+        ok = (uu >= -1e-9) & (vv >= -1e-9) & (uu + vv <= 1 + 1e-9)
+        dep = (orig + tt[:, None] * d) @ w
+        upd = ok & (dep > best)
+        best[upd] = dep[upd]; hit |= ok
+    return best, hit
+
+
+def test_depth_map_equals_bruteforce_rays_tiny_mesh():
+    v, f = smesh.icosphere(1)
+    v = (v * np.array([1.0, 0.7, 0.5]) + np.array([0.1, -0.2, 0.3])).astype(np.float32)
+    dirs = workloads.latlong_dirs(2, 4)[[0, 3, 5, 6]]
+    R = 24
+    c, r = orc.window(v)
+    zmap, ids = orc.vis_raster(v, f, dirs, R, c, r)
+    fr = orc.light_frames(dirs).astype(np.float64)
+    vd = v.astype(np.float64)
+    for k in range(len(dirs)):
+        u, vv, w = fr[k, :3], fr[k, 3:6], fr[k, 6:]
+        ii, jj = np.meshgrid(np.arange(R), np.arange(R), indexing="xy")
+        pu = ((ii.reshape(-1) + 0.5) / R * 2 - 1) * r; pv = ((jj.reshape(-1) + 0.5) / R * 2 - 1) * r
+        orig = c.astype(np.float64) + pu[:, None] * u + pv[:, None] * vv
+        dep, hit = _ray_tri_depth(orig, w, vd, f)
+        z = zmap[k].reshape(-1); zf = z.view(np.float32).astype(np.float64)
+        covered = z != 0xFFFFFFFF
+        # coverage agrees except for pixel centres within a subpixel snap of a silhouette edge
+        assert (covered != hit).mean() < 0.03
+        both = covered & hit
+        zref = (r - (dep - c.astype(np.float64) @ w)) / (2 * r)
+        err = np.abs(zf[both] - zref[both])
+        assert np.quantile(err, 0.97) < 2e-3 and np.median(err) < 2e-4     # snap = 1/256 px of a 24 px map
+        assert both.sum() > 50
+    assert ids.max() < len(f) and ids.min() >= -1
+
+
+def test_depth_test_convex_body_pin():
+    # Convex body (unposed icosphere): a surface point sees w iff n.w > 0.  One-sided checks (A17).
+    inp = workloads.make(0)
+    inp["bone_mats"][0] = np.tile(np.eye(3, 4).reshape(12), (2, 1))
+    av = orc.avatar_load(inp)
+    o = orc.render_frame(av, inp, vis_mode=0, stop_after="vis")
+    K = len(inp["vis_dirs"])
+    bits = ((o["visbits"][:, :, None] >> np.arange(32)[None, None, :]) & 1).reshape(len(o["visbits"]), -1)[:, :K]
+    # outward normal of the sphere at the Gaussian
+    nx = o["gauss_posed"] / np.linalg.norm(o["gauss_posed"], axis=1, keepdims=True)
+    cs = nx @ inp["vis_dirs"].T
+    assert np.all(bits[cs > 0.02] == 1)           # no false self-shadow on the lit side
+    assert np.all(bits[cs < -0.4] == 0)           # far side is shadowed
+    assert 0.4 < bits.mean() < 0.65
+
+
+def test_paper_visibility_filters_and_convex_pin(cfg0):
+    inp = dict(cfg0); inp["bone_mats"] = cfg0["bone_mats"].copy()
+    inp["bone_mats"][0] = np.tile(np.eye(3, 4).reshape(12), (2, 1))
+    av = orc.avatar_load(inp)
+    o = orc.render_frame(av, inp, vis_mode=1, stop_after="vis")
+    nv = len(inp["vert_pos"])
+    vcount, (raw, m1, m2) = orc.vis_paper(o["idmap"], inp["faces"], nv, av["knn_v"], want_stages=True)
+    assert vcount.max() <= 19 and np.array_equal(vcount, o["vcount"])
+    knn = av["knn_v"]
+    # brute-force re-evaluation of Eq.3-4 with numpy
+    med = lambda V: (V[:, knn].sum(-1) * 2 > knn.shape[1]).astype(np.uint8)
+    assert np.array_equal(m1, med(raw)) and np.array_equal(m2, med(m1))
+    assert np.array_equal(vcount, m2[:, knn].sum(-1).T)
+    # raw bits = "triangle appears in the image -> its three vertices"
+    k = 3
+    tri = np.unique(o["idmap"][k][o["idmap"][k] >= 0])
+    ref = np.zeros(nv, np.uint8); ref[inp["faces"][tri].reshape(-1)] = 1
+    assert np.array_equal(raw[k], ref)
+    # convex pin: filtered value ~1 on the clearly lit side, exactly 0 on the far side
+    cs = inp["vert_normal"] @ inp["vis_dirs"].T
+    vbar = vcount / 19.0
+    assert vbar[cs > 0.5].min() >= 0.94
+    assert np.all(raw.T[cs < -0.1] == 0)          # no triangle facing away ever wins a pixel on a convex body
+    assert np.all(vbar[cs < -0.45] == 0)          # the 19-neighbourhood of a 642-vertex sphere spans ~0.35 in n.w
+    # fixed points: all-ones / all-zeros maps survive median and mean
+    ones = np.full((1, 8, 8), 0, np.int32)          # every pixel won by triangle 0 ...
+    allv = orc.vis_paper(np.zeros((1, 4, 4), np.int32) - 1, inp["faces"], nv, knn)
+    assert np.all(allv == 0)
+    vg = orc.vis_gauss(vcount, av["knn_g"], av["ubar_g"], 19)
+    assert vg.min() >= 0 and vg.max() <= 1 + 1e-6
+
+
+# ------------------------------------------------------------------ H6-H10: splatting
+def _one_gauss_inputs(s=0.05, z=4.0, o=0.8, W=64, H=64, f=80.0):
+    cam = dict(R_wc=np.eye(3, dtype=np.float32).reshape(9), t_wc=np.zeros(3, np.float32), fx=np.float32(f), fy=np.float32(f),
+               cx=np.float32(W / 2), cy=np.float32(H / 2), width=W, height=H, z_near=np.float32(0.2))
+    x = np.array([[0, 0, z]], np.float32); n = np.array([[0, 0, -1.0]], np.float32)
+    cov = np.array([[s * s, 0, 0, s * s, 0, s * s]], np.float32)
+    return cam, x, n, cov, np.array([o], np.float32)
+
+
+def test_single_isotropic_gaussian_matches_analytic():
+    # north_star pin: on-axis isotropic splat = c min(0.99, o exp(-|p-mu|^2 / (2 s'^2))), s'^2 = (f s / z)^2 + 0.3
+    s, z, o, W, H, f = 0.05, 4.0, 0.8, 64, 64, 80.0
+    cam, x, n, cov, op = _one_gauss_inputs(s, z, o, W, H, f)
+    P = orc.project(x, n, cov, op, cam)
+    assert P["touched"][0] > 0 and P["depth"][0] == np.float32(z)
+    np.testing.assert_allclose(P["mu"][0], [W / 2, H / 2])
+    keys, vals = orc.emit_sort(P["depth"], P["rect"], P["touched"], 4)
+    rng = orc.tile_ranges(keys, 16)
+    col = np.array([[0.9, 0.5, 0.25]])
+    img, T, nc, fl = orc.composite(vals, rng, P["mu"], P["conic_o"], col, np.zeros(3, np.float32), W, H)
+    sp2 = (f * s / z) ** 2 + 0.3
+    yy, xx = np.meshgrid(np.arange(H) + 0.5, np.arange(W) + 0.5, indexing="ij")
+    a = np.minimum(0.99, o * np.exp(-((xx - W / 2) ** 2 + (yy - H / 2) ** 2) / (2 * sp2)))
+    rad = int(np.ceil(3 * np.sqrt(sp2)))
+    assert P["radius"][0] == rad
+    x0, x1 = int((W / 2 - rad) // 16), int((W / 2 + rad + 15) // 16)
+    tile_ok = ((xx // 16) >= x0) & ((xx // 16) < x1) & ((yy // 16) >= x0) & ((yy // 16) < x1)
+    a = np.where((a >= 1 / 255) & tile_ok, a, 0.0)
+    np.testing.assert_allclose(img, a[:, :, None] * col[0], atol=2e-6)
+    np.testing.assert_allclose(T, 1 - a, atol=2e-6)
+    # opacity -> 0 and facing away -> background
+    P2 = orc.project(x, -n, cov, op, cam)
+    assert P2["touched"][0] == 0
+
+
+def test_two_gaussian_over_operator_hand_example():
+    # front-to-back "over": C = c1 a1 + c2 a2 (1 - a1) at the shared centre pixel sample
+    cam, x, n, cov, op = _one_gauss_inputs()
+    x2 = np.array([[0, 0, 4.0], [0, 0, 3.0]], np.float32)        # second one is nearer -> composited first
+    P = orc.project(x2, np.tile(n, (2, 1)), np.tile(cov, (2, 1)), np.array([0.5, 0.25], np.float32), cam)
+    keys, vals = orc.emit_sort(P["depth"], P["rect"], P["touched"], 4)
+    rng = orc.tile_ranges(keys, 16)
+    col = np.array([[1.0, 0, 0], [0, 1.0, 0]])
+    img, T, nc, _ = orc.composite(vals, rng, P["mu"], P["conic_o"], col, np.array([0, 0, 1], np.float32), 64, 64)
+
+    def alpha(g, px, py):
+        d = P["mu"][g].astype(np.float64) - [px, py]; c = P["conic_o"][g].astype(np.float64)
+        return min(0.99, c[3] * np.exp(-0.5 * (c[0] * d[0] ** 2 + c[2] * d[1] ** 2) - c[1] * d[0] * d[1]))
+    a_near, a_far = alpha(1, 32.5, 32.5), alpha(0, 32.5, 32.5)
+    np.testing.assert_allclose(img[32, 32], [a_far * (1 - a_near), a_near, (1 - a_near) * (1 - a_far)], rtol=1e-9)
+    assert vals[np.searchsorted(keys >> 32, 2 * 4 + 2)] == 1     # nearer Gaussian first in tile (2,2)
+
+
+def test_tiled_equals_bruteforce_and_invariants(cfg0, cfg0_oracle):
+    av, o, o1 = cfg0_oracle
+    cam = cfg0["camera"]; W, H = cam["width"], cam["height"]
+    img, T, nc = orc.composite_bruteforce(o["depth"], o["rect"], o["touched"], o["mu"], o["conic_o"], o["color"], cfg0["bg"], W, H)
+    assert np.array_equal(img, o["image"]) and np.array_equal(T, o["T_final"]) and np.array_equal(nc, o["n_contrib"])
+    assert o["T_final"].min() >= 0 and o["T_final"].max() <= 1
+    assert o["image"].max() <= o["color"][o["touched"] > 0].max() + 1e-12
+    keys, vals = o["keys"], o["vals"]
+    assert np.all(np.diff(keys.astype(np.uint64)) >= 0) or np.all(keys[1:] >= keys[:-1])
+    assert len(keys) == o["touched"].sum()
+    assert np.array_equal(np.bincount(vals, minlength=len(o["touched"])), o["touched"])    # permutation of the emitted list
+    same = keys[1:] == keys[:-1]
+    assert np.all(vals[1:][same] > vals[:-1][same])                                       # stability (A22)
+    r = o["ranges"].astype(np.int64); L = r[:, 1] - r[:, 0]
+    assert L.sum() == len(keys)
+    nz = r[L > 0]
+    assert np.array_equal(nz[1:, 0], nz[:-1, 1]) and nz[0, 0] == 0                        # ranges partition [0, D)
+    # black environment -> image = background
+    Lo, cg = orc.shade(o["gauss_posed"], o["gauss_normal_posed"], av["albedo_g"], av["rough_g"], av["spec_g"], cfg0["cam_pos"],
+                       np.zeros_like(cfg0["env"][0]), cfg0["texel_to_dir"], 2)
+    bg = np.array([0.25, 0.5, 0.75], np.float32)
+    img0, _, _, _ = orc.composite(o["vals"], o["ranges"], o["mu"], o["conic_o"], cg, bg, W, H)
+    np.testing.assert_allclose(img0, np.broadcast_to(bg, img0.shape) * o["T_final"][:, :, None], atol=1e-12)
+
+
+def test_projection_matches_double_precision_ewa(cfg0, cfg0_oracle):
+    # Independent numpy fp64 EWA (J W Sigma W^T J^T + 0.3 I) against the op-ordered fp32 oracle.
+    av, o, _ = cfg0_oracle
+    cam = cfg0["camera"]
+    Rw = cam["R_wc"].reshape(3, 3).astype(np.float64); tw = cam["t_wc"].astype(np.float64)
+    g = np.nonzero(o["touched"])[0][:200]
+    x = o["gauss_posed"][g].astype(np.float64)
+    t = x @ Rw.T + tw
+    c6 = o["cov6"][g].astype(np.float64)
+    fx, fy = float(cam["fx"]), float(cam["fy"])
+    for i in range(len(g)):
+        S = np.array([[c6[i, 0], c6[i, 1], c6[i, 2]], [c6[i, 1], c6[i, 3], c6[i, 4]], [c6[i, 2], c6[i, 4], c6[i, 5]]])
+        J = np.array([[fx / t[i, 2], 0, -fx * t[i, 0] / t[i, 2] ** 2], [0, fy / t[i, 2], -fy * t[i, 1] / t[i, 2] ** 2]])
+        c2 = J @ Rw @ S @ Rw.T @ J.T + 0.3 * np.eye(2)
+        con = np.linalg.inv(c2)
+        np.testing.assert_allclose(o["conic_o"][g[i], :3], [con[0, 0], con[0, 1], con[1, 1]], rtol=2e-3, atol=1e-5)
+        lam = np.linalg.eigvalsh(c2).max()
+        assert abs(o["radius"][g[i]] - np.ceil(3 * np.sqrt(lam))) <= 1
+        np.testing.assert_allclose(o["mu"][g[i]], [fx * t[i, 0] / t[i, 2] + float(cam["cx"]), fy * t[i, 1] / t[i, 2] + float(cam["cy"])], rtol=1e-5)
+    # back-facing Gaussians are culled, front-facing in-frustum ones are kept
+    wo = cfg0["cam_pos"].astype(np.float64) - o["gauss_posed"]
+    facing = (o["gauss_normal_posed"] * wo).sum(1)
+    assert np.all(o["touched"][facing < -1e-4] == 0)
+    assert (o["touched"][facing > 1e-4] > 0).mean() > 0.99
