@@ -1,0 +1,183 @@
+/* rga.h -- C ABI of the B200 (sm_100a) per-frame forward render of arXiv 2407.10707
+ * ("Interactive Rendering of Relightable and Animatable Gaussian Avatars").
+ *
+ * Problem statement: an avatar A = {M, G, L} -- canonical mesh M with per-vertex attributes, Gaussians G
+ * near the mesh, light probes L -- is rendered to an image I' for a novel pose, a new environment map and a viewpoint.
+ * Test-time flow (Fig.1 :84): skin -> visibility -> shade -> splat.  One call per stage:
+ *
+ *   avatar_load        L0  KNN sets S_g (K_g=3), S_v (K_v=19) and Eq.1 interpolation of the pose-independent
+ *                          attributes
+ *   pose_skin          H1/H2 forward LBS of mesh and Gaussians
+ *   visibility_raster  H3/H4 orthographic mesh rasterisation per light direction, then either the shadow-map depth
+ *                          test (mode 0, BASELINE.json north_star (b)) or the paper's triangle-ID
+ *                          visibility with the median/median/mean filters (mode 1, Eq.3-4)
+ *   shade_gaussians    H5  Eq.2 with the Appendix-A BRDF, then gamma
+ *   splat_render       H6-H10 back-face opacity kill and the 3DGS tile rasteriser
+ *
+ * Conventions
+ *  - Every pointer marked "dev" is DEVICE memory owned by the caller (row-major, fp32 / int32); pointers marked "host"
+ *    are host memory read during the call.  The library never frees or keeps caller pointers after avatar_load returns
+ *    (it copies what it needs), except that per-frame calls read their dev arguments asynchronously on `stream`, so
+ *    the caller keeps them alive until the stream has passed the call.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  The four per-frame calls only enqueue
+ *    work: no allocation, no host synchronisation, no host-side data-dependent size, so a frame can be captured into
+ *    a CUDA graph.  All scratch is allocated in avatar_load at the declared maxima.
+ *  - Errors: every call returns an rga_status; nothing throws across the ABI.  rga_last_error() gives a thread-local
+ *    message.  Device-side capacity overflow (more (Gaussian,tile) duplicates than max_duplicates) sets a sticky
+ *    device status word that rga_check() reads back; the frame's image is then undefined.
+ *  - Calling a stage before its producer in the same pose returns RGA_ERR_STATE.
+ *  - Quaternions are (w,x,y,z).  World is z-up.  Camera looks down +z, x right, y down; image origin top-left;
+ *    pixel (i,j) samples at (i+1/2, j+1/2).  Bone matrices are posed-global x inverse-bind, row-major 3x4.
+ *  - There is no CPU fallback: without a CUDA device every entry point that computes returns RGA_ERR_CUDA.
+ */
+#ifndef RGA_H_
+#define RGA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define RGA_API __attribute__((visibility("default")))
+#else
+#define RGA_API
+#endif
+
+typedef struct rga_avatar rga_avatar; /* opaque; owns all device scratch */
+
+typedef enum {
+  RGA_OK = 0,
+  RGA_ERR_INVALID_ARG = 1,
+  RGA_ERR_CUDA = 2,
+  RGA_ERR_OOM = 3,
+  RGA_ERR_STATE = 4,
+  RGA_ERR_CAPACITY = 5
+} rga_status;
+
+/* avatar_load input.  PAPER.md:86 lists the vertex attributes {r,s,a,gamma,p,w,n,dx}; PAPER.md:88 the Gaussians. */
+typedef struct {
+  int32_t n_verts, n_faces, n_bones, n_gauss;
+  int32_t k_g;                 /* neighbours per Gaussian, 1..3 (paper: 3)          */
+  int32_t k_v;                 /* neighbours per vertex, odd, 1..31 (paper: 19); clamped to n_verts */
+  const float*   vert_pos;     /* dev [n_verts][3]  canonical x                                      */
+  const int32_t* faces;        /* dev [n_faces][3]                                                   */
+  const float*   vert_normal;  /* dev [n_verts][3]  unit normals n                                   */
+  const float*   vert_skin_w;  /* dev [n_verts][n_bones] LBS weights w, rows sum to 1                */
+  const float*   vert_disp;    /* dev [n_verts][3]  static average displacement or NULL = 0 */
+  const float*   vert_albedo;  /* dev [n_verts][3]  a                                                */
+  const float*   vert_rough;   /* dev [n_verts]     gamma                                            */
+  const float*   vert_spec;    /* dev [n_verts]     specular tint p                                  */
+  const float*   gauss_pos;    /* dev [n_gauss][3]  canonical x_g                                    */
+  const float*   gauss_quat;   /* dev [n_gauss][4]  (w,x,y,z), any non-zero norm                      */
+  const float*   gauss_scale;  /* dev [n_gauss][3]                                                   */
+  const float*   gauss_opacity;/* dev [n_gauss] or NULL = 1 ("always set the opacity ... to 1") */
+  int32_t max_width, max_height;   /* largest camera this avatar will be rendered with                 */
+  int32_t max_vis_dirs;            /* largest K_vis (multiple of 32 not required)                      */
+  int32_t max_vis_res;             /* largest depth-map side R_v, <= 1024                               */
+  int32_t max_env_texels;          /* largest rows*cols of an environment map                           */
+  int64_t max_duplicates;          /* capacity of the (tile,depth) key buffers; 0 = library picks       */
+} rga_avatar_desc;
+
+typedef struct {
+  float R_wc[9];   /* row-major world->camera rotation */
+  float t_wc[3];
+  float fx, fy, cx, cy;
+  int32_t width, height;
+  float z_near;    /* Gaussians with camera z <= z_near are culled (3DGS: 0.2) */
+} rga_camera;
+
+typedef struct {
+  int32_t n_dirs;            /* K_vis                                                                   */
+  int32_t res;               /* R_v: depth maps are res x res                                           */
+  int32_t mode;              /* 0 = shadow-map depth test, 1 = paper (triangle-ID + Eq.3-4 filters)     */
+  const float* dirs;         /* dev [n_dirs][3] unit vectors pointing TOWARD the light                  */
+  float depth_bias_texels;   /* mode 0: slope-scaled bias, in depth-map texels (default 1)              */
+  float depth_bias_world;    /* mode 0: constant bias in world units (default 0.015)                    */
+  float slope_max;           /* mode 0: clamp of the slope factor tan(theta) (default 8)                */
+  int32_t keep_maps;         /* non-zero: also keep the triangle-ID maps in mode 0 (parity / debug)     */
+} rga_vis_params;
+
+typedef struct {
+  int32_t rows, cols;              /* equirectangular, z-up; texel (i,j) centre theta=(i+1/2)pi/rows, phi=(j+1/2)2pi/cols */
+  const float* radiance;           /* dev [rows][cols][3]                                                */
+  const int32_t* texel_to_dir;     /* dev [rows*cols] visibility direction used by each texel, or NULL = identity */
+  float gamma;                     /* colour = clamp(L_o,0,1)^(1/gamma)                                   */
+  int32_t use_visibility;          /* 0 = ignore visibility (v = 1; the paper's "no visibility" variant) */
+} rga_env;
+
+/* L0.  Copies / derives everything it needs from `desc`; allocates all scratch.  Synchronises `stream` before it
+ * returns.  *out is NULL on failure. */
+RGA_API rga_status avatar_load(const rga_avatar_desc* desc, void* stream, rga_avatar** out);
+RGA_API rga_status avatar_free(rga_avatar* av);
+
+/* H1 + H2.  bone_mats: dev [n_bones][12].  Produces posed vertices/normals, posed Gaussians/normals/covariances and
+ * the orthographic window (centre, radius) used by every light direction. */
+RGA_API rga_status pose_skin(rga_avatar* av, const float* bone_mats, void* stream);
+
+/* H3 + H4.  Needs pose_skin.  Produces per-Gaussian visibility bits (mode 0) or per-vertex counts 0..k_v (mode 1). */
+RGA_API rga_status visibility_raster(rga_avatar* av, const rga_vis_params* params, void* stream);
+
+/* H5.  Needs pose_skin, and visibility_raster unless env->use_visibility == 0.  cam_pos: host float[3]. */
+RGA_API rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const float cam_pos[3], void* stream);
+
+/* H6-H10.  Needs shade_gaussians.  bg: host float[3].  out_image: dev [height][width][3] fp32, caller-owned. */
+RGA_API rga_status splat_render(rga_avatar* av, const rga_camera* cam, const float bg[3], float* out_image, void* stream);
+
+/* Intermediates (parity tests, debugging).  Layouts are documented next to each id. */
+typedef enum {
+  RGA_BUF_KNN_G = 0,          /* i32 [n_gauss][k_g]                                  */
+  RGA_BUF_UBAR_G = 1,         /* f32 [n_gauss][k_g]  normalised Eq.1 weights         */
+  RGA_BUF_KNN_V = 2,          /* i32 [n_verts][k_v]                                  */
+  RGA_BUF_GAUSS_STATIC = 3,   /* f32 [n_gauss][16]: xbar(3) pad, n(3) pad, albedo(3) rough, spec pad pad pad */
+  RGA_BUF_GAUSS_SKIN_W = 4,   /* f32 [n_gauss][n_bones]                              */
+  RGA_BUF_VERT_POSED = 5,     /* f32 [n_verts][4]  x' (xyz, w unused)                */
+  RGA_BUF_VERT_NORMAL_POSED = 6, /* f32 [n_verts][4]                                 */
+  RGA_BUF_GAUSS_POSED = 7,    /* f32 [n_gauss][4]  xbar_gd                           */
+  RGA_BUF_GAUSS_NORMAL_POSED = 8, /* f32 [n_gauss][4] n_gd                           */
+  RGA_BUF_GAUSS_COV = 9,      /* f32 [n_gauss][6]  xx,xy,xz,yy,yz,zz                 */
+  RGA_BUF_WINDOW = 10,        /* f32 [4]  centre xyz, radius                         */
+  RGA_BUF_ZMAP = 11,          /* u32 [n_dirs][res][res] float bits of depth, 0xFFFFFFFF = empty */
+  RGA_BUF_IDMAP = 12,         /* i32 [n_dirs][res][res] winning triangle, -1 = empty (mode 1 or keep_maps) */
+  RGA_BUF_VISBITS = 13,       /* u32 [n_gauss][ceil(n_dirs/32)]  bit (k%32) of word k/32 */
+  RGA_BUF_VCOUNT = 14,        /* u8  [n_verts][n_dirs]  mean-filter numerators 0..k_v (mode 1) */
+  RGA_BUF_RADIANCE = 15,      /* f32 [n_gauss][4]  linear L_o rgb, w unused          */
+  RGA_BUF_COLOR = 16,         /* f32 [n_gauss][4]  gamma-corrected colour            */
+  RGA_BUF_MU2D = 17,          /* f32 [n_gauss][2]                                    */
+  RGA_BUF_DEPTH = 18,         /* f32 [n_gauss]                                       */
+  RGA_BUF_CONIC_OPACITY = 19, /* f32 [n_gauss][4]                                    */
+  RGA_BUF_RECT = 20,          /* i32 [n_gauss][4]  x0,y0,x1,y1 (tiles, half-open)    */
+  RGA_BUF_TOUCHED = 21,       /* u32 [n_gauss]                                       */
+  RGA_BUF_NUM_DUPLICATES = 22,/* u32 [1]  D                                          */
+  RGA_BUF_KEYS_SORTED = 23,   /* u64 [D]  tile << 32 | depth bits                    */
+  RGA_BUF_VALS_SORTED = 24,   /* u32 [D]  Gaussian index                             */
+  RGA_BUF_TILE_RANGES = 25,   /* u32 [tiles][2]                                      */
+  RGA_BUF_T_FINAL = 26,       /* f32 [height][width]                                 */
+  RGA_BUF_N_CONTRIB = 27,     /* u32 [height][width]                                 */
+  RGA_BUF_VERT_BITS_RAW = 28, /* u32 [n_verts][ceil(n_dirs/32)] raw vertex visibility (mode 1) */
+  RGA_BUF_COUNT_ = 29
+} rga_buffer_id;
+
+/* Returns the device pointer and current size in bytes of an internal buffer (valid until the next call that
+ * rewrites it).  For data-dependent sizes (KEYS/VALS) this synchronises `stream` to read D. */
+RGA_API rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, const void** dev_ptr, size_t* bytes);
+
+/* Copies an internal buffer to HOST memory `host_dst` (capacity bytes); *bytes = size copied.  Synchronises `stream`.
+ * RGA_ERR_INVALID_ARG if capacity is too small (then *bytes holds the required size). */
+RGA_API rga_status rga_read_buffer(rga_avatar* av, int which, void* stream, void* host_dst, size_t capacity, size_t* bytes);
+
+/* Synchronises `stream` and returns the sticky device status (RGA_OK or RGA_ERR_CAPACITY); clears it. */
+RGA_API rga_status rga_check(rga_avatar* av, void* stream);
+
+/* Number of kernels the library has launched since the avatar was loaded (bench.py's gpu_launches claim). */
+RGA_API int64_t rga_launch_count(const rga_avatar* av);
+
+RGA_API const char* rga_last_error(void);
+RGA_API const char* rga_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RGA_H_ */

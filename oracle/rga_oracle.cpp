@@ -153,14 +153,17 @@ ORC void orc_light_frames(const float* dirs, int K, float* uvw) {
   }
 }
 
-// Light-space projection of one point: continuous pixel coords (px,py) and normalised depth z (0 = nearest the light).
+// Light-space projection of one point (reading A13): continuous pixel coords (px,py) and normalised depth z
+// (0 = nearest the light).  Per-pose constants sR = (R/2)/r, hR = R/2, inv2r = 1/(2r) are formed once, so the per-point
+// work is multiply-add only:  px = (u.d) sR + hR,  py = (v.d) sR + hR,  z = (r - w.d) inv2r,  d = p - c.
 static inline void light_project(const float* p, const float* c, float r, const float* u, const float* v, const float* w,
                                  int R, float* px, float* py, float* z) {
+  float hR = 0.5f * (float)R, sR = hR / r, inv2r = 1.0f / (2.0f * r);
   float d[3] = {p[0] - c[0], p[1] - c[1], p[2] - c[2]};
   float pu = dot3(u, d), pv = dot3(v, d), pw = dot3(w, d);
-  float t = pu / r; t = t * 0.5f; t = t + 0.5f; *px = t * (float)R;
-  t = pv / r; t = t * 0.5f; t = t + 0.5f; *py = t * (float)R;
-  *z = (r - pw) / (2.0f * r);
+  *px = pu * sR + hR;
+  *py = pv * sR + hR;
+  *z = (r - pw) * inv2r;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -243,7 +246,7 @@ ORC void orc_vis_depth_test(const float* xg, const float* ng_, int ng, const flo
           tau = std::sqrt(s2) / cs;
           tau = std::fmin(std::fmax(tau, 1.0f), slope_max);
         } else tau = slope_max;
-        float beta = ((bias_texels * ((2.0f * r) / (float)R)) * tau + bias_world) / (2.0f * r);
+        float beta = (bias_texels / (float)R) * tau + bias_world * (1.0f / (2.0f * r));   // texel = 1/R in normalised depth
         vis = z <= bitsf(zb) + beta;
       }
       if (vis) bits[(size_t)g * words + (k >> 5)] |= 1u << (k & 31);

@@ -1,0 +1,235 @@
+// C ABI of librga (include/rga.h): argument checks, scratch ownership, stage ordering.  All compute is in the kernels.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "rga_internal.h"
+
+int rga_shade_init_attributes(int max_env);
+int rga_vis_init_attributes();
+
+static thread_local char g_err[512] = "";
+static rga_status fail(rga_status st, const char* fmt, ...) {
+  va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof g_err, fmt, ap); va_end(ap);
+  return st;
+}
+#define CU(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, \
+    "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+
+extern "C" const char* rga_last_error(void) { return g_err; }
+extern "C" const char* rga_version(void) { return "rga 0.1 (sm_100a)"; }
+extern "C" int64_t rga_launch_count(const rga_avatar* av) { return av ? av->launches : 0; }
+
+template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)); }
+
+extern "C" rga_status avatar_free(rga_avatar* av) {
+  if (!av) return RGA_OK;
+  void* ptrs[] = {av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
+                  av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
+                  av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
+                  av->radiance, av->color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->offsets, av->keys[0],
+                  av->keys[1], av->vals[0], av->vals[1], av->sort_hist, av->num_dup, av->ranges, av->t_final, av->n_contrib,
+                  av->status};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  delete av;
+  return RGA_OK;
+}
+
+extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_avatar** out) {
+  if (out) *out = nullptr;
+  if (!d || !out) return fail(RGA_ERR_INVALID_ARG, "avatar_load: null argument");
+  if (d->n_verts < 1 || d->n_faces < 1 || d->n_bones < 1 || d->n_gauss < 1) return fail(RGA_ERR_INVALID_ARG, "avatar_load: empty avatar");
+  if (d->k_g < 1 || d->k_g > 3) return fail(RGA_ERR_INVALID_ARG, "avatar_load: k_g must be 1..3");
+  if (d->k_v < 1 || d->k_v > 31 || !(d->k_v & 1)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: k_v must be odd, 1..31");
+  if (!d->vert_pos || !d->faces || !d->vert_normal || !d->vert_skin_w || !d->vert_albedo || !d->vert_rough || !d->vert_spec ||
+      !d->gauss_pos || !d->gauss_quat || !d->gauss_scale) return fail(RGA_ERR_INVALID_ARG, "avatar_load: missing table");
+  if (d->max_width < 1 || d->max_height < 1 || d->max_vis_dirs < 1 || d->max_vis_res < 1 || d->max_vis_res > 1024 ||
+      d->max_env_texels < 1 || d->max_env_texels > 65535) return fail(RGA_ERR_INVALID_ARG, "avatar_load: bad maxima");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(RGA_ERR_CUDA, "avatar_load: no CUDA device (there is no CPU fallback)");
+  cudaStream_t s = (cudaStream_t)stream;
+  rga_avatar* av = new (std::nothrow) rga_avatar();
+  if (!av) return fail(RGA_ERR_OOM, "avatar_load: host allocation");
+  memset(av, 0, sizeof *av);
+  av->n_verts = d->n_verts; av->n_faces = d->n_faces; av->n_bones = d->n_bones; av->n_gauss = d->n_gauss;
+  av->k_g = d->k_g; av->k_v = d->k_v;
+  if (av->k_v > d->n_verts) av->k_v = (d->n_verts & 1) ? d->n_verts : d->n_verts - 1;      // largest odd count available
+  av->max_w = d->max_width; av->max_h = d->max_height; av->max_dirs = d->max_vis_dirs; av->max_res = d->max_vis_res;
+  av->max_env = d->max_env_texels;
+  av->max_dup = d->max_duplicates > 0 ? d->max_duplicates : (long long)d->n_gauss * 16 + (1 << 20);
+  if (av->max_dup > 0xfffffff0ll) av->max_dup = 0xfffffff0ll;
+  int dev = 0; cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&av->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  const size_t nv = av->n_verts, ng = av->n_gauss, B = av->n_bones, words = (av->max_dirs + 31) / 32;
+  const size_t ntiles = (size_t)((av->max_w + 15) / 16) * ((av->max_h + 15) / 16), npix = (size_t)av->max_w * av->max_h;
+  const size_t nmap = (size_t)av->max_dirs * av->max_res * av->max_res;
+  rga_status st = RGA_OK;
+  float* d2 = nullptr;
+#define A(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, \
+    "avatar_load: %s: %s", #call, cudaGetErrorString(e_)); goto done; } } while (0)
+  A(dalloc(&av->v_xbar, nv)); A(dalloc(&av->v_normal, nv)); A(dalloc(&av->v_skin_w, nv * B)); A(dalloc(&av->faces, 3 * (size_t)av->n_faces));
+  A(dalloc(&av->knn_v, nv * av->k_v)); A(dalloc(&av->knn_g, ng * av->k_g)); A(dalloc(&av->ubar_g, ng * av->k_g));
+  A(dalloc(&av->g_static, 4 * ng)); A(dalloc(&av->g_skin_w, ng * B)); A(dalloc(&av->g_quat, ng)); A(dalloc(&av->g_scale_op, ng));
+  A(dalloc(&av->v_posed, nv)); A(dalloc(&av->v_nposed, nv)); A(dalloc(&av->g_posed, ng)); A(dalloc(&av->g_nposed, ng));
+  A(dalloc(&av->g_cov, 6 * ng)); A(dalloc(&av->window, 4)); A(dalloc(&av->aabb, 6));
+  A(dalloc(&av->zmap, nmap)); A(dalloc(&av->idmap, nmap)); A(dalloc(&av->visbits, ng * words));
+  A(dalloc(&av->vbits_a, nv * words)); A(dalloc(&av->vbits_b, nv * words)); A(dalloc(&av->vbits_raw, nv * words));
+  A(dalloc(&av->vcount, nv * (size_t)av->max_dirs + 32)); A(dalloc(&av->env_table, 8 * (size_t)av->max_env));
+  A(dalloc(&av->radiance, ng)); A(dalloc(&av->color, ng));
+  A(dalloc(&av->mu2d, ng)); A(dalloc(&av->depth, ng)); A(dalloc(&av->conic_o, ng)); A(dalloc(&av->rect, ng)); A(dalloc(&av->touched, ng));
+  A(dalloc(&av->offsets, (ng + 255) / 256 + 1));
+  A(dalloc(&av->keys[0], (size_t)av->max_dup)); A(dalloc(&av->keys[1], (size_t)av->max_dup));
+  A(dalloc(&av->vals[0], (size_t)av->max_dup)); A(dalloc(&av->vals[1], (size_t)av->max_dup));
+  A(dalloc(&av->sort_hist, 256 * (size_t)av->num_sms * 2)); A(dalloc(&av->num_dup, 1)); A(dalloc(&av->ranges, ntiles));
+  A(dalloc(&av->t_final, npix)); A(dalloc(&av->n_contrib, npix)); A(dalloc(&av->status, 1));
+  A(cudaMemsetAsync(av->status, 0, sizeof(int), s)); A(cudaMemsetAsync(av->num_dup, 0, sizeof(unsigned), s));
+  {
+    unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
+    A(cudaMemcpyAsync(av->aabb, init, sizeof init, cudaMemcpyHostToDevice, s));
+    A(cudaStreamSynchronize(s));
+  }
+  A(cudaMemcpyAsync(av->v_skin_w, d->vert_skin_w, nv * B * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  A(cudaMemcpyAsync(av->faces, d->faces, 3 * (size_t)av->n_faces * sizeof(int), cudaMemcpyDeviceToDevice, s));
+  A(rga_launch_load_verts(av, d->vert_pos, d->vert_disp, d->vert_normal, s));
+  // KNN: S_v = K_v nearest vertices of each vertex (self included), S_g = K_g nearest of each Gaussian
+  A(dalloc(&d2, (ng * av->k_g > nv * av->k_v ? ng * av->k_g : nv * av->k_v)));
+  A(rga_launch_knn(d->vert_pos, av->n_verts, d->vert_pos, av->n_verts, av->k_v, av->knn_v, d2, s));
+  A(rga_launch_knn(d->gauss_pos, av->n_gauss, d->vert_pos, av->n_verts, av->k_g, av->knn_g, d2, s));
+  A(rga_launch_load_gauss(av, d, d2, s));
+  av->launches += 4;
+  if (rga_shade_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
+  A(cudaStreamSynchronize(s));
+done:
+  if (d2) cudaFree(d2);
+  if (st != RGA_OK) { avatar_free(av); return st; }
+  *out = av;
+  return RGA_OK;
+#undef A
+}
+
+extern "C" rga_status pose_skin(rga_avatar* av, const float* bone_mats, void* stream) {
+  if (!av || !bone_mats) return fail(RGA_ERR_INVALID_ARG, "pose_skin: null argument");
+  av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
+  CU(rga_launch_skin(av, bone_mats, (cudaStream_t)stream));
+  av->have_skin = 1;
+  return RGA_OK;
+}
+
+extern "C" rga_status visibility_raster(rga_avatar* av, const rga_vis_params* p, void* stream) {
+  if (!av || !p || !p->dirs) return fail(RGA_ERR_INVALID_ARG, "visibility_raster: null argument");
+  if (!av->have_skin) return fail(RGA_ERR_STATE, "visibility_raster: call pose_skin first");
+  if (p->n_dirs < 1 || p->n_dirs > av->max_dirs || p->res < 1 || p->res > av->max_res || (p->mode != 0 && p->mode != 1))
+    return fail(RGA_ERR_INVALID_ARG, "visibility_raster: n_dirs/res/mode out of range");
+  cudaStream_t s = (cudaStream_t)stream;
+  av->have_vis = av->have_shade = av->have_splat = 0;
+  CU(rga_launch_vis_raster(av, p, s));
+  if (p->mode == 0) CU(rga_launch_vis_depth_test(av, p, s));
+  else CU(rga_launch_vis_paper(av, p, s));
+  av->vis_mode = p->mode; av->vis_dirs = p->n_dirs; av->vis_res = p->res; av->vis_words = (p->n_dirs + 31) / 32;
+  av->keep_maps = p->keep_maps || p->mode == 1;
+  av->have_vis = 1;
+  return RGA_OK;
+}
+
+extern "C" rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const float cam_pos[3], void* stream) {
+  if (!av || !env || !env->radiance || !cam_pos) return fail(RGA_ERR_INVALID_ARG, "shade_gaussians: null argument");
+  if (!av->have_skin) return fail(RGA_ERR_STATE, "shade_gaussians: call pose_skin first");
+  if (env->use_visibility && !av->have_vis) return fail(RGA_ERR_STATE, "shade_gaussians: call visibility_raster first");
+  if (env->rows < 1 || env->cols < 1 || env->rows * env->cols > av->max_env || !(env->gamma > 0.f))
+    return fail(RGA_ERR_INVALID_ARG, "shade_gaussians: env size/gamma out of range");
+  if (env->use_visibility && !env->texel_to_dir && env->rows * env->cols != av->vis_dirs)
+    return fail(RGA_ERR_INVALID_ARG, "shade_gaussians: identity texel_to_dir needs rows*cols == n_dirs");
+  cudaStream_t s = (cudaStream_t)stream;
+  av->have_shade = av->have_splat = 0;
+  CU(rga_launch_env_table(av, env, s));
+  CU(rga_launch_shade(av, env, make_float3(cam_pos[0], cam_pos[1], cam_pos[2]), env->use_visibility ? av->vis_mode : 2, s));
+  av->have_shade = 1;
+  return RGA_OK;
+}
+
+extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const float bg[3], float* out_image, void* stream) {
+  if (!av || !cam || !bg || !out_image) return fail(RGA_ERR_INVALID_ARG, "splat_render: null argument");
+  if (!av->have_shade) return fail(RGA_ERR_STATE, "splat_render: call shade_gaussians first");
+  if (cam->width < 1 || cam->height < 1 || cam->width > av->max_w || cam->height > av->max_h)
+    return fail(RGA_ERR_INVALID_ARG, "splat_render: camera larger than max_width/max_height");
+  cudaStream_t s = (cudaStream_t)stream;
+  int TX = (cam->width + 15) / 16, TY = (cam->height + 15) / 16, ntiles = TX * TY;
+  int tile_bits = 0; while ((1 << tile_bits) < ntiles) ++tile_bits;
+  CU(rga_launch_project(av, cam, s));
+  CU(rga_launch_scan_emit(av, TX, s));
+  CU(rga_launch_sort(av, 32 + tile_bits, s));
+  CU(rga_launch_ranges(av, ntiles, s));
+  CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), out_image, s));
+  av->cam_w = cam->width; av->cam_h = cam->height;
+  av->have_splat = 1;
+  return RGA_OK;
+}
+
+extern "C" rga_status rga_check(rga_avatar* av, void* stream) {
+  if (!av) return fail(RGA_ERR_INVALID_ARG, "rga_check: null avatar");
+  int st = 0;
+  CU(cudaMemcpyAsync(&st, av->status, sizeof st, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CU(cudaStreamSynchronize((cudaStream_t)stream));
+  if (st != 0) { cudaMemsetAsync(av->status, 0, sizeof(int), (cudaStream_t)stream); return fail((rga_status)st, "device status %d (capacity overflow: raise max_duplicates)", st); }
+  return RGA_OK;
+}
+
+extern "C" rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, const void** dev_ptr, size_t* bytes) {
+  if (!av || !dev_ptr || !bytes) return fail(RGA_ERR_INVALID_ARG, "rga_get_buffer: null argument");
+  const size_t nv = av->n_verts, ng = av->n_gauss, words = av->vis_words, K = av->vis_dirs, R = av->vis_res;
+  const size_t npix = (size_t)av->cam_w * av->cam_h, ntiles = (size_t)((av->cam_w + 15) / 16) * ((av->cam_h + 15) / 16);
+  size_t D = 0;
+  if (which == RGA_BUF_KEYS_SORTED || which == RGA_BUF_VALS_SORTED) {
+    unsigned d = 0;
+    CU(cudaMemcpyAsync(&d, av->num_dup, 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    D = d;
+  }
+  const void* p = nullptr; size_t n = 0;
+  switch (which) {
+    case RGA_BUF_KNN_G: p = av->knn_g; n = ng * av->k_g * 4; break;
+    case RGA_BUF_UBAR_G: p = av->ubar_g; n = ng * av->k_g * 4; break;
+    case RGA_BUF_KNN_V: p = av->knn_v; n = nv * av->k_v * 4; break;
+    case RGA_BUF_GAUSS_STATIC: p = av->g_static; n = ng * 64; break;
+    case RGA_BUF_GAUSS_SKIN_W: p = av->g_skin_w; n = ng * av->n_bones * 4; break;
+    case RGA_BUF_VERT_POSED: p = av->v_posed; n = nv * 16; break;
+    case RGA_BUF_VERT_NORMAL_POSED: p = av->v_nposed; n = nv * 16; break;
+    case RGA_BUF_GAUSS_POSED: p = av->g_posed; n = ng * 16; break;
+    case RGA_BUF_GAUSS_NORMAL_POSED: p = av->g_nposed; n = ng * 16; break;
+    case RGA_BUF_GAUSS_COV: p = av->g_cov; n = ng * 24; break;
+    case RGA_BUF_WINDOW: p = av->window; n = 16; break;
+    case RGA_BUF_ZMAP: p = av->zmap; n = K * R * R * 4; break;
+    case RGA_BUF_IDMAP: p = av->idmap; n = av->keep_maps ? K * R * R * 4 : 0; break;
+    case RGA_BUF_VISBITS: p = av->visbits; n = ng * words * 4; break;
+    case RGA_BUF_VCOUNT: p = av->vcount; n = nv * K; break;
+    case RGA_BUF_RADIANCE: p = av->radiance; n = ng * 16; break;
+    case RGA_BUF_COLOR: p = av->color; n = ng * 16; break;
+    case RGA_BUF_MU2D: p = av->mu2d; n = ng * 8; break;
+    case RGA_BUF_DEPTH: p = av->depth; n = ng * 4; break;
+    case RGA_BUF_CONIC_OPACITY: p = av->conic_o; n = ng * 16; break;
+    case RGA_BUF_RECT: p = av->rect; n = ng * 16; break;
+    case RGA_BUF_TOUCHED: p = av->touched; n = ng * 4; break;
+    case RGA_BUF_NUM_DUPLICATES: p = av->num_dup; n = 4; break;
+    case RGA_BUF_KEYS_SORTED: p = av->keys[av->sorted_buf]; n = D * 8; break;
+    case RGA_BUF_VALS_SORTED: p = av->vals[av->sorted_buf]; n = D * 4; break;
+    case RGA_BUF_TILE_RANGES: p = av->ranges; n = ntiles * 8; break;
+    case RGA_BUF_T_FINAL: p = av->t_final; n = npix * 4; break;
+    case RGA_BUF_N_CONTRIB: p = av->n_contrib; n = npix * 4; break;
+    case RGA_BUF_VERT_BITS_RAW: p = av->vbits_raw; n = nv * words * 4; break;
+    default: return fail(RGA_ERR_INVALID_ARG, "rga_get_buffer: unknown id %d", which);
+  }
+  *dev_ptr = p; *bytes = n;
+  return RGA_OK;
+}
+
+extern "C" rga_status rga_read_buffer(rga_avatar* av, int which, void* stream, void* host_dst, size_t capacity, size_t* bytes) {
+  const void* p = nullptr; size_t n = 0;
+  rga_status st = rga_get_buffer(av, which, stream, &p, &n);
+  if (st != RGA_OK) return st;
+  if (bytes) *bytes = n;
+  if (!host_dst || capacity < n) return fail(RGA_ERR_INVALID_ARG, "rga_read_buffer: need %zu bytes", n);
+  if (n) CU(cudaMemcpyAsync(host_dst, p, n, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CU(cudaStreamSynchronize((cudaStream_t)stream));
+  return RGA_OK;
+}

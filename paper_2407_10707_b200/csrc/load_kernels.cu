@@ -1,0 +1,118 @@
+// L0 avatar_load kernels: brute-force KNN and Eq.1 interpolation of the
+// pose-independent attributes.  EXACT file: compiled with -fmad=false; only + - * / sqrt so results are bit-identical
+// to any IEEE-754 implementation that follows the same operation order.
+#include "rga_internal.h"
+
+#define KNN_TILE 1024
+#define KNN_MAXK 32
+
+// One thread per query; vertices staged through shared memory in tiles; K best kept sorted ascending.
+// Scanning j upward with a strict '<' keeps the lower index on equal distances.
+template <int KT>
+__global__ void __launch_bounds__(256) knn_kernel(const float* __restrict__ q, int nq, const float* __restrict__ v, int nv,
+                                                  int Krt, int* __restrict__ idx, float* __restrict__ d2out) {
+  __shared__ float sv[KNN_TILE * 3];
+  const int K = KT > 0 ? KT : Krt;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  float qx = 0.f, qy = 0.f, qz = 0.f;
+  if (i < nq) { qx = q[3 * (size_t)i]; qy = q[3 * (size_t)i + 1]; qz = q[3 * (size_t)i + 2]; }
+  float bd[KT > 0 ? KT : KNN_MAXK];
+  int bi[KT > 0 ? KT : KNN_MAXK];
+#pragma unroll
+  for (int k = 0; k < (KT > 0 ? KT : KNN_MAXK); ++k) { bd[k] = __int_as_float(0x7f800000); bi[k] = -1; }
+  for (int base = 0; base < nv; base += KNN_TILE) {
+    int cnt = min(KNN_TILE, nv - base);
+    __syncthreads();
+    for (int t = threadIdx.x; t < cnt * 3; t += blockDim.x) sv[t] = v[(size_t)base * 3 + t];
+    __syncthreads();
+    if (i < nq) {
+      for (int j = 0; j < cnt; ++j) {
+        float dx = qx - sv[3 * j], dy = qy - sv[3 * j + 1], dz = qz - sv[3 * j + 2];
+        float d = (dx * dx + dy * dy) + dz * dz;
+        if (d < bd[K - 1]) {
+          if (KT > 0) {
+#pragma unroll
+            for (int p = (KT > 0 ? KT : 1) - 1; p >= 0; --p) {        // static indices: the list stays in registers
+              if (p > 0 && d < bd[p - 1]) { bd[p] = bd[p - 1]; bi[p] = bi[p - 1]; }
+              else { bd[p] = d; bi[p] = base + j; break; }
+            }
+          } else {
+            int p = K - 1;
+            while (p > 0 && d < bd[p - 1]) { bd[p] = bd[p - 1]; bi[p] = bi[p - 1]; --p; }
+            bd[p] = d; bi[p] = base + j;
+          }
+        }
+      }
+    }
+  }
+  if (i < nq)
+    for (int k = 0; k < K; ++k) { idx[(size_t)i * K + k] = bi[k]; d2out[(size_t)i * K + k] = bd[k]; }
+}
+
+cudaError_t rga_launch_knn(const float* q, int nq, const float* v, int nv, int K, int* idx, float* d2, cudaStream_t s) {
+  int grid = (nq + 255) / 256;
+  if (K == 3) knn_kernel<3><<<grid, 256, 0, s>>>(q, nq, v, nv, K, idx, d2);
+  else if (K == 19) knn_kernel<19><<<grid, 256, 0, s>>>(q, nq, v, nv, K, idx, d2);
+  else knn_kernel<0><<<grid, 256, 0, s>>>(q, nq, v, nv, K, idx, d2);
+  return cudaGetLastError();
+}
+
+__global__ void load_verts_kernel(int n, const float* __restrict__ pos, const float* __restrict__ disp,
+                                  const float* __restrict__ nrm, float4* __restrict__ xbar, float4* __restrict__ nout) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float dx = disp ? disp[3 * i] : 0.f, dy = disp ? disp[3 * i + 1] : 0.f, dz = disp ? disp[3 * i + 2] : 0.f;
+  xbar[i] = make_float4(pos[3 * i] + dx, pos[3 * i + 1] + dy, pos[3 * i + 2] + dz, 0.f);
+  nout[i] = make_float4(nrm[3 * i], nrm[3 * i + 1], nrm[3 * i + 2], 0.f);
+}
+
+cudaError_t rga_launch_load_verts(rga_avatar* av, const float* pos, const float* disp, const float* nrm, cudaStream_t s) {
+  load_verts_kernel<<<(av->n_verts + 255) / 256, 256, 0, s>>>(av->n_verts, pos, disp, nrm, av->v_xbar, av->v_normal);
+  return cudaGetLastError();
+}
+
+// Eq.1 for one Gaussian: weights from the K_g squared distances, then every static attribute.
+__global__ void __launch_bounds__(128) load_gauss_kernel(int n, int K, int B, const int* __restrict__ knn, const float* __restrict__ d2,
+                                  const float* __restrict__ gpos, const float* __restrict__ vdisp,
+                                  const float* __restrict__ vnrm, const float* __restrict__ valb,
+                                  const float* __restrict__ vrough, const float* __restrict__ vspec,
+                                  const float* __restrict__ vw, const float* __restrict__ gquat,
+                                  const float* __restrict__ gscale, const float* __restrict__ gop,
+                                  float* __restrict__ ubar, float4* __restrict__ gst, float* __restrict__ gw,
+                                  float4* __restrict__ quat, float4* __restrict__ scale_op) {
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n) return;
+  float u[4]; int id[4];
+  float U = 0.f;
+  for (int k = 0; k < K; ++k) {
+    id[k] = knn[(size_t)g * K + k];
+    float dist = sqrtf(d2[(size_t)g * K + k]);
+    u[k] = 1.0f / fmaxf(dist, 1e-12f);
+    U = (k == 0) ? u[0] : U + u[k];
+  }
+  for (int k = 0; k < K; ++k) { u[k] = u[k] / U; ubar[(size_t)g * K + k] = u[k]; }
+  auto interp = [&](const float* a, int C, int c) {
+    float acc = u[0] * a[(size_t)id[0] * C + c];
+    for (int k = 1; k < K; ++k) acc = acc + u[k] * a[(size_t)id[k] * C + c];
+    return acc;
+  };
+  float d0 = vdisp ? interp(vdisp, 3, 0) : 0.f, d1 = vdisp ? interp(vdisp, 3, 1) : 0.f, d2v = vdisp ? interp(vdisp, 3, 2) : 0.f;
+  gst[4 * (size_t)g + 0] = make_float4(gpos[3 * (size_t)g] + d0, gpos[3 * (size_t)g + 1] + d1, gpos[3 * (size_t)g + 2] + d2v, 0.f);
+  float nx = interp(vnrm, 3, 0), ny = interp(vnrm, 3, 1), nz = interp(vnrm, 3, 2);
+  float len = sqrtf((nx * nx + ny * ny) + nz * nz);
+  if (len > 0.f) { nx = nx / len; ny = ny / len; nz = nz / len; }
+  gst[4 * (size_t)g + 1] = make_float4(nx, ny, nz, 0.f);
+  gst[4 * (size_t)g + 2] = make_float4(interp(valb, 3, 0), interp(valb, 3, 1), interp(valb, 3, 2), interp(vrough, 1, 0));
+  gst[4 * (size_t)g + 3] = make_float4(interp(vspec, 1, 0), 0.f, 0.f, 0.f);
+  for (int b = 0; b < B; ++b) gw[(size_t)g * B + b] = interp(vw, B, b);
+  quat[g] = make_float4(gquat[4 * (size_t)g], gquat[4 * (size_t)g + 1], gquat[4 * (size_t)g + 2], gquat[4 * (size_t)g + 3]);
+  scale_op[g] = make_float4(gscale[3 * (size_t)g], gscale[3 * (size_t)g + 1], gscale[3 * (size_t)g + 2], gop ? gop[g] : 1.0f);
+}
+
+cudaError_t rga_launch_load_gauss(rga_avatar* av, const rga_avatar_desc* d, const float* d2, cudaStream_t s) {
+  load_gauss_kernel<<<(av->n_gauss + 127) / 128, 128, 0, s>>>(
+      av->n_gauss, av->k_g, av->n_bones, av->knn_g, d2, d->gauss_pos, d->vert_disp, d->vert_normal, d->vert_albedo,
+      d->vert_rough, d->vert_spec, d->vert_skin_w, d->gauss_quat, d->gauss_scale, d->gauss_opacity, av->ubar_g,
+      av->g_static, av->g_skin_w, av->g_quat, av->g_scale_op);
+  return cudaGetLastError();
+}

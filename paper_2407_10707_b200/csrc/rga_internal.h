@@ -1,0 +1,86 @@
+// Internal state and kernel launchers of librga (CUDA path).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/rga.h"
+
+#define RGA_TILE 16
+
+struct rga_avatar {
+  // sizes
+  int n_verts, n_faces, n_bones, n_gauss, k_g, k_v;
+  int max_w, max_h, max_dirs, max_res, max_env;
+  long long max_dup;
+  int num_sms;
+  // static (load-time) tables
+  float4* v_xbar;      // [n_verts]  x + dx
+  float4* v_normal;    // [n_verts]
+  float* v_skin_w;     // [n_verts][B]
+  int* faces;          // [n_faces][3]
+  int* knn_v;          // [n_verts][k_v]
+  int* knn_g;          // [n_gauss][k_g]
+  float* ubar_g;       // [n_gauss][k_g]
+  float4* g_static;    // [n_gauss][4]: (xbar,_), (n,_), (albedo,rough), (spec,_,_,_)
+  float* g_skin_w;     // [n_gauss][B]
+  float4* g_quat;      // [n_gauss]
+  float4* g_scale_op;  // [n_gauss] (sx,sy,sz,opacity)
+  // per-pose
+  float4* v_posed;     // [n_verts]
+  float4* v_nposed;    // [n_verts]
+  float4* g_posed;     // [n_gauss]
+  float4* g_nposed;    // [n_gauss]
+  float* g_cov;        // [n_gauss][6]
+  float* window;       // [4] centre, radius; [4..9] scratch AABB as ordered ints
+  unsigned* aabb;      // [6] ordered-uint min xyz, max xyz
+  // visibility
+  unsigned* zmap;      // [max_dirs][res*res]
+  int* idmap;          // [max_dirs][res*res]  (allocated lazily at load: always, sized like zmap)
+  unsigned* visbits;   // [n_gauss][words]
+  unsigned* vbits_a;   // [n_verts][words]
+  unsigned* vbits_b;   // [n_verts][words]
+  unsigned* vbits_raw; // [n_verts][words]
+  unsigned char* vcount;  // [n_verts][max_dirs]
+  float* env_table;    // [max_env][8]: w(3), pad, L*A (3), pad
+  // shading out
+  float4* radiance;    // [n_gauss]
+  float4* color;       // [n_gauss]
+  // splat
+  float2* mu2d; float* depth; float4* conic_o; int4* rect; unsigned* touched; unsigned* offsets;
+  unsigned* scan_state;        // decoupled look-back tile states
+  unsigned long long* keys[2]; unsigned* vals[2];
+  unsigned* sort_hist;         // radix histograms
+  unsigned* num_dup;           // [1] D (device)
+  uint2* ranges;               // [tiles]
+  float* t_final; unsigned* n_contrib;
+  int* status;                 // sticky device status
+  int sorted_buf;              // which of keys[]/vals[] holds the sorted result
+  // state of the current pose
+  int have_skin, have_vis, have_shade, have_splat;
+  int vis_mode, vis_dirs, vis_res, vis_words, keep_maps;
+  int cam_w, cam_h;
+  long long launches;
+};
+
+// ---- launchers (each returns cudaGetLastError()) ----
+// load_kernels.cu
+cudaError_t rga_launch_knn(const float* q, int nq, const float* v, int nv, int K, int* idx, float* d2, cudaStream_t s);
+cudaError_t rga_launch_load_verts(rga_avatar* av, const float* pos, const float* disp, const float* nrm, cudaStream_t s);
+cudaError_t rga_launch_load_gauss(rga_avatar* av, const rga_avatar_desc* d, const float* d2, cudaStream_t s);
+// skin_kernels.cu
+cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, cudaStream_t s);
+// vis_kernels.cu
+cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
+cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
+cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
+size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows);
+// shade_kernels.cu
+cudaError_t rga_launch_env_table(rga_avatar* av, const rga_env* env, cudaStream_t s);
+cudaError_t rga_launch_shade(rga_avatar* av, const rga_env* env, float3 cam, int vis_mode, cudaStream_t s);
+// splat_kernels.cu
+cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream_t s);
+cudaError_t rga_launch_scan_emit(rga_avatar* av, int tiles_x, cudaStream_t s);
+cudaError_t rga_launch_sort(rga_avatar* av, int key_bits, cudaStream_t s);
+cudaError_t rga_launch_ranges(rga_avatar* av, int ntiles, cudaStream_t s);
+cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s);
+int rga_init_kernel_attributes();

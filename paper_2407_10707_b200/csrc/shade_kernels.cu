@@ -1,0 +1,160 @@
+// H5 shade_gaussians: Eq.2 with the Appendix-A BRDF (Eq.12-15), then gamma.
+// FAST file (default FMA contraction, MUFU intrinsics): the result is compared with the fp64 oracle under the
+// north_star tolerance (2e-3 max-abs on colour), not bit-exactly.
+//
+// Layout: LANES threads cooperate on one Gaussian; each walks a strided subset of the environment texels.  The env
+// table (w_k, L_k A_k) is staged in shared memory once per CTA; visibility comes as bits (mode 0), as vertex counts
+// gathered through S_g (mode 1) or is 1 (mode 2).
+#include "rga_internal.h"
+
+#define PI_F 3.14159265358979323846f
+
+// Reading A6: equirectangular z-up grid; A = exact solid angle of the texel = 2 sin(theta_c) sin(pi/(2R)) 2pi/C
+// (the product form of cos(i pi/R) - cos((i+1) pi/R), free of cancellation in fp32).
+__global__ void env_table_kernel(int rows, int cols, const float* __restrict__ radiance, float* __restrict__ table) {
+  int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= rows * cols) return;
+  int i = k / cols, j = k - i * cols;
+  float st, ct, sp, cp;
+  sincospif(((float)i + 0.5f) / (float)rows, &st, &ct);
+  sincospif(2.0f * ((float)j + 0.5f) / (float)cols, &sp, &cp);
+  float A = 2.0f * st * sinpif(0.5f / (float)rows) * (2.0f * PI_F / (float)cols);
+  float4* t = reinterpret_cast<float4*>(table) + 2 * (size_t)k;
+  t[0] = make_float4(st * cp, st * sp, ct, 0.f);
+  t[1] = make_float4(radiance[3 * k] * A, radiance[3 * k + 1] * A, radiance[3 * k + 2] * A, 0.f);
+}
+
+cudaError_t rga_launch_env_table(rga_avatar* av, const rga_env* env, cudaStream_t s) {
+  int n = env->rows * env->cols;
+  env_table_kernel<<<(n + 127) / 128, 128, 0, s>>>(env->rows, env->cols, env->radiance, av->env_table);
+  av->launches += 1;
+  return cudaGetLastError();
+}
+
+template <int LANES, int MODE>
+__global__ void __launch_bounds__(128) shade_kernel(int ng, int ne, int K, int words, int Kg, int Kv,
+    const float4* __restrict__ g_posed, const float4* __restrict__ g_nposed, const float4* __restrict__ g_static,
+    const float* __restrict__ env_table, const int* __restrict__ t2d, const unsigned* __restrict__ visbits,
+    const unsigned char* __restrict__ vcount, const int* __restrict__ knn_g, const float* __restrict__ ubar_g,
+    float3 cam, float inv_gamma, float4* __restrict__ radiance, float4* __restrict__ color) {
+  extern __shared__ __align__(16) float smem[];
+  float4* sE = reinterpret_cast<float4*>(smem);                          // [ne][2]
+  unsigned short* sD = reinterpret_cast<unsigned short*>(sE + 2 * ne);   // [ne] texel -> direction
+  for (int t = threadIdx.x; t < 2 * ne; t += blockDim.x) sE[t] = reinterpret_cast<const float4*>(env_table)[t];
+  if (MODE != 2) for (int t = threadIdx.x; t < ne; t += blockDim.x) sD[t] = (unsigned short)(t2d ? t2d[t] : t);
+  __syncthreads();
+  const int GPB = 128 / LANES;                                           // Gaussians per block
+  const int lane = threadIdx.x % LANES;
+  const int g = blockIdx.x * GPB + threadIdx.x / LANES;
+  if (g >= ng) return;                                                   // whole LANES-group exits together
+  const float4 x = g_posed[g], n = g_nposed[g];
+  float wox = cam.x - x.x, woy = cam.y - x.y, woz = cam.z - x.z;
+  const float wl2 = wox * wox + woy * woy + woz * woz;
+  const float facing = n.x * wox + n.y * woy + n.z * woz;
+  // a Gaussian facing away from the camera gets opacity 0, so its colour is never used.  Skip it only
+  // when the sign is certain (the exact test lives in the projection kernel).
+  if (facing < -1e-4f * sqrtf(wl2)) {
+    if (lane == 0) { radiance[g] = make_float4(0.f, 0.f, 0.f, 0.f); color[g] = make_float4(0.f, 0.f, 0.f, 0.f); }
+    return;
+  }
+  const float winv = rsqrtf(wl2);
+  wox *= winv; woy *= winv; woz *= winv;
+  const float4 ar = g_static[4 * (size_t)g + 2];                         // albedo rgb, roughness
+  const float spec = g_static[4 * (size_t)g + 3].x;
+  const float nwo_raw = n.x * wox + n.y * woy + n.z * woz;
+  const float nwo = fmaxf(nwo_raw, 0.f);
+  const float rough = ar.w, al = rough * rough, al2 = al * al;           // Eq.13: alpha = gamma^2
+  const float kk = (rough + 1.f) * (rough + 1.f) * 0.125f, omk = 1.f - kk;   // Eq.15
+  const float go = nwo * omk + kk;
+  // n x w_o, for 1 - (n.h)^2 = |n x (w_i + w_o)|^2 / |w_i + w_o|^2 (the direct form cancels badly for alpha^2 ~ 1e-4)
+  const float cox = n.y * woz - n.z * woy, coy = n.z * wox - n.x * woz, coz = n.x * woy - n.y * wox;
+  const float cS = al2 / (4.f * PI_F * go);                              // D F G /(4 ni no) = cS F / (den^2 gi)
+  float u0 = 0.f, u1 = 0.f, u2 = 0.f; int j0 = 0, j1 = 0, j2 = 0;
+  if (MODE == 1) {
+    const float ikv = 1.0f / (float)Kv;
+    j0 = knn_g[(size_t)g * Kg]; u0 = ubar_g[(size_t)g * Kg] * ikv;
+    if (Kg > 1) { j1 = knn_g[(size_t)g * Kg + 1]; u1 = ubar_g[(size_t)g * Kg + 1] * ikv; }
+    if (Kg > 2) { j2 = knn_g[(size_t)g * Kg + 2]; u2 = ubar_g[(size_t)g * Kg + 2] * ikv; }
+  }
+  const unsigned* vb = visbits + (size_t)g * words;
+  float d0 = 0.f, d1 = 0.f, d2 = 0.f, s0 = 0.f, s1 = 0.f, s2 = 0.f;
+  for (int k = lane; k < ne; k += LANES) {
+    const float4 wi = sE[2 * k];
+    const float cs = n.x * wi.x + n.y * wi.y + n.z * wi.z;
+    if (cs <= 0.f) continue;                                             // max(0, w_i . n)
+    float v = 1.f;
+    if (MODE == 0) {
+      const int d = sD[k];
+      if (!((__ldg(vb + (d >> 5)) >> (d & 31)) & 1u)) continue;
+    } else if (MODE == 1) {
+      const int d = sD[k];
+      v = u0 * (float)__ldg(vcount + (size_t)j0 * K + d);
+      if (Kg > 1) v += u1 * (float)__ldg(vcount + (size_t)j1 * K + d);
+      if (Kg > 2) v += u2 * (float)__ldg(vcount + (size_t)j2 * K + d);
+      if (v == 0.f) continue;
+    }
+    const float4 LA = sE[2 * k + 1];
+    const float ow = wox * wi.x + woy * wi.y + woz * wi.z;
+    const float hl2 = fmaxf(2.f + 2.f * ow, 1e-12f);                     // |w_i + w_o|^2
+    const float hinv = rsqrtf(hl2);
+    const float nh = (cs + nwo_raw) * hinv;
+    const float oh = (1.f + ow) * hinv;
+    const float cx = fmaf(n.y, wi.z, -n.z * wi.y) + cox, cy = fmaf(n.z, wi.x, -n.x * wi.z) + coy,
+                cz = fmaf(n.x, wi.y, -n.y * wi.x) + coz;
+    const float den = fmaf(al2 * nh, nh, (cx * cx + cy * cy + cz * cz) * (hinv * hinv));   // (n.h)^2 (a^2 - 1) + 1, Eq.13
+    const float F = 0.04f + 0.96f * exp2f((-5.55473f * oh - 6.98316f) * oh);   // Eq.14
+    const float gi = cs * omk + kk;
+    const float sp = cS * F * __frcp_rn(den * den * gi);
+    const float w = v * cs;
+    const float ws = w * sp;
+    d0 = fmaf(LA.x, w, d0); d1 = fmaf(LA.y, w, d1); d2 = fmaf(LA.z, w, d2);
+    s0 = fmaf(LA.x, ws, s0); s1 = fmaf(LA.y, ws, s1); s2 = fmaf(LA.z, ws, s2);
+  }
+  // the LANES-group always exits together, so its own lane mask is the legal one for the shuffles
+  const unsigned gmask = (LANES == 32) ? 0xffffffffu : (((1u << LANES) - 1u) << (((threadIdx.x & 31) / LANES) * LANES));
+#pragma unroll
+  for (int o = LANES / 2; o > 0; o >>= 1) {
+    d0 += __shfl_xor_sync(gmask, d0, o, LANES); d1 += __shfl_xor_sync(gmask, d1, o, LANES);
+    d2 += __shfl_xor_sync(gmask, d2, o, LANES); s0 += __shfl_xor_sync(gmask, s0, o, LANES);
+    s1 += __shfl_xor_sync(gmask, s1, o, LANES); s2 += __shfl_xor_sync(gmask, s2, o, LANES);
+  }
+  if (lane == 0) {
+    const float ip = 1.f / PI_F;
+    float L0 = ar.x * ip * d0 + spec * s0, L1 = ar.y * ip * d1 + spec * s1, L2 = ar.z * ip * d2 + spec * s2;   // Eq.12
+    radiance[g] = make_float4(L0, L1, L2, 0.f);
+    float c0 = exp2f(inv_gamma * log2f(fminf(fmaxf(L0, 0.f), 1.f)));
+    float c1 = exp2f(inv_gamma * log2f(fminf(fmaxf(L1, 0.f), 1.f)));
+    float c2 = exp2f(inv_gamma * log2f(fminf(fmaxf(L2, 0.f), 1.f)));
+    color[g] = make_float4(c0, c1, c2, 0.f);
+  }
+}
+
+#ifndef RGA_SHADE_LANES
+#define RGA_SHADE_LANES 4
+#endif
+
+cudaError_t rga_launch_shade(rga_avatar* av, const rga_env* env, float3 cam, int vis_mode, cudaStream_t s) {
+  const int L = RGA_SHADE_LANES;
+  int ne = env->rows * env->cols;
+  int gpb = 128 / L, grid = (av->n_gauss + gpb - 1) / gpb;
+  size_t smem = (size_t)ne * 32 + (size_t)ne * 2;
+  float ig = 1.0f / env->gamma;
+#define SHADE_ARGS av->n_gauss, ne, av->vis_dirs, av->vis_words, av->k_g, av->k_v, av->g_posed, av->g_nposed, av->g_static, \
+    av->env_table, env->texel_to_dir, av->visbits, av->vcount, av->knn_g, av->ubar_g, cam, ig, av->radiance, av->color
+  if (vis_mode == 0) shade_kernel<L, 0><<<grid, 128, smem, s>>>(SHADE_ARGS);
+  else if (vis_mode == 1) shade_kernel<L, 1><<<grid, 128, smem, s>>>(SHADE_ARGS);
+  else shade_kernel<L, 2><<<grid, 128, smem, s>>>(SHADE_ARGS);
+  av->launches += 1;
+  return cudaGetLastError();
+}
+
+int rga_shade_init_attributes(int max_env) {
+  size_t smem = (size_t)max_env * 34;
+  cudaError_t e = cudaSuccess;
+  if (smem > 48 * 1024) {
+    e = cudaFuncSetAttribute(shade_kernel<RGA_SHADE_LANES, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(shade_kernel<RGA_SHADE_LANES, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(shade_kernel<RGA_SHADE_LANES, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  }
+  return (int)e;
+}

@@ -1,0 +1,319 @@
+// H3/H4 visibility_raster: orthographic rasterisation of the posed mesh from every light direction
+// into a shared-memory depth map (atomicMin on packed depth), then either the per-Gaussian shadow-map depth test
+// (mode 0; BASELINE.json north_star (b)) or the paper's triangle-ID visibility with the
+// median/median/mean vertex filters (mode 1; Eq.3-4).
+// EXACT file: -fmad=false; + - * / sqrt and integer arithmetic only.
+#include "rga_internal.h"
+
+struct LightFrame { float u[3], v[3], w[3]; };
+
+// DESIGN.md A13: u = normalize(e x w), e = z unless |w_z| > 0.999 then x; v = w x u.
+__device__ __forceinline__ LightFrame make_frame(const float* __restrict__ dir) {
+  LightFrame f;
+  f.w[0] = dir[0]; f.w[1] = dir[1]; f.w[2] = dir[2];
+  float e0 = 0.f, e1 = 0.f, e2 = 1.f;
+  if (fabsf(f.w[2]) > 0.999f) { e0 = 1.f; e2 = 0.f; }
+  float c0 = e1 * f.w[2] - e2 * f.w[1], c1 = e2 * f.w[0] - e0 * f.w[2], c2 = e0 * f.w[1] - e1 * f.w[0];
+  float len = sqrtf((c0 * c0 + c1 * c1) + c2 * c2);
+  f.u[0] = c0 / len; f.u[1] = c1 / len; f.u[2] = c2 / len;
+  f.v[0] = f.w[1] * f.u[2] - f.w[2] * f.u[1];
+  f.v[1] = f.w[2] * f.u[0] - f.w[0] * f.u[2];
+  f.v[2] = f.w[0] * f.u[1] - f.w[1] * f.u[0];
+  return f;
+}
+
+struct WinConst { float cx, cy, cz, r, sR, hR, inv2r; };
+__device__ __forceinline__ WinConst make_win(const float* __restrict__ window, int R) {
+  WinConst W;
+  W.cx = window[0]; W.cy = window[1]; W.cz = window[2]; W.r = window[3];
+  W.hR = 0.5f * (float)R; W.sR = W.hR / W.r; W.inv2r = 1.0f / (2.0f * W.r);
+  return W;
+}
+__device__ __forceinline__ void light_project(float x, float y, float z, const WinConst& W, const LightFrame& f,
+                                              float& px, float& py, float& pz) {
+  float dx = x - W.cx, dy = y - W.cy, dz = z - W.cz;
+  float pu = (f.u[0] * dx + f.u[1] * dy) + f.u[2] * dz;
+  float pv = (f.v[0] * dx + f.v[1] * dy) + f.v[2] * dz;
+  float pw = (f.w[0] * dx + f.w[1] * dy) + f.w[2] * dz;
+  px = pu * W.sR + W.hR;
+  py = pv * W.sR + W.hR;
+  pz = (W.r - pw) * W.inv2r;
+}
+
+// ------------------------------------------------------------------------------------------------------------- H3
+// One CTA per (direction, band of rows).  The band's depth map lives in shared memory: u32 depth (mode 0) or
+// u64 depth<<32|triangle (WITH_ID).  Every thread walks triangles with a block stride, projects the three corners,
+// and scans the (tiny) pixel bounding box with int64 edge functions at 1/256-pixel snapped coordinates.
+template <bool WITH_ID>
+__global__ void __launch_bounds__(512) vis_raster_kernel(int nf, int R, int band_rows, int n_bands, int nv_words,
+    const float4* __restrict__ v_posed, const int* __restrict__ faces, const float* __restrict__ dirs,
+    const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
+    unsigned* __restrict__ vbits_raw, int words, int n_verts) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int k = blockIdx.x / n_bands, band = blockIdx.x % n_bands;
+  const int row0 = band * band_rows, rows = min(band_rows, R - row0);
+  const int npix = rows * R;
+  unsigned* sz32 = reinterpret_cast<unsigned*>(smem_raw);
+  unsigned long long* sz64 = reinterpret_cast<unsigned long long*>(smem_raw);
+  unsigned* svert = reinterpret_cast<unsigned*>(smem_raw + (size_t)band_rows * R * 8);     // WITH_ID only: vertex bitset
+  if (WITH_ID) {
+    for (int p = threadIdx.x; p < npix; p += blockDim.x) sz64[p] = ~0ull;
+    for (int p = threadIdx.x; p < nv_words; p += blockDim.x) svert[p] = 0u;
+  } else {
+    for (int p = threadIdx.x; p < npix; p += blockDim.x) sz32[p] = 0xffffffffu;
+  }
+  const LightFrame F = make_frame(dirs + 3 * k);
+  const WinConst W = make_win(window, R);
+  __syncthreads();
+  const long long ylo = 256ll * row0, yhi = 256ll * (row0 + rows);        // band covers pixel centres 256j+128, j in [row0,row0+rows)
+  for (int t = threadIdx.x; t < nf; t += blockDim.x) {
+    int i0 = __ldg(faces + 3 * t), i1 = __ldg(faces + 3 * t + 1), i2 = __ldg(faces + 3 * t + 2);
+    float4 a = __ldg(v_posed + i0), b = __ldg(v_posed + i1), c = __ldg(v_posed + i2);
+    float px, py, z0, z1, z2;
+    light_project(a.x, a.y, a.z, W, F, px, py, z0);
+    long long x0 = __float2int_rn(px * 256.0f), y0 = __float2int_rn(py * 256.0f);
+    light_project(b.x, b.y, b.z, W, F, px, py, z1);
+    long long x1 = __float2int_rn(px * 256.0f), y1 = __float2int_rn(py * 256.0f);
+    light_project(c.x, c.y, c.z, W, F, px, py, z2);
+    long long x2 = __float2int_rn(px * 256.0f), y2 = __float2int_rn(py * 256.0f);
+    long long mny = min(y0, min(y1, y2)), mxy = max(y0, max(y1, y2));
+    if (mxy < ylo + 128 || mny > yhi - 128) continue;                       // no pixel centre of this band inside
+    long long area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
+    if (area == 0) continue;
+    long long mnx = min(x0, min(x1, x2)), mxx = max(x0, max(x1, x2));
+    int ia = (int)max((mnx - 128 + 255) >> 8, 0ll), ib = (int)min((mxx - 128) >> 8, (long long)(R - 1));
+    int ja = (int)max((mny - 128 + 255) >> 8, (long long)row0), jb = (int)min((mxy - 128) >> 8, (long long)(row0 + rows - 1));
+    float fa = (float)area;
+    for (int j = ja; j <= jb; ++j) {
+      long long qy = 256ll * j + 128;
+      for (int i = ia; i <= ib; ++i) {
+        long long qx = 256ll * i + 128;
+        long long e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
+        long long e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
+        long long e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
+        bool in = (e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0);
+        if (!in) continue;
+        float t1 = (float)e1 / fa, t2 = (float)e2 / fa;
+        float z = (z0 + t1 * (z1 - z0)) + t2 * (z2 - z0);
+        z = fmaxf(z, 0.0f);
+        int p = (j - row0) * R + i;
+        if (WITH_ID) atomicMin(sz64 + p, ((unsigned long long)__float_as_uint(z) << 32) | (unsigned)t);
+        else atomicMin(sz32 + p, __float_as_uint(z));
+      }
+    }
+  }
+  __syncthreads();
+  size_t base = ((size_t)k * R + row0) * R;
+  if (WITH_ID) {
+    for (int p = threadIdx.x; p < npix; p += blockDim.x) {
+      unsigned long long key = sz64[p];
+      zmap[base + p] = (unsigned)(key >> 32);
+      int tri = (key == ~0ull) ? -1 : (int)(unsigned)(key & 0xffffffffu);
+      idmap[base + p] = tri;
+      if (vbits_raw && tri >= 0) {                      // a triangle that appears marks its 3 vertices
+        int v0 = __ldg(faces + 3 * tri), v1 = __ldg(faces + 3 * tri + 1), v2 = __ldg(faces + 3 * tri + 2);
+        atomicOr(svert + (v0 >> 5), 1u << (v0 & 31));
+        atomicOr(svert + (v1 >> 5), 1u << (v1 & 31));
+        atomicOr(svert + (v2 >> 5), 1u << (v2 & 31));
+      }
+    }
+    if (vbits_raw) {
+      __syncthreads();
+      const unsigned bit = 1u << (k & 31);
+      for (int wd = threadIdx.x; wd < nv_words; wd += blockDim.x) {
+        unsigned m = svert[wd];
+        while (m) {
+          int b = __ffs(m) - 1; m &= m - 1;
+          int vtx = wd * 32 + b;
+          if (vtx < n_verts) atomicOr(vbits_raw + (size_t)vtx * words + (k >> 5), bit);
+        }
+      }
+    }
+  } else {
+    for (int p = threadIdx.x; p < npix; p += blockDim.x) zmap[base + p] = sz32[p];
+  }
+}
+
+size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows) {
+  const size_t budget = 200 * 1024;
+  size_t per_row = (size_t)res * (with_id ? 8 : 4);
+  size_t extra = with_id ? (size_t)((n_verts + 31) / 32) * 4 : 0;
+  int rows = (int)((budget - extra) / per_row);
+  if (rows > res) rows = res;
+  if (rows < 1) rows = 1;
+  int bands = (res + rows - 1) / rows;
+  rows = (res + bands - 1) / bands;                       // even bands
+  *band_rows = rows;
+  return per_row * rows + extra;
+}
+
+cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {
+  const bool with_id = p->mode == 1 || p->keep_maps;
+  int band_rows = 0;
+  size_t smem = rga_vis_raster_smem(p->res, with_id, av->n_verts, &band_rows);
+  int n_bands = (p->res + band_rows - 1) / band_rows;
+  int words = (p->n_dirs + 31) / 32, nv_words = (av->n_verts + 31) / 32;
+  dim3 grid(p->n_dirs * n_bands);
+  if (with_id) {
+    unsigned* raw = (p->mode == 1) ? av->vbits_raw : nullptr;
+    if (raw) cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s);
+    vis_raster_kernel<true><<<grid, 512, smem, s>>>(av->n_faces, p->res, band_rows, n_bands, nv_words, av->v_posed, av->faces,
+                                                   p->dirs, av->window, av->zmap, av->idmap, raw, words, av->n_verts);
+  } else {
+    vis_raster_kernel<false><<<grid, 512, smem, s>>>(av->n_faces, p->res, band_rows, n_bands, nv_words, av->v_posed, av->faces,
+                                                    p->dirs, av->window, av->zmap, av->idmap, nullptr, words, av->n_verts);
+  }
+  av->launches += 1;
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------ H4a
+// Shadow-map test, Gaussian-major: one thread per Gaussian keeps its position/normal in registers and walks all
+// directions; neighbouring (Morton-ordered) Gaussians hit neighbouring texels, so the depth-map gathers stay in
+// L1/L2.  32 directions are packed into one output word.  The slope factor tau (sqrt and divide) is only evaluated when
+// the two monotone bounds beta(1) <= beta(tau) <= beta(slope_max) do not already decide the comparison.
+#define DT_THREADS 128
+__global__ void __launch_bounds__(DT_THREADS) vis_depth_test_kernel(int ng, int K, int R, const float4* __restrict__ g_posed,
+    const float4* __restrict__ g_nposed, const float* __restrict__ dirs, const float* __restrict__ window,
+    const unsigned* __restrict__ zmap, float bias_texels, float bias_world, float slope_max, unsigned* __restrict__ visbits) {
+  extern __shared__ float sF[];                                   // K x 9 light frames
+  for (int k = threadIdx.x; k < K; k += blockDim.x) {
+    LightFrame f = make_frame(dirs + 3 * k);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { sF[9 * k + c] = f.u[c]; sF[9 * k + 3 + c] = f.v[c]; sF[9 * k + 6 + c] = f.w[c]; }
+  }
+  __syncthreads();
+  int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= ng) return;
+  const WinConst W = make_win(window, R);
+  const float bt = bias_texels / (float)R, bw = bias_world * W.inv2r;
+  const float beta_lo = bt * 1.0f + bw, beta_hi = bt * slope_max + bw;
+  const bool bounds_ok = bt >= 0.f && slope_max >= 1.0f;
+  const float Rm1 = (float)(R - 1);
+  float4 x = g_posed[g], n = g_nposed[g];
+  const float dx = x.x - W.cx, dy = x.y - W.cy, dz = x.z - W.cz;
+  const int words = (K + 31) >> 5;
+  for (int wd = 0; wd < words; ++wd) {
+    unsigned bits = 0;
+    int kend = min(32, K - wd * 32);
+    for (int b = 0; b < kend; ++b) {
+      int k = wd * 32 + b;
+      const float* f = sF + 9 * k;
+      float pu = (f[0] * dx + f[1] * dy) + f[2] * dz;
+      float pv = (f[3] * dx + f[4] * dy) + f[5] * dz;
+      float pw = (f[6] * dx + f[7] * dy) + f[8] * dz;
+      float px = pu * W.sR + W.hR, py = pv * W.sR + W.hR, z = (W.r - pw) * W.inv2r;
+      int ix = (int)fminf(fmaxf(floorf(px), 0.0f), Rm1), iy = (int)fminf(fmaxf(floorf(py), 0.0f), Rm1);
+      unsigned zb = __ldg(zmap + ((size_t)k * R + iy) * R + ix);
+      bool vis;
+      if (zb == 0xffffffffu) vis = true;
+      else {
+        float zm = __uint_as_float(zb);
+        if (bounds_ok && z <= zm + beta_lo) vis = true;
+        else if (bounds_ok && !(z <= zm + beta_hi)) vis = false;
+        else {
+          float cs = (n.x * f[6] + n.y * f[7]) + n.z * f[8], tau;
+          if (cs > 0.0f) {
+            float s2 = fmaxf(1.0f - cs * cs, 0.0f);
+            tau = sqrtf(s2) / cs;
+            tau = fminf(fmaxf(tau, 1.0f), slope_max);
+          } else tau = slope_max;
+          vis = z <= zm + (bt * tau + bw);
+        }
+      }
+      bits |= (vis ? 1u : 0u) << b;
+    }
+    visbits[(size_t)g * words + wd] = bits;
+  }
+}
+
+cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {
+  int grid = (av->n_gauss + DT_THREADS - 1) / DT_THREADS;
+  vis_depth_test_kernel<<<grid, DT_THREADS, (size_t)p->n_dirs * 9 * sizeof(float), s>>>(
+      av->n_gauss, p->n_dirs, p->res, av->g_posed, av->g_nposed, p->dirs, av->window, av->zmap, p->depth_bias_texels,
+      p->depth_bias_world, p->slope_max, av->visbits);
+  av->launches += 1;
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------ H4b
+// Eq.3-4 on bit-packed maps: thread = (vertex, word of 32 directions).  The K_v neighbour words are
+// summed with a bit-sliced (carry-save) counter, so 32 directions are filtered at once.
+__device__ __forceinline__ void sliced_count(const int* __restrict__ nb, int Kv, const unsigned* __restrict__ bits, int words,
+                                             int wd, unsigned c[5]) {
+#pragma unroll
+  for (int s = 0; s < 5; ++s) c[s] = 0u;
+  for (int q = 0; q < Kv; ++q) {
+    unsigned carry = __ldg(bits + (size_t)__ldg(nb + q) * words + wd);
+#pragma unroll
+    for (int s = 0; s < 5; ++s) { unsigned t = c[s] & carry; c[s] ^= carry; carry = t; }
+  }
+}
+
+__global__ void __launch_bounds__(256) vis_median_kernel(int nv, int words, int Kv, const int* __restrict__ knn_v,
+                                                         const unsigned* __restrict__ in, unsigned* __restrict__ out) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nv * words) return;
+  int j = t / words, wd = t - j * words;
+  unsigned c[5];
+  sliced_count(knn_v + (size_t)j * Kv, Kv, in, words, wd, c);
+  const int T = (Kv + 1) / 2;                                      // median of Kv (odd) bits = count >= T
+  unsigned gt = 0u, eq = ~0u;
+#pragma unroll
+  for (int s = 4; s >= 0; --s) {
+    unsigned tb = ((T >> s) & 1) ? ~0u : 0u;
+    gt |= eq & c[s] & ~tb;
+    eq &= ~(c[s] ^ tb);
+  }
+  out[t] = gt | eq;
+}
+
+__global__ void __launch_bounds__(256) vis_mean_kernel(int nv, int words, int K, int Kv, const int* __restrict__ knn_v,
+                                                       const unsigned* __restrict__ in, unsigned char* __restrict__ vcount) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nv * words) return;
+  int j = t / words, wd = t - j * words;
+  unsigned c[5];
+  sliced_count(knn_v + (size_t)j * Kv, Kv, in, words, wd, c);
+  unsigned char* dst = vcount + (size_t)j * K + wd * 32;
+  int kend = min(32, K - wd * 32);
+  if (kend == 32 && (K & 15) == 0) {
+    unsigned out[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      unsigned v = 0;
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        int bit = q * 4 + b;
+        unsigned cnt = ((c[0] >> bit) & 1) | (((c[1] >> bit) & 1) << 1) | (((c[2] >> bit) & 1) << 2) |
+                       (((c[3] >> bit) & 1) << 3) | (((c[4] >> bit) & 1) << 4);
+        v |= cnt << (8 * b);
+      }
+      out[q] = v;
+    }
+    uint4* d4 = reinterpret_cast<uint4*>(dst);
+    d4[0] = make_uint4(out[0], out[1], out[2], out[3]);
+    d4[1] = make_uint4(out[4], out[5], out[6], out[7]);
+  } else {
+    for (int bit = 0; bit < kend; ++bit)
+      dst[bit] = (unsigned char)(((c[0] >> bit) & 1) | (((c[1] >> bit) & 1) << 1) | (((c[2] >> bit) & 1) << 2) |
+                                 (((c[3] >> bit) & 1) << 3) | (((c[4] >> bit) & 1) << 4));
+  }
+}
+
+cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {
+  int words = (p->n_dirs + 31) / 32;
+  int n = av->n_verts * words, grid = (n + 255) / 256;
+  vis_median_kernel<<<grid, 256, 0, s>>>(av->n_verts, words, av->k_v, av->knn_v, av->vbits_raw, av->vbits_a);
+  vis_median_kernel<<<grid, 256, 0, s>>>(av->n_verts, words, av->k_v, av->knn_v, av->vbits_a, av->vbits_b);
+  vis_mean_kernel<<<grid, 256, 0, s>>>(av->n_verts, words, p->n_dirs, av->k_v, av->knn_v, av->vbits_b, av->vcount);
+  av->launches += 3;
+  return cudaGetLastError();
+}
+
+int rga_vis_init_attributes() {
+  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_depth_test_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+  return (int)e;
+}

@@ -1,0 +1,105 @@
+"""Shared helper of the GPU parity tests: run the CUDA path through the C-ABI binding and the oracle on the same seeded
+inputs and compare every stage.  Integer / index / bit outputs must be identical; radiance, colour and image obey the
+north_star tolerances (max-abs 2e-3, mean-abs 2e-4 on [0,1] values)."""
+import numpy as np
+
+IMG_MAX, IMG_MEAN, FLAG_MAX = 2e-3, 2e-4, 1.0 / 255.0 + 2e-3
+
+
+def run_gpu(inp, vis_mode=0, frame=0, keep_maps=True, use_visibility=True, max_duplicates=0, camera=None):
+    import torch
+    from paper_2407_10707_b200 import binding as rga
+    cam = camera or inp["camera"]
+    W, H = cam["width"], cam["height"]
+    dev = "cuda"
+    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=len(inp["vis_dirs"]), max_vis_res=inp["vis_res"],
+                    max_env_texels=inp["env_rows"] * inp["env_cols"], max_duplicates=max_duplicates)
+    bones = torch.as_tensor(inp["bone_mats"][frame]).to(dev)
+    dirs = torch.as_tensor(inp["vis_dirs"]).to(dev)
+    env = torch.as_tensor(inp["env"][inp["env_of_frame"][frame]]).to(dev)
+    t2d = torch.as_tensor(inp["texel_to_dir"]).to(dev)
+    img = torch.empty((H, W, 3), dtype=torch.float32, device=dev)
+    rga.pose_skin(av.h, bones)
+    if use_visibility:
+        rga.visibility_raster(av.h, dirs, inp["vis_res"], vis_mode, inp["depth_bias_texels"], inp["depth_bias_world"],
+                              inp["slope_max"], keep_maps)
+    rga.shade_gaussians(av.h, env, inp["cam_pos"], t2d, inp["gamma"], use_visibility)
+    rga.splat_render(av.h, cam, inp["bg"], img)
+    rga.rga_check(av.h)
+    torch.cuda.synchronize()
+    return av, img.cpu().numpy()
+
+
+def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=None):
+    """Assert stage-by-stage parity.  `o` is oracle.render_frame's dict, `orc_av` oracle.avatar_load's."""
+    rep = report if report is not None else {}
+    ng, nv = len(inp["gauss_pos"]), len(inp["vert_pos"])
+    K, R = len(inp["vis_dirs"]), inp["vis_res"]
+    words = (K + 31) // 32
+    rd = av.read
+    eq = np.array_equal
+
+    # L0
+    assert eq(rd("KNN_G").reshape(ng, -1), orc_av["knn_g"]), "knn_g"
+    assert eq(rd("KNN_V").reshape(nv, -1), orc_av["knn_v"]), "knn_v"
+    assert eq(rd("UBAR_G").reshape(ng, -1), orc_av["ubar_g"]), "ubar_g"
+    st = rd("GAUSS_STATIC").reshape(ng, 16)
+    assert eq(st[:, 0:3], inp["gauss_pos"] + orc_av["disp_g"]), "xbar_g"
+    assert eq(st[:, 4:7], orc_av["normal_g"]), "normal_g"
+    assert eq(st[:, 8:11], orc_av["albedo_g"]) and eq(st[:, 11], orc_av["rough_g"]) and eq(st[:, 12], orc_av["spec_g"]), "materials"
+    assert eq(rd("GAUSS_SKIN_W").reshape(ng, -1), orc_av["skin_w_g"]), "skin_w_g"
+    # H1/H2 (bit-exact fp32)
+    assert eq(rd("VERT_POSED").reshape(nv, 4)[:, :3], o["vert_posed"]), "vert_posed"
+    assert eq(rd("VERT_NORMAL_POSED").reshape(nv, 4)[:, :3], o["vert_normal_posed"]), "vert_normal_posed"
+    assert eq(rd("GAUSS_POSED").reshape(ng, 4)[:, :3], o["gauss_posed"]), "gauss_posed"
+    assert eq(rd("GAUSS_NORMAL_POSED").reshape(ng, 4)[:, :3], o["gauss_normal_posed"]), "gauss_normal_posed"
+    assert eq(rd("GAUSS_COV").reshape(ng, 6), o["cov6"]), "cov6"
+    win = rd("WINDOW")
+    assert eq(win[:3], o["win_c"]) and win[3] == o["win_r"], "window"
+    # H3/H4
+    if use_visibility:
+        assert eq(rd("ZMAP").reshape(K, R, R), o["zmap"]), "zmap"
+        ids = rd("IDMAP")
+        if ids.size:
+            assert eq(ids.reshape(K, R, R), o["idmap"]), "idmap"
+        if vis_mode == 0:
+            assert eq(rd("VISBITS").reshape(ng, words), o["visbits"]), "visbits"
+        else:
+            assert eq(rd("VCOUNT").reshape(nv, K), o["vcount"]), "vcount"
+    # H6 (bit-exact)
+    assert eq(rd("TOUCHED"), o["touched"]), "touched"
+    assert eq(rd("RECT").reshape(ng, 4), o["rect"]), "rect"
+    assert eq(rd("MU2D").reshape(ng, 2), o["mu"]), "mu2d"
+    assert eq(rd("DEPTH"), o["depth"]), "depth"
+    assert eq(rd("CONIC_OPACITY").reshape(ng, 4), o["conic_o"]), "conic_opacity"
+    # H5 on non-culled Gaussians
+    live = o["touched"] > 0
+    Lo = rd("RADIANCE").reshape(ng, 4)[:, :3].astype(np.float64)
+    col = rd("COLOR").reshape(ng, 4)[:, :3].astype(np.float64)
+    if live.any():
+        dL = np.abs(Lo[live] - o["L_o"][live]) / np.maximum(1.0, np.abs(o["L_o"][live]))
+        dc = np.abs(col[live] - o["color"][live])
+        rep["radiance_max"], rep["color_max"], rep["color_mean"] = dL.max(), dc.max(), dc.mean()
+        assert dL.max() <= IMG_MAX, "radiance max %g" % dL.max()
+        assert dc.max() <= IMG_MAX and dc.mean() <= IMG_MEAN, "colour max %g mean %g" % (dc.max(), dc.mean())
+    # H7-H9 (bit-exact)
+    D = int(rd("NUM_DUPLICATES")[0])
+    assert D == len(o["keys"]), "D %d vs %d" % (D, len(o["keys"]))
+    assert eq(rd("KEYS_SORTED"), o["keys"]), "sorted keys"
+    assert eq(rd("VALS_SORTED"), o["vals"]), "sorted vals"
+    assert eq(rd("TILE_RANGES").reshape(-1, 2), o["ranges"]), "tile ranges"
+    # H10
+    d = np.abs(img.astype(np.float64) - o["image"]).max(-1)
+    fl = o["flags"].astype(bool)
+    rep["image_max"], rep["image_mean"], rep["flagged"] = d[~fl].max() if (~fl).any() else 0.0, d.mean(), int(fl.sum())
+    assert rep["image_max"] <= IMG_MAX, "image max %g" % rep["image_max"]
+    assert d.mean() <= IMG_MEAN, "image mean %g" % d.mean()
+    if fl.any():
+        assert d[fl].max() <= FLAG_MAX, "flagged pixels max %g" % d[fl].max()
+    H, W = img.shape[:2]
+    T = rd("T_FINAL").reshape(H, W).astype(np.float64)
+    assert np.abs(T - o["T_final"])[~fl].max() <= IMG_MAX, "T_final"
+    nc = rd("N_CONTRIB").reshape(H, W)
+    rep["n_contrib_mismatch"] = float((nc != o["n_contrib"])[~fl].mean())
+    assert rep["n_contrib_mismatch"] < 1e-3, "n_contrib"
+    return rep
