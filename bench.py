@@ -1,0 +1,245 @@
+#!/usr/bin/env python
+"""bench.py -- relit posed frames/sec of the arXiv 2407.10707 forward render on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (pose_skin -> visibility_raster -> shade_gaussians -> splat_render, all
+SURVEY.md 8(a) rows H1..H10) for one frame of BASELINE.json configs[1]: 100k Gaussians on the 6,890-vertex body,
+512 light directions at 128^2, 16x32 HDR environment map, 512x512 camera; seeded synthetic inputs (synth/).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--vis-mode 0|1]
+
+Prints ONE JSON line (rank 0).  `value` = frames/s with inputs resident in HBM; `e2e` = the same through the C-ABI
+calls with host (pinned) pose / env-map buffers copied in and the image copied out inside the timed region;
+`roofline` = the dominant kernel against its bound; `cpu_baseline` = the oracle on this box's host cores.
+N > 1: replicas only: every rank renders its own frames, no data-path collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "relit posed frames/sec (100k Gaussians, 512x512)"
+WORKLOAD = "configs[1] SMPL-sized: 6,890 v / 13,776 f / 24 bones, 100k Gaussians, 16x32 env, 512 dirs @128^2, 512x512"
+# algorithmic work per unit of each kernel (fp32 flop, FMA = 2)
+FLOP_PER_UNIT = {"shade": 70.0, "vis_depth_test": 40.0, "vis_raster": 220.0, "composite": 30.0}
+FP32_PEAK_TFLOPS = 2 * 128 * 148 * 1.965e9 / 1e12          # 74.4: 148 SMs x 128 FP32 lanes x FMA x 1.965 GHz (guide)
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.stop, self.th = index, [], False, None
+
+    def _run(self):
+        while not self.stop:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([t.strip() for t in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def __enter__(self):
+        self.th = threading.Thread(target=self._run, daemon=True); self.th.start(); return self
+
+    def __exit__(self, *a):
+        self.stop = True; self.th.join(timeout=6)
+
+    def summary(self):
+        sm = sorted(float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit())
+        reasons = set()
+        for r in self.rows:
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx[0] if mx else None, "reasons": sorted(reasons),
+                "samples": len(self.rows)}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle, as it stands, on the host cores (this tier's reference arm)."""
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    from synth import workloads
+    inp = workloads.make(1)
+    cores = os.cpu_count()
+    av = orc.avatar_load(inp)
+    for _ in range(max(args.warmup, 1)):
+        orc.render_frame(av, inp, vis_mode=args.vis_mode)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.render_frame(av, inp, vis_mode=args.vis_mode)
+    dt = (time.perf_counter() - t0) / args.steps
+    fps = 1.0 / dt
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": {"workload": WORKLOAD, "vis_mode": args.vis_mode},
+        "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle",
+                         "sample": "%d full frames of configs[1] (every step of the path, OpenMP on outer loops)" % args.steps},
+        "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--vis-mode", type=int, default=0, help="0 = depth test (north_star, default), 1 = paper filters")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        if args.steps == 200 and args.warmup == 20:
+            args.steps, args.warmup = 10, 1
+        return run_reference(args, rank)
+    args.warmup = max(args.warmup, 3)
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2407_10707_b200 import binding as rga
+    from synth import workloads
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    dev = torch.device("cuda", local)
+    inp = workloads.make(1, seed=1 + 1000 * rank if world > 1 else None)
+    cam = inp["camera"]; W, H = cam["width"], cam["height"]
+    K, R = len(inp["vis_dirs"]), inp["vis_res"]
+    t0 = time.perf_counter()
+    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=K, max_vis_res=R, max_env_texels=512)
+    torch.cuda.synchronize(); load_ms = (time.perf_counter() - t0) * 1e3
+    bones = torch.as_tensor(inp["bone_mats"][0]).to(dev); dirs = torch.as_tensor(inp["vis_dirs"]).to(dev)
+    env = torch.as_tensor(inp["env"][0]).to(dev); t2d = torch.as_tensor(inp["texel_to_dir"]).to(dev)
+    img = torch.empty((H, W, 3), dtype=torch.float32, device=dev)
+    camc = rga.make_camera(cam)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)            # > 126 MB L2
+    bias = (inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
+
+    def frame(b=bones, e=env):
+        av.render(b, dirs, R, e, t2d, inp["cam_pos"], camc, inp["bg"], img, vis_mode=args.vis_mode, bias=bias)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, do_flush=True):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        barrier()
+        for a, b in evs:
+            if do_flush:
+                flush.fill_(1)
+            a.record(); fn(); b.record()
+        barrier()
+        return sum(a.elapsed_time(b) for a, b in evs) / steps
+
+    for _ in range(args.warmup):
+        frame()
+    rga.rga_check(av.h)
+    l0 = rga.rga_launch_count(av.h)
+    with ClockSampler(local) as cs:
+        ms = timed(frame, args.steps)
+        launches = rga.rga_launch_count(av.h) - l0
+        ms_warm = timed(frame, args.steps, do_flush=False)
+    clocks = cs.summary()
+
+    # end to end: host (pinned) pose + env in, image out, every step, through the same C-ABI calls
+    h_bones = torch.as_tensor(inp["bone_mats"][0]).pin_memory(); h_env = torch.as_tensor(inp["env"][0]).pin_memory()
+    h_img = torch.empty((H, W, 3), dtype=torch.float32).pin_memory()
+    d_bones = torch.empty_like(bones); d_env = torch.empty_like(env)
+
+    def frame_e2e():
+        d_bones.copy_(h_bones, non_blocking=True); d_env.copy_(h_env, non_blocking=True)
+        frame(d_bones, d_env)
+        h_img.copy_(img, non_blocking=True)
+    for _ in range(3):
+        frame_e2e()
+    ms_e2e = timed(frame_e2e, args.steps)
+
+    # per-kernel times (CUDA events recorded by the library after each of its kernels), same flush protocol
+    rga.rga_profile_enable(av.h, True)
+    acc = {}
+    for _ in range(args.steps):
+        flush.fill_(1)
+        frame()
+        for name, t in rga.rga_profile_read(av.h):
+            acc.setdefault(name, []).append(t)
+    rga.rga_profile_enable(av.h, False)
+    kern_ms = {k: float(np.mean(v)) for k, v in acc.items()}
+    rga.rga_check(av.h)
+
+    # algorithmic units of each candidate dominant kernel: counted from the frame that was rendered
+    gp = av.read("GAUSS_POSED").reshape(-1, 4)[:, :3]; gn = av.read("GAUSS_NORMAL_POSED").reshape(-1, 4)[:, :3]
+    front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
+    rg = av.read("TILE_RANGES").reshape(-1, 2).astype(np.int64)
+    units = {"shade": front * 512 * 0.5, "vis_depth_test": len(gp) * K, "vis_raster": len(inp["faces"]) * K,
+             "composite": float(((rg[:, 1] - rg[:, 0]) * 256).sum())}
+    dom = max((k for k in kern_ms if k in units), key=lambda k: kern_ms[k])
+    ach = units[dom] * FLOP_PER_UNIT[dom] / (kern_ms[dom] * 1e-3) / 1e12
+    pk, pk_kind = peaks()
+    roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": ach / FP32_PEAK_TFLOPS, "traffic": None,
+                "note": "fp32 FMA-pipe peak derived from the guide (148 SM x 128 lanes x 2 x 1.965 GHz); "
+                        "HBM peak %s %.0f GB/s is not the bound of this kernel" % (pk_kind, pk["hbm_gbs"]),
+                "units_per_launch": units[dom], "flop_per_unit": FLOP_PER_UNIT[dom], "kernel_ms": kern_ms[dom]}
+
+    t = torch.tensor([ms, ms_e2e, ms_warm], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, ms_e2e, ms_warm = [float(v) for v in t.cpu()]
+    out = {
+        "metric": METRIC, "value": world * 1e3 / ms, "unit": "frames/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "vis_mode": args.vis_mode, "l2": "flushed between steps (256 MiB fill)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU", "paper_context": "6.9 fps on RTX 4090 (PAPER.md:314)"},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": {"value": world * 1e3 / ms_e2e, "unit": "frames/s", "h2d_bytes_per_step": int(h_bones.numel() * 4 + h_env.numel() * 4),
+                "d2h_bytes_per_step": int(h_img.numel() * 4)},
+        "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as orc                 # cpu_baseline leg: the oracle, untuned, on the host cores
+        oav = orc.avatar_load(inp)
+        orc.render_frame(oav, inp, vis_mode=args.vis_mode)
+        n, t0 = 0, time.perf_counter()
+        while n < 3 or (time.perf_counter() - t0 < 10.0 and n < 50):
+            orc.render_frame(oav, inp, vis_mode=args.vis_mode); n += 1
+        dt = (time.perf_counter() - t0) / n
+        out["cpu_baseline"] = {"value": 1.0 / dt, "unit": "frames/s", "cores": os.cpu_count(), "kind": "oracle",
+                               "sample": "%d full frames of configs[1], all steps, OpenMP outer loops" % n}
+    if rank == 0:
+        print(json.dumps(out))
+    av.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

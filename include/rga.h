@@ -174,6 +174,12 @@ RGA_API rga_status rga_check(rga_avatar* av, void* stream);
 /* Number of kernels the library has launched since the avatar was loaded (bench.py's gpu_launches claim). */
 RGA_API int64_t rga_launch_count(const rga_avatar* av);
 
+/* Optional per-kernel timing.  While enabled, the library records a CUDA event on `stream` after each of its kernels.
+ * rga_profile_read synchronises `stream`, writes up to `capacity` entries (names: capacity x 32 chars, ms: elapsed
+ * milliseconds of each kernel since the previous event) and clears the log.  Not graph-capturable while enabled. */
+RGA_API rga_status rga_profile_enable(rga_avatar* av, int on);
+RGA_API rga_status rga_profile_read(rga_avatar* av, void* stream, char* names, float* ms, int capacity, int* count);
+
 RGA_API const char* rga_last_error(void);
 RGA_API const char* rga_version(void);
 

@@ -79,6 +79,8 @@ def lib():
         L.rga_get_buffer.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
         L.rga_read_buffer.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
         L.rga_check.argtypes = [C.c_void_p, C.c_void_p]
+        L.rga_profile_enable.argtypes = [C.c_void_p, C.c_int]
+        L.rga_profile_read.argtypes = [C.c_void_p, C.c_void_p, C.c_char_p, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_int)]
         _lib = L
     return _lib
 
@@ -168,6 +170,19 @@ def splat_render(h, camera, bg, out_image):
 
 def rga_check(h):
     _chk(lib().rga_check(h, _stream()))
+
+
+def rga_profile_enable(h, on):
+    _chk(lib().rga_profile_enable(h, int(on)))
+
+
+def rga_profile_read(h, capacity=96):
+    """-> list of (kernel name, milliseconds) recorded since the last read."""
+    names = C.create_string_buffer(32 * capacity)
+    ms = (C.c_float * capacity)()
+    n = C.c_int(0)
+    _chk(lib().rga_profile_read(h, _stream(), names, ms, capacity, C.byref(n)))
+    return [(names.raw[32 * i:32 * i + 32].split(b"\0")[0].decode(), float(ms[i])) for i in range(n.value)]
 
 
 def rga_launch_count(h):

@@ -21,6 +21,34 @@ extern "C" const char* rga_last_error(void) { return g_err; }
 extern "C" const char* rga_version(void) { return "rga 0.1 (sm_100a)"; }
 extern "C" int64_t rga_launch_count(const rga_avatar* av) { return av ? av->launches : 0; }
 
+void rga_prof_mark(rga_avatar* av, const char* name, cudaStream_t s) {
+  if (!av->prof_on || av->prof_n >= RGA_MAX_PROF) return;
+  if (!av->prof_ev[av->prof_n]) cudaEventCreate(&av->prof_ev[av->prof_n]);
+  cudaEventRecord(av->prof_ev[av->prof_n], s);
+  av->prof_name[av->prof_n++] = name;
+}
+
+extern "C" rga_status rga_profile_enable(rga_avatar* av, int on) {
+  if (!av) return fail(RGA_ERR_INVALID_ARG, "rga_profile_enable: null avatar");
+  av->prof_on = on; av->prof_n = 0;
+  return RGA_OK;
+}
+
+extern "C" rga_status rga_profile_read(rga_avatar* av, void* stream, char* names, float* ms, int capacity, int* count) {
+  if (!av || !names || !ms || !count) return fail(RGA_ERR_INVALID_ARG, "rga_profile_read: null argument");
+  CU(cudaStreamSynchronize((cudaStream_t)stream));
+  int n = 0;
+  for (int i = 1; i < av->prof_n && n < capacity; ++i) {
+    if (av->prof_name[i][0] == '-') continue;                      // API-entry boundary marks carry no kernel
+    float t = 0.f;
+    CU(cudaEventElapsedTime(&t, av->prof_ev[i - 1], av->prof_ev[i]));
+    snprintf(names + 32 * n, 32, "%s", av->prof_name[i]);
+    ms[n++] = t;
+  }
+  *count = n; av->prof_n = 0;
+  return RGA_OK;
+}
+
 template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)); }
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
@@ -32,6 +60,7 @@ extern "C" rga_status avatar_free(rga_avatar* av) {
                   av->keys[1], av->vals[0], av->vals[1], av->sort_hist, av->num_dup, av->ranges, av->t_final, av->n_contrib,
                   av->status};
   for (void* p : ptrs) if (p) cudaFree(p);
+  for (int i = 0; i < RGA_MAX_PROF; ++i) if (av->prof_ev[i]) cudaEventDestroy(av->prof_ev[i]);
   delete av;
   return RGA_OK;
 }
@@ -111,6 +140,7 @@ done:
 extern "C" rga_status pose_skin(rga_avatar* av, const float* bone_mats, void* stream) {
   if (!av || !bone_mats) return fail(RGA_ERR_INVALID_ARG, "pose_skin: null argument");
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
+  rga_prof_mark(av, "-", (cudaStream_t)stream);
   CU(rga_launch_skin(av, bone_mats, (cudaStream_t)stream));
   av->have_skin = 1;
   return RGA_OK;
@@ -123,6 +153,7 @@ extern "C" rga_status visibility_raster(rga_avatar* av, const rga_vis_params* p,
     return fail(RGA_ERR_INVALID_ARG, "visibility_raster: n_dirs/res/mode out of range");
   cudaStream_t s = (cudaStream_t)stream;
   av->have_vis = av->have_shade = av->have_splat = 0;
+  rga_prof_mark(av, "-", s);
   CU(rga_launch_vis_raster(av, p, s));
   if (p->mode == 0) CU(rga_launch_vis_depth_test(av, p, s));
   else CU(rga_launch_vis_paper(av, p, s));
@@ -142,6 +173,7 @@ extern "C" rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const 
     return fail(RGA_ERR_INVALID_ARG, "shade_gaussians: identity texel_to_dir needs rows*cols == n_dirs");
   cudaStream_t s = (cudaStream_t)stream;
   av->have_shade = av->have_splat = 0;
+  rga_prof_mark(av, "-", s);
   CU(rga_launch_env_table(av, env, s));
   CU(rga_launch_shade(av, env, make_float3(cam_pos[0], cam_pos[1], cam_pos[2]), env->use_visibility ? av->vis_mode : 2, s));
   av->have_shade = 1;
@@ -156,6 +188,7 @@ extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const 
   cudaStream_t s = (cudaStream_t)stream;
   int TX = (cam->width + 15) / 16, TY = (cam->height + 15) / 16, ntiles = TX * TY;
   int tile_bits = 0; while ((1 << tile_bits) < ntiles) ++tile_bits;
+  rga_prof_mark(av, "-", s);
   CU(rga_launch_project(av, cam, s));
   CU(rga_launch_scan_emit(av, TX, s));
   CU(rga_launch_sort(av, 32 + tile_bits, s));

@@ -58,5 +58,6 @@ cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 b
   composite_kernel<<<dim3(TX, TY), CB, 0, s>>>(cam->width, cam->height, TX, av->ranges, av->vals[av->sorted_buf], av->mu2d,
                                                av->conic_o, av->color, bg, out, av->t_final, av->n_contrib);
   av->launches += 1;
+  rga_prof_mark(av, "composite", s);
   return cudaGetLastError();
 }

@@ -104,5 +104,6 @@ cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream
   project_kernel<<<grid, 256, 0, s>>>(av->n_gauss, k, av->g_posed, av->g_nposed, av->g_cov, av->g_scale_op, av->mu2d,
                                       av->depth, av->conic_o, av->rect, av->touched, av->offsets);
   av->launches += 1;
+  rga_prof_mark(av, "project", s);
   return cudaGetLastError();
 }

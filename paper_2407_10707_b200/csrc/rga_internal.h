@@ -6,6 +6,7 @@
 #include "../../include/rga.h"
 
 #define RGA_TILE 16
+#define RGA_MAX_PROF 96
 
 struct rga_avatar {
   // sizes
@@ -60,7 +61,12 @@ struct rga_avatar {
   int vis_mode, vis_dirs, vis_res, vis_words, keep_maps;
   int cam_w, cam_h;
   long long launches;
+  // optional per-kernel timing (rga_profile_enable): an event after every kernel, one at every API entry
+  int prof_on, prof_n;
+  cudaEvent_t prof_ev[RGA_MAX_PROF];
+  const char* prof_name[RGA_MAX_PROF];
 };
+void rga_prof_mark(rga_avatar* av, const char* name, cudaStream_t s);
 
 // ---- launchers (each returns cudaGetLastError()) ----
 // load_kernels.cu

@@ -28,6 +28,7 @@ cudaError_t rga_launch_env_table(rga_avatar* av, const rga_env* env, cudaStream_
   int n = env->rows * env->cols;
   env_table_kernel<<<(n + 127) / 128, 128, 0, s>>>(env->rows, env->cols, env->radiance, av->env_table);
   av->launches += 1;
+  rga_prof_mark(av, "env_table", s);
   return cudaGetLastError();
 }
 
@@ -145,6 +146,7 @@ cudaError_t rga_launch_shade(rga_avatar* av, const rga_env* env, float3 cam, int
   else if (vis_mode == 1) shade_kernel<L, 1><<<grid, 128, smem, s>>>(SHADE_ARGS);
   else shade_kernel<L, 2><<<grid, 128, smem, s>>>(SHADE_ARGS);
   av->launches += 1;
+  rga_prof_mark(av, "shade", s);
   return cudaGetLastError();
 }
 

@@ -123,7 +123,9 @@ cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, cudaStream_t
   skin_kernel<<<vblocks + gblocks, 256, av->n_bones * 12 * sizeof(float), s>>>(
       av->n_verts, av->n_gauss, av->n_bones, vblocks, bone_mats, av->v_xbar, av->v_normal, av->v_skin_w, av->g_static,
       av->g_skin_w, av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->aabb);
+  rga_prof_mark(av, "skin", s);
   window_kernel<<<1, 1, 0, s>>>(av->aabb, av->window);
+  rga_prof_mark(av, "window", s);
   av->launches += 2;
   return cudaGetLastError();
 }

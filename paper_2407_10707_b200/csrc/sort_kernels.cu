@@ -55,6 +55,7 @@ cudaError_t rga_launch_scan_emit(rga_avatar* av, int tiles_x, cudaStream_t s) {
   emit_kernel<<<nblocks, 256, 0, s>>>(av->n_gauss, nblocks, tiles_x, av->max_dup, av->offsets, av->touched, av->rect, av->depth,
                                       av->keys[0], av->vals[0], av->num_dup, av->status);
   av->launches += 1;
+  rga_prof_mark(av, "scan_emit", s);
   return cudaGetLastError();
 }
 
@@ -164,6 +165,7 @@ cudaError_t rga_launch_sort(rga_avatar* av, int key_bits, cudaStream_t s) {
   }
   av->sorted_buf = cur;
   av->launches += 3 * passes;
+  rga_prof_mark(av, "radix_sort", s);
   return cudaGetLastError();
 }
 
@@ -182,5 +184,6 @@ cudaError_t rga_launch_ranges(rga_avatar* av, int ntiles, cudaStream_t s) {
   cudaMemsetAsync(av->ranges, 0, (size_t)ntiles * sizeof(uint2), s);
   ranges_kernel<<<av->num_sms * 4, 256, 0, s>>>(av->keys[av->sorted_buf], av->num_dup, av->ranges);
   av->launches += 1;
+  rga_prof_mark(av, "tile_ranges", s);
   return cudaGetLastError();
 }

@@ -164,6 +164,7 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
                                                     p->dirs, av->window, av->zmap, av->idmap, nullptr, words, av->n_verts);
   }
   av->launches += 1;
+  rga_prof_mark(av, "vis_raster", s);
   return cudaGetLastError();
 }
 
@@ -233,6 +234,7 @@ cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, c
       av->n_gauss, p->n_dirs, p->res, av->g_posed, av->g_nposed, p->dirs, av->window, av->zmap, p->depth_bias_texels,
       p->depth_bias_world, p->slope_max, av->visbits);
   av->launches += 1;
+  rga_prof_mark(av, "vis_depth_test", s);
   return cudaGetLastError();
 }
 
@@ -305,8 +307,11 @@ cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaSt
   int words = (p->n_dirs + 31) / 32;
   int n = av->n_verts * words, grid = (n + 255) / 256;
   vis_median_kernel<<<grid, 256, 0, s>>>(av->n_verts, words, av->k_v, av->knn_v, av->vbits_raw, av->vbits_a);
+  rga_prof_mark(av, "vis_median1", s);
   vis_median_kernel<<<grid, 256, 0, s>>>(av->n_verts, words, av->k_v, av->knn_v, av->vbits_a, av->vbits_b);
+  rga_prof_mark(av, "vis_median2", s);
   vis_mean_kernel<<<grid, 256, 0, s>>>(av->n_verts, words, p->n_dirs, av->k_v, av->knn_v, av->vbits_b, av->vcount);
+  rga_prof_mark(av, "vis_mean", s);
   av->launches += 3;
   return cudaGetLastError();
 }
