@@ -8,6 +8,7 @@
 
 int rga_shade_init_attributes(int max_env);
 int rga_vis_init_attributes();
+int rga_composite_init_attributes();
 
 static thread_local char g_err[512] = "";
 static rga_status fail(rga_status st, const char* fmt, ...) {
@@ -56,8 +57,8 @@ extern "C" rga_status avatar_free(rga_avatar* av) {
   void* ptrs[] = {av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
-                  av->radiance, av->color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->offsets, av->keys[0],
-                  av->keys[1], av->vals[0], av->vals[1], av->sort_hist, av->num_dup, av->ranges, av->t_final, av->n_contrib,
+                  av->radiance, av->color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->cursor, av->keys[0],
+                  av->keys[1], av->vals[0], av->num_dup, av->ranges, av->t_final, av->n_contrib,
                   av->status};
   for (void* p : ptrs) if (p) cudaFree(p);
   for (int i = 0; i < RGA_MAX_PROF; ++i) if (av->prof_ev[i]) cudaEventDestroy(av->prof_ev[i]);
@@ -107,10 +108,10 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->vcount, nv * (size_t)av->max_dirs + 32)); A(dalloc(&av->env_table, 8 * (size_t)av->max_env));
   A(dalloc(&av->radiance, ng)); A(dalloc(&av->color, ng));
   A(dalloc(&av->mu2d, ng)); A(dalloc(&av->depth, ng)); A(dalloc(&av->conic_o, ng)); A(dalloc(&av->rect, ng)); A(dalloc(&av->touched, ng));
-  A(dalloc(&av->offsets, (ng + 255) / 256 + 1));
+  A(dalloc(&av->tile_count, ntiles)); A(dalloc(&av->cursor, ntiles));
   A(dalloc(&av->keys[0], (size_t)av->max_dup)); A(dalloc(&av->keys[1], (size_t)av->max_dup));
-  A(dalloc(&av->vals[0], (size_t)av->max_dup)); A(dalloc(&av->vals[1], (size_t)av->max_dup));
-  A(dalloc(&av->sort_hist, 256 * (size_t)av->num_sms * 2)); A(dalloc(&av->num_dup, 1)); A(dalloc(&av->ranges, ntiles));
+  A(dalloc(&av->vals[0], (size_t)av->max_dup));
+  A(dalloc(&av->num_dup, 1)); A(dalloc(&av->ranges, ntiles));
   A(dalloc(&av->t_final, npix)); A(dalloc(&av->n_contrib, npix)); A(dalloc(&av->status, 1));
   A(cudaMemsetAsync(av->status, 0, sizeof(int), s)); A(cudaMemsetAsync(av->num_dup, 0, sizeof(unsigned), s));
   {
@@ -127,7 +128,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(rga_launch_knn(d->gauss_pos, av->n_gauss, d->vert_pos, av->n_verts, av->k_g, av->knn_g, d2, s));
   A(rga_launch_load_gauss(av, d, d2, s));
   av->launches += 4;
-  if (rga_shade_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
+  if (rga_shade_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_composite_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
   A(cudaStreamSynchronize(s));
 done:
   if (d2) cudaFree(d2);
@@ -187,12 +188,9 @@ extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const 
     return fail(RGA_ERR_INVALID_ARG, "splat_render: camera larger than max_width/max_height");
   cudaStream_t s = (cudaStream_t)stream;
   int TX = (cam->width + 15) / 16, TY = (cam->height + 15) / 16, ntiles = TX * TY;
-  int tile_bits = 0; while ((1 << tile_bits) < ntiles) ++tile_bits;
   rga_prof_mark(av, "-", s);
   CU(rga_launch_project(av, cam, s));
-  CU(rga_launch_scan_emit(av, TX, s));
-  CU(rga_launch_sort(av, 32 + tile_bits, s));
-  CU(rga_launch_ranges(av, ntiles, s));
+  CU(rga_launch_bin(av, TX, ntiles, s));
   CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
   av->have_splat = 1;
@@ -217,7 +215,7 @@ extern "C" rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, co
     unsigned d = 0;
     CU(cudaMemcpyAsync(&d, av->num_dup, 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CU(cudaStreamSynchronize((cudaStream_t)stream));
-    D = d;
+    D = d; if ((long long)D > av->max_dup) D = (size_t)av->max_dup;
   }
   const void* p = nullptr; size_t n = 0;
   switch (which) {
@@ -244,8 +242,8 @@ extern "C" rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, co
     case RGA_BUF_RECT: p = av->rect; n = ng * 16; break;
     case RGA_BUF_TOUCHED: p = av->touched; n = ng * 4; break;
     case RGA_BUF_NUM_DUPLICATES: p = av->num_dup; n = 4; break;
-    case RGA_BUF_KEYS_SORTED: p = av->keys[av->sorted_buf]; n = D * 8; break;
-    case RGA_BUF_VALS_SORTED: p = av->vals[av->sorted_buf]; n = D * 4; break;
+    case RGA_BUF_KEYS_SORTED: p = av->keys[1]; n = D * 8; break;
+    case RGA_BUF_VALS_SORTED: p = av->vals[0]; n = D * 4; break;
     case RGA_BUF_TILE_RANGES: p = av->ranges; n = ntiles * 8; break;
     case RGA_BUF_T_FINAL: p = av->t_final; n = npix * 4; break;
     case RGA_BUF_N_CONTRIB: p = av->n_contrib; n = npix * 4; break;

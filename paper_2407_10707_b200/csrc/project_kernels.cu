@@ -1,7 +1,7 @@
 // H6 projection + culling (PAPER.md:101 back-face rule; "the Gaussian rasterizer of 3DGS" -> ref [8];
 // DESIGN.md readings A8, A18, A21).  EXACT file (-fmad=false): tile rects and sort keys are integer outputs of this
 // arithmetic, so the operation order is the one fixed in DESIGN.md "Arithmetic contract".
-// Also accumulates per-block sums of tiles_touched for the offset scan of H7.
+// Also accumulates the per-tile histogram (the tile digit of the H8 sort).
 #include "rga_internal.h"
 
 struct CamK {
@@ -12,7 +12,7 @@ struct CamK {
 __global__ void __launch_bounds__(256) project_kernel(int ng, CamK cam, const float4* __restrict__ g_posed,
     const float4* __restrict__ g_nposed, const float* __restrict__ g_cov, const float4* __restrict__ g_scale_op,
     float2* __restrict__ mu2d, float* __restrict__ depth, float4* __restrict__ conic_o, int4* __restrict__ rect,
-    unsigned* __restrict__ touched, unsigned* __restrict__ block_sums) {
+    unsigned* __restrict__ touched, unsigned* __restrict__ tile_count) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   unsigned cnt = 0;
   if (g < ng) {
@@ -66,18 +66,9 @@ __global__ void __launch_bounds__(256) project_kernel(int ng, CamK cam, const fl
       }
     }
     mu2d[g] = mu; depth[g] = dep; conic_o[g] = co; rect[g] = rc; touched[g] = cnt;
-  }
-  // block sum of tiles touched (input of the H7 offset scan)
-  __shared__ unsigned wsum[8];
-  unsigned v = cnt;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = v;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    unsigned tot = 0;
-    for (int w = 0; w < 8; ++w) tot += wsum[w];
-    block_sums[blockIdx.x] = tot;
+    // histogram of the tile digit (first pass of the (tile, depth) sort, sort_kernels.cu)
+    for (int y = rc.y; y < rc.w; ++y)
+      for (int x = rc.x; x < rc.z; ++x) atomicAdd(tile_count + (y * cam.TX + x), 1u);
   }
 }
 
@@ -101,8 +92,9 @@ cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream
     k.C[r] = -abc;
   }
   int grid = (av->n_gauss + 255) / 256;
+  cudaMemsetAsync(av->tile_count, 0, (size_t)k.TX * k.TY * sizeof(unsigned), s);
   project_kernel<<<grid, 256, 0, s>>>(av->n_gauss, k, av->g_posed, av->g_nposed, av->g_cov, av->g_scale_op, av->mu2d,
-                                      av->depth, av->conic_o, av->rect, av->touched, av->offsets);
+                                      av->depth, av->conic_o, av->rect, av->touched, av->tile_count);
   av->launches += 1;
   rga_prof_mark(av, "project", s);
   return cudaGetLastError();

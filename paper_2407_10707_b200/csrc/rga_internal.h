@@ -47,10 +47,9 @@ struct rga_avatar {
   float4* radiance;    // [n_gauss]
   float4* color;       // [n_gauss]
   // splat
-  float2* mu2d; float* depth; float4* conic_o; int4* rect; unsigned* touched; unsigned* offsets;
-  unsigned* scan_state;        // decoupled look-back tile states
-  unsigned long long* keys[2]; unsigned* vals[2];
-  unsigned* sort_hist;         // radix histograms
+  float2* mu2d; float* depth; float4* conic_o; int4* rect; unsigned* touched;
+  unsigned* tile_count; unsigned* cursor;   // [tiles] histogram of the tile digit, scatter cursors
+  unsigned long long* keys[2]; unsigned* vals[2];   // keys[0]: binned local keys (depth<<32|g); keys[1]/vals[0]: sorted output
   unsigned* num_dup;           // [1] D (device)
   uint2* ranges;               // [tiles]
   float* t_final; unsigned* n_contrib;
@@ -85,8 +84,6 @@ cudaError_t rga_launch_env_table(rga_avatar* av, const rga_env* env, cudaStream_
 cudaError_t rga_launch_shade(rga_avatar* av, const rga_env* env, float3 cam, int vis_mode, cudaStream_t s);
 // splat_kernels.cu
 cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream_t s);
-cudaError_t rga_launch_scan_emit(rga_avatar* av, int tiles_x, cudaStream_t s);
-cudaError_t rga_launch_sort(rga_avatar* av, int key_bits, cudaStream_t s);
-cudaError_t rga_launch_ranges(rga_avatar* av, int ntiles, cudaStream_t s);
+cudaError_t rga_launch_bin(rga_avatar* av, int TX, int ntiles, cudaStream_t s);
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s);
 int rga_init_kernel_attributes();

@@ -42,14 +42,61 @@ __device__ __forceinline__ void light_project(float x, float y, float z, const W
 
 // ------------------------------------------------------------------------------------------------------------- H3
 // One CTA per (direction, band of rows).  The band's depth map lives in shared memory: u32 depth (mode 0) or
-// u64 depth<<32|triangle (WITH_ID).  Every thread walks triangles with a block stride, projects the three corners,
-// and scans the (tiny) pixel bounding box with int64 edge functions at 1/256-pixel snapped coordinates.
+// u64 depth<<32|triangle (WITH_ID).  Threads walk the triangles with a block stride.  A triangle whose clipped pixel
+// box is small is rasterised by its own thread with incremental int32 edge functions; the rare large ones (slivers,
+// close-ups) are queued in shared memory and rasterised cooperatively, one warp per triangle and one lane per pixel,
+// so a long triangle never stalls the 31 other lanes of its warp (ncu on the first version: 7 of 32 lanes active).
+// Coverage and depth follow DESIGN.md "Arithmetic contract" exactly: vertices snapped to 1/256 pixel, integer edge
+// functions (inclusive, two-sided), z = (z0 + (e1/area)(z1-z0)) + (e2/area)(z2-z0) in fp32, clamped at 0.
+#define RAST_THREADS 512
+#define RAST_QCAP 2048
+#define RAST_SMALL 12          // pixel-box size up to which a thread rasterises its own triangle
+
+struct TriSetup {
+  int x0, y0, x1, y1, x2, y2;          // 1/256-pixel coordinates
+  float z0, z1, z2;
+  int ia, ib, ja, jb;                  // pixel box clipped to the map and the band
+  bool ok;                             // non-degenerate and touching the band
+  bool narrow;                         // unclipped box below 2^14 sub-pixels in x and y: edge functions fit int32
+};
+
+__device__ __forceinline__ TriSetup tri_setup(int t, const int* __restrict__ faces, const float4* __restrict__ v_posed,
+                                              const WinConst& W, const LightFrame& F, int R, int row0, int rows) {
+  TriSetup s;
+  int i0 = __ldg(faces + 3 * t), i1 = __ldg(faces + 3 * t + 1), i2 = __ldg(faces + 3 * t + 2);
+  float4 a = __ldg(v_posed + i0), b = __ldg(v_posed + i1), c = __ldg(v_posed + i2);
+  float px, py;
+  light_project(a.x, a.y, a.z, W, F, px, py, s.z0);
+  s.x0 = __float2int_rn(px * 256.0f); s.y0 = __float2int_rn(py * 256.0f);
+  light_project(b.x, b.y, b.z, W, F, px, py, s.z1);
+  s.x1 = __float2int_rn(px * 256.0f); s.y1 = __float2int_rn(py * 256.0f);
+  light_project(c.x, c.y, c.z, W, F, px, py, s.z2);
+  s.x2 = __float2int_rn(px * 256.0f); s.y2 = __float2int_rn(py * 256.0f);
+  int mnx = min(s.x0, min(s.x1, s.x2)), mxx = max(s.x0, max(s.x1, s.x2));
+  int mny = min(s.y0, min(s.y1, s.y2)), mxy = max(s.y0, max(s.y1, s.y2));
+  // pixel i has its centre at 256 i + 128: first centre >= mn, last centre <= mx
+  s.ia = max((mnx + 127) >> 8, 0); s.ib = min((mxx - 128) >> 8, R - 1);
+  s.ja = max((mny + 127) >> 8, row0); s.jb = min((mxy - 128) >> 8, row0 + rows - 1);
+  s.narrow = (mxx - mnx) < 16384 && (mxy - mny) < 16384;
+  s.ok = s.ia <= s.ib && s.ja <= s.jb;
+  return s;
+}
+
 template <bool WITH_ID>
-__global__ void __launch_bounds__(512) vis_raster_kernel(int nf, int R, int band_rows, int n_bands, int nv_words,
+__device__ __forceinline__ void put_sample(unsigned* sz32, unsigned long long* sz64, int p, float z, int t) {
+  z = fmaxf(z, 0.0f);
+  if (WITH_ID) atomicMin(sz64 + p, ((unsigned long long)__float_as_uint(z) << 32) | (unsigned)t);
+  else atomicMin(sz32 + p, __float_as_uint(z));
+}
+
+template <bool WITH_ID>
+__global__ void __launch_bounds__(RAST_THREADS) vis_raster_kernel(int nf, int R, int band_rows, int n_bands, int nv_words,
     const float4* __restrict__ v_posed, const int* __restrict__ faces, const float* __restrict__ dirs,
     const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
     unsigned* __restrict__ vbits_raw, int words, int n_verts) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ int s_queue[RAST_QCAP];
+  __shared__ int s_qn;
   const int k = blockIdx.x / n_bands, band = blockIdx.x % n_bands;
   const int row0 = band * band_rows, rows = min(band_rows, R - row0);
   const int npix = rows * R;
@@ -62,54 +109,85 @@ __global__ void __launch_bounds__(512) vis_raster_kernel(int nf, int R, int band
   } else {
     for (int p = threadIdx.x; p < npix; p += blockDim.x) sz32[p] = 0xffffffffu;
   }
+  if (threadIdx.x == 0) s_qn = 0;
   const LightFrame F = make_frame(dirs + 3 * k);
   const WinConst W = make_win(window, R);
   __syncthreads();
-  const long long ylo = 256ll * row0, yhi = 256ll * (row0 + rows);        // band covers pixel centres 256j+128, j in [row0,row0+rows)
-  for (int t = threadIdx.x; t < nf; t += blockDim.x) {
-    int i0 = __ldg(faces + 3 * t), i1 = __ldg(faces + 3 * t + 1), i2 = __ldg(faces + 3 * t + 2);
-    float4 a = __ldg(v_posed + i0), b = __ldg(v_posed + i1), c = __ldg(v_posed + i2);
-    float px, py, z0, z1, z2;
-    light_project(a.x, a.y, a.z, W, F, px, py, z0);
-    long long x0 = __float2int_rn(px * 256.0f), y0 = __float2int_rn(py * 256.0f);
-    light_project(b.x, b.y, b.z, W, F, px, py, z1);
-    long long x1 = __float2int_rn(px * 256.0f), y1 = __float2int_rn(py * 256.0f);
-    light_project(c.x, c.y, c.z, W, F, px, py, z2);
-    long long x2 = __float2int_rn(px * 256.0f), y2 = __float2int_rn(py * 256.0f);
-    long long mny = min(y0, min(y1, y2)), mxy = max(y0, max(y1, y2));
-    if (mxy < ylo + 128 || mny > yhi - 128) continue;                       // no pixel centre of this band inside
-    long long area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
-    if (area == 0) continue;
-    long long mnx = min(x0, min(x1, x2)), mxx = max(x0, max(x1, x2));
-    int ia = (int)max((mnx - 128 + 255) >> 8, 0ll), ib = (int)min((mxx - 128) >> 8, (long long)(R - 1));
-    int ja = (int)max((mny - 128 + 255) >> 8, (long long)row0), jb = (int)min((mxy - 128) >> 8, (long long)(row0 + rows - 1));
-    float fa = (float)area;
-    for (int j = ja; j <= jb; ++j) {
-      long long qy = 256ll * j + 128;
-      for (int i = ia; i <= ib; ++i) {
-        long long qx = 256ll * i + 128;
-        long long e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
-        long long e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
-        long long e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
-        bool in = (e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0);
-        if (!in) continue;
-        float t1 = (float)e1 / fa, t2 = (float)e2 / fa;
-        float z = (z0 + t1 * (z1 - z0)) + t2 * (z2 - z0);
-        z = fmaxf(z, 0.0f);
-        int p = (j - row0) * R + i;
-        if (WITH_ID) atomicMin(sz64 + p, ((unsigned long long)__float_as_uint(z) << 32) | (unsigned)t);
-        else atomicMin(sz32 + p, __float_as_uint(z));
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+
+  for (int base = 0; base < nf; base += blockDim.x) {
+    const int t = base + threadIdx.x;
+    if (t < nf) {
+      const TriSetup s = tri_setup(t, faces, v_posed, W, F, R, row0, rows);
+      if (s.ok) {
+        const int bw = s.ib - s.ia + 1, bh = s.jb - s.ja + 1;
+        if (s.narrow && bw * bh <= RAST_SMALL) {
+          // int32 edge functions, orientation normalised so that "inside" is e0,e1,e2 >= 0
+          int area = (s.x1 - s.x0) * (s.y2 - s.y0) - (s.y1 - s.y0) * (s.x2 - s.x0);
+          if (area != 0) {
+            const int sg = area > 0 ? 1 : -1;
+            const int qx = 256 * s.ia + 128, qy = 256 * s.ja + 128;
+            int r0 = sg * ((s.x2 - s.x1) * (qy - s.y1) - (s.y2 - s.y1) * (qx - s.x1));
+            int r1 = sg * ((s.x0 - s.x2) * (qy - s.y2) - (s.y0 - s.y2) * (qx - s.x2));
+            int r2 = sg * ((s.x1 - s.x0) * (qy - s.y0) - (s.y1 - s.y0) * (qx - s.x0));
+            const int ax0 = -sg * 256 * (s.y2 - s.y1), ax1 = -sg * 256 * (s.y0 - s.y2), ax2 = -sg * 256 * (s.y1 - s.y0);
+            const int ay0 = sg * 256 * (s.x2 - s.x1), ay1 = sg * 256 * (s.x0 - s.x2), ay2 = sg * 256 * (s.x1 - s.x0);
+            const float fa = (float)(sg * area), d1 = s.z1 - s.z0, d2 = s.z2 - s.z0;
+            for (int j = s.ja; j <= s.jb; ++j) {
+              int e0 = r0, e1 = r1, e2 = r2;
+              for (int i = s.ia; i <= s.ib; ++i) {
+                if ((e0 | e1 | e2) >= 0) {
+                  float t1 = (float)e1 / fa, t2 = (float)e2 / fa;
+                  put_sample<WITH_ID>(sz32, sz64, (j - row0) * R + i, (s.z0 + t1 * d1) + t2 * d2, t);
+                }
+                e0 += ax0; e1 += ax1; e2 += ax2;
+              }
+              r0 += ay0; r1 += ay1; r2 += ay2;
+            }
+          }
+        } else {
+          int slot = atomicAdd(&s_qn, 1);
+          if (slot < RAST_QCAP) s_queue[slot] = t;       // cannot overflow: drained whenever fewer than blockDim slots remain
+        }
       }
     }
+    __syncthreads();
+    const int qn = s_qn;
+    const bool last = base + (int)blockDim.x >= nf;
+    if (qn > 0 && (last || qn > RAST_QCAP - (int)blockDim.x)) {
+      for (int e = warp; e < qn; e += nwarps) {            // one warp per queued triangle, one lane per pixel of its box
+        const int tq = s_queue[e];
+        const TriSetup s = tri_setup(tq, faces, v_posed, W, F, R, row0, rows);
+        const long long x0 = s.x0, y0 = s.y0, x1 = s.x1, y1 = s.y1, x2 = s.x2, y2 = s.y2;
+        const long long area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
+        if (area == 0) continue;
+        const int bw = s.ib - s.ia + 1, cnt = bw * (s.jb - s.ja + 1);
+        const float fa = (float)area, d1 = s.z1 - s.z0, d2 = s.z2 - s.z0;
+        for (int q = lane; q < cnt; q += 32) {
+          const int j = s.ja + q / bw, i = s.ia + q % bw;
+          const long long qx = 256ll * i + 128, qy = 256ll * j + 128;
+          const long long e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
+          const long long e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
+          const long long e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
+          if ((e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0)) {
+            float t1 = (float)e1 / fa, t2 = (float)e2 / fa;
+            put_sample<WITH_ID>(sz32, sz64, (j - row0) * R + i, (s.z0 + t1 * d1) + t2 * d2, tq);
+          }
+        }
+      }
+      __syncthreads();
+      if (threadIdx.x == 0) s_qn = 0;
+    }
+    __syncthreads();
   }
-  __syncthreads();
-  size_t base = ((size_t)k * R + row0) * R;
+
+  size_t gbase = ((size_t)k * R + row0) * R;
   if (WITH_ID) {
     for (int p = threadIdx.x; p < npix; p += blockDim.x) {
       unsigned long long key = sz64[p];
-      zmap[base + p] = (unsigned)(key >> 32);
+      zmap[gbase + p] = (unsigned)(key >> 32);
       int tri = (key == ~0ull) ? -1 : (int)(unsigned)(key & 0xffffffffu);
-      idmap[base + p] = tri;
+      idmap[gbase + p] = tri;
       if (vbits_raw && tri >= 0) {                      // a triangle that appears marks its 3 vertices
         int v0 = __ldg(faces + 3 * tri), v1 = __ldg(faces + 3 * tri + 1), v2 = __ldg(faces + 3 * tri + 2);
         atomicOr(svert + (v0 >> 5), 1u << (v0 & 31));
@@ -130,7 +208,7 @@ __global__ void __launch_bounds__(512) vis_raster_kernel(int nf, int R, int band
       }
     }
   } else {
-    for (int p = threadIdx.x; p < npix; p += blockDim.x) zmap[base + p] = sz32[p];
+    for (int p = threadIdx.x; p < npix; p += blockDim.x) zmap[gbase + p] = sz32[p];
   }
 }
 
@@ -157,10 +235,10 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
   if (with_id) {
     unsigned* raw = (p->mode == 1) ? av->vbits_raw : nullptr;
     if (raw) cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s);
-    vis_raster_kernel<true><<<grid, 512, smem, s>>>(av->n_faces, p->res, band_rows, n_bands, nv_words, av->v_posed, av->faces,
+    vis_raster_kernel<true><<<grid, RAST_THREADS, smem, s>>>(av->n_faces, p->res, band_rows, n_bands, nv_words, av->v_posed, av->faces,
                                                    p->dirs, av->window, av->zmap, av->idmap, raw, words, av->n_verts);
   } else {
-    vis_raster_kernel<false><<<grid, 512, smem, s>>>(av->n_faces, p->res, band_rows, n_bands, nv_words, av->v_posed, av->faces,
+    vis_raster_kernel<false><<<grid, RAST_THREADS, smem, s>>>(av->n_faces, p->res, band_rows, n_bands, nv_words, av->v_posed, av->faces,
                                                     p->dirs, av->window, av->zmap, av->idmap, nullptr, words, av->n_verts);
   }
   av->launches += 1;
@@ -176,12 +254,17 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
 #define DT_THREADS 128
 __global__ void __launch_bounds__(DT_THREADS) vis_depth_test_kernel(int ng, int K, int R, const float4* __restrict__ g_posed,
     const float4* __restrict__ g_nposed, const float* __restrict__ dirs, const float* __restrict__ window,
-    const unsigned* __restrict__ zmap, float bias_texels, float bias_world, float slope_max, unsigned* __restrict__ visbits) {
-  extern __shared__ float sF[];                                   // K x 9 light frames
-  for (int k = threadIdx.x; k < K; k += blockDim.x) {
+    const unsigned* __restrict__ zmap, float bias_texels, float bias_world, float slope_max, int words_per_part,
+    unsigned* __restrict__ visbits) {
+  extern __shared__ float sF[];                                   // light frames of this CTA's slice of directions
+  const int words = (K + 31) >> 5;
+  const int wd0 = blockIdx.y * words_per_part, wd1 = min(words, wd0 + words_per_part);
+  const int k0 = wd0 * 32, k1 = min(K, wd1 * 32);
+  for (int k = k0 + threadIdx.x; k < k1; k += blockDim.x) {
     LightFrame f = make_frame(dirs + 3 * k);
+    float* o = sF + 9 * (k - k0);
 #pragma unroll
-    for (int c = 0; c < 3; ++c) { sF[9 * k + c] = f.u[c]; sF[9 * k + 3 + c] = f.v[c]; sF[9 * k + 6 + c] = f.w[c]; }
+    for (int c = 0; c < 3; ++c) { o[c] = f.u[c]; o[3 + c] = f.v[c]; o[6 + c] = f.w[c]; }
   }
   __syncthreads();
   int g = blockIdx.x * blockDim.x + threadIdx.x;
@@ -193,13 +276,12 @@ __global__ void __launch_bounds__(DT_THREADS) vis_depth_test_kernel(int ng, int 
   const float Rm1 = (float)(R - 1);
   float4 x = g_posed[g], n = g_nposed[g];
   const float dx = x.x - W.cx, dy = x.y - W.cy, dz = x.z - W.cz;
-  const int words = (K + 31) >> 5;
-  for (int wd = 0; wd < words; ++wd) {
+  for (int wd = wd0; wd < wd1; ++wd) {
     unsigned bits = 0;
     int kend = min(32, K - wd * 32);
     for (int b = 0; b < kend; ++b) {
       int k = wd * 32 + b;
-      const float* f = sF + 9 * k;
+      const float* f = sF + 9 * (k - k0);
       float pu = (f[0] * dx + f[1] * dy) + f[2] * dz;
       float pv = (f[3] * dx + f[4] * dy) + f[5] * dz;
       float pw = (f[6] * dx + f[7] * dy) + f[8] * dz;
@@ -229,10 +311,16 @@ __global__ void __launch_bounds__(DT_THREADS) vis_depth_test_kernel(int ng, int 
 }
 
 cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {
-  int grid = (av->n_gauss + DT_THREADS - 1) / DT_THREADS;
-  vis_depth_test_kernel<<<grid, DT_THREADS, (size_t)p->n_dirs * 9 * sizeof(float), s>>>(
+  // directions are split over blockIdx.y so that small avatars still fill the machine (100k Gaussians alone give
+  // 676 threads per SM); neighbouring threads stay neighbouring Gaussians, whose texel gathers coalesce in L1
+  int words = (p->n_dirs + 31) / 32;
+  int parts = words < 4 ? words : 4;
+  int wpp = (words + parts - 1) / parts;
+  parts = (words + wpp - 1) / wpp;
+  dim3 grid((av->n_gauss + DT_THREADS - 1) / DT_THREADS, parts);
+  vis_depth_test_kernel<<<grid, DT_THREADS, (size_t)wpp * 32 * 9 * sizeof(float), s>>>(
       av->n_gauss, p->n_dirs, p->res, av->g_posed, av->g_nposed, p->dirs, av->window, av->zmap, p->depth_bias_texels,
-      p->depth_bias_world, p->slope_max, av->visbits);
+      p->depth_bias_world, p->slope_max, wpp, av->visbits);
   av->launches += 1;
   rga_prof_mark(av, "vis_depth_test", s);
   return cudaGetLastError();
@@ -317,8 +405,8 @@ cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaSt
 }
 
 int rga_vis_init_attributes() {
-  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
+  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_depth_test_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   return (int)e;
 }
