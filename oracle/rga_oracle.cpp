@@ -4,8 +4,8 @@
 //
 // Precision: every quantity that decides an integer output (KNN order, tile
 // rects, sort keys, depth maps, visibility bits) is computed in fp32 with the operation order written here and NO
-// fused multiply-add (build with -ffp-contract=off); only + - * / sqrt, which IEEE-754 rounds identically on
-// every machine.  Everything compared under a tolerance (shading, compositing) is computed in double.
+// IMPLICIT fused multiply-add (build with -ffp-contract=off); only + - * / sqrt and, where written, an explicit
+// std::fma -- all of which IEEE-754 rounds identically on every machine.  Everything compared under a tolerance (shading, compositing) is computed in double.
 //
 // Pins (tests/test_oracle_pins.py): see DESIGN.md "Oracle pins".  "parity unpinned" for: gamma exponent (A9),
 // shadow-map bias constants (A17), 3DGS rasteriser constants (A18) -- PAPER.md prints no value for them.
@@ -154,16 +154,21 @@ ORC void orc_light_frames(const float* dirs, int K, float* uvw) {
 }
 
 // Light-space projection of one point (reading A13): continuous pixel coords (px,py) and normalised depth z
-// (0 = nearest the light).  Per-pose constants sR = (R/2)/r, hR = R/2, inv2r = 1/(2r) are formed once, so the per-point
-// work is multiply-add only:  px = (u.d) sR + hR,  py = (v.d) sR + hR,  z = (r - w.d) inv2r,  d = p - c.
+// (0 = nearest the light).  Per direction the frame is pre-scaled once, u_s = u sR, v_s = v sR, w_n = -w inv2r with
+// sR = (R/2)/r, hR = R/2, inv2r = 1/(2r); per point the work is three fused multiply-add chains on d = p - c:
+//   px = fma(u_s.z, d.z, fma(u_s.y, d.y, fma(u_s.x, d.x, hR)))      = (u.d) sR + R/2
+//   py = likewise with v_s
+//   z  = fma(w_n.z, d.z, fma(w_n.y, d.y, fma(w_n.x, d.x, 0.5)))     = (r - w.d) / (2r)
+// std::fma is the correctly rounded fused operation on every IEEE-754 machine, so this stays bit-reproducible.
 static inline void light_project(const float* p, const float* c, float r, const float* u, const float* v, const float* w,
                                  int R, float* px, float* py, float* z) {
   float hR = 0.5f * (float)R, sR = hR / r, inv2r = 1.0f / (2.0f * r);
+  float us[3] = {u[0] * sR, u[1] * sR, u[2] * sR}, vs[3] = {v[0] * sR, v[1] * sR, v[2] * sR};
+  float wn[3] = {-(w[0] * inv2r), -(w[1] * inv2r), -(w[2] * inv2r)};
   float d[3] = {p[0] - c[0], p[1] - c[1], p[2] - c[2]};
-  float pu = dot3(u, d), pv = dot3(v, d), pw = dot3(w, d);
-  *px = pu * sR + hR;
-  *py = pv * sR + hR;
-  *z = (r - pw) * inv2r;
+  *px = std::fma(us[2], d[2], std::fma(us[1], d[1], std::fma(us[0], d[0], hR)));
+  *py = std::fma(vs[2], d[2], std::fma(vs[1], d[1], std::fma(vs[0], d[0], hR)));
+  *z = std::fma(wn[2], d[2], std::fma(wn[1], d[1], std::fma(wn[0], d[0], 0.5f)));
 }
 
 // ---------------------------------------------------------------------------------------------------------------

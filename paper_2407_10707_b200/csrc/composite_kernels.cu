@@ -61,7 +61,7 @@ __global__ void __launch_bounds__(CB) composite_kernel(int W, int H, int TX, uns
   const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;        // DESIGN.md A21: sample at the pixel centre
   bool done = !inside;
   float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
-  unsigned contributor = 0, last = 0;
+  unsigned last = 0;
   for (int b = 0; b < n; b += CB) {
     if (__syncthreads_count(done) == CB) break;
     const int m = min(CB, n - b);
@@ -70,20 +70,31 @@ __global__ void __launch_bounds__(CB) composite_kernel(int W, int H, int TX, uns
       s_mu[threadIdx.x] = mu2d[g]; s_co[threadIdx.x] = conic_o[g]; s_col[threadIdx.x] = color[g];
     }
     __syncthreads();
-    for (int j = 0; !done && j < m; ++j) {
-      ++contributor;
-      float2 mm = s_mu[j]; float4 co = s_co[j];
-      float dx = mm.x - fx, dy = mm.y - fy;
-      float power = -0.5f * (co.x * dx * dx + co.z * dy * dy) - co.y * dx * dy;
-      if (power > 0.f) continue;
-      float alpha = fminf(0.99f, co.w * __expf(power));
-      if (alpha < 1.f / 255.f) continue;
-      float test_T = T * (1.f - alpha);
-      if (test_T < 1e-4f) { done = true; continue; }
-      float4 c = s_col[j];
-      float w = alpha * T;
-      C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
-      T = test_T; last = contributor;
+    // four entries per trip: their alphas are independent (ILP for the exp chain); only the blend is sequential
+    for (int j = 0; j < m && !done; j += 4) {
+      float a[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const float2 mm = s_mu[j + u]; const float4 co = s_co[j + u];
+        const float dx = mm.x - fx, dy = mm.y - fy;
+        const float power = -0.5f * (co.x * dx * dx + co.z * dy * dy) - co.y * dx * dy;
+        const float al = fminf(0.99f, co.w * __expf(power));
+        a[u] = (power > 0.f || j + u >= m) ? 0.f : al;
+      }
+      if (fmaxf(fmaxf(a[0], a[1]), fmaxf(a[2], a[3])) < 1.f / 255.f) continue;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (!done && a[u] >= 1.f / 255.f) {
+          const float test_T = T * (1.f - a[u]);
+          if (test_T < 1e-4f) done = true;
+          else {
+            const float4 c = s_col[j + u];
+            const float w = a[u] * T;
+            C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+            T = test_T; last = (unsigned)(b + j + u + 1);
+          }
+        }
+      }
     }
   }
   if (inside) {
