@@ -76,7 +76,7 @@ typedef struct {
   const float*   gauss_opacity;/* dev [n_gauss] or NULL = 1 ("always set the opacity ... to 1") */
   int32_t max_width, max_height;   /* largest camera this avatar will be rendered with                 */
   int32_t max_vis_dirs;            /* largest K_vis (multiple of 32 not required)                      */
-  int32_t max_vis_res;             /* largest depth-map side R_v, <= 1024                               */
+  int32_t max_vis_res;             /* largest depth-map side R_v, <= 256 (snapped raster coordinates are 16-bit) */
   int32_t max_env_texels;          /* largest rows*cols of an environment map                           */
   int64_t max_duplicates;          /* capacity of the (tile,depth) key buffers; 0 = library picks       */
 } rga_avatar_desc;

@@ -54,7 +54,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
+  void* ptrs[] = {av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
                   av->radiance, av->color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->cursor, av->keys[0],
@@ -74,8 +74,14 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   if (d->k_v < 1 || d->k_v > 31 || !(d->k_v & 1)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: k_v must be odd, 1..31");
   if (!d->vert_pos || !d->faces || !d->vert_normal || !d->vert_skin_w || !d->vert_albedo || !d->vert_rough || !d->vert_spec ||
       !d->gauss_pos || !d->gauss_quat || !d->gauss_scale) return fail(RGA_ERR_INVALID_ARG, "avatar_load: missing table");
-  if (d->max_width < 1 || d->max_height < 1 || d->max_vis_dirs < 1 || d->max_vis_res < 1 || d->max_vis_res > 1024 ||
+  if (d->max_width < 1 || d->max_height < 1 || d->max_vis_dirs < 1 || d->max_vis_res < 1 || d->max_vis_res > 256 ||
       d->max_env_texels < 1 || d->max_env_texels > 65535) return fail(RGA_ERR_INVALID_ARG, "avatar_load: bad maxima");
+  if (d->n_verts >= (1 << 21)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: n_verts must be below 2^21 (packed faces)");
+  {
+    int rows = 0, zs = 0;
+    rga_vis_raster_smem(d->max_vis_res, 1, d->n_verts, &rows, &zs);
+    if (rows < 1) return fail(RGA_ERR_INVALID_ARG, "avatar_load: mesh too large for the shared-memory vertex table of the rasteriser");
+  }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(RGA_ERR_CUDA, "avatar_load: no CUDA device (there is no CPU fallback)");
   cudaStream_t s = (cudaStream_t)stream;
@@ -98,7 +104,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   float* d2 = nullptr;
 #define A(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, \
     "avatar_load: %s: %s", #call, cudaGetErrorString(e_)); goto done; } } while (0)
-  A(dalloc(&av->v_xbar, nv)); A(dalloc(&av->v_normal, nv)); A(dalloc(&av->v_skin_w, nv * B)); A(dalloc(&av->faces, 3 * (size_t)av->n_faces));
+  A(dalloc(&av->v_xbar, nv)); A(dalloc(&av->v_normal, nv)); A(dalloc(&av->v_skin_w, nv * B)); A(dalloc(&av->faces, 3 * (size_t)av->n_faces)); A(dalloc(&av->faces_packed, (size_t)av->n_faces));
   A(dalloc(&av->knn_v, nv * av->k_v)); A(dalloc(&av->knn_g, ng * av->k_g)); A(dalloc(&av->ubar_g, ng * av->k_g));
   A(dalloc(&av->g_static, 4 * ng)); A(dalloc(&av->g_skin_w, ng * B)); A(dalloc(&av->g_quat, ng)); A(dalloc(&av->g_scale_op, ng));
   A(dalloc(&av->v_posed, nv)); A(dalloc(&av->v_nposed, nv)); A(dalloc(&av->g_posed, ng)); A(dalloc(&av->g_nposed, ng));
@@ -121,13 +127,14 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   }
   A(cudaMemcpyAsync(av->v_skin_w, d->vert_skin_w, nv * B * sizeof(float), cudaMemcpyDeviceToDevice, s));
   A(cudaMemcpyAsync(av->faces, d->faces, 3 * (size_t)av->n_faces * sizeof(int), cudaMemcpyDeviceToDevice, s));
+  A(rga_launch_pack_faces(av, s));
   A(rga_launch_load_verts(av, d->vert_pos, d->vert_disp, d->vert_normal, s));
   // KNN: S_v = K_v nearest vertices of each vertex (self included), S_g = K_g nearest of each Gaussian
   A(dalloc(&d2, (ng * av->k_g > nv * av->k_v ? ng * av->k_g : nv * av->k_v)));
   A(rga_launch_knn(d->vert_pos, av->n_verts, d->vert_pos, av->n_verts, av->k_v, av->knn_v, d2, s));
   A(rga_launch_knn(d->gauss_pos, av->n_gauss, d->vert_pos, av->n_verts, av->k_g, av->knn_g, d2, s));
   A(rga_launch_load_gauss(av, d, d2, s));
-  av->launches += 4;
+  av->launches += 5;
   if (rga_shade_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_composite_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
   A(cudaStreamSynchronize(s));
 done:

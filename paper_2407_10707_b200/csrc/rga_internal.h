@@ -19,6 +19,7 @@ struct rga_avatar {
   float4* v_normal;    // [n_verts]
   float* v_skin_w;     // [n_verts][B]
   int* faces;          // [n_faces][3]
+  unsigned long long* faces_packed;  // [n_faces] 3 x 21-bit vertex indices (one 8-byte load per triangle)
   int* knn_v;          // [n_verts][k_v]
   int* knn_g;          // [n_gauss][k_g]
   float* ubar_g;       // [n_gauss][k_g]
@@ -78,7 +79,8 @@ cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, cudaStream_t
 cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
 cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
 cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
-size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows);
+size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* z_smem);
+cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s);
 // shade_kernels.cu
 cudaError_t rga_launch_env_table(rga_avatar* av, const rga_env* env, cudaStream_t s);
 cudaError_t rga_launch_shade(rga_avatar* av, const rga_env* env, float3 cam, int vis_mode, cudaStream_t s);

@@ -43,225 +43,287 @@ __device__ __forceinline__ float light_project_z(float dx, float dy, float dz, c
 }
 
 // ------------------------------------------------------------------------------------------------------------- H3
-// One CTA per (direction, band of rows).  The band's depth map lives in shared memory: u32 depth (mode 0) or
-// u64 depth<<32|triangle (WITH_ID).  Each warp walks triangles with a block stride, one per lane.  A triangle whose
-// clipped pixel box is small is rasterised by its own lane with incremental int32 edge functions; the rare large ones
-// (slivers, close-ups) go to the warp's queue in shared memory and are rasterised by the whole warp, one lane per
-// pixel, so a long triangle never stalls the 31 other lanes (ncu on the first version: 7 of 32 lanes active).  There
-// is no block barrier inside the triangle loop.
+// Persistent CTAs (one per SM, 1,024 threads) walk the (direction, band of rows) units.  Per unit:
+//   A. every vertex is projected ONCE into shared memory: snapped (X,Y) packed in 32 bits (X,Y < 2^16 because the
+//      window contains every posed vertex and R <= 256) and, when it fits, its light-space depth z;
+//   B. each lane takes one triangle: one 8-byte packed face, three shared-memory gathers, pixel box; triangles whose
+//      box holds no pixel centre (most, at ~1 pixel per triangle) end there.  The others are compacted into the warp's
+//      queue; whenever 32 are queued their pixel samples are spread over all lanes (warp scan + head bitmask), so a
+//      sliver or a close-up triangle never idles the other lanes;
+//   C. a covered sample interpolates z and does atomicMin on the shared-memory map (u32 depth, or u64 depth<<32|tri).
+// The finished band is written to HBM once, coalesced.  ncu on the first version (one projection per triangle corner,
+// per-lane pixel loops): 693 warp instructions per 32 triangles at 17.9 active lanes (profiles/r01a_ncu_full.md).
 // Coverage and depth follow DESIGN.md "Arithmetic contract" exactly: vertices snapped to 1/256 pixel, integer edge
-// functions (inclusive, two-sided), z = (z0 + (e1/area)(z1-z0)) + (e2/area)(z2-z0) in fp32, clamped at 0.
-#define RAST_THREADS 512
-#define RAST_QW 96             // per-warp queue slots (drained when fewer than 32 remain)
-#define RAST_SMALL 12          // pixel-box size up to which a lane rasterises its own triangle
+// functions (inclusive, two-sided; int32 when the triangle spans < 64 pixels, else int64), area = e0+e1+e2 (exact
+// identity), z = (z0 + (e1/area)(z1-z0)) + (e2/area)(z2-z0) in fp32, clamped at 0.
+#define RAST_THREADS 1024
+#define RAST_WARPS (RAST_THREADS / 32)
+#define RAST_Q 64              // per-warp queue entries: < 32 left over + <= 32 pushed per batch
+#define RAST_MAX_RES 256       // snapped coordinates must fit 16 bits
 
-struct TriSetup {
-  int x0, y0, x1, y1, x2, y2;          // 1/256-pixel coordinates
-  float d0[3], d1[3], d2[3];           // vertex - window centre (depth is projected only when needed)
-  int ia, ib, ja, jb;                  // pixel box clipped to the map and the band
-  bool ok;                             // pixel box not empty
-  bool narrow;                         // unclipped box below 2^14 sub-pixels in x and y: edge functions fit int32
+__device__ __forceinline__ void face_unpack(unsigned long long f, int& i0, int& i1, int& i2) {
+  i0 = (int)(f & 0x1fffffull); i1 = (int)((f >> 21) & 0x1fffffull); i2 = (int)((f >> 42) & 0x1fffffull);
+}
+
+__global__ void pack_faces_kernel(int nf, const int* __restrict__ faces, unsigned long long* __restrict__ packed) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nf) return;
+  unsigned long long a = (unsigned)faces[3 * t], b = (unsigned)faces[3 * t + 1], c = (unsigned)faces[3 * t + 2];
+  packed[t] = a | (b << 21) | (c << 42);
+}
+
+cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s) {
+  pack_faces_kernel<<<(av->n_faces + 255) / 256, 256, 0, s>>>(av->n_faces, av->faces, av->faces_packed);
+  return cudaGetLastError();
+}
+
+struct RasterCtx {
+  int R, row0, rows;
+  const unsigned* sXY; const float* sZ;
+  const float4* v_posed; const unsigned long long* faces_packed;
+  unsigned* sz32; unsigned long long* sz64;
+  WinConst W; LightFrame F;
 };
 
-__device__ __forceinline__ TriSetup tri_setup(int t, const int* __restrict__ faces, const float4* __restrict__ v_posed,
-                                              const WinConst& W, const LightFrame& F, int R, int row0, int rows) {
-  TriSetup s;
-  int i0 = __ldg(faces + 3 * t), i1 = __ldg(faces + 3 * t + 1), i2 = __ldg(faces + 3 * t + 2);
-  float4 a = __ldg(v_posed + i0), b = __ldg(v_posed + i1), c = __ldg(v_posed + i2);
-  s.d0[0] = a.x - W.cx; s.d0[1] = a.y - W.cy; s.d0[2] = a.z - W.cz;
-  s.d1[0] = b.x - W.cx; s.d1[1] = b.y - W.cy; s.d1[2] = b.z - W.cz;
-  s.d2[0] = c.x - W.cx; s.d2[1] = c.y - W.cy; s.d2[2] = c.z - W.cz;
-  float px, py;
-  light_project_xy(s.d0[0], s.d0[1], s.d0[2], W, F, px, py);
-  s.x0 = __float2int_rn(px * 256.0f); s.y0 = __float2int_rn(py * 256.0f);
-  light_project_xy(s.d1[0], s.d1[1], s.d1[2], W, F, px, py);
-  s.x1 = __float2int_rn(px * 256.0f); s.y1 = __float2int_rn(py * 256.0f);
-  light_project_xy(s.d2[0], s.d2[1], s.d2[2], W, F, px, py);
-  s.x2 = __float2int_rn(px * 256.0f); s.y2 = __float2int_rn(py * 256.0f);
-  int mnx = min(s.x0, min(s.x1, s.x2)), mxx = max(s.x0, max(s.x1, s.x2));
-  int mny = min(s.y0, min(s.y1, s.y2)), mxy = max(s.y0, max(s.y1, s.y2));
+// pixel box of a triangle given its packed corners, clipped to the map and the band; returns the sample count
+__device__ __forceinline__ int tri_box(unsigned P0, unsigned P1, unsigned P2, const int R, const int row0, const int rows,
+                                       int& ia, int& ja, int& bw, bool& narrow) {
+  const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
+  const int mnx = min(x0, min(x1, x2)), mxx = max(x0, max(x1, x2));
+  const int mny = min(y0, min(y1, y2)), mxy = max(y0, max(y1, y2));
   // pixel i has its centre at 256 i + 128: first centre >= mn, last centre <= mx
-  s.ia = max((mnx + 127) >> 8, 0); s.ib = min((mxx - 128) >> 8, R - 1);
-  s.ja = max((mny + 127) >> 8, row0); s.jb = min((mxy - 128) >> 8, row0 + rows - 1);
-  s.narrow = (mxx - mnx) < 16384 && (mxy - mny) < 16384;
-  s.ok = s.ia <= s.ib && s.ja <= s.jb;
-  return s;
+  ia = max((mnx + 127) >> 8, 0); const int ib = min((mxx - 128) >> 8, R - 1);
+  ja = max((mny + 127) >> 8, row0); const int jb = min((mxy - 128) >> 8, row0 + rows - 1);
+  narrow = (mxx - mnx) < 16384 && (mxy - mny) < 16384;
+  bw = ib - ia + 1;
+  const int bh = jb - ja + 1;
+  return (bw > 0 && bh > 0) ? bw * bh : 0;
 }
 
-template <bool WITH_ID>
-__device__ __forceinline__ void put_sample(unsigned* sz32, unsigned long long* sz64, int p, float z, int t) {
-  z = fmaxf(z, 0.0f);
-  if (WITH_ID) atomicMin(sz64 + p, ((unsigned long long)__float_as_uint(z) << 32) | (unsigned)t);
-  else atomicMin(sz32 + p, __float_as_uint(z));
-}
-
-// whole warp, one lane per pixel of the triangle's box; int64 edge functions (any size)
-template <bool WITH_ID>
-__device__ __forceinline__ void raster_big(int tq, int lane, const int* __restrict__ faces, const float4* __restrict__ v_posed,
-    const WinConst& W, const LightFrame& F, int R, int row0, int rows, unsigned* sz32, unsigned long long* sz64) {
-  const TriSetup s = tri_setup(tq, faces, v_posed, W, F, R, row0, rows);
-  const long long x0 = s.x0, y0 = s.y0, x1 = s.x1, y1 = s.y1, x2 = s.x2, y2 = s.y2;
-  const long long area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
-  if (area == 0) return;
-  const float z0 = light_project_z(s.d0[0], s.d0[1], s.d0[2], F), z1 = light_project_z(s.d1[0], s.d1[1], s.d1[2], F),
-              z2 = light_project_z(s.d2[0], s.d2[1], s.d2[2], F);
-  const int bw = s.ib - s.ia + 1, cnt = bw * (s.jb - s.ja + 1);
-  const float fa = (float)area, d1 = z1 - z0, d2 = z2 - z0;
-  for (int q = lane; q < cnt; q += 32) {
-    const int j = s.ja + q / bw, i = s.ia + q % bw;
-    const long long qx = 256ll * i + 128, qy = 256ll * j + 128;
-    const long long e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
-    const long long e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
-    const long long e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
-    if ((e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0)) {
-      float t1 = (float)e1 / fa, t2 = (float)e2 / fa;
-      put_sample<WITH_ID>(sz32, sz64, (j - row0) * R + i, (z0 + t1 * d1) + t2 * d2, tq);
-    }
-  }
-}
-
-template <bool WITH_ID>
-__global__ void __launch_bounds__(RAST_THREADS) vis_raster_kernel(int nf, int R, int band_rows, int n_bands, int nv_words,
-    const float4* __restrict__ v_posed, const int* __restrict__ faces, const float* __restrict__ dirs,
-    const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
-    unsigned* __restrict__ vbits_raw, int words, int n_verts) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ int s_queue[RAST_THREADS / 32][RAST_QW];
-  const int k = blockIdx.x / n_bands, band = blockIdx.x % n_bands;
-  const int row0 = band * band_rows, rows = min(band_rows, R - row0);
-  const int npix = rows * R;
-  unsigned* sz32 = reinterpret_cast<unsigned*>(smem_raw);
-  unsigned long long* sz64 = reinterpret_cast<unsigned long long*>(smem_raw);
-  unsigned* svert = reinterpret_cast<unsigned*>(smem_raw + (size_t)band_rows * R * 8);     // WITH_ID only: vertex bitset
-  if (WITH_ID) {
-    for (int p = threadIdx.x; p < npix; p += blockDim.x) sz64[p] = ~0ull;
-    for (int p = threadIdx.x; p < nv_words; p += blockDim.x) svert[p] = 0u;
+template <bool WITH_ID, bool Z_SMEM>
+__device__ __forceinline__ void raster_sample(const RasterCtx& c, uint4 d, bool narrow, int i, int j) {
+  const int x0 = d.x & 0xffff, y0 = d.x >> 16, x1 = d.y & 0xffff, y1 = d.y >> 16, x2 = d.z & 0xffff, y2 = d.z >> 16;
+  const int qx = 256 * i + 128, qy = 256 * j + 128;
+  bool cov; float f1, f2, fa;
+  if (narrow) {
+    const int e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
+    const int e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
+    const int e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
+    const int area = e0 + e1 + e2;
+    cov = (min(e0, min(e1, e2)) >= 0 || max(e0, max(e1, e2)) <= 0) && area != 0;
+    f1 = (float)e1; f2 = (float)e2; fa = (float)area;
   } else {
-    for (int p = threadIdx.x; p < npix; p += blockDim.x) sz32[p] = 0xffffffffu;
+    const long long e0 = (long long)(x2 - x1) * (qy - y1) - (long long)(y2 - y1) * (qx - x1);
+    const long long e1 = (long long)(x0 - x2) * (qy - y2) - (long long)(y0 - y2) * (qx - x2);
+    const long long e2 = (long long)(x1 - x0) * (qy - y0) - (long long)(y1 - y0) * (qx - x0);
+    const long long area = e0 + e1 + e2;
+    cov = ((e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0)) && area != 0;
+    f1 = (float)e1; f2 = (float)e2; fa = (float)area;
   }
-  const WinConst W = make_win(window, R);
-  const LightFrame F = make_frame(dirs + 3 * k, W);
-  __syncthreads();
+  if (!cov) return;
+  int i0, i1, i2;
+  face_unpack(__ldg(c.faces_packed + d.w), i0, i1, i2);
+  float z0, z1, z2;
+  if (Z_SMEM) { z0 = c.sZ[i0]; z1 = c.sZ[i1]; z2 = c.sZ[i2]; }
+  else {
+    const float4 a = __ldg(c.v_posed + i0), b = __ldg(c.v_posed + i1), e = __ldg(c.v_posed + i2);
+    z0 = light_project_z(a.x - c.W.cx, a.y - c.W.cy, a.z - c.W.cz, c.F);
+    z1 = light_project_z(b.x - c.W.cx, b.y - c.W.cy, b.z - c.W.cz, c.F);
+    z2 = light_project_z(e.x - c.W.cx, e.y - c.W.cy, e.z - c.W.cz, c.F);
+  }
+  const float t1 = f1 / fa, t2 = f2 / fa;
+  float z = (z0 + t1 * (z1 - z0)) + t2 * (z2 - z0);
+  z = fmaxf(z, 0.0f);
+  const int p = (j - c.row0) * c.R + i;
+  if (WITH_ID) atomicMin(c.sz64 + p, ((unsigned long long)__float_as_uint(z) << 32) | d.w);
+  else atomicMin(c.sz32 + p, __float_as_uint(z));
+}
+
+// One round: lane l owns queue entry l (l < n); the samples of all n pixel boxes are dealt out 32 at a time.
+template <bool WITH_ID, bool Z_SMEM>
+__device__ __forceinline__ void raster_round(const RasterCtx& c, const uint4* qb, int n, int lane) {
+  uint4 d = make_uint4(0u, 0u, 0u, 0u);
+  int ia = 0, ja = 0, bw = 1, cnt = 0; bool narrow = true;
+  if (lane < n) { d = qb[lane]; cnt = tri_box(d.x, d.y, d.z, c.R, c.row0, c.rows, ia, ja, bw, narrow); }
+  const unsigned boxpack = (unsigned)ia | ((unsigned)ja << 8) | ((unsigned)(bw - 1) << 16) | (narrow ? (1u << 24) : 0u);
+  const float invbw = 1.0f / (float)bw;
+  int inc = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+  const int exc = inc - cnt;
+  const int total = __shfl_sync(0xffffffffu, inc, 31);
+  int headbase = 0;
+  for (int c0 = 0; c0 < total; c0 += 32) {
+    const unsigned bit = (cnt > 0 && exc >= c0 && exc < c0 + 32) ? (1u << (exc - c0)) : 0u;
+    const unsigned H = __reduce_or_sync(0xffffffffu, bit);
+    // entries are all non-empty, so the index among heads is the owning lane
+    const int owner = max(headbase + __popc(H & (0xffffffffu >> (31 - lane))) - 1, 0);
+    headbase += __popc(H);
+    const int oexc = __shfl_sync(0xffffffffu, exc, owner);
+    const unsigned obox = __shfl_sync(0xffffffffu, boxpack, owner);
+    const float oinv = __shfl_sync(0xffffffffu, invbw, owner);
+    const int s = c0 + lane;
+    if (s < total) {
+      const uint4 od = qb[owner];
+      const int li = s - oexc, obw = (int)((obox >> 16) & 0xffu) + 1;
+      const int row = (int)(((float)li + 0.5f) * oinv);              // li / obw: (li+0.5)/obw is >= 1/512 from an integer
+      const int col = li - row * obw;
+      raster_sample<WITH_ID, Z_SMEM>(c, od, (obox >> 24) & 1u, (int)(obox & 0xffu) + col, (int)((obox >> 8) & 0xffu) + row);
+    }
+  }
+}
+
+template <bool WITH_ID, bool Z_SMEM>
+__global__ void __launch_bounds__(RAST_THREADS, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
+    const float4* __restrict__ v_posed, const unsigned long long* __restrict__ faces_packed, const float* __restrict__ dirs,
+    const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
+    unsigned* __restrict__ vbits_raw, int words) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  // layout: [queues 32 x 64 x 16 B][map band_rows*R*(4|8)][sXY nv*4][sZ nv*4 if Z_SMEM][svert (WITH_ID)]
+  uint4* s_queue = reinterpret_cast<uint4*>(smem_raw);
+  unsigned char* mp = smem_raw + (size_t)RAST_WARPS * RAST_Q * sizeof(uint4);
+  unsigned* sz32 = reinterpret_cast<unsigned*>(mp);
+  unsigned long long* sz64 = reinterpret_cast<unsigned long long*>(mp);
+  const size_t map_bytes = (((size_t)band_rows * R * (WITH_ID ? 8 : 4)) + 15) & ~(size_t)15;
+  unsigned* sXY = reinterpret_cast<unsigned*>(mp + map_bytes);
+  float* sZ = reinterpret_cast<float*>(sXY + nv);
+  unsigned* svert = reinterpret_cast<unsigned*>(Z_SMEM ? (sZ + nv) : sZ);
+  const int nv_words = (nv + 31) >> 5;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  int* myq = s_queue[warp];
-  int qn = 0;                                             // warp-uniform
+  uint4* myq = s_queue + warp * RAST_Q;
+  const WinConst W = make_win(window, R);
 
-  for (int base = warp * 32; base < nf; base += blockDim.x) {
-    const int t = base + lane;
-    bool big = false;
-    if (t < nf) {
-      const TriSetup s = tri_setup(t, faces, v_posed, W, F, R, row0, rows);
-      if (s.ok) {
-        const int bw = s.ib - s.ia + 1, bh = s.jb - s.ja + 1;
-        if (s.narrow && bw * bh <= RAST_SMALL) {
-          // int32 edge functions, orientation normalised so that "inside" is e0,e1,e2 >= 0
-          const int area = (s.x1 - s.x0) * (s.y2 - s.y0) - (s.y1 - s.y0) * (s.x2 - s.x0);
-          if (area != 0) {
-            const int sg = area > 0 ? 1 : -1;
-            const int qx = 256 * s.ia + 128, qy = 256 * s.ja + 128;
-            int r0 = sg * ((s.x2 - s.x1) * (qy - s.y1) - (s.y2 - s.y1) * (qx - s.x1));
-            int r1 = sg * ((s.x0 - s.x2) * (qy - s.y2) - (s.y0 - s.y2) * (qx - s.x2));
-            int r2 = sg * ((s.x1 - s.x0) * (qy - s.y0) - (s.y1 - s.y0) * (qx - s.x0));
-            const int ax0 = -sg * 256 * (s.y2 - s.y1), ax1 = -sg * 256 * (s.y0 - s.y2), ax2 = -sg * 256 * (s.y1 - s.y0);
-            const int ay0 = sg * 256 * (s.x2 - s.x1), ay1 = sg * 256 * (s.x0 - s.x2), ay2 = sg * 256 * (s.x1 - s.x0);
-            float z0 = 0.f, d1 = 0.f, d2 = 0.f;
-            const float fa = (float)(sg * area);
-            bool have_z = false;
-            for (int j = s.ja; j <= s.jb; ++j) {
-              int e0 = r0, e1 = r1, e2 = r2;
-              for (int i = s.ia; i <= s.ib; ++i) {
-                if ((e0 | e1 | e2) >= 0) {
-                  if (!have_z) {                                      // most sub-pixel triangles never get here
-                    z0 = light_project_z(s.d0[0], s.d0[1], s.d0[2], F);
-                    d1 = light_project_z(s.d1[0], s.d1[1], s.d1[2], F) - z0;
-                    d2 = light_project_z(s.d2[0], s.d2[1], s.d2[2], F) - z0;
-                    have_z = true;
-                  }
-                  float t1 = (float)e1 / fa, t2 = (float)e2 / fa;
-                  put_sample<WITH_ID>(sz32, sz64, (j - row0) * R + i, (z0 + t1 * d1) + t2 * d2, t);
-                }
-                e0 += ax0; e1 += ax1; e2 += ax2;
-              }
-              r0 += ay0; r1 += ay1; r2 += ay2;
-            }
-          }
-        } else big = true;
-      }
+  for (int unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+    const int k = unit / n_bands, band = unit - k * n_bands;
+    const int row0 = band * band_rows, rows = min(band_rows, R - row0);
+    const int npix = rows * R;
+    const LightFrame F = make_frame(dirs + 3 * k, W);
+    // clear the band
+    if (WITH_ID) { for (int p = threadIdx.x; p < npix; p += RAST_THREADS) sz64[p] = ~0ull; }
+    else {
+      uint4* m4 = reinterpret_cast<uint4*>(sz32);
+      const uint4 ones = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
+      for (int p = threadIdx.x; p < (npix + 3) >> 2; p += RAST_THREADS) m4[p] = ones;
     }
-    const unsigned bm = __ballot_sync(0xffffffffu, big);
-    if (bm) {
-      if (big) myq[qn + __popc(bm & ((1u << lane) - 1u))] = t;
-      qn += __popc(bm);
-      __syncwarp();
-      if (qn > RAST_QW - 32) {
-        for (int e = 0; e < qn; ++e) raster_big<WITH_ID>(myq[e], lane, faces, v_posed, W, F, R, row0, rows, sz32, sz64);
-        qn = 0;
+    if (WITH_ID && vbits_raw) for (int p = threadIdx.x; p < nv_words; p += RAST_THREADS) svert[p] = 0u;
+    // A. project every vertex once
+    for (int v = threadIdx.x; v < nv; v += RAST_THREADS) {
+      const float4 a = __ldg(v_posed + v);
+      const float dx = a.x - W.cx, dy = a.y - W.cy, dz = a.z - W.cz;
+      float px, py;
+      light_project_xy(dx, dy, dz, W, F, px, py);
+      const int X = min(max(__float2int_rn(px * 256.0f), 0), 65535), Y = min(max(__float2int_rn(py * 256.0f), 0), 65535);
+      sXY[v] = (unsigned)X | ((unsigned)Y << 16);
+      if (Z_SMEM) sZ[v] = light_project_z(dx, dy, dz, F);
+    }
+    __syncthreads();
+
+    RasterCtx c;
+    c.R = R; c.row0 = row0; c.rows = rows; c.sXY = sXY; c.sZ = sZ; c.v_posed = v_posed; c.faces_packed = faces_packed;
+    c.sz32 = sz32; c.sz64 = sz64; c.W = W; c.F = F;
+    // B. triangles: one per lane, non-empty boxes queued
+    int qn = 0;                                             // warp-uniform
+    for (int base = warp * 32; base < nf; base += RAST_THREADS) {
+      const int t = base + lane;
+      bool ne = false;
+      uint4 d = make_uint4(0u, 0u, 0u, (unsigned)t);
+      if (t < nf) {
+        int i0, i1, i2;
+        face_unpack(__ldg(faces_packed + t), i0, i1, i2);
+        d.x = sXY[i0]; d.y = sXY[i1]; d.z = sXY[i2];
+        int ia, ja, bw; bool narrow;
+        ne = tri_box(d.x, d.y, d.z, R, row0, rows, ia, ja, bw, narrow) > 0;
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, ne);
+      if (m) {
+        if (ne) myq[qn + __popc(m & ((1u << lane) - 1u))] = d;
+        qn += __popc(m);
         __syncwarp();
-      }
-    }
-  }
-  for (int e = 0; e < qn; ++e) raster_big<WITH_ID>(myq[e], lane, faces, v_posed, W, F, R, row0, rows, sz32, sz64);
-  __syncthreads();
-
-  size_t gbase = ((size_t)k * R + row0) * R;
-  if (WITH_ID) {
-    for (int p = threadIdx.x; p < npix; p += blockDim.x) {
-      unsigned long long key = sz64[p];
-      zmap[gbase + p] = (unsigned)(key >> 32);
-      int tri = (key == ~0ull) ? -1 : (int)(unsigned)(key & 0xffffffffu);
-      idmap[gbase + p] = tri;
-      if (vbits_raw && tri >= 0) {                      // a triangle that appears marks its 3 vertices
-        int v0 = __ldg(faces + 3 * tri), v1 = __ldg(faces + 3 * tri + 1), v2 = __ldg(faces + 3 * tri + 2);
-        atomicOr(svert + (v0 >> 5), 1u << (v0 & 31));
-        atomicOr(svert + (v1 >> 5), 1u << (v1 & 31));
-        atomicOr(svert + (v2 >> 5), 1u << (v2 & 31));
-      }
-    }
-    if (vbits_raw) {
-      __syncthreads();
-      const unsigned bit = 1u << (k & 31);
-      for (int wd = threadIdx.x; wd < nv_words; wd += blockDim.x) {
-        unsigned m = svert[wd];
-        while (m) {
-          int b = __ffs(m) - 1; m &= m - 1;
-          int vtx = wd * 32 + b;
-          if (vtx < n_verts) atomicOr(vbits_raw + (size_t)vtx * words + (k >> 5), bit);
+        if (qn >= 32) {
+          qn -= 32;
+          raster_round<WITH_ID, Z_SMEM>(c, myq + qn, 32, lane);
+          __syncwarp();
         }
       }
     }
-  } else {
-    for (int p = threadIdx.x; p < npix; p += blockDim.x) zmap[gbase + p] = sz32[p];
+    if (qn) raster_round<WITH_ID, Z_SMEM>(c, myq, qn, lane);
+    __syncthreads();
+
+    // write the band out
+    const size_t gbase = ((size_t)k * R + row0) * R;
+    if (WITH_ID) {
+      for (int p = threadIdx.x; p < npix; p += RAST_THREADS) {
+        const unsigned long long key = sz64[p];
+        zmap[gbase + p] = (unsigned)(key >> 32);
+        const int tri = (key == ~0ull) ? -1 : (int)(unsigned)(key & 0xffffffffu);
+        idmap[gbase + p] = tri;
+        if (vbits_raw && tri >= 0) {                      // a triangle that appears marks its 3 vertices
+          int v0, v1, v2;
+          face_unpack(__ldg(faces_packed + tri), v0, v1, v2);
+          atomicOr(svert + (v0 >> 5), 1u << (v0 & 31));
+          atomicOr(svert + (v1 >> 5), 1u << (v1 & 31));
+          atomicOr(svert + (v2 >> 5), 1u << (v2 & 31));
+        }
+      }
+      if (vbits_raw) {
+        __syncthreads();
+        const unsigned bit = 1u << (k & 31);
+        for (int wd = threadIdx.x; wd < nv_words; wd += RAST_THREADS) {
+          unsigned m = svert[wd];
+          while (m) {
+            const int b = __ffs(m) - 1; m &= m - 1;
+            const int vtx = wd * 32 + b;
+            if (vtx < nv) atomicOr(vbits_raw + (size_t)vtx * words + (k >> 5), bit);
+          }
+        }
+      }
+    } else if ((R & 3) == 0) {
+      const uint4* m4 = reinterpret_cast<const uint4*>(sz32);
+      uint4* g4 = reinterpret_cast<uint4*>(zmap + gbase);
+      for (int p = threadIdx.x; p < npix >> 2; p += RAST_THREADS) g4[p] = m4[p];
+    } else {
+      for (int p = threadIdx.x; p < npix; p += RAST_THREADS) zmap[gbase + p] = sz32[p];
+    }
+    __syncthreads();                                      // the map and the vertex tables are reused by the next unit
   }
 }
 
-size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows) {
-  const size_t budget = 200 * 1024;
-  size_t per_row = (size_t)res * (with_id ? 8 : 4);
-  size_t extra = with_id ? (size_t)((n_verts + 31) / 32) * 4 : 0;
-  int rows = (int)((budget - extra) / per_row);
+// shared-memory plan: returns bytes, band rows and whether per-vertex z fits
+size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* z_smem) {
+  const size_t budget = 227 * 1024;
+  const size_t fixed = (size_t)RAST_WARPS * RAST_Q * 16 + (size_t)n_verts * 4 + (with_id ? (size_t)((n_verts + 31) / 32) * 4 : 0) + 32;
+  const size_t per_row = (size_t)res * (with_id ? 8 : 4);
+  const size_t zbytes = (size_t)n_verts * 4;
+  *z_smem = (fixed + zbytes + per_row * res <= budget) ? 1 : 0;      // z only when the whole map still fits in one band
+  size_t avail = budget > fixed + (*z_smem ? zbytes : 0) ? budget - fixed - (*z_smem ? zbytes : 0) : 0;
+  int rows = (int)(avail / per_row);
   if (rows > res) rows = res;
-  if (rows < 1) rows = 1;
+  if (rows < 1) { *band_rows = 0; return 0; }                         // mesh too large for the shared-memory vertex table
   int bands = (res + rows - 1) / rows;
-  rows = (res + bands - 1) / bands;                       // even bands
+  rows = (res + bands - 1) / bands;                                   // even bands
   *band_rows = rows;
-  return per_row * rows + extra;
+  return fixed + (*z_smem ? zbytes : 0) + ((per_row * rows + 15) & ~(size_t)15);
 }
 
 cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {
   const bool with_id = p->mode == 1 || p->keep_maps;
-  int band_rows = 0;
-  size_t smem = rga_vis_raster_smem(p->res, with_id, av->n_verts, &band_rows);
-  int n_bands = (p->res + band_rows - 1) / band_rows;
-  int words = (p->n_dirs + 31) / 32, nv_words = (av->n_verts + 31) / 32;
-  dim3 grid(p->n_dirs * n_bands);
+  int band_rows = 0, z_smem = 0;
+  const size_t smem = rga_vis_raster_smem(p->res, with_id, av->n_verts, &band_rows, &z_smem);
+  if (band_rows < 1) return cudaErrorInvalidConfiguration;
+  const int n_bands = (p->res + band_rows - 1) / band_rows;
+  const int words = (p->n_dirs + 31) / 32;
+  const int n_units = p->n_dirs * n_bands;
+  const int grid = n_units < av->num_sms ? n_units : av->num_sms;
+  unsigned* raw = (with_id && p->mode == 1) ? av->vbits_raw : nullptr;
+  if (raw) cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s);
+#define RAST_ARGS av->n_faces, av->n_verts, p->res, band_rows, n_bands, n_units, av->v_posed, av->faces_packed, p->dirs, av->window, \
+    av->zmap, av->idmap, raw, words
   if (with_id) {
-    unsigned* raw = (p->mode == 1) ? av->vbits_raw : nullptr;
-    if (raw) cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s);
-    vis_raster_kernel<true><<<grid, RAST_THREADS, smem, s>>>(av->n_faces, p->res, band_rows, n_bands, nv_words, av->v_posed, av->faces,
-                                                   p->dirs, av->window, av->zmap, av->idmap, raw, words, av->n_verts);
+    if (z_smem) vis_raster_kernel<true, true><<<grid, RAST_THREADS, smem, s>>>(RAST_ARGS);
+    else vis_raster_kernel<true, false><<<grid, RAST_THREADS, smem, s>>>(RAST_ARGS);
   } else {
-    vis_raster_kernel<false><<<grid, RAST_THREADS, smem, s>>>(av->n_faces, p->res, band_rows, n_bands, nv_words, av->v_posed, av->faces,
-                                                    p->dirs, av->window, av->zmap, av->idmap, nullptr, words, av->n_verts);
+    if (z_smem) vis_raster_kernel<false, true><<<grid, RAST_THREADS, smem, s>>>(RAST_ARGS);
+    else vis_raster_kernel<false, false><<<grid, RAST_THREADS, smem, s>>>(RAST_ARGS);
   }
   av->launches += 1;
   rga_prof_mark(av, "vis_raster", s);
@@ -432,8 +494,11 @@ cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaSt
 }
 
 int rga_vis_init_attributes() {
-  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
+  const int mx = 227 * 1024;
+  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_depth_test_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   return (int)e;
 }
