@@ -78,8 +78,8 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
       d->max_env_texels < 1 || d->max_env_texels > 65535) return fail(RGA_ERR_INVALID_ARG, "avatar_load: bad maxima");
   if (d->n_verts >= (1 << 21)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: n_verts must be below 2^21 (packed faces)");
   {
-    int rows = 0, zs = 0;
-    rga_vis_raster_smem(d->max_vis_res, 1, d->n_verts, &rows, &zs);
+    int rows = 0, th = 0;
+    rga_vis_raster_smem(d->max_vis_res, 1, d->n_verts, &rows, &th);
     if (rows < 1) return fail(RGA_ERR_INVALID_ARG, "avatar_load: mesh too large for the shared-memory vertex table of the rasteriser");
   }
   int ndev = 0;

@@ -79,7 +79,7 @@ cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, cudaStream_t
 cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
 cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
 cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
-size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* z_smem);
+size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads);
 cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s);
 // shade_kernels.cu
 cudaError_t rga_launch_env_table(rga_avatar* av, const rga_env* env, cudaStream_t s);

@@ -43,22 +43,22 @@ __device__ __forceinline__ float light_project_z(float dx, float dy, float dz, c
 }
 
 // ------------------------------------------------------------------------------------------------------------- H3
-// Persistent CTAs (one per SM, 1,024 threads) walk the (direction, band of rows) units.  Per unit:
-//   A. every vertex is projected ONCE into shared memory: snapped (X,Y) packed in 32 bits (X,Y < 2^16 because the
-//      window contains every posed vertex and R <= 256) and, when it fits, its light-space depth z;
-//   B. each lane takes one triangle: one 8-byte packed face, three shared-memory gathers, pixel box; triangles whose
-//      box holds no pixel centre (most, at ~1 pixel per triangle) end there.  The others are compacted into the warp's
-//      queue; whenever 32 are queued their pixel samples are spread over all lanes (warp scan + head bitmask), so a
-//      sliver or a close-up triangle never idles the other lanes;
-//   C. a covered sample interpolates z and does atomicMin on the shared-memory map (u32 depth, or u64 depth<<32|tri).
+// Persistent CTAs (one per SM) walk the (direction, band of rows) units.  Per unit:
+//   A.  every vertex is projected ONCE into shared memory: snapped (X,Y) packed in 32 bits (X,Y < 2^16 because the
+//       window contains every posed vertex and R <= 256);
+//   B1. warps fetch 32 triangles at a time (dynamic counter), one per lane: one 8-byte packed face, three shared-memory
+//       gathers, pixel box; triangles whose box holds no pixel centre (53 % at config 1) end there, the others are
+//       compacted into the warp's queue;
+//   B2. whenever 32 are queued, each lane writes its triangle's edge-function coefficients to the warp's table and the
+//       pixel samples of all 32 boxes are dealt out over all lanes (warp scan + head bitmask), so a sliver never idles
+//       the other lanes; a sample costs three 2-IMAD edge functions; covered samples (13 %) are compacted again;
+//   C.  whenever 32 covered samples are queued their depth is interpolated (vertex z projected on demand) and
+//       atomicMin'ed into the shared-memory map (u32 depth, or u64 depth<<32|tri).
 // The finished band is written to HBM once, coalesced.  ncu on the first version (one projection per triangle corner,
 // per-lane pixel loops): 693 warp instructions per 32 triangles at 17.9 active lanes (profiles/r01a_ncu_full.md).
 // Coverage and depth follow DESIGN.md "Arithmetic contract" exactly: vertices snapped to 1/256 pixel, integer edge
 // functions (inclusive, two-sided; int32 when the triangle spans < 64 pixels, else int64), area = e0+e1+e2 (exact
 // identity), z = (z0 + (e1/area)(z1-z0)) + (e2/area)(z2-z0) in fp32, clamped at 0.
-#define RAST_THREADS 1024
-#define RAST_WARPS (RAST_THREADS / 32)
-#define RAST_Q 64              // per-warp queue entries: < 32 left over + <= 32 pushed per batch
 #define RAST_MAX_RES 256       // snapped coordinates must fit 16 bits
 
 __device__ __forceinline__ void face_unpack(unsigned long long f, int& i0, int& i1, int& i2) {
@@ -77,9 +77,18 @@ cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s) {
   return cudaGetLastError();
 }
 
+// Per-warp working set in shared memory (RAST_WARP_BYTES each)
+#define RAST_Q 64              // queue entries: < 32 left over + <= 32 pushed
+struct RasterWarp {
+  uint4 tab[32][4];            // round table: edge-function coefficients and box of the 32 triangles being sampled
+  uint4 q2[RAST_Q];            // covered samples waiting for depth: {triangle, pixel, float(e1), float(e2)}
+  float q2a[RAST_Q];           //   and float(area)
+  int q1[RAST_Q];              // triangles whose pixel box is not empty
+};
+
 struct RasterCtx {
   int R, row0, rows;
-  const unsigned* sXY; const float* sZ;
+  const unsigned* sXY;
   const float4* v_posed; const unsigned long long* faces_packed;
   unsigned* sz32; unsigned long long* sz64;
   WinConst W; LightFrame F;
@@ -100,97 +109,136 @@ __device__ __forceinline__ int tri_box(unsigned P0, unsigned P1, unsigned P2, co
   return (bw > 0 && bh > 0) ? bw * bh : 0;
 }
 
-template <bool WITH_ID, bool Z_SMEM>
-__device__ __forceinline__ void raster_sample(const RasterCtx& c, uint4 d, bool narrow, int i, int j) {
-  const int x0 = d.x & 0xffff, y0 = d.x >> 16, x1 = d.y & 0xffff, y1 = d.y >> 16, x2 = d.z & 0xffff, y2 = d.z >> 16;
-  const int qx = 256 * i + 128, qy = 256 * j + 128;
-  bool cov; float f1, f2, fa;
-  if (narrow) {
-    const int e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
-    const int e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
-    const int e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
-    const int area = e0 + e1 + e2;
-    cov = (min(e0, min(e1, e2)) >= 0 || max(e0, max(e1, e2)) <= 0) && area != 0;
-    f1 = (float)e1; f2 = (float)e2; fa = (float)area;
-  } else {
-    const long long e0 = (long long)(x2 - x1) * (qy - y1) - (long long)(y2 - y1) * (qx - x1);
-    const long long e1 = (long long)(x0 - x2) * (qy - y2) - (long long)(y0 - y2) * (qx - x2);
-    const long long e2 = (long long)(x1 - x0) * (qy - y0) - (long long)(y1 - y0) * (qx - x0);
-    const long long area = e0 + e1 + e2;
-    cov = ((e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0)) && area != 0;
-    f1 = (float)e1; f2 = (float)e2; fa = (float)area;
-  }
-  if (!cov) return;
+// C. depth of up to 32 covered samples (one per lane) and the atomicMin on the map
+template <bool WITH_ID>
+__device__ __forceinline__ void raster_depth(const RasterCtx& c, const RasterWarp* w, int base, int n, int lane) {
+  if (lane >= n) return;
+  const uint4 q = w->q2[base + lane];
+  const float fa = w->q2a[base + lane];
   int i0, i1, i2;
-  face_unpack(__ldg(c.faces_packed + d.w), i0, i1, i2);
-  float z0, z1, z2;
-  if (Z_SMEM) { z0 = c.sZ[i0]; z1 = c.sZ[i1]; z2 = c.sZ[i2]; }
-  else {
-    const float4 a = __ldg(c.v_posed + i0), b = __ldg(c.v_posed + i1), e = __ldg(c.v_posed + i2);
-    z0 = light_project_z(a.x - c.W.cx, a.y - c.W.cy, a.z - c.W.cz, c.F);
-    z1 = light_project_z(b.x - c.W.cx, b.y - c.W.cy, b.z - c.W.cz, c.F);
-    z2 = light_project_z(e.x - c.W.cx, e.y - c.W.cy, e.z - c.W.cz, c.F);
-  }
-  const float t1 = f1 / fa, t2 = f2 / fa;
+  face_unpack(__ldg(c.faces_packed + q.x), i0, i1, i2);
+  const float4 a = __ldg(c.v_posed + i0), b = __ldg(c.v_posed + i1), e = __ldg(c.v_posed + i2);
+  const float z0 = light_project_z(a.x - c.W.cx, a.y - c.W.cy, a.z - c.W.cz, c.F);
+  const float z1 = light_project_z(b.x - c.W.cx, b.y - c.W.cy, b.z - c.W.cz, c.F);
+  const float z2 = light_project_z(e.x - c.W.cx, e.y - c.W.cy, e.z - c.W.cz, c.F);
+  const float t1 = __uint_as_float(q.z) / fa, t2 = __uint_as_float(q.w) / fa;
   float z = (z0 + t1 * (z1 - z0)) + t2 * (z2 - z0);
   z = fmaxf(z, 0.0f);
-  const int p = (j - c.row0) * c.R + i;
-  if (WITH_ID) atomicMin(c.sz64 + p, ((unsigned long long)__float_as_uint(z) << 32) | d.w);
-  else atomicMin(c.sz32 + p, __float_as_uint(z));
+  if (WITH_ID) atomicMin(c.sz64 + q.y, ((unsigned long long)__float_as_uint(z) << 32) | q.x);
+  else atomicMin(c.sz32 + q.y, __float_as_uint(z));
 }
 
-// One round: lane l owns queue entry l (l < n); the samples of all n pixel boxes are dealt out 32 at a time.
-template <bool WITH_ID, bool Z_SMEM>
-__device__ __forceinline__ void raster_round(const RasterCtx& c, const uint4* qb, int n, int lane) {
-  uint4 d = make_uint4(0u, 0u, 0u, 0u);
-  int ia = 0, ja = 0, bw = 1, cnt = 0; bool narrow = true;
-  if (lane < n) { d = qb[lane]; cnt = tri_box(d.x, d.y, d.z, c.R, c.row0, c.rows, ia, ja, bw, narrow); }
-  const unsigned boxpack = (unsigned)ia | ((unsigned)ja << 8) | ((unsigned)(bw - 1) << 16) | (narrow ? (1u << 24) : 0u);
-  const float invbw = 1.0f / (float)bw;
+// B2. one round: lane l owns queued triangle l (l < n); the samples of all n pixel boxes are dealt out 32 at a time.
+// Returns the new fill of the covered-sample queue.
+template <bool WITH_ID>
+__device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, int qbase, int n, int lane, int q2n) {
+  int cnt = 0;
+  uint4 r0 = make_uint4(0u, 0u, 0u, 0u), r1 = r0, r3 = r0;
+  unsigned boxw = 0u, ay2u = 0u; float invbw = 1.0f;
+  if (lane < n) {
+    const int t = w->q1[qbase + lane];
+    int i0, i1, i2;
+    face_unpack(__ldg(c.faces_packed + t), i0, i1, i2);
+    const unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
+    int ia, ja, bw; bool narrow;
+    cnt = tri_box(P0, P1, P2, c.R, c.row0, c.rows, ia, ja, bw, narrow);
+    const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
+    const int qx = 256 * ia + 128, qy = 256 * ja + 128;
+    int C0 = -1, C1 = 1, C2 = 0, ax0 = 0, ax1 = 0, ax2 = 0, ay0 = 0, ay1 = 0, ay2 = 0;      // "never covered"
+    if (narrow) {
+      // e_k at sample (ia + col, ja + row) = C_k + ax_k col + ay_k row  (all int32: the box spans < 2^14 sub-pixels)
+      const int e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
+      const int e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
+      const int e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
+      if (e0 + e1 + e2 != 0) {                                        // area == 0: skipped (contract)
+        C0 = e0; C1 = e1; C2 = e2;
+        ax0 = -256 * (y2 - y1); ax1 = -256 * (y0 - y2); ax2 = -256 * (y1 - y0);
+        ay0 = 256 * (x2 - x1); ay1 = 256 * (x0 - x2); ay2 = 256 * (x1 - x0);
+      }
+    }
+    r0 = make_uint4((unsigned)C0, (unsigned)ax0, (unsigned)ay0, (unsigned)C1);
+    r1 = make_uint4((unsigned)ax1, (unsigned)ay1, (unsigned)C2, (unsigned)ax2);
+    boxw = (unsigned)((ja - c.row0) * c.R + ia) | ((unsigned)(bw - 1) << 16) | (narrow ? (1u << 24) : 0u);
+    invbw = 1.0f / (float)bw;
+    r3 = make_uint4((unsigned)t, (unsigned)ia | ((unsigned)ja << 16), 0u, 0u);
+    w->tab[lane][0] = r0; w->tab[lane][1] = r1; w->tab[lane][3] = r3;
+    ay2u = (unsigned)ay2;
+  }
   int inc = cnt;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
   const int exc = inc - cnt;
   const int total = __shfl_sync(0xffffffffu, inc, 31);
+  if (lane < n) w->tab[lane][2] = make_uint4(ay2u, (unsigned)exc, boxw, __float_as_uint(invbw));
+  __syncwarp();
   int headbase = 0;
   for (int c0 = 0; c0 < total; c0 += 32) {
-    const unsigned bit = (cnt > 0 && exc >= c0 && exc < c0 + 32) ? (1u << (exc - c0)) : 0u;
+    const unsigned rel = (unsigned)(exc - c0);
+    const unsigned bit = (rel < 32u && cnt > 0) ? (1u << rel) : 0u;
     const unsigned H = __reduce_or_sync(0xffffffffu, bit);
-    // entries are all non-empty, so the index among heads is the owning lane
+    // queued triangles all have samples, so the index among the heads is the owning lane
     const int owner = max(headbase + __popc(H & (0xffffffffu >> (31 - lane))) - 1, 0);
     headbase += __popc(H);
-    const int oexc = __shfl_sync(0xffffffffu, exc, owner);
-    const unsigned obox = __shfl_sync(0xffffffffu, boxpack, owner);
-    const float oinv = __shfl_sync(0xffffffffu, invbw, owner);
     const int s = c0 + lane;
+    bool cov = false;
+    uint4 out = make_uint4(0u, 0u, 0u, 0u); float fa = 1.0f;
     if (s < total) {
-      const uint4 od = qb[owner];
-      const int li = s - oexc, obw = (int)((obox >> 16) & 0xffu) + 1;
-      const int row = (int)(((float)li + 0.5f) * oinv);              // li / obw: (li+0.5)/obw is >= 1/512 from an integer
+      const uint4 a = w->tab[owner][0], b = w->tab[owner][1], d = w->tab[owner][2];
+      const int li = s - (int)d.y, obw = (int)((d.z >> 16) & 0xffu) + 1;
+      const int row = (int)(((float)li + 0.5f) * __uint_as_float(d.w));   // li / obw: (li+0.5)/obw is >= 1/512 from an integer
       const int col = li - row * obw;
-      raster_sample<WITH_ID, Z_SMEM>(c, od, (obox >> 24) & 1u, (int)(obox & 0xffu) + col, (int)((obox >> 8) & 0xffu) + row);
+      out.y = (d.z & 0xffffu) + (unsigned)(row * c.R + col);
+      if (d.z & (1u << 24)) {
+        const int e0 = (int)a.x + (int)a.y * col + (int)a.z * row;
+        const int e1 = (int)a.w + (int)b.x * col + (int)b.y * row;
+        const int e2 = (int)b.z + (int)b.w * col + (int)d.x * row;
+        cov = min(e0, min(e1, e2)) >= 0 || max(e0, max(e1, e2)) <= 0;
+        if (cov) { out.z = __float_as_uint((float)e1); out.w = __float_as_uint((float)e2); fa = (float)(e0 + e1 + e2); }
+      } else {                                                        // triangle spanning >= 64 pixels: int64 edge functions
+        const uint4 e = w->tab[owner][3];
+        int i0, i1, i2;
+        face_unpack(__ldg(c.faces_packed + e.x), i0, i1, i2);
+        const unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
+        const long long x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
+        const long long qx = 256ll * ((int)(e.y & 0xffffu) + col) + 128, qy = 256ll * ((int)(e.y >> 16) + row) + 128;
+        const long long e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
+        const long long e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
+        const long long e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
+        const long long area = e0 + e1 + e2;
+        cov = ((e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0)) && area != 0;
+        if (cov) { out.z = __float_as_uint((float)e1); out.w = __float_as_uint((float)e2); fa = (float)area; }
+      }
+      if (cov) out.x = w->tab[owner][3].x;
+    }
+    const unsigned cm = __ballot_sync(0xffffffffu, cov);
+    if (cm) {
+      if (cov) { const int slot = q2n + __popc(cm & ((1u << lane) - 1u)); w->q2[slot] = out; w->q2a[slot] = fa; }
+      q2n += __popc(cm);
+      __syncwarp();
+      if (q2n >= 32) { q2n -= 32; raster_depth<WITH_ID>(c, w, q2n, 32, lane); __syncwarp(); }
     }
   }
+  return q2n;
 }
 
-template <bool WITH_ID, bool Z_SMEM>
-__global__ void __launch_bounds__(RAST_THREADS, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
+template <bool WITH_ID>
+__global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
     const float4* __restrict__ v_posed, const unsigned long long* __restrict__ faces_packed, const float* __restrict__ dirs,
     const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
     unsigned* __restrict__ vbits_raw, int words) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  // layout: [queues 32 x 64 x 16 B][map band_rows*R*(4|8)][sXY nv*4][sZ nv*4 if Z_SMEM][svert (WITH_ID)]
-  uint4* s_queue = reinterpret_cast<uint4*>(smem_raw);
-  unsigned char* mp = smem_raw + (size_t)RAST_WARPS * RAST_Q * sizeof(uint4);
+  __shared__ int s_next;
+  // layout: [RasterWarp x warps][map band_rows*R*(4|8)][sXY nv*4][svert (WITH_ID)]
+  const int nthreads = blockDim.x, nwarps = nthreads >> 5;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  RasterWarp* w = reinterpret_cast<RasterWarp*>(smem_raw) + warp;
+  unsigned char* mp = smem_raw + (size_t)nwarps * sizeof(RasterWarp);
   unsigned* sz32 = reinterpret_cast<unsigned*>(mp);
   unsigned long long* sz64 = reinterpret_cast<unsigned long long*>(mp);
   const size_t map_bytes = (((size_t)band_rows * R * (WITH_ID ? 8 : 4)) + 15) & ~(size_t)15;
   unsigned* sXY = reinterpret_cast<unsigned*>(mp + map_bytes);
-  float* sZ = reinterpret_cast<float*>(sXY + nv);
-  unsigned* svert = reinterpret_cast<unsigned*>(Z_SMEM ? (sZ + nv) : sZ);
+  unsigned* svert = sXY + nv;
   const int nv_words = (nv + 31) >> 5;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  uint4* myq = s_queue + warp * RAST_Q;
   const WinConst W = make_win(window, R);
 
   for (int unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
@@ -198,61 +246,63 @@ __global__ void __launch_bounds__(RAST_THREADS, 1) vis_raster_kernel(int nf, int
     const int row0 = band * band_rows, rows = min(band_rows, R - row0);
     const int npix = rows * R;
     const LightFrame F = make_frame(dirs + 3 * k, W);
+    if (threadIdx.x == 0) s_next = 0;
     // clear the band
-    if (WITH_ID) { for (int p = threadIdx.x; p < npix; p += RAST_THREADS) sz64[p] = ~0ull; }
+    if (WITH_ID) { for (int p = threadIdx.x; p < npix; p += nthreads) sz64[p] = ~0ull; }
     else {
       uint4* m4 = reinterpret_cast<uint4*>(sz32);
       const uint4 ones = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
-      for (int p = threadIdx.x; p < (npix + 3) >> 2; p += RAST_THREADS) m4[p] = ones;
+      for (int p = threadIdx.x; p < (npix + 3) >> 2; p += nthreads) m4[p] = ones;
     }
-    if (WITH_ID && vbits_raw) for (int p = threadIdx.x; p < nv_words; p += RAST_THREADS) svert[p] = 0u;
+    if (WITH_ID && vbits_raw) for (int p = threadIdx.x; p < nv_words; p += nthreads) svert[p] = 0u;
     // A. project every vertex once
-    for (int v = threadIdx.x; v < nv; v += RAST_THREADS) {
+    for (int v = threadIdx.x; v < nv; v += nthreads) {
       const float4 a = __ldg(v_posed + v);
-      const float dx = a.x - W.cx, dy = a.y - W.cy, dz = a.z - W.cz;
       float px, py;
-      light_project_xy(dx, dy, dz, W, F, px, py);
+      light_project_xy(a.x - W.cx, a.y - W.cy, a.z - W.cz, W, F, px, py);
       const int X = min(max(__float2int_rn(px * 256.0f), 0), 65535), Y = min(max(__float2int_rn(py * 256.0f), 0), 65535);
       sXY[v] = (unsigned)X | ((unsigned)Y << 16);
-      if (Z_SMEM) sZ[v] = light_project_z(dx, dy, dz, F);
     }
     __syncthreads();
 
     RasterCtx c;
-    c.R = R; c.row0 = row0; c.rows = rows; c.sXY = sXY; c.sZ = sZ; c.v_posed = v_posed; c.faces_packed = faces_packed;
+    c.R = R; c.row0 = row0; c.rows = rows; c.sXY = sXY; c.v_posed = v_posed; c.faces_packed = faces_packed;
     c.sz32 = sz32; c.sz64 = sz64; c.W = W; c.F = F;
-    // B. triangles: one per lane, non-empty boxes queued
-    int qn = 0;                                             // warp-uniform
-    for (int base = warp * 32; base < nf; base += RAST_THREADS) {
+    // B1. triangles: one per lane, 32 per warp fetched dynamically; non-empty boxes queued
+    int qn = 0, q2n = 0;                                    // warp-uniform queue fills
+    for (;;) {
+      int base = 0;
+      if (lane == 0) base = atomicAdd(&s_next, 32);
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (base >= nf) break;
       const int t = base + lane;
       bool ne = false;
-      uint4 d = make_uint4(0u, 0u, 0u, (unsigned)t);
       if (t < nf) {
         int i0, i1, i2;
         face_unpack(__ldg(faces_packed + t), i0, i1, i2);
-        d.x = sXY[i0]; d.y = sXY[i1]; d.z = sXY[i2];
         int ia, ja, bw; bool narrow;
-        ne = tri_box(d.x, d.y, d.z, R, row0, rows, ia, ja, bw, narrow) > 0;
+        ne = tri_box(sXY[i0], sXY[i1], sXY[i2], R, row0, rows, ia, ja, bw, narrow) > 0;
       }
       const unsigned m = __ballot_sync(0xffffffffu, ne);
       if (m) {
-        if (ne) myq[qn + __popc(m & ((1u << lane) - 1u))] = d;
+        if (ne) w->q1[qn + __popc(m & ((1u << lane) - 1u))] = t;
         qn += __popc(m);
         __syncwarp();
         if (qn >= 32) {
           qn -= 32;
-          raster_round<WITH_ID, Z_SMEM>(c, myq + qn, 32, lane);
+          q2n = raster_round<WITH_ID>(c, w, qn, 32, lane, q2n);
           __syncwarp();
         }
       }
     }
-    if (qn) raster_round<WITH_ID, Z_SMEM>(c, myq, qn, lane);
+    if (qn) { q2n = raster_round<WITH_ID>(c, w, 0, qn, lane, q2n); __syncwarp(); }
+    if (q2n) raster_depth<WITH_ID>(c, w, 0, q2n, lane);
     __syncthreads();
 
     // write the band out
     const size_t gbase = ((size_t)k * R + row0) * R;
     if (WITH_ID) {
-      for (int p = threadIdx.x; p < npix; p += RAST_THREADS) {
+      for (int p = threadIdx.x; p < npix; p += nthreads) {
         const unsigned long long key = sz64[p];
         zmap[gbase + p] = (unsigned)(key >> 32);
         const int tri = (key == ~0ull) ? -1 : (int)(unsigned)(key & 0xffffffffu);
@@ -268,7 +318,7 @@ __global__ void __launch_bounds__(RAST_THREADS, 1) vis_raster_kernel(int nf, int
       if (vbits_raw) {
         __syncthreads();
         const unsigned bit = 1u << (k & 31);
-        for (int wd = threadIdx.x; wd < nv_words; wd += RAST_THREADS) {
+        for (int wd = threadIdx.x; wd < nv_words; wd += nthreads) {
           unsigned m = svert[wd];
           while (m) {
             const int b = __ffs(m) - 1; m &= m - 1;
@@ -280,35 +330,40 @@ __global__ void __launch_bounds__(RAST_THREADS, 1) vis_raster_kernel(int nf, int
     } else if ((R & 3) == 0) {
       const uint4* m4 = reinterpret_cast<const uint4*>(sz32);
       uint4* g4 = reinterpret_cast<uint4*>(zmap + gbase);
-      for (int p = threadIdx.x; p < npix >> 2; p += RAST_THREADS) g4[p] = m4[p];
+      for (int p = threadIdx.x; p < npix >> 2; p += nthreads) g4[p] = m4[p];
     } else {
-      for (int p = threadIdx.x; p < npix; p += RAST_THREADS) zmap[gbase + p] = sz32[p];
+      for (int p = threadIdx.x; p < npix; p += nthreads) zmap[gbase + p] = sz32[p];
     }
-    __syncthreads();                                      // the map and the vertex tables are reused by the next unit
+    __syncthreads();                                      // the map and the vertex table are reused by the next unit
   }
 }
 
-// shared-memory plan: returns bytes, band rows and whether per-vertex z fits
-size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* z_smem) {
-  const size_t budget = 227 * 1024;
-  const size_t fixed = (size_t)RAST_WARPS * RAST_Q * 16 + (size_t)n_verts * 4 + (with_id ? (size_t)((n_verts + 31) / 32) * 4 : 0) + 32;
+// shared-memory plan: picks the CTA size (1024 / 512 / 256 threads) that minimises bands / warps; returns bytes
+size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads) {
+  const size_t budget = 227 * 1024 - 256;
   const size_t per_row = (size_t)res * (with_id ? 8 : 4);
-  const size_t zbytes = (size_t)n_verts * 4;
-  *z_smem = (fixed + zbytes + per_row * res <= budget) ? 1 : 0;      // z only when the whole map still fits in one band
-  size_t avail = budget > fixed + (*z_smem ? zbytes : 0) ? budget - fixed - (*z_smem ? zbytes : 0) : 0;
-  int rows = (int)(avail / per_row);
-  if (rows > res) rows = res;
-  if (rows < 1) { *band_rows = 0; return 0; }                         // mesh too large for the shared-memory vertex table
-  int bands = (res + rows - 1) / rows;
-  rows = (res + bands - 1) / bands;                                   // even bands
-  *band_rows = rows;
-  return fixed + (*z_smem ? zbytes : 0) + ((per_row * rows + 15) & ~(size_t)15);
+  size_t best = 0; double best_score = 1e30;
+  *band_rows = 0; *threads = 0;
+  for (int th = 1024; th >= 256; th >>= 1) {
+    const size_t fixed = (size_t)(th / 32) * sizeof(RasterWarp) + (size_t)n_verts * 4 + (with_id ? (size_t)((n_verts + 31) / 32) * 4 : 0) + 32;
+    if (fixed + per_row > budget) continue;
+    int rows = (int)((budget - fixed) / per_row);
+    if (rows > res) rows = res;
+    int bands = (res + rows - 1) / rows;
+    rows = (res + bands - 1) / bands;                                 // even bands
+    const double score = (double)bands / (double)(th / 32);
+    if (score < best_score) {
+      best_score = score; *band_rows = rows; *threads = th;
+      best = fixed + ((per_row * rows + 15) & ~(size_t)15);
+    }
+  }
+  return best;                                                        // 0: mesh too large for the shared-memory vertex table
 }
 
 cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {
   const bool with_id = p->mode == 1 || p->keep_maps;
-  int band_rows = 0, z_smem = 0;
-  const size_t smem = rga_vis_raster_smem(p->res, with_id, av->n_verts, &band_rows, &z_smem);
+  int band_rows = 0, threads = 0;
+  const size_t smem = rga_vis_raster_smem(p->res, with_id, av->n_verts, &band_rows, &threads);
   if (band_rows < 1) return cudaErrorInvalidConfiguration;
   const int n_bands = (p->res + band_rows - 1) / band_rows;
   const int words = (p->n_dirs + 31) / 32;
@@ -318,13 +373,8 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
   if (raw) cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s);
 #define RAST_ARGS av->n_faces, av->n_verts, p->res, band_rows, n_bands, n_units, av->v_posed, av->faces_packed, p->dirs, av->window, \
     av->zmap, av->idmap, raw, words
-  if (with_id) {
-    if (z_smem) vis_raster_kernel<true, true><<<grid, RAST_THREADS, smem, s>>>(RAST_ARGS);
-    else vis_raster_kernel<true, false><<<grid, RAST_THREADS, smem, s>>>(RAST_ARGS);
-  } else {
-    if (z_smem) vis_raster_kernel<false, true><<<grid, RAST_THREADS, smem, s>>>(RAST_ARGS);
-    else vis_raster_kernel<false, false><<<grid, RAST_THREADS, smem, s>>>(RAST_ARGS);
-  }
+  if (with_id) vis_raster_kernel<true><<<grid, threads, smem, s>>>(RAST_ARGS);
+  else vis_raster_kernel<false><<<grid, threads, smem, s>>>(RAST_ARGS);
   av->launches += 1;
   rga_prof_mark(av, "vis_raster", s);
   return cudaGetLastError();
@@ -494,11 +544,9 @@ cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaSt
 }
 
 int rga_vis_init_attributes() {
-  const int mx = 227 * 1024;
-  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  const int mx = 227 * 1024 - 256;            // the static s_next counts against the 227 KB block limit
+  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_depth_test_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   return (int)e;
 }
