@@ -26,7 +26,7 @@ sys.path.insert(0, ROOT)
 METRIC = "relit posed frames/sec (100k Gaussians, 512x512)"
 WORKLOAD = "configs[1] SMPL-sized: 6,890 v / 13,776 f / 24 bones, 100k Gaussians, 16x32 env, 512 dirs @128^2, 512x512"
 # algorithmic work per unit of each kernel (fp32 flop, FMA = 2)
-FLOP_PER_UNIT = {"shade": 70.0, "vis_depth_test": 40.0, "vis_raster": 220.0, "composite": 30.0}
+FLOP_PER_UNIT = {"shade": 70.0, "vis_depth_test": 40.0, "vis_raster": 220.0, "composite_segments": 30.0}
 FP32_PEAK_TFLOPS = 2 * 128 * 148 * 1.965e9 / 1e12          # 74.4: 148 SMs x 128 FP32 lanes x FMA x 1.965 GHz (guide)
 
 
@@ -199,7 +199,7 @@ def main():
     front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
     rg = av.read("TILE_RANGES").reshape(-1, 2).astype(np.int64)
     units = {"shade": front * 512 * 0.5, "vis_depth_test": len(gp) * K, "vis_raster": len(inp["faces"]) * K,
-             "composite": float(((rg[:, 1] - rg[:, 0]) * 256).sum())}
+             "composite_segments": float(((rg[:, 1] - rg[:, 0]) * 256).sum())}
     dom = max((k for k in kern_ms if k in units), key=lambda k: kern_ms[k])
     ach = units[dom] * FLOP_PER_UNIT[dom] / (kern_ms[dom] * 1e-3) / 1e12
     pk, pk_kind = peaks()

@@ -1,13 +1,27 @@
 // H8 (depth digit) + H10: per-tile sort and front-to-back alpha compositing (PAPER.md:103 -> 3DGS rasteriser, DESIGN.md
 // A18; black background PAPER.md:239-241 is the default of the bg parameter).
-// One CTA per 16x16 tile.  The tile's bucket of (depth bits << 32 | Gaussian) keys (binned by sort_kernels.cu) is
-// loaded into shared memory, sorted there with an ascending-only bitonic network (exact integer compare, so the order
-// equals the stable (tile, depth) sort of the emission order), written back as the sorted key/value lists, and then
-// blended front to back straight from shared memory in batches of 256; a CTA stops as soon as every pixel has saturated
-// (T(1-alpha) < 1e-4).  The blend is FAST arithmetic (FMA, ex2.approx): compared with the fp64 oracle under tolerance.
+//
+// Three kernels (the first version did all of this in one CTA per tile and left the SMs 63 % idle: 208 active tiles on
+// 148 SMs, each walking up to 1,304 entries serially -- profiles/r01a_ncu_full.md):
+//   tile_sort_kernel        one CTA per tile: the tile's bucket of (depth bits << 32 | Gaussian) keys (binned by
+//                           sort_kernels.cu) is sorted in shared memory by an ascending-only bitonic network (exact
+//                           integer compare, so the order equals the stable (tile, depth) sort of the emission order)
+//                           and written out as the sorted key/value lists; it also lists the tile's work items.
+//   composite_segment_kernel  front-to-back "over" is associative: (C,T) o (C',T') = (C + T C', T T').  A work item is
+//                           one segment of RGA_SEG consecutive list entries of one tile; persistent CTAs blend every
+//                           segment from T = 1 for the tile's 256 pixels, in parallel over all segments of all tiles.
+//   composite_resolve_kernel  folds the segment partials of each pixel in order.  The 3DGS stopping rule (stop before
+//                           the Gaussian that would take T below 1e-4) is not associative: a pixel whose running T
+//                           times the next segment's T falls below the threshold stops folding and flags that segment.
+//                           Also writes the background for empty tiles.
+//   composite_replay_kernel   replays every flagged segment entry by entry with the exact rule for the pixels that
+//                           stopped in it -- all flagged segments of the frame in parallel (inside one CTA per tile
+//                           these serial replays took 209 us at config 1).
+// The blend is FAST arithmetic (FMA, ex2.approx): compared with the fp64 oracle under tolerance.
 #include "rga_internal.h"
 
 #define CB 256
+#define LOG2E_F 1.4426950408889634f
 
 // ascending-only bitonic network on buf[0..n): every compare-exchange puts the minimum at the lower index, so virtual
 // +inf padding above n never moves and n need not be a power of two.
@@ -30,20 +44,17 @@ __device__ __forceinline__ void bitonic_sort(unsigned long long* buf, int n) {
 
 // Handles the tiles whose bucket length n satisfies n_lo < n <= n_hi (others return at once); buckets longer than the
 // shared-memory capacity `scap` are sorted in place in global memory by the same network.
-__global__ void __launch_bounds__(CB) composite_kernel(int W, int H, int TX, unsigned capacity, int scap, int n_lo, int n_hi,
-    const uint2* __restrict__ ranges, unsigned long long* __restrict__ lkeys, unsigned long long* __restrict__ keys_out,
-    unsigned* __restrict__ vals_out, const float2* __restrict__ mu2d, const float4* __restrict__ conic_o,
-    const float4* __restrict__ color, float3 bg, float* __restrict__ image, float* __restrict__ t_final,
-    unsigned* __restrict__ n_contrib) {
+__global__ void __launch_bounds__(CB) tile_sort_kernel(unsigned capacity, int scap, int n_lo, int n_hi,
+    const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, unsigned long long* __restrict__ lkeys,
+    unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ item_tab) {
   extern __shared__ __align__(16) unsigned long long s_keys[];
-  __shared__ float2 s_mu[CB];
-  __shared__ float4 s_co[CB];
-  __shared__ float4 s_col[CB];
-  const int tile = blockIdx.y * TX + blockIdx.x;
+  const int tile = blockIdx.x;
   uint2 rg = ranges[tile];
   rg.x = min(rg.x, capacity); rg.y = min(rg.y, capacity);
   const int n = (int)(rg.y - rg.x);
   if (n <= n_lo || n > n_hi) return;
+  const unsigned so = seg_off[tile];
+  for (int j = threadIdx.x; j < (n + RGA_SEG - 1) / RGA_SEG; j += CB) item_tab[so + j] = (unsigned)tile;
   unsigned long long* buf = lkeys + rg.x;
   if (n <= scap) {
     for (int i = threadIdx.x; i < n; i += CB) s_keys[i] = buf[i];
@@ -56,80 +67,214 @@ __global__ void __launch_bounds__(CB) composite_kernel(int W, int H, int TX, uns
     keys_out[rg.x + i] = ((unsigned long long)(unsigned)tile << 32) | (k >> 32);
     vals_out[rg.x + i] = (unsigned)k;
   }
-  const int px = blockIdx.x * RGA_TILE + (threadIdx.x & 15), py = blockIdx.y * RGA_TILE + (threadIdx.x >> 4);
-  const bool inside = px < W && py < H;
-  const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;        // DESIGN.md A21: sample at the pixel centre
-  bool done = !inside;
-  float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
-  unsigned last = 0;
-  for (int b = 0; b < n; b += CB) {
-    if (__syncthreads_count(done) == CB) break;
-    const int m = min(CB, n - b);
-    if ((int)threadIdx.x < m) {
-      unsigned g = (unsigned)buf[b + threadIdx.x];
-      s_mu[threadIdx.x] = mu2d[g]; s_co[threadIdx.x] = conic_o[g]; s_col[threadIdx.x] = color[g];
-    }
+}
+
+// shared-memory staging of one segment: centre, conic pre-scaled so that alpha = o * 2^(x(A x + B y) + C y^2), colour
+struct SegStage { float2 mu[RGA_SEG]; float4 co[RGA_SEG]; float4 col[RGA_SEG]; };
+
+__device__ __forceinline__ void stage_segment(SegStage& st, int m, const unsigned* __restrict__ vals, const float2* __restrict__ mu2d,
+                                              const float4* __restrict__ conic_o, const float4* __restrict__ color) {
+  if ((int)threadIdx.x < m) {
+    const unsigned g = vals[threadIdx.x];
+    const float4 c = conic_o[g];
+    st.mu[threadIdx.x] = mu2d[g];
+    st.co[threadIdx.x] = make_float4(-0.5f * LOG2E_F * c.x, -LOG2E_F * c.y, -0.5f * LOG2E_F * c.z, c.w);
+    st.col[threadIdx.x] = color[g];
+  }
+}
+
+// alpha of entry j at pixel centre (fx, fy); 0 when the 3DGS rules skip it (power > 0, alpha < 1/255)
+__device__ __forceinline__ float seg_alpha(const SegStage& st, int j, float fx, float fy) {
+  const float2 mm = st.mu[j]; const float4 co = st.co[j];
+  const float dx = mm.x - fx, dy = mm.y - fy;
+  const float p2 = dx * (co.x * dx + co.y * dy) + co.z * dy * dy;        // log2(e) * power
+  const float al = fminf(0.99f, co.w * exp2f(p2));
+  return (p2 > 0.f || al < 1.f / 255.f) ? 0.f : al;
+}
+
+__global__ void __launch_bounds__(CB) composite_segment_kernel(int W, int H, int TX, const unsigned* __restrict__ num_items,
+    const unsigned* __restrict__ item_tab, const unsigned* __restrict__ seg_off, const uint2* __restrict__ ranges,
+    const unsigned* __restrict__ vals, const float2* __restrict__ mu2d, const float4* __restrict__ conic_o,
+    const float4* __restrict__ color, float4* __restrict__ part, unsigned* __restrict__ part_last) {
+  __shared__ SegStage st;
+  const unsigned n_items = *num_items;
+  for (unsigned item = blockIdx.x; item < n_items; item += gridDim.x) {
+    const unsigned tile = item_tab[item];
+    const unsigned seg = item - seg_off[tile];
+    const uint2 rg = ranges[tile];
+    const unsigned b0 = rg.x + seg * RGA_SEG;
+    const int m = (int)min((unsigned)RGA_SEG, rg.y - b0);
     __syncthreads();
-    // four entries per trip: their alphas are independent (ILP for the exp chain); only the blend is sequential
-    for (int j = 0; j < m && !done; j += 4) {
+    stage_segment(st, m, vals + b0, mu2d, conic_o, color);
+    __syncthreads();
+    const int px = (int)(tile % TX) * RGA_TILE + (threadIdx.x & 15), py = (int)(tile / TX) * RGA_TILE + (threadIdx.x >> 4);
+    const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;        // DESIGN.md A21: sample at the pixel centre
+    float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
+    unsigned last = 0;
+    bool stop = !(px < W && py < H);
+    // four entries per trip: their alphas are independent (ILP for the ex2 chain); only the blend is sequential
+    for (int j = 0; j < m && !stop; j += 4) {
       float a[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const float2 mm = s_mu[j + u]; const float4 co = s_co[j + u];
-        const float dx = mm.x - fx, dy = mm.y - fy;
-        const float power = -0.5f * (co.x * dx * dx + co.z * dy * dy) - co.y * dx * dy;
-        const float al = fminf(0.99f, co.w * __expf(power));
-        a[u] = (power > 0.f || j + u >= m) ? 0.f : al;
-      }
-      if (fmaxf(fmaxf(a[0], a[1]), fmaxf(a[2], a[3])) < 1.f / 255.f) continue;
+      for (int u = 0; u < 4; ++u) a[u] = (j + u < m) ? seg_alpha(st, j + u, fx, fy) : 0.f;
+      if (fmaxf(fmaxf(a[0], a[1]), fmaxf(a[2], a[3])) == 0.f) continue;
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
-        if (!done && a[u] >= 1.f / 255.f) {
+        if (!stop && a[u] > 0.f) {
           const float test_T = T * (1.f - a[u]);
-          if (test_T < 1e-4f) done = true;
+          // below the threshold from T = 1 means below it from any start: the resolve pass replays this segment
+          if (test_T < 1e-4f) { stop = true; T = 0.f; }
           else {
-            const float4 c = s_col[j + u];
+            const float4 c = st.col[j + u];
             const float w = a[u] * T;
             C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
-            T = test_T; last = (unsigned)(b + j + u + 1);
+            T = test_T; last = (unsigned)(j + u + 1);
           }
         }
       }
     }
-  }
-  if (inside) {
-    size_t p = (size_t)py * W + px;
-    image[3 * p] = C0 + T * bg.x; image[3 * p + 1] = C1 + T * bg.y; image[3 * p + 2] = C2 + T * bg.z;
-    t_final[p] = T; n_contrib[p] = last;
+    part[(size_t)item * CB + threadIdx.x] = make_float4(C0, C1, C2, T);
+    part_last[(size_t)item * CB + threadIdx.x] = last;
   }
 }
 
-// empty tiles: background only
-__global__ void __launch_bounds__(256) clear_kernel(int npix, float3 bg, float* __restrict__ image, float* __restrict__ t_final,
-                                                    unsigned* __restrict__ n_contrib) {
-  int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= npix) return;
-  image[3 * p] = bg.x; image[3 * p + 1] = bg.y; image[3 * p + 2] = bg.z; t_final[p] = 1.f; n_contrib[p] = 0u;
+// one entry of the exact sequential rule, read straight from global memory (rare continuation path of the replay)
+__device__ __forceinline__ float global_alpha(unsigned g, float fx, float fy, const float2* __restrict__ mu2d,
+                                              const float4* __restrict__ conic_o) {
+  const float2 mm = mu2d[g]; const float4 c = conic_o[g];
+  const float dx = mm.x - fx, dy = mm.y - fy;
+  const float p2 = dx * ((-0.5f * LOG2E_F * c.x) * dx + (-LOG2E_F * c.y) * dy) + (-0.5f * LOG2E_F * c.z) * dy * dy;
+  const float al = fminf(0.99f, c.w * exp2f(p2));
+  return (p2 > 0.f || al < 1.f / 255.f) ? 0.f : al;
+}
+
+// Folds the segment partials of each pixel in order (no shared memory, no barrier).  A pixel whose running T times the
+// next segment's T falls below the stopping threshold stops folding there: its accumulated (C, T, last) are written
+// out as they stand, the segment index goes to stop_seg and the work item is flagged for composite_replay_kernel.
+__global__ void __launch_bounds__(CB) composite_resolve_kernel(int W, int H, int TX, unsigned capacity,
+    const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, const float4* __restrict__ part,
+    const unsigned* __restrict__ part_last, float3 bg, float* __restrict__ image, float* __restrict__ t_final,
+    unsigned* __restrict__ n_contrib, int* __restrict__ stop_seg, unsigned char* __restrict__ item_flag) {
+  const int tile = blockIdx.y * TX + blockIdx.x;
+  uint2 rg = ranges[tile];
+  rg.x = min(rg.x, capacity); rg.y = min(rg.y, capacity);
+  const int n = (int)(rg.y - rg.x), nseg = (n + RGA_SEG - 1) / RGA_SEG;
+  const unsigned so = seg_off[tile];
+  const int px = blockIdx.x * RGA_TILE + (threadIdx.x & 15), py = blockIdx.y * RGA_TILE + (threadIdx.x >> 4);
+  if (!(px < W && py < H)) return;
+  float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
+  unsigned last = 0;
+  int stop = -1;
+  const float4* pp = part + (size_t)so * CB + threadIdx.x;
+  const unsigned* pl = part_last + (size_t)so * CB + threadIdx.x;
+  for (int s0 = 0; s0 < nseg && stop < 0; s0 += 4) {       // four segments per trip: their loads are independent
+    float4 p[4]; unsigned l[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (s0 + u < nseg) { p[u] = pp[(size_t)(s0 + u) * CB]; l[u] = pl[(size_t)(s0 + u) * CB]; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (s0 + u < nseg && stop < 0) {
+        if (T * p[u].w >= 1.00001e-4f) {                   // the whole segment passes the stopping rule
+          C0 = fmaf(T, p[u].x, C0); C1 = fmaf(T, p[u].y, C1); C2 = fmaf(T, p[u].z, C2);
+          T *= p[u].w;
+          if (l[u]) last = (unsigned)((s0 + u) * RGA_SEG) + l[u];
+        } else stop = s0 + u;
+      }
+    }
+  }
+  const size_t p = (size_t)py * W + px;
+  if (stop >= 0) {                                         // unfinished: background is added by the replay
+    image[3 * p] = C0; image[3 * p + 1] = C1; image[3 * p + 2] = C2;
+    item_flag[so + stop] = 1;
+  } else {
+    image[3 * p] = C0 + T * bg.x; image[3 * p + 1] = C1 + T * bg.y; image[3 * p + 2] = C2 + T * bg.z;
+  }
+  t_final[p] = T; n_contrib[p] = last; stop_seg[p] = stop;
+}
+
+// Replays flagged segments entry by entry with the exact 3DGS stopping rule for the pixels that stopped in them, all
+// flagged (tile, segment) items of the frame in parallel.
+__global__ void __launch_bounds__(CB) composite_replay_kernel(int W, int H, int TX, const unsigned* __restrict__ num_items,
+    const unsigned* __restrict__ item_tab, const unsigned* __restrict__ seg_off, const uint2* __restrict__ ranges,
+    const unsigned* __restrict__ vals, const float2* __restrict__ mu2d, const float4* __restrict__ conic_o,
+    const float4* __restrict__ color, float3 bg, float* __restrict__ image, float* __restrict__ t_final,
+    unsigned* __restrict__ n_contrib, const int* __restrict__ stop_seg, unsigned char* __restrict__ item_flag) {
+  __shared__ SegStage st;
+  const unsigned n_items = *num_items;
+  for (unsigned item = blockIdx.x; item < n_items; item += gridDim.x) {
+    if (!item_flag[item]) continue;                        // block-uniform
+    __syncthreads();
+    if (threadIdx.x == 0) item_flag[item] = 0;             // re-armed for the next frame
+    const unsigned tile = item_tab[item];
+    const int seg = (int)(item - seg_off[tile]);
+    const uint2 rg = ranges[tile];
+    const int n = (int)(rg.y - rg.x);
+    const int m = min(RGA_SEG, n - seg * RGA_SEG);
+    stage_segment(st, m, vals + rg.x + seg * RGA_SEG, mu2d, conic_o, color);
+    __syncthreads();
+    const int px = (int)(tile % TX) * RGA_TILE + (threadIdx.x & 15), py = (int)(tile / TX) * RGA_TILE + (threadIdx.x >> 4);
+    if (!(px < W && py < H)) continue;
+    const size_t p = (size_t)py * W + px;
+    if (stop_seg[p] != seg) continue;
+    const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;
+    float T = t_final[p], C0 = image[3 * p], C1 = image[3 * p + 1], C2 = image[3 * p + 2];
+    unsigned last = n_contrib[p];
+    bool done = false;
+    for (int j = 0; j < m; ++j) {
+      const float a = seg_alpha(st, j, fx, fy);
+      if (a > 0.f) {
+        const float test_T = T * (1.f - a);
+        if (test_T < 1e-4f) { done = true; break; }
+        const float4 c = st.col[j];
+        const float w = a * T;
+        C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+        T = test_T; last = (unsigned)(seg * RGA_SEG + j + 1);
+      }
+    }
+    // the fold's threshold has a 1e-5 relative guard band: a pixel inside it may not stop here after all and walks the
+    // rest of its list from global memory (rare)
+    for (int i = (seg + 1) * RGA_SEG; i < n && !done; ++i) {
+      const unsigned g = vals[rg.x + i];
+      const float a = global_alpha(g, fx, fy, mu2d, conic_o);
+      if (a > 0.f) {
+        const float test_T = T * (1.f - a);
+        if (test_T < 1e-4f) { done = true; break; }
+        const float4 c = color[g];
+        const float w = a * T;
+        C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+        T = test_T; last = (unsigned)(i + 1);
+      }
+    }
+    image[3 * p] = C0 + T * bg.x; image[3 * p + 1] = C1 + T * bg.y; image[3 * p + 2] = C2 + T * bg.z;
+    t_final[p] = T; n_contrib[p] = last;
+  }
 }
 
 #define SCAP_SMALL 2048
 #define SCAP_LARGE 24576
 
 int rga_composite_init_attributes() {
-  return (int)cudaFuncSetAttribute(composite_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SCAP_LARGE * 8);
+  return (int)cudaFuncSetAttribute(tile_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SCAP_LARGE * 8);
 }
 
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s) {
-  int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
-  int npix = cam->width * cam->height;
-  clear_kernel<<<(npix + 255) / 256, 256, 0, s>>>(npix, bg, out, av->t_final, av->n_contrib);
-  rga_prof_mark(av, "clear", s);
-#define COMP_ARGS(scap, lo, hi) cam->width, cam->height, TX, (unsigned)av->max_dup, scap, lo, hi, av->ranges, av->keys[0], av->keys[1], \
-    av->vals[0], av->mu2d, av->conic_o, av->color, bg, out, av->t_final, av->n_contrib
-  composite_kernel<<<dim3(TX, TY), CB, SCAP_SMALL * 8, s>>>(COMP_ARGS(SCAP_SMALL, 0, SCAP_SMALL));
-  rga_prof_mark(av, "composite", s);
-  composite_kernel<<<dim3(TX, TY), CB, SCAP_LARGE * 8, s>>>(COMP_ARGS(SCAP_LARGE, SCAP_SMALL, 0x7fffffff));
-  rga_prof_mark(av, "composite_long", s);
-  av->launches += 3;
+  const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
+  const int ntiles = TX * TY;
+#define SORT_ARGS(scap, lo, hi) (unsigned)av->max_dup, scap, lo, hi, av->ranges, av->seg_off, av->keys[0], av->keys[1], av->vals[0], av->item_tab
+  tile_sort_kernel<<<ntiles, CB, SCAP_SMALL * 8, s>>>(SORT_ARGS(SCAP_SMALL, 0, SCAP_SMALL));
+  rga_prof_mark(av, "tile_sort", s);
+  tile_sort_kernel<<<ntiles, CB, SCAP_LARGE * 8, s>>>(SORT_ARGS(SCAP_LARGE, SCAP_SMALL, 0x7fffffff));
+  rga_prof_mark(av, "tile_sort_long", s);
+  composite_segment_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
+      av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, av->part, av->part_last);
+  rga_prof_mark(av, "composite_segments", s);
+  composite_resolve_kernel<<<dim3(TX, TY), CB, 0, s>>>(cam->width, cam->height, TX, (unsigned)av->max_dup, av->ranges, av->seg_off,
+      av->part, av->part_last, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
+  rga_prof_mark(av, "composite_resolve", s);
+  composite_replay_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
+      av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
+  rga_prof_mark(av, "composite_replay", s);
+  av->launches += 5;
   return cudaGetLastError();
 }

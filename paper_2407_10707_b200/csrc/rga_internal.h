@@ -7,6 +7,7 @@
 
 #define RGA_TILE 16
 #define RGA_MAX_PROF 96
+#define RGA_SEG 64               // compositing segment: list entries blended by one work item
 
 struct rga_avatar {
   // sizes
@@ -53,6 +54,14 @@ struct rga_avatar {
   unsigned long long* keys[2]; unsigned* vals[2];   // keys[0]: binned local keys (depth<<32|g); keys[1]/vals[0]: sorted output
   unsigned* num_dup;           // [1] D (device)
   uint2* ranges;               // [tiles]
+  unsigned* seg_off;           // [tiles + 1] exclusive scan of ceil(n_t / RGA_SEG)
+  unsigned* num_items;         // [1] number of (tile, segment) work items (device)
+  unsigned* item_tab;          // [items_cap] tile of each work item
+  float4* part;                // [items_cap][256] per-pixel partial (C, T) of each segment
+  unsigned* part_last;         // [items_cap][256] last contributing entry of the segment (1-based, 0 = none)
+  long long items_cap;
+  int* stop_seg;               // [pixels] segment in which the pixel's blend stops (-1: list exhausted)
+  unsigned char* item_flag;    // [items_cap] work item has pixels to replay (cleared by the replay kernel)
   float* t_final; unsigned* n_contrib;
   int* status;                 // sticky device status
   int sorted_buf;              // which of keys[]/vals[] holds the sorted result
