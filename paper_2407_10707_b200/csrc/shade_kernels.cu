@@ -32,6 +32,11 @@ cudaError_t rga_launch_env_table(rga_avatar* av, const rga_env* env, cudaStream_
   return cudaGetLastError();
 }
 
+// MUFU approximations (relative error ~1e-6; the result is compared under the 2e-3 tolerance)
+__device__ __forceinline__ float rsq_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float ex2_approx(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
 template <int LANES, int MODE>
 __global__ void __launch_bounds__(128) shade_kernel(int ng, int ne, int K, int words, int Kg, int Kv,
     const float4* __restrict__ g_posed, const float4* __restrict__ g_nposed, const float4* __restrict__ g_static,
@@ -67,8 +72,9 @@ __global__ void __launch_bounds__(128) shade_kernel(int ng, int ne, int K, int w
   const float rough = ar.w, al = rough * rough, al2 = al * al;           // Eq.13: alpha = gamma^2
   const float kk = (rough + 1.f) * (rough + 1.f) * 0.125f, omk = 1.f - kk;   // Eq.15
   const float go = nwo * omk + kk;
-  // n x w_o, for 1 - (n.h)^2 = |n x (w_i + w_o)|^2 / |w_i + w_o|^2 (the direct form cancels badly for alpha^2 ~ 1e-4)
-  const float cox = n.y * woz - n.z * woy, coy = n.z * wox - n.x * woz, coz = n.x * woy - n.y * wox;
+  // 1 - (n.h)^2 = |t|^2 / |w_i + w_o|^2 with t the part of w_i + w_o tangent to n, summed from the two tangent parts
+  // (the direct form 1 - nh^2 cancels badly for alpha^2 ~ 1e-4); this is w_o's
+  const float tox = fmaf(-nwo_raw, n.x, wox), toy = fmaf(-nwo_raw, n.y, woy), toz = fmaf(-nwo_raw, n.z, woz);
   const float cS = al2 / (4.f * PI_F * go);                              // D F G /(4 ni no) = cS F / (den^2 gi)
   float u0 = 0.f, u1 = 0.f, u2 = 0.f; int j0 = 0, j1 = 0, j2 = 0;
   if (MODE == 1) {
@@ -97,15 +103,14 @@ __global__ void __launch_bounds__(128) shade_kernel(int ng, int ne, int K, int w
     const float4 LA = sE[2 * k + 1];
     const float ow = wox * wi.x + woy * wi.y + woz * wi.z;
     const float hl2 = fmaxf(2.f + 2.f * ow, 1e-12f);                     // |w_i + w_o|^2
-    const float hinv = rsqrtf(hl2);
+    const float hinv = rsq_approx(hl2);
     const float nh = (cs + nwo_raw) * hinv;
-    const float oh = (1.f + ow) * hinv;
-    const float cx = fmaf(n.y, wi.z, -n.z * wi.y) + cox, cy = fmaf(n.z, wi.x, -n.x * wi.z) + coy,
-                cz = fmaf(n.x, wi.y, -n.y * wi.x) + coz;
-    const float den = fmaf(al2 * nh, nh, (cx * cx + cy * cy + cz * cz) * (hinv * hinv));   // (n.h)^2 (a^2 - 1) + 1, Eq.13
-    const float F = 0.04f + 0.96f * exp2f((-5.55473f * oh - 6.98316f) * oh);   // Eq.14
-    const float gi = cs * omk + kk;
-    const float sp = cS * F * __frcp_rn(den * den * gi);
+    const float oh = (0.5f * hl2) * hinv;                                // w_o . h = (1 + w_o.w_i) / |w_i + w_o|
+    const float tx = fmaf(-cs, n.x, wi.x) + tox, ty = fmaf(-cs, n.y, wi.y) + toy, tz = fmaf(-cs, n.z, wi.z) + toz;
+    const float den = fmaf(al2 * nh, nh, (tx * tx + ty * ty + tz * tz) * (hinv * hinv));   // (n.h)^2 (a^2 - 1) + 1, Eq.13
+    const float F = fmaf(0.96f, ex2_approx((-5.55473f * oh - 6.98316f) * oh), 0.04f);     // Eq.14
+    const float gi = fmaf(cs, omk, kk);
+    const float sp = cS * F * rcp_approx(den * den * gi);
     const float w = v * cs;
     const float ws = w * sp;
     d0 = fmaf(LA.x, w, d0); d1 = fmaf(LA.y, w, d1); d2 = fmaf(LA.z, w, d2);
