@@ -21,52 +21,107 @@
 #include "rga_internal.h"
 
 #define CB 256
+#define SCAP_SMALL RGA_SORT_SMALL
+#define SCAP_LARGE 24576
 #define LOG2E_F 1.4426950408889634f
 
-// ascending-only bitonic network on buf[0..n): every compare-exchange puts the minimum at the lower index, so virtual
-// +inf padding above n never moves and n need not be a power of two.
-__device__ __forceinline__ void bitonic_sort(unsigned long long* buf, int n) {
-  for (int k = 2; (k >> 1) < n; k <<= 1) {
-    for (int i = threadIdx.x; i < n; i += CB) {             // mirror step: i <-> i ^ (k-1)
-      int p = i ^ (k - 1);
-      if (p > i && p < n) { unsigned long long a = buf[i], b = buf[p]; if (b < a) { buf[i] = b; buf[p] = a; } }
-    }
-    __syncthreads();
-    for (int j = k >> 2; j > 0; j >>= 1) {
-      for (int i = threadIdx.x; i < n; i += CB) {
-        int p = i ^ j;
-        if (p > i && p < n) { unsigned long long a = buf[i], b = buf[p]; if (b < a) { buf[i] = b; buf[p] = a; } }
-      }
-      __syncthreads();
-    }
+// Ascending-only bitonic network on buf[0..n): every compare-exchange puts the minimum at the lower index, so virtual
+// +inf padding above n never moves and n need not be a power of two.  One thread per PAIR (no idle half), and every
+// stage whose partner distance is below 64 stays inside one warp's 64-element block and only needs __syncwarp: of the
+// 66 stages of a 2,048-entry sort only 15 take a block barrier.
+#define SORT_THREADS 512
+
+__device__ __forceinline__ void cmpx(unsigned long long* buf, int i, int p, int n) {
+  if (p < n) { const unsigned long long a = buf[i], b = buf[p]; if (b < a) { buf[i] = b; buf[p] = a; } }
+}
+
+// stages j = jmax .. 1 (jmax <= 32) of one 64-element block, by one warp; `mirror` makes the first stage i <-> i ^ (2 jmax - 1)
+__device__ __forceinline__ void warp_stages(unsigned long long* buf, int base, int n, int jmax, bool mirror, int lane) {
+  int j = jmax;
+  if (mirror) {
+    const int k = 2 * jmax, r = lane & (jmax - 1), blk = lane / jmax;            // pair `lane` of the 32 pairs of this block
+    const int i = base + blk * k + r, p = base + blk * k + (k - 1 - r);
+    cmpx(buf, i, p, n);
+    __syncwarp();
+    j >>= 1;
+  }
+  for (; j > 0; j >>= 1) {
+    const int i = base + 2 * lane - (lane & (j - 1));
+    cmpx(buf, i, i + j, n);
+    __syncwarp();
   }
 }
 
-// Handles the tiles whose bucket length n satisfies n_lo < n <= n_hi (others return at once); buckets longer than the
-// shared-memory capacity `scap` are sorted in place in global memory by the same network.
-__global__ void __launch_bounds__(CB) tile_sort_kernel(unsigned capacity, int scap, int n_lo, int n_hi,
+__device__ __forceinline__ void bitonic_sort(unsigned long long* buf, int n) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = SORT_THREADS / 32;
+  // k = 2 .. 64: each 64-block on its own
+  for (int base = warp * 64; base < n; base += nwarps * 64)
+    for (int k = 2; k <= 64; k <<= 1) warp_stages(buf, base, n, k >> 1, true, lane);
+  __syncthreads();
+  for (int k = 128; (k >> 1) < n; k <<= 1) {
+    const int half = k >> 1;
+    const int npairs = ((n + k - 1) / k) * half;                                  // every k-block that holds an element
+    for (int t = threadIdx.x; t < npairs; t += SORT_THREADS) {                    // mirror step: i <-> i ^ (k-1)
+      const int blk = t / half, r = t - blk * half;
+      cmpx(buf, blk * k + r, blk * k + (k - 1 - r), n);
+    }
+    __syncthreads();
+    for (int j = k >> 2; j >= 64; j >>= 1) {
+      for (int t = threadIdx.x; t * 2 < n; t += SORT_THREADS) {
+        const int i = 2 * t - (t & (j - 1));
+        cmpx(buf, i, i + j, n);
+      }
+      __syncthreads();
+    }
+    for (int base = warp * 64; base < n; base += nwarps * 64) warp_stages(buf, base, n, 32, false, lane);
+    __syncthreads();
+  }
+}
+
+__device__ __forceinline__ void sort_tile(int tile, unsigned capacity, int scap, unsigned long long* s_keys,
     const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, unsigned long long* __restrict__ lkeys,
     unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ item_tab) {
-  extern __shared__ __align__(16) unsigned long long s_keys[];
-  const int tile = blockIdx.x;
   uint2 rg = ranges[tile];
   rg.x = min(rg.x, capacity); rg.y = min(rg.y, capacity);
   const int n = (int)(rg.y - rg.x);
-  if (n <= n_lo || n > n_hi) return;
   const unsigned so = seg_off[tile];
-  for (int j = threadIdx.x; j < (n + RGA_SEG - 1) / RGA_SEG; j += CB) item_tab[so + j] = (unsigned)tile;
+  for (int j = threadIdx.x; j < (n + RGA_SEG - 1) / RGA_SEG; j += SORT_THREADS) item_tab[so + j] = (unsigned)tile;
   unsigned long long* buf = lkeys + rg.x;
   if (n <= scap) {
-    for (int i = threadIdx.x; i < n; i += CB) s_keys[i] = buf[i];
+    for (int i = threadIdx.x; i < n; i += SORT_THREADS) s_keys[i] = buf[i];
     buf = s_keys;
   }
   __syncthreads();
   bitonic_sort(buf, n);
-  for (int i = threadIdx.x; i < n; i += CB) {                // the sorted (tile, depth) keys and values (H8 output)
-    unsigned long long k = buf[i];
+  for (int i = threadIdx.x; i < n; i += SORT_THREADS) {      // the sorted (tile, depth) keys and values (H8 output)
+    const unsigned long long k = buf[i];
     keys_out[rg.x + i] = ((unsigned long long)(unsigned)tile << 32) | (k >> 32);
     vals_out[rg.x + i] = (unsigned)k;
   }
+  __syncthreads();
+}
+
+// one CTA per tile; tiles with more than SCAP_SMALL entries are left to tile_sort_long_kernel
+__global__ void __launch_bounds__(SORT_THREADS) tile_sort_kernel(unsigned capacity, int scap,
+    const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, unsigned long long* __restrict__ lkeys,
+    unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ item_tab) {
+  extern __shared__ __align__(16) unsigned long long s_keys[];
+  const uint2 rg = ranges[blockIdx.x];
+  const unsigned n = min(rg.y, capacity) - min(rg.x, capacity);
+  if (n == 0 || n > (unsigned)scap) return;
+  sort_tile(blockIdx.x, capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, item_tab);
+}
+
+// the tiles listed by tile_scan_kernel as long (usually none): persistent CTAs with the large shared-memory buffer;
+// buckets beyond it are sorted in place in global memory by the same network
+__global__ void __launch_bounds__(SORT_THREADS) tile_sort_long_kernel(unsigned capacity, int scap, const unsigned* __restrict__ num_long,
+    const unsigned* __restrict__ long_list, const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off,
+    unsigned long long* __restrict__ lkeys, unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out,
+    unsigned* __restrict__ item_tab) {
+  extern __shared__ __align__(16) unsigned long long s_keys[];
+  const unsigned nl = *num_long;
+  for (unsigned q = blockIdx.x; q < nl; q += gridDim.x)
+    sort_tile((int)long_list[q], capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, item_tab);
 }
 
 // shared-memory staging of one segment: centre, conic pre-scaled so that alpha = o * 2^(x(A x + B y) + C y^2), colour
@@ -251,20 +306,19 @@ __global__ void __launch_bounds__(CB) composite_replay_kernel(int W, int H, int 
   }
 }
 
-#define SCAP_SMALL 2048
-#define SCAP_LARGE 24576
 
 int rga_composite_init_attributes() {
-  return (int)cudaFuncSetAttribute(tile_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SCAP_LARGE * 8);
+  return (int)cudaFuncSetAttribute(tile_sort_long_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SCAP_LARGE * 8);
 }
 
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
   const int ntiles = TX * TY;
-#define SORT_ARGS(scap, lo, hi) (unsigned)av->max_dup, scap, lo, hi, av->ranges, av->seg_off, av->keys[0], av->keys[1], av->vals[0], av->item_tab
-  tile_sort_kernel<<<ntiles, CB, SCAP_SMALL * 8, s>>>(SORT_ARGS(SCAP_SMALL, 0, SCAP_SMALL));
+  tile_sort_kernel<<<ntiles, SORT_THREADS, SCAP_SMALL * 8, s>>>((unsigned)av->max_dup, SCAP_SMALL, av->ranges, av->seg_off, av->keys[0],
+                                                           av->keys[1], av->vals[0], av->item_tab);
   rga_prof_mark(av, "tile_sort", s);
-  tile_sort_kernel<<<ntiles, CB, SCAP_LARGE * 8, s>>>(SORT_ARGS(SCAP_LARGE, SCAP_SMALL, 0x7fffffff));
+  tile_sort_long_kernel<<<av->num_sms, SORT_THREADS, SCAP_LARGE * 8, s>>>((unsigned)av->max_dup, SCAP_LARGE, av->num_long, av->long_list,
+      av->ranges, av->seg_off, av->keys[0], av->keys[1], av->vals[0], av->item_tab);
   rga_prof_mark(av, "tile_sort_long", s);
   composite_segment_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
       av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, av->part, av->part_last);
