@@ -66,9 +66,15 @@ __global__ void __launch_bounds__(256) project_kernel(int ng, CamK cam, const fl
       }
     }
     mu2d[g] = mu; depth[g] = dep; conic_o[g] = co; rect[g] = rc; touched[g] = cnt;
-    // histogram of the tile digit (first pass of the (tile, depth) sort, sort_kernels.cu)
+    // histogram of the tile digit (first pass of the (tile, depth) sort, sort_kernels.cu).  Gaussians are stored in
+    // spatial order, so the lanes of a warp mostly hit the same few tiles: lanes with equal tile ids elect a leader
+    // that adds their count once (the per-address serialisation of 1,300 single atomics on a hot tile was the cost)
     for (int y = rc.y; y < rc.w; ++y)
-      for (int x = rc.x; x < rc.z; ++x) atomicAdd(tile_count + (y * cam.TX + x), 1u);
+      for (int x = rc.x; x < rc.z; ++x) {
+        const int tile = y * cam.TX + x;
+        const unsigned peers = __match_any_sync(__activemask(), tile);
+        if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(tile_count + tile, (unsigned)__popc(peers));
+      }
   }
 }
 

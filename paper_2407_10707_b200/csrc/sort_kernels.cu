@@ -74,9 +74,17 @@ __global__ void __launch_bounds__(256) tile_scatter_kernel(int ng, int TX, long 
   if (g >= ng || touched[g] == 0) return;
   int4 r = rect[g];
   unsigned long long key = ((unsigned long long)__float_as_uint(depth[g]) << 32) | (unsigned)g;
+  const unsigned lane = threadIdx.x & 31;
   for (int y = r.y; y < r.w; ++y)
     for (int x = r.x; x < r.z; ++x) {
-      unsigned pos = atomicAdd(cursor + (y * TX + x), 1u);
+      // lanes of the warp that hit the same tile take consecutive slots from ONE atomic (spatially ordered Gaussians)
+      const int tile = y * TX + x;
+      const unsigned peers = __match_any_sync(__activemask(), tile);
+      const int leader = __ffs(peers) - 1;
+      unsigned base = 0;
+      if ((int)lane == leader) base = atomicAdd(cursor + tile, (unsigned)__popc(peers));
+      base = __shfl_sync(peers, base, leader);
+      const unsigned pos = base + __popc(peers & ((1u << lane) - 1u));
       if ((long long)pos < capacity) lkeys[pos] = key;
     }
 }
