@@ -124,8 +124,16 @@ __global__ void __launch_bounds__(SORT_THREADS) tile_sort_long_kernel(unsigned c
     sort_tile((int)long_list[q], capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, item_tab);
 }
 
-// shared-memory staging of one segment: centre, conic pre-scaled so that alpha = o * 2^(x(A x + B y) + C y^2), colour
-struct SegStage { float2 mu[RGA_SEG]; float4 co[RGA_SEG]; float4 col[RGA_SEG]; };
+// Thread -> pixel of the 16x16 tile: a warp owns an 8x4 block of pixels (2 x 4 blocks per tile), so that a Gaussian
+// whose footprint misses the block is skipped by the whole warp.
+__device__ __forceinline__ int tile_px(unsigned t) { return (int)(((t >> 5) & 1u) * 8u + (t & 7u)); }
+__device__ __forceinline__ int tile_py(unsigned t) { return (int)((t >> 6) * 4u + ((t >> 3) & 3u)); }
+
+// shared-memory staging of one segment: centre, conic pre-scaled so that alpha = o * 2^(x(A x + B y) + C y^2), colour,
+// and the half-extents of the bounding box of the region where alpha can reach 1/255
+struct SegStage { float2 mu[RGA_SEG]; float4 co[RGA_SEG]; float4 col[RGA_SEG]; float2 ext[RGA_SEG]; };
+
+__device__ __forceinline__ float ex2_approx(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
 __device__ __forceinline__ void stage_segment(SegStage& st, int m, const unsigned* __restrict__ vals, const float2* __restrict__ mu2d,
                                               const float4* __restrict__ conic_o, const float4* __restrict__ color) {
@@ -135,6 +143,12 @@ __device__ __forceinline__ void stage_segment(SegStage& st, int m, const unsigne
     st.mu[threadIdx.x] = mu2d[g];
     st.co[threadIdx.x] = make_float4(-0.5f * LOG2E_F * c.x, -LOG2E_F * c.y, -0.5f * LOG2E_F * c.z, c.w);
     st.col[threadIdx.x] = color[g];
+    // alpha >= 1/255  <=>  d^T Q d <= 2 ln(255 o), Q = conic: an ellipse whose bounding box has half-extents
+    // sqrt(2 L (Q^-1)_xx), sqrt(2 L (Q^-1)_yy); padded by 0.1 % + 0.01 px against rounding (such pixels have alpha ~ 1/255)
+    const float L2 = 2.0f * __logf(255.0f * c.w), det = c.x * c.z - c.y * c.y;
+    float hx = -1.f, hy = -1.f;                                          // opacity below 1/255: never contributes
+    if (L2 > 0.f && det > 0.f) { hx = sqrtf(L2 * c.z / det) * 1.001f + 0.01f; hy = sqrtf(L2 * c.x / det) * 1.001f + 0.01f; }
+    st.ext[threadIdx.x] = make_float2(hx, hy);
   }
 }
 
@@ -143,7 +157,7 @@ __device__ __forceinline__ float seg_alpha(const SegStage& st, int j, float fx, 
   const float2 mm = st.mu[j]; const float4 co = st.co[j];
   const float dx = mm.x - fx, dy = mm.y - fy;
   const float p2 = dx * (co.x * dx + co.y * dy) + co.z * dy * dy;        // log2(e) * power
-  const float al = fminf(0.99f, co.w * exp2f(p2));
+  const float al = fminf(0.99f, co.w * ex2_approx(p2));
   return (p2 > 0.f || al < 1.f / 255.f) ? 0.f : al;
 }
 
@@ -162,29 +176,27 @@ __global__ void __launch_bounds__(CB) composite_segment_kernel(int W, int H, int
     __syncthreads();
     stage_segment(st, m, vals + b0, mu2d, conic_o, color);
     __syncthreads();
-    const int px = (int)(tile % TX) * RGA_TILE + (threadIdx.x & 15), py = (int)(tile / TX) * RGA_TILE + (threadIdx.x >> 4);
+    const int px = (int)(tile % TX) * RGA_TILE + tile_px(threadIdx.x), py = (int)(tile / TX) * RGA_TILE + tile_py(threadIdx.x);
     const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;        // DESIGN.md A21: sample at the pixel centre
     float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
     unsigned last = 0;
     bool stop = !(px < W && py < H);
-    // four entries per trip: their alphas are independent (ILP for the ex2 chain); only the blend is sequential
-    for (int j = 0; j < m && !stop; j += 4) {
-      float a[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) a[u] = (j + u < m) ? seg_alpha(st, j + u, fx, fy) : 0.f;
-      if (fmaxf(fmaxf(a[0], a[1]), fmaxf(a[2], a[3])) == 0.f) continue;
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        if (!stop && a[u] > 0.f) {
-          const float test_T = T * (1.f - a[u]);
-          // below the threshold from T = 1 means below it from any start: the resolve pass replays this segment
-          if (test_T < 1e-4f) { stop = true; T = 0.f; }
-          else {
-            const float4 c = st.col[j + u];
-            const float w = a[u] * T;
-            C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
-            T = test_T; last = (unsigned)(j + u + 1);
-          }
+    // warp-uniform cull: the centre of the warp's 8x4 pixel block against the entry's bounding box
+    const float bcx = (float)((int)(tile % TX) * RGA_TILE + tile_px(threadIdx.x & ~31u)) + 4.0f;
+    const float bcy = (float)((int)(tile / TX) * RGA_TILE + tile_py(threadIdx.x & ~31u)) + 2.0f;
+    for (int j = 0; j < m; ++j) {
+      const float2 mm = st.mu[j], ex = st.ext[j];
+      if (fabsf(mm.x - bcx) > ex.x + 3.5f || fabsf(mm.y - bcy) > ex.y + 1.5f) continue;      // pixel centres are at +-3.5, +-1.5
+      const float a = seg_alpha(st, j, fx, fy);
+      if (!stop && a > 0.f) {
+        const float test_T = T * (1.f - a);
+        // below the threshold from T = 1 means below it from any start: the resolve pass replays this segment
+        if (test_T < 1e-4f) { stop = true; T = 0.f; }
+        else {
+          const float4 c = st.col[j];
+          const float w = a * T;
+          C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+          T = test_T; last = (unsigned)(j + 1);
         }
       }
     }
@@ -215,7 +227,7 @@ __global__ void __launch_bounds__(CB) composite_resolve_kernel(int W, int H, int
   rg.x = min(rg.x, capacity); rg.y = min(rg.y, capacity);
   const int n = (int)(rg.y - rg.x), nseg = (n + RGA_SEG - 1) / RGA_SEG;
   const unsigned so = seg_off[tile];
-  const int px = blockIdx.x * RGA_TILE + (threadIdx.x & 15), py = blockIdx.y * RGA_TILE + (threadIdx.x >> 4);
+  const int px = blockIdx.x * RGA_TILE + tile_px(threadIdx.x), py = blockIdx.y * RGA_TILE + tile_py(threadIdx.x);
   if (!(px < W && py < H)) return;
   float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
   unsigned last = 0;
@@ -256,11 +268,13 @@ __global__ void __launch_bounds__(CB) composite_replay_kernel(int W, int H, int 
     const float4* __restrict__ color, float3 bg, float* __restrict__ image, float* __restrict__ t_final,
     unsigned* __restrict__ n_contrib, const int* __restrict__ stop_seg, unsigned char* __restrict__ item_flag) {
   __shared__ SegStage st;
+  __shared__ int s_cnt;
+  __shared__ unsigned short s_pix[CB];
   const unsigned n_items = *num_items;
   for (unsigned item = blockIdx.x; item < n_items; item += gridDim.x) {
     if (!item_flag[item]) continue;                        // block-uniform
     __syncthreads();
-    if (threadIdx.x == 0) item_flag[item] = 0;             // re-armed for the next frame
+    if (threadIdx.x == 0) { item_flag[item] = 0; s_cnt = 0; }   // flag re-armed for the next frame
     const unsigned tile = item_tab[item];
     const int seg = (int)(item - seg_off[tile]);
     const uint2 rg = ranges[tile];
@@ -268,23 +282,38 @@ __global__ void __launch_bounds__(CB) composite_replay_kernel(int W, int H, int 
     const int m = min(RGA_SEG, n - seg * RGA_SEG);
     stage_segment(st, m, vals + rg.x + seg * RGA_SEG, mu2d, conic_o, color);
     __syncthreads();
-    const int px = (int)(tile % TX) * RGA_TILE + (threadIdx.x & 15), py = (int)(tile / TX) * RGA_TILE + (threadIdx.x >> 4);
-    if (!(px < W && py < H)) continue;
+    // the pixels of the tile that stop in this segment are usually a minority: compact them so that whole warps
+    // either replay or leave (7 of 32 lanes were active before)
+    {
+      const int qx = (int)(tile % TX) * RGA_TILE + tile_px(threadIdx.x), qy = (int)(tile / TX) * RGA_TILE + tile_py(threadIdx.x);
+      if (qx < W && qy < H && stop_seg[(size_t)qy * W + qx] == seg) s_pix[atomicAdd(&s_cnt, 1)] = (unsigned short)threadIdx.x;
+    }
+    __syncthreads();
+    if ((int)threadIdx.x >= s_cnt) continue;
+    const unsigned q = s_pix[threadIdx.x];
+    const int px = (int)(tile % TX) * RGA_TILE + tile_px(q), py = (int)(tile / TX) * RGA_TILE + tile_py(q);
     const size_t p = (size_t)py * W + px;
-    if (stop_seg[p] != seg) continue;
     const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;
     float T = t_final[p], C0 = image[3 * p], C1 = image[3 * p + 1], C2 = image[3 * p + 2];
     unsigned last = n_contrib[p];
     bool done = false;
-    for (int j = 0; j < m; ++j) {
-      const float a = seg_alpha(st, j, fx, fy);
-      if (a > 0.f) {
-        const float test_T = T * (1.f - a);
-        if (test_T < 1e-4f) { done = true; break; }
-        const float4 c = st.col[j];
-        const float w = a * T;
-        C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
-        T = test_T; last = (unsigned)(seg * RGA_SEG + j + 1);
+    // few threads replay, so latency rules: eight independent alphas per trip, then the short sequential blend
+    for (int j0 = 0; j0 < m && !done; j0 += 8) {
+      float a[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) a[u] = (j0 + u < m) ? seg_alpha(st, j0 + u, fx, fy) : 0.f;
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        if (!done && a[u] > 0.f) {
+          const float test_T = T * (1.f - a[u]);
+          if (test_T < 1e-4f) done = true;
+          else {
+            const float4 c = st.col[j0 + u];
+            const float w = a[u] * T;
+            C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+            T = test_T; last = (unsigned)(seg * RGA_SEG + j0 + u + 1);
+          }
+        }
       }
     }
     // the fold's threshold has a 1e-5 relative guard band: a pixel inside it may not stop here after all and walks the
