@@ -408,7 +408,10 @@ __global__ void __launch_bounds__(DT_THREADS) vis_depth_test_kernel(int ng, int 
   const float bt = bias_texels / (float)R, bw = bias_world * W.inv2r;
   const float beta_lo = bt * 1.0f + bw, beta_hi = bt * slope_max + bw;
   const bool bounds_ok = bt >= 0.f && slope_max >= 1.0f;
-  const float Rm1 = (float)(R - 1);
+  const float INF = __int_as_float(0x7f800000);
+  const float blo = bounds_ok ? beta_lo : -INF, bhi = bounds_ok ? beta_hi : INF;      // no shortcut unless beta is monotone
+  const float margin = 1e-6f + 1e-5f * fabsf(bt) * fmaxf(slope_max, 1.0f);             // >> error of the approximate threshold
+  const float Rm1 = (float)(R - 1), Rf = (float)R;
   const float4 x = g_posed[g], n = g_nposed[g];
   const float dx = x.x - W.cx, dy = x.y - W.cy, dz = x.z - W.cz;
   const size_t RR = (size_t)R * R;
@@ -423,24 +426,36 @@ __global__ void __launch_bounds__(DT_THREADS) vis_depth_test_kernel(int ng, int 
       const float px = __fmaf_rn(fu.z, dz, __fmaf_rn(fu.y, dy, __fmaf_rn(fu.x, dx, W.hR)));
       const float py = __fmaf_rn(fv.z, dz, __fmaf_rn(fv.y, dy, __fmaf_rn(fv.x, dx, W.hR)));
       const float z = __fmaf_rn(fw.z, dz, __fmaf_rn(fw.y, dy, __fmaf_rn(fw.x, dx, 0.5f)));
-      // floor-then-clamp of the contract == clamp-then-truncate for every finite px
-      const int ix = __float2int_rz(fminf(fmaxf(px, 0.0f), Rm1)), iy = __float2int_rz(fminf(fmaxf(py, 0.0f), Rm1));
-      const unsigned zb = __ldg(zk + (size_t)b * RR + iy * R + ix);
-      bool vis;
-      if (zb == 0xffffffffu) vis = true;
-      else {
-        const float zm = __uint_as_float(zb);
-        if (bounds_ok && z <= zm + beta_lo) vis = true;
-        else if (bounds_ok && !(z <= zm + beta_hi)) vis = false;
+      // floor-then-clamp of the contract == clamp-then-floor for every finite px.  floor without the XU pipe: adding
+      // 2^23 rounding DOWN leaves floor(x) in the mantissa (0 <= x < 2^23); iy R + ix is then formed exactly in fp32
+      const float fxm = __fadd_rd(fminf(fmaxf(px, 0.0f), Rm1), 8388608.0f);
+      const float fym = __fadd_rd(fminf(fmaxf(py, 0.0f), Rm1), 8388608.0f);
+      const int idx = __float_as_int(__fmaf_rn(__fadd_rn(fym, -8388608.0f), Rf, fxm)) & 0x7fffff;
+      const float zm = __uint_as_float(__ldg(zk + (size_t)b * RR + idx));      // empty texel = 0xffffffff = NaN
+      // visible iff z <= zm + beta(tau); NaN compares false, so "not (z > ...)" also covers the empty texel.
+      // beta is monotone in tau in [1, slope_max]: most tests are decided by the two ends without evaluating tau.
+      bool vis = !(z > __fadd_rn(zm, blo));
+      if (!vis && !(z > __fadd_rn(zm, bhi))) {
+        // in between: an approximate tau (MUFU sqrt / rcp, ~1e-6 relative) decides unless z is within `margin` of the
+        // threshold; only then the exact IEEE sqrt and divide of the contract are evaluated -- the bit is the same
+        const float cs = __fadd_rn(__fadd_rn(__fmul_rn(n.x, fu.w), __fmul_rn(n.y, fv.w)), __fmul_rn(n.z, fw.w));
+        float tau = slope_max;
+        if (cs > 0.0f) {
+          float sq, rc; const float s2 = fmaxf(__fmaf_rn(-cs, cs, 1.0f), 0.0f);
+          asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sq) : "f"(s2));
+          asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rc) : "f"(cs));
+          tau = fminf(fmaxf(__fmul_rn(sq, rc), 1.0f), slope_max);
+        }
+        const float dlt = __fadd_rn(z, -__fadd_rn(zm, __fmaf_rn(bt, tau, bw)));
+        if (fabsf(dlt) > margin) vis = dlt < 0.0f;
         else {
-          const float cs = (n.x * fu.w + n.y * fv.w) + n.z * fw.w;
-          float tau;
+          float te = slope_max;
           if (cs > 0.0f) {
-            float s2 = fmaxf(1.0f - cs * cs, 0.0f);
-            tau = sqrtf(s2) / cs;
-            tau = fminf(fmaxf(tau, 1.0f), slope_max);
-          } else tau = slope_max;
-          vis = z <= zm + (bt * tau + bw);
+            const float s2 = fmaxf(1.0f - cs * cs, 0.0f);
+            te = sqrtf(s2) / cs;
+            te = fminf(fmaxf(te, 1.0f), slope_max);
+          }
+          vis = z <= zm + (bt * te + bw);
         }
       }
       bits |= (vis ? 1u : 0u) << b;
