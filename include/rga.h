@@ -126,6 +126,15 @@ RGA_API rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const flo
 /* H6-H10.  Needs shade_gaussians.  bg: host float[3].  out_image: dev [height][width][3] fp32, caller-owned. */
 RGA_API rga_status splat_render(rga_avatar* av, const rga_camera* cam, const float bg[3], float* out_image, void* stream);
 
+/* One whole frame: pose_skin, visibility_raster (skipped when vis == NULL, which needs
+ * env->use_visibility == 0), shade_gaussians and splat_render with the same arguments, results and intermediates as the
+ * four calls above.  Enqueue-only like them.  The steps that depend neither on visibility nor on shading (H6-H9 and
+ * the environment table) are issued on a second stream owned by the avatar and joined before the blend, so `stream`
+ * observes the whole frame in order; the call can be captured into a CUDA graph. */
+RGA_API rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, const rga_vis_params* vis, const rga_env* env,
+                                    const float cam_pos[3], const rga_camera* cam, const float bg[3], float* out_image,
+                                    void* stream);
+
 /* Intermediates (parity tests, debugging).  Layouts are documented next to each id. */
 typedef enum {
   RGA_BUF_KNN_G = 0,          /* i32 [n_gauss][k_g]                                  */

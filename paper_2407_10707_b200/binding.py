@@ -76,6 +76,8 @@ def lib():
         L.visibility_raster.argtypes = [C.c_void_p, C.POINTER(_VisParams), C.c_void_p]
         L.shade_gaussians.argtypes = [C.c_void_p, C.POINTER(_Env), C.POINTER(C.c_float), C.c_void_p]
         L.splat_render.argtypes = [C.c_void_p, C.POINTER(_Camera), C.POINTER(C.c_float), C.c_void_p, C.c_void_p]
+        L.rga_render_frame.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_VisParams), C.POINTER(_Env), C.POINTER(C.c_float),
+                                       C.POINTER(_Camera), C.POINTER(C.c_float), C.c_void_p, C.c_void_p]
         L.rga_get_buffer.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
         L.rga_read_buffer.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
         L.rga_check.argtypes = [C.c_void_p, C.c_void_p]
@@ -168,6 +170,21 @@ def splat_render(h, camera, bg, out_image):
     _chk(lib().splat_render(h, C.byref(cam), b, _ptr(out_image), _stream()))
 
 
+def rga_render_frame(h, bone_mats, dirs, vis_res, radiance, texel_to_dir, cam_pos, camera, bg, out_image, vis_mode=0,
+                     use_visibility=True, gamma=2.2, bias=(1.0, 0.015, 8.0), keep_maps=False):
+    """One whole frame in one C-ABI call (include/rga.h rga_render_frame)."""
+    e = _Env(int(radiance.shape[0]), int(radiance.shape[1]), radiance.data_ptr(),
+             0 if texel_to_dir is None else texel_to_dir.data_ptr(), gamma, int(use_visibility))
+    cp = (C.c_float * 3)(*[float(v) for v in cam_pos])
+    cam = camera if isinstance(camera, _Camera) else make_camera(camera)
+    b = (C.c_float * 3)(*[float(v) for v in bg])
+    vp = None
+    if use_visibility:
+        vp = C.byref(_VisParams(int(dirs.shape[0]), int(vis_res), int(vis_mode), dirs.data_ptr(), bias[0], bias[1], bias[2],
+                                int(keep_maps)))
+    _chk(lib().rga_render_frame(h, _ptr(bone_mats), vp, C.byref(e), cp, C.byref(cam), b, _ptr(out_image), _stream()))
+
+
 def rga_check(h):
     _chk(lib().rga_check(h, _stream()))
 
@@ -221,12 +238,9 @@ class Avatar:
 
     def render(self, bone_mats, dirs, vis_res, radiance, texel_to_dir, cam_pos, camera, bg, out_image, vis_mode=0,
                use_visibility=True, gamma=2.2, bias=(1.0, 0.015, 8.0)):
-        """One relit posed frame: the four per-frame C-ABI calls in the paper's order."""
-        pose_skin(self.h, bone_mats)
-        if use_visibility:
-            visibility_raster(self.h, dirs, vis_res, vis_mode, bias[0], bias[1], bias[2])
-        shade_gaussians(self.h, radiance, cam_pos, texel_to_dir, gamma, use_visibility)
-        splat_render(self.h, camera, bg, out_image)
+        """One relit posed frame through rga_render_frame."""
+        rga_render_frame(self.h, bone_mats, dirs, vis_res, radiance, texel_to_dir, cam_pos, camera, bg, out_image, vis_mode,
+                         use_visibility, gamma, bias)
         return out_image
 
     def read(self, which):

@@ -62,6 +62,10 @@ extern "C" rga_status avatar_free(rga_avatar* av) {
                   av->status};
   for (void* p : ptrs) if (p) cudaFree(p);
   for (int i = 0; i < RGA_MAX_PROF; ++i) if (av->prof_ev[i]) cudaEventDestroy(av->prof_ev[i]);
+  if (av->side) cudaStreamDestroy(av->side);
+  if (av->ev_fork) cudaEventDestroy(av->ev_fork);
+  if (av->ev_env) cudaEventDestroy(av->ev_env);
+  if (av->ev_join) cudaEventDestroy(av->ev_join);
   delete av;
   return RGA_OK;
 }
@@ -125,6 +129,9 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->stop_seg, npix)); A(dalloc(&av->item_flag, (size_t)av->items_cap));
   A(cudaMemsetAsync(av->item_flag, 0, (size_t)av->items_cap, s));
   A(dalloc(&av->t_final, npix)); A(dalloc(&av->n_contrib, npix)); A(dalloc(&av->status, 1));
+  A(cudaStreamCreateWithFlags(&av->side, cudaStreamNonBlocking));
+  A(cudaEventCreateWithFlags(&av->ev_fork, cudaEventDisableTiming)); A(cudaEventCreateWithFlags(&av->ev_env, cudaEventDisableTiming));
+  A(cudaEventCreateWithFlags(&av->ev_join, cudaEventDisableTiming));
   A(cudaMemsetAsync(av->status, 0, sizeof(int), s)); A(cudaMemsetAsync(av->num_dup, 0, sizeof(unsigned), s));
   {
     unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
@@ -204,6 +211,58 @@ extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const 
   rga_prof_mark(av, "-", s);
   CU(rga_launch_project(av, cam, s));
   CU(rga_launch_bin(av, TX, ntiles, s));
+  CU(rga_launch_tile_sort(av, cam, s));
+  CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), out_image, s));
+  av->cam_w = cam->width; av->cam_h = cam->height;
+  av->have_splat = 1;
+  return RGA_OK;
+}
+
+// One whole frame.  Same kernels as the four calls above, but the splat preparation (H6 projection, H7 binning, H8 sort,
+// H9 ranges) and the environment table do not depend on visibility or shading, so they run on the avatar's second stream
+// beside H3-H5 and join before the blend (fork / join by events: still CUDA-graph-capturable).
+extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, const rga_vis_params* vis, const rga_env* env,
+                                       const float cam_pos[3], const rga_camera* cam, const float bg[3], float* out_image,
+                                       void* stream) {
+  if (!av || !bone_mats || !env || !env->radiance || !cam_pos || !cam || !bg || !out_image)
+    return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: null argument");
+  if (env->use_visibility && !vis) return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: use_visibility needs vis params");
+  if (vis && (!vis->dirs || vis->n_dirs < 1 || vis->n_dirs > av->max_dirs || vis->res < 1 || vis->res > av->max_res ||
+              (vis->mode != 0 && vis->mode != 1)))
+    return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: n_dirs/res/mode out of range");
+  if (env->rows < 1 || env->cols < 1 || env->rows * env->cols > av->max_env || !(env->gamma > 0.f))
+    return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: env size/gamma out of range");
+  if (env->use_visibility && !env->texel_to_dir && env->rows * env->cols != vis->n_dirs)
+    return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: identity texel_to_dir needs rows*cols == n_dirs");
+  if (cam->width < 1 || cam->height < 1 || cam->width > av->max_w || cam->height > av->max_h)
+    return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: camera larger than max_width/max_height");
+  cudaStream_t s = (cudaStream_t)stream;
+  const bool overlap = !av->prof_on;                       // per-kernel events need one stream
+  cudaStream_t s2 = overlap ? av->side : s;
+  const int TX = (cam->width + 15) / 16, TY = (cam->height + 15) / 16, ntiles = TX * TY;
+  av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
+  rga_prof_mark(av, "-", s);
+  CU(rga_launch_skin(av, bone_mats, s));
+  av->have_skin = 1;
+  if (overlap) { CU(cudaEventRecord(av->ev_fork, s)); CU(cudaStreamWaitEvent(s2, av->ev_fork, 0)); }
+  CU(rga_launch_env_table(av, env, s2));
+  if (overlap) CU(cudaEventRecord(av->ev_env, s2));
+  CU(rga_launch_project(av, cam, s2));
+  CU(rga_launch_bin(av, TX, ntiles, s2));
+  CU(rga_launch_tile_sort(av, cam, s2));
+  if (overlap) CU(cudaEventRecord(av->ev_join, s2));
+  if (vis) {
+    CU(rga_launch_vis_raster(av, vis, s));
+    if (vis->mode == 0) CU(rga_launch_vis_depth_test(av, vis, s));
+    else CU(rga_launch_vis_paper(av, vis, s));
+    av->vis_mode = vis->mode; av->vis_dirs = vis->n_dirs; av->vis_res = vis->res; av->vis_words = (vis->n_dirs + 31) / 32;
+    av->keep_maps = vis->keep_maps || vis->mode == 1;
+    av->have_vis = 1;
+  }
+  if (overlap) CU(cudaStreamWaitEvent(s, av->ev_env, 0));
+  CU(rga_launch_shade(av, env, make_float3(cam_pos[0], cam_pos[1], cam_pos[2]), env->use_visibility ? av->vis_mode : 2, s));
+  av->have_shade = 1;
+  if (overlap) CU(cudaStreamWaitEvent(s, av->ev_join, 0));
   CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
   av->have_splat = 1;

@@ -340,7 +340,8 @@ int rga_composite_init_attributes() {
   return (int)cudaFuncSetAttribute(tile_sort_long_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SCAP_LARGE * 8);
 }
 
-cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s) {
+// H8 second digit: per-tile sort of the binned keys (needs only the projection, not the shading)
+cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
   const int ntiles = TX * TY;
   tile_sort_kernel<<<ntiles, SORT_THREADS, SCAP_SMALL * 8, s>>>((unsigned)av->max_dup, SCAP_SMALL, av->ranges, av->seg_off, av->keys[0],
@@ -349,6 +350,13 @@ cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 b
   tile_sort_long_kernel<<<av->num_sms, SORT_THREADS, SCAP_LARGE * 8, s>>>((unsigned)av->max_dup, SCAP_LARGE, av->num_long, av->long_list,
       av->ranges, av->seg_off, av->keys[0], av->keys[1], av->vals[0], av->item_tab);
   rga_prof_mark(av, "tile_sort_long", s);
+  av->launches += 2;
+  return cudaGetLastError();
+}
+
+// H10: blend (needs the sorted lists and the shaded colours)
+cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s) {
+  const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
   composite_segment_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
       av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, av->part, av->part_last);
   rga_prof_mark(av, "composite_segments", s);
@@ -358,6 +366,6 @@ cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 b
   composite_replay_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
       av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
   rga_prof_mark(av, "composite_replay", s);
-  av->launches += 5;
+  av->launches += 3;
   return cudaGetLastError();
 }

@@ -73,6 +73,9 @@ struct rga_avatar {
   int vis_mode, vis_dirs, vis_res, vis_words, keep_maps;
   int cam_w, cam_h;
   long long launches;
+  // rga_render_frame: the splat preparation (H6-H9) runs on a second stream beside visibility and shading
+  cudaStream_t side;
+  cudaEvent_t ev_fork, ev_env, ev_join;
   // optional per-kernel timing (rga_profile_enable): an event after every kernel, one at every API entry
   int prof_on, prof_n;
   cudaEvent_t prof_ev[RGA_MAX_PROF];
@@ -99,5 +102,6 @@ cudaError_t rga_launch_shade(rga_avatar* av, const rga_env* env, float3 cam, int
 // splat_kernels.cu
 cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream_t s);
 cudaError_t rga_launch_bin(rga_avatar* av, int TX, int ntiles, cudaStream_t s);
+cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStream_t s);
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s);
 int rga_init_kernel_attributes();

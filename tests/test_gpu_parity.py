@@ -109,3 +109,41 @@ def test_edge_cases_state_capacity_and_args():
     assert int(av.read("NUM_DUPLICATES")[0]) == 0
     assert np.allclose(img.cpu().numpy(), [0.25, 0.5, 0.75])
     av.close()
+
+
+def test_render_frame_equals_the_four_calls():
+    # rga_render_frame overlaps H6-H9 with H3-H5 on a second stream: same kernels, so every output must be identical
+    import torch
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import run_gpu
+    inp = workloads.make(1, n_gauss=30_000)
+    av, img4 = run_gpu(inp, vis_mode=0, keep_maps=False)
+    keys4, vis4, col4 = av.read("KEYS_SORTED"), av.read("VISBITS"), av.read("COLOR")
+    cam = inp["camera"]
+    img = torch.empty((cam["height"], cam["width"], 3), dtype=torch.float32, device="cuda")
+    bias = (inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
+    for _ in range(3):                                              # repeated frames reuse the scratch and the flags
+        av.render(torch.as_tensor(inp["bone_mats"][0]).cuda(), torch.as_tensor(inp["vis_dirs"]).cuda(), inp["vis_res"],
+                  torch.as_tensor(inp["env"][0]).cuda(), torch.as_tensor(inp["texel_to_dir"]).cuda(), inp["cam_pos"], cam,
+                  inp["bg"], img, vis_mode=0, gamma=inp["gamma"], bias=bias)
+        rga.rga_check(av.h)
+        assert np.array_equal(av.read("KEYS_SORTED"), keys4) and np.array_equal(av.read("VISBITS"), vis4)
+        assert np.array_equal(av.read("COLOR"), col4)
+        assert np.array_equal(img.cpu().numpy(), img4)
+    # the same call inside a CUDA graph (fork / join on the avatar's second stream is capturable)
+    bones = torch.as_tensor(inp["bone_mats"][0]).cuda(); dirs = torch.as_tensor(inp["vis_dirs"]).cuda()
+    env = torch.as_tensor(inp["env"][0]).cuda(); t2d = torch.as_tensor(inp["texel_to_dir"]).cuda()
+    img.zero_()
+    g = torch.cuda.CUDAGraph()
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(g, stream=st):
+            av.render(bones, dirs, inp["vis_res"], env, t2d, inp["cam_pos"], cam, inp["bg"], img, vis_mode=0,
+                      gamma=inp["gamma"], bias=bias)
+    torch.cuda.current_stream().wait_stream(st)
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(img.cpu().numpy(), img4)
+    av.close()
