@@ -27,6 +27,10 @@ METRIC = "relit posed frames/sec (100k Gaussians, 512x512)"
 WORKLOAD = "configs[1] SMPL-sized: 6,890 v / 13,776 f / 24 bones, 100k Gaussians, 16x32 env, 512 dirs @128^2, 512x512"
 # algorithmic work per unit of each kernel (fp32 flop, FMA = 2)
 FLOP_PER_UNIT = {"shade": 70.0, "vis_depth_test": 40.0, "vis_raster": 220.0, "composite_segments": 30.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
+NCU_DRAM_BYTES = {"vis_raster": 256768 + 4864, "vis_depth_test": 13870592, "shade": 9590272, "composite_segments": 2549504}
+NCU_SOURCE = {"vis_raster": "profiles/r01c_raster.md", "vis_depth_test": "profiles/r01f_depth_test.md",
+              "shade": "profiles/r01a_ncu_full.md", "composite_segments": "profiles/r01e_splat.md"}
 FP32_PEAK_TFLOPS = 2 * 128 * 148 * 1.965e9 / 1e12          # 74.4: 148 SMs x 128 FP32 lanes x FMA x 1.965 GHz (guide)
 
 
@@ -204,7 +208,7 @@ def main():
     ach = units[dom] * FLOP_PER_UNIT[dom] / (kern_ms[dom] * 1e-3) / 1e12
     pk, pk_kind = peaks()
     roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": ach / FP32_PEAK_TFLOPS, "traffic": None,
+                "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES.get(dom), "traffic_source": NCU_SOURCE.get(dom),
                 "note": "fp32 FMA-pipe peak derived from the guide (148 SM x 128 lanes x 2 x 1.965 GHz); "
                         "HBM peak %s %.0f GB/s is not the bound of this kernel" % (pk_kind, pk["hbm_gbs"]),
                 "units_per_launch": units[dom], "flop_per_unit": FLOP_PER_UNIT[dom], "kernel_ms": kern_ms[dom]}

@@ -38,14 +38,22 @@ def test_cfg1_smpl_sized_full_parity(vis_mode):
     print(rep)
 
 
-def test_cfg2_highres_reduced_gaussians():
-    # configs[2] structure (27.5k-vertex body, 32x64 env on 16x32 directions, 256^2 maps in 2 bands, 1024^2 image)
-    rep = _both(2, 0, n_gauss=60_000)
+def test_cfg2_highres_full_size():
+    # configs[2] at full size: 27.5k-vertex body, 300k Gaussians, 32x64 env on 16x32 directions, 256^2 maps in bands,
+    # 1024^2 image
+    rep = _both(2, 0)
     print(rep)
 
 
-def test_cfg4_stress_reduced_gaussians_paper_mode():
-    # configs[4] structure (1,024 directions at 256^2, 1920x1080 with ragged 68th tile row) in paper mode
+def test_cfg4_stress_full_size():
+    # configs[4] at full size: 1M Gaussians, 1,024 directions at 256^2, 1920x1080 with a ragged 68th tile row; tiles with
+    # more than 2,048 entries take the long-sort kernel
+    rep = _both(4, 0)
+    print(rep)
+
+
+def test_cfg4_structure_paper_mode():
+    # configs[4] structure in paper mode (triangle-ID maps of 256^2 in bands, 1,024 directions) with 40k Gaussians
     rep = _both(4, 1, n_gauss=40_000)
     print(rep)
 
