@@ -155,3 +155,48 @@ def test_render_frame_equals_the_four_calls():
     torch.cuda.synchronize()
     assert np.array_equal(img.cpu().numpy(), img4)
     av.close()
+
+
+def _retarget_camera(inp, W, H):
+    cam = dict(inp["camera"])
+    fy = np.float32(0.5 * H / np.tan(np.deg2rad(20.0)))
+    cam.update(width=W, height=H, fx=fy, fy=fy, cx=np.float32(W / 2), cy=np.float32(H / 2))
+    inp["camera"] = cam
+
+
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_ragged_shapes_and_displacement(vis_mode):
+    # nothing is a multiple of anything: 777 Gaussians, 40 directions (partial last bit word), 100^2 depth maps (scalar
+    # write-out path), 5x8 environment map, 70x50 image (ragged tile row and column), non-black background, and a
+    # non-zero static displacement (reading A4)
+    from oracle import oracle as orc
+    from parity_util import compare_all, run_gpu
+    inp = workloads.make(0, n_gauss=777)
+    inp["vis_dirs"] = workloads.latlong_dirs(5, 8); inp["texel_to_dir"] = np.arange(40, dtype=np.int32)
+    inp["vis_res"] = 100
+    rs = np.random.default_rng(5)
+    inp["env"] = rs.uniform(0.0, 2.0, (1, 5, 8, 3)).astype(np.float32); inp["env_rows"], inp["env_cols"] = 5, 8
+    inp["vert_disp"] = (0.02 * rs.standard_normal(inp["vert_pos"].shape)).astype(np.float32)
+    inp["bg"] = np.array([0.1, 0.2, 0.3], np.float32)
+    _retarget_camera(inp, 70, 50)
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=vis_mode)
+    av, img = run_gpu(inp, vis_mode=vis_mode)
+    print(compare_all(inp, av, img, orc_av, o, vis_mode))
+    av.close()
+
+
+@pytest.mark.parametrize("n_gauss", [1, 12_000, 60_000])
+def test_one_tile_lists_of_every_length(n_gauss):
+    # a 16x16 image is ONE tile: its list holds every front-facing Gaussian -- 1 entry, ~6k (long-sort kernel in shared
+    # memory) and ~30k (beyond 24,576: the global-memory network); hundreds of segments fold into each pixel
+    from oracle import oracle as orc
+    from parity_util import compare_all, run_gpu
+    inp = workloads.make(0, n_gauss=n_gauss)
+    _retarget_camera(inp, 16, 16)
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=0)
+    av, img = run_gpu(inp, vis_mode=0)
+    rep = compare_all(inp, av, img, orc_av, o, 0)
+    print(rep, int(av.read("NUM_DUPLICATES")[0]))
+    av.close()
