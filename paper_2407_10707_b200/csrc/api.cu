@@ -65,6 +65,7 @@ extern "C" rga_status avatar_free(rga_avatar* av) {
   if (av->side) cudaStreamDestroy(av->side);
   if (av->ev_fork) cudaEventDestroy(av->ev_fork);
   if (av->ev_env) cudaEventDestroy(av->ev_env);
+  if (av->ev_gskin) cudaEventDestroy(av->ev_gskin);
   if (av->ev_join) cudaEventDestroy(av->ev_join);
   delete av;
   return RGA_OK;
@@ -131,6 +132,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->t_final, npix)); A(dalloc(&av->n_contrib, npix)); A(dalloc(&av->status, 1));
   A(cudaStreamCreateWithFlags(&av->side, cudaStreamNonBlocking));
   A(cudaEventCreateWithFlags(&av->ev_fork, cudaEventDisableTiming)); A(cudaEventCreateWithFlags(&av->ev_env, cudaEventDisableTiming));
+  A(cudaEventCreateWithFlags(&av->ev_gskin, cudaEventDisableTiming));
   A(cudaEventCreateWithFlags(&av->ev_join, cudaEventDisableTiming));
   A(cudaMemsetAsync(av->status, 0, sizeof(int), s)); A(cudaMemsetAsync(av->num_dup, 0, sizeof(unsigned), s));
   {
@@ -162,7 +164,7 @@ extern "C" rga_status pose_skin(rga_avatar* av, const float* bone_mats, void* st
   if (!av || !bone_mats) return fail(RGA_ERR_INVALID_ARG, "pose_skin: null argument");
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
   rga_prof_mark(av, "-", (cudaStream_t)stream);
-  CU(rga_launch_skin(av, bone_mats, (cudaStream_t)stream));
+  CU(rga_launch_skin(av, bone_mats, 0, (cudaStream_t)stream));
   av->have_skin = 1;
   return RGA_OK;
 }
@@ -242,9 +244,14 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   const int TX = (cam->width + 15) / 16, TY = (cam->height + 15) / 16, ntiles = TX * TY;
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
   rga_prof_mark(av, "-", s);
-  CU(rga_launch_skin(av, bone_mats, s));
+  if (overlap) {
+    // the rasteriser only needs the posed mesh and the window: the Gaussians are skinned on the second stream
+    CU(cudaEventRecord(av->ev_fork, s)); CU(cudaStreamWaitEvent(s2, av->ev_fork, 0));
+    CU(rga_launch_skin(av, bone_mats, 1, s));
+    CU(rga_launch_skin(av, bone_mats, 2, s2));
+    CU(cudaEventRecord(av->ev_gskin, s2));
+  } else CU(rga_launch_skin(av, bone_mats, 0, s));
   av->have_skin = 1;
-  if (overlap) { CU(cudaEventRecord(av->ev_fork, s)); CU(cudaStreamWaitEvent(s2, av->ev_fork, 0)); }
   CU(rga_launch_env_table(av, env, s2));
   if (overlap) CU(cudaEventRecord(av->ev_env, s2));
   CU(rga_launch_project(av, cam, s2));
@@ -253,13 +260,14 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   if (overlap) CU(cudaEventRecord(av->ev_join, s2));
   if (vis) {
     CU(rga_launch_vis_raster(av, vis, s));
+    if (overlap) CU(cudaStreamWaitEvent(s, av->ev_gskin, 0));
     if (vis->mode == 0) CU(rga_launch_vis_depth_test(av, vis, s));
     else CU(rga_launch_vis_paper(av, vis, s));
     av->vis_mode = vis->mode; av->vis_dirs = vis->n_dirs; av->vis_res = vis->res; av->vis_words = (vis->n_dirs + 31) / 32;
     av->keep_maps = vis->keep_maps || vis->mode == 1;
     av->have_vis = 1;
   }
-  if (overlap) CU(cudaStreamWaitEvent(s, av->ev_env, 0));
+  if (overlap) { if (!vis) CU(cudaStreamWaitEvent(s, av->ev_gskin, 0)); CU(cudaStreamWaitEvent(s, av->ev_env, 0)); }
   CU(rga_launch_shade(av, env, make_float3(cam_pos[0], cam_pos[1], cam_pos[2]), env->use_visibility ? av->vis_mode : 2, s));
   av->have_shade = 1;
   if (overlap) CU(cudaStreamWaitEvent(s, av->ev_join, 0));

@@ -75,7 +75,7 @@ struct rga_avatar {
   long long launches;
   // rga_render_frame: the splat preparation (H6-H9) runs on a second stream beside visibility and shading
   cudaStream_t side;
-  cudaEvent_t ev_fork, ev_env, ev_join;
+  cudaEvent_t ev_fork, ev_gskin, ev_env, ev_join;
   // optional per-kernel timing (rga_profile_enable): an event after every kernel, one at every API entry
   int prof_on, prof_n;
   cudaEvent_t prof_ev[RGA_MAX_PROF];
@@ -89,7 +89,7 @@ cudaError_t rga_launch_knn(const float* q, int nq, const float* v, int nv, int K
 cudaError_t rga_launch_load_verts(rga_avatar* av, const float* pos, const float* disp, const float* nrm, cudaStream_t s);
 cudaError_t rga_launch_load_gauss(rga_avatar* av, const rga_avatar_desc* d, const float* d2, cudaStream_t s);
 // skin_kernels.cu
-cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, cudaStream_t s);
+cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, int which, cudaStream_t s);
 // vis_kernels.cu
 cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
 cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);

@@ -36,7 +36,7 @@ __device__ __forceinline__ void blend(const float* __restrict__ w, int B, const 
   }
 }
 
-__global__ void __launch_bounds__(256) skin_kernel(int nv, int ng, int B, int vblocks, const float* __restrict__ bone,
+__global__ void __launch_bounds__(256) skin_kernel(int nv, int ng, int B, int vblocks, int block_base, const float* __restrict__ bone,
     const float4* __restrict__ v_xbar, const float4* __restrict__ v_n, const float* __restrict__ v_w,
     const float4* __restrict__ g_static, const float* __restrict__ g_w, const float4* __restrict__ g_quat,
     const float4* __restrict__ g_scale_op,
@@ -45,8 +45,9 @@ __global__ void __launch_bounds__(256) skin_kernel(int nv, int ng, int B, int vb
   extern __shared__ float sG[];
   for (int t = threadIdx.x; t < B * 12; t += blockDim.x) sG[t] = bone[t];
   __syncthreads();
-  const bool is_vert = blockIdx.x < vblocks;
-  int i = (is_vert ? blockIdx.x : blockIdx.x - vblocks) * blockDim.x + threadIdx.x;
+  const int blk = blockIdx.x + block_base;                 // vertex blocks first, then Gaussian blocks
+  const bool is_vert = blk < vblocks;
+  int i = (is_vert ? blk : blk - vblocks) * blockDim.x + threadIdx.x;
   int n = is_vert ? nv : ng;
   float M[12];
   float px = 0.f, py = 0.f, pz = 0.f;
@@ -118,14 +119,20 @@ __global__ void window_kernel(unsigned* aabb, float* window) {
   for (int c = 0; c < 3; ++c) { aabb[c] = 0xffffffffu; aabb[3 + c] = 0u; }
 }
 
-cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, cudaStream_t s) {
-  int vblocks = (av->n_verts + 255) / 256, gblocks = (av->n_gauss + 255) / 256;
-  skin_kernel<<<vblocks + gblocks, 256, av->n_bones * 12 * sizeof(float), s>>>(
-      av->n_verts, av->n_gauss, av->n_bones, vblocks, bone_mats, av->v_xbar, av->v_normal, av->v_skin_w, av->g_static,
+// which: 0 = mesh and Gaussians (pose_skin), 1 = mesh + window only, 2 = Gaussians only.  rga_render_frame issues 1 on
+// the main stream (the rasteriser needs nothing else) and 2 on the second stream.
+cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, int which, cudaStream_t s) {
+  const int vblocks = (av->n_verts + 255) / 256, gblocks = (av->n_gauss + 255) / 256;
+  const int base = which == 2 ? vblocks : 0, nblocks = which == 0 ? vblocks + gblocks : (which == 1 ? vblocks : gblocks);
+  skin_kernel<<<nblocks, 256, av->n_bones * 12 * sizeof(float), s>>>(
+      av->n_verts, av->n_gauss, av->n_bones, vblocks, base, bone_mats, av->v_xbar, av->v_normal, av->v_skin_w, av->g_static,
       av->g_skin_w, av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->aabb);
-  rga_prof_mark(av, "skin", s);
-  window_kernel<<<1, 1, 0, s>>>(av->aabb, av->window);
-  rga_prof_mark(av, "window", s);
-  av->launches += 2;
+  rga_prof_mark(av, which == 2 ? "skin_gauss" : (which == 1 ? "skin_mesh" : "skin"), s);
+  av->launches += 1;
+  if (which != 2) {
+    window_kernel<<<1, 1, 0, s>>>(av->aabb, av->window);
+    rga_prof_mark(av, "window", s);
+    av->launches += 1;
+  }
   return cudaGetLastError();
 }
