@@ -82,6 +82,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   if (d->max_width < 1 || d->max_height < 1 || d->max_vis_dirs < 1 || d->max_vis_res < 1 || d->max_vis_res > 256 ||
       d->max_env_texels < 1 || d->max_env_texels > 65535) return fail(RGA_ERR_INVALID_ARG, "avatar_load: bad maxima");
   if (d->n_verts >= (1 << 21)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: n_verts must be below 2^21 (packed faces)");
+  if (d->n_faces >= (1 << 24)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: n_faces must be below 2^24 (rasteriser queue entries)");
   {
     int rows = 0, th = 0;
     rga_vis_raster_smem(d->max_vis_res, 1, d->n_verts, &rows, &th);

@@ -49,11 +49,12 @@ __device__ __forceinline__ float light_project_z(float dx, float dy, float dz, c
 //   B1. warps fetch 32 triangles at a time (dynamic counter), one per lane: one 8-byte packed face, three shared-memory
 //       gathers, pixel box; triangles whose box holds no pixel centre (53 % at config 1) end there, the others are
 //       compacted into the warp's queue;
-//   B2. whenever 32 are queued, each lane writes its triangle's edge-function coefficients to the warp's table and the
-//       pixel samples of all 32 boxes are dealt out over all lanes (warp scan + head bitmask), so a sliver never idles
-//       the other lanes; a sample costs three 2-IMAD edge functions; covered samples (13 %) are compacted again;
-//   C.  whenever 32 covered samples are queued their depth is interpolated (vertex z projected on demand) and
-//       atomicMin'ed into the shared-memory map (u32 depth, or u64 depth<<32|tri).
+//   B2. whenever 32 are queued, each lane writes its triangle's edge-function coefficients to the warp's table; every
+//       box row is cut into runs of up to 4 pixel centres and the runs of all 32 boxes are dealt out over all lanes
+//       (warp scan + head bitmask), so a sliver never idles the other lanes; a lane steps three int32 edge functions
+//       along its run (3 IADD per sample); runs with a covered sample (most have none) are compacted again;
+//   C.  whenever 32 such runs are queued, the triangle's vertex depths are projected on demand and the covered samples
+//       are interpolated and atomicMin'ed into the shared-memory map (u32 depth, or u64 depth<<32|tri).
 // The finished band is written to HBM once, coalesced.  ncu on the first version (one projection per triangle corner,
 // per-lane pixel loops): 693 warp instructions per 32 triangles at 17.9 active lanes (profiles/r01a_ncu_full.md).
 // Coverage and depth follow DESIGN.md "Arithmetic contract" exactly: vertices snapped to 1/256 pixel, integer edge
@@ -77,12 +78,13 @@ cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s) {
   return cudaGetLastError();
 }
 
-// Per-warp working set in shared memory (RAST_WARP_BYTES each)
+// Per-warp working set in shared memory
 #define RAST_Q 64              // queue entries: < 32 left over + <= 32 pushed
+#define RAST_SEGW 4            // a sampling unit is a run of up to 4 pixel centres of one box row
 struct RasterWarp {
-  uint4 tab[32][4];            // round table: edge-function coefficients and box of the 32 triangles being sampled
-  uint4 q2[RAST_Q];            // covered samples waiting for depth: {triangle, pixel, float(e1), float(e2)}
-  float q2a[RAST_Q];           //   and float(area)
+  uint4 tab[4][32];            // round table (component-major: lanes read neighbouring owners without bank conflicts):
+                               // edge-function coefficients and box of the 32 triangles being sampled
+  uint4 q2[RAST_Q];            // row segments with covered samples: {triangle | mask << 24 | wide << 31, pixel, e1, e2}
   int q1[RAST_Q];              // triangles whose pixel box is not empty
 };
 
@@ -91,12 +93,12 @@ struct RasterCtx {
   const unsigned* sXY;
   const float4* v_posed; const unsigned long long* faces_packed;
   unsigned* sz32; unsigned long long* sz64;
-  WinConst W; LightFrame F;
+  const float* zf;             // shared memory: window centre (3) and the depth row of the light frame wn (3)
 };
 
 // pixel box of a triangle given its packed corners, clipped to the map and the band; returns the sample count
 __device__ __forceinline__ int tri_box(unsigned P0, unsigned P1, unsigned P2, const int R, const int row0, const int rows,
-                                       int& ia, int& ja, int& bw, bool& narrow) {
+                                       int& ia, int& ja, int& bw, int& bh, bool& narrow) {
   const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
   const int mnx = min(x0, min(x1, x2)), mxx = max(x0, max(x1, x2));
   const int mny = min(y0, min(y1, y2)), mxy = max(y0, max(y1, y2));
@@ -105,43 +107,78 @@ __device__ __forceinline__ int tri_box(unsigned P0, unsigned P1, unsigned P2, co
   ja = max((mny + 127) >> 8, row0); const int jb = min((mxy - 128) >> 8, row0 + rows - 1);
   narrow = (mxx - mnx) < 16384 && (mxy - mny) < 16384;
   bw = ib - ia + 1;
-  const int bh = jb - ja + 1;
+  bh = jb - ja + 1;
   return (bw > 0 && bh > 0) ? bw * bh : 0;
 }
 
-// C. depth of up to 32 covered samples (one per lane) and the atomicMin on the map
+template <bool WITH_ID>
+__device__ __forceinline__ void put_depth(const RasterCtx& c, int p, unsigned t, float f1, float f2, float fa, float z0, float z1,
+                                          float z2) {
+  const float t1 = f1 / fa, t2 = f2 / fa;
+  float z = (z0 + t1 * (z1 - z0)) + t2 * (z2 - z0);
+  z = fmaxf(z, 0.0f);
+  if (WITH_ID) atomicMin(c.sz64 + p, ((unsigned long long)__float_as_uint(z) << 32) | t);
+  else atomicMin(c.sz32 + p, __float_as_uint(z));
+}
+
+// C. depth of the covered samples of up to 32 row segments (one per lane) and the atomicMin on the map.  The vertex
+// depths are projected here, once per segment; e1, e2 step along the row by their x-coefficients.
 template <bool WITH_ID>
 __device__ __forceinline__ void raster_depth(const RasterCtx& c, const RasterWarp* w, int base, int n, int lane) {
   if (lane >= n) return;
   const uint4 q = w->q2[base + lane];
-  const float fa = w->q2a[base + lane];
+  const unsigned t = q.x & 0xffffffu, mask = (q.x >> 24) & 0xfu;
   int i0, i1, i2;
-  face_unpack(__ldg(c.faces_packed + q.x), i0, i1, i2);
+  face_unpack(__ldg(c.faces_packed + t), i0, i1, i2);
   const float4 a = __ldg(c.v_posed + i0), b = __ldg(c.v_posed + i1), e = __ldg(c.v_posed + i2);
-  const float z0 = light_project_z(a.x - c.W.cx, a.y - c.W.cy, a.z - c.W.cz, c.F);
-  const float z1 = light_project_z(b.x - c.W.cx, b.y - c.W.cy, b.z - c.W.cz, c.F);
-  const float z2 = light_project_z(e.x - c.W.cx, e.y - c.W.cy, e.z - c.W.cz, c.F);
-  const float t1 = __uint_as_float(q.z) / fa, t2 = __uint_as_float(q.w) / fa;
-  float z = (z0 + t1 * (z1 - z0)) + t2 * (z2 - z0);
-  z = fmaxf(z, 0.0f);
-  if (WITH_ID) atomicMin(c.sz64 + q.y, ((unsigned long long)__float_as_uint(z) << 32) | q.x);
-  else atomicMin(c.sz32 + q.y, __float_as_uint(z));
+  const unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
+  const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
+  // z = fma(wn.z, d.z, fma(wn.y, d.y, fma(wn.x, d.x, 0.5))): the frame is read from shared memory (kept in registers it
+  // cost the sampling loop 20 registers it never uses)
+  const float cx = c.zf[0], cy = c.zf[1], cz = c.zf[2], wnx = c.zf[3], wny = c.zf[4], wnz = c.zf[5];
+  const float z0 = __fmaf_rn(wnz, a.z - cz, __fmaf_rn(wny, a.y - cy, __fmaf_rn(wnx, a.x - cx, 0.5f)));
+  const float z1 = __fmaf_rn(wnz, b.z - cz, __fmaf_rn(wny, b.y - cy, __fmaf_rn(wnx, b.x - cx, 0.5f)));
+  const float z2 = __fmaf_rn(wnz, e.z - cz, __fmaf_rn(wny, e.y - cy, __fmaf_rn(wnx, e.x - cx, 0.5f)));
+  if (!(q.x >> 31)) {
+    const int area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
+    const int ax1 = -256 * (y0 - y2), ax2 = -256 * (y1 - y0);
+    const float fa = (float)area;
+    for (unsigned m = mask; m; m &= m - 1u) {                         // usually one covered sample per run
+      const int u = __ffs(m) - 1;
+      put_depth<WITH_ID>(c, (int)q.y + u, t, (float)((int)q.z + u * ax1), (float)((int)q.w + u * ax2), fa, z0, z1, z2);
+    }
+  } else {                                                          // triangle spanning >= 64 pixels: int64 edge functions
+    const int prow = (int)q.y / c.R, pcol = (int)q.y - prow * c.R;
+    const long long X0 = x0, Y0 = y0, X1 = x1, Y1 = y1, X2 = x2, Y2 = y2;
+    const long long area = (X1 - X0) * (Y2 - Y0) - (Y1 - Y0) * (X2 - X0);
+    const long long qy = 256ll * (prow + c.row0) + 128;
+    for (int u = 0; u < RAST_SEGW; ++u) {
+      if ((mask >> u) & 1u) {
+        const long long qx = 256ll * (pcol + u) + 128;
+        const long long e1 = (X0 - X2) * (qy - Y2) - (Y0 - Y2) * (qx - X2);
+        const long long e2 = (X1 - X0) * (qy - Y0) - (Y1 - Y0) * (qx - X0);
+        put_depth<WITH_ID>(c, (int)q.y + u, t, (float)e1, (float)e2, (float)area, z0, z1, z2);
+      }
+    }
+  }
 }
 
-// B2. one round: lane l owns queued triangle l (l < n); the samples of all n pixel boxes are dealt out 32 at a time.
-// Returns the new fill of the covered-sample queue.
+// B2. one round: lane l owns queued triangle l (l < n).  Every box row is cut into segments of up to RAST_SEGW pixel
+// centres; the segments of all n boxes are dealt out 32 at a time, one per lane, and a lane steps its edge functions
+// along the row.  Returns the new fill of the covered-segment queue.
 template <bool WITH_ID>
 __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, int qbase, int n, int lane, int q2n) {
   int cnt = 0;
-  uint4 r0 = make_uint4(0u, 0u, 0u, 0u), r1 = r0, r3 = r0;
-  unsigned boxw = 0u, ay2u = 0u; float invbw = 1.0f;
+  unsigned boxw = 0u, ay2u = 0u; float inv = 1.0f;
   if (lane < n) {
     const int t = w->q1[qbase + lane];
     int i0, i1, i2;
     face_unpack(__ldg(c.faces_packed + t), i0, i1, i2);
     const unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
-    int ia, ja, bw; bool narrow;
-    cnt = tri_box(P0, P1, P2, c.R, c.row0, c.rows, ia, ja, bw, narrow);
+    int ia, ja, bw, bh; bool narrow;
+    tri_box(P0, P1, P2, c.R, c.row0, c.rows, ia, ja, bw, bh, narrow);
+    const int nsr = (bw + RAST_SEGW - 1) / RAST_SEGW;                 // segments per row
+    cnt = bh * nsr;
     const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
     const int qx = 256 * ia + 128, qy = 256 * ja + 128;
     int C0 = -1, C1 = 1, C2 = 0, ax0 = 0, ax1 = 0, ax2 = 0, ay0 = 0, ay1 = 0, ay2 = 0;      // "never covered"
@@ -156,20 +193,19 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
         ay0 = 256 * (x2 - x1); ay1 = 256 * (x0 - x2); ay2 = 256 * (x1 - x0);
       }
     }
-    r0 = make_uint4((unsigned)C0, (unsigned)ax0, (unsigned)ay0, (unsigned)C1);
-    r1 = make_uint4((unsigned)ax1, (unsigned)ay1, (unsigned)C2, (unsigned)ax2);
     boxw = (unsigned)((ja - c.row0) * c.R + ia) | ((unsigned)(bw - 1) << 16) | (narrow ? (1u << 24) : 0u);
-    invbw = 1.0f / (float)bw;
-    r3 = make_uint4((unsigned)t, (unsigned)ia | ((unsigned)ja << 16), 0u, 0u);
-    w->tab[lane][0] = r0; w->tab[lane][1] = r1; w->tab[lane][3] = r3;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"((float)nsr));       // only splits an index (error analysis below)
     ay2u = (unsigned)ay2;
+    w->tab[0][lane] = make_uint4((unsigned)C0, (unsigned)ax0, (unsigned)ay0, (unsigned)C1);
+    w->tab[1][lane] = make_uint4((unsigned)ax1, (unsigned)ay1, (unsigned)C2, (unsigned)ax2);
+    w->tab[3][lane] = make_uint4((unsigned)t, (unsigned)ia | ((unsigned)ja << 16), 0u, 0u);
   }
   int inc = cnt;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
   const int exc = inc - cnt;
   const int total = __shfl_sync(0xffffffffu, inc, 31);
-  if (lane < n) w->tab[lane][2] = make_uint4(ay2u, (unsigned)exc, boxw, __float_as_uint(invbw));
+  if (lane < n) w->tab[2][lane] = make_uint4(ay2u, (unsigned)exc, boxw, __float_as_uint(inv));
   __syncwarp();
   int headbase = 0;
   for (int c0 = 0; c0 < total; c0 += 32) {
@@ -180,39 +216,47 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
     const int owner = max(headbase + __popc(H & (0xffffffffu >> (31 - lane))) - 1, 0);
     headbase += __popc(H);
     const int s = c0 + lane;
-    bool cov = false;
-    uint4 out = make_uint4(0u, 0u, 0u, 0u); float fa = 1.0f;
+    unsigned mask = 0u;
+    uint4 out = make_uint4(0u, 0u, 0u, 0u);
     if (s < total) {
-      const uint4 a = w->tab[owner][0], b = w->tab[owner][1], d = w->tab[owner][2];
-      const int li = s - (int)d.y, obw = (int)((d.z >> 16) & 0xffu) + 1;
-      const int row = (int)(((float)li + 0.5f) * __uint_as_float(d.w));   // li / obw: (li+0.5)/obw is >= 1/512 from an integer
-      const int col = li - row * obw;
-      out.y = (d.z & 0xffffu) + (unsigned)(row * c.R + col);
+      const uint4 a = w->tab[0][owner], b = w->tab[1][owner], d = w->tab[2][owner];
+      const int li = s - (int)d.y, obw = (int)((d.z >> 16) & 0xffu) + 1, nsr = (obw + RAST_SEGW - 1) / RAST_SEGW;
+      // li / nsr: (li + 0.5) / nsr is >= 1/128 away from an integer, the approximate reciprocal is within 2^-22
+      const int row = (int)(((float)li + 0.5f) * __uint_as_float(d.w));
+      const int col0 = (li - row * nsr) * RAST_SEGW, ncol = min(RAST_SEGW, obw - col0);
+      out.y = (d.z & 0xffffu) + (unsigned)(row * c.R + col0);
       if (d.z & (1u << 24)) {
-        const int e0 = (int)a.x + (int)a.y * col + (int)a.z * row;
-        const int e1 = (int)a.w + (int)b.x * col + (int)b.y * row;
-        const int e2 = (int)b.z + (int)b.w * col + (int)d.x * row;
-        cov = min(e0, min(e1, e2)) >= 0 || max(e0, max(e1, e2)) <= 0;
-        if (cov) { out.z = __float_as_uint((float)e1); out.w = __float_as_uint((float)e2); fa = (float)(e0 + e1 + e2); }
+        int e0 = (int)a.x + (int)a.y * col0 + (int)a.z * row;
+        int e1 = (int)a.w + (int)b.x * col0 + (int)b.y * row;
+        int e2 = (int)b.z + (int)b.w * col0 + (int)d.x * row;
+        out.z = (unsigned)e1; out.w = (unsigned)e2;
+#pragma unroll
+        for (int u = 0; u < RAST_SEGW; ++u) {
+          if (u < ncol && (min(e0, min(e1, e2)) >= 0 || max(e0, max(e1, e2)) <= 0)) mask |= 1u << u;
+          e0 += (int)a.y; e1 += (int)b.x; e2 += (int)b.w;
+        }
       } else {                                                        // triangle spanning >= 64 pixels: int64 edge functions
-        const uint4 e = w->tab[owner][3];
+        const uint4 e = w->tab[3][owner];
         int i0, i1, i2;
         face_unpack(__ldg(c.faces_packed + e.x), i0, i1, i2);
         const unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
         const long long x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
-        const long long qx = 256ll * ((int)(e.y & 0xffffu) + col) + 128, qy = 256ll * ((int)(e.y >> 16) + row) + 128;
-        const long long e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
-        const long long e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
-        const long long e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
-        const long long area = e0 + e1 + e2;
-        cov = ((e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0)) && area != 0;
-        if (cov) { out.z = __float_as_uint((float)e1); out.w = __float_as_uint((float)e2); fa = (float)area; }
+        const long long qy = 256ll * ((int)(e.y >> 16) + row) + 128;
+        const long long area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
+        for (int u = 0; u < ncol; ++u) {
+          const long long qx = 256ll * ((int)(e.y & 0xffffu) + col0 + u) + 128;
+          const long long e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
+          const long long e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
+          const long long e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
+          if (((e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0)) && area != 0) mask |= 1u << u;
+        }
+        out.x = 1u << 31;
       }
-      if (cov) out.x = w->tab[owner][3].x;
+      if (mask) out.x |= w->tab[3][owner].x | (mask << 24);
     }
-    const unsigned cm = __ballot_sync(0xffffffffu, cov);
+    const unsigned cm = __ballot_sync(0xffffffffu, mask != 0u);
     if (cm) {
-      if (cov) { const int slot = q2n + __popc(cm & ((1u << lane) - 1u)); w->q2[slot] = out; w->q2a[slot] = fa; }
+      if (mask) w->q2[q2n + __popc(cm & ((1u << lane) - 1u))] = out;
       q2n += __popc(cm);
       __syncwarp();
       if (q2n >= 32) { q2n -= 32; raster_depth<WITH_ID>(c, w, q2n, 32, lane); __syncwarp(); }
@@ -228,6 +272,7 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
     unsigned* __restrict__ vbits_raw, int words) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_next;
+  __shared__ float s_zf[8];
   // layout: [RasterWarp x warps][map band_rows*R*(4|8)][sXY nv*4][svert (WITH_ID)]
   const int nthreads = blockDim.x, nwarps = nthreads >> 5;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -239,14 +284,18 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
   unsigned* sXY = reinterpret_cast<unsigned*>(mp + map_bytes);
   unsigned* svert = sXY + nv;
   const int nv_words = (nv + 31) >> 5;
-  const WinConst W = make_win(window, R);
 
   for (int unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
     const int k = unit / n_bands, band = unit - k * n_bands;
     const int row0 = band * band_rows, rows = min(band_rows, R - row0);
     const int npix = rows * R;
+    {                                                       // frame and window live only through phase A
+    const WinConst W = make_win(window, R);
     const LightFrame F = make_frame(dirs + 3 * k, W);
-    if (threadIdx.x == 0) s_next = 0;
+    if (threadIdx.x == 0) {
+      s_next = 0;
+      s_zf[0] = W.cx; s_zf[1] = W.cy; s_zf[2] = W.cz; s_zf[3] = F.wn[0]; s_zf[4] = F.wn[1]; s_zf[5] = F.wn[2];
+    }
     // clear the band
     if (WITH_ID) { for (int p = threadIdx.x; p < npix; p += nthreads) sz64[p] = ~0ull; }
     else {
@@ -263,35 +312,39 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
       const int X = min(max(__float2int_rn(px * 256.0f), 0), 65535), Y = min(max(__float2int_rn(py * 256.0f), 0), 65535);
       sXY[v] = (unsigned)X | ((unsigned)Y << 16);
     }
+    }
     __syncthreads();
 
     RasterCtx c;
     c.R = R; c.row0 = row0; c.rows = rows; c.sXY = sXY; c.v_posed = v_posed; c.faces_packed = faces_packed;
-    c.sz32 = sz32; c.sz64 = sz64; c.W = W; c.F = F;
+    c.sz32 = sz32; c.sz64 = sz64; c.zf = s_zf;
     // B1. triangles: one per lane, 32 per warp fetched dynamically; non-empty boxes queued
     int qn = 0, q2n = 0;                                    // warp-uniform queue fills
     for (;;) {
-      int base = 0;
-      if (lane == 0) base = atomicAdd(&s_next, 32);
-      base = __shfl_sync(0xffffffffu, base, 0);
-      if (base >= nf) break;
-      const int t = base + lane;
-      bool ne = false;
-      if (t < nf) {
-        int i0, i1, i2;
-        face_unpack(__ldg(faces_packed + t), i0, i1, i2);
-        int ia, ja, bw; bool narrow;
-        ne = tri_box(sXY[i0], sXY[i1], sXY[i2], R, row0, rows, ia, ja, bw, narrow) > 0;
-      }
-      const unsigned m = __ballot_sync(0xffffffffu, ne);
-      if (m) {
-        if (ne) w->q1[qn + __popc(m & ((1u << lane) - 1u))] = t;
-        qn += __popc(m);
-        __syncwarp();
-        if (qn >= 32) {
-          qn -= 32;
-          q2n = raster_round<WITH_ID>(c, w, qn, 32, lane, q2n);
+      int base4 = 0;
+      if (lane == 0) base4 = atomicAdd(&s_next, 128);          // four batches per fetch
+      base4 = __shfl_sync(0xffffffffu, base4, 0);
+      if (base4 >= nf) break;
+#pragma unroll 1
+      for (int base = base4; base < min(base4 + 128, nf); base += 32) {
+        const int t = base + lane;
+        bool ne = false;
+        if (t < nf) {
+          int i0, i1, i2;
+          face_unpack(__ldg(faces_packed + t), i0, i1, i2);
+          int ia, ja, bw, bh; bool narrow;
+          ne = tri_box(sXY[i0], sXY[i1], sXY[i2], R, row0, rows, ia, ja, bw, bh, narrow) > 0;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, ne);
+        if (m) {
+          if (ne) w->q1[qn + __popc(m & ((1u << lane) - 1u))] = t;
+          qn += __popc(m);
           __syncwarp();
+          if (qn >= 32) {
+            qn -= 32;
+            q2n = raster_round<WITH_ID>(c, w, qn, 32, lane, q2n);
+            __syncwarp();
+          }
         }
       }
     }
