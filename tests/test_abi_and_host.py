@@ -82,3 +82,27 @@ def test_workload_shapes_match_baseline_configs():
     assert np.array_equal(c1["texel_to_dir"], np.arange(512))
     # deterministic
     assert np.array_equal(workloads.make(0)["gauss_pos"], c0["gauss_pos"])
+
+
+def test_argument_checks_need_no_device(built_lib):
+    # invalid arguments are rejected before any CUDA call: the status is the same with or without a GPU
+    from paper_2407_10707_b200 import binding as rga
+    lib = rga.lib()
+    assert lib.rga_render_frame(None, None, None, None, None, None, None, None, None) == rga.RGA_ERR_INVALID_ARG
+    assert lib.pose_skin(None, None, None) == rga.RGA_ERR_INVALID_ARG
+    assert lib.rga_check(None, None) == rga.RGA_ERR_INVALID_ARG
+    assert b"null" in lib.rga_last_error()
+    h = C.c_void_p()
+    d = rga._Desc(); d.n_verts = d.n_faces = d.n_bones = d.n_gauss = 4; d.k_g = 3; d.k_v = 19
+    for f in ("vert_pos", "faces", "vert_normal", "vert_skin_w", "vert_albedo", "vert_rough", "vert_spec", "gauss_pos",
+              "gauss_quat", "gauss_scale"):
+        setattr(d, f, 8)
+    d.max_width = d.max_height = d.max_vis_dirs = d.max_env_texels = 16
+    d.max_vis_res = 512                                           # snapped raster coordinates are 16-bit: R <= 256
+    assert lib.avatar_load(C.byref(d), None, C.byref(h)) == rga.RGA_ERR_INVALID_ARG and not h.value
+    d.max_vis_res = 64; d.n_verts = 1 << 21                       # three vertex indices share one 64-bit packed face
+    assert lib.avatar_load(C.byref(d), None, C.byref(h)) == rga.RGA_ERR_INVALID_ARG and b"2^21" in lib.rga_last_error()
+    d.n_verts = 60_000                                            # vertex table larger than the rasteriser's shared memory
+    assert lib.avatar_load(C.byref(d), None, C.byref(h)) == rga.RGA_ERR_INVALID_ARG
+    d.n_verts = 4; d.k_v = 4                                      # the median of Eq.3 needs an odd K_v
+    assert lib.avatar_load(C.byref(d), None, C.byref(h)) == rga.RGA_ERR_INVALID_ARG
