@@ -126,6 +126,15 @@ RGA_API rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const flo
 /* H6-H10.  Needs shade_gaussians.  bg: host float[3].  out_image: dev [height][width][3] fp32, caller-owned. */
 RGA_API rga_status splat_render(rga_avatar* av, const rga_camera* cam, const float bg[3], float* out_image, void* stream);
 
+/* Attribute maps: the same splat (H6-H10, incl. the back-face opacity kill) with the Gaussian's albedo a_g
+ * (RGA_ATTR_ALBEDO; the albedo map of PAPER.md:177 and :239) or its posed normal n_gd, signed components
+ * (RGA_ATTR_NORMAL; the normal maps behind the paper's normal-error metric) as the splatted colour.  Needs
+ * pose_skin only; no visibility, no shading.  out_image: dev [height][width][3] fp32; pixels not covered get bg. */
+#define RGA_ATTR_ALBEDO 1
+#define RGA_ATTR_NORMAL 2
+RGA_API rga_status splat_attribute(rga_avatar* av, const rga_camera* cam, const float bg[3], int which, float* out_image,
+                                   void* stream);
+
 /* One whole frame: pose_skin, visibility_raster (skipped when vis == NULL, which needs
  * env->use_visibility == 0), shade_gaussians and splat_render with the same arguments, results and intermediates as the
  * four calls above.  Enqueue-only like them.  The steps that depend neither on visibility nor on shading (H6-H9 and

@@ -76,6 +76,7 @@ def lib():
         L.visibility_raster.argtypes = [C.c_void_p, C.POINTER(_VisParams), C.c_void_p]
         L.shade_gaussians.argtypes = [C.c_void_p, C.POINTER(_Env), C.POINTER(C.c_float), C.c_void_p]
         L.splat_render.argtypes = [C.c_void_p, C.POINTER(_Camera), C.POINTER(C.c_float), C.c_void_p, C.c_void_p]
+        L.splat_attribute.argtypes = [C.c_void_p, C.POINTER(_Camera), C.POINTER(C.c_float), C.c_int, C.c_void_p, C.c_void_p]
         L.rga_render_frame.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_VisParams), C.POINTER(_Env), C.POINTER(C.c_float),
                                        C.POINTER(_Camera), C.POINTER(C.c_float), C.c_void_p, C.c_void_p]
         L.rga_get_buffer.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
@@ -168,6 +169,16 @@ def splat_render(h, camera, bg, out_image):
     cam = camera if isinstance(camera, _Camera) else make_camera(camera)
     b = (C.c_float * 3)(*[float(v) for v in bg])
     _chk(lib().splat_render(h, C.byref(cam), b, _ptr(out_image), _stream()))
+
+
+RGA_ATTR_ALBEDO, RGA_ATTR_NORMAL = 1, 2
+
+
+def splat_attribute(h, camera, bg, which, out_image):
+    """Albedo / normal map of the current pose (include/rga.h splat_attribute)."""
+    cam = camera if isinstance(camera, _Camera) else make_camera(camera)
+    b = (C.c_float * 3)(*[float(v) for v in bg])
+    _chk(lib().splat_attribute(h, C.byref(cam), b, int(which), _ptr(out_image), _stream()))
 
 
 def rga_render_frame(h, bone_mats, dirs, vis_res, radiance, texel_to_dir, cam_pos, camera, bg, out_image, vis_mode=0,

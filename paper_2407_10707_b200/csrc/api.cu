@@ -57,7 +57,7 @@ extern "C" rga_status avatar_free(rga_avatar* av) {
   void* ptrs[] = {av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
-                  av->radiance, av->color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->cursor, av->keys[0],
+                  av->radiance, av->color, av->attr_color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->cursor, av->keys[0],
                   av->keys[1], av->vals[0], av->num_dup, av->ranges, av->t_final, av->n_contrib, av->seg_off, av->num_items, av->item_tab, av->part, av->part_last, av->stop_seg, av->item_flag, av->num_long, av->long_list,
                   av->status};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -118,7 +118,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->zmap, nmap)); A(dalloc(&av->idmap, nmap)); A(dalloc(&av->visbits, ng * words));
   A(dalloc(&av->vbits_a, nv * words)); A(dalloc(&av->vbits_b, nv * words)); A(dalloc(&av->vbits_raw, nv * words));
   A(dalloc(&av->vcount, nv * (size_t)av->max_dirs + 32)); A(dalloc(&av->env_table, 8 * (size_t)av->max_env));
-  A(dalloc(&av->radiance, ng)); A(dalloc(&av->color, ng));
+  A(dalloc(&av->radiance, ng)); A(dalloc(&av->color, ng)); A(dalloc(&av->attr_color, ng));
   A(dalloc(&av->mu2d, ng)); A(dalloc(&av->depth, ng)); A(dalloc(&av->conic_o, ng)); A(dalloc(&av->rect, ng)); A(dalloc(&av->touched, ng));
   A(dalloc(&av->tile_count, ntiles)); A(dalloc(&av->cursor, ntiles));
   A(dalloc(&av->keys[0], (size_t)av->max_dup)); A(dalloc(&av->keys[1], (size_t)av->max_dup));
@@ -215,7 +215,27 @@ extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const 
   CU(rga_launch_project(av, cam, s));
   CU(rga_launch_bin(av, TX, ntiles, s));
   CU(rga_launch_tile_sort(av, cam, s));
-  CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), out_image, s));
+  CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->color, out_image, s));
+  av->cam_w = cam->width; av->cam_h = cam->height;
+  av->have_splat = 1;
+  return RGA_OK;
+}
+
+extern "C" rga_status splat_attribute(rga_avatar* av, const rga_camera* cam, const float bg[3], int which, float* out_image,
+                                      void* stream) {
+  if (!av || !cam || !bg || !out_image) return fail(RGA_ERR_INVALID_ARG, "splat_attribute: null argument");
+  if (which != RGA_ATTR_ALBEDO && which != RGA_ATTR_NORMAL) return fail(RGA_ERR_INVALID_ARG, "splat_attribute: unknown attribute %d", which);
+  if (!av->have_skin) return fail(RGA_ERR_STATE, "splat_attribute: call pose_skin first");
+  if (cam->width < 1 || cam->height < 1 || cam->width > av->max_w || cam->height > av->max_h)
+    return fail(RGA_ERR_INVALID_ARG, "splat_attribute: camera larger than max_width/max_height");
+  cudaStream_t s = (cudaStream_t)stream;
+  const int TX = (cam->width + 15) / 16, TY = (cam->height + 15) / 16, ntiles = TX * TY;
+  rga_prof_mark(av, "-", s);
+  CU(rga_launch_attr_color(av, which, s));
+  CU(rga_launch_project(av, cam, s));
+  CU(rga_launch_bin(av, TX, ntiles, s));
+  CU(rga_launch_tile_sort(av, cam, s));
+  CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->attr_color, out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
   av->have_splat = 1;
   return RGA_OK;
@@ -272,7 +292,7 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   CU(rga_launch_shade(av, env, make_float3(cam_pos[0], cam_pos[1], cam_pos[2]), env->use_visibility ? av->vis_mode : 2, s));
   av->have_shade = 1;
   if (overlap) CU(cudaStreamWaitEvent(s, av->ev_join, 0));
-  CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), out_image, s));
+  CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->color, out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
   av->have_splat = 1;
   return RGA_OK;

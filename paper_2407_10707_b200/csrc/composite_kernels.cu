@@ -340,6 +340,23 @@ int rga_composite_init_attributes() {
   return (int)cudaFuncSetAttribute(tile_sort_long_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SCAP_LARGE * 8);
 }
 
+// Attribute maps (PAPER.md:177 albedo map for editing; PAPER.md:239 albedo and normal maps for the metrics): the colour
+// that is splatted is the Gaussian's albedo a_g or its posed normal n_gd instead of the shaded colour.
+__global__ void attr_color_kernel(int ng, int which, const float4* __restrict__ g_static, const float4* __restrict__ g_nposed,
+                                  float4* __restrict__ out) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= ng) return;
+  const float4 v = which == 1 ? g_static[4 * (size_t)g + 2] : g_nposed[g];
+  out[g] = make_float4(v.x, v.y, v.z, 0.f);
+}
+
+cudaError_t rga_launch_attr_color(rga_avatar* av, int which, cudaStream_t s) {
+  attr_color_kernel<<<(av->n_gauss + 255) / 256, 256, 0, s>>>(av->n_gauss, which, av->g_static, av->g_nposed, av->attr_color);
+  rga_prof_mark(av, "attr_color", s);
+  av->launches += 1;
+  return cudaGetLastError();
+}
+
 // H8 second digit: per-tile sort of the binned keys (needs only the projection, not the shading)
 cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
@@ -355,16 +372,16 @@ cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStre
 }
 
 // H10: blend (needs the sorted lists and the shaded colours)
-cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s) {
+cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, const float4* color, float* out, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
   composite_segment_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
-      av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, av->part, av->part_last);
+      av->ranges, av->vals[0], av->mu2d, av->conic_o, color, av->part, av->part_last);
   rga_prof_mark(av, "composite_segments", s);
   composite_resolve_kernel<<<dim3(TX, TY), CB, 0, s>>>(cam->width, cam->height, TX, (unsigned)av->max_dup, av->ranges, av->seg_off,
       av->part, av->part_last, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
   rga_prof_mark(av, "composite_resolve", s);
   composite_replay_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
-      av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
+      av->ranges, av->vals[0], av->mu2d, av->conic_o, color, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
   rga_prof_mark(av, "composite_replay", s);
   av->launches += 3;
   return cudaGetLastError();

@@ -49,6 +49,7 @@ struct rga_avatar {
   // shading out
   float4* radiance;    // [n_gauss]
   float4* color;       // [n_gauss]
+  float4* attr_color;  // [n_gauss] albedo or posed normal as splat colour (splat_attribute)
   // splat
   float2* mu2d; float* depth; float4* conic_o; int4* rect; unsigned* touched;
   unsigned* tile_count; unsigned* cursor;   // [tiles] histogram of the tile digit, scatter cursors
@@ -103,5 +104,6 @@ cudaError_t rga_launch_shade(rga_avatar* av, const rga_env* env, float3 cam, int
 cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream_t s);
 cudaError_t rga_launch_bin(rga_avatar* av, int TX, int ntiles, cudaStream_t s);
 cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStream_t s);
-cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, float* out, cudaStream_t s);
+cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, const float4* color, float* out, cudaStream_t s);
+cudaError_t rga_launch_attr_color(rga_avatar* av, int which, cudaStream_t s);
 int rga_init_kernel_attributes();

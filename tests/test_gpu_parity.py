@@ -200,3 +200,52 @@ def test_one_tile_lists_of_every_length(n_gauss):
     rep = compare_all(inp, av, img, orc_av, o, 0)
     print(rep, int(av.read("NUM_DUPLICATES")[0]))
     av.close()
+
+
+def test_albedo_and_normal_maps_and_views_after_one_visibility_pass():
+    # (a) albedo / normal maps = the same splat with a_g or n_gd as colour;
+    # (b) visibility is view- and light-independent for a pose: one pose_skin + visibility_raster, then shade + splat per
+    # camera and environment map
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import IMG_MAX, IMG_MEAN
+    inp = workloads.make(1, n_gauss=30_000)
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=0)
+    cam = inp["camera"]; W, H = cam["width"], cam["height"]
+    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=512, max_vis_res=128, max_env_texels=512)
+    img = torch.empty((H, W, 3), dtype=torch.float32, device="cuda")
+    rga.pose_skin(av.h, torch.as_tensor(inp["bone_mats"][0]).cuda())
+    bg = np.array([0.5, 0.25, 0.0], np.float32)
+    for which, col in ((rga.RGA_ATTR_ALBEDO, orc_av["albedo_g"]), (rga.RGA_ATTR_NORMAL, o["gauss_normal_posed"])):
+        rga.splat_attribute(av.h, cam, bg, which, img)
+        rga.rga_check(av.h)
+        ref, _, _, fl = orc.composite(o["vals"], o["ranges"], o["mu"], o["conic_o"], col.astype(np.float64), bg, W, H)
+        assert np.array_equal(av.read("KEYS_SORTED"), o["keys"])
+        d = np.abs(img.cpu().numpy().astype(np.float64) - ref).max(-1)
+        assert d[fl == 0].max() <= IMG_MAX and d.mean() <= IMG_MEAN, (which, d[fl == 0].max(), d.mean())
+    # two cameras and two environment maps after ONE visibility pass
+    dirs = torch.as_tensor(inp["vis_dirs"]).cuda(); t2d = torch.as_tensor(inp["texel_to_dir"]).cuda()
+    rga.visibility_raster(av.h, dirs, inp["vis_res"], 0, inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
+    rs = np.random.default_rng(11)
+    for view in range(2):
+        inp2 = dict(inp)
+        if view == 1:                                                # second camera: from +x, second light
+            cp = inp["cam_pos"].astype(np.float64)
+            look = cp.copy(); look[1] = 0.0                            # the point the first camera looks at lies on its +y ray
+            dist = abs(cp[1])
+            pos = look + np.array([dist, 0.0, 0.0])
+            R_wc = np.array([[0.0, 1.0, 0.0], [0.0, 0.0, -1.0], [-1.0, 0.0, 0.0]])
+            c2 = dict(cam); c2["R_wc"] = R_wc.astype(np.float32).reshape(9); c2["t_wc"] = (-R_wc @ pos).astype(np.float32)
+            inp2["camera"] = c2; inp2["cam_pos"] = pos.astype(np.float32)
+            inp2["env"] = np.exp(rs.normal(0.0, 1.0, inp["env"].shape)).astype(np.float32)
+        ov = orc.render_frame(orc_av, inp2, vis_mode=0)
+        rga.shade_gaussians(av.h, torch.as_tensor(inp2["env"][0]).cuda(), inp2["cam_pos"], t2d, inp["gamma"], True)
+        rga.splat_render(av.h, inp2["camera"], inp["bg"], img)
+        rga.rga_check(av.h)
+        assert np.array_equal(av.read("VISBITS").reshape(len(inp["gauss_pos"]), -1), ov["visbits"])
+        assert np.array_equal(av.read("KEYS_SORTED"), ov["keys"]) and np.array_equal(av.read("VALS_SORTED"), ov["vals"])
+        d = np.abs(img.cpu().numpy().astype(np.float64) - ov["image"]).max(-1)
+        assert d[ov["flags"] == 0].max() <= IMG_MAX and d.mean() <= IMG_MEAN, (view, d[ov["flags"] == 0].max())
+    av.close()
