@@ -227,7 +227,9 @@ def main():
     dom = max((k for k in kern_ms if k in units), key=lambda k: kern_ms[k])
     ach = units[dom] * FLOP_PER_UNIT[dom] / (kern_ms[dom] * 1e-3) / 1e12
     pk, pk_kind = peaks()
+    fma_meas = rga.rga_measure_fp32_peak()
     roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "peak_fma_measured": fma_meas, "frac_of_measured": ach / fma_meas if fma_meas > 0 else None,
                 "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES.get(dom), "traffic_source": NCU_SOURCE.get(dom),
                 "note": "fp32 FMA-pipe peak derived from the guide (148 SM x 128 lanes x 2 x 1.965 GHz); "
                         "HBM peak %s %.0f GB/s is not the bound of this kernel" % (pk_kind, pk["hbm_gbs"]),

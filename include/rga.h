@@ -198,6 +198,10 @@ RGA_API int64_t rga_launch_count(const rga_avatar* av);
 RGA_API rga_status rga_profile_enable(rga_avatar* av, int on);
 RGA_API rga_status rga_profile_read(rga_avatar* av, void* stream, char* names, float* ms, int capacity, int* count);
 
+/* Measures the device's FP32 FMA throughput (register-resident FFMA chains on every SM, best of 3, ~5 ms) -- the
+ * denominator bench.py quotes beside the ALU-bound kernels.  Synchronises `stream`. */
+RGA_API rga_status rga_measure_fp32_peak(void* stream, float* tflops);
+
 RGA_API const char* rga_last_error(void);
 RGA_API const char* rga_version(void);
 

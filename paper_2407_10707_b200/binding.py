@@ -213,6 +213,14 @@ def rga_profile_read(h, capacity=96):
     return [(names.raw[32 * i:32 * i + 32].split(b"\0")[0].decode(), float(ms[i])) for i in range(n.value)]
 
 
+def rga_measure_fp32_peak():
+    """Measured FP32 FMA throughput of the current device in TFLOP/s (include/rga.h)."""
+    v = C.c_float(0)
+    lib().rga_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    _chk(lib().rga_measure_fp32_peak(_stream(), C.byref(v)))
+    return float(v.value)
+
+
 def rga_launch_count(h):
     return int(lib().rga_launch_count(h))
 

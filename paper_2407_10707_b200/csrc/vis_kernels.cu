@@ -267,6 +267,7 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
 
 template <bool WITH_ID>
 __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
+    int tail_first, int split,
     const float4* __restrict__ v_posed, const unsigned long long* __restrict__ faces_packed, const float* __restrict__ dirs,
     const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
     unsigned* __restrict__ vbits_raw, int words) {
@@ -285,7 +286,18 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
   unsigned* svert = sXY + nv;
   const int nv_words = (nv + 31) >> 5;
 
-  for (int unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+  // Work slots: units [0, tail_first) one CTA each; the units of the last, partial round of the persistent grid are cut
+  // into `split` triangle ranges so that every SM works in that round too; their CTAs merge into the (pre-cleared)
+  // global map with atomicMin.
+  const int n_slots = tail_first + (n_units - tail_first) * split;
+  for (int slot = blockIdx.x; slot < n_slots; slot += gridDim.x) {
+    int unit = slot, t_begin = 0, t_end = nf;
+    const bool shared_unit = slot >= tail_first && split > 1;
+    if (shared_unit) {
+      const int q = slot - tail_first, part = q % split;
+      unit = tail_first + q / split;
+      t_begin = (int)((long long)nf * part / split); t_end = (int)((long long)nf * (part + 1) / split);
+    }
     const int k = unit / n_bands, band = unit - k * n_bands;
     const int row0 = band * band_rows, rows = min(band_rows, R - row0);
     const int npix = rows * R;
@@ -293,7 +305,7 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
     const WinConst W = make_win(window, R);
     const LightFrame F = make_frame(dirs + 3 * k, W);
     if (threadIdx.x == 0) {
-      s_next = 0;
+      s_next = t_begin;
       s_zf[0] = W.cx; s_zf[1] = W.cy; s_zf[2] = W.cz; s_zf[3] = F.wn[0]; s_zf[4] = F.wn[1]; s_zf[5] = F.wn[2];
     }
     // clear the band
@@ -324,12 +336,12 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
       int base4 = 0;
       if (lane == 0) base4 = atomicAdd(&s_next, 128);          // four batches per fetch
       base4 = __shfl_sync(0xffffffffu, base4, 0);
-      if (base4 >= nf) break;
+      if (base4 >= t_end) break;
 #pragma unroll 1
-      for (int base = base4; base < min(base4 + 128, nf); base += 32) {
+      for (int base = base4; base < min(base4 + 128, t_end); base += 32) {
         const int t = base + lane;
         bool ne = false;
-        if (t < nf) {
+        if (t < t_end) {
           int i0, i1, i2;
           face_unpack(__ldg(faces_packed + t), i0, i1, i2);
           int ia, ja, bw, bh; bool narrow;
@@ -380,6 +392,8 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
           }
         }
       }
+    } else if (shared_unit) {
+      for (int p = threadIdx.x; p < npix; p += nthreads) { const unsigned v = sz32[p]; if (v != 0xffffffffu) atomicMin(zmap + gbase + p, v); }
     } else if ((R & 3) == 0) {
       const uint4* m4 = reinterpret_cast<const uint4*>(sz32);
       uint4* g4 = reinterpret_cast<uint4*>(zmap + gbase);
@@ -424,7 +438,17 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
   const int grid = n_units < av->num_sms ? n_units : av->num_sms;
   unsigned* raw = (with_id && p->mode == 1) ? av->vbits_raw : nullptr;
   if (raw) cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s);
-#define RAST_ARGS av->n_faces, av->n_verts, p->res, band_rows, n_bands, n_units, av->v_posed, av->faces_packed, p->dirs, av->window, \
+  // last, partial round of the persistent grid: cut its units into triangle ranges (depth-only maps merge with atomicMin)
+  int tail_first = n_units, split = 1;
+  const int rem = n_units > grid ? n_units % grid : 0;
+  if (rem > 0 && !with_id && grid / rem >= 2) {
+    split = grid / rem > 4 ? 4 : grid / rem;
+    tail_first = n_units - rem;
+    const size_t unit_px = (size_t)band_rows * p->res;       // bands are even; the last may be shorter (covered anyway)
+    const size_t first_px = (size_t)(tail_first / n_bands) * p->res * p->res + (size_t)(tail_first % n_bands) * unit_px;
+    cudaMemsetAsync(av->zmap + first_px, 0xff, ((size_t)p->n_dirs * p->res * p->res - first_px) * 4, s);
+  }
+#define RAST_ARGS av->n_faces, av->n_verts, p->res, band_rows, n_bands, n_units, tail_first, split, av->v_posed, av->faces_packed, p->dirs, av->window, \
     av->zmap, av->idmap, raw, words
   if (with_id) vis_raster_kernel<true><<<grid, threads, smem, s>>>(RAST_ARGS);
   else vis_raster_kernel<false><<<grid, threads, smem, s>>>(RAST_ARGS);
