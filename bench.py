@@ -234,6 +234,28 @@ def main():
                         "HBM peak %s %.0f GB/s is not the bound of this kernel" % (pk_kind, pk["hbm_gbs"]),
                 "units_per_launch": units[dom], "flop_per_unit": FLOP_PER_UNIT[dom], "kernel_ms": kern_ms[dom]}
 
+    # SURVEY 8(f) item 2 (beside the metric): the displacement network d(x, theta) on the tensor cores (tcgen05, TF32)
+    mlp = workloads.make_disp_mlp(seed=1)
+    mlp_d = {k: (torch.as_tensor(v).to(dev) if isinstance(v, np.ndarray) else v) for k, v in mlp.items()}
+    def run_mlp():
+        rga.displacement_mlp(av.h, mlp_d, mlp_d["theta"])
+    for _ in range(3):
+        run_mlp()
+    prof_was = rga.rga_profile_enable(av.h, True)
+    mlp_t = []
+    for _ in range(20):
+        run_mlp()
+        mlp_t += [t for name, t in rga.rga_profile_read(av.h) if name == "disp_mlp"]
+    rga.rga_profile_enable(av.h, False)
+    nvv = len(inp["vert_pos"])
+    mlp_flop = 2.0 * nvv * (2 * mlp["n_freq"] * 256 + 3 * 256 * 256 + 3 * 256)
+    mlp_ms = float(np.mean(mlp_t))
+    tf32_peak = pk.get("bf16_tflops", 1590.0) * (1.1 / 2.25)          # measured bf16 peak x the guide's nominal tf32 : bf16 ratio
+    mlp_obj = {"kernel": "disp_mlp", "bound": "tensor", "ms": mlp_ms, "achieved": mlp_flop / (mlp_ms * 1e-3) / 1e12, "peak": tf32_peak,
+               "unit": "TFLOP/s", "frac": mlp_flop / (mlp_ms * 1e-3) / 1e12 / tf32_peak, "dtype": "tf32 operands, f32 accumulate",
+               "vertices": nvv, "note": "one CTA per 128 vertices (54 CTAs at config 1), all four layers and the head fused"}
+    rga.displacement_mlp  # the static (zero) displacement of the benchmarked avatar is not restored: the avatar is closed below
+
     from paper_2407_10707_b200 import replica
     ms, ms_e2e, ms_warm = replica.max_over_ranks([ms, ms_e2e, ms_warm], device=dev)      # slowest rank sets the job time
     out = {
@@ -246,6 +268,7 @@ def main():
         "e2e": {"value": world * 1e3 / ms_e2e, "unit": "frames/s", "h2d_bytes_per_step": int(h_bones.numel() * 4 + h_env.numel() * 4),
                 "d2h_bytes_per_step": int(h_img.numel() * 4)},
         "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
+        "disp_mlp": mlp_obj,
         "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

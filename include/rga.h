@@ -126,6 +126,25 @@ RGA_API rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const flo
 /* H6-H10.  Needs shade_gaussians.  bg: host float[3].  out_image: dev [height][width][3] fp32, caller-owned. */
 RGA_API rga_status splat_render(rga_avatar* av, const rga_camera* cam, const float bg[3], float* out_image, void* stream);
 
+/* Displacement network d(x, theta): dx_i = MLP([gamma(x_i), theta]) for every canonical vertex, with
+ * gamma(x) = [sin(2 pi B x), cos(2 pi B x)] (random Fourier features, B = rff), four hidden layers of width 256 with ReLU
+ * and a linear 256 -> 3 head (readings A26-A28).  Runs on the tensor cores (tcgen05, TF32 operands, fp32
+ * accumulation); the result replaces the avatar's displacement attribute: vertices become x + dx, Gaussians x_g + Eq.1(dx),
+ * exactly as avatar_load does with a static displacement.  Call pose_skin (or rga_render_frame) afterwards.
+ * All pointers are DEVICE memory, row-major fp32; W1's columns are [sin block | cos block | theta]. */
+typedef struct {
+  int32_t n_freq;             /* F = rows of B; a multiple of 16 in [16, 128]                         */
+  int32_t n_pose;             /* length of theta (72 in the paper)                                    */
+  const float* rff;           /* dev [F][3]                                                           */
+  const float* W1;            /* dev [256][2 F + n_pose]                                              */
+  const float* b1;            /* dev [256]                                                            */
+  const float* Wh;            /* dev [3][256][256]  layers 2..4                                       */
+  const float* bh;            /* dev [3][256]                                                         */
+  const float* Wo;            /* dev [3][256]                                                         */
+  const float* bo;            /* dev [3]                                                              */
+} rga_disp_mlp;
+RGA_API rga_status displacement_mlp(rga_avatar* av, const rga_disp_mlp* mlp, const float* theta, void* stream);
+
 /* Attribute maps: the same splat (H6-H10, incl. the back-face opacity kill) with the Gaussian's albedo a_g
  * (RGA_ATTR_ALBEDO; the albedo map of PAPER.md:177 and :239) or its posed normal n_gd, signed components
  * (RGA_ATTR_NORMAL; the normal maps behind the paper's normal-error metric) as the splatted colour.  Needs
@@ -175,7 +194,8 @@ typedef enum {
   RGA_BUF_T_FINAL = 26,       /* f32 [height][width]                                 */
   RGA_BUF_N_CONTRIB = 27,     /* u32 [height][width]                                 */
   RGA_BUF_VERT_BITS_RAW = 28, /* u32 [n_verts][ceil(n_dirs/32)] raw vertex visibility (mode 1) */
-  RGA_BUF_COUNT_ = 29
+  RGA_BUF_VERT_DISP = 29,     /* f32 [n_verts][4] per-pose displacement of displacement_mlp (xyz, w unused) */
+  RGA_BUF_COUNT_ = 30
 } rga_buffer_id;
 
 /* Returns the device pointer and current size in bytes of an internal buffer (valid until the next call that

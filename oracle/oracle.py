@@ -206,6 +206,19 @@ def composite_bruteforce(depth, rect, touched, mu, conic_o, col, bg, W, H):
 K_G, K_V = 3, 19
 
 
+def disp_mlp(x, theta, m):
+    """Displacement network d(x, theta) (readings A26-A28), fp64, plain matrix products:
+    h0 = [sin(2 pi B x), cos(2 pi B x), theta]; h_l = relu(W_l h_{l-1} + b_l) for the hidden layers; dx = W_o h + b_o.
+    m: dict with rff [F,3], W1 [width, 2F+P], b1, Wh [L-1, width, width], bh [L-1, width], Wo [3, width], bo [3]."""
+    x = np.asarray(x, np.float64); theta = np.asarray(theta, np.float64)
+    p = 2.0 * np.pi * (x @ np.asarray(m["rff"], np.float64).T)
+    h = np.concatenate([np.sin(p), np.cos(p), np.broadcast_to(theta, (len(x), len(theta)))], axis=1)
+    h = np.maximum(h @ np.asarray(m["W1"], np.float64).T + np.asarray(m["b1"], np.float64), 0.0)
+    for W, b in zip(np.asarray(m["Wh"], np.float64), np.asarray(m["bh"], np.float64)):
+        h = np.maximum(h @ W.T + b, 0.0)
+    return h @ np.asarray(m["Wo"], np.float64).T + np.asarray(m["bo"], np.float64)
+
+
 def avatar_load(inp):
     """L0: KNN sets S_g, S_v and Eq.1 interpolation of the pose-independent attributes."""
     av = {}

@@ -15,12 +15,12 @@ RGA_OK, RGA_ERR_INVALID_ARG, RGA_ERR_CUDA, RGA_ERR_OOM, RGA_ERR_STATE, RGA_ERR_C
 BUF = dict(KNN_G=0, UBAR_G=1, KNN_V=2, GAUSS_STATIC=3, GAUSS_SKIN_W=4, VERT_POSED=5, VERT_NORMAL_POSED=6, GAUSS_POSED=7,
            GAUSS_NORMAL_POSED=8, GAUSS_COV=9, WINDOW=10, ZMAP=11, IDMAP=12, VISBITS=13, VCOUNT=14, RADIANCE=15, COLOR=16,
            MU2D=17, DEPTH=18, CONIC_OPACITY=19, RECT=20, TOUCHED=21, NUM_DUPLICATES=22, KEYS_SORTED=23, VALS_SORTED=24,
-           TILE_RANGES=25, T_FINAL=26, N_CONTRIB=27, VERT_BITS_RAW=28)
+           TILE_RANGES=25, T_FINAL=26, N_CONTRIB=27, VERT_BITS_RAW=28, VERT_DISP=29)
 _BUF_DTYPE = {0: np.int32, 1: np.float32, 2: np.int32, 3: np.float32, 4: np.float32, 5: np.float32, 6: np.float32,
               7: np.float32, 8: np.float32, 9: np.float32, 10: np.float32, 11: np.uint32, 12: np.int32, 13: np.uint32,
               14: np.uint8, 15: np.float32, 16: np.float32, 17: np.float32, 18: np.float32, 19: np.float32, 20: np.int32,
               21: np.uint32, 22: np.uint32, 23: np.uint64, 24: np.uint32, 25: np.uint32, 26: np.float32, 27: np.uint32,
-              28: np.uint32}
+              28: np.uint32, 29: np.float32}
 
 
 class RgaError(RuntimeError):
@@ -169,6 +169,19 @@ def splat_render(h, camera, bg, out_image):
     cam = camera if isinstance(camera, _Camera) else make_camera(camera)
     b = (C.c_float * 3)(*[float(v) for v in bg])
     _chk(lib().splat_render(h, C.byref(cam), b, _ptr(out_image), _stream()))
+
+
+class _DispMlp(C.Structure):
+    _fields_ = [("n_freq", C.c_int32), ("n_pose", C.c_int32), ("rff", C.c_void_p), ("W1", C.c_void_p), ("b1", C.c_void_p),
+                ("Wh", C.c_void_p), ("bh", C.c_void_p), ("Wo", C.c_void_p), ("bo", C.c_void_p)]
+
+
+def displacement_mlp(h, mlp, theta):
+    """d(x, theta) on the tensor cores (include/rga.h displacement_mlp).  mlp: dict of CUDA tensors rff, W1, b1, Wh, bh, Wo,
+    bo plus n_freq, n_pose; theta: CUDA tensor [n_pose]."""
+    m = _DispMlp(int(mlp["n_freq"]), int(mlp["n_pose"]), *[mlp[k].data_ptr() for k in ("rff", "W1", "b1", "Wh", "bh", "Wo", "bo")])
+    lib().displacement_mlp.argtypes = [C.c_void_p, C.POINTER(_DispMlp), C.c_void_p, C.c_void_p]
+    _chk(lib().displacement_mlp(h, C.byref(m), _ptr(theta), _stream()))
 
 
 RGA_ATTR_ALBEDO, RGA_ATTR_NORMAL = 1, 2

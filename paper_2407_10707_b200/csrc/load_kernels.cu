@@ -58,16 +58,18 @@ cudaError_t rga_launch_knn(const float* q, int nq, const float* v, int nv, int K
 }
 
 __global__ void load_verts_kernel(int n, const float* __restrict__ pos, const float* __restrict__ disp,
-                                  const float* __restrict__ nrm, float4* __restrict__ xbar, float4* __restrict__ nout) {
+                                  const float* __restrict__ nrm, float4* __restrict__ xbar, float4* __restrict__ nout,
+                                  float4* __restrict__ vpos) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   float dx = disp ? disp[3 * i] : 0.f, dy = disp ? disp[3 * i + 1] : 0.f, dz = disp ? disp[3 * i + 2] : 0.f;
   xbar[i] = make_float4(pos[3 * i] + dx, pos[3 * i + 1] + dy, pos[3 * i + 2] + dz, 0.f);
+  vpos[i] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], 0.f);
   nout[i] = make_float4(nrm[3 * i], nrm[3 * i + 1], nrm[3 * i + 2], 0.f);
 }
 
 cudaError_t rga_launch_load_verts(rga_avatar* av, const float* pos, const float* disp, const float* nrm, cudaStream_t s) {
-  load_verts_kernel<<<(av->n_verts + 255) / 256, 256, 0, s>>>(av->n_verts, pos, disp, nrm, av->v_xbar, av->v_normal);
+  load_verts_kernel<<<(av->n_verts + 255) / 256, 256, 0, s>>>(av->n_verts, pos, disp, nrm, av->v_xbar, av->v_normal, av->v_pos);
   return cudaGetLastError();
 }
 
@@ -79,7 +81,7 @@ __global__ void __launch_bounds__(128) load_gauss_kernel(int n, int K, int B, co
                                   const float* __restrict__ vw, const float* __restrict__ gquat,
                                   const float* __restrict__ gscale, const float* __restrict__ gop,
                                   float* __restrict__ ubar, float4* __restrict__ gst, float* __restrict__ gw,
-                                  float4* __restrict__ quat, float4* __restrict__ scale_op) {
+                                  float4* __restrict__ quat, float4* __restrict__ scale_op, float4* __restrict__ gpos4) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n) return;
   float u[4]; int id[4];
@@ -98,6 +100,7 @@ __global__ void __launch_bounds__(128) load_gauss_kernel(int n, int K, int B, co
   };
   float d0 = vdisp ? interp(vdisp, 3, 0) : 0.f, d1 = vdisp ? interp(vdisp, 3, 1) : 0.f, d2v = vdisp ? interp(vdisp, 3, 2) : 0.f;
   gst[4 * (size_t)g + 0] = make_float4(gpos[3 * (size_t)g] + d0, gpos[3 * (size_t)g + 1] + d1, gpos[3 * (size_t)g + 2] + d2v, 0.f);
+  gpos4[g] = make_float4(gpos[3 * (size_t)g], gpos[3 * (size_t)g + 1], gpos[3 * (size_t)g + 2], 0.f);
   float nx = interp(vnrm, 3, 0), ny = interp(vnrm, 3, 1), nz = interp(vnrm, 3, 2);
   float len = sqrtf((nx * nx + ny * ny) + nz * nz);
   if (len > 0.f) { nx = nx / len; ny = ny / len; nz = nz / len; }
@@ -113,6 +116,38 @@ cudaError_t rga_launch_load_gauss(rga_avatar* av, const rga_avatar_desc* d, cons
   load_gauss_kernel<<<(av->n_gauss + 127) / 128, 128, 0, s>>>(
       av->n_gauss, av->k_g, av->n_bones, av->knn_g, d2, d->gauss_pos, d->vert_disp, d->vert_normal, d->vert_albedo,
       d->vert_rough, d->vert_spec, d->vert_skin_w, d->gauss_quat, d->gauss_scale, d->gauss_opacity, av->ubar_g,
-      av->g_static, av->g_skin_w, av->g_quat, av->g_scale_op);
+      av->g_static, av->g_skin_w, av->g_quat, av->g_scale_op, av->g_pos);
+  return cudaGetLastError();
+}
+
+// Applies a per-pose vertex displacement (displacement_mlp): x + dx for the mesh, and Eq.1 of dx over S_g
+// for the Gaussians, in the operation order of load_gauss_kernel / DESIGN.md "Arithmetic contract".
+__global__ void __launch_bounds__(256) disp_apply_kernel(int nv, int ng, int K, const float4* __restrict__ v_pos,
+    const float4* __restrict__ v_disp, float4* __restrict__ v_xbar, const float4* __restrict__ g_pos,
+    const int* __restrict__ knn_g, const float* __restrict__ ubar_g, float4* __restrict__ g_static) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < nv) {
+    const float4 p = v_pos[i], d = v_disp[i];
+    v_xbar[i] = make_float4(p.x + d.x, p.y + d.y, p.z + d.z, 0.f);
+  } else if (i - nv < ng) {
+    const int g = i - nv;
+    float ax = 0.f, ay = 0.f, az = 0.f;
+    for (int k = 0; k < K; ++k) {
+      const float u = ubar_g[(size_t)g * K + k];
+      const float4 d = v_disp[knn_g[(size_t)g * K + k]];
+      if (k == 0) { ax = u * d.x; ay = u * d.y; az = u * d.z; }
+      else { ax = ax + u * d.x; ay = ay + u * d.y; az = az + u * d.z; }
+    }
+    const float4 p = g_pos[g];
+    g_static[4 * (size_t)g] = make_float4(p.x + ax, p.y + ay, p.z + az, 0.f);
+  }
+}
+
+cudaError_t rga_launch_disp_apply(rga_avatar* av, cudaStream_t s) {
+  const int n = av->n_verts + av->n_gauss;
+  disp_apply_kernel<<<(n + 255) / 256, 256, 0, s>>>(av->n_verts, av->n_gauss, av->k_g, av->v_pos, av->v_disp, av->v_xbar, av->g_pos,
+                                                    av->knn_g, av->ubar_g, av->g_static);
+  av->launches += 1;
+  rga_prof_mark(av, "disp_apply", s);
   return cudaGetLastError();
 }

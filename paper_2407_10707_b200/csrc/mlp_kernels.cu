@@ -1,0 +1,188 @@
+// Displacement MLP d(x, theta) ("dx = d(x, theta) ... d is a multilayer perceptron", "four
+// layers, each with a width of 256 and activated by ReLU", "Random Fourier Features"; readings A26-A28) -- the
+// one dense contraction of the method, so it runs on the 5th-generation tensor cores:
+//   tcgen05.mma kind::tf32, M = 128 vertices per CTA, N = 256 = the layer width, K = 8 per instruction, issued by one
+//   thread; A (activations) and B (weights) in shared memory in the canonical K-major no-swizzle layout (8-row x 16-byte
+//   core matrices); the fp32 accumulator (128 lanes x 256 columns) in tensor memory, read back with tcgen05.ld for the
+//   bias + ReLU epilogue, which writes the next layer's A operand straight back into shared memory.
+// All four hidden layers and the 256 -> 3 head run in one kernel: activations never leave the SM.
+// Weights stream from L2 in 256 x 32 chunks through two buffers; a chunk's buffer is released by tcgen05.commit on an
+// mbarrier.  theta is the same for every vertex, so its part of layer 1 is folded into that layer's bias per CTA.
+// FAST file: the result is compared with the fp64 oracle under the TF32 tolerance derived in DESIGN.md.
+#include "rga_internal.h"
+
+#define MLP_M 128              // vertices per CTA (UMMA M)
+#define MLP_W 256              // layer width (UMMA N)
+#define MLP_KC 32              // weight chunk along K
+#define MLP_LBO 128u           // bytes between core matrices adjacent in K
+#define MLP_SBO_A (MLP_W / 4 * 128u)    // bytes between 8-row groups of the activation tile (K up to 256)
+#define MLP_SBO_B (MLP_KC / 4 * 128u)   // ... of a weight chunk
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// shared-memory matrix descriptor (no swizzle, K-major): start >> 4, leading (K) byte offset >> 4, stride (M/N) byte
+// offset >> 4, version 1
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+  return (uint64_t)((saddr >> 4) & 0x3fffu) | ((uint64_t)((lbo >> 4) & 0x3fffu) << 16) | ((uint64_t)((sbo >> 4) & 0x3fffu) << 32) |
+         ((uint64_t)1 << 46);
+}
+
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  while (!done)
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+}
+
+// canonical K-major offset of element (row r, column k) of a tile whose 8-row groups are `sbo` bytes apart
+__device__ __forceinline__ uint32_t canon(int r, int k, uint32_t sbo) {
+  return (uint32_t)(r & 7) * 16u + (uint32_t)(r >> 3) * sbo + (uint32_t)(k >> 2) * MLP_LBO + (uint32_t)(k & 3) * 4u;
+}
+
+__global__ void __launch_bounds__(MLP_M, 1) disp_mlp_kernel(int nv, int F, int n_pose, const float4* __restrict__ v_pos,
+    const float* __restrict__ rff, const float* __restrict__ theta, const float* __restrict__ W1, const float* __restrict__ b1,
+    const float* __restrict__ Wh, const float* __restrict__ bh, const float* __restrict__ Wo, const float* __restrict__ bo,
+    float4* __restrict__ v_disp) {
+  extern __shared__ __align__(1024) unsigned char smem[];
+  unsigned char* sA = smem;                                          // 128 x 256 tf32, canonical: 128 KB
+  unsigned char* sB = smem + (size_t)MLP_M * MLP_W * 4;               // 2 x (256 x 32): 64 KB
+  float* sBias = reinterpret_cast<float*>(sB + 2 * (size_t)MLP_W * MLP_KC * 4);     // [4][256]
+  float* sWo = sBias + 4 * MLP_W;                                     // [3][256]
+  float* sRff = sWo + 3 * MLP_W;                                      // [F][3]
+  __shared__ __align__(8) unsigned long long bars[3];                 // weight buffer 0 / 1 free, accumulator ready
+  __shared__ uint32_t tmem_base_s;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int K1 = 2 * F, in1 = K1 + n_pose;
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "r"((uint32_t)MLP_W));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  if (tid == 0) {
+    for (int i = 0; i < 3; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&bars[i])), "r"(1u));
+    asm volatile("fence.mbarrier_init.release.cluster;");
+  }
+  // biases (layer 1 with the pose folded in), head weights, Fourier matrix
+  for (int n = tid; n < MLP_W; n += MLP_M) {
+    float acc = b1[n];
+    for (int j = 0; j < n_pose; ++j) acc = fmaf(W1[(size_t)n * in1 + K1 + j], theta[j], acc);
+    sBias[n] = acc;
+    for (int l = 0; l < 3; ++l) sBias[(l + 1) * MLP_W + n] = bh[l * MLP_W + n];
+    for (int c = 0; c < 3; ++c) sWo[c * MLP_W + n] = Wo[c * MLP_W + n];
+  }
+  for (int i = tid; i < 3 * F; i += MLP_M) sRff[i] = rff[i];
+  __syncthreads();
+  // layer-1 operand: gamma(x) = [sin(2 pi B x), cos(2 pi B x)] of this thread's vertex
+  const int v = blockIdx.x * MLP_M + tid;
+  {
+    float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (v < nv) x = v_pos[v];
+    for (int f = 0; f < F; ++f) {
+      const float p = fmaf(sRff[3 * f + 2], x.z, fmaf(sRff[3 * f + 1], x.y, sRff[3 * f] * x.x));
+      float sn, cs;
+      sincospif(2.0f * p, &sn, &cs);
+      *reinterpret_cast<float*>(sA + canon(tid, f, MLP_SBO_A)) = sn;
+      *reinterpret_cast<float*>(sA + canon(tid, F + f, MLP_SBO_A)) = cs;
+    }
+  }
+  const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(MLP_W >> 3) << 17) | ((uint32_t)(MLP_M >> 4) << 24);
+  uint32_t par_buf[2] = {0u, 0u}, par_acc = 0u;
+  bool pending[2] = {false, false};
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;");
+  const uint32_t tmem_base = tmem_base_s;
+  float out0 = 0.f, out1 = 0.f, out2 = 0.f;
+
+  for (int layer = 0; layer < 4; ++layer) {
+    const int Kl = layer == 0 ? K1 : MLP_W;
+    const float* Wl = layer == 0 ? W1 : Wh + (size_t)(layer - 1) * MLP_W * MLP_W;
+    const int ldw = layer == 0 ? in1 : MLP_W;
+    const int nchunks = Kl / MLP_KC;
+    for (int c = 0; c < nchunks; ++c) {
+      const int b = c & 1;
+      if (pending[b]) { mbar_wait(smem_u32(&bars[b]), par_buf[b]); par_buf[b] ^= 1u; pending[b] = false; }
+      unsigned char* buf = sB + (size_t)b * MLP_W * MLP_KC * 4;
+      // 256 rows x 32 columns of W_l, 16 bytes at a time; eight consecutive threads read 128 contiguous bytes of a row
+      for (int q = tid; q < MLP_W * MLP_KC / 4; q += MLP_M) {
+        const int n = q >> 3, kq = q & 7;
+        const float* src = Wl + (size_t)n * ldw + c * MLP_KC + 4 * kq;
+        float4 w4;
+        if ((ldw & 3) == 0) w4 = *reinterpret_cast<const float4*>(src);
+        else w4 = make_float4(src[0], src[1], src[2], src[3]);
+        *reinterpret_cast<float4*>(buf + (uint32_t)(n & 7) * 16u + (uint32_t)(n >> 3) * MLP_SBO_B + (uint32_t)kq * MLP_LBO) = w4;
+      }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic-proxy writes -> the tensor core's async proxy
+      asm volatile("tcgen05.fence::before_thread_sync;");
+      __syncthreads();
+      if (tid == 0) {
+        asm volatile("tcgen05.fence::after_thread_sync;");
+#pragma unroll
+        for (int j = 0; j < MLP_KC / 8; ++j) {
+          const uint64_t da = umma_desc(smem_u32(sA) + (uint32_t)(c * (MLP_KC / 4) + 2 * j) * MLP_LBO, MLP_LBO, MLP_SBO_A);
+          const uint64_t db = umma_desc(smem_u32(buf) + (uint32_t)(2 * j) * MLP_LBO, MLP_LBO, MLP_SBO_B);
+          const uint32_t acc = (c > 0 || j > 0) ? 1u : 0u;
+          asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                       "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                       :: "r"(tmem_base), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
+        }
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[b])) : "memory");
+        if (c == nchunks - 1)
+          asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[2])) : "memory");
+      }
+      pending[b] = true;
+    }
+    // accumulator ready: every MMA of the layer has read its operands, so sA may be overwritten
+    mbar_wait(smem_u32(&bars[2]), par_acc); par_acc ^= 1u;
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const float* bias = sBias + layer * MLP_W;
+    for (int c0 = 0; c0 < MLP_W; c0 += 32) {
+      uint32_t r[32];
+      const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)c0;
+      asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                   "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                   : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                     "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
+                     "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
+                     "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+                   : "r"(taddr) : "memory");
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      if (layer < 3) {
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) {
+          float4 h;
+          h.x = fmaxf(__uint_as_float(r[j]) + bias[c0 + j], 0.f);         h.y = fmaxf(__uint_as_float(r[j + 1]) + bias[c0 + j + 1], 0.f);
+          h.z = fmaxf(__uint_as_float(r[j + 2]) + bias[c0 + j + 2], 0.f); h.w = fmaxf(__uint_as_float(r[j + 3]) + bias[c0 + j + 3], 0.f);
+          *reinterpret_cast<float4*>(sA + canon(tid, c0 + j, MLP_SBO_A)) = h;
+        }
+      } else {                                                         // head: 256 -> 3, fp32 on the CUDA cores
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          const float h = fmaxf(__uint_as_float(r[j]) + bias[c0 + j], 0.f);
+          out0 = fmaf(sWo[c0 + j], h, out0); out1 = fmaf(sWo[MLP_W + c0 + j], h, out1); out2 = fmaf(sWo[2 * MLP_W + c0 + j], h, out2);
+        }
+      }
+    }
+    // (the next layer's first staging barrier orders these shared-memory writes and TMEM reads before its MMAs)
+  }
+  if (v < nv) v_disp[v] = make_float4(out0 + bo[0], out1 + bo[1], out2 + bo[2], 0.f);
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"((uint32_t)MLP_W));
+}
+
+size_t rga_mlp_smem(int F) {
+  return (size_t)MLP_M * MLP_W * 4 + 2 * (size_t)MLP_W * MLP_KC * 4 + (size_t)(4 + 3) * MLP_W * 4 + (size_t)3 * F * 4 + 64;
+}
+
+int rga_mlp_init_attributes() {
+  return (int)cudaFuncSetAttribute(disp_mlp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rga_mlp_smem(128));
+}
+
+cudaError_t rga_launch_disp_mlp(rga_avatar* av, const rga_disp_mlp* m, const float* theta, cudaStream_t s) {
+  const int grid = (av->n_verts + MLP_M - 1) / MLP_M;
+  disp_mlp_kernel<<<grid, MLP_M, rga_mlp_smem(m->n_freq), s>>>(av->n_verts, m->n_freq, m->n_pose, av->v_pos, m->rff, theta, m->W1, m->b1,
+                                                               m->Wh, m->bh, m->Wo, m->bo, av->v_disp);
+  av->launches += 1;
+  rga_prof_mark(av, "disp_mlp", s);
+  return cudaGetLastError();
+}

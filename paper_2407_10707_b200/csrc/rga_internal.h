@@ -17,6 +17,9 @@ struct rga_avatar {
   long long max_dup;
   int num_sms;
   // static (load-time) tables
+  float4* v_pos;       // [n_verts]  canonical x (displacement_mlp re-derives x + dx from it)
+  float4* v_disp;      // [n_verts]  per-pose displacement written by displacement_mlp
+  float4* g_pos;       // [n_gauss]  canonical x_g
   float4* v_xbar;      // [n_verts]  x + dx
   float4* v_normal;    // [n_verts]
   float* v_skin_w;     // [n_verts][B]
@@ -107,3 +110,7 @@ cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStre
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, const float4* color, float* out, cudaStream_t s);
 cudaError_t rga_launch_attr_color(rga_avatar* av, int which, cudaStream_t s);
 int rga_init_kernel_attributes();
+// mlp_kernels.cu / load_kernels.cu
+cudaError_t rga_launch_disp_mlp(rga_avatar* av, const rga_disp_mlp* m, const float* theta, cudaStream_t s);
+cudaError_t rga_launch_disp_apply(rga_avatar* av, cudaStream_t s);
+int rga_mlp_init_attributes();

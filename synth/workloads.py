@@ -204,3 +204,19 @@ def make(cfg_id, seed=None, n_gauss=None, morton=True):
     out["cam_pos"] = cam_pos.astype(np.float32)
     out["bg"] = np.zeros(3, dtype=np.float32)
     return out
+
+
+def make_disp_mlp(seed=0, n_freq=64, n_pose=72, width=256, n_hidden=4, rff_sigma=1.0, out_scale=0.01):
+    """Random weights of the displacement network d(x, theta): the trained weights are not
+    available, so these are seeded stand-ins with the architecture of DESIGN.md readings A26-A28 (He-initialised hidden
+    layers, a head scaled so that |dx| is about a centimetre) and a random pose vector theta.  Inputs only."""
+    r = _rng(seed, 7)
+    d_in = 2 * n_freq + n_pose
+    he = lambda fan_in, shape: (r.standard_normal(shape) * np.sqrt(2.0 / fan_in)).astype(np.float32)
+    return dict(
+        n_freq=n_freq, n_pose=n_pose,
+        rff=(rff_sigma * r.standard_normal((n_freq, 3))).astype(np.float32),
+        W1=he(d_in, (width, d_in)), b1=(0.1 * r.standard_normal(width)).astype(np.float32),
+        Wh=he(width, (n_hidden - 1, width, width)), bh=(0.1 * r.standard_normal((n_hidden - 1, width))).astype(np.float32),
+        Wo=(out_scale * he(width, (3, width))).astype(np.float32), bo=(0.001 * r.standard_normal(3)).astype(np.float32),
+        theta=np.deg2rad(r.uniform(-30.0, 30.0, n_pose)).astype(np.float32))

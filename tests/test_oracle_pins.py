@@ -400,3 +400,53 @@ def test_projection_matches_double_precision_ewa(cfg0, cfg0_oracle):
     facing = (o["gauss_normal_posed"] * wo).sum(1)
     assert np.all(o["touched"][facing < -1e-4] == 0)
     assert (o["touched"][facing > 1e-4] > 0).mean() > 0.99
+
+
+# --------------------------------------------------------------------------------------------- displacement network
+def _tiny_mlp(width=2, F=1, P=1):
+    z = lambda *s: np.zeros(s)
+    return dict(rff=np.array([[0.25, 0.0, 0.0]]), W1=z(width, 2 * F + P), b1=z(width), Wh=z(3, width, width), bh=z(3, width),
+                Wo=z(3, width), bo=z(3))
+
+
+def test_disp_mlp_hand_example():
+    # PAPER.md:86, :191-193 (readings A26-A28).  x = (1,0,0), B = (0.25,0,0): 2 pi B.x = pi/2, so gamma = (sin, cos) = (1, 0).
+    from oracle import oracle as orc
+    m = _tiny_mlp()
+    m["W1"][:] = [[2.0, 5.0, 3.0], [-1.0, 7.0, 0.0]]           # columns: sin, cos, theta
+    m["b1"][:] = [0.5, 0.25]                                   # h1 = relu(2*1 + 3*0.5 + 0.5, -1 + 0.25) = (4, 0)
+    for l in range(3):
+        m["Wh"][l] = np.eye(2)                                 # identity layers keep (4, 0)
+    m["bh"][2] = [1.0, -1.0]                                   # last hidden: relu(5, -1) = (5, 0)
+    m["Wo"][:] = [[1.0, 9.0], [0.5, 9.0], [-2.0, 9.0]]; m["bo"][:] = [0.0, 1.0, 2.0]
+    dx = orc.disp_mlp(np.array([[1.0, 0.0, 0.0]]), np.array([0.5]), m)
+    assert np.allclose(dx, [[5.0, 3.5, -8.0]], atol=1e-12)
+
+
+def test_disp_mlp_relu_and_affine_regime():
+    from oracle import oracle as orc
+    from synth import workloads
+    m = workloads.make_disp_mlp(seed=3)
+    m64 = {k: (np.asarray(v, np.float64) if isinstance(v, np.ndarray) else v) for k, v in m.items()}
+    x = np.random.default_rng(0).uniform(-1, 1, (50, 3))
+    # all first-layer pre-activations negative: every hidden unit is dead, dx = W_o relu(b_4 ...) is the same for all x
+    dead = dict(m64); dead["b1"] = m64["b1"] - 1e3
+    dx = orc.disp_mlp(x, m64["theta"], dead)
+    h = np.maximum(m64["bh"][0], 0.0)
+    for l in (1, 2):
+        h = np.maximum(m64["Wh"][l] @ h + m64["bh"][l], 0.0)
+    assert np.allclose(dx, np.broadcast_to(m64["Wo"] @ h + m64["bo"], dx.shape), atol=1e-12)
+    # all pre-activations positive (a large first bias, non-negative hidden weights and biases): no ReLU clips, the
+    # network is affine, dx = W_o W_4 W_3 W_2 (W_1 h0 + b1) + ... composed by hand
+    aff = dict(m64); aff["b1"] = m64["b1"] + 1e3; aff["Wh"] = np.abs(m64["Wh"]); aff["bh"] = np.abs(m64["bh"]) + 1.0
+    p = 2 * np.pi * x @ m64["rff"].T
+    h0 = np.concatenate([np.sin(p), np.cos(p), np.broadcast_to(m64["theta"], (50, 72))], 1)
+    A, c = aff["W1"], aff["b1"]
+    for l in range(3):
+        A, c = aff["Wh"][l] @ A, aff["Wh"][l] @ c + aff["bh"][l]
+    A, c = aff["Wo"] @ A, aff["Wo"] @ c + aff["bo"]
+    assert np.allclose(orc.disp_mlp(x, m64["theta"], aff), h0 @ A.T + c, rtol=1e-9, atol=1e-6)
+    # gamma(x) is 1-periodic along B's rows: shifting x by a vector v with B v integer leaves dx unchanged
+    Bm = np.zeros_like(m64["rff"]); Bm[:, 0] = np.arange(1, 65)            # integer frequencies along x
+    per = dict(m64); per["rff"] = Bm
+    assert np.allclose(orc.disp_mlp(x, m64["theta"], per), orc.disp_mlp(x + np.array([1.0, 0.3, -2.0]), m64["theta"], per), atol=1e-9)
