@@ -55,7 +55,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->v_pos, av->v_disp, av->g_pos, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
+  void* ptrs[] = {av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
                   av->radiance, av->color, av->attr_color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->cursor, av->keys[0],
@@ -111,7 +111,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   float* d2 = nullptr;
 #define A(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, \
     "avatar_load: %s: %s", #call, cudaGetErrorString(e_)); goto done; } } while (0)
-  A(dalloc(&av->v_pos, nv)); A(dalloc(&av->v_disp, nv)); A(dalloc(&av->g_pos, ng));
+  A(dalloc(&av->v_pos, nv)); A(dalloc(&av->v_disp, nv)); A(dalloc(&av->g_pos, ng)); A(dalloc(&av->mlp_bias1, 256));
   A(dalloc(&av->v_xbar, nv)); A(dalloc(&av->v_normal, nv)); A(dalloc(&av->v_skin_w, nv * B)); A(dalloc(&av->faces, 3 * (size_t)av->n_faces)); A(dalloc(&av->faces_packed, (size_t)av->n_faces));
   A(dalloc(&av->knn_v, nv * av->k_v)); A(dalloc(&av->knn_g, ng * av->k_g)); A(dalloc(&av->ubar_g, ng * av->k_g));
   A(dalloc(&av->g_static, 4 * ng)); A(dalloc(&av->g_skin_w, ng * B)); A(dalloc(&av->g_quat, ng)); A(dalloc(&av->g_scale_op, ng));
@@ -228,6 +228,7 @@ extern "C" rga_status displacement_mlp(rga_avatar* av, const rga_disp_mlp* mlp, 
     return fail(RGA_ERR_INVALID_ARG, "displacement_mlp: null argument");
   if (mlp->n_freq < 16 || mlp->n_freq > 128 || (mlp->n_freq & 15) || mlp->n_pose < 0 || mlp->n_pose > 1024)
     return fail(RGA_ERR_INVALID_ARG, "displacement_mlp: n_freq must be a multiple of 16 in [16,128], n_pose in [0,1024]");
+  if (mlp->n_pose & 3) return fail(RGA_ERR_INVALID_ARG, "displacement_mlp: n_pose must be a multiple of 4 (16-byte rows of W1)");
   cudaStream_t s = (cudaStream_t)stream;
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;     // the canonical positions change: skin again
   rga_prof_mark(av, "-", s);

@@ -6,17 +6,21 @@
 //   core matrices); the fp32 accumulator (128 lanes x 256 columns) in tensor memory, read back with tcgen05.ld for the
 //   bias + ReLU epilogue, which writes the next layer's A operand straight back into shared memory.
 // All four hidden layers and the 256 -> 3 head run in one kernel: activations never leave the SM.
-// Weights stream from L2 in 256 x 32 chunks through two buffers; a chunk's buffer is released by tcgen05.commit on an
-// mbarrier.  theta is the same for every vertex, so its part of layer 1 is folded into that layer's bias per CTA.
+// Weights stream from L2 in 256 x 16 chunks through four cp.async buffers (three chunks in flight); a chunk's buffer is
+// released by tcgen05.commit on an
+// mbarrier.  theta is the same for every vertex, so its part of layer 1 is folded into that layer's bias once per call.
 // FAST file: the result is compared with the fp64 oracle under the TF32 tolerance derived in DESIGN.md.
 #include "rga_internal.h"
 
 #define MLP_M 128              // vertices per CTA (UMMA M)
 #define MLP_W 256              // layer width (UMMA N)
-#define MLP_KC 32              // weight chunk along K
+#define MLP_KC 16              // weight chunk along K (two K = 8 instructions)
+#define MLP_NBUF 4             // weight chunk buffers (cp.async prefetch distance 3)
+#define MLP_THREADS 256
 #define MLP_LBO 128u           // bytes between core matrices adjacent in K
 #define MLP_SBO_A (MLP_W / 4 * 128u)    // bytes between 8-row groups of the activation tile (K up to 256)
 #define MLP_SBO_B (MLP_KC / 4 * 128u)   // ... of a weight chunk
+#define MLP_CHUNK_BYTES (MLP_W * MLP_KC * 4)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -39,105 +43,125 @@ __device__ __forceinline__ uint32_t canon(int r, int k, uint32_t sbo) {
   return (uint32_t)(r & 7) * 16u + (uint32_t)(r >> 3) * sbo + (uint32_t)(k >> 2) * MLP_LBO + (uint32_t)(k & 3) * 4u;
 }
 
-__global__ void __launch_bounds__(MLP_M, 1) disp_mlp_kernel(int nv, int F, int n_pose, const float4* __restrict__ v_pos,
-    const float* __restrict__ rff, const float* __restrict__ theta, const float* __restrict__ W1, const float* __restrict__ b1,
+// theta is the same for every vertex: its columns of W1 are folded into layer 1's bias once per call, one warp per row
+__global__ void __launch_bounds__(256) mlp_bias1_kernel(int K1, int n_pose, const float* __restrict__ W1, const float* __restrict__ b1,
+                                                        const float* __restrict__ theta, float* __restrict__ bias1) {
+  const int n = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  float acc = 0.f;
+  for (int j = lane; j < n_pose; j += 32) acc = fmaf(W1[(size_t)n * (K1 + n_pose) + K1 + j], theta[j], acc);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0) bias1[n] = b1[n] + acc;
+}
+
+__global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F, int n_pose, const float4* __restrict__ v_pos,
+    const float* __restrict__ rff, const float* __restrict__ bias1, const float* __restrict__ W1,
     const float* __restrict__ Wh, const float* __restrict__ bh, const float* __restrict__ Wo, const float* __restrict__ bo,
     float4* __restrict__ v_disp) {
   extern __shared__ __align__(1024) unsigned char smem[];
   unsigned char* sA = smem;                                          // 128 x 256 tf32, canonical: 128 KB
-  unsigned char* sB = smem + (size_t)MLP_M * MLP_W * 4;               // 2 x (256 x 32): 64 KB
-  float* sBias = reinterpret_cast<float*>(sB + 2 * (size_t)MLP_W * MLP_KC * 4);     // [4][256]
+  unsigned char* sB = smem + (size_t)MLP_M * MLP_W * 4;               // MLP_NBUF x (256 x 16): 64 KB
+  float* sBias = reinterpret_cast<float*>(sB + (size_t)MLP_NBUF * MLP_CHUNK_BYTES);     // [4][256]
   float* sWo = sBias + 4 * MLP_W;                                     // [3][256]
   float* sRff = sWo + 3 * MLP_W;                                      // [F][3]
-  __shared__ __align__(8) unsigned long long bars[3];                 // weight buffer 0 / 1 free, accumulator ready
+  float* sOut = sRff + 3 * 128;                                       // [128][3] partial head sums of the upper column half
+  __shared__ __align__(8) unsigned long long bars[MLP_NBUF + 1];      // weight buffers free, accumulator ready
   __shared__ uint32_t tmem_base_s;
-  const int tid = threadIdx.x, warp = tid >> 5;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int K1 = 2 * F, in1 = K1 + n_pose;
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "r"((uint32_t)MLP_W));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (tid == 0) {
-    for (int i = 0; i < 3; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&bars[i])), "r"(1u));
+    for (int i = 0; i <= MLP_NBUF; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&bars[i])), "r"(1u));
     asm volatile("fence.mbarrier_init.release.cluster;");
   }
-  // biases (layer 1 with the pose folded in), head weights, Fourier matrix
-  for (int n = tid; n < MLP_W; n += MLP_M) {
-    float acc = b1[n];
-    for (int j = 0; j < n_pose; ++j) acc = fmaf(W1[(size_t)n * in1 + K1 + j], theta[j], acc);
-    sBias[n] = acc;
+  // chunk t of the whole network: layer, weight matrix and row stride, first column
+  const int nch1 = K1 / MLP_KC, total = nch1 + 3 * (MLP_W / MLP_KC);
+  constexpr int nchh = MLP_W / MLP_KC;
+  auto stage = [&](int t) {                                           // cp.async: 256 rows x 16 columns, 16 bytes per copy
+    const int layer = t < nch1 ? 0 : 1 + (t - nch1) / nchh, c = t < nch1 ? t : (t - nch1) % nchh;
+    const float* Wl = layer == 0 ? W1 : Wh + (size_t)(layer - 1) * MLP_W * MLP_W;
+    const int ldw = layer == 0 ? in1 : MLP_W;
+    unsigned char* buf = sB + (size_t)(t % MLP_NBUF) * MLP_CHUNK_BYTES;
+    for (int q = tid; q < MLP_W * MLP_KC / 4; q += MLP_THREADS) {     // four consecutive threads read 64 contiguous bytes of a row
+      const int n = q >> 2, kq = q & 3;
+      const float* src = Wl + (size_t)n * ldw + c * MLP_KC + 4 * kq;
+      const uint32_t dst = smem_u32(buf) + (uint32_t)(n & 7) * 16u + (uint32_t)(n >> 3) * MLP_SBO_B + (uint32_t)kq * MLP_LBO;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(src) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  // biases (layer 1's already holds the pose, mlp_bias1_kernel), head weights, Fourier matrix
+  for (int n = tid; n < MLP_W; n += MLP_THREADS) {
+    sBias[n] = bias1[n];
     for (int l = 0; l < 3; ++l) sBias[(l + 1) * MLP_W + n] = bh[l * MLP_W + n];
     for (int c = 0; c < 3; ++c) sWo[c * MLP_W + n] = Wo[c * MLP_W + n];
   }
-  for (int i = tid; i < 3 * F; i += MLP_M) sRff[i] = rff[i];
+  for (int i = tid; i < 3 * F; i += MLP_THREADS) sRff[i] = rff[i];
+  stage(0); stage(1); stage(2);                                       // the first weight chunks fly during the prologue
   __syncthreads();
-  // layer-1 operand: gamma(x) = [sin(2 pi B x), cos(2 pi B x)] of this thread's vertex
-  const int v = blockIdx.x * MLP_M + tid;
+  // layer-1 operand: gamma(x) = [sin(2 pi B x), cos(2 pi B x)] of the row's vertex; the two thread halves share the features
+  const int row = tid & (MLP_M - 1), half = tid >> 7;
+  const int v = blockIdx.x * MLP_M + row;
   {
     float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
     if (v < nv) x = v_pos[v];
-    for (int f = 0; f < F; ++f) {
+    for (int f = half * (F / 2); f < (half + 1) * (F / 2); ++f) {
       const float p = fmaf(sRff[3 * f + 2], x.z, fmaf(sRff[3 * f + 1], x.y, sRff[3 * f] * x.x));
       float sn, cs;
       sincospif(2.0f * p, &sn, &cs);
-      *reinterpret_cast<float*>(sA + canon(tid, f, MLP_SBO_A)) = sn;
-      *reinterpret_cast<float*>(sA + canon(tid, F + f, MLP_SBO_A)) = cs;
+      *reinterpret_cast<float*>(sA + canon(row, f, MLP_SBO_A)) = sn;
+      *reinterpret_cast<float*>(sA + canon(row, F + f, MLP_SBO_A)) = cs;
     }
   }
   const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(MLP_W >> 3) << 17) | ((uint32_t)(MLP_M >> 4) << 24);
-  uint32_t par_buf[2] = {0u, 0u}, par_acc = 0u;
-  bool pending[2] = {false, false};
+  uint32_t par_acc = 0u;
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;");
   const uint32_t tmem_base = tmem_base_s;
   float out0 = 0.f, out1 = 0.f, out2 = 0.f;
 
-  for (int layer = 0; layer < 4; ++layer) {
-    const int Kl = layer == 0 ? K1 : MLP_W;
-    const float* Wl = layer == 0 ? W1 : Wh + (size_t)(layer - 1) * MLP_W * MLP_W;
-    const int ldw = layer == 0 ? in1 : MLP_W;
-    const int nchunks = Kl / MLP_KC;
-    for (int c = 0; c < nchunks; ++c) {
-      const int b = c & 1;
-      if (pending[b]) { mbar_wait(smem_u32(&bars[b]), par_buf[b]); par_buf[b] ^= 1u; pending[b] = false; }
-      unsigned char* buf = sB + (size_t)b * MLP_W * MLP_KC * 4;
-      // 256 rows x 32 columns of W_l, 16 bytes at a time; eight consecutive threads read 128 contiguous bytes of a row
-      for (int q = tid; q < MLP_W * MLP_KC / 4; q += MLP_M) {
-        const int n = q >> 3, kq = q & 7;
-        const float* src = Wl + (size_t)n * ldw + c * MLP_KC + 4 * kq;
-        float4 w4;
-        if ((ldw & 3) == 0) w4 = *reinterpret_cast<const float4*>(src);
-        else w4 = make_float4(src[0], src[1], src[2], src[3]);
-        *reinterpret_cast<float4*>(buf + (uint32_t)(n & 7) * 16u + (uint32_t)(n >> 3) * MLP_SBO_B + (uint32_t)kq * MLP_LBO) = w4;
-      }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic-proxy writes -> the tensor core's async proxy
-      asm volatile("tcgen05.fence::before_thread_sync;");
-      __syncthreads();
-      if (tid == 0) {
-        asm volatile("tcgen05.fence::after_thread_sync;");
+  for (int t = 0; t < total; ++t) {
+    const int layer = t < nch1 ? 0 : 1 + (t - nch1) / nchh, c = t < nch1 ? t : (t - nch1) % nchh;
+    const int nchunks = layer == 0 ? nch1 : nchh;
+    asm volatile("cp.async.wait_group 2;" ::: "memory");              // chunk t has landed (this thread's copies); t+1, t+2 fly
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> the tensor core's async proxy
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (tid == 0) {
+      asm volatile("tcgen05.fence::after_thread_sync;");
+      const uint32_t buf = smem_u32(sB + (size_t)(t % MLP_NBUF) * MLP_CHUNK_BYTES);
 #pragma unroll
-        for (int j = 0; j < MLP_KC / 8; ++j) {
-          const uint64_t da = umma_desc(smem_u32(sA) + (uint32_t)(c * (MLP_KC / 4) + 2 * j) * MLP_LBO, MLP_LBO, MLP_SBO_A);
-          const uint64_t db = umma_desc(smem_u32(buf) + (uint32_t)(2 * j) * MLP_LBO, MLP_LBO, MLP_SBO_B);
-          const uint32_t acc = (c > 0 || j > 0) ? 1u : 0u;
-          asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                       "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-                       :: "r"(tmem_base), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
-        }
-        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[b])) : "memory");
-        if (c == nchunks - 1)
-          asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[2])) : "memory");
+      for (int j = 0; j < MLP_KC / 8; ++j) {
+        const uint64_t da = umma_desc(smem_u32(sA) + (uint32_t)(c * (MLP_KC / 4) + 2 * j) * MLP_LBO, MLP_LBO, MLP_SBO_A);
+        const uint64_t db = umma_desc(buf + (uint32_t)(2 * j) * MLP_LBO, MLP_LBO, MLP_SBO_B);
+        const uint32_t acc = (c > 0 || j > 0) ? 1u : 0u;
+        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                     "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                     :: "r"(tmem_base), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
       }
-      pending[b] = true;
+      asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[t % MLP_NBUF])) : "memory");
+      if (c == nchunks - 1)
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[MLP_NBUF])) : "memory");
     }
-    // accumulator ready: every MMA of the layer has read its operands, so sA may be overwritten
-    mbar_wait(smem_u32(&bars[2]), par_acc); par_acc ^= 1u;
+    // keep three chunks in flight: chunk t+3 reuses the buffer of chunk t-1, whose MMAs were issued one iteration ago
+    if (t + 3 < total) {
+      if (t >= 1) mbar_wait(smem_u32(&bars[(t + 3) % MLP_NBUF]), (uint32_t)(((t - 1) / MLP_NBUF) & 1));
+      stage(t + 3);
+    } else asm volatile("cp.async.commit_group;" ::: "memory");      // keeps the group count uniform
+    if (c != nchunks - 1) continue;
+    // accumulator ready: every MMA of the layer has read its operands, so sA may be overwritten.  Warp w reads TMEM lanes
+    // 32 (w & 3) .. +31 (its row) and the column half w >> 2.
+    mbar_wait(smem_u32(&bars[MLP_NBUF]), par_acc); par_acc ^= 1u;
     asm volatile("tcgen05.fence::after_thread_sync;");
     const float* bias = sBias + layer * MLP_W;
-    for (int c0 = 0; c0 < MLP_W; c0 += 32) {
+    const int erow = (warp & 3) * 32 + lane;
+    for (int c0 = (warp >> 2) * (MLP_W / 2); c0 < (warp >> 2) * (MLP_W / 2) + MLP_W / 2; c0 += 32) {
       uint32_t r[32];
-      const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)c0;
+      const uint32_t taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)c0;
       asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
                    "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
                    : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
@@ -152,7 +176,7 @@ __global__ void __launch_bounds__(MLP_M, 1) disp_mlp_kernel(int nv, int F, int n
           float4 h;
           h.x = fmaxf(__uint_as_float(r[j]) + bias[c0 + j], 0.f);         h.y = fmaxf(__uint_as_float(r[j + 1]) + bias[c0 + j + 1], 0.f);
           h.z = fmaxf(__uint_as_float(r[j + 2]) + bias[c0 + j + 2], 0.f); h.w = fmaxf(__uint_as_float(r[j + 3]) + bias[c0 + j + 3], 0.f);
-          *reinterpret_cast<float4*>(sA + canon(tid, c0 + j, MLP_SBO_A)) = h;
+          *reinterpret_cast<float4*>(sA + canon(erow, c0 + j, MLP_SBO_A)) = h;
         }
       } else {                                                         // head: 256 -> 3, fp32 on the CUDA cores
 #pragma unroll
@@ -162,16 +186,22 @@ __global__ void __launch_bounds__(MLP_M, 1) disp_mlp_kernel(int nv, int F, int n
         }
       }
     }
-    // (the next layer's first staging barrier orders these shared-memory writes and TMEM reads before its MMAs)
+    // (the next chunk's staging barrier orders these shared-memory writes and TMEM reads before the next layer's MMAs)
   }
-  if (v < nv) v_disp[v] = make_float4(out0 + bo[0], out1 + bo[1], out2 + bo[2], 0.f);
+  // head: the lower column half adds the upper half's partial sums (fixed order: lower + upper)
+  const int erow = (warp & 3) * 32 + lane;
+  if (warp >= 4) { sOut[3 * erow] = out0; sOut[3 * erow + 1] = out1; sOut[3 * erow + 2] = out2; }
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
+  const int ev = blockIdx.x * MLP_M + erow;
+  if (warp < 4 && ev < nv)
+    v_disp[ev] = make_float4((out0 + sOut[3 * erow]) + bo[0], (out1 + sOut[3 * erow + 1]) + bo[1], (out2 + sOut[3 * erow + 2]) + bo[2], 0.f);
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"((uint32_t)MLP_W));
 }
 
 size_t rga_mlp_smem(int F) {
-  return (size_t)MLP_M * MLP_W * 4 + 2 * (size_t)MLP_W * MLP_KC * 4 + (size_t)(4 + 3) * MLP_W * 4 + (size_t)3 * F * 4 + 64;
+  (void)F;
+  return (size_t)MLP_M * MLP_W * 4 + (size_t)MLP_NBUF * MLP_CHUNK_BYTES + (size_t)(4 + 3) * MLP_W * 4 + (size_t)3 * 128 * 4 + (size_t)3 * MLP_M * 4 + 64;
 }
 
 int rga_mlp_init_attributes() {
@@ -180,9 +210,11 @@ int rga_mlp_init_attributes() {
 
 cudaError_t rga_launch_disp_mlp(rga_avatar* av, const rga_disp_mlp* m, const float* theta, cudaStream_t s) {
   const int grid = (av->n_verts + MLP_M - 1) / MLP_M;
-  disp_mlp_kernel<<<grid, MLP_M, rga_mlp_smem(m->n_freq), s>>>(av->n_verts, m->n_freq, m->n_pose, av->v_pos, m->rff, theta, m->W1, m->b1,
+  mlp_bias1_kernel<<<MLP_W / 8, 256, 0, s>>>(2 * m->n_freq, m->n_pose, m->W1, m->b1, theta, av->mlp_bias1);
+  rga_prof_mark(av, "mlp_bias1", s);
+  disp_mlp_kernel<<<grid, MLP_THREADS, rga_mlp_smem(m->n_freq), s>>>(av->n_verts, m->n_freq, m->n_pose, av->v_pos, m->rff, av->mlp_bias1, m->W1,
                                                                m->Wh, m->bh, m->Wo, m->bo, av->v_disp);
-  av->launches += 1;
+  av->launches += 2;
   rga_prof_mark(av, "disp_mlp", s);
   return cudaGetLastError();
 }

@@ -20,6 +20,7 @@ struct rga_avatar {
   float4* v_pos;       // [n_verts]  canonical x (displacement_mlp re-derives x + dx from it)
   float4* v_disp;      // [n_verts]  per-pose displacement written by displacement_mlp
   float4* g_pos;       // [n_gauss]  canonical x_g
+  float* mlp_bias1;    // [256] layer-1 bias of the displacement network with the pose folded in
   float4* v_xbar;      // [n_verts]  x + dx
   float4* v_normal;    // [n_verts]
   float* v_skin_w;     // [n_verts][B]
