@@ -184,6 +184,36 @@ def main():
         frame_e2e()
     ms_e2e = timed(frame_e2e, args.steps)
 
+    # the same with the image read-back of step i on a copy stream beside step i+1 (two image buffers): what a viewer
+    # loop does.  Reported as e2e.pipelined_value; e2e.value stays the serial number above.
+    copy_stream = torch.cuda.Stream(device=dev)
+    imgs = [torch.empty_like(img) for _ in range(2)]
+    h_imgs = [torch.empty((H, W, 3), dtype=torch.float32).pin_memory() for _ in range(2)]
+    copied = [None, None]
+
+    def run_pipelined(steps):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        last_copy = None
+        barrier()
+        for i, (a, b) in enumerate(evs):
+            flush.fill_(1)
+            a.record()
+            if copied[i & 1] is not None:
+                torch.cuda.current_stream().wait_event(copied[i & 1])     # buffer i&1 has been read back
+            d_bones.copy_(h_bones, non_blocking=True); d_env.copy_(h_env, non_blocking=True)
+            av.render(d_bones, dirs, R, d_env, t2d, inp["cam_pos"], camc, inp["bg"], imgs[i & 1], vis_mode=args.vis_mode, bias=bias)
+            b.record()
+            copy_stream.wait_event(b)
+            with torch.cuda.stream(copy_stream):
+                h_imgs[i & 1].copy_(imgs[i & 1], non_blocking=True)
+                copied[i & 1] = torch.cuda.Event(enable_timing=True); copied[i & 1].record()
+                last_copy = copied[i & 1]
+        barrier(); copy_stream.synchronize()
+        tail = max(evs[-1][1].elapsed_time(last_copy), 0.0)                # the last read-back is not hidden by a next step
+        return (sum(a.elapsed_time(b) for a, b in evs) + tail) / steps
+    run_pipelined(3)
+    ms_e2e_pipe = run_pipelined(args.steps)
+
     # per-kernel times (CUDA events recorded by the library after each of its kernels), same flush protocol
     rga.rga_profile_enable(av.h, True)
     acc = {}
@@ -266,7 +296,9 @@ def main():
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "paper_context": "6.9 fps on RTX 4090 (PAPER.md:314)"},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": world * 1e3 / ms_e2e, "unit": "frames/s", "h2d_bytes_per_step": int(h_bones.numel() * 4 + h_env.numel() * 4),
-                "d2h_bytes_per_step": int(h_img.numel() * 4)},
+                "d2h_bytes_per_step": int(h_img.numel() * 4),
+                "pipelined_value": world * 1e3 / ms_e2e_pipe,
+                "pipelined_note": "image read-back of step i on a copy stream beside step i+1; per-step events plus the last copy's tail"},
         "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
         "disp_mlp": mlp_obj,
         "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},

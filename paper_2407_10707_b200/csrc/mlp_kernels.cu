@@ -7,8 +7,8 @@
 //   bias + ReLU epilogue, which writes the next layer's A operand straight back into shared memory.
 // All four hidden layers and the 256 -> 3 head run in one kernel: activations never leave the SM.
 // Weights stream from L2 in 256 x 16 chunks through four cp.async buffers (three chunks in flight); a chunk's buffer is
-// released by tcgen05.commit on an
-// mbarrier.  theta is the same for every vertex, so its part of layer 1 is folded into that layer's bias once per call.
+// released by tcgen05.commit on an mbarrier.  theta is the same for every vertex, so its part of layer 1 is folded into
+// that layer's bias once per call (mlp_bias1_kernel).
 // FAST file: the result is compared with the fp64 oracle under the TF32 tolerance derived in DESIGN.md.
 #include "rga_internal.h"
 
