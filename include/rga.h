@@ -59,7 +59,8 @@ typedef enum {
 
 /* avatar_load input.  PAPER.md:86 lists the vertex attributes {r,s,a,gamma,p,w,n,dx}; PAPER.md:88 the Gaussians. */
 typedef struct {
-  int32_t n_verts, n_faces, n_bones, n_gauss;
+  int32_t n_verts, n_faces, n_bones, n_gauss;   /* n_verts < 2^21 and small enough for the rasteriser's shared-memory
+                                                    vertex table (about 49k), n_faces < 2^24                           */
   int32_t k_g;                 /* neighbours per Gaussian, 1..3 (paper: 3)          */
   int32_t k_v;                 /* neighbours per vertex, odd, 1..31 (paper: 19); clamped to n_verts */
   const float*   vert_pos;     /* dev [n_verts][3]  canonical x                                      */

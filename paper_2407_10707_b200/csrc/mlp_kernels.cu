@@ -2,33 +2,35 @@
 // layers, each with a width of 256 and activated by ReLU", "Random Fourier Features"; readings A26-A28) -- the
 // one dense contraction of the method, so it runs on the 5th-generation tensor cores:
 //   tcgen05.mma kind::tf32, M = 128 vertices per CTA, N = 256 = the layer width, K = 8 per instruction, issued by one
-//   thread; A (activations) and B (weights) in shared memory in the canonical K-major no-swizzle layout (8-row x 16-byte
-//   core matrices); the fp32 accumulator (128 lanes x 256 columns) in tensor memory, read back with tcgen05.ld for the
+//   thread; A (activations) and B (weights) in shared memory in the K-major 128-byte-swizzle layout (8-row x 128-byte
+//   atoms); the fp32 accumulator (128 lanes x 256 columns) in tensor memory, read back with tcgen05.ld for the
 //   bias + ReLU epilogue, which writes the next layer's A operand straight back into shared memory.
 // All four hidden layers and the 256 -> 3 head run in one kernel: activations never leave the SM.
-// Weights stream from L2 in 256 x 16 chunks through four cp.async buffers (three chunks in flight); a chunk's buffer is
-// released by tcgen05.commit on an mbarrier.  theta is the same for every vertex, so its part of layer 1 is folded into
+// Weights stream from L2 in 256 x 32 chunks through two cp.async buffers; a chunk's buffer is released by tcgen05.commit
+// on an mbarrier.  theta is the same for every vertex, so its part of layer 1 is folded into
 // that layer's bias once per call (mlp_bias1_kernel).
 // FAST file: the result is compared with the fp64 oracle under the TF32 tolerance derived in DESIGN.md.
 #include "rga_internal.h"
 
 #define MLP_M 128              // vertices per CTA (UMMA M)
 #define MLP_W 256              // layer width (UMMA N)
-#define MLP_KC 16              // weight chunk along K (two K = 8 instructions)
-#define MLP_NBUF 4             // weight chunk buffers (cp.async prefetch distance 3)
+#define MLP_KC 32              // weight chunk along K (four K = 8 instructions): every chunk costs ~1,000 cycles of
+                               // barriers and fences whatever its size, so few large chunks beat many small ones
+#define MLP_NBUF 2             // weight chunk buffers (cp.async prefetch distance 1)
+#define MLP_PD (MLP_NBUF - 1)
 #define MLP_THREADS 256
-#define MLP_LBO 128u           // bytes between core matrices adjacent in K
-#define MLP_SBO_A (MLP_W / 4 * 128u)    // bytes between 8-row groups of the activation tile (K up to 256)
-#define MLP_SBO_B (MLP_KC / 4 * 128u)   // ... of a weight chunk
+#define MLP_SBO 1024u          // 128-byte swizzle, K-major: an atom is 8 rows x 128 bytes (32 tf32), 8-row groups 1 KB apart
+#define MLP_ATOM_A (MLP_M * 128u)       // bytes between K atoms of the activation tile (128 rows x 128 bytes)
 #define MLP_CHUNK_BYTES (MLP_W * MLP_KC * 4)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-// shared-memory matrix descriptor (no swizzle, K-major): start >> 4, leading (K) byte offset >> 4, stride (M/N) byte
-// offset >> 4, version 1
-__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
-  return (uint64_t)((saddr >> 4) & 0x3fffu) | ((uint64_t)((lbo >> 4) & 0x3fffu) << 16) | ((uint64_t)((sbo >> 4) & 0x3fffu) << 32) |
-         ((uint64_t)1 << 46);
+// shared-memory matrix descriptor (K-major, SWIZZLE_128B): start >> 4, leading byte offset (unused: K stays inside one
+// atom) >> 4, stride (8-row group) byte offset >> 4, version 1, layout type 2.  The no-swizzle layout is correct too but
+// the tensor core then reads its operands at a quarter of the rate (measured: ~550 cycles per 128x256x8 instruction).
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
+  return (uint64_t)((saddr >> 4) & 0x3fffu) | ((uint64_t)1 << 16) | ((uint64_t)((MLP_SBO >> 4) & 0x3fffu) << 32) |
+         ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
 
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
@@ -38,9 +40,11 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
                  : "=r"(done) : "r"(bar), "r"(parity) : "memory");
 }
 
-// canonical K-major offset of element (row r, column k) of a tile whose 8-row groups are `sbo` bytes apart
-__device__ __forceinline__ uint32_t canon(int r, int k, uint32_t sbo) {
-  return (uint32_t)(r & 7) * 16u + (uint32_t)(r >> 3) * sbo + (uint32_t)(k >> 2) * MLP_LBO + (uint32_t)(k & 3) * 4u;
+// offset of element (row r, column k) of the activation tile: K atom k / 32, 8-row group r / 8, row r % 8 (128 bytes), and the
+// 16-byte piece (k % 32) / 4 XOR-swizzled with the row (Swizzle<3,4,3>)
+__device__ __forceinline__ uint32_t swz(int r, int k) {
+  return (uint32_t)(k >> 5) * MLP_ATOM_A + (uint32_t)(r >> 3) * MLP_SBO + (uint32_t)(r & 7) * 128u +
+         ((((uint32_t)(k >> 2) & 7u) ^ (uint32_t)(r & 7)) << 4) + (uint32_t)(k & 3) * 4u;
 }
 
 // theta is the same for every vertex: its columns of W1 are folded into layer 1's bias once per call, one warp per row
@@ -59,8 +63,8 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
     const float* __restrict__ Wh, const float* __restrict__ bh, const float* __restrict__ Wo, const float* __restrict__ bo,
     float4* __restrict__ v_disp) {
   extern __shared__ __align__(1024) unsigned char smem[];
-  unsigned char* sA = smem;                                          // 128 x 256 tf32, canonical: 128 KB
-  unsigned char* sB = smem + (size_t)MLP_M * MLP_W * 4;               // MLP_NBUF x (256 x 16): 64 KB
+  unsigned char* sA = smem;                                          // 128 x 256 tf32, eight swizzled K atoms: 128 KB
+  unsigned char* sB = smem + (size_t)MLP_M * MLP_W * 4;               // MLP_NBUF x (256 x 32): 64 KB
   float* sBias = reinterpret_cast<float*>(sB + (size_t)MLP_NBUF * MLP_CHUNK_BYTES);     // [4][256]
   float* sWo = sBias + 4 * MLP_W;                                     // [3][256]
   float* sRff = sWo + 3 * MLP_W;                                      // [F][3]
@@ -85,10 +89,12 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
     const float* Wl = layer == 0 ? W1 : Wh + (size_t)(layer - 1) * MLP_W * MLP_W;
     const int ldw = layer == 0 ? in1 : MLP_W;
     unsigned char* buf = sB + (size_t)(t % MLP_NBUF) * MLP_CHUNK_BYTES;
-    for (int q = tid; q < MLP_W * MLP_KC / 4; q += MLP_THREADS) {     // four consecutive threads read 64 contiguous bytes of a row
-      const int n = q >> 2, kq = q & 3;
+    // 16-byte piece q of the chunk in shared-memory order (destination 16 q: conflict-free): row r = (q >> 3) & 7 of row
+    // group g = q >> 6, physical slot q & 7 of the row, which holds K piece (q & 7) ^ r; a warp reads 4 rows x 128 bytes
+    for (int q = tid; q < MLP_W * MLP_KC / 4; q += MLP_THREADS) {
+      const int r = (q >> 3) & 7, n = ((q >> 6) << 3) | r, kq = (q & 7) ^ r;
       const float* src = Wl + (size_t)n * ldw + c * MLP_KC + 4 * kq;
-      const uint32_t dst = smem_u32(buf) + (uint32_t)(n & 7) * 16u + (uint32_t)(n >> 3) * MLP_SBO_B + (uint32_t)kq * MLP_LBO;
+      const uint32_t dst = smem_u32(buf) + 16u * (uint32_t)q;
       asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(src) : "memory");
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
@@ -100,7 +106,7 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
     for (int c = 0; c < 3; ++c) sWo[c * MLP_W + n] = Wo[c * MLP_W + n];
   }
   for (int i = tid; i < 3 * F; i += MLP_THREADS) sRff[i] = rff[i];
-  stage(0); stage(1); stage(2);                                       // the first weight chunks fly during the prologue
+  for (int t = 0; t < MLP_PD; ++t) stage(t);                          // the first weight chunk flies during the prologue
   __syncthreads();
   // layer-1 operand: gamma(x) = [sin(2 pi B x), cos(2 pi B x)] of the row's vertex; the two thread halves share the features
   const int row = tid & (MLP_M - 1), half = tid >> 7;
@@ -112,8 +118,8 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
       const float p = fmaf(sRff[3 * f + 2], x.z, fmaf(sRff[3 * f + 1], x.y, sRff[3 * f] * x.x));
       float sn, cs;
       sincospif(2.0f * p, &sn, &cs);
-      *reinterpret_cast<float*>(sA + canon(row, f, MLP_SBO_A)) = sn;
-      *reinterpret_cast<float*>(sA + canon(row, F + f, MLP_SBO_A)) = cs;
+      *reinterpret_cast<float*>(sA + swz(row, f)) = sn;
+      *reinterpret_cast<float*>(sA + swz(row, F + f)) = cs;
     }
   }
   const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(MLP_W >> 3) << 17) | ((uint32_t)(MLP_M >> 4) << 24);
@@ -127,7 +133,13 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
   for (int t = 0; t < total; ++t) {
     const int layer = t < nch1 ? 0 : 1 + (t - nch1) / nchh, c = t < nch1 ? t : (t - nch1) % nchh;
     const int nchunks = layer == 0 ? nch1 : nchh;
-    asm volatile("cp.async.wait_group 2;" ::: "memory");              // chunk t has landed (this thread's copies); t+1, t+2 fly
+    // chunk t+1 goes into the buffer of chunk t-1 (its MMAs were issued an iteration ago) BEFORE chunk t is awaited, so
+    // every copy has a whole iteration to land
+    if (t + MLP_PD < total) {
+      if (t >= 1) mbar_wait(smem_u32(&bars[(t + MLP_PD) % MLP_NBUF]), (uint32_t)(((t - 1) / MLP_NBUF) & 1));
+      stage(t + MLP_PD);
+    } else asm volatile("cp.async.commit_group;" ::: "memory");      // keeps the group count uniform
+    asm volatile("cp.async.wait_group %0;" :: "n"(MLP_PD) : "memory");       // chunk t has landed (this thread's copies)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> the tensor core's async proxy
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
@@ -136,8 +148,8 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
       const uint32_t buf = smem_u32(sB + (size_t)(t % MLP_NBUF) * MLP_CHUNK_BYTES);
 #pragma unroll
       for (int j = 0; j < MLP_KC / 8; ++j) {
-        const uint64_t da = umma_desc(smem_u32(sA) + (uint32_t)(c * (MLP_KC / 4) + 2 * j) * MLP_LBO, MLP_LBO, MLP_SBO_A);
-        const uint64_t db = umma_desc(buf + (uint32_t)(2 * j) * MLP_LBO, MLP_LBO, MLP_SBO_B);
+        const uint64_t da = umma_desc(smem_u32(sA) + (uint32_t)c * MLP_ATOM_A + 32u * j);     // chunk c = K atom c; 32 bytes per K = 8
+        const uint64_t db = umma_desc(buf + 32u * j);
         const uint32_t acc = (c > 0 || j > 0) ? 1u : 0u;
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
@@ -147,11 +159,6 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
       if (c == nchunks - 1)
         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[MLP_NBUF])) : "memory");
     }
-    // keep three chunks in flight: chunk t+3 reuses the buffer of chunk t-1, whose MMAs were issued one iteration ago
-    if (t + 3 < total) {
-      if (t >= 1) mbar_wait(smem_u32(&bars[(t + 3) % MLP_NBUF]), (uint32_t)(((t - 1) / MLP_NBUF) & 1));
-      stage(t + 3);
-    } else asm volatile("cp.async.commit_group;" ::: "memory");      // keeps the group count uniform
     if (c != nchunks - 1) continue;
     // accumulator ready: every MMA of the layer has read its operands, so sA may be overwritten.  Warp w reads TMEM lanes
     // 32 (w & 3) .. +31 (its row) and the column half w >> 2.
@@ -176,7 +183,7 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
           float4 h;
           h.x = fmaxf(__uint_as_float(r[j]) + bias[c0 + j], 0.f);         h.y = fmaxf(__uint_as_float(r[j + 1]) + bias[c0 + j + 1], 0.f);
           h.z = fmaxf(__uint_as_float(r[j + 2]) + bias[c0 + j + 2], 0.f); h.w = fmaxf(__uint_as_float(r[j + 3]) + bias[c0 + j + 3], 0.f);
-          *reinterpret_cast<float4*>(sA + canon(erow, c0 + j, MLP_SBO_A)) = h;
+          *reinterpret_cast<float4*>(sA + swz(erow, c0 + j)) = h;
         }
       } else {                                                         // head: 256 -> 3, fp32 on the CUDA cores
 #pragma unroll
