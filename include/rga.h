@@ -127,6 +127,12 @@ RGA_API rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const flo
 /* H6-H10.  Needs shade_gaussians.  bg: host float[3].  out_image: dev [height][width][3] fp32, caller-owned. */
 RGA_API rga_status splat_render(rga_avatar* av, const rga_camera* cam, const float bg[3], float* out_image, void* stream);
 
+/* Moving Gaussians (the paper's training / editing regime, where x_g are free parameters and the KNN step is repeated
+ * every frame -- PAPER.md:88-93, Table 4 "KNN" :300-302): recomputes S_g (K_g nearest canonical vertices of every new
+ * position), the Eq.1 weights and every interpolated attribute {n, a, gamma, p, w, dx} exactly as avatar_load does; rotation,
+ * scale and opacity are kept.  gauss_pos: dev [n_gauss][3].  Enqueue-only; call pose_skin afterwards. */
+RGA_API rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, void* stream);
+
 /* Displacement network d(x, theta): dx_i = MLP([gamma(x_i), theta]) for every canonical vertex, with
  * gamma(x) = [sin(2 pi B x), cos(2 pi B x)] (random Fourier features, B = rff), four hidden layers of width 256 with ReLU
  * and a linear 256 -> 3 head (readings A26-A28).  Runs on the tensor cores (tcgen05, TF32 operands, fp32

@@ -171,6 +171,12 @@ def splat_render(h, camera, bg, out_image):
     _chk(lib().splat_render(h, C.byref(cam), b, _ptr(out_image), _stream()))
 
 
+def gaussians_update(h, gauss_pos):
+    """Per-frame KNN + Eq.1 re-interpolation for moved Gaussians (include/rga.h gaussians_update)."""
+    lib().gaussians_update.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    _chk(lib().gaussians_update(h, _ptr(gauss_pos), _stream()))
+
+
 class _DispMlp(C.Structure):
     _fields_ = [("n_freq", C.c_int32), ("n_pose", C.c_int32), ("rff", C.c_void_p), ("W1", C.c_void_p), ("b1", C.c_void_p),
                 ("Wh", C.c_void_p), ("bh", C.c_void_p), ("Wo", C.c_void_p), ("bo", C.c_void_p)]

@@ -55,7 +55,8 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
+  void* ptrs[] = {av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
+                  av->vt_spec, av->knn_d2, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
                   av->radiance, av->color, av->attr_color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->cursor, av->keys[0],
@@ -145,13 +146,24 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   }
   A(cudaMemcpyAsync(av->v_skin_w, d->vert_skin_w, nv * B * sizeof(float), cudaMemcpyDeviceToDevice, s));
   A(cudaMemcpyAsync(av->faces, d->faces, 3 * (size_t)av->n_faces * sizeof(int), cudaMemcpyDeviceToDevice, s));
+  A(dalloc(&av->vt_pos, 3 * nv)); A(dalloc(&av->vt_normal, 3 * nv)); A(dalloc(&av->vt_albedo, 3 * nv));
+  A(dalloc(&av->vt_rough, nv)); A(dalloc(&av->vt_spec, nv)); A(dalloc(&av->knn_d2, ng * av->k_g));
+  A(cudaMemcpyAsync(av->vt_pos, d->vert_pos, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  A(cudaMemcpyAsync(av->vt_normal, d->vert_normal, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  A(cudaMemcpyAsync(av->vt_albedo, d->vert_albedo, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  A(cudaMemcpyAsync(av->vt_rough, d->vert_rough, nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  A(cudaMemcpyAsync(av->vt_spec, d->vert_spec, nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  if (d->vert_disp) {
+    A(dalloc(&av->vt_disp, 3 * nv));
+    A(cudaMemcpyAsync(av->vt_disp, d->vert_disp, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  }
   A(rga_launch_pack_faces(av, s));
   A(rga_launch_load_verts(av, d->vert_pos, d->vert_disp, d->vert_normal, s));
   // KNN: S_v = K_v nearest vertices of each vertex (self included), S_g = K_g nearest of each Gaussian
-  A(dalloc(&d2, (ng * av->k_g > nv * av->k_v ? ng * av->k_g : nv * av->k_v)));
+  A(dalloc(&d2, nv * av->k_v));
   A(rga_launch_knn(d->vert_pos, av->n_verts, d->vert_pos, av->n_verts, av->k_v, av->knn_v, d2, s));
-  A(rga_launch_knn(d->gauss_pos, av->n_gauss, d->vert_pos, av->n_verts, av->k_g, av->knn_g, d2, s));
-  A(rga_launch_load_gauss(av, d, d2, s));
+  A(rga_launch_knn(d->gauss_pos, av->n_gauss, d->vert_pos, av->n_verts, av->k_g, av->knn_g, av->knn_d2, s));
+  A(rga_launch_load_gauss(av, d->gauss_pos, d->gauss_quat, d->gauss_scale, d->gauss_opacity, av->knn_d2, s));
   av->launches += 5;
   if (rga_shade_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_composite_init_attributes() != 0 || rga_mlp_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
   A(cudaStreamSynchronize(s));
@@ -220,6 +232,19 @@ extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const 
   CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->color, out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
   av->have_splat = 1;
+  return RGA_OK;
+}
+
+extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, void* stream) {
+  if (!av || !gauss_pos) return fail(RGA_ERR_INVALID_ARG, "gaussians_update: null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
+  rga_prof_mark(av, "-", s);
+  CU(rga_launch_knn(gauss_pos, av->n_gauss, av->vt_pos, av->n_verts, av->k_g, av->knn_g, av->knn_d2, s));
+  rga_prof_mark(av, "knn_g", s);
+  CU(rga_launch_load_gauss(av, gauss_pos, nullptr, nullptr, nullptr, av->knn_d2, s));
+  rga_prof_mark(av, "load_gauss", s);
+  av->launches += 2;
   return RGA_OK;
 }
 

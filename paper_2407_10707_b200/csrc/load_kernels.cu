@@ -108,14 +108,19 @@ __global__ void __launch_bounds__(128) load_gauss_kernel(int n, int K, int B, co
   gst[4 * (size_t)g + 2] = make_float4(interp(valb, 3, 0), interp(valb, 3, 1), interp(valb, 3, 2), interp(vrough, 1, 0));
   gst[4 * (size_t)g + 3] = make_float4(interp(vspec, 1, 0), 0.f, 0.f, 0.f);
   for (int b = 0; b < B; ++b) gw[(size_t)g * B + b] = interp(vw, B, b);
-  quat[g] = make_float4(gquat[4 * (size_t)g], gquat[4 * (size_t)g + 1], gquat[4 * (size_t)g + 2], gquat[4 * (size_t)g + 3]);
-  scale_op[g] = make_float4(gscale[3 * (size_t)g], gscale[3 * (size_t)g + 1], gscale[3 * (size_t)g + 2], gop ? gop[g] : 1.0f);
+  if (gquat) {                                               // NULL on gaussians_update: rotation, scale and opacity stay
+    quat[g] = make_float4(gquat[4 * (size_t)g], gquat[4 * (size_t)g + 1], gquat[4 * (size_t)g + 2], gquat[4 * (size_t)g + 3]);
+    scale_op[g] = make_float4(gscale[3 * (size_t)g], gscale[3 * (size_t)g + 1], gscale[3 * (size_t)g + 2], gop ? gop[g] : 1.0f);
+  }
 }
 
-cudaError_t rga_launch_load_gauss(rga_avatar* av, const rga_avatar_desc* d, const float* d2, cudaStream_t s) {
+// Eq.1 of every static attribute from the library's own copies of the vertex tables (so that gaussians_update can run
+// after the caller's arrays are gone); gauss_quat == NULL keeps rotation / scale / opacity.
+cudaError_t rga_launch_load_gauss(rga_avatar* av, const float* gauss_pos, const float* gauss_quat, const float* gauss_scale,
+                                  const float* gauss_opacity, const float* d2, cudaStream_t s) {
   load_gauss_kernel<<<(av->n_gauss + 127) / 128, 128, 0, s>>>(
-      av->n_gauss, av->k_g, av->n_bones, av->knn_g, d2, d->gauss_pos, d->vert_disp, d->vert_normal, d->vert_albedo,
-      d->vert_rough, d->vert_spec, d->vert_skin_w, d->gauss_quat, d->gauss_scale, d->gauss_opacity, av->ubar_g,
+      av->n_gauss, av->k_g, av->n_bones, av->knn_g, d2, gauss_pos, av->vt_disp, av->vt_normal, av->vt_albedo,
+      av->vt_rough, av->vt_spec, av->v_skin_w, gauss_quat, gauss_scale, gauss_opacity, av->ubar_g,
       av->g_static, av->g_skin_w, av->g_quat, av->g_scale_op, av->g_pos);
   return cudaGetLastError();
 }

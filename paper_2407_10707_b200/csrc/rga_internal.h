@@ -20,6 +20,9 @@ struct rga_avatar {
   float4* v_pos;       // [n_verts]  canonical x (displacement_mlp re-derives x + dx from it)
   float4* v_disp;      // [n_verts]  per-pose displacement written by displacement_mlp
   float4* g_pos;       // [n_gauss]  canonical x_g
+  // the library's copies of the vertex tables Eq.1 reads (gaussians_update re-interpolates from them)
+  float *vt_pos, *vt_disp, *vt_normal, *vt_albedo, *vt_rough, *vt_spec;   // [n_verts][3] x4 (disp NULL = 0), [n_verts] x2
+  float* knn_d2;       // [n_gauss][k_g] squared distances of the last Gaussian KNN
   float* mlp_bias1;    // [256] layer-1 bias of the displacement network with the pose folded in
   float4* v_xbar;      // [n_verts]  x + dx
   float4* v_normal;    // [n_verts]
@@ -92,7 +95,8 @@ void rga_prof_mark(rga_avatar* av, const char* name, cudaStream_t s);
 // load_kernels.cu
 cudaError_t rga_launch_knn(const float* q, int nq, const float* v, int nv, int K, int* idx, float* d2, cudaStream_t s);
 cudaError_t rga_launch_load_verts(rga_avatar* av, const float* pos, const float* disp, const float* nrm, cudaStream_t s);
-cudaError_t rga_launch_load_gauss(rga_avatar* av, const rga_avatar_desc* d, const float* d2, cudaStream_t s);
+cudaError_t rga_launch_load_gauss(rga_avatar* av, const float* gauss_pos, const float* gauss_quat, const float* gauss_scale,
+                                  const float* gauss_opacity, const float* d2, cudaStream_t s);
 // skin_kernels.cu
 cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, int which, cudaStream_t s);
 // vis_kernels.cu

@@ -288,3 +288,31 @@ def test_displacement_mlp_tensor_core_parity(cfg):
     rga.rga_check(av.h)
     compare_all(inp2, av, img.cpu().numpy(), orc_av, o, 0)
     av.close()
+
+
+def test_gaussians_update_equals_a_fresh_load():
+    # moved Gaussians -> KNN + Eq.1 again (the paper's per-frame KNN step); every table and everything
+    # downstream must equal what avatar_load computes for the new positions, bit for bit
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import compare_all
+    inp = workloads.make(1, n_gauss=20_000)
+    cam = inp["camera"]; W, H = cam["width"], cam["height"]
+    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=512, max_vis_res=128, max_env_texels=512)
+    rs = np.random.default_rng(21)
+    inp2 = dict(inp)
+    inp2["gauss_pos"] = (inp["gauss_pos"] + rs.normal(0.0, 0.01, inp["gauss_pos"].shape)).astype(np.float32)   # ~1 cm moves
+    rga.gaussians_update(av.h, torch.as_tensor(inp2["gauss_pos"]).cuda())
+    orc_av = orc.avatar_load(inp2)
+    o = orc.render_frame(orc_av, inp2, vis_mode=0)
+    img = torch.empty((H, W, 3), dtype=torch.float32, device="cuda")
+    av.render(torch.as_tensor(inp["bone_mats"][0]).cuda(), torch.as_tensor(inp["vis_dirs"]).cuda(), inp["vis_res"],
+              torch.as_tensor(inp["env"][0]).cuda(), torch.as_tensor(inp["texel_to_dir"]).cuda(), inp["cam_pos"], cam, inp["bg"], img,
+              vis_mode=0, gamma=inp["gamma"], bias=(inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"]))
+    rga.rga_check(av.h)
+    assert (orc_av["knn_g"] != orc.avatar_load(inp)["knn_g"]).any()          # the move does change neighbour sets
+    # keep_maps was off in this frame: compare everything except the triangle-id maps
+    rep = compare_all(inp2, av, img.cpu().numpy(), orc_av, o, 0)
+    print(rep)
+    av.close()
