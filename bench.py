@@ -286,6 +286,13 @@ def main():
                "vertices": nvv, "note": "one CTA per 128 vertices (54 CTAs at config 1), all four layers and the head fused; profiles/r01e_mlp.md"}
     # (the avatar now carries the network's displacement; it is not rendered again and is closed below)
 
+    # per-frame KNN + Eq.1 re-interpolation for moved Gaussians (the paper's KNN step: 0.93 ms per frame
+    # on an RTX 4090), exact uniform-grid search
+    gp = torch.as_tensor(inp["gauss_pos"]).to(dev)
+    for _ in range(3):
+        rga.gaussians_update(av.h, gp)
+    ms_knn = timed(lambda: rga.gaussians_update(av.h, gp), 20)
+
     from paper_2407_10707_b200 import replica
     ms, ms_e2e, ms_warm = replica.max_over_ranks([ms, ms_e2e, ms_warm], device=dev)      # slowest rank sets the job time
     out = {
@@ -300,7 +307,7 @@ def main():
                 "pipelined_value": world * 1e3 / ms_e2e_pipe,
                 "pipelined_note": "image read-back of step i on a copy stream beside step i+1; per-step events plus the last copy's tail"},
         "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
-        "disp_mlp": mlp_obj,
+        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn,
         "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -1,6 +1,7 @@
 // C ABI of librga (include/rga.h): argument checks, scratch ownership, stage ordering.  All compute is in the kernels.
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -56,7 +57,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
   void* ptrs[] = {av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
-                  av->vt_spec, av->knn_d2, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
+                  av->vt_spec, av->knn_d2, av->grid_start, av->grid_verts, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
                   av->radiance, av->color, av->attr_color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->cursor, av->keys[0],
@@ -162,7 +163,21 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   // KNN: S_v = K_v nearest vertices of each vertex (self included), S_g = K_g nearest of each Gaussian
   A(dalloc(&d2, nv * av->k_v));
   A(rga_launch_knn(d->vert_pos, av->n_verts, d->vert_pos, av->n_verts, av->k_v, av->knn_v, d2, s));
-  A(rga_launch_knn(d->gauss_pos, av->n_gauss, d->vert_pos, av->n_verts, av->k_g, av->knn_g, av->knn_d2, s));
+  {
+    // canonical-vertex AABB for the KNN grid: one pass over a host copy (load time)
+    float* hv = (float*)malloc(3 * nv * sizeof(float));
+    if (!hv) { st = fail(RGA_ERR_OOM, "avatar_load: host allocation"); goto done; }
+    cudaError_t ce = cudaMemcpyAsync(hv, av->vt_pos, 3 * nv * sizeof(float), cudaMemcpyDeviceToHost, s);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
+    float bb[6] = {1e30f, 1e30f, 1e30f, -1e30f, -1e30f, -1e30f};
+    if (ce == cudaSuccess)
+      for (size_t i = 0; i < nv; ++i)
+        for (int c = 0; c < 3; ++c) { float x = hv[3 * i + c]; if (x < bb[c]) bb[c] = x; if (x > bb[3 + c]) bb[3 + c] = x; }
+    free(hv);
+    if (ce != cudaSuccess) { st = fail(RGA_ERR_CUDA, "avatar_load: %s", cudaGetErrorString(ce)); goto done; }
+    A(rga_build_knn_grid(av, bb, s));
+  }
+  A(rga_launch_knn_gauss(av, d->gauss_pos, s));
   A(rga_launch_load_gauss(av, d->gauss_pos, d->gauss_quat, d->gauss_scale, d->gauss_opacity, av->knn_d2, s));
   av->launches += 5;
   if (rga_shade_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_composite_init_attributes() != 0 || rga_mlp_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
@@ -240,7 +255,7 @@ extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, v
   cudaStream_t s = (cudaStream_t)stream;
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
   rga_prof_mark(av, "-", s);
-  CU(rga_launch_knn(gauss_pos, av->n_gauss, av->vt_pos, av->n_verts, av->k_g, av->knn_g, av->knn_d2, s));
+  CU(rga_launch_knn_gauss(av, gauss_pos, s));
   rga_prof_mark(av, "knn_g", s);
   CU(rga_launch_load_gauss(av, gauss_pos, nullptr, nullptr, nullptr, av->knn_d2, s));
   rga_prof_mark(av, "load_gauss", s);

@@ -156,3 +156,127 @@ cudaError_t rga_launch_disp_apply(rga_avatar* av, cudaStream_t s) {
   rga_prof_mark(av, "disp_apply", s);
   return cudaGetLastError();
 }
+
+// ------------------------------------------------------------------------------------------- uniform-grid KNN (exact)
+// The canonical vertices are binned once into a uniform grid (counting sort: count, scan, fill).  A query walks the cells
+// ring by ring (Chebyshev distance r from its own cell) and keeps the K best by (d2, index) -- the same order the brute
+// force produces by scanning indices upward with a strict '<' -- and stops once the K-th distance is below ((r-1) h)^2, the
+// least any vertex of a cell of ring r or beyond can have (with a 1e-4 relative guard against the fp32 rounding of the cell
+// assignment).  d2 is computed with the brute force's operation order, so indices AND distances are bit-identical.
+struct KnnGrid { float ox, oy, oz, h, inv_h; int G; };
+
+__device__ __forceinline__ int grid_coord(float x, float o, float inv_h, int G) {
+  int c = (int)floorf((x - o) * inv_h);
+  return c < 0 ? 0 : (c >= G ? G - 1 : c);
+}
+
+__global__ void grid_count_kernel(int nv, KnnGrid g, const float* __restrict__ v, unsigned* __restrict__ cell_count,
+                                  int* __restrict__ cell_of) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nv) return;
+  int cx = grid_coord(v[3 * i], g.ox, g.inv_h, g.G), cy = grid_coord(v[3 * i + 1], g.oy, g.inv_h, g.G),
+      cz = grid_coord(v[3 * i + 2], g.oz, g.inv_h, g.G);
+  int c = (cz * g.G + cy) * g.G + cx;
+  cell_of[i] = c;
+  atomicAdd(cell_count + c, 1u);
+}
+
+// exclusive scan of the cell counts by one block (load time only); cell_start has ncell + 1 entries
+__global__ void __launch_bounds__(1024) grid_scan_kernel(int ncell, const unsigned* __restrict__ cell_count, unsigned* __restrict__ cell_start,
+                                                         unsigned* __restrict__ cursor) {
+  __shared__ unsigned part[1024];
+  const int per = (ncell + 1023) / 1024, lo = threadIdx.x * per, hi = min(ncell, lo + per);
+  unsigned s = 0;
+  for (int i = lo; i < hi; ++i) s += cell_count[i];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) { unsigned acc = 0; for (int t = 0; t < 1024; ++t) { unsigned v = part[t]; part[t] = acc; acc += v; } cell_start[ncell] = acc; }
+  __syncthreads();
+  unsigned acc = part[threadIdx.x];
+  for (int i = lo; i < hi; ++i) { cell_start[i] = acc; cursor[i] = acc; acc += cell_count[i]; }
+}
+
+__global__ void grid_fill_kernel(int nv, const int* __restrict__ cell_of, unsigned* __restrict__ cursor, int* __restrict__ cell_verts) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nv) return;
+  cell_verts[atomicAdd(cursor + cell_of[i], 1u)] = i;
+}
+
+template <int KT>
+__global__ void __launch_bounds__(128) knn_grid_kernel(const float* __restrict__ q, int nq, const float* __restrict__ v, KnnGrid g,
+    const unsigned* __restrict__ cell_start, const int* __restrict__ cell_verts, int* __restrict__ idx, float* __restrict__ d2out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nq) return;
+  const float qx = q[3 * (size_t)i], qy = q[3 * (size_t)i + 1], qz = q[3 * (size_t)i + 2];
+  float bd[KT]; int bi[KT];
+#pragma unroll
+  for (int k = 0; k < KT; ++k) { bd[k] = __int_as_float(0x7f800000); bi[k] = 0x7fffffff; }
+  const int cx = grid_coord(qx, g.ox, g.inv_h, g.G), cy = grid_coord(qy, g.oy, g.inv_h, g.G), cz = grid_coord(qz, g.oz, g.inv_h, g.G);
+  for (int r = 0; r <= g.G; ++r) {
+    if (r > 1) {                              // rings < r are done: every unvisited vertex is at least (r - 1) h away (see header)
+      const float reach = (float)(r - 1) * g.h;
+      if (bd[KT - 1] < reach * reach * 0.9999f) break;
+    }
+    const int z0 = max(cz - r, 0), z1 = min(cz + r, g.G - 1), y0 = max(cy - r, 0), y1 = min(cy + r, g.G - 1);
+    const int x0 = max(cx - r, 0), x1 = min(cx + r, g.G - 1);
+    for (int z = z0; z <= z1; ++z)
+      for (int y = y0; y <= y1; ++y) {
+        const bool shell_zy = abs(z - cz) == r || abs(y - cy) == r;
+        for (int x = x0; x <= x1; ++x) {
+          if (!shell_zy && abs(x - cx) != r) continue;          // inside the cube: visited in an earlier ring
+          const int c = (z * g.G + y) * g.G + x;
+          for (unsigned e = cell_start[c]; e < cell_start[c + 1]; ++e) {
+            const int j = cell_verts[e];
+            const float dx = qx - v[3 * (size_t)j], dy = qy - v[3 * (size_t)j + 1], dz = qz - v[3 * (size_t)j + 2];
+            const float d = (dx * dx + dy * dy) + dz * dz;
+            if (d < bd[KT - 1] || (d == bd[KT - 1] && j < bi[KT - 1])) {
+#pragma unroll
+              for (int p = KT - 1; p >= 0; --p) {
+                if (p > 0 && (d < bd[p - 1] || (d == bd[p - 1] && j < bi[p - 1]))) { bd[p] = bd[p - 1]; bi[p] = bi[p - 1]; }
+                else { bd[p] = d; bi[p] = j; break; }
+              }
+            }
+          }
+        }
+      }
+  }
+  for (int k = 0; k < KT; ++k) { idx[(size_t)i * KT + k] = bi[k]; d2out[(size_t)i * KT + k] = bd[k]; }
+}
+
+// builds the grid over av->vt_pos; returns cudaSuccess with av->grid_G == 0 when no grid is used (degenerate extent)
+cudaError_t rga_build_knn_grid(rga_avatar* av, const float* aabb_host, cudaStream_t s) {
+  av->grid_G = 0;
+  const float ex = aabb_host[3] - aabb_host[0], ey = aabb_host[4] - aabb_host[1], ez = aabb_host[5] - aabb_host[2];
+  const float ext = fmaxf(ex, fmaxf(ey, ez));
+  if (!(ext > 0.f) || av->n_verts < 64) return cudaSuccess;
+  int G = (int)(2.5f * cbrtf((float)av->n_verts) + 0.5f);
+  G = G < 4 ? 4 : (G > 128 ? 128 : G);
+  av->grid_G = G; av->grid_h = ext * 1.0001f / (float)G;
+  av->grid_o[0] = aabb_host[0]; av->grid_o[1] = aabb_host[1]; av->grid_o[2] = aabb_host[2];
+  const int ncell = G * G * G;
+  cudaError_t e;
+  if ((e = cudaMalloc((void**)&av->grid_start, (size_t)(ncell + 1) * 4)) != cudaSuccess) return e;
+  if ((e = cudaMalloc((void**)&av->grid_verts, (size_t)av->n_verts * 4)) != cudaSuccess) return e;
+  unsigned *count = nullptr, *cursor = nullptr; int* cell_of = nullptr;
+  if ((e = cudaMalloc((void**)&count, (size_t)ncell * 4)) != cudaSuccess) return e;
+  if ((e = cudaMalloc((void**)&cursor, (size_t)ncell * 4)) != cudaSuccess) return e;
+  if ((e = cudaMalloc((void**)&cell_of, (size_t)av->n_verts * 4)) != cudaSuccess) return e;
+  cudaMemsetAsync(count, 0, (size_t)ncell * 4, s);
+  KnnGrid g = {av->grid_o[0], av->grid_o[1], av->grid_o[2], av->grid_h, 1.0f / av->grid_h, G};
+  grid_count_kernel<<<(av->n_verts + 255) / 256, 256, 0, s>>>(av->n_verts, g, av->vt_pos, count, cell_of);
+  grid_scan_kernel<<<1, 1024, 0, s>>>(ncell, count, av->grid_start, cursor);
+  grid_fill_kernel<<<(av->n_verts + 255) / 256, 256, 0, s>>>(av->n_verts, cell_of, cursor, av->grid_verts);
+  e = cudaStreamSynchronize(s);
+  cudaFree(count); cudaFree(cursor); cudaFree(cell_of);
+  av->launches += 3;
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+// K_g nearest canonical vertices of the queries through the grid (brute force when there is no grid or K_g is not 3)
+cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s) {
+  if (av->grid_G == 0 || av->k_g != 3) return rga_launch_knn(q, av->n_gauss, av->vt_pos, av->n_verts, av->k_g, av->knn_g, av->knn_d2, s);
+  KnnGrid g = {av->grid_o[0], av->grid_o[1], av->grid_o[2], av->grid_h, 1.0f / av->grid_h, av->grid_G};
+  knn_grid_kernel<3><<<(av->n_gauss + 127) / 128, 128, 0, s>>>(q, av->n_gauss, av->vt_pos, g, av->grid_start, av->grid_verts, av->knn_g,
+                                                                av->knn_d2);
+  return cudaGetLastError();
+}

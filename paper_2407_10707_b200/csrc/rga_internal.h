@@ -23,6 +23,8 @@ struct rga_avatar {
   // the library's copies of the vertex tables Eq.1 reads (gaussians_update re-interpolates from them)
   float *vt_pos, *vt_disp, *vt_normal, *vt_albedo, *vt_rough, *vt_spec;   // [n_verts][3] x4 (disp NULL = 0), [n_verts] x2
   float* knn_d2;       // [n_gauss][k_g] squared distances of the last Gaussian KNN
+  // uniform grid over the canonical vertices (exact KNN of the Gaussians); grid_G == 0: brute force
+  int grid_G; float grid_h, grid_o[3]; unsigned* grid_start; int* grid_verts;
   float* mlp_bias1;    // [256] layer-1 bias of the displacement network with the pose folded in
   float4* v_xbar;      // [n_verts]  x + dx
   float4* v_normal;    // [n_verts]
@@ -118,4 +120,6 @@ int rga_init_kernel_attributes();
 // mlp_kernels.cu / load_kernels.cu
 cudaError_t rga_launch_disp_mlp(rga_avatar* av, const rga_disp_mlp* m, const float* theta, cudaStream_t s);
 cudaError_t rga_launch_disp_apply(rga_avatar* av, cudaStream_t s);
+cudaError_t rga_build_knn_grid(rga_avatar* av, const float* aabb_host, cudaStream_t s);
+cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s);
 int rga_mlp_init_attributes();
