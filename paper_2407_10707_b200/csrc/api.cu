@@ -162,7 +162,6 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(rga_launch_load_verts(av, d->vert_pos, d->vert_disp, d->vert_normal, s));
   // KNN: S_v = K_v nearest vertices of each vertex (self included), S_g = K_g nearest of each Gaussian
   A(dalloc(&d2, nv * av->k_v));
-  A(rga_launch_knn(d->vert_pos, av->n_verts, d->vert_pos, av->n_verts, av->k_v, av->knn_v, d2, s));
   {
     // canonical-vertex AABB for the KNN grid: one pass over a host copy (load time)
     float* hv = (float*)malloc(3 * nv * sizeof(float));
@@ -177,6 +176,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
     if (ce != cudaSuccess) { st = fail(RGA_ERR_CUDA, "avatar_load: %s", cudaGetErrorString(ce)); goto done; }
     A(rga_build_knn_grid(av, bb, s));
   }
+  A(rga_launch_knn_verts(av, d2, s));
   A(rga_launch_knn_gauss(av, d->gauss_pos, s));
   A(rga_launch_load_gauss(av, d->gauss_pos, d->gauss_quat, d->gauss_scale, d->gauss_opacity, av->knn_d2, s));
   av->launches += 5;

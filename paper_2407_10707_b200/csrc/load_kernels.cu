@@ -272,6 +272,15 @@ cudaError_t rga_build_knn_grid(rga_avatar* av, const float* aabb_host, cudaStrea
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+// S_v: K_v nearest vertices of every vertex (self included) through the grid when K_v is the paper's 19
+cudaError_t rga_launch_knn_verts(rga_avatar* av, float* d2, cudaStream_t s) {
+  if (av->grid_G == 0 || av->k_v != 19) return rga_launch_knn(av->vt_pos, av->n_verts, av->vt_pos, av->n_verts, av->k_v, av->knn_v, d2, s);
+  KnnGrid g = {av->grid_o[0], av->grid_o[1], av->grid_o[2], av->grid_h, 1.0f / av->grid_h, av->grid_G};
+  knn_grid_kernel<19><<<(av->n_verts + 127) / 128, 128, 0, s>>>(av->vt_pos, av->n_verts, av->vt_pos, g, av->grid_start, av->grid_verts,
+                                                                 av->knn_v, d2);
+  return cudaGetLastError();
+}
+
 // K_g nearest canonical vertices of the queries through the grid (brute force when there is no grid or K_g is not 3)
 cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s) {
   if (av->grid_G == 0 || av->k_g != 3) return rga_launch_knn(q, av->n_gauss, av->vt_pos, av->n_verts, av->k_g, av->knn_g, av->knn_d2, s);

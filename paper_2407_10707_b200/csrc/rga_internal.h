@@ -122,4 +122,5 @@ cudaError_t rga_launch_disp_mlp(rga_avatar* av, const rga_disp_mlp* m, const flo
 cudaError_t rga_launch_disp_apply(rga_avatar* av, cudaStream_t s);
 cudaError_t rga_build_knn_grid(rga_avatar* av, const float* aabb_host, cudaStream_t s);
 cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s);
+cudaError_t rga_launch_knn_verts(rga_avatar* av, float* d2, cudaStream_t s);
 int rga_mlp_init_attributes();
