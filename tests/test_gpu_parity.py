@@ -316,3 +316,34 @@ def test_gaussians_update_equals_a_fresh_load():
     rep = compare_all(inp2, av, img.cpu().numpy(), orc_av, o, 0)
     print(rep)
     av.close()
+
+
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_other_neighbour_counts_and_identity_texel_map(vis_mode, monkeypatch):
+    # K_g = 2 and K_v = 7 instead of the paper's 3 and 19 (brute-force KNN path, 7-bit majority filters), an 2x8 environment
+    # map whose texels ARE the 16 directions (texel_to_dir = NULL), 3 bones (a bone count that is not a multiple of 4)
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import compare_all
+    monkeypatch.setattr(orc, "K_G", 2); monkeypatch.setattr(orc, "K_V", 7)
+    inp = workloads.make(0, n_gauss=1500)
+    rs = np.random.default_rng(9)
+    inp["env"] = rs.uniform(0.0, 2.0, (1, 2, 8, 3)).astype(np.float32); inp["env_rows"], inp["env_cols"] = 2, 8
+    inp["texel_to_dir"] = np.arange(16, dtype=np.int32)
+    w = inp["vert_skin_w"]; w3 = np.concatenate([w * np.float32(0.5), w[:, :1] * np.float32(0.5) + w[:, 1:] * np.float32(0.5)], 1)
+    inp["vert_skin_w"] = np.ascontiguousarray(w3, np.float32)       # three bones; rows still sum to 1
+    inp["bone_mats"] = np.ascontiguousarray(np.concatenate([inp["bone_mats"], inp["bone_mats"][:, 1:2]], 1)); inp["n_bones"] = 3
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=vis_mode)
+    cam = inp["camera"]; W, H = cam["width"], cam["height"]
+    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=16, max_vis_res=64, max_env_texels=16, k_g=2, k_v=7)
+    img = torch.empty((H, W, 3), dtype=torch.float32, device="cuda")
+    rga.pose_skin(av.h, torch.as_tensor(inp["bone_mats"][0]).cuda())
+    rga.visibility_raster(av.h, torch.as_tensor(inp["vis_dirs"]).cuda(), 64, vis_mode, inp["depth_bias_texels"], inp["depth_bias_world"],
+                          inp["slope_max"], True)
+    rga.shade_gaussians(av.h, torch.as_tensor(inp["env"][0]).cuda(), inp["cam_pos"], None, inp["gamma"], True)
+    rga.splat_render(av.h, cam, inp["bg"], img)
+    rga.rga_check(av.h)
+    print(compare_all(inp, av, img.cpu().numpy(), orc_av, o, vis_mode))
+    av.close()
