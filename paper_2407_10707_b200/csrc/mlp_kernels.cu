@@ -16,8 +16,9 @@
 #define MLP_W 256              // layer width (UMMA N)
 #define MLP_KC 32              // weight chunk along K (four K = 8 instructions): every chunk costs ~1,000 cycles of
                                // barriers and fences whatever its size, so few large chunks beat many small ones
-#define MLP_NBUF 2             // weight chunk buffers (cp.async prefetch distance 1)
-#define MLP_PD (MLP_NBUF - 1)
+#define MLP_NBUF 6             // weight chunk buffers: the activations live in tensor memory, so shared memory is all theirs
+#define MLP_LAG 2              // a buffer is refilled two chunks after its MMAs were issued
+#define MLP_PD (MLP_NBUF - MLP_LAG)   // cp.async prefetch distance in chunks
 #define MLP_THREADS 256
 #define MLP_SBO 1024u          // 128-byte swizzle, K-major: an atom is 8 rows x 128 bytes (32 tf32), 8-row groups 1 KB apart
 #define MLP_ATOM_A (MLP_M * 128u)       // bytes between K atoms of the activation tile (128 rows x 128 bytes)
@@ -58,13 +59,29 @@ __global__ void __launch_bounds__(256) mlp_bias1_kernel(int K1, int n_pose, cons
   if (lane == 0) bias1[n] = b1[n] + acc;
 }
 
+// 32 consecutive fp32 columns of this thread's TMEM lane -> registers / registers -> TMEM
+#define TMEM_LD32(taddr, r)                                                                                                    \
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "                                                                     \
+               "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];" \
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), \
+                 "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), \
+                 "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), \
+                 "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])                                                              \
+               : "r"(taddr) : "memory")
+#define TMEM_ST32(taddr, r)                                                                                                    \
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "                                                               \
+               "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" \
+               :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), \
+                  "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), \
+                  "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), \
+                  "r"(r[30]), "r"(r[31]) : "memory")
+
 __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F, int n_pose, const float4* __restrict__ v_pos,
     const float* __restrict__ rff, const float* __restrict__ bias1, const float* __restrict__ W1,
     const float* __restrict__ Wh, const float* __restrict__ bh, const float* __restrict__ Wo, const float* __restrict__ bo,
     float4* __restrict__ v_disp) {
   extern __shared__ __align__(1024) unsigned char smem[];
-  unsigned char* sA = smem;                                          // 128 x 256 tf32, eight swizzled K atoms: 128 KB
-  unsigned char* sB = smem + (size_t)MLP_M * MLP_W * 4;               // MLP_NBUF x (256 x 32): 64 KB
+  unsigned char* sB = smem;                                           // MLP_NBUF x (256 x 32 tf32, swizzled): 6 x 32 KB
   float* sBias = reinterpret_cast<float*>(sB + (size_t)MLP_NBUF * MLP_CHUNK_BYTES);     // [4][256]
   float* sWo = sBias + 4 * MLP_W;                                     // [3][256]
   float* sRff = sWo + 3 * MLP_W;                                      // [F][3]
@@ -73,8 +90,8 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
   __shared__ uint32_t tmem_base_s;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int K1 = 2 * F, in1 = K1 + n_pose;
-  if (warp == 0) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "r"((uint32_t)MLP_W));
+  if (warp == 0) {                                                    // all 512 columns: accumulator [0,256), activations [256,512)
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "r"(512u));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (tid == 0) {
@@ -84,7 +101,7 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
   // chunk t of the whole network: layer, weight matrix and row stride, first column
   const int nch1 = K1 / MLP_KC, total = nch1 + 3 * (MLP_W / MLP_KC);
   constexpr int nchh = MLP_W / MLP_KC;
-  auto stage = [&](int t) {                                           // cp.async: 256 rows x 16 columns, 16 bytes per copy
+  auto stage = [&](int t) {                                           // cp.async: 256 rows x 32 columns, 16 bytes per copy
     const int layer = t < nch1 ? 0 : 1 + (t - nch1) / nchh, c = t < nch1 ? t : (t - nch1) % nchh;
     const float* Wl = layer == 0 ? W1 : Wh + (size_t)(layer - 1) * MLP_W * MLP_W;
     const int ldw = layer == 0 ? in1 : MLP_W;
@@ -106,39 +123,49 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
     for (int c = 0; c < 3; ++c) sWo[c * MLP_W + n] = Wo[c * MLP_W + n];
   }
   for (int i = tid; i < 3 * F; i += MLP_THREADS) sRff[i] = rff[i];
-  for (int t = 0; t < MLP_PD; ++t) stage(t);                          // the first weight chunk flies during the prologue
-  __syncthreads();
-  // layer-1 operand: gamma(x) = [sin(2 pi B x), cos(2 pi B x)] of the row's vertex; the two thread halves share the features
-  const int row = tid & (MLP_M - 1), half = tid >> 7;
-  const int v = blockIdx.x * MLP_M + row;
-  {
-    float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (v < nv) x = v_pos[v];
-    for (int f = half * (F / 2); f < (half + 1) * (F / 2); ++f) {
-      const float p = fmaf(sRff[3 * f + 2], x.z, fmaf(sRff[3 * f + 1], x.y, sRff[3 * f] * x.x));
-      // sin / cos of 2 pi p: the period is removed exactly (p - rint(p) is exact in fp32), then the MUFU approximations
-      // (absolute error ~1e-6, far below the TF32 rounding of the operand) -- sincospif cost 8,400 cycles per CTA here
-      float sn, cs;
-      __sincosf(6.283185307179586f * (p - rintf(p)), &sn, &cs);
-      *reinterpret_cast<float*>(sA + swz(row, f)) = sn;
-      *reinterpret_cast<float*>(sA + swz(row, F + f)) = cs;
-    }
-  }
-  const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(MLP_W >> 3) << 17) | ((uint32_t)(MLP_M >> 4) << 24);
-  uint32_t par_acc = 0u;
+  for (int t = 0; t < MLP_PD; ++t) stage(t);                          // the first weight chunks fly during the prologue
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;");
   const uint32_t tmem_base = tmem_base_s;
+  // Thread -> TMEM: warp w owns lanes 32 (w & 3) .. +31 (the tile's rows) and the column half w >> 2.
+  const int erow = (warp & 3) * 32 + lane, half = warp >> 2;
+  const uint32_t tlane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
+  const int v = blockIdx.x * MLP_M + erow;
+  // layer-1 operand: gamma(x) = [sin(2 pi B x), cos(2 pi B x)] of the row's vertex, straight into the activation columns
+  {
+    float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (v < nv) x = v_pos[v];
+    for (int f0 = half * (F / 2); f0 < (half + 1) * (F / 2); f0 += 8) {
+      uint32_t sn8[8], cs8[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int f = f0 + j;
+        const float p = fmaf(sRff[3 * f + 2], x.z, fmaf(sRff[3 * f + 1], x.y, sRff[3 * f] * x.x));
+        // sin / cos of 2 pi p: the period is removed exactly (p - rint(p) is exact in fp32), then the MUFU approximations
+        float sn, cs;
+        __sincosf(6.283185307179586f * (p - rintf(p)), &sn, &cs);
+        sn8[j] = __float_as_uint(sn); cs8[j] = __float_as_uint(cs);
+      }
+      asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                   :: "r"(tlane + 256u + (uint32_t)f0), "r"(sn8[0]), "r"(sn8[1]), "r"(sn8[2]), "r"(sn8[3]), "r"(sn8[4]), "r"(sn8[5]),
+                      "r"(sn8[6]), "r"(sn8[7]) : "memory");
+      asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                   :: "r"(tlane + 256u + (uint32_t)(F + f0)), "r"(cs8[0]), "r"(cs8[1]), "r"(cs8[2]), "r"(cs8[3]), "r"(cs8[4]), "r"(cs8[5]),
+                      "r"(cs8[6]), "r"(cs8[7]) : "memory");
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+  }
+  const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(MLP_W >> 3) << 17) | ((uint32_t)(MLP_M >> 4) << 24);
+  uint32_t par_acc = 0u;
   float out0 = 0.f, out1 = 0.f, out2 = 0.f;
 
   for (int t = 0; t < total; ++t) {
     const int layer = t < nch1 ? 0 : 1 + (t - nch1) / nchh, c = t < nch1 ? t : (t - nch1) % nchh;
     const int nchunks = layer == 0 ? nch1 : nchh;
-    // chunk t+1 goes into the buffer of chunk t-1 (its MMAs were issued an iteration ago) BEFORE chunk t is awaited, so
-    // every copy has a whole iteration to land
+    // chunk t+PD goes into the buffer of chunk t-LAG, whose MMAs were issued LAG iterations ago
     if (t + MLP_PD < total) {
-      if (t >= 1) mbar_wait(smem_u32(&bars[(t + MLP_PD) % MLP_NBUF]), (uint32_t)(((t - 1) / MLP_NBUF) & 1));
+      if (t >= MLP_LAG) mbar_wait(smem_u32(&bars[(t + MLP_PD) % MLP_NBUF]), (uint32_t)(((t - MLP_LAG) / MLP_NBUF) & 1));
       stage(t + MLP_PD);
     } else asm volatile("cp.async.commit_group;" ::: "memory");      // keeps the group count uniform
     asm volatile("cp.async.wait_group %0;" :: "n"(MLP_PD) : "memory");       // chunk t has landed (this thread's copies)
@@ -150,43 +177,30 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
       const uint32_t buf = smem_u32(sB + (size_t)(t % MLP_NBUF) * MLP_CHUNK_BYTES);
 #pragma unroll
       for (int j = 0; j < MLP_KC / 8; ++j) {
-        const uint64_t da = umma_desc(smem_u32(sA) + (uint32_t)c * MLP_ATOM_A + 32u * j);     // chunk c = K atom c; 32 bytes per K = 8
+        const uint32_t ta = tmem_base + 256u + (uint32_t)(c * MLP_KC + 8 * j);        // A from tensor memory: row = lane, K = column
         const uint64_t db = umma_desc(buf + 32u * j);
         const uint32_t acc = (c > 0 || j > 0) ? 1u : 0u;
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                     "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-                     :: "r"(tmem_base), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
+                     "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
+                     :: "r"(tmem_base), "r"(ta), "l"(db), "r"(idesc), "r"(acc) : "memory");
       }
       asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[t % MLP_NBUF])) : "memory");
       if (c == nchunks - 1)
         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&bars[MLP_NBUF])) : "memory");
     }
     if (c != nchunks - 1) continue;
-    // accumulator ready: every MMA of the layer has read its operands, so sA may be overwritten.  Warp w reads TMEM lanes
-    // 32 (w & 3) .. +31 (its row) and the column half w >> 2.
+    // accumulator ready: every MMA of the layer has read its A operand, so the activation columns may be overwritten
     mbar_wait(smem_u32(&bars[MLP_NBUF]), par_acc); par_acc ^= 1u;
     asm volatile("tcgen05.fence::after_thread_sync;");
     const float* bias = sBias + layer * MLP_W;
-    const int erow = (warp & 3) * 32 + lane;
-    for (int c0 = (warp >> 2) * (MLP_W / 2); c0 < (warp >> 2) * (MLP_W / 2) + MLP_W / 2; c0 += 32) {
+    for (int c0 = half * (MLP_W / 2); c0 < half * (MLP_W / 2) + MLP_W / 2; c0 += 32) {
       uint32_t r[32];
-      const uint32_t taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)c0;
-      asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-                   "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-                   : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
-                     "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
-                     "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
-                     "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-                   : "r"(taddr) : "memory");
+      TMEM_LD32(tlane + (uint32_t)c0, r);
       asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
       if (layer < 3) {
 #pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-          float4 h;
-          h.x = fmaxf(__uint_as_float(r[j]) + bias[c0 + j], 0.f);         h.y = fmaxf(__uint_as_float(r[j + 1]) + bias[c0 + j + 1], 0.f);
-          h.z = fmaxf(__uint_as_float(r[j + 2]) + bias[c0 + j + 2], 0.f); h.w = fmaxf(__uint_as_float(r[j + 3]) + bias[c0 + j + 3], 0.f);
-          *reinterpret_cast<float4*>(sA + swz(erow, c0 + j)) = h;
-        }
+        for (int j = 0; j < 32; ++j) r[j] = __float_as_uint(fmaxf(__uint_as_float(r[j]) + bias[c0 + j], 0.f));
+        TMEM_ST32(tlane + 256u + (uint32_t)c0, r);                     // the next layer's A operand never leaves tensor memory
       } else {                                                         // head: 256 -> 3, fp32 on the CUDA cores
 #pragma unroll
         for (int j = 0; j < 32; ++j) {
@@ -195,22 +209,21 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
         }
       }
     }
-    // (the next chunk's staging barrier orders these shared-memory writes and TMEM reads before the next layer's MMAs)
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    // (the next chunk's fence + barrier order these TMEM reads and writes before the next layer's MMAs)
   }
   // head: the lower column half adds the upper half's partial sums (fixed order: lower + upper)
-  const int erow = (warp & 3) * 32 + lane;
   if (warp >= 4) { sOut[3 * erow] = out0; sOut[3 * erow + 1] = out1; sOut[3 * erow + 2] = out2; }
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
-  const int ev = blockIdx.x * MLP_M + erow;
-  if (warp < 4 && ev < nv)
-    v_disp[ev] = make_float4((out0 + sOut[3 * erow]) + bo[0], (out1 + sOut[3 * erow + 1]) + bo[1], (out2 + sOut[3 * erow + 2]) + bo[2], 0.f);
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"((uint32_t)MLP_W));
+  if (warp < 4 && v < nv)
+    v_disp[v] = make_float4((out0 + sOut[3 * erow]) + bo[0], (out1 + sOut[3 * erow + 1]) + bo[1], (out2 + sOut[3 * erow + 2]) + bo[2], 0.f);
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"(512u));
 }
 
 size_t rga_mlp_smem(int F) {
   (void)F;
-  return (size_t)MLP_M * MLP_W * 4 + (size_t)MLP_NBUF * MLP_CHUNK_BYTES + (size_t)(4 + 3) * MLP_W * 4 + (size_t)3 * 128 * 4 + (size_t)3 * MLP_M * 4 + 64;
+  return (size_t)MLP_NBUF * MLP_CHUNK_BYTES + (size_t)(4 + 3) * MLP_W * 4 + (size_t)3 * 128 * 4 + (size_t)3 * MLP_M * 4 + 64;
 }
 
 int rga_mlp_init_attributes() {
