@@ -108,7 +108,8 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
     unsigned char* buf = sB + (size_t)(t % MLP_NBUF) * MLP_CHUNK_BYTES;
     // 16-byte piece q of the chunk in shared-memory order (destination 16 q: conflict-free): row r = (q >> 3) & 7 of row
     // group g = q >> 6, physical slot q & 7 of the row, which holds K piece (q & 7) ^ r; a warp reads 4 rows x 128 bytes
-    for (int q = tid; q < MLP_W * MLP_KC / 4; q += MLP_THREADS) {
+    // (warps 0..6 stage; warp 7 issues the MMAs and stays off the staging path)
+    for (int q = tid; q < MLP_W * MLP_KC / 4 && tid < MLP_THREADS - 32; q += MLP_THREADS - 32) {
       const int r = (q >> 3) & 7, n = ((q >> 6) << 3) | r, kq = (q & 7) ^ r;
       const float* src = Wl + (size_t)n * ldw + c * MLP_KC + 4 * kq;
       const uint32_t dst = smem_u32(buf) + 16u * (uint32_t)q;
@@ -172,7 +173,7 @@ __global__ void __launch_bounds__(MLP_THREADS, 1) disp_mlp_kernel(int nv, int F,
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy writes -> the tensor core's async proxy
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
-    if (tid == 0) {
+    if (tid == MLP_THREADS - 32) {
       asm volatile("tcgen05.fence::after_thread_sync;");
       const uint32_t buf = smem_u32(sB + (size_t)(t % MLP_NBUF) * MLP_CHUNK_BYTES);
 #pragma unroll
