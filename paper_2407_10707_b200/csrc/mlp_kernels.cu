@@ -2,13 +2,14 @@
 // layers, each with a width of 256 and activated by ReLU", "Random Fourier Features"; readings A26-A28) -- the
 // one dense contraction of the method, so it runs on the 5th-generation tensor cores:
 //   tcgen05.mma kind::tf32, M = 128 vertices per CTA, N = 256 = the layer width, K = 8 per instruction, issued by one
-//   thread; A (activations) and B (weights) in shared memory in the K-major 128-byte-swizzle layout (8-row x 128-byte
-//   atoms); the fp32 accumulator (128 lanes x 256 columns) in tensor memory, read back with tcgen05.ld for the
-//   bias + ReLU epilogue, which writes the next layer's A operand straight back into shared memory.
-// All four hidden layers and the 256 -> 3 head run in one kernel: activations never leave the SM.
-// Weights stream from L2 in 256 x 32 chunks through two cp.async buffers; a chunk's buffer is released by tcgen05.commit
-// on an mbarrier.  theta is the same for every vertex, so its part of layer 1 is folded into
-// that layer's bias once per call (mlp_bias1_kernel).
+//   thread (warp 7, which does nothing else in the main loop).  The activations never leave TENSOR MEMORY: columns
+//   [256, 512) hold the A operand (row = lane, K = column; the "TS" form of the instruction), columns [0, 256) the fp32
+//   accumulator; the epilogue reads the accumulator with tcgen05.ld, applies bias + ReLU and writes the next layer's A
+//   operand back with tcgen05.st.  Shared memory therefore belongs to the weights: six 256 x 32 chunk buffers in the
+//   K-major 128-byte-swizzle layout (8-row x 128-byte atoms), filled by cp.async four chunks ahead and released by
+//   tcgen05.commit on an mbarrier.
+// All four hidden layers and the 256 -> 3 head run in one kernel.  theta is the same for every vertex, so its part of
+// layer 1 is folded into that layer's bias once per call (mlp_bias1_kernel).
 // FAST file: the result is compared with the fp64 oracle under the TF32 tolerance derived in DESIGN.md.
 #include "rga_internal.h"
 
@@ -21,7 +22,6 @@
 #define MLP_PD (MLP_NBUF - MLP_LAG)   // cp.async prefetch distance in chunks
 #define MLP_THREADS 256
 #define MLP_SBO 1024u          // 128-byte swizzle, K-major: an atom is 8 rows x 128 bytes (32 tf32), 8-row groups 1 KB apart
-#define MLP_ATOM_A (MLP_M * 128u)       // bytes between K atoms of the activation tile (128 rows x 128 bytes)
 #define MLP_CHUNK_BYTES (MLP_W * MLP_KC * 4)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -39,13 +39,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   while (!done)
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                  : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-}
-
-// offset of element (row r, column k) of the activation tile: K atom k / 32, 8-row group r / 8, row r % 8 (128 bytes), and the
-// 16-byte piece (k % 32) / 4 XOR-swizzled with the row (Swizzle<3,4,3>)
-__device__ __forceinline__ uint32_t swz(int r, int k) {
-  return (uint32_t)(k >> 5) * MLP_ATOM_A + (uint32_t)(r >> 3) * MLP_SBO + (uint32_t)(r & 7) * 128u +
-         ((((uint32_t)(k >> 2) & 7u) ^ (uint32_t)(r & 7)) << 4) + (uint32_t)(k & 3) * 4u;
 }
 
 // theta is the same for every vertex: its columns of W1 are folded into layer 1's bias once per call, one warp per row
