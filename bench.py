@@ -283,7 +283,7 @@ def main():
     tf32_peak = pk.get("bf16_tflops", 1590.0) * (1.1 / 2.25)          # measured bf16 peak x the guide's nominal tf32 : bf16 ratio
     mlp_obj = {"kernel": "disp_mlp", "bound": "tensor", "ms": mlp_ms, "achieved": mlp_flop / (mlp_ms * 1e-3) / 1e12, "peak": tf32_peak,
                "unit": "TFLOP/s", "frac": mlp_flop / (mlp_ms * 1e-3) / 1e12 / tf32_peak, "dtype": "tf32 operands, f32 accumulate",
-               "vertices": nvv, "note": "one CTA per 128 vertices (54 CTAs at config 1), all four layers and the head fused; profiles/r01e_mlp.md"}
+               "vertices": nvv, "note": "one CTA per 128 vertices (54 CTAs at config 1), all four layers and the head fused; profiles/r01g_mlp.md"}
     # (the avatar now carries the network's displacement; it is not rendered again and is closed below)
 
     # per-frame KNN + Eq.1 re-interpolation for moved Gaussians (the paper's KNN step: 0.93 ms per frame
