@@ -219,6 +219,53 @@ def disp_mlp(x, theta, m):
     return h @ np.asarray(m["Wo"], np.float64).T + np.asarray(m["bo"], np.float64)
 
 
+def densify_density(knn_g, faces, vert_pos, d0, p0, rnd):
+    """Algorithm 1, "Gaussian densification based on density" (text :475-479 and :173), step by step
+    in the paper's order and names.  knn_g: S_g [N_g, K_g]; faces [N_f, 3]; vert_pos [N_v, 3] canonical x; rnd: uint32
+    [3 * n] raw random numbers drawn by the caller (one for the multinomial draw, two for the placement of each added
+    Gaussian); at most len(rnd) // 3 Gaussians are produced.
+    Readings (A29-A31): d_f and P are fp32; the multinomial sample is n draws by inverse CDF over P held in
+    fixed point (P * 2^16 rounded to nearest), so that sums are exact integers: N' = floor(sum(P) * p0), draw j picks the
+    first triangle whose running sum exceeds floor(rnd[3j] / 2^32 * sum); "randomly add on the triangle" = the uniform
+    barycentric map (1 - sqrt(r1), sqrt(r1)(1 - r2), sqrt(r1) r2) with r = (rnd >> 8) / 2^24.
+    Returns dict: D_v int32 [N_v], P_fix uint32 [N_f], n_add (N'), tri int32 [n], n_g int32 [N_f] (histogram of tri),
+    pos float32 [n, 3]."""
+    knn_g = np.asarray(knn_g); faces = np.asarray(faces); x = _f32(vert_pos)
+    rnd = np.asarray(rnd, dtype=np.uint32)
+    N_v, N_f, K_g = len(x), len(faces), knn_g.shape[1]
+    # "for Gaussian index i: for vertex index k in S_g^i: D_v[k] += 1"
+    D_v = np.zeros(N_v, np.int64)
+    np.add.at(D_v, knn_g.reshape(-1), 1)
+    # "for triangle index i: for vertex index k in f^i: d_f[i] += D_v[k];  d_f[i] /= (6 x K_g)"
+    d_f = np.zeros(N_f, np.float32)
+    for c in range(3):
+        d_f = d_f + D_v[faces[:, c]].astype(np.float32)            # integers < 2^24: exact in fp32
+    d_f = d_f / np.float32(6 * K_g)
+    # "P = max(0, d_0 - d_f)"
+    P = np.maximum(np.float32(0.0), np.float32(d0) - d_f)
+    P_fix = np.rint(P.astype(np.float64) * 65536.0).astype(np.uint64)
+    total = int(P_fix.sum())
+    # "N_g' = sum(P) x p_0"
+    n_add = int(np.floor(float(total) * float(np.float32(p0)) / 65536.0))
+    n = min(n_add, len(rnd) // 3)
+    # "n_g = MultinomialSample(P / sum(P), N_g')"
+    cdf = np.cumsum(P_fix)
+    tri = np.empty(n, np.int32)
+    for j in range(n):
+        target = (int(rnd[3 * j]) * total) >> 32
+        tri[j] = int(np.searchsorted(cdf, np.uint64(target), side="right"))
+    n_g = np.bincount(tri, minlength=N_f).astype(np.int32)
+    # "randomly add n_g[i] Gaussians on the i-th triangle"
+    r1 = (rnd[1:3 * n:3] >> np.uint32(8)).astype(np.float32) * np.float32(2.0 ** -24)
+    r2 = (rnd[2:3 * n:3] >> np.uint32(8)).astype(np.float32) * np.float32(2.0 ** -24)
+    sq = np.sqrt(r1)
+    b0 = np.float32(1.0) - sq; b1 = sq * (np.float32(1.0) - r2); b2 = sq * r2
+    f = faces[tri]
+    pos = (b0[:, None] * x[f[:, 0]] + b1[:, None] * x[f[:, 1]]) + b2[:, None] * x[f[:, 2]]
+    return {"D_v": D_v.astype(np.int32), "P_fix": P_fix.astype(np.uint32), "n_add": n_add, "tri": tri, "n_g": n_g,
+            "pos": pos.astype(np.float32)}
+
+
 def avatar_load(inp):
     """L0: KNN sets S_g, S_v and Eq.1 interpolation of the pose-independent attributes."""
     av = {}

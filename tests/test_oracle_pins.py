@@ -450,3 +450,85 @@ def test_disp_mlp_relu_and_affine_regime():
     Bm = np.zeros_like(m64["rff"]); Bm[:, 0] = np.arange(1, 65)            # integer frequencies along x
     per = dict(m64); per["rff"] = Bm
     assert np.allclose(orc.disp_mlp(x, m64["theta"], per), orc.disp_mlp(x + np.array([1.0, 0.3, -2.0]), m64["theta"], per), atol=1e-9)
+
+
+# ------------------------------------------------------------------ Algorithm 1: density-based densification
+def _tiny_densify_case():
+    # a strip of 4 triangles over 6 vertices; 5 Gaussians with hand-written K_g = 3 neighbour sets
+    x = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [1, 1, 0], [0, 2, 0], [1, 2, 0]], np.float32)
+    faces = np.array([[0, 1, 2], [1, 3, 2], [2, 3, 4], [3, 5, 4]], np.int32)
+    knn = np.array([[0, 1, 2], [0, 1, 2], [1, 2, 3], [0, 2, 1], [2, 1, 0]], np.int32)
+    return x, faces, knn
+
+
+def test_densify_hand_example_counts_density_and_budget():
+    # PAPER.md:489-503 by hand.  D_v = occurrences of each vertex in S_g: v0 4, v1 5, v2 5, v3 1, v4 0, v5 0.
+    # d_f = (sum of the three D_v) / (6 K_g = 18): 14/18, 11/18, 6/18, 1/18.  With d_0 = 1: P = 4/18, 7/18, 12/18, 17/18,
+    # sum(P) = 40/18; N' = floor(sum(P) p_0) = floor(2.222 * 0.9) = 2 (the algorithm's "sum(P) x p_0").
+    x, faces, knn = _tiny_densify_case()
+    rnd = np.zeros(3 * 8, np.uint32)
+    r = orc.densify_density(knn, faces, x, 1.0, 0.9, rnd)
+    assert r["D_v"].tolist() == [4, 5, 5, 1, 0, 0]
+    assert r["D_v"].sum() == knn.size                                      # every (Gaussian, neighbour) pair counted once
+    assert np.allclose(r["P_fix"] / 65536.0, np.array([4, 7, 12, 17]) / 18.0, atol=2.0 ** -17)
+    assert r["n_add"] == 2 and len(r["tri"]) == 2 and r["n_g"].sum() == 2
+    # a triangle at or above the threshold gets probability 0 ("below d_0")
+    r = orc.densify_density(knn, faces, x, 0.5, 0.9, rnd)
+    assert r["P_fix"][0] == 0 and r["P_fix"][1] == 0 and r["P_fix"][2] > 0
+    # "we need a total of sum(P) Gaussians ... but only add a small percent p_0" (:477): p_0 = 1 asks for floor(sum(P))
+    assert orc.densify_density(knn, faces, x, 1.0, 1.0, rnd)["n_add"] == 2
+    assert orc.densify_density(knn, faces, x, 4.0, 1.0, rnd)["n_add"] == int(np.floor(4 * 4 - 32 / 18.0))
+
+
+def test_densify_multinomial_extremes_and_frequencies():
+    x, faces, knn = _tiny_densify_case()
+    n = 40000
+    # inverse CDF end points: u = 0 picks the first triangle with P > 0, u -> 1 the last
+    lo = np.zeros(3 * 4, np.uint32); hi = np.full(3 * 4, 2 ** 32 - 1, np.uint32)
+    assert set(orc.densify_density(knn, faces, x, 1.0, 1.9, lo)["tri"].tolist()) == {0}
+    assert set(orc.densify_density(knn, faces, x, 1.0, 1.9, hi)["tri"].tolist()) == {3}
+    assert set(orc.densify_density(knn, faces, x, 0.5, 5.0, lo)["tri"].tolist()) == {2}     # triangles 0, 1 have P = 0
+    # frequencies follow P / sum(P) (multinomial): chi-square against the hand-computed P
+    rnd = np.random.default_rng(3).integers(0, 2 ** 32, size=3 * n, dtype=np.uint64).astype(np.uint32)
+    r = orc.densify_density(knn, faces, x, 1.0, 1e9, rnd)           # budget far above n: all n draws are made
+    assert len(r["tri"]) == n and r["n_g"].sum() == n
+    assert np.array_equal(r["n_g"], np.bincount(r["tri"], minlength=4))
+    expect = n * np.array([4, 7, 12, 17]) / 40.0
+    chi2 = (((r["n_g"] - expect) ** 2) / expect).sum()
+    assert chi2 < 25.0                                                # 3 dof: P(chi2 > 25) ~ 1.5e-5
+
+
+def test_densify_placement_is_uniform_on_the_triangle():
+    # one triangle, no Gaussians anywhere: all draws land on it; the points are uniform over its area (:479 "randomly
+    # place").  Uniform-on-triangle moments: E[b_i] = 1/3, E[b_i^2] = 1/6, E[b_i b_j] = 1/12.
+    x = np.array([[0.2, 0.1, 0.3], [1.3, 0.4, -0.2], [0.1, 1.7, 0.9]], np.float32)
+    faces = np.array([[0, 1, 2]], np.int32)
+    knn = np.zeros((0, 3), np.int32)
+    n = 60000
+    rnd = np.random.default_rng(4).integers(0, 2 ** 32, size=3 * n, dtype=np.uint64).astype(np.uint32)
+    r = orc.densify_density(knn, faces, x, 1.0, 1e9, rnd)
+    assert len(r["pos"]) == n and np.all(r["tri"] == 0)
+    A = np.concatenate([x.astype(np.float64).T, np.ones((1, 3))], 0)          # solve for barycentric coordinates
+    b = np.linalg.lstsq(A, np.concatenate([r["pos"].astype(np.float64).T, np.ones((1, n))], 0), rcond=None)[0].T
+    assert b.min() > -1e-6 and np.allclose(b.sum(1), 1.0, atol=1e-6)          # inside the triangle, on its plane
+    assert np.allclose(b.mean(0), 1 / 3, atol=4e-3)
+    assert np.allclose((b ** 2).mean(0), 1 / 6, atol=4e-3)
+    assert np.allclose([(b[:, 0] * b[:, 1]).mean(), (b[:, 0] * b[:, 2]).mean(), (b[:, 1] * b[:, 2]).mean()], 1 / 12, atol=4e-3)
+    # corners of the random square map to corners / edges of the triangle
+    c = orc.densify_density(knn, faces, x, 1.0, 1e9, np.array([0, 0, 0, 0, 2 ** 32 - 1, 0], np.uint32))["pos"]
+    assert np.allclose(c[0], x[0]) and np.allclose(c[1], x[1], atol=1e-3)
+
+
+def test_densify_uniform_density_closed_form():
+    # regular situation the algorithm's "each vertex is connected with 6 triangles" assumes (:497): every vertex has the
+    # same count D -> d_f = 3 D / (6 K_g) = D / (2 K_g) on every triangle, N' = floor(N_f (d_0 - D / (2 K_g)) p_0)
+    ico = smesh.icosphere(2)
+    x, faces = ico[0], ico[1]
+    nv = len(x)
+    D, Kg = 2, 3
+    knn = np.stack([np.repeat(np.arange(nv), D)] * 3, 1).astype(np.int32)  # N_g = D N_v rows (k, k, k): D_v = 3 D
+    r = orc.densify_density(knn, faces, x, 2.0, 0.25, np.zeros(3, np.uint32))
+    assert np.all(r["D_v"] == 3 * D)
+    d_f = 3 * (3 * D) / (6.0 * Kg)
+    assert np.allclose(r["P_fix"] / 65536.0, 2.0 - d_f, atol=2.0 ** -16)
+    assert r["n_add"] == int(np.floor(len(faces) * (2.0 - d_f) * 0.25))
