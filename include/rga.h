@@ -133,6 +133,20 @@ RGA_API rga_status splat_render(rga_avatar* av, const rga_camera* cam, const flo
  * scale and opacity are kept.  gauss_pos: dev [n_gauss][3].  Enqueue-only; call pose_skin afterwards. */
 RGA_API rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, void* stream);
 
+/* Algorithm 1, "Gaussian densification based on density": from the avatar's current
+ * S_g (avatar_load / gaussians_update) and its mesh, counts the Gaussians near every vertex (D_v), estimates the Gaussian
+ * density of every triangle d_f = sum of its three D_v / (6 K_g), sets P = max(0, d0 - d_f), asks for
+ * N' = floor(sum(P) * p0) new Gaussians, draws their triangles by multinomial sampling from P / sum(P) and places each
+ * uniformly at random on its triangle of the CANONICAL mesh.  The paper's values are d0 = 1, p0 = 0.02.
+ * The random numbers are the caller's: rnd, dev uint32 [3 * max_out], raw 32-bit draws -- rnd[3j] picks the triangle of
+ * new Gaussian j (inverse CDF), rnd[3j+1] and rnd[3j+2] place it (readings A29-A31 fix the arithmetic).
+ * out_pos: dev f32 [max_out][3]; out_tri: dev i32 [max_out] or NULL; out_count: dev i32 [1] or NULL, receives N'.
+ * min(N', max_out) entries are written, in draw order.  D_v, P, n_g and {sum(P), N'} stay readable through
+ * rga_get_buffer (RGA_BUF_DENS_*).  Enqueue-only; the avatar itself is not changed: append the positions to the
+ * Gaussian set and load (or gaussians_update) again.  Requires 0 < d0 <= 32768 and p0 >= 0. */
+RGA_API rga_status densify_density(rga_avatar* av, float d0, float p0, const uint32_t* rnd, int max_out, float* out_pos,
+                                   int32_t* out_tri, int32_t* out_count, void* stream);
+
 /* Displacement network d(x, theta): dx_i = MLP([gamma(x_i), theta]) for every canonical vertex, with
  * gamma(x) = [sin(2 pi B x), cos(2 pi B x)] (random Fourier features, B = rff), four hidden layers of width 256 with ReLU
  * and a linear 256 -> 3 head (readings A26-A28).  Runs on the tensor cores (tcgen05, TF32 operands, fp32
@@ -202,7 +216,11 @@ typedef enum {
   RGA_BUF_N_CONTRIB = 27,     /* u32 [height][width]                                 */
   RGA_BUF_VERT_BITS_RAW = 28, /* u32 [n_verts][ceil(n_dirs/32)] raw vertex visibility (mode 1) */
   RGA_BUF_VERT_DISP = 29,     /* f32 [n_verts][4] per-pose displacement of displacement_mlp (xyz, w unused) */
-  RGA_BUF_COUNT_ = 30
+  RGA_BUF_DENS_DV = 30,       /* i32 [n_verts]  Algorithm 1: Gaussians near each vertex              */
+  RGA_BUF_DENS_P = 31,        /* u32 [n_faces]  P = max(0, d0 - d_f) in fixed point (P * 2^16)         */
+  RGA_BUF_DENS_NG = 32,       /* i32 [n_faces]  Gaussians added per triangle by the last call          */
+  RGA_BUF_DENS_HDR = 33,      /* u64 [2]        sum of the fixed-point P, N'                            */
+  RGA_BUF_COUNT_ = 34
 } rga_buffer_id;
 
 /* Returns the device pointer and current size in bytes of an internal buffer (valid until the next call that

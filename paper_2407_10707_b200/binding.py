@@ -15,12 +15,13 @@ RGA_OK, RGA_ERR_INVALID_ARG, RGA_ERR_CUDA, RGA_ERR_OOM, RGA_ERR_STATE, RGA_ERR_C
 BUF = dict(KNN_G=0, UBAR_G=1, KNN_V=2, GAUSS_STATIC=3, GAUSS_SKIN_W=4, VERT_POSED=5, VERT_NORMAL_POSED=6, GAUSS_POSED=7,
            GAUSS_NORMAL_POSED=8, GAUSS_COV=9, WINDOW=10, ZMAP=11, IDMAP=12, VISBITS=13, VCOUNT=14, RADIANCE=15, COLOR=16,
            MU2D=17, DEPTH=18, CONIC_OPACITY=19, RECT=20, TOUCHED=21, NUM_DUPLICATES=22, KEYS_SORTED=23, VALS_SORTED=24,
-           TILE_RANGES=25, T_FINAL=26, N_CONTRIB=27, VERT_BITS_RAW=28, VERT_DISP=29)
+           TILE_RANGES=25, T_FINAL=26, N_CONTRIB=27, VERT_BITS_RAW=28, VERT_DISP=29,
+           DENS_DV=30, DENS_P=31, DENS_NG=32, DENS_HDR=33)
 _BUF_DTYPE = {0: np.int32, 1: np.float32, 2: np.int32, 3: np.float32, 4: np.float32, 5: np.float32, 6: np.float32,
               7: np.float32, 8: np.float32, 9: np.float32, 10: np.float32, 11: np.uint32, 12: np.int32, 13: np.uint32,
               14: np.uint8, 15: np.float32, 16: np.float32, 17: np.float32, 18: np.float32, 19: np.float32, 20: np.int32,
               21: np.uint32, 22: np.uint32, 23: np.uint64, 24: np.uint32, 25: np.uint32, 26: np.float32, 27: np.uint32,
-              28: np.uint32, 29: np.float32}
+              28: np.uint32, 29: np.float32, 30: np.int32, 31: np.uint32, 32: np.int32, 33: np.uint64}
 
 
 class RgaError(RuntimeError):
@@ -175,6 +176,17 @@ def gaussians_update(h, gauss_pos):
     """Per-frame KNN + Eq.1 re-interpolation for moved Gaussians (include/rga.h gaussians_update)."""
     lib().gaussians_update.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     _chk(lib().gaussians_update(h, _ptr(gauss_pos), _stream()))
+
+
+def densify_density(h, d0, p0, rnd, out_pos, out_tri=None, out_count=None):
+    """Algorithm 1, density-based densification (include/rga.h densify_density).  rnd: CUDA int32/uint32 tensor [3 * max_out]
+    of raw 32-bit random numbers; out_pos: CUDA float32 [max_out, 3]; out_tri / out_count: CUDA int32 [max_out] / [1] or None."""
+    max_out = int(out_pos.shape[0]) if out_pos is not None else 0
+    if max_out and rnd.numel() < 3 * max_out:
+        raise ValueError("densify_density: rnd needs 3 numbers per output row")
+    lib().densify_density.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                      C.c_void_p]
+    _chk(lib().densify_density(h, float(d0), float(p0), _ptr(rnd), max_out, _ptr(out_pos), _ptr(out_tri), _ptr(out_count), _stream()))
 
 
 class _DispMlp(C.Structure):

@@ -56,7 +56,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
+  void* ptrs[] = {av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
                   av->vt_spec, av->knn_d2, av->grid_start, av->grid_verts, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
@@ -113,6 +113,8 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   float* d2 = nullptr;
 #define A(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, \
     "avatar_load: %s: %s", #call, cudaGetErrorString(e_)); goto done; } } while (0)
+  A(dalloc(&av->dens_dv, nv)); A(dalloc(&av->dens_pfix, (size_t)av->n_faces)); A(dalloc(&av->dens_cdf, (size_t)av->n_faces));
+  A(dalloc(&av->dens_ng, (size_t)av->n_faces)); A(dalloc(&av->dens_block, (size_t)av->n_faces / 2048 + 1)); A(dalloc(&av->dens_hdr, 2));
   A(dalloc(&av->v_pos, nv)); A(dalloc(&av->v_disp, nv)); A(dalloc(&av->g_pos, ng)); A(dalloc(&av->mlp_bias1, 256));
   A(dalloc(&av->v_xbar, nv)); A(dalloc(&av->v_normal, nv)); A(dalloc(&av->v_skin_w, nv * B)); A(dalloc(&av->faces, 3 * (size_t)av->n_faces)); A(dalloc(&av->faces_packed, (size_t)av->n_faces));
   A(dalloc(&av->knn_v, nv * av->k_v)); A(dalloc(&av->knn_g, ng * av->k_g)); A(dalloc(&av->ubar_g, ng * av->k_g));
@@ -263,6 +265,18 @@ extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, v
   return RGA_OK;
 }
 
+extern "C" rga_status densify_density(rga_avatar* av, float d0, float p0, const uint32_t* rnd, int max_out, float* out_pos,
+                                      int32_t* out_tri, int32_t* out_count, void* stream) {
+  if (!av) return fail(RGA_ERR_INVALID_ARG, "densify_density: null avatar");
+  if (!(d0 > 0.0f) || d0 > 32768.0f || !(p0 >= 0.0f)) return fail(RGA_ERR_INVALID_ARG, "densify_density: need 0 < d0 <= 32768 and p0 >= 0");
+  if (max_out < 0 || (max_out > 0 && (!rnd || !out_pos))) return fail(RGA_ERR_INVALID_ARG, "densify_density: max_out > 0 needs rnd and out_pos");
+  if (av->n_faces < 1) return fail(RGA_ERR_INVALID_ARG, "densify_density: the avatar has no triangles");
+  cudaStream_t s = (cudaStream_t)stream;
+  rga_prof_mark(av, "-", s);
+  CU(rga_launch_densify(av, d0, p0, rnd, max_out, out_pos, out_tri, out_count, s));
+  return RGA_OK;
+}
+
 extern "C" rga_status displacement_mlp(rga_avatar* av, const rga_disp_mlp* mlp, const float* theta, void* stream) {
   if (!av || !mlp || !theta || !mlp->rff || !mlp->W1 || !mlp->b1 || !mlp->Wh || !mlp->bh || !mlp->Wo || !mlp->bo)
     return fail(RGA_ERR_INVALID_ARG, "displacement_mlp: null argument");
@@ -406,6 +420,10 @@ extern "C" rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, co
     case RGA_BUF_N_CONTRIB: p = av->n_contrib; n = npix * 4; break;
     case RGA_BUF_VERT_BITS_RAW: p = av->vbits_raw; n = nv * words * 4; break;
     case RGA_BUF_VERT_DISP: p = av->v_disp; n = nv * 16; break;
+    case RGA_BUF_DENS_DV: p = av->dens_dv; n = nv * 4; break;
+    case RGA_BUF_DENS_P: p = av->dens_pfix; n = (size_t)av->n_faces * 4; break;
+    case RGA_BUF_DENS_NG: p = av->dens_ng; n = (size_t)av->n_faces * 4; break;
+    case RGA_BUF_DENS_HDR: p = av->dens_hdr; n = 16; break;
     default: return fail(RGA_ERR_INVALID_ARG, "rga_get_buffer: unknown id %d", which);
   }
   *dev_ptr = p; *bytes = n;

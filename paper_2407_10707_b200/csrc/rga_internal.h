@@ -25,6 +25,8 @@ struct rga_avatar {
   float* knn_d2;       // [n_gauss][k_g] squared distances of the last Gaussian KNN
   // uniform grid over the canonical vertices (exact KNN of the Gaussians); grid_G == 0: brute force
   int grid_G; float grid_h, grid_o[3]; unsigned* grid_start; int* grid_verts;
+  // Algorithm 1 (density-based densification): D_v, P in fixed point, its running sum, n_g, per-tile sums, {sum, N'}
+  int* dens_dv; unsigned* dens_pfix; unsigned long long* dens_cdf; int* dens_ng; unsigned long long* dens_block; unsigned long long* dens_hdr;
   float* mlp_bias1;    // [256] layer-1 bias of the displacement network with the pose folded in
   float4* v_xbar;      // [n_verts]  x + dx
   float4* v_normal;    // [n_verts]
@@ -124,3 +126,6 @@ cudaError_t rga_build_knn_grid(rga_avatar* av, const float* aabb_host, cudaStrea
 cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s);
 cudaError_t rga_launch_knn_verts(rga_avatar* av, float* d2, cudaStream_t s);
 int rga_mlp_init_attributes();
+// densify_kernels.cu
+cudaError_t rga_launch_densify(rga_avatar* av, float d0, float p0, const unsigned* rnd, int max_out, float* out_pos, int* out_tri,
+                               int* out_count, cudaStream_t s);

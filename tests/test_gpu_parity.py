@@ -347,3 +347,48 @@ def test_other_neighbour_counts_and_identity_texel_map(vis_mode, monkeypatch):
     rga.rga_check(av.h)
     print(compare_all(inp, av, img.cpu().numpy(), orc_av, o, vis_mode))
     av.close()
+
+
+@pytest.mark.parametrize("cfg,n_gauss,d0,p0", [(0, 2000, 1.0, 0.02), (0, 2000, 6.0, 0.5), (1, 100_000, 1.0, 0.02), (1, 100_000, 12.0, 0.25),
+                                               (2, 100_000, 1.0, 0.02)])
+def test_densify_density_matches_algorithm_1(cfg, n_gauss, d0, p0):
+    # SURVEY 8(f) item 4, Algorithm 1: D_v, P (fixed point), N', the drawn triangles, n_g and the
+    # placed positions are all bit-exact (integers; positions are contract-order fp32).  (d0, p0) = (1, 0.02) are the paper's;
+    # the larger pairs make tens of thousands of draws; config 2 is the paper-sized mesh (40k vertices / 80k triangles).
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    inp = workloads.make(cfg, n_gauss=n_gauss)
+    cam = inp["camera"]
+    av = rga.Avatar(inp, max_width=cam["width"], max_height=cam["height"], max_vis_dirs=16, max_vis_res=32, max_env_texels=512)
+    knn_g = av.read("KNN_G").reshape(-1, 3)
+    max_out = 70_000
+    rnd = np.random.default_rng(77 + cfg).integers(0, 2 ** 32, size=3 * max_out, dtype=np.uint64).astype(np.uint32)
+    ref = orc.densify_density(orc.avatar_load(inp)["knn_g"], inp["faces"], inp["vert_pos"], d0, p0, rnd)
+    assert np.array_equal(knn_g, orc.avatar_load(inp)["knn_g"])
+    d_rnd = torch.as_tensor(rnd.view(np.int32)).cuda()
+    pos = torch.full((max_out, 3), float("nan"), dtype=torch.float32, device="cuda")
+    tri = torch.full((max_out,), -1, dtype=torch.int32, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int32, device="cuda")
+    rga.densify_density(av.h, d0, p0, d_rnd, pos, tri, cnt)
+    rga.rga_check(av.h)
+    n_add = int(cnt.item())
+    hdr = av.read("DENS_HDR")
+    assert n_add == ref["n_add"] and int(hdr[1]) == n_add and int(hdr[0]) == int(ref["P_fix"].astype(np.uint64).sum())
+    n = min(n_add, max_out)
+    assert n == len(ref["tri"])
+    if (d0, p0) != (1.0, 0.02):
+        assert n > 2000                                                    # the big cases do exercise the sampler
+    assert np.array_equal(av.read("DENS_DV"), ref["D_v"])
+    assert np.array_equal(av.read("DENS_P"), ref["P_fix"])
+    assert np.array_equal(tri.cpu().numpy()[:n], ref["tri"])
+    assert np.all(tri.cpu().numpy()[n:] == -1)                             # nothing written past the count
+    assert np.array_equal(av.read("DENS_NG"), ref["n_g"])
+    assert np.array_equal(pos.cpu().numpy()[:n].view(np.uint32), ref["pos"].view(np.uint32))
+    # a second call with a smaller output capacity writes only that many, in the same order
+    pos2 = torch.zeros((max(n // 2, 1), 3), dtype=torch.float32, device="cuda")
+    rga.densify_density(av.h, d0, p0, d_rnd, pos2, None, None)
+    m = min(n, len(pos2))
+    assert np.array_equal(pos2.cpu().numpy()[:m].view(np.uint32), ref["pos"][:m].view(np.uint32))
+    assert av.read("DENS_NG").sum() == m
+    av.close()
