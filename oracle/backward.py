@@ -1,0 +1,124 @@
+"""Oracle of the splat's backward pass ("backward of H5-H10").  TEST INFRASTRUCTURE ONLY: imported
+by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline legs; never by the product package.
+
+The definition: the gradient of  L = sum_p <G(p), I(p)>  (G = dL/dimage, given) where I is the forward image of H6 + H10
+(defers to 3DGS [8] :338; readings A16-A21) with its discrete decisions FROZEN -- the tile
+lists and their order (H7-H9), which Gaussians are culled (near plane, facing away :101, degenerate footprint), and per
+(pixel, entry) the skips (power > 0, alpha < 1/255) and the stopping rule (T < 1e-4).  Written as the forward in plain
+PyTorch CPU ops in fp64 and differentiated by torch.autograd (a library primitive), so a reader can check the forward
+against the paper / rga_oracle.cpp by eye and the derivative is the library's.  Where alpha is clamped to 0.99 the
+derivative of the clamp is 0 (reading A32: mathematics, not the 3DGS code, which lets the gradient pass).
+
+Pins (tests/test_backward_pins.py): the forward here equals rga_oracle.cpp's orc_project / orc_composite (independent
+code); finite differences THROUGH rga_oracle.cpp reproduce the gradients; hand-derived one- and two-Gaussian closed
+forms; torch.autograd.gradcheck on a tiny scene.
+"""
+import numpy as np
+import torch
+
+F64 = torch.float64
+
+
+def _t(a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64))
+
+
+def project_torch(x, cov6, cam):
+    """H6 (EWA projection) of the Gaussians that survive culling, differentiable.  x [n,3] posed means, cov6 [n,6]
+    (xx,xy,xz,yy,yz,zz).  Same formulas and order as orc_project (rga_oracle.cpp): t = R x + t_w, clamped t_x/t_z and
+    t_y/t_z (1.3 x the half field of view) inside the Jacobian only, cov2D = T Sigma T^T + 0.3 I, conic = cov2D^-1,
+    mu = (fx t_x / t_z + cx, fy t_y / t_z + cy).  Returns mu [n,2], conic [n,3] (a, b, c of a dx^2 + 2 b dx dy + c dy^2)."""
+    R = _t(cam["R_wc"]).reshape(3, 3); tw = _t(cam["t_wc"]).reshape(3)
+    fx, fy, cx, cy = float(cam["fx"]), float(cam["fy"]), float(cam["cx"]), float(cam["cy"])
+    W, H = int(cam["width"]), int(cam["height"])
+    t = x @ R.T + tw
+    limx, limy = 1.3 * (W / (2.0 * fx)), 1.3 * (H / (2.0 * fy))
+    t0, t1, t2 = t[:, 0], t[:, 1], t[:, 2]
+    txz = torch.clamp(t0 / t2, -limx, limx) * t2
+    tyz = torch.clamp(t1 / t2, -limy, limy) * t2
+    J00, J02 = fx / t2, -(fx * txz) / (t2 * t2)
+    J11, J12 = fy / t2, -(fy * tyz) / (t2 * t2)
+    T0 = J00[:, None] * R[0][None, :] + J02[:, None] * R[2][None, :]
+    T1 = J11[:, None] * R[1][None, :] + J12[:, None] * R[2][None, :]
+    s = cov6
+    S = torch.stack([torch.stack([s[:, 0], s[:, 1], s[:, 2]], 1), torch.stack([s[:, 1], s[:, 3], s[:, 4]], 1),
+                     torch.stack([s[:, 2], s[:, 4], s[:, 5]], 1)], 1)                    # [n,3,3] symmetric
+    V0 = torch.einsum("na,nab->nb", T0, S); V1 = torch.einsum("na,nab->nb", T1, S)
+    c00 = (V0 * T0).sum(1) + 0.3; c01 = (V0 * T1).sum(1); c11 = (V1 * T1).sum(1) + 0.3
+    det = c00 * c11 - c01 * c01
+    conic = torch.stack([c11 / det, -c01 / det, c00 / det], 1)
+    mu = torch.stack([fx * t0 / t2 + cx, fy * t1 / t2 + cy], 1)
+    return mu, conic
+
+
+def composite_tile(mu, conic, opac, col, ids, pxc, pyc, bg):
+    """H10 for the pixels of one tile: front-to-back "over" blend of the tile's sorted list `ids` at pixel centres
+    (pxc, pyc) [P].  Same rules as blend_pixel (rga_oracle.cpp): power = -1/2 (a dx^2 + c dy^2) - b dx dy with
+    d = mu - pixel; skip when power > 0; alpha = min(0.99, o exp(power)); skip when alpha < 1/255; stop before the entry
+    that would take T below 1e-4; C = sum c_i alpha_i T_i + T_final bg.  The skip / stop masks are computed without
+    gradient (frozen decisions).  Returns C [P,3], T_final [P], n_contrib [P] (1-based index of the last contributor)."""
+    P = pxc.shape[0]
+    if len(ids) == 0:
+        return bg[None, :].expand(P, 3).clone(), torch.ones(P, dtype=F64), torch.zeros(P, dtype=torch.int64)
+    m, q, o, c = mu[ids], conic[ids], opac[ids], col[ids]
+    dx = m[None, :, 0] - pxc[:, None]; dy = m[None, :, 1] - pyc[:, None]
+    power = -0.5 * (q[None, :, 0] * dx * dx + q[None, :, 2] * dy * dy) - q[None, :, 1] * dx * dy
+    alpha = torch.minimum(torch.full_like(power, 0.99), o[None, :] * torch.exp(torch.clamp(power, max=0.0)))
+    with torch.no_grad():
+        skip = (power > 0.0) | (alpha < 1.0 / 255.0)
+    alpha = torch.where(skip, torch.zeros_like(alpha), alpha)
+    with torch.no_grad():
+        live = torch.cumprod(1.0 - alpha, 1) >= 1e-4          # monotone: false from the stopping entry on
+        idx = torch.arange(1, len(ids) + 1)[None, :].expand(P, -1)
+        n_contrib = torch.where(live & ~skip, idx, torch.zeros_like(idx)).max(1).values
+    alpha = torch.where(live, alpha, torch.zeros_like(alpha))
+    T_incl = torch.cumprod(1.0 - alpha, 1)
+    T_excl = torch.cat([torch.ones(P, 1, dtype=F64), T_incl[:, :-1]], 1)
+    C = ((alpha * T_excl)[:, :, None] * c[None, :, :]).sum(1) + T_incl[:, -1:] * bg[None, :]
+    return C, T_incl[:, -1], n_contrib
+
+
+def splat_backward(xg, cov6, col, opac, cam, bg, vals, ranges, touched, G, mu32=None, conic32=None):
+    """Forward image and the gradient of L = sum(G * image).  xg [N,3] posed means, cov6 [N,6], col [N,3] splatted
+    colours, opac [N] or None (= 1), vals / ranges / touched = the frozen tile lists of H7-H9 (oracle
+    outputs), G [H,W,3].  Chain rule in two stages so that only one tile's graph is alive at a time: stage 1 differentiates
+    the blend w.r.t. (colour, opacity, mu, conic) tile by tile; stage 2 pulls d_mu, d_conic back through the projection.
+    mu32 / conic32 (optional): the fp32 projection outputs of orc_project; when given, stage 1 blends exactly those
+    values (the numbers the forward pass of either side blends), so its frozen decisions are the forward oracle's own;
+    stage 2 is evaluated at the fp64 point either way.
+    Returns dict with image, T_final, n_contrib, d_col, d_opac, d_mu, d_conic, d_x, d_cov6 (numpy fp64; rows of culled
+    Gaussians are 0)."""
+    N = len(xg); W, H = int(cam["width"]), int(cam["height"]); TX, TY = (W + 15) // 16, (H + 15) // 16
+    alive = np.nonzero(np.asarray(touched) > 0)[0]
+    x_a = _t(np.asarray(xg)[alive]).requires_grad_(True)
+    cov_a = _t(np.asarray(cov6)[alive]).requires_grad_(True)
+    mu_a, conic_a = project_torch(x_a, cov_a, cam)
+    mu = torch.zeros(N, 2, dtype=F64); conic = torch.zeros(N, 3, dtype=F64)
+    ia = torch.as_tensor(alive)
+    mu[ia] = mu_a.detach(); conic[ia] = conic_a.detach()
+    if mu32 is not None:
+        mu = _t(mu32).clone(); conic = _t(np.asarray(conic32)[:, :3]).clone()
+    mu.requires_grad_(True); conic.requires_grad_(True)
+    colt = _t(col).requires_grad_(True)
+    opt = (torch.ones(N, dtype=F64) if opac is None else _t(opac)).requires_grad_(True)
+    bgt = _t(bg); Gt = _t(G)
+    image = np.zeros((H, W, 3)); Tf = np.ones((H, W)); nc = np.zeros((H, W), np.int64)
+    vals = np.asarray(vals).astype(np.int64); ranges = np.asarray(ranges).reshape(-1, 2)
+    for ty in range(TY):
+        for tx in range(TX):
+            t = ty * TX + tx
+            ys, xs = np.meshgrid(np.arange(ty * 16, min(ty * 16 + 16, H)), np.arange(tx * 16, min(tx * 16 + 16, W)), indexing="ij")
+            ys, xs = ys.reshape(-1), xs.reshape(-1)
+            ids = torch.as_tensor(vals[int(ranges[t, 0]):int(ranges[t, 1])])
+            C, T, n = composite_tile(mu, conic, opt, colt, ids, _t(xs + 0.5), _t(ys + 0.5), bgt)
+            image[ys, xs] = C.detach().numpy(); Tf[ys, xs] = T.detach().numpy(); nc[ys, xs] = n.numpy()
+            if len(ids):
+                (C * Gt[ys, xs]).sum().backward()
+    z = lambda v, shape: np.zeros(shape) if v.grad is None else v.grad.numpy().copy()
+    d_mu, d_conic = z(mu, (N, 2)), z(conic, (N, 3))
+    torch.autograd.backward([mu_a, conic_a], [_t(d_mu[alive]), _t(d_conic[alive])])
+    d_x = np.zeros((N, 3)); d_cov = np.zeros((N, 6))
+    if len(alive):
+        d_x[alive] = x_a.grad.numpy(); d_cov[alive] = cov_a.grad.numpy()
+    return {"image": image, "T_final": Tf, "n_contrib": nc, "d_col": z(colt, (N, 3)), "d_opac": z(opt, (N,)), "d_mu": d_mu,
+            "d_conic": d_conic, "d_x": d_x, "d_cov6": d_cov}

@@ -220,3 +220,9 @@ def make_disp_mlp(seed=0, n_freq=64, n_pose=72, width=256, n_hidden=4, rff_sigma
         Wh=he(width, (n_hidden - 1, width, width)), bh=(0.1 * r.standard_normal((n_hidden - 1, width))).astype(np.float32),
         Wo=(out_scale * he(width, (3, width))).astype(np.float32), bo=(0.001 * r.standard_normal(3)).astype(np.float32),
         theta=np.deg2rad(r.uniform(-30.0, 30.0, n_pose)).astype(np.float32))
+
+
+def make_image_cotangent(seed, width, height):
+    """dL/dimage for the backward pass: a seeded standard-normal field [height, width, 3] (fp32).  An input of both the
+    oracle and the library; the loss that would produce it (Eq.5) is not part of this module."""
+    return np.random.default_rng(1000 + seed).normal(size=(height, width, 3)).astype(np.float32)

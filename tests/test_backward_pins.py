@@ -1,0 +1,177 @@
+"""Pins for the backward oracle (oracle/backward.py): its forward against the independent C++ forward oracle, its
+gradients against finite differences taken THROUGH the C++ oracle, hand-derived closed forms, and gradcheck.  No GPU."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import backward as bwd
+from oracle import oracle as orc
+from synth import workloads
+
+
+@pytest.fixture(scope="module")
+def scene0():
+    inp = workloads.make(0)
+    av = orc.avatar_load(inp)
+    o = orc.render_frame(av, inp, vis_mode=0)
+    cam = inp["camera"]
+    G = workloads.make_image_cotangent(3, cam["width"], cam["height"])
+    r = bwd.splat_backward(o["gauss_posed"], o["cov6"], o["color"], inp["gauss_opacity"], cam, inp["bg"], o["vals"], o["ranges"],
+                           o["touched"], G, mu32=o["mu"], conic32=o["conic_o"])
+    return inp, o, G, r
+
+
+def test_backward_oracle_forward_equals_cpp_oracle(scene0):
+    inp, o, G, r = scene0
+    # stage 1 blends the C++ oracle's own fp32 mu / conic: same decisions, same image (both fp64 blends)
+    assert np.array_equal(r["n_contrib"], o["n_contrib"])
+    assert np.abs(r["image"] - o["image"]).max() < 1e-12
+    assert np.abs(r["T_final"] - o["T_final"]).max() < 1e-12
+    # the fp64 projection written in torch agrees with orc_project (fp32 arithmetic) on every surviving Gaussian
+    alive = o["touched"] > 0
+    mu, conic = bwd.project_torch(torch.as_tensor(o["gauss_posed"][alive].astype(np.float64)),
+                                  torch.as_tensor(o["cov6"][alive].astype(np.float64)), inp["camera"])
+    assert np.abs(mu.numpy() - o["mu"][alive]).max() < 2e-3                       # pixels, fp32 rounding of ~1e2 px values
+    assert np.allclose(conic.numpy(), o["conic_o"][alive, :3], rtol=2e-3, atol=1e-5)
+    # without the override the decisions come from the fp64 projection: still the same image to fp32 rounding of mu
+    cam = inp["camera"]
+    r2 = bwd.splat_backward(o["gauss_posed"], o["cov6"], o["color"], inp["gauss_opacity"], cam, inp["bg"], o["vals"], o["ranges"],
+                            o["touched"], G)
+    assert np.abs(r2["image"] - o["image"]).max() < 1e-4
+    assert np.abs(r2["d_col"] - r["d_col"]).max() < 1e-3 * np.abs(r["d_col"]).max()
+
+
+def _loss_cpp(o, inp, G, mu=None, conic_o=None, col=None):
+    cam = inp["camera"]
+    img, _, _, _ = orc.composite(o["vals"], o["ranges"], o["mu"] if mu is None else mu, o["conic_o"] if conic_o is None else conic_o,
+                                 o["color"] if col is None else col, inp["bg"], cam["width"], cam["height"])
+    return float((img * G).sum())
+
+
+def test_stage1_gradients_match_finite_differences_through_cpp_composite(scene0):
+    # perturbations are exactly representable in fp32 (the C++ blend takes fp32 mu / conic and works in fp64)
+    inp, o, G, r = scene0
+    rs = np.random.default_rng(0)
+    score = np.abs(r["d_mu"]).sum(1) + np.abs(r["d_conic"]).sum(1)
+    pick = np.argsort(-score)[:40][rs.permutation(40)[:10]]
+    ok = 0
+    for g in pick:
+        for name, arr, grad, comps in (("mu", o["mu"], r["d_mu"], 2), ("conic", o["conic_o"], r["d_conic"], 3), ("opac", o["conic_o"], r["d_opac"], 1)):
+            for c in range(comps):
+                col = 3 if name == "opac" else c
+                a_p, a_m = arr.copy(), arr.copy()
+                h = np.float32(2.0 ** -9) if name == "mu" else np.float32(abs(arr[g, col]) * 2.0 ** -9 + 1e-6)
+                a_p[g, col] = arr[g, col] + h; a_m[g, col] = arr[g, col] - h
+                kw = "mu" if name == "mu" else "conic_o"
+                fd = (_loss_cpp(o, inp, G, **{kw: a_p}) - _loss_cpp(o, inp, G, **{kw: a_m})) / (float(a_p[g, col]) - float(a_m[g, col]))
+                an = grad[g] if name == "opac" else grad[g, c]
+                if name == "opac" and arr[g, 3] + h > 0.99:
+                    continue                                              # opacity 1: alpha clamps for part of the footprint, FD is one-sided
+                if abs(fd - an) <= 2e-2 * abs(an) + 2e-3 * np.abs(grad).max():
+                    ok += 1
+                else:                                                     # a frozen decision flipped under the perturbation: rare
+                    ok -= 5
+    assert ok > 30
+    # colour is linear: finite differences are exact
+    for g in pick[:4]:
+        for c in range(3):
+            cp = o["color"].astype(np.float64).copy(); cp[g, c] += 0.25
+            fd = (_loss_cpp(o, inp, G, col=cp) - _loss_cpp(o, inp, G)) / 0.25
+            assert abs(fd - r["d_col"][g, c]) < 1e-9 * (1 + abs(fd))
+
+
+def test_stage2_gradients_match_finite_differences_through_cpp_projection(scene0):
+    # L2 = <d_mu, mu(x, Sigma)> + <d_conic, conic(x, Sigma)> through orc_project (fp32 arithmetic -> coarse steps, 1 % tolerance)
+    inp, o, G, r = scene0
+    cam = inp["camera"]
+
+    def L2(x, cov):
+        p = orc.project(x, o["gauss_normal_posed"], cov, inp["gauss_opacity"], cam)
+        return (p["mu"].astype(np.float64) * r["d_mu"]).sum(1) + (p["conic_o"][:, :3].astype(np.float64) * r["d_conic"]).sum(1)   # per Gaussian
+
+    alive = np.nonzero(o["touched"] > 0)[0]
+    x0, c0 = o["gauss_posed"].astype(np.float32), o["cov6"].astype(np.float32)
+    for c in range(3):
+        xp, xm = x0.copy(), x0.copy(); xp[:, c] += np.float32(1e-3); xm[:, c] -= np.float32(1e-3)
+        fd = (L2(xp, c0) - L2(xm, c0)) / (xp[:, c].astype(np.float64) - xm[:, c])
+        err = np.abs(fd[alive] - r["d_x"][alive, c])
+        assert np.median(err / (np.abs(r["d_x"][alive, c]) + 1e-3 * np.abs(r["d_x"]).max())) < 1e-2
+        assert (err < 3e-2 * np.abs(r["d_x"][alive, c]) + 3e-3 * np.abs(r["d_x"]).max()).mean() > 0.97
+    for c in range(6):
+        h = (np.abs(c0).max(1) * 0.02).astype(np.float32)
+        cp, cm = c0.copy(), c0.copy(); cp[:, c] += h; cm[:, c] -= h
+        fd = (L2(x0, cp) - L2(x0, cm)) / (cp[:, c].astype(np.float64) - cm[:, c])
+        err = np.abs(fd[alive] - r["d_cov6"][alive, c])
+        assert (err < 3e-2 * np.abs(r["d_cov6"][alive, c]) + 3e-3 * np.abs(r["d_cov6"]).max()).mean() > 0.97
+
+
+def test_one_and_two_gaussian_closed_forms():
+    # I = c a + (1 - a) bg,  a = o exp(p),  p = -1/2 (A dx^2 + C dy^2) - B dx dy,  d = mu - pixel   (hand derivatives)
+    t = lambda v: torch.tensor(v, dtype=torch.float64, requires_grad=True)
+    mu, conic, o, col = t([[5.2, 7.9]]), t([[0.31, 0.07, 0.22]]), t([0.8]), t([[0.9, 0.2, 0.4]])
+    bg = torch.tensor([0.1, 0.3, 0.2], dtype=torch.float64); G = np.array([0.7, -1.1, 0.4])
+    C, T, n = bwd.composite_tile(mu, conic, o, col, torch.tensor([0]), torch.tensor([4.5], dtype=torch.float64),
+                                 torch.tensor([6.5], dtype=torch.float64), bg)
+    (C * torch.as_tensor(G)).sum().backward()
+    dx, dy = 5.2 - 4.5, 7.9 - 6.5
+    p = -0.5 * (0.31 * dx * dx + 0.22 * dy * dy) - 0.07 * dx * dy
+    a = 0.8 * np.exp(p)
+    s = float(((np.array([0.9, 0.2, 0.4]) - bg.numpy()) * G).sum())
+    assert int(n[0]) == 1 and abs(float(T[0].detach()) - (1 - a)) < 1e-15
+    assert np.allclose(col.grad.numpy()[0], a * G)
+    assert np.isclose(o.grad.item(), np.exp(p) * s)
+    assert np.allclose(mu.grad.numpy()[0], [a * s * -(0.31 * dx + 0.07 * dy), a * s * -(0.22 * dy + 0.07 * dx)])
+    assert np.allclose(conic.grad.numpy()[0], [a * s * -0.5 * dx * dx, a * s * -dx * dy, a * s * -0.5 * dy * dy])
+    # two Gaussians at the same pixel: dI/da1 = c1 - c2 a2 - (1 - a2) bg;  dI/da2 = (1 - a1)(c2 - bg)
+    mu, conic = t([[4.5, 6.5], [4.5, 6.5]]), t([[1, 0, 1.0], [1, 0, 1.0]])
+    o, col = t([0.6, 0.5]), t([[1.0, 0.0, 0.0], [0.0, 1.0, 0.0]])
+    C, T, n = bwd.composite_tile(mu, conic, o, col, torch.tensor([0, 1]), torch.tensor([4.5], dtype=torch.float64),
+                                 torch.tensor([6.5], dtype=torch.float64), bg)
+    (C * torch.as_tensor(G)).sum().backward()
+    c1, c2, b = np.array([1.0, 0, 0]), np.array([0, 1.0, 0]), bg.numpy()
+    assert np.allclose(o.grad.numpy(), [((c1 - c2 * 0.5 - 0.5 * b) * G).sum(), (0.4 * (c2 - b) * G).sum()])
+    assert np.allclose(col.grad.numpy(), [0.6 * G, 0.4 * 0.5 * G])
+    # clamp (reading A32): o exp(p) = 1.2 > 0.99 -> alpha = 0.99 and no gradient reaches o, mu or the conic
+    mu, conic, o, col = t([[4.5, 6.5]]), t([[1, 0, 1.0]]), t([1.2]), t([[0.9, 0.2, 0.4]])
+    C, T, n = bwd.composite_tile(mu, conic, o, col, torch.tensor([0]), torch.tensor([4.5], dtype=torch.float64),
+                                 torch.tensor([6.5], dtype=torch.float64), bg)
+    (C * torch.as_tensor(G)).sum().backward()
+    assert abs(float(T[0].detach()) - 0.01) < 1e-15 and o.grad.item() == 0.0 and np.all(conic.grad.numpy() == 0) and np.allclose(col.grad.numpy()[0], 0.99 * G)
+
+
+def test_projection_closed_form_and_gradcheck():
+    # identity camera, isotropic Sigma = s2 I: cov2D_xx = (fx / z)^2 s2 (1 + (x/z)^2) + 0.3 on the x axis; mu_x = fx x / z + cx
+    cam = {"R_wc": np.eye(3), "t_wc": np.zeros(3), "fx": 100.0, "fy": 100.0, "cx": 32.0, "cy": 32.0, "width": 64, "height": 64, "z_near": 0.1}
+    x = torch.tensor([[0.2, 0.0, 2.0]], dtype=torch.float64, requires_grad=True)
+    s2 = 0.01
+    cov = torch.tensor([[s2, 0, 0, s2, 0, s2]], dtype=torch.float64, requires_grad=True)
+    mu, conic = bwd.project_torch(x, cov, cam)
+    assert np.allclose(mu.detach().numpy(), [[100 * 0.2 / 2 + 32, 32.0]])
+    cxx = (100 / 2.0) ** 2 * s2 * (1 + 0.1 ** 2) + 0.3; cyy = (100 / 2.0) ** 2 * s2 + 0.3
+    assert np.allclose(conic.detach().numpy(), [[1 / cxx, 0.0, 1 / cyy]])
+    mu[0, 0].backward(retain_graph=True)
+    assert np.allclose(x.grad.numpy(), [[100 / 2.0, 0, -100 * 0.2 / 4.0]])          # d mu_x / d(x, y, z)
+    x.grad = None; cov.grad = None
+    conic[0, 2].backward()
+    assert np.allclose(cov.grad.numpy()[0, 3], -(1 / cyy) ** 2 * (100 / 2.0) ** 2)   # d(1/cyy)/d Sigma_yy
+    assert np.allclose(cov.grad.numpy()[0, [0, 1, 2]], 0.0)
+    # gradcheck of projection + blend on a tiny scene kept away from every threshold
+    rs = np.random.default_rng(2)
+    n = 5
+    X = torch.tensor(np.c_[rs.uniform(-0.05, 0.05, (n, 2)) - [[0.24, 0.24]], rs.uniform(1.8, 2.2, n)], dtype=torch.float64, requires_grad=True)
+    A = rs.normal(size=(n, 3, 3)) * 0.02
+    S = A @ A.transpose(0, 2, 1) + 0.02 ** 2 * np.eye(3)
+    COV = torch.tensor(np.stack([S[:, 0, 0], S[:, 0, 1], S[:, 0, 2], S[:, 1, 1], S[:, 1, 2], S[:, 2, 2]], 1), dtype=torch.float64, requires_grad=True)
+    COL = torch.tensor(rs.uniform(0, 1, (n, 3)), dtype=torch.float64, requires_grad=True)
+    OP = torch.tensor(rs.uniform(0.3, 0.6, n), dtype=torch.float64, requires_grad=True)
+    ys, xs = np.meshgrid(np.arange(16), np.arange(16), indexing="ij")
+    px, py = torch.tensor(xs.reshape(-1) + 0.5, dtype=torch.float64), torch.tensor(ys.reshape(-1) + 0.5, dtype=torch.float64)
+    sel = torch.tensor([17, 40, 100, 119, 136, 200])
+    bg = torch.tensor([0.1, 0.3, 0.2], dtype=torch.float64)
+
+    def f(X, COV, COL, OP):
+        mu, conic = bwd.project_torch(X, COV, cam)
+        C, T, nc = bwd.composite_tile(mu, conic, OP, COL, torch.arange(n), px[sel], py[sel], bg)
+        return C
+
+    assert torch.autograd.gradcheck(f, (X, COV, COL, OP), eps=1e-7, atol=1e-6, rtol=1e-4)
