@@ -247,6 +247,25 @@ def main():
         pose_with_views()
     ms_views = timed(pose_with_views, max(args.steps // 4, 5))
 
+    # backward of the splat (H10 + H6) for the frame just rendered, seeded dL/dimage
+    dLdI = torch.as_tensor(workloads.make_image_cotangent(1, camc.width, camc.height)).to(dev)
+    ng_all = len(inp["gauss_pos"])
+    d_col = torch.empty((ng_all, 3), device=dev); d_op = torch.empty((ng_all,), device=dev)
+    d_x = torch.empty((ng_all, 3), device=dev); d_cov = torch.empty((ng_all, 6), device=dev)
+    run_bwd = lambda: rga.splat_backward(av.h, camc, inp["bg"], dLdI, d_col, d_op, d_x, d_cov)
+    for _ in range(3):
+        run_bwd()
+    ms_bwd = timed(run_bwd, 20)
+    rga.rga_profile_enable(av.h, True)
+    bwd_k = {}
+    for _ in range(10):
+        run_bwd()
+        for name, t in rga.rga_profile_read(av.h):
+            bwd_k.setdefault(name, []).append(t)
+    rga.rga_profile_enable(av.h, False)
+    bwd_obj = {"ms": ms_bwd, "kernel_ms": {k: float(np.mean(v)) for k, v in bwd_k.items() if k != "-"},
+               "note": "gradients w.r.t. colour, opacity, posed mean and 3D covariance of every Gaussian; L2 flushed between calls"}
+
     # algorithmic units of each candidate dominant kernel: counted from the frame that was rendered
     gp = av.read("GAUSS_POSED").reshape(-1, 4)[:, :3]; gn = av.read("GAUSS_NORMAL_POSED").reshape(-1, 4)[:, :3]
     front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
@@ -317,7 +336,7 @@ def main():
                 "pipelined_value": world * 1e3 / ms_e2e_pipe,
                 "pipelined_note": "image read-back of step i on a copy stream beside step i+1; per-step events plus the last copy's tail"},
         "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
-        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj,
+        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj,
         "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -133,6 +133,19 @@ RGA_API rga_status splat_render(rga_avatar* av, const rga_camera* cam, const flo
  * scale and opacity are kept.  gauss_pos: dev [n_gauss][3].  Enqueue-only; call pose_skin afterwards. */
 RGA_API rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, void* stream);
 
+/* Backward of splat_render (training / editing regime, PAPER.md:128 "the same image loss as 3DGS", :185): for the frame
+ * last rendered by splat_render or rga_render_frame with THIS camera and background, and dL_dimage = dL/d(out_image)
+ * (dev [height][width][3] fp32), the gradient of L with respect to every Gaussian's splatted colour c_g, opacity o_g,
+ * posed mean xbar_gd and posed 3D covariance (the 6 unique entries xx,xy,xz,yy,yz,zz; an off-diagonal entry's gradient
+ * counts both of its positions).  The forward's discrete decisions are frozen: tile lists and their order, culled
+ * Gaussians (rows of zeros), per-pixel skips (power > 0, alpha < 1/255) and the stopping entry; where alpha is clamped
+ * to 0.99 no gradient reaches opacity, mean or covariance (reading A32).  The dependence of the colour on the
+ * position through shading is NOT included (that is the backward of shade_gaussians).
+ * Outputs are DEVICE buffers, each may be NULL: out_dcolor [n_gauss][3], out_dopacity [n_gauss], out_dmean [n_gauss][3],
+ * out_dcov [n_gauss][6].  dL/dmu2D and dL/dconic stay readable through RGA_BUF_SPLAT_GRAD.  Enqueue-only. */
+RGA_API rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* dL_dimage,
+                                  float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, void* stream);
+
 /* Algorithm 1, "Gaussian densification based on density": from the avatar's current
  * S_g (avatar_load / gaussians_update) and its mesh, counts the Gaussians near every vertex (D_v), estimates the Gaussian
  * density of every triangle d_f = sum of its three D_v / (6 K_g), sets P = max(0, d0 - d_f), asks for
@@ -220,7 +233,8 @@ typedef enum {
   RGA_BUF_DENS_P = 31,        /* u32 [n_faces]  P = max(0, d0 - d_f) in fixed point (P * 2^16)         */
   RGA_BUF_DENS_NG = 32,       /* i32 [n_faces]  Gaussians added per triangle by the last call          */
   RGA_BUF_DENS_HDR = 33,      /* u64 [2]        sum of the fixed-point P, N'                            */
-  RGA_BUF_COUNT_ = 34
+  RGA_BUF_SPLAT_GRAD = 34,    /* f32 [n_gauss][12] splat_backward: d_colour(3), d_opacity, d_mu2D(2), d_conic(3), pad(3) */
+  RGA_BUF_COUNT_ = 35
 } rga_buffer_id;
 
 /* Returns the device pointer and current size in bytes of an internal buffer (valid until the next call that

@@ -56,7 +56,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
+  void* ptrs[] = {av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
                   av->vt_spec, av->knn_d2, av->grid_start, av->grid_verts, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
@@ -113,7 +113,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   float* d2 = nullptr;
 #define A(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, \
     "avatar_load: %s: %s", #call, cudaGetErrorString(e_)); goto done; } } while (0)
-  A(dalloc(&av->dens_dv, nv)); A(dalloc(&av->dens_pfix, (size_t)av->n_faces)); A(dalloc(&av->dens_cdf, (size_t)av->n_faces));
+  A(dalloc(&av->splat_grad, 12 * ng)); A(dalloc(&av->dens_dv, nv)); A(dalloc(&av->dens_pfix, (size_t)av->n_faces)); A(dalloc(&av->dens_cdf, (size_t)av->n_faces));
   A(dalloc(&av->dens_ng, (size_t)av->n_faces)); A(dalloc(&av->dens_block, (size_t)av->n_faces / 2048 + 1)); A(dalloc(&av->dens_hdr, 2));
   A(dalloc(&av->v_pos, nv)); A(dalloc(&av->v_disp, nv)); A(dalloc(&av->g_pos, ng)); A(dalloc(&av->mlp_bias1, 256));
   A(dalloc(&av->v_xbar, nv)); A(dalloc(&av->v_normal, nv)); A(dalloc(&av->v_skin_w, nv * B)); A(dalloc(&av->faces, 3 * (size_t)av->n_faces)); A(dalloc(&av->faces_packed, (size_t)av->n_faces));
@@ -262,6 +262,17 @@ extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, v
   CU(rga_launch_load_gauss(av, gauss_pos, nullptr, nullptr, nullptr, av->knn_d2, s));
   rga_prof_mark(av, "load_gauss", s);
   av->launches += 2;
+  return RGA_OK;
+}
+
+extern "C" rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* dL_dimage, float* out_dcolor,
+                                     float* out_dopacity, float* out_dmean, float* out_dcov, void* stream) {
+  if (!av || !cam || !bg || !dL_dimage) return fail(RGA_ERR_INVALID_ARG, "splat_backward: null argument");
+  if (!av->have_splat) return fail(RGA_ERR_STATE, "splat_backward: call splat_render (or rga_render_frame) first");
+  if (cam->width != av->cam_w || cam->height != av->cam_h) return fail(RGA_ERR_INVALID_ARG, "splat_backward: not the camera of the last splat_render");
+  cudaStream_t s = (cudaStream_t)stream;
+  rga_prof_mark(av, "-", s);
+  CU(rga_launch_splat_backward(av, cam, make_float3(bg[0], bg[1], bg[2]), dL_dimage, out_dcolor, out_dopacity, out_dmean, out_dcov, s));
   return RGA_OK;
 }
 
@@ -420,6 +431,7 @@ extern "C" rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, co
     case RGA_BUF_N_CONTRIB: p = av->n_contrib; n = npix * 4; break;
     case RGA_BUF_VERT_BITS_RAW: p = av->vbits_raw; n = nv * words * 4; break;
     case RGA_BUF_VERT_DISP: p = av->v_disp; n = nv * 16; break;
+    case RGA_BUF_SPLAT_GRAD: p = av->splat_grad; n = ng * 48; break;
     case RGA_BUF_DENS_DV: p = av->dens_dv; n = nv * 4; break;
     case RGA_BUF_DENS_P: p = av->dens_pfix; n = (size_t)av->n_faces * 4; break;
     case RGA_BUF_DENS_NG: p = av->dens_ng; n = (size_t)av->n_faces * 4; break;

@@ -78,6 +78,7 @@ struct rga_avatar {
   int* stop_seg;               // [pixels] segment in which the pixel's blend stops (-1: list exhausted)
   unsigned char* item_flag;    // [items_cap] work item has pixels to replay (cleared by the replay kernel)
   float* t_final; unsigned* n_contrib;
+  float* splat_grad;           // [n_gauss][12] splat_backward: d_colour(3), d_opacity, d_mu(2), d_conic(3), pad
   int* status;                 // sticky device status
   int sorted_buf;              // which of keys[]/vals[] holds the sorted result
   // state of the current pose
@@ -126,6 +127,9 @@ cudaError_t rga_build_knn_grid(rga_avatar* av, const float* aabb_host, cudaStrea
 cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s);
 cudaError_t rga_launch_knn_verts(rga_avatar* av, float* d2, cudaStream_t s);
 int rga_mlp_init_attributes();
+// backward_kernels.cu
+cudaError_t rga_launch_splat_backward(rga_avatar* av, const rga_camera* cam, float3 bg, const float* dL_dimage, float* out_dcolor,
+                                      float* out_dopacity, float* out_dmean, float* out_dcov, cudaStream_t s);
 // densify_kernels.cu
 cudaError_t rga_launch_densify(rga_avatar* av, float d0, float p0, const unsigned* rnd, int max_out, float* out_pos, int* out_tri,
                                int* out_count, cudaStream_t s);
