@@ -252,7 +252,7 @@ def main():
     ng_all = len(inp["gauss_pos"])
     d_col = torch.empty((ng_all, 3), device=dev); d_op = torch.empty((ng_all,), device=dev)
     d_x = torch.empty((ng_all, 3), device=dev); d_cov = torch.empty((ng_all, 6), device=dev)
-    run_bwd = lambda: rga.splat_backward(av.h, camc, inp["bg"], dLdI, d_col, d_op, d_x, d_cov)
+    run_bwd = lambda: rga.splat_backward(av.h, camc, inp["bg"], img, dLdI, d_col, d_op, d_x, d_cov)
     for _ in range(3):
         run_bwd()
     ms_bwd = timed(run_bwd, 20)

@@ -134,8 +134,8 @@ RGA_API rga_status splat_render(rga_avatar* av, const rga_camera* cam, const flo
 RGA_API rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, void* stream);
 
 /* Backward of splat_render (training / editing regime, PAPER.md:128 "the same image loss as 3DGS", :185): for the frame
- * last rendered by splat_render or rga_render_frame with THIS camera and background, and dL_dimage = dL/d(out_image)
- * (dev [height][width][3] fp32), the gradient of L with respect to every Gaussian's splatted colour c_g, opacity o_g,
+ * last rendered by splat_render or rga_render_frame with THIS camera and background, image = the out_image that call
+ * wrote (unchanged) and dL_dimage = dL/d(out_image) (both dev [height][width][3] fp32), the gradient of L with respect to every Gaussian's splatted colour c_g, opacity o_g,
  * posed mean xbar_gd and posed 3D covariance (the 6 unique entries xx,xy,xz,yy,yz,zz; an off-diagonal entry's gradient
  * counts both of its positions).  The forward's discrete decisions are frozen: tile lists and their order, culled
  * Gaussians (rows of zeros), per-pixel skips (power > 0, alpha < 1/255) and the stopping entry; where alpha is clamped
@@ -143,7 +143,7 @@ RGA_API rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, void
  * position through shading is NOT included (that is the backward of shade_gaussians).
  * Outputs are DEVICE buffers, each may be NULL: out_dcolor [n_gauss][3], out_dopacity [n_gauss], out_dmean [n_gauss][3],
  * out_dcov [n_gauss][6].  dL/dmu2D and dL/dconic stay readable through RGA_BUF_SPLAT_GRAD.  Enqueue-only. */
-RGA_API rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* dL_dimage,
+RGA_API rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* image, const float* dL_dimage,
                                   float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, void* stream);
 
 /* Algorithm 1, "Gaussian densification based on density": from the avatar's current

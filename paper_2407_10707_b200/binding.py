@@ -178,12 +178,13 @@ def gaussians_update(h, gauss_pos):
     _chk(lib().gaussians_update(h, _ptr(gauss_pos), _stream()))
 
 
-def splat_backward(h, camera, bg, dL_dimage, out_dcolor=None, out_dopacity=None, out_dmean=None, out_dcov=None):
-    """Backward of splat_render for the last rendered frame (include/rga.h splat_backward).  All tensors CUDA float32."""
+def splat_backward(h, camera, bg, image, dL_dimage, out_dcolor=None, out_dopacity=None, out_dmean=None, out_dcov=None):
+    """Backward of splat_render for the last rendered frame (include/rga.h splat_backward); image = the tensor that frame was
+    rendered into.  All tensors CUDA float32."""
     cam = camera if isinstance(camera, _Camera) else make_camera(camera)
     b = (C.c_float * 3)(*[float(v) for v in bg])
-    lib().splat_backward.argtypes = [C.c_void_p, C.POINTER(_Camera), C.c_float * 3] + [C.c_void_p] * 6
-    _chk(lib().splat_backward(h, C.byref(cam), b, _ptr(dL_dimage), _ptr(out_dcolor), _ptr(out_dopacity), _ptr(out_dmean), _ptr(out_dcov),
+    lib().splat_backward.argtypes = [C.c_void_p, C.POINTER(_Camera), C.c_float * 3] + [C.c_void_p] * 7
+    _chk(lib().splat_backward(h, C.byref(cam), b, _ptr(image), _ptr(dL_dimage), _ptr(out_dcolor), _ptr(out_dopacity), _ptr(out_dmean), _ptr(out_dcov),
                               _stream()))
 
 

@@ -265,14 +265,14 @@ extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, v
   return RGA_OK;
 }
 
-extern "C" rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* dL_dimage, float* out_dcolor,
-                                     float* out_dopacity, float* out_dmean, float* out_dcov, void* stream) {
-  if (!av || !cam || !bg || !dL_dimage) return fail(RGA_ERR_INVALID_ARG, "splat_backward: null argument");
+extern "C" rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* image, const float* dL_dimage,
+                                     float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, void* stream) {
+  if (!av || !cam || !bg || !image || !dL_dimage) return fail(RGA_ERR_INVALID_ARG, "splat_backward: null argument");
   if (!av->have_splat) return fail(RGA_ERR_STATE, "splat_backward: call splat_render (or rga_render_frame) first");
   if (cam->width != av->cam_w || cam->height != av->cam_h) return fail(RGA_ERR_INVALID_ARG, "splat_backward: not the camera of the last splat_render");
   cudaStream_t s = (cudaStream_t)stream;
   rga_prof_mark(av, "-", s);
-  CU(rga_launch_splat_backward(av, cam, make_float3(bg[0], bg[1], bg[2]), dL_dimage, out_dcolor, out_dopacity, out_dmean, out_dcov, s));
+  CU(rga_launch_splat_backward(av, cam, make_float3(bg[0], bg[1], bg[2]), image, dL_dimage, out_dcolor, out_dopacity, out_dmean, out_dcov, s));
   return RGA_OK;
 }
 

@@ -26,8 +26,6 @@ __device__ __forceinline__ int btile_px(unsigned t) { return (int)(((t >> 5) & 1
 __device__ __forceinline__ int btile_py(unsigned t) { return (int)((t >> 6) * 4u + ((t >> 3) & 3u)); }
 __device__ __forceinline__ float bex2_approx(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
-struct BwdStage { float2 mu[BB]; float4 co[BB]; float4 col[BB]; float2 ext[BB]; unsigned id[BB]; float acc[BB][9]; };
-
 // sum of v[0..7] over the warp: afterwards lane 4 k holds the total of v[k]
 __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
   const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
@@ -49,40 +47,32 @@ __device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
   return z;          // value index = (lane >> 2) & 7
 }
 
-__global__ void __launch_bounds__(BB) composite_backward_kernel(int W, int H, int TX, float3 bg, const uint2* __restrict__ ranges,
+// one work item = one RGA_SEG-entry segment of one tile's list (the forward's work items and its per-segment partials)
+struct BwdSeg { float2 mu[RGA_SEG]; float4 co[RGA_SEG]; float4 col[RGA_SEG]; float2 ext[RGA_SEG]; unsigned id[RGA_SEG]; float acc[RGA_SEG][9]; };
+
+__global__ void __launch_bounds__(BB) composite_backward_kernel(int W, int H, int TX, float3 bg, const unsigned* __restrict__ num_items,
+    const unsigned* __restrict__ item_tab, const unsigned* __restrict__ seg_off, const uint2* __restrict__ ranges,
     const unsigned* __restrict__ vals, const float2* __restrict__ mu2d, const float4* __restrict__ conic_o,
-    const float4* __restrict__ color, const float* __restrict__ t_final, const unsigned* __restrict__ n_contrib,
-    const float* __restrict__ dL_dimage, float* __restrict__ grad) {
-  __shared__ BwdStage st;
-  __shared__ unsigned s_max;
-  const unsigned tile = blockIdx.x;
-  const uint2 rg = ranges[tile];
-  const int n = (int)(rg.y - rg.x);
-  if (n <= 0) return;
+    const float4* __restrict__ color, const float4* __restrict__ part, const unsigned* __restrict__ n_contrib,
+    const float* __restrict__ image, const float* __restrict__ dL_dimage, float* __restrict__ grad) {
+  __shared__ BwdSeg st;
+  const unsigned n_items = *num_items;
   const int tid = threadIdx.x, lane = tid & 31;
-  const int px = (int)(tile % TX) * RGA_TILE + btile_px(tid), py = (int)(tile / TX) * RGA_TILE + btile_py(tid);
-  const bool inside = px < W && py < H;
-  const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;
-  const size_t p = (size_t)py * W + px;
-  const float Tfin = inside ? t_final[p] : 0.f;
-  const int last = inside ? (int)n_contrib[p] : 0;
-  float g0 = 0.f, g1 = 0.f, g2 = 0.f;
-  if (inside) { g0 = dL_dimage[3 * p]; g1 = dL_dimage[3 * p + 1]; g2 = dL_dimage[3 * p + 2]; }
-  const float bgdot = bg.x * g0 + bg.y * g1 + bg.z * g2;
-  if (tid == 0) s_max = 0u;
-  __syncthreads();
-  int wlast = last;
+  for (unsigned item = blockIdx.x; item < n_items; item += gridDim.x) {
+    const unsigned tile = item_tab[item];
+    const unsigned so = seg_off[tile];
+    const int seg = (int)(item - so);
+    const uint2 rg = ranges[tile];
+    const int b0 = seg * RGA_SEG;
+    const int m = min(RGA_SEG, (int)(rg.y - rg.x) - b0);
+    const int px = (int)(tile % TX) * RGA_TILE + btile_px(tid), py = (int)(tile / TX) * RGA_TILE + btile_py(tid);
+    const bool inside = px < W && py < H;
+    const size_t p = (size_t)py * W + px;
+    const int last = inside ? (int)n_contrib[p] : 0;                     // entries [0, last) can contribute to this pixel
+    int wlast = last;
 #pragma unroll
-  for (int o = 16; o; o >>= 1) wlast = max(wlast, __shfl_xor_sync(0xffffffffu, wlast, o));
-  if (lane == 0) atomicMax(&s_max, (unsigned)wlast);
-  __syncthreads();
-  const int nlast = (int)s_max;                         // entries [0, nlast) have a contributor somewhere in the tile
-  const float bcx = (float)((int)(tile % TX) * RGA_TILE + btile_px(tid & ~31u)) + 4.0f;
-  const float bcy = (float)((int)(tile / TX) * RGA_TILE + btile_py(tid & ~31u)) + 2.0f;
-  float T = Tfin, ac0 = 0.f, ac1 = 0.f, ac2 = 0.f, la = 0.f, lc0 = 0.f, lc1 = 0.f, lc2 = 0.f;
-  for (int b1 = nlast; b1 > 0; b1 -= BB) {
-    const int b0 = max(b1 - BB, 0), m = b1 - b0;
-    __syncthreads();
+    for (int o = 16; o; o >>= 1) wlast = max(wlast, __shfl_xor_sync(0xffffffffu, wlast, o));
+    if (!__syncthreads_or(b0 < wlast)) continue;                         // no pixel of the tile reaches this segment
     if (tid < m) {
       const unsigned g = vals[rg.x + b0 + tid];
       const float4 c = conic_o[g];
@@ -93,43 +83,62 @@ __global__ void __launch_bounds__(BB) composite_backward_kernel(int W, int H, in
       if (L2 > 0.f && det > 0.f) { hx = sqrtf(L2 * c.z / det) * 1.001f + 0.01f; hy = sqrtf(L2 * c.x / det) * 1.001f + 0.01f; }
       st.ext[tid] = make_float2(hx, hy);
     }
-#pragma unroll
-    for (int k = 0; k < 9; ++k) st.acc[tid][k] = 0.f;
+    for (int k = tid; k < RGA_SEG * 9; k += BB) (&st.acc[0][0])[k] = 0.f;
     __syncthreads();
-    for (int j = min(m, wlast - b0) - 1; j >= 0; --j) {                  // entries at or past the warp's last contributor: none
-      const float2 mm = st.mu[j], ex = st.ext[j];
-      if (fabsf(mm.x - bcx) > ex.x + 3.5f || fabsf(mm.y - bcy) > ex.y + 1.5f) continue;
-      const float4 co = st.co[j];
-      const float dx = mm.x - fx, dy = mm.y - fy;
-      const float p2 = dx * (co.x * dx + co.y * dy) + co.z * dy * dy;     // log2(e) * power, as in the forward
-      const float raw = co.w * bex2_approx(p2);
-      const float a = fminf(0.99f, raw);
-      const bool valid = (b0 + j < last) && !(p2 > 0.f || a < 1.f / 255.f);
-      if (!__any_sync(0xffffffffu, valid)) continue;
-      float v[8], s0 = 0.f;
-#pragma unroll
-      for (int k = 0; k < 8; ++k) v[k] = 0.f;
-      if (valid) {
-        const float4 c = st.col[j];
-        const float om = 1.f - a;
-        T = T / om;                                                       // transmittance in front of this entry
-        const float wgt = a * T;
-        v[0] = wgt * g0; v[1] = wgt * g1; v[2] = wgt * g2;
-        ac0 = la * lc0 + (1.f - la) * ac0; ac1 = la * lc1 + (1.f - la) * ac1; ac2 = la * lc2 + (1.f - la) * ac2;
-        la = a; lc0 = c.x; lc1 = c.y; lc2 = c.z;
-        float dLda = (c.x - ac0) * g0 + (c.y - ac1) * g1 + (c.z - ac2) * g2;
-        dLda = dLda * T - __fdividef(Tfin, om) * bgdot;
-        const float w = raw > 0.99f ? 0.f : a * dLda;
-        s0 = w;
-        v[3] = w * dx; v[4] = w * dy; v[5] = w * dx * dx; v[6] = w * dx * dy; v[7] = w * dy * dy;
+    if (b0 < wlast) {
+      const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;
+      float g0 = 0.f, g1 = 0.f, g2 = 0.f, sI = 0.f;
+      if (inside) {
+        g0 = dL_dimage[3 * p]; g1 = dL_dimage[3 * p + 1]; g2 = dL_dimage[3 * p + 2];
+        sI = image[3 * p] * g0 + image[3 * p + 1] * g1 + image[3 * p + 2] * g2;           // <G, final colour of the pixel>
       }
-      const float z = warp_reduce8(v, lane);
+      // transmittance and <G, colour composited so far> in front of this segment, from the forward's segment partials
+      float T = 1.f, sF = 0.f;
+      const float4* pp = part + (size_t)so * BB + tid;
+      for (int s0 = 0; s0 < seg; s0 += 4) {
+        float4 q[4];
 #pragma unroll
-      for (int o = 16; o; o >>= 1) s0 += __shfl_xor_sync(0xffffffffu, s0, o);
-      if ((lane & 3) == 0) {
-        const int k = lane >> 2;                                          // 0..7 -> acc slots 0,1,2 (colour) and 4..8 (moments)
-        atomicAdd(&st.acc[j][k < 3 ? k : k + 1], z);
-        if (lane == 0) atomicAdd(&st.acc[j][3], s0);
+        for (int u = 0; u < 4; ++u) if (s0 + u < seg) q[u] = pp[(size_t)(s0 + u) * BB];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (s0 + u < seg) { sF = fmaf(T, q[u].x * g0 + q[u].y * g1 + q[u].z * g2, sF); T *= q[u].w; }
+      }
+      const float bcx = (float)((int)(tile % TX) * RGA_TILE + btile_px(tid & ~31u)) + 4.0f;
+      const float bcy = (float)((int)(tile / TX) * RGA_TILE + btile_py(tid & ~31u)) + 2.0f;
+      const int jend = min(m, wlast - b0);
+      for (int j = 0; j < jend; ++j) {
+        const float2 mm = st.mu[j], ex = st.ext[j];
+        if (fabsf(mm.x - bcx) > ex.x + 3.5f || fabsf(mm.y - bcy) > ex.y + 1.5f) continue;
+        const float4 co = st.co[j];
+        const float dx = mm.x - fx, dy = mm.y - fy;
+        const float p2 = dx * (co.x * dx + co.y * dy) + co.z * dy * dy;   // log2(e) * power, as in the forward
+        const float raw = co.w * bex2_approx(p2);
+        const float a = fminf(0.99f, raw);
+        const bool valid = (b0 + j < last) && !(p2 > 0.f || a < 1.f / 255.f);
+        if (!__any_sync(0xffffffffu, valid)) continue;
+        float v[8], s0 = 0.f;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = 0.f;
+        if (valid) {
+          const float4 c = st.col[j];
+          const float wgt = a * T, sc = c.x * g0 + c.y * g1 + c.z * g2, om = 1.f - a;
+          v[0] = wgt * g0; v[1] = wgt * g1; v[2] = wgt * g2;
+          sF = fmaf(wgt, sc, sF);
+          // dL/dalpha = T <G, c> - <G, everything behind this entry> / (1 - alpha); "behind" = final colour - prefix
+          const float dLda = T * sc - __fdividef(sI - sF, om);
+          T *= om;
+          const float w = raw > 0.99f ? 0.f : a * dLda;
+          s0 = w;
+          v[3] = w * dx; v[4] = w * dy; v[5] = w * dx * dx; v[6] = w * dx * dy; v[7] = w * dy * dy;
+        }
+        const float z = warp_reduce8(v, lane);
+#pragma unroll
+        for (int o = 16; o; o >>= 1) s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+        if ((lane & 3) == 0) {
+          const int k = lane >> 2;                                        // 0..7 -> acc slots 0,1,2 (colour) and 4..8 (moments)
+          atomicAdd(&st.acc[j][k < 3 ? k : k + 1], z);
+          if (lane == 0) atomicAdd(&st.acc[j][3], s0);
+        }
       }
     }
     __syncthreads();
@@ -138,6 +147,7 @@ __global__ void __launch_bounds__(BB) composite_backward_kernel(int W, int H, in
 #pragma unroll
       for (int k = 0; k < 9; ++k) { const float x = st.acc[tid][k]; if (x != 0.f) atomicAdd(gdst + k, x); }
     }
+    __syncthreads();
   }
 }
 
@@ -213,13 +223,14 @@ __global__ void __launch_bounds__(256) project_backward_kernel(int ng, CamB cam,
   }
 }
 
-cudaError_t rga_launch_splat_backward(rga_avatar* av, const rga_camera* cam, float3 bg, const float* dL_dimage, float* out_dcolor,
-                                      float* out_dopacity, float* out_dmean, float* out_dcov, cudaStream_t s) {
-  const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
+cudaError_t rga_launch_splat_backward(rga_avatar* av, const rga_camera* cam, float3 bg, const float* image, const float* dL_dimage,
+                                      float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, cudaStream_t s) {
+  const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE;
   cudaError_t e = cudaMemsetAsync(av->splat_grad, 0, sizeof(float) * 12 * (size_t)av->n_gauss, s);
   if (e != cudaSuccess) return e;
-  composite_backward_kernel<<<TX * TY, BB, 0, s>>>(cam->width, cam->height, TX, bg, av->ranges, av->vals[0], av->mu2d, av->conic_o,
-                                                   av->color, av->t_final, av->n_contrib, dL_dimage, av->splat_grad);
+  composite_backward_kernel<<<av->num_sms * 4, BB, 0, s>>>(cam->width, cam->height, TX, bg, av->num_items, av->item_tab, av->seg_off,
+                                                           av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, av->part,
+                                                           av->n_contrib, image, dL_dimage, av->splat_grad);
   rga_prof_mark(av, "composite_backward", s);
   CamB k;
   for (int i = 0; i < 9; ++i) k.R[i] = cam->R_wc[i];

@@ -128,8 +128,8 @@ cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s)
 cudaError_t rga_launch_knn_verts(rga_avatar* av, float* d2, cudaStream_t s);
 int rga_mlp_init_attributes();
 // backward_kernels.cu
-cudaError_t rga_launch_splat_backward(rga_avatar* av, const rga_camera* cam, float3 bg, const float* dL_dimage, float* out_dcolor,
-                                      float* out_dopacity, float* out_dmean, float* out_dcov, cudaStream_t s);
+cudaError_t rga_launch_splat_backward(rga_avatar* av, const rga_camera* cam, float3 bg, const float* image, const float* dL_dimage,
+                                      float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, cudaStream_t s);
 // densify_kernels.cu
 cudaError_t rga_launch_densify(rga_avatar* av, float d0, float p0, const unsigned* rnd, int max_out, float* out_pos, int* out_tri,
                                int* out_count, cudaStream_t s);

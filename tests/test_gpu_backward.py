@@ -32,7 +32,7 @@ def _run(cfg, n_gauss=None, vis_mode=0, use_visibility=True, bg=None):
     dev = "cuda"
     d_col = torch.full((N, 3), float("nan"), device=dev); d_op = torch.full((N,), float("nan"), device=dev)
     d_x = torch.full((N, 3), float("nan"), device=dev); d_cov = torch.full((N, 6), float("nan"), device=dev)
-    rga.splat_backward(av.h, cam, inp["bg"], torch.as_tensor(G).to(dev), d_col, d_op, d_x, d_cov)
+    rga.splat_backward(av.h, cam, inp["bg"], torch.as_tensor(np.ascontiguousarray(img, np.float32)).to(dev), torch.as_tensor(G).to(dev), d_col, d_op, d_x, d_cov)
     rga.rga_check(av.h)
     sg = av.read("SPLAT_GRAD").reshape(N, 12)
     got = {"d_col": d_col.cpu().numpy(), "d_opac": d_op.cpu().numpy(), "d_mu": sg[:, 4:6], "d_conic": sg[:, 6:9],
@@ -68,5 +68,5 @@ def test_splat_backward_argument_checks():
     av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=16, max_vis_res=32, max_env_texels=512)
     G = torch.zeros((H, W, 3), device="cuda")
     with pytest.raises(RuntimeError):
-        rga.splat_backward(av.h, cam, inp["bg"], G)                      # nothing rendered yet
+        rga.splat_backward(av.h, cam, inp["bg"], G, G)                   # nothing rendered yet
     av.close()
