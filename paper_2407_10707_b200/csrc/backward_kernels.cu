@@ -3,13 +3,18 @@
 // lists and order, culled Gaussians, per-pixel skips and the stopping entry) with respect to every Gaussian's splatted
 // colour, opacity, posed mean and 3D covariance.  FAST source: compared with the fp64 autograd oracle under tolerance.
 //
-//   composite_backward_kernel   one CTA per tile, one thread per pixel (the forward's 8x4-pixel warp blocks).  The list
-//                               is walked BACK TO FRONT from the tile's last contributing entry in batches of 256
-//                               staged in shared memory; a pixel recovers T_i = T_{i+1} / (1 - alpha_i) from its final
-//                               transmittance, keeps the colour composited behind it (accum) and forms dL/dalpha_i.
+//   composite_backward_kernel   persistent CTAs over the forward's work items (one RGA_SEG-entry segment of one tile's
+//                               list), one thread per pixel of the tile (the forward's 8x4-pixel warp blocks).  With
+//                               F_i the colour composited up to and including entry i and I the pixel's final colour,
+//                                   dL/dalpha_i = T_i <G, c_i> - <G, I - F_i> / (1 - alpha_i),
+//                               so the list can be walked FRONT TO BACK like the forward, and a segment can start on
+//                               its own: T and <G, F> in front of it are folded from the per-segment partials (C, T)
+//                               the forward left in `part`; I is the rendered image.  (The first version walked each
+//                               tile's list back to front in one CTA, recovering T by division: 383 us at config 1
+//                               against 89 us, for the same reason the forward is segment-parallel.)
 //                               Per entry a warp reduces nine sums over its 32 pixels with a transposed butterfly
-//                               (14 shuffles instead of 45), adds them to the batch's shared-memory accumulators, and
-//                               after the batch one thread per entry issues the global atomics.
+//                               (14 shuffles instead of 45) into the segment's shared-memory accumulators; after the
+//                               segment one thread per entry issues the global atomics.
 //                               The nine sums: dL/dc (3) and the moments S = sum w, sum w dx, sum w dy, sum w dx^2,
 //                               sum w dx dy, sum w dy^2 of w = alpha dL/dalpha (0 where alpha is clamped to 0.99: the
 //                               clamp has derivative 0, reading A32) with d = mu - pixel, from which
