@@ -122,3 +122,75 @@ def splat_backward(xg, cov6, col, opac, cam, bg, vals, ranges, touched, G, mu32=
         d_x[alive] = x_a.grad.numpy(); d_cov[alive] = cov_a.grad.numpy()
     return {"image": image, "T_final": Tf, "n_contrib": nc, "d_col": z(colt, (N, 3)), "d_opac": z(opt, (N,)), "d_mu": d_mu,
             "d_conic": d_conic, "d_x": d_x, "d_cov6": d_cov}
+
+
+# ------------------------------------------------------------------------------------------------ H5 (shading)
+def texel_visibility(n_gauss, n_texels, t2d, vis_mode, bits=None, vg=None):
+    """v_g[k] per (Gaussian, env texel) as a dense fp64 array, the way orc_shade reads it: mode 0 = bit texel_to_dir[k] of
+    bits[g]; mode 1 = vg[g][texel_to_dir[k]]; mode 2 = 1."""
+    d = np.arange(n_texels) if t2d is None else np.asarray(t2d, np.int64)
+    if vis_mode == 0:
+        b = np.asarray(bits).reshape(n_gauss, -1)
+        return ((b[:, d >> 5] >> (d & 31).astype(np.uint32)[None, :]) & 1).astype(np.float64)
+    if vis_mode == 1:
+        return np.asarray(vg, np.float64)[:, d]
+    return np.ones((n_gauss, n_texels))
+
+
+def shade_torch(x, n, alb, rough, spec, cam_pos, env, W, A, v, gamma):
+    """H5 for a block of Gaussians, differentiable: Eq.2 with the Appendix-A BRDF (Eq.12-15, :454-471),
+    same formulas and rules as orc_shade / brdf (rga_oracle.cpp): w_o = normalize(cam - x); texels with w_i.n <= 0 or
+    v = 0 are skipped; s = D F / (4 ((n.w_i)(1-k)+k) ((n.w_o)^+ (1-k)+k)); L_o = sum_k L_k A_k (a/pi + p s) v (w_i.n);
+    colour = clamp(L_o, 0, 1)^(1/gamma), with derivative 0 at and beyond the clamp limits (reading A33).
+    x, n, alb [m,3], rough, spec [m], env [ne,3], W [ne,3], A [ne], v [m,ne].  Returns L_o [m,3], colour [m,3]."""
+    PI = np.pi
+    wo = cam_pos[None, :] - x
+    wo = wo / wo.norm(dim=1, keepdim=True)
+    cs = n @ W.T                                                     # [m,ne]  w_i . n
+    with torch.no_grad():
+        live = (cs > 0.0) & (v != 0.0)
+    h = W[None, :, :] + wo[:, None, :]
+    hl = h.norm(dim=2)
+    ok = hl > 0.0
+    h = h / torch.where(ok, hl, torch.ones_like(hl))[:, :, None]
+    nh = (n[:, None, :] * h).sum(2); oh = (wo[:, None, :] * h).sum(2)
+    no = torch.clamp((n * wo).sum(1), min=0.0)[:, None]
+    al2 = (rough * rough)[:, None] ** 2                              # Eq.13: alpha = gamma^2
+    den = nh * nh * (al2 - 1.0) + 1.0
+    D = al2 / (PI * den * den)
+    F = 0.04 + 0.96 * torch.exp2((-5.55473 * oh - 6.98316) * oh)     # Eq.14
+    k = ((rough + 1.0) ** 2 / 8.0)[:, None]                          # Eq.15
+    s = D * F / (4.0 * (cs * (1.0 - k) + k) * (no * (1.0 - k) + k))
+    s = torch.where(ok, s, torch.zeros_like(s))
+    R = alb[:, None, :] / PI + spec[:, None, None] * s[:, :, None]   # Eq.12
+    term = env[None, :, :] * A[None, :, None] * R * (v * cs)[:, :, None]
+    Lo = torch.where(live[:, :, None], term, torch.zeros_like(term)).sum(1)
+    inside = (Lo > 0.0) & (Lo < 1.0)
+    col = torch.where(inside, torch.where(inside, Lo, torch.ones_like(Lo)) ** (1.0 / gamma), (Lo >= 1.0).to(F64))
+    return Lo, col
+
+
+def shade_backward(xg, ng, alb, rough, spec, cam_pos, env, v, gamma, d_col, block=2048):
+    """Forward radiance / colour of H5 and the gradient of L = sum(d_col * colour) w.r.t. the posed position (through w_o),
+    posed normal, albedo, roughness, specular of every Gaussian and the environment map.  env [rows, cols, 3]; v dense
+    visibility [N, rows*cols] (texel_visibility).  Gaussians are processed in blocks (one autograd graph at a time); the
+    environment gradient accumulates over blocks.  Returns numpy fp64 arrays."""
+    from . import oracle as _orc
+    rows, cols = env.shape[0], env.shape[1]
+    Wn, An = _orc.env_table(rows, cols)
+    W, A = _t(Wn), _t(An)
+    envt = _t(np.asarray(env).reshape(-1, 3)).requires_grad_(True)
+    cam = _t(cam_pos)
+    N = len(xg)
+    out = {k: np.zeros(s) for k, s in (("Lo", (N, 3)), ("color", (N, 3)), ("d_x", (N, 3)), ("d_n", (N, 3)), ("d_alb", (N, 3)),
+                                      ("d_rough", (N,)), ("d_spec", (N,)))}
+    for b0 in range(0, N, block):
+        sl = slice(b0, min(b0 + block, N))
+        leaves = [_t(np.asarray(a)[sl]).requires_grad_(True) for a in (xg, ng, alb, rough, spec)]
+        Lo, col = shade_torch(*leaves, cam, envt, W, A, _t(np.asarray(v)[sl]), gamma)
+        (col * _t(np.asarray(d_col)[sl])).sum().backward()
+        out["Lo"][sl] = Lo.detach().numpy(); out["color"][sl] = col.detach().numpy()
+        for name, leaf in zip(("d_x", "d_n", "d_alb", "d_rough", "d_spec"), leaves):
+            out[name][sl] = leaf.grad.numpy()
+    out["d_env"] = (np.zeros((rows * cols, 3)) if envt.grad is None else envt.grad.numpy()).reshape(rows, cols, 3)
+    return out

@@ -226,3 +226,8 @@ def make_image_cotangent(seed, width, height):
     """dL/dimage for the backward pass: a seeded standard-normal field [height, width, 3] (fp32).  An input of both the
     oracle and the library; the loss that would produce it (Eq.5) is not part of this module."""
     return np.random.default_rng(1000 + seed).normal(size=(height, width, 3)).astype(np.float32)
+
+
+def make_color_cotangent(seed, n_gauss):
+    """dL/dcolour per Gaussian for the backward of the shading step: seeded standard normal [n_gauss, 3] (fp32)."""
+    return np.random.default_rng(2000 + seed).normal(size=(n_gauss, 3)).astype(np.float32)

@@ -175,3 +175,106 @@ def test_projection_closed_form_and_gradcheck():
         return C
 
     assert torch.autograd.gradcheck(f, (X, COV, COL, OP), eps=1e-7, atol=1e-6, rtol=1e-4)
+
+
+# ------------------------------------------------------------------------------------------------ H5 backward
+@pytest.fixture(scope="module")
+def shade0():
+    inp = workloads.make(0)
+    av = orc.avatar_load(inp)
+    o = orc.render_frame(av, inp, vis_mode=0)
+    env = inp["env"][inp["env_of_frame"][0]]
+    N = len(inp["gauss_pos"]); ne = env.shape[0] * env.shape[1]
+    v = bwd.texel_visibility(N, ne, inp["texel_to_dir"], 0, bits=o["visbits"])
+    d_col = workloads.make_color_cotangent(5, N)
+    r = bwd.shade_backward(o["gauss_posed"], o["gauss_normal_posed"], av["albedo_g"], av["rough_g"], av["spec_g"], inp["cam_pos"], env, v,
+                           inp["gamma"], d_col)
+    return inp, av, o, env, v, d_col, r
+
+
+def test_shade_backward_oracle_forward_equals_cpp_oracle(shade0):
+    inp, av, o, env, v, d_col, r = shade0
+    assert np.abs(r["Lo"] - o["L_o"]).max() < 1e-12 and np.abs(r["color"] - o["color"]).max() < 1e-12
+    # the paper's visibility (mode 1: fractional v_g) through the same function
+    o1 = orc.render_frame(av, inp, vis_mode=1)
+    v1 = bwd.texel_visibility(len(v), v.shape[1], inp["texel_to_dir"], 1, vg=o1["vis_g"])
+    r1 = bwd.shade_backward(o1["gauss_posed"], o1["gauss_normal_posed"], av["albedo_g"], av["rough_g"], av["spec_g"], inp["cam_pos"], env, v1,
+                            inp["gamma"], d_col)
+    assert np.abs(r1["Lo"] - o1["L_o"]).max() < 1e-12
+
+
+def test_shade_gradients_match_finite_differences_through_cpp_shade(shade0):
+    inp, av, o, env, v, d_col, r = shade0
+    base = dict(xg=o["gauss_posed"].astype(np.float32), ng=o["gauss_normal_posed"].astype(np.float32), alb=av["albedo_g"].astype(np.float32),
+                rough=av["rough_g"].astype(np.float32), spec=av["spec_g"].astype(np.float32), env=env.astype(np.float32))
+
+    def loss(**kw):
+        a = dict(base); a.update(kw)
+        Lo, col = orc.shade(a["xg"], a["ng"], a["alb"], a["rough"], a["spec"], inp["cam_pos"], a["env"], inp["texel_to_dir"], 0,
+                            bits=o["visbits"], K=len(inp["vis_dirs"]), gamma=inp["gamma"])
+        return (col * d_col).sum(1)                                      # per Gaussian: they are independent
+
+    lit = np.nonzero((o["L_o"] > 1e-3).all(1) & (o["L_o"] < 0.98).all(1))[0]          # away from the clamp limits
+    for key, grad, h in (("xg", r["d_x"], 2.0 ** -10), ("ng", r["d_n"], 2.0 ** -12), ("alb", r["d_alb"], 2.0 ** -10),
+                         ("rough", r["d_rough"], 2.0 ** -12), ("spec", r["d_spec"], 2.0 ** -10)):
+        arr = base[key]
+        for c in range(arr.shape[1] if arr.ndim == 2 else 1):
+            ap, am = arr.copy(), arr.copy()
+            if arr.ndim == 2:
+                ap[:, c] += np.float32(h); am[:, c] -= np.float32(h)
+                step = ap[:, c].astype(np.float64) - am[:, c]; an = grad[:, c]
+            else:
+                ap += np.float32(h); am -= np.float32(h)
+                step = ap.astype(np.float64) - am; an = grad
+            fd = (loss(**{key: ap}) - loss(**{key: am})) / step
+            err = np.abs(fd[lit] - an[lit])
+            good = err < 2e-3 * np.abs(an[lit]) + 2e-4 * np.abs(an[lit]).max()
+            assert good.mean() > 0.98, (key, c, good.mean())              # the few misses: a texel's w_i.n changes sign inside the step
+    # environment: L is linear in it up to the gamma curve; perturb single texels
+    rs = np.random.default_rng(1)
+    for _ in range(6):
+        i, j, c = rs.integers(env.shape[0]), rs.integers(env.shape[1]), rs.integers(3)
+        ep, em = base["env"].copy(), base["env"].copy(); ep[i, j, c] += np.float32(2.0 ** -8); em[i, j, c] -= np.float32(2.0 ** -8)
+        fd = (loss(env=ep)[lit].sum() - loss(env=em)[lit].sum()) / (float(ep[i, j, c]) - float(em[i, j, c]))
+        rl = bwd.shade_backward(base["xg"][lit], base["ng"][lit], base["alb"][lit], base["rough"][lit], base["spec"][lit], inp["cam_pos"], env,
+                                v[lit], inp["gamma"], d_col[lit])
+        assert abs(fd - rl["d_env"][i, j, c]) < 2e-3 * abs(fd) + 1e-4 * np.abs(rl["d_env"]).max()
+
+
+def test_shade_backward_lambert_closed_form_and_clamp():
+    # spec = 0, v = 1, gamma = 1: colour = L_o = a / pi * E(n), E = sum_k L_k A_k max(0, w_k.n)  (the white-furnace pin's
+    # setting).  Hand derivatives: d/da = g E / pi, d/dL_k = g a A_k (w_k.n)^+ / pi, d/dn = g a / pi sum_{w_k.n > 0} L_k A_k w_k
+    rows, cols = 8, 16
+    W, A = orc.env_table(rows, cols)
+    rs = np.random.default_rng(3)
+    env = rs.uniform(0.05, 0.3, (rows, cols, 3))
+    n = np.array([[0.3, -0.5, 0.81]]); n /= np.linalg.norm(n)
+    x = np.array([[0.1, 0.2, 0.3]]); alb = np.array([[0.5, 0.6, 0.7]]); g = np.array([[0.7, -0.4, 1.1]])
+    r = bwd.shade_backward(x, n, alb, np.array([0.5]), np.array([0.0]), np.array([0.0, -3.0, 0.5]), env, np.ones((1, rows * cols)), 1.0, g)
+    cs = np.maximum(W @ n[0], 0.0)
+    E = (env.reshape(-1, 3) * (A * cs)[:, None]).sum(0)
+    assert np.allclose(r["Lo"][0], alb[0] / np.pi * E)
+    assert np.allclose(r["d_alb"][0], g[0] * E / np.pi)
+    assert np.allclose(r["d_env"].reshape(-1, 3), (A * cs)[:, None] * (alb[0] * g[0])[None, :] / np.pi)
+    assert np.allclose(r["d_n"][0], ((env.reshape(-1, 3) * (alb[0] * g[0])[None, :]).sum(1) * A * (cs > 0)) @ W / np.pi)
+    assert np.allclose(r["d_x"][0], 0.0) and r["d_spec"][0] != 0.0      # Lambert term ignores w_o; the specular slot still has slope
+    # clamp (reading A33): radiance above 1 (or 0) has colour 1 (0) and no gradient at all
+    r = bwd.shade_backward(x, n, alb, np.array([0.5]), np.array([0.0]), np.array([0.0, -3.0, 0.5]), env * 100.0, np.ones((1, rows * cols)), 2.2, g)
+    assert np.all(r["color"] == 1.0) and not r["d_alb"].any() and not r["d_env"].any()
+    r = bwd.shade_backward(x, n, alb, np.array([0.5]), np.array([0.3]), np.array([0.0, -3.0, 0.5]), env, np.zeros((1, rows * cols)), 2.2, g)
+    assert np.all(r["color"] == 0.0) and not r["d_alb"].any() and not r["d_n"].any()
+
+
+def test_shade_backward_gradcheck():
+    rows, cols = 4, 8
+    Wn, An = orc.env_table(rows, cols)
+    rs = np.random.default_rng(4)
+    m = 3
+    t = lambda a: torch.tensor(a, dtype=torch.float64, requires_grad=True)
+    nn = rs.normal(size=(m, 3)); nn /= np.linalg.norm(nn, axis=1, keepdims=True)
+    args = (t(rs.normal(size=(m, 3)) * 0.2), t(nn), t(rs.uniform(0.2, 0.8, (m, 3))), t(rs.uniform(0.3, 0.8, m)), t(rs.uniform(0.2, 0.8, m)))
+    env = t(rs.uniform(0.05, 0.2, (rows * cols, 3)))
+    cam = torch.tensor([0.3, -2.5, 0.4], dtype=torch.float64)
+    v = torch.tensor(rs.uniform(0.2, 1.0, (m, rows * cols)) * (rs.uniform(size=(m, rows * cols)) > 0.3))
+    f = lambda x, n, a, r, s, e: bwd.shade_torch(x, n, a, r, s, cam, e, torch.tensor(Wn), torch.tensor(An), v, 2.2)[1]
+    assert torch.autograd.gradcheck(f, args + (env,), eps=1e-7, atol=1e-6, rtol=1e-4)
