@@ -266,6 +266,19 @@ def main():
     bwd_obj = {"ms": ms_bwd, "kernel_ms": {k: float(np.mean(v)) for k, v in bwd_k.items() if k != "-"},
                "note": "gradients w.r.t. colour, opacity, posed mean and 3D covariance of every Gaussian; L2 flushed between calls"}
 
+    # ... and of the shading step H5, fed with the colour gradient the splat's backward just produced
+    ne_all = int(env.shape[0] * env.shape[1])
+    sb = dict(out_dalbedo=torch.empty((ng_all, 3), device=dev), out_drough=torch.empty((ng_all,), device=dev),
+              out_dspec=torch.empty((ng_all,), device=dev), out_dnormal=torch.empty((ng_all, 3), device=dev),
+              out_dpos=torch.empty((ng_all, 3), device=dev), out_denv=torch.empty((ne_all, 3), device=dev))
+    run_sb = lambda: rga.shade_backward(av.h, env, inp["cam_pos"], d_col, texel_to_dir=t2d, gamma=inp["gamma"], use_visibility=True, **sb)
+    for _ in range(3):
+        run_sb()
+    ms_sb = timed(run_sb, 20)
+    n_grad = int((d_col.abs().sum(1) > 0).sum().item())
+    sb_obj = {"ms": ms_sb, "gaussians_with_gradient": n_grad, "texels": ne_all,
+              "note": "albedo, roughness, specular, normal, position and environment-map gradients; env table rebuilt inside the call"}
+
     # algorithmic units of each candidate dominant kernel: counted from the frame that was rendered
     gp = av.read("GAUSS_POSED").reshape(-1, 4)[:, :3]; gn = av.read("GAUSS_NORMAL_POSED").reshape(-1, 4)[:, :3]
     front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
@@ -336,7 +349,7 @@ def main():
                 "pipelined_value": world * 1e3 / ms_e2e_pipe,
                 "pipelined_note": "image read-back of step i on a copy stream beside step i+1; per-step events plus the last copy's tail"},
         "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
-        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj,
+        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj, "shade_backward": sb_obj,
         "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -146,6 +146,19 @@ RGA_API rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, void
 RGA_API rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* image, const float* dL_dimage,
                                   float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, void* stream);
 
+/* Backward of shade_gaussians (the material / lighting side of training): for the shading last
+ * computed by shade_gaussians or rga_render_frame with THIS env and cam_pos, and dL_dcolor = dL/d(colour) per Gaussian
+ * (dev [n_gauss][3], e.g. splat_backward's out_dcolor), the gradient of L with respect to every Gaussian's albedo
+ * a_g, roughness gamma_g, specular p_g, posed normal n_gd (as a free 3-vector) and posed position (through w_o only),
+ * and with respect to the environment map L.  Visibility is a frozen input.  colour = clamp(L_o, 0, 1)^(1/gamma) has
+ * derivative 0 at and beyond the clamp limits (reading A33), so a Gaussian whose radiance is 0 (hidden,
+ * facing away) or >= 1 in a channel gets no gradient from that channel.
+ * Outputs are DEVICE buffers, each may be NULL: out_dalbedo [n_gauss][3], out_drough [n_gauss], out_dspec [n_gauss],
+ * out_dnormal [n_gauss][3], out_dpos [n_gauss][3], out_denv [rows][cols][3].  Enqueue-only. */
+RGA_API rga_status shade_backward(rga_avatar* av, const rga_env* env, const float cam_pos[3], const float* dL_dcolor,
+                                  float* out_dalbedo, float* out_drough, float* out_dspec, float* out_dnormal, float* out_dpos,
+                                  float* out_denv, void* stream);
+
 /* Algorithm 1, "Gaussian densification based on density": from the avatar's current
  * S_g (avatar_load / gaussians_update) and its mesh, counts the Gaussians near every vertex (D_v), estimates the Gaussian
  * density of every triangle d_f = sum of its three D_v / (6 K_g), sets P = max(0, d0 - d_f), asks for

@@ -166,6 +166,17 @@ def shade_gaussians(h, radiance, cam_pos, texel_to_dir=None, gamma=2.2, use_visi
     _chk(lib().shade_gaussians(h, C.byref(e), cp, _stream()))
 
 
+def shade_backward(h, radiance, cam_pos, dL_dcolor, texel_to_dir=None, gamma=2.2, use_visibility=True, out_dalbedo=None, out_drough=None,
+                   out_dspec=None, out_dnormal=None, out_dpos=None, out_denv=None):
+    """Backward of shade_gaussians for the last shaded frame (include/rga.h shade_backward).  All tensors CUDA float32."""
+    e = _Env(int(radiance.shape[0]), int(radiance.shape[1]), radiance.data_ptr(),
+             0 if texel_to_dir is None else texel_to_dir.data_ptr(), gamma, int(use_visibility))
+    cp = (C.c_float * 3)(*[float(v) for v in cam_pos])
+    lib().shade_backward.argtypes = [C.c_void_p, C.POINTER(_Env), C.c_float * 3] + [C.c_void_p] * 8
+    _chk(lib().shade_backward(h, C.byref(e), cp, _ptr(dL_dcolor), _ptr(out_dalbedo), _ptr(out_drough), _ptr(out_dspec), _ptr(out_dnormal),
+                              _ptr(out_dpos), _ptr(out_denv), _stream()))
+
+
 def splat_render(h, camera, bg, out_image):
     cam = camera if isinstance(camera, _Camera) else make_camera(camera)
     b = (C.c_float * 3)(*[float(v) for v in bg])

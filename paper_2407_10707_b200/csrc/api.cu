@@ -182,7 +182,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(rga_launch_knn_gauss(av, d->gauss_pos, s));
   A(rga_launch_load_gauss(av, d->gauss_pos, d->gauss_quat, d->gauss_scale, d->gauss_opacity, av->knn_d2, s));
   av->launches += 5;
-  if (rga_shade_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_composite_init_attributes() != 0 || rga_mlp_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
+  if (rga_shade_init_attributes(av->max_env) != 0 || rga_shade_backward_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_composite_init_attributes() != 0 || rga_mlp_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
   A(cudaStreamSynchronize(s));
 done:
   if (d2) cudaFree(d2);
@@ -273,6 +273,23 @@ extern "C" rga_status splat_backward(rga_avatar* av, const rga_camera* cam, cons
   cudaStream_t s = (cudaStream_t)stream;
   rga_prof_mark(av, "-", s);
   CU(rga_launch_splat_backward(av, cam, make_float3(bg[0], bg[1], bg[2]), image, dL_dimage, out_dcolor, out_dopacity, out_dmean, out_dcov, s));
+  return RGA_OK;
+}
+
+extern "C" rga_status shade_backward(rga_avatar* av, const rga_env* env, const float cam_pos[3], const float* dL_dcolor, float* out_dalbedo,
+                                     float* out_drough, float* out_dspec, float* out_dnormal, float* out_dpos, float* out_denv, void* stream) {
+  if (!av || !env || !env->radiance || !cam_pos || !dL_dcolor) return fail(RGA_ERR_INVALID_ARG, "shade_backward: null argument");
+  if (!av->have_shade) return fail(RGA_ERR_STATE, "shade_backward: call shade_gaussians (or rga_render_frame) first");
+  if (env->use_visibility && !av->have_vis) return fail(RGA_ERR_STATE, "shade_backward: no visibility for this pose");
+  if (env->rows < 1 || env->cols < 1 || env->rows * env->cols > av->max_env || !(env->gamma > 0.f))
+    return fail(RGA_ERR_INVALID_ARG, "shade_backward: env size/gamma out of range");
+  if (env->use_visibility && !env->texel_to_dir && env->rows * env->cols != av->vis_dirs)
+    return fail(RGA_ERR_INVALID_ARG, "shade_backward: identity texel_to_dir needs rows*cols == n_dirs");
+  cudaStream_t s = (cudaStream_t)stream;
+  rga_prof_mark(av, "-", s);
+  CU(rga_launch_env_table(av, env, s));
+  CU(rga_launch_shade_backward(av, env, make_float3(cam_pos[0], cam_pos[1], cam_pos[2]), env->use_visibility ? av->vis_mode : 2, dL_dcolor,
+                               out_dalbedo, out_drough, out_dspec, out_dnormal, out_dpos, out_denv, s));
   return RGA_OK;
 }
 

@@ -130,6 +130,10 @@ int rga_mlp_init_attributes();
 // backward_kernels.cu
 cudaError_t rga_launch_splat_backward(rga_avatar* av, const rga_camera* cam, float3 bg, const float* image, const float* dL_dimage,
                                       float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, cudaStream_t s);
+// shade_backward_kernels.cu
+cudaError_t rga_launch_shade_backward(rga_avatar* av, const rga_env* env, float3 cam, int vis_mode, const float* dL_dcolor, float* out_dalbedo,
+                                      float* out_drough, float* out_dspec, float* out_dnormal, float* out_dpos, float* out_denv, cudaStream_t s);
+int rga_shade_backward_init_attributes(int max_env);
 // densify_kernels.cu
 cudaError_t rga_launch_densify(rga_avatar* av, float d0, float p0, const unsigned* rnd, int max_out, float* out_pos, int* out_tri,
                                int* out_count, cudaStream_t s);

@@ -20,7 +20,7 @@ __global__ void env_table_kernel(int rows, int cols, const float* __restrict__ r
   sincospif(2.0f * ((float)j + 0.5f) / (float)cols, &sp, &cp);
   float A = 2.0f * st * sinpif(0.5f / (float)rows) * (2.0f * PI_F / (float)cols);
   float4* t = reinterpret_cast<float4*>(table) + 2 * (size_t)k;
-  t[0] = make_float4(st * cp, st * sp, ct, 0.f);
+  t[0] = make_float4(st * cp, st * sp, ct, A);                       // .w = A_k: read by the backward pass only
   t[1] = make_float4(radiance[3 * k] * A, radiance[3 * k + 1] * A, radiance[3 * k + 2] * A, 0.f);
 }
 

@@ -70,3 +70,61 @@ def test_splat_backward_argument_checks():
     with pytest.raises(RuntimeError):
         rga.splat_backward(av.h, cam, inp["bg"], G, G)                   # nothing rendered yet
     av.close()
+
+
+# shading backward: the gradients scale with (1/gamma) L_o^(1/gamma - 1), i.e. they are largest for the darkest lit
+# Gaussians, whose fp32 forward radiance carries the largest relative error; tolerances as fractions of the largest
+# reference magnitude of each array (measured values in DESIGN.md)
+SH_TOL_MAX, SH_TOL_MEAN = 2e-3, 5e-6          # measured: <= 7.5e-4 (d_x) and <= 9e-7
+
+
+@pytest.mark.parametrize("cfg,vis_mode,use_vis", [(0, 0, True), (0, 1, True), (0, 0, False), (1, 0, True), (1, 1, True)])
+def test_shade_backward_matches_autograd_oracle(cfg, vis_mode, use_vis):
+    import torch
+    from oracle import backward as bwd
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import run_gpu
+    inp = workloads.make(cfg, n_gauss=30_000 if cfg == 1 else None)
+    orc_av = orc.avatar_load(inp)
+    mode = vis_mode if use_vis else 2
+    o = orc.render_frame(orc_av, inp, vis_mode=mode, stop_after="shade")
+    env = inp["env"][inp["env_of_frame"][0]]
+    N = len(inp["gauss_pos"]); ne = env.shape[0] * env.shape[1]
+    v = bwd.texel_visibility(N, ne, inp["texel_to_dir"], mode, bits=o.get("visbits"), vg=o.get("vis_g"))
+    d_col = workloads.make_color_cotangent(cfg, N)
+    ref = bwd.shade_backward(o["gauss_posed"], o["gauss_normal_posed"], orc_av["albedo_g"], orc_av["rough_g"], orc_av["spec_g"], inp["cam_pos"],
+                             env, v, inp["gamma"], d_col)
+    av, img = run_gpu(inp, vis_mode=vis_mode, use_visibility=use_vis, keep_maps=False)
+    dev = "cuda"
+    nanf = lambda *s: torch.full(s, float("nan"), device=dev)
+    outs = dict(out_dalbedo=nanf(N, 3), out_drough=nanf(N), out_dspec=nanf(N), out_dnormal=nanf(N, 3), out_dpos=nanf(N, 3),
+                out_denv=nanf(env.shape[0], env.shape[1], 3))
+    rga.shade_backward(av.h, torch.as_tensor(env).to(dev), inp["cam_pos"], torch.as_tensor(d_col).to(dev),
+                       texel_to_dir=torch.as_tensor(inp["texel_to_dir"]).to(dev), gamma=inp["gamma"], use_visibility=use_vis, **outs)
+    rga.rga_check(av.h)
+    # the library skips Gaussians that face away from the camera (their colour is never splatted); the
+    # oracle's shade function does not know the camera's cull, so compare the Gaussians the forward pass keeps
+    facing = ((inp["cam_pos"][None, :] - o["gauss_posed"]) * o["gauss_normal_posed"]).sum(1) >= 1e-3
+    keep = facing
+    rep = {}
+    for name, key in (("d_alb", "out_dalbedo"), ("d_rough", "out_drough"), ("d_spec", "out_dspec"), ("d_n", "out_dnormal"), ("d_x", "out_dpos")):
+        g = outs[key].cpu().numpy(); r = ref[name]
+        assert np.isfinite(g).all(), name
+        scale = np.abs(r[keep]).max()
+        rep[name] = (float(np.abs(g[keep] - r[keep]).max() / scale), float(np.abs(g[keep] - r[keep]).mean() / scale), float(scale))
+    # environment gradient: sums over all Gaussians, so the oracle's is recomputed over the kept ones only
+    ref_env = bwd.shade_backward(o["gauss_posed"][keep], o["gauss_normal_posed"][keep], orc_av["albedo_g"][keep], orc_av["rough_g"][keep],
+                                 orc_av["spec_g"][keep], inp["cam_pos"], env, v[keep], inp["gamma"], d_col[keep])["d_env"]
+    # ... and the library's over exactly those: zero the cotangent of the others
+    d_col2 = d_col.copy(); d_col2[~keep] = 0.0
+    rga.shade_backward(av.h, torch.as_tensor(env).to(dev), inp["cam_pos"], torch.as_tensor(d_col2).to(dev),
+                       texel_to_dir=torch.as_tensor(inp["texel_to_dir"]).to(dev), gamma=inp["gamma"], use_visibility=use_vis, out_denv=outs["out_denv"])
+    ge = outs["out_denv"].cpu().numpy()
+    scale = np.abs(ref_env).max()
+    rep["d_env"] = (float(np.abs(ge - ref_env).max() / scale), float(np.abs(ge - ref_env).mean() / scale), float(scale))
+    print(rep)
+    for k, (emax, emean, scale) in rep.items():
+        assert scale > 0, k
+        assert emax < SH_TOL_MAX and emean < SH_TOL_MEAN, (k, emax, emean, scale)
+    av.close()
