@@ -78,6 +78,7 @@ struct rga_avatar {
   int* stop_seg;               // [pixels] segment in which the pixel's blend stops (-1: list exhausted)
   unsigned char* item_flag;    // [items_cap] work item has pixels to replay (cleared by the replay kernel)
   float* t_final; unsigned* n_contrib;
+  int* work_counter;           // [1] dynamic work distribution of persistent kernels (zeroed before the launch)
   float* splat_grad;           // [n_gauss][12] splat_backward: d_colour(3), d_opacity, d_mu(2), d_conic(3), pad
   int* status;                 // sticky device status
   int sorted_buf;              // which of keys[]/vals[] holds the sorted result

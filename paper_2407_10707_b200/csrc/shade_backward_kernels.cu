@@ -28,7 +28,7 @@ __global__ void __launch_bounds__(SB_THREADS) shade_backward_kernel(int ng, int 
     const unsigned char* __restrict__ vcount, const int* __restrict__ knn_g, const float* __restrict__ ubar_g,
     float3 cam, float inv_gamma, const float4* __restrict__ radiance, const float* __restrict__ dL_dcolor,
     float* __restrict__ out_dalbedo, float* __restrict__ out_drough, float* __restrict__ out_dspec, float* __restrict__ out_dnormal,
-    float* __restrict__ out_dpos, float* __restrict__ out_denv) {
+    float* __restrict__ out_dpos, float* __restrict__ out_denv, int* __restrict__ work) {
   extern __shared__ __align__(16) float smem[];
   float4* sE = reinterpret_cast<float4*>(smem);                          // [ne][2]: (w, A), (L A, 0)
   float* sG = reinterpret_cast<float*>(sE + 2 * ne);                     // [ne][3] environment gradient of this CTA
@@ -40,7 +40,14 @@ __global__ void __launch_bounds__(SB_THREADS) shade_backward_kernel(int ng, int 
   const int GPB = SB_THREADS / SB_LANES;
   const int lane = threadIdx.x % SB_LANES;
   const float ip = 1.f / PI_F;
-  for (int gbase = blockIdx.x * GPB; gbase < ng; gbase += gridDim.x * GPB) {
+  __shared__ int s_base;
+  for (;;) {
+    // groups of GPB Gaussians are handed out dynamically: their cost varies with the share that faces the camera
+    __syncthreads();
+    if (threadIdx.x == 0) s_base = atomicAdd(work, GPB);
+    __syncthreads();
+    const int gbase = s_base;
+    if (gbase >= ng) break;
     const int g = gbase + threadIdx.x / SB_LANES;
     bool active = g < ng;
     float4 x = make_float4(0.f, 0.f, 0.f, 0.f), n = x, ar = x;
@@ -196,11 +203,12 @@ cudaError_t rga_launch_shade_backward(rga_avatar* av, const rga_env* env, float3
   const float ig = 1.0f / env->gamma;
   cudaError_t e = cudaSuccess;
   if (out_denv && (e = cudaMemsetAsync(out_denv, 0, sizeof(float) * 3 * (size_t)ne, s)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(av->work_counter, 0, sizeof(int), s)) != cudaSuccess) return e;
   const int gpb = SB_THREADS / SB_LANES;
   const int grid = min((av->n_gauss + gpb - 1) / gpb, av->num_sms * 8);
 #define SB_ARGS av->n_gauss, ne, av->vis_dirs, av->vis_words, av->k_g, av->k_v, av->g_posed, av->g_nposed, av->g_static, av->env_table, \
     env->texel_to_dir, av->visbits, av->vcount, av->knn_g, av->ubar_g, cam, ig, av->radiance, dL_dcolor, out_dalbedo, out_drough, out_dspec, \
-    out_dnormal, out_dpos, out_denv
+    out_dnormal, out_dpos, out_denv, av->work_counter
   if (vis_mode == 0) shade_backward_kernel<0><<<grid, SB_THREADS, smem, s>>>(SB_ARGS);
   else if (vis_mode == 1) shade_backward_kernel<1><<<grid, SB_THREADS, smem, s>>>(SB_ARGS);
   else shade_backward_kernel<2><<<grid, SB_THREADS, smem, s>>>(SB_ARGS);
