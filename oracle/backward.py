@@ -194,3 +194,35 @@ def shade_backward(xg, ng, alb, rough, spec, cam_pos, env, v, gamma, d_col, bloc
             out[name][sl] = leaf.grad.numpy()
     out["d_env"] = (np.zeros((rows * cols, 3)) if envt.grad is None else envt.grad.numpy()).reshape(rows, cols, 3)
     return out
+
+
+# ------------------------------------------------------------------------------------------------ losses, Eq.5-9
+def ssim_window(size=11, sigma=1.5):
+    """The SSIM window of 3DGS [8] (the paper applies "the same image loss as 3DGS"): normalised 1-D
+    Gaussian, outer product with itself."""
+    g = np.exp(-((np.arange(size) - size // 2) ** 2) / (2.0 * sigma * sigma))
+    return g / g.sum()
+
+
+def image_loss(image, target, lam=0.2):
+    """Eq.5: L_img = (1 - lambda) L_1 + lambda L_D-SSIM, lambda = 0.2, and dL_img/d(image) by autograd.
+    Reading A34: L_1 = mean |I - I^|; L_D-SSIM = 1 - SSIM(I, I^) as in 3DGS: per channel, 11x11 Gaussian window
+    (sigma 1.5), zero padding, mu = w * I, sigma^2 = w * I^2 - mu^2, sigma_12 = w * (I I^) - mu mu^, C1 = 0.01^2,
+    C2 = 0.03^2, SSIM = mean over pixels and channels of (2 mu mu^ + C1)(2 sigma_12 + C2) / ((mu^2 + mu^^2 + C1)(sigma^2 + sigma^^2 + C2)).
+    image, target [H,W,3].  Returns dict loss, l1, ssim (floats) and d_image [H,W,3] (fp64)."""
+    import torch.nn.functional as Fn
+    I = _t(image).permute(2, 0, 1)[None].clone().requires_grad_(True)        # [1,3,H,W]
+    J = _t(target).permute(2, 0, 1)[None]
+    w1 = _t(ssim_window())
+    w = (w1[:, None] * w1[None, :])[None, None].expand(3, 1, 11, 11).contiguous()
+    conv = lambda x: Fn.conv2d(x, w, padding=5, groups=3)
+    mu1, mu2 = conv(I), conv(J)
+    s1 = conv(I * I) - mu1 * mu1; s2 = conv(J * J) - mu2 * mu2; s12 = conv(I * J) - mu1 * mu2
+    C1, C2 = 0.01 ** 2, 0.03 ** 2
+    ssim_map = ((2 * mu1 * mu2 + C1) * (2 * s12 + C2)) / ((mu1 * mu1 + mu2 * mu2 + C1) * (s1 + s2 + C2))
+    ssim = ssim_map.mean()
+    l1 = (I - J).abs().mean()
+    loss = (1.0 - lam) * l1 + lam * (1.0 - ssim)
+    loss.backward()
+    return {"loss": float(loss), "l1": float(l1), "ssim": float(ssim), "d_image": I.grad[0].permute(1, 2, 0).numpy().copy(),
+            "ssim_map": ssim_map.detach()[0].permute(1, 2, 0).numpy().copy()}

@@ -278,3 +278,42 @@ def test_shade_backward_gradcheck():
     v = torch.tensor(rs.uniform(0.2, 1.0, (m, rows * cols)) * (rs.uniform(size=(m, rows * cols)) > 0.3))
     f = lambda x, n, a, r, s, e: bwd.shade_torch(x, n, a, r, s, cam, e, torch.tensor(Wn), torch.tensor(An), v, 2.2)[1]
     assert torch.autograd.gradcheck(f, args + (env,), eps=1e-7, atol=1e-6, rtol=1e-4)
+
+
+# ------------------------------------------------------------------------------------------------ Eq.5 image loss
+def test_image_loss_closed_forms_and_bruteforce():
+    rs = np.random.default_rng(6)
+    H, W = 24, 20
+    I = rs.uniform(0, 1, (H, W, 3)); J = np.clip(I + rs.normal(0, 0.1, (H, W, 3)), 0, 1)
+    w = bwd.ssim_window()
+    assert abs(w.sum() - 1.0) < 1e-15 and np.allclose(w, w[::-1]) and w.argmax() == 5
+    # identical images: SSIM = 1 everywhere, loss 0, gradient 0 (SSIM is at its maximum, |.| at its kink with subgradient 0)
+    r = bwd.image_loss(I, I)
+    assert abs(r["ssim"] - 1.0) < 1e-12 and abs(r["loss"]) < 1e-12 and np.abs(r["d_image"]).max() < 1e-9
+    # constant images a, b: interior pixels have mu = a, mu^ = b, all variances 0 -> SSIM = (2ab + C1) / (a^2 + b^2 + C1)
+    a, b = 0.7, 0.4
+    r = bwd.image_loss(np.full((H, W, 3), a), np.full((H, W, 3), b))
+    assert np.allclose(r["ssim_map"][5:-5, 5:-5], (2 * a * b + 1e-4) / (a * a + b * b + 1e-4), atol=1e-12)
+    assert abs(r["l1"] - (a - b)) < 1e-15
+    # brute force at a few pixels (also on the border: zero padding), written with explicit window sums
+    r = bwd.image_loss(I, J, lam=0.2)
+    for (y, x, c) in [(0, 0, 0), (3, 17, 1), (12, 10, 2), (23, 19, 0), (23, 0, 1)]:
+        acc = np.zeros(5)
+        for dy in range(-5, 6):
+            for dx in range(-5, 6):
+                yy, xx = y + dy, x + dx
+                if 0 <= yy < H and 0 <= xx < W:
+                    p, q = I[yy, xx, c], J[yy, xx, c]
+                    acc += w[dy + 5] * w[dx + 5] * np.array([p, q, p * p, q * q, p * q])
+        m1, m2 = acc[0], acc[1]; s1, s2, s12 = acc[2] - m1 * m1, acc[3] - m2 * m2, acc[4] - m1 * m2
+        ref = ((2 * m1 * m2 + 1e-4) * (2 * s12 + 9e-4)) / ((m1 * m1 + m2 * m2 + 1e-4) * (s1 + s2 + 9e-4))
+        assert abs(r["ssim_map"][y, x, c] - ref) < 1e-12
+    assert abs(r["loss"] - (0.8 * np.abs(I - J).mean() + 0.2 * (1 - r["ssim_map"].mean()))) < 1e-14
+    # gradient: central differences of the loss itself at a few pixels
+    for (y, x, c) in [(0, 0, 0), (7, 9, 1), (23, 19, 2)]:
+        Ip, Im = I.copy(), I.copy(); Ip[y, x, c] += 1e-6; Im[y, x, c] -= 1e-6
+        fd = (bwd.image_loss(Ip, J)["loss"] - bwd.image_loss(Im, J)["loss"]) / 2e-6
+        assert abs(fd - r["d_image"][y, x, c]) < 1e-8
+    # lambda = 0: pure L1, gradient sign(I - I^) / (3 H W)
+    r0 = bwd.image_loss(I, J, lam=0.0)
+    assert np.allclose(r0["d_image"], np.sign(I - J) / I.size)
