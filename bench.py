@@ -279,6 +279,15 @@ def main():
     sb_obj = {"ms": ms_sb, "gaussians_with_gradient": n_grad, "texels": ne_all,
               "note": "albedo, roughness, specular, normal, position and environment-map gradients; env table rebuilt inside the call"}
 
+    # ... and Eq.5, the image loss that produces dL/dimage (target: a seeded stand-in image of the same size)
+    _, tgt_np = workloads.make_image_pair(1, camc.width, camc.height)
+    tgt_d = torch.as_tensor(tgt_np).to(dev); loss_d = torch.zeros(3, device=dev)
+    run_il = lambda: rga.image_loss(av.h, img, tgt_d, 0.2, loss_d, dLdI)
+    for _ in range(3):
+        run_il()
+    ms_il = timed(run_il, 20)
+    il_obj = {"ms": ms_il, "pixels": int(camc.width * camc.height), "lambda": 0.2}
+
     # algorithmic units of each candidate dominant kernel: counted from the frame that was rendered
     gp = av.read("GAUSS_POSED").reshape(-1, 4)[:, :3]; gn = av.read("GAUSS_NORMAL_POSED").reshape(-1, 4)[:, :3]
     front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
@@ -349,7 +358,7 @@ def main():
                 "pipelined_value": world * 1e3 / ms_e2e_pipe,
                 "pipelined_note": "image read-back of step i on a copy stream beside step i+1; per-step events plus the last copy's tail"},
         "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
-        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj, "shade_backward": sb_obj,
+        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj, "shade_backward": sb_obj, "image_loss": il_obj,
         "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

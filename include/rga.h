@@ -159,6 +159,15 @@ RGA_API rga_status shade_backward(rga_avatar* av, const rga_env* env, const floa
                                   float* out_dalbedo, float* out_drough, float* out_dspec, float* out_dnormal, float* out_dpos,
                                   float* out_denv, void* stream);
 
+/* Eq.5: L_img = (1 - lambda) L_1 + lambda L_D-SSIM between a rendered image and its target, both DEVICE
+ * [height][width][3] fp32, width <= max_width and height <= max_height of the avatar (whose scratch it uses), with the
+ * gradient dL_img/d(image) -- the dL_dimage of splat_backward.  L_1 = mean |I - I^|; L_D-SSIM = 1 - SSIM with the 11x11
+ * Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2, C2 = 0.03^2, averaged over pixels and channels, as in 3DGS
+ * (reading A34); the paper's lambda is 0.2.  out_loss: dev f32 [3] = {L_img, L_1, SSIM} or NULL;
+ * out_dL_dimage: dev [height][width][3] or NULL.  Enqueue-only. */
+RGA_API rga_status image_loss(rga_avatar* av, const float* image, const float* target, int width, int height, float lambda,
+                              float* out_loss, float* out_dL_dimage, void* stream);
+
 /* Algorithm 1, "Gaussian densification based on density": from the avatar's current
  * S_g (avatar_load / gaussians_update) and its mesh, counts the Gaussians near every vertex (D_v), estimates the Gaussian
  * density of every triangle d_f = sum of its three D_v / (6 K_g), sets P = max(0, d0 - d_f), asks for

@@ -224,5 +224,5 @@ def image_loss(image, target, lam=0.2):
     l1 = (I - J).abs().mean()
     loss = (1.0 - lam) * l1 + lam * (1.0 - ssim)
     loss.backward()
-    return {"loss": float(loss), "l1": float(l1), "ssim": float(ssim), "d_image": I.grad[0].permute(1, 2, 0).numpy().copy(),
+    return {"loss": float(loss.detach()), "l1": float(l1.detach()), "ssim": float(ssim.detach()), "d_image": I.grad[0].permute(1, 2, 0).numpy().copy(),
             "ssim_map": ssim_map.detach()[0].permute(1, 2, 0).numpy().copy()}

@@ -199,6 +199,13 @@ def splat_backward(h, camera, bg, image, dL_dimage, out_dcolor=None, out_dopacit
                               _stream()))
 
 
+def image_loss(h, image, target, lam=0.2, out_loss=None, out_dL_dimage=None):
+    """Eq.5 image loss and its gradient (include/rga.h image_loss).  image, target: CUDA float32 [H, W, 3]."""
+    lib().image_loss.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
+    _chk(lib().image_loss(h, _ptr(image), _ptr(target), int(image.shape[1]), int(image.shape[0]), float(lam), _ptr(out_loss),
+                          _ptr(out_dL_dimage), _stream()))
+
+
 def densify_density(h, d0, p0, rnd, out_pos, out_tri=None, out_count=None):
     """Algorithm 1, density-based densification (include/rga.h densify_density).  rnd: CUDA int32/uint32 tensor [3 * max_out]
     of raw 32-bit random numbers; out_pos: CUDA float32 [max_out, 3]; out_tri / out_count: CUDA int32 [max_out] / [1] or None."""

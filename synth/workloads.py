@@ -231,3 +231,19 @@ def make_image_cotangent(seed, width, height):
 def make_color_cotangent(seed, n_gauss):
     """dL/dcolour per Gaussian for the backward of the shading step: seeded standard normal [n_gauss, 3] (fp32)."""
     return np.random.default_rng(2000 + seed).normal(size=(n_gauss, 3)).astype(np.float32)
+
+
+def make_image_pair(seed, width, height):
+    """(rendered, target) stand-ins for the image loss: a smooth seeded random field in [0,1] (sum of a few low-frequency
+    cosines per channel) as target, and the same plus small-scale noise, clipped, as the rendered image.  fp32 [H,W,3]."""
+    rs = np.random.default_rng(3000 + seed)
+    y, x = np.meshgrid(np.arange(height) / max(height, 1), np.arange(width) / max(width, 1), indexing="ij")
+    tgt = np.zeros((height, width, 3))
+    for c in range(3):
+        for _ in range(6):
+            fx, fy, ph = rs.uniform(0.5, 6.0), rs.uniform(0.5, 6.0), rs.uniform(0, 2 * np.pi)
+            tgt[:, :, c] += rs.uniform(0.05, 0.2) * np.cos(2 * np.pi * (fx * x + fy * y) + ph)
+    tgt = np.clip(0.5 + tgt, 0.0, 1.0)
+    img = np.clip(tgt + rs.normal(0.0, 0.05, tgt.shape), 0.0, 1.0)
+    img[: height // 4, : width // 4] = 0.0                                # a black corner: zero-variance windows on one side
+    return img.astype(np.float32), tgt.astype(np.float32)

@@ -128,3 +128,27 @@ def test_shade_backward_matches_autograd_oracle(cfg, vis_mode, use_vis):
         assert scale > 0, k
         assert emax < SH_TOL_MAX and emean < SH_TOL_MEAN, (k, emax, emean, scale)
     av.close()
+
+
+@pytest.mark.parametrize("W,H,lam", [(64, 64, 0.2), (70, 45, 0.2), (512, 512, 0.2), (512, 512, 0.0), (33, 17, 1.0)])
+def test_image_loss_matches_oracle(W, H, lam):
+    # Eq.5: loss value and dL/dimage; fp32 window sums of 121 taps against fp64 -> 1e-5 relative on the loss, 2e-4 of the
+    # largest gradient entry (sigma^2 = w*I^2 - mu^2 cancels in fp32 where the window is flat)
+    import torch
+    from oracle import backward as bwd
+    from paper_2407_10707_b200 import binding as rga
+    inp = workloads.make(0)
+    av = rga.Avatar(inp, max_width=512, max_height=512, max_vis_dirs=16, max_vis_res=32, max_env_texels=512)
+    img, tgt = workloads.make_image_pair(W + H, W, H)
+    ref = bwd.image_loss(img, tgt, lam)
+    out = torch.full((3,), float("nan"), device="cuda"); dI = torch.full((H, W, 3), float("nan"), device="cuda")
+    rga.image_loss(av.h, torch.as_tensor(img).cuda(), torch.as_tensor(tgt).cuda(), lam, out, dI)
+    rga.rga_check(av.h)
+    got = out.cpu().numpy(); g = dI.cpu().numpy()
+    assert abs(got[0] - ref["loss"]) < 1e-5 * max(ref["loss"], 1e-3), (got, ref["loss"])
+    assert abs(got[1] - ref["l1"]) < 1e-6 and abs(got[2] - ref["ssim"]) < 2e-5
+    scale = np.abs(ref["d_image"]).max()
+    err = np.abs(g - ref["d_image"])
+    print(W, H, lam, "loss", got, "grad err max/mean rel", err.max() / scale, err.mean() / scale)
+    assert np.isfinite(g).all() and err.max() < 2e-4 * scale and err.mean() < 1e-5 * scale
+    av.close()
