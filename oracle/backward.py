@@ -226,3 +226,28 @@ def image_loss(image, target, lam=0.2):
     loss.backward()
     return {"loss": float(loss.detach()), "l1": float(l1.detach()), "ssim": float(ssim.detach()), "d_image": I.grad[0].permute(1, 2, 0).numpy().copy(),
             "ssim_map": ssim_map.detach()[0].permute(1, 2, 0).numpy().copy()}
+
+
+def regularisers(vert_albedo, vert_rough, vert_spec, knn_v, gauss_pos, vert_pos, knn_g, vert_disp, gauss_scale, s0=0.005):
+    """Eq.6-9, each written as its sum, with gradients by autograd (fp64):
+    Eq.6 L_smooth = sum_i sum_{k in S_v^i} ||*^i - *^k||_1 over the material attributes * in {a, gamma, p};
+    Eq.7 L_mdist  = sum_i sum_{k in S_g^i} ||x_g^i - x^k||_2;   Eq.8 L_disp = sum_i ||dx^i||_2;
+    Eq.9 L_scale  = sum_i max(0, s_g^i - s_0) summed over the three scale components, s_0 = 0.005.
+    Reading A35: the 1-norm's slope at 0 and the 2-norm's slope at the origin are taken as 0; max(0, .) has slope 0 at 0.
+    Returns dict of the four losses and d_albedo [N_v,3], d_rough [N_v], d_spec [N_v], d_gauss_pos [N_g,3], d_disp [N_v,3],
+    d_scale [N_g,3]."""
+    a = _t(vert_albedo).requires_grad_(True); r = _t(vert_rough).requires_grad_(True); p = _t(vert_spec).requires_grad_(True)
+    xg = _t(gauss_pos).requires_grad_(True); dx = _t(vert_disp).requires_grad_(True); s = _t(gauss_scale).requires_grad_(True)
+    xv = _t(vert_pos)
+    kv = torch.as_tensor(np.asarray(knn_v).astype(np.int64)); kg = torch.as_tensor(np.asarray(knn_g).astype(np.int64))
+    smooth = (a[:, None, :] - a[kv]).abs().sum() + (r[:, None] - r[kv]).abs().sum() + (p[:, None] - p[kv]).abs().sum()
+    d = xg[:, None, :] - xv[kg]
+    n2 = (d * d).sum(2)
+    mdist = torch.where(n2 > 0, torch.where(n2 > 0, n2, torch.ones_like(n2)).sqrt(), torch.zeros_like(n2)).sum()
+    m2 = (dx * dx).sum(1)
+    disp = torch.where(m2 > 0, torch.where(m2 > 0, m2, torch.ones_like(m2)).sqrt(), torch.zeros_like(m2)).sum()
+    scale = torch.where(s > s0, s - s0, torch.zeros_like(s)).sum()      # slope 0 at s = s_0 (torch.clamp would pass 1 there)
+    (smooth + mdist + disp + scale).backward()                           # the four terms share no parameter
+    return {"smooth": float(smooth.detach()), "mdist": float(mdist.detach()), "disp": float(disp.detach()), "scale": float(scale.detach()),
+            "d_albedo": a.grad.numpy(), "d_rough": r.grad.numpy(), "d_spec": p.grad.numpy(), "d_gauss_pos": xg.grad.numpy(),
+            "d_disp": dx.grad.numpy(), "d_scale": s.grad.numpy()}

@@ -317,3 +317,38 @@ def test_image_loss_closed_forms_and_bruteforce():
     # lambda = 0: pure L1, gradient sign(I - I^) / (3 H W)
     r0 = bwd.image_loss(I, J, lam=0.0)
     assert np.allclose(r0["d_image"], np.sign(I - J) / I.size)
+
+
+# ------------------------------------------------------------------------------------------------ Eq.6-9 regularisers
+def test_regularisers_hand_example_and_finite_differences():
+    # three vertices on a line, K_v = 2 neighbour sets written by hand; two Gaussians with K_g = 2
+    alb = np.array([[0.1, 0.2, 0.3], [0.4, 0.2, 0.1], [0.9, 0.8, 0.7]]); rough = np.array([0.2, 0.5, 0.9]); spec = np.array([0.3, 0.3, 0.6])
+    knn_v = np.array([[0, 1], [1, 0], [2, 1]])
+    xv = np.array([[0.0, 0, 0], [1.0, 0, 0], [2.0, 0, 0]]); xg = np.array([[0.0, 3.0, 4.0], [1.0, 0.0, 0.0]]); knn_g = np.array([[0, 1], [1, 2]])
+    disp = np.array([[0.0, 0.0, 0.0], [0.003, 0.004, 0.0], [0.0, 0.0, -0.01]])
+    scale = np.array([[0.004, 0.005, 0.006], [0.02, 0.001, 0.0051]])
+    r = bwd.regularisers(alb, rough, spec, knn_v, xg, xv, knn_g, disp, scale)
+    # Eq.6 by hand: pairs (0,1), (1,0), (2,1) (self pairs give 0): albedo 0.5 + 0.5 + 1.7, roughness 0.3 + 0.3 + 0.4, specular 0 + 0 + 0.3
+    assert np.isclose(r["smooth"], 2.7 + 1.0 + 0.3)
+    assert np.allclose(r["d_rough"], [-2.0, 2.0 - 1.0, 1.0])             # vertex 1 appears as i once (+1) ... and as k twice
+    assert np.allclose(r["d_spec"], [0.0, -1.0, 1.0])                    # equal values: slope 0 (reading A35)
+    # Eq.7: |(0,3,4)| + |(-1,3,4)| + 0 + |(-1,0,0)| = 5 + sqrt(26) + 0 + 1
+    assert np.isclose(r["mdist"], 5.0 + np.sqrt(26.0) + 1.0)
+    assert np.allclose(r["d_gauss_pos"][0], np.array([0, 3, 4]) / 5.0 + np.array([-1, 3, 4]) / np.sqrt(26.0))
+    assert np.allclose(r["d_gauss_pos"][1], [-1.0, 0.0, 0.0])            # the coincident vertex contributes no slope
+    # Eq.8: 0 + 0.005 + 0.01;  Eq.9 with s0 = 0.005: 0.001 + 0.015 + 0.0001
+    assert np.isclose(r["disp"], 0.015) and np.allclose(r["d_disp"], [[0, 0, 0], [0.6, 0.8, 0], [0, 0, -1.0]])
+    assert np.isclose(r["scale"], 0.0161) and np.array_equal(r["d_scale"], [[0, 0, 1.0], [1.0, 0, 1.0]])
+    # central differences on a seeded case without ties
+    rs = np.random.default_rng(8)
+    nv, ng = 30, 40
+    args = [rs.uniform(0, 1, (nv, 3)), rs.uniform(0, 1, nv), rs.uniform(0, 1, nv), rs.integers(0, nv, (nv, 5)), rs.normal(size=(ng, 3)),
+            rs.normal(size=(nv, 3)), rs.integers(0, nv, (ng, 3)), rs.normal(size=(nv, 3)) * 0.01, rs.uniform(0.001, 0.01, (ng, 3))]
+    r = bwd.regularisers(*args)
+    tot = lambda q: sum(q[k] for k in ("smooth", "mdist", "disp", "scale"))
+    for ai, key in ((0, "d_albedo"), (1, "d_rough"), (2, "d_spec"), (4, "d_gauss_pos"), (7, "d_disp"), (8, "d_scale")):
+        idx = tuple(rs.integers(0, s) for s in args[ai].shape)
+        ap = [x.copy() if isinstance(x, np.ndarray) else x for x in args]; am = [x.copy() if isinstance(x, np.ndarray) else x for x in args]
+        ap[ai][idx] += 1e-7; am[ai][idx] -= 1e-7
+        fd = (tot(bwd.regularisers(*ap)) - tot(bwd.regularisers(*am))) / 2e-7
+        assert abs(fd - r[key][idx]) < 1e-5 * (1 + abs(fd)), key
