@@ -168,6 +168,19 @@ RGA_API rga_status shade_backward(rga_avatar* av, const rga_env* env, const floa
 RGA_API rga_status image_loss(rga_avatar* av, const float* image, const float* target, int width, int height, float lambda,
                               float* out_loss, float* out_dL_dimage, void* stream);
 
+/* Regularisers of the training objective Eq.10, evaluated on the avatar's own tables, each as the plain
+ * sum the paper writes (the lambdas of Eq.10 are the caller's), with gradients:
+ *   Eq.6 L_smooth = sum_i sum_{k in S_v^i} ||*^i - *^k||_1 over the vertex attributes * in {albedo, roughness, specular};
+ *   Eq.7 L_mdist  = sum_i sum_{k in S_g^i} ||x_g^i - x^k||_2  (canonical Gaussian positions vs their K_g vertices);
+ *   Eq.8 L_disp   = sum_i ||dx^i||_2  (the current per-vertex displacement: displacement_mlp's if it ran, else the static one);
+ *   Eq.9 L_scale  = sum_i max(0, s_g^i - s0) over the three scale components; the paper's s0 is 0.005.
+ * Slopes at the kinks (equal attributes, zero distance or displacement, s = s0) are 0 (reading A35).
+ * out_losses: dev f32 [4] = {L_smooth, L_mdist, L_disp, L_scale} or NULL.  Gradient outputs, DEVICE, each may be NULL:
+ * out_dalbedo [n_verts][3], out_drough [n_verts], out_dspec [n_verts] (Eq.6); out_dgauss_pos [n_gauss][3] (Eq.7);
+ * out_ddisp [n_verts][3] (Eq.8); out_dscale [n_gauss][3] (Eq.9).  Enqueue-only. */
+RGA_API rga_status regularisers(rga_avatar* av, float s0, float* out_losses, float* out_dalbedo, float* out_drough, float* out_dspec,
+                                float* out_dgauss_pos, float* out_ddisp, float* out_dscale, void* stream);
+
 /* Algorithm 1, "Gaussian densification based on density": from the avatar's current
  * S_g (avatar_load / gaussians_update) and its mesh, counts the Gaussians near every vertex (D_v), estimates the Gaussian
  * density of every triangle d_f = sum of its three D_v / (6 K_g), sets P = max(0, d0 - d_f), asks for

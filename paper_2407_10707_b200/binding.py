@@ -206,6 +206,14 @@ def image_loss(h, image, target, lam=0.2, out_loss=None, out_dL_dimage=None):
                           _ptr(out_dL_dimage), _stream()))
 
 
+def regularisers(h, s0=0.005, out_losses=None, out_dalbedo=None, out_drough=None, out_dspec=None, out_dgauss_pos=None, out_ddisp=None,
+                 out_dscale=None):
+    """Eq.6-9 and their gradients on the avatar's own tables (include/rga.h regularisers)."""
+    lib().regularisers.argtypes = [C.c_void_p, C.c_float] + [C.c_void_p] * 8
+    _chk(lib().regularisers(h, float(s0), _ptr(out_losses), _ptr(out_dalbedo), _ptr(out_drough), _ptr(out_dspec), _ptr(out_dgauss_pos),
+                            _ptr(out_ddisp), _ptr(out_dscale), _stream()))
+
+
 def densify_density(h, d0, p0, rnd, out_pos, out_tri=None, out_count=None):
     """Algorithm 1, density-based densification (include/rga.h densify_density).  rnd: CUDA int32/uint32 tensor [3 * max_out]
     of raw 32-bit random numbers; out_pos: CUDA float32 [max_out, 3]; out_tri / out_count: CUDA int32 [max_out] / [1] or None."""

@@ -158,3 +158,93 @@ cudaError_t rga_launch_image_loss(rga_avatar* av, const float* image, const floa
   av->launches += 1 + (out_dimage != nullptr) + (out_loss != nullptr);
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Regularisers Eq.6-9, reading A35 (slope 0 at the kinks).  One thread per vertex does Eq.6
+// (its own K_v neighbour set: the gradient of its own attributes stays in registers, the opposite sign goes to the
+// neighbour by an atomic; sums of +-1 are exact in fp32, so the result does not depend on the order) and Eq.8; one thread
+// per Gaussian does Eq.7 and Eq.9.  Loss sums: block reduction, then one double atomic per CTA.
+__device__ __forceinline__ float sgnf(float d) { return d > 0.f ? 1.f : (d < 0.f ? -1.f : 0.f); }
+
+__global__ void __launch_bounds__(256) reg_vertex_kernel(int nv, int Kv, const float* __restrict__ alb, const float* __restrict__ rough,
+    const float* __restrict__ spec, const int* __restrict__ knn_v, const float4* __restrict__ disp4, const float* __restrict__ disp3,
+    float* __restrict__ d_alb, float* __restrict__ d_rough, float* __restrict__ d_spec, float* __restrict__ d_disp, double* __restrict__ sums) {
+  __shared__ float s_red[8];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  float smooth = 0.f, dl = 0.f;
+  if (i < nv) {
+    const float a0 = alb[3 * i], a1 = alb[3 * i + 1], a2 = alb[3 * i + 2], r = rough[i], p = spec[i];
+    float g0 = 0.f, g1 = 0.f, g2 = 0.f, gr = 0.f, gp = 0.f;
+    for (int j = 0; j < Kv; ++j) {
+      const int k = knn_v[(size_t)i * Kv + j];
+      if (k == i) continue;
+      const float e0 = a0 - alb[3 * k], e1 = a1 - alb[3 * k + 1], e2 = a2 - alb[3 * k + 2], er = r - rough[k], ep = p - spec[k];
+      smooth += fabsf(e0) + fabsf(e1) + fabsf(e2) + fabsf(er) + fabsf(ep);
+      const float s0 = sgnf(e0), s1 = sgnf(e1), s2 = sgnf(e2), sr = sgnf(er), sp = sgnf(ep);
+      g0 += s0; g1 += s1; g2 += s2; gr += sr; gp += sp;
+      if (d_alb) { if (s0 != 0.f) atomicAdd(d_alb + 3 * k, -s0); if (s1 != 0.f) atomicAdd(d_alb + 3 * k + 1, -s1); if (s2 != 0.f) atomicAdd(d_alb + 3 * k + 2, -s2); }
+      if (d_rough && sr != 0.f) atomicAdd(d_rough + k, -sr);
+      if (d_spec && sp != 0.f) atomicAdd(d_spec + k, -sp);
+    }
+    if (d_alb) { atomicAdd(d_alb + 3 * i, g0); atomicAdd(d_alb + 3 * i + 1, g1); atomicAdd(d_alb + 3 * i + 2, g2); }
+    if (d_rough) atomicAdd(d_rough + i, gr);
+    if (d_spec) atomicAdd(d_spec + i, gp);
+    float x = 0.f, y = 0.f, z = 0.f;
+    if (disp4) { const float4 d = disp4[i]; x = d.x; y = d.y; z = d.z; }
+    else if (disp3) { x = disp3[3 * i]; y = disp3[3 * i + 1]; z = disp3[3 * i + 2]; }
+    const float n2 = x * x + y * y + z * z;
+    float inv = 0.f;
+    if (n2 > 0.f) { dl = sqrtf(n2); inv = 1.f / dl; }
+    if (d_disp) { d_disp[3 * i] = x * inv; d_disp[3 * i + 1] = y * inv; d_disp[3 * i + 2] = z * inv; }
+  }
+  const float t0 = block_sum256(smooth, s_red), t1 = block_sum256(dl, s_red);
+  if (threadIdx.x == 0) { atomicAdd(sums, (double)t0); atomicAdd(sums + 2, (double)t1); }
+}
+
+__global__ void __launch_bounds__(256) reg_gauss_kernel(int ng, int Kg, float s0, const float4* __restrict__ g_pos, const float* __restrict__ v_pos,
+    const int* __restrict__ knn_g, const float4* __restrict__ g_scale_op, float* __restrict__ d_gpos, float* __restrict__ d_scale,
+    double* __restrict__ sums) {
+  __shared__ float s_red[8];
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  float md = 0.f, sc = 0.f;
+  if (g < ng) {
+    const float4 x = g_pos[g];
+    float gx = 0.f, gy = 0.f, gz = 0.f;
+    for (int j = 0; j < Kg; ++j) {
+      const int k = knn_g[(size_t)g * Kg + j];
+      const float dx = x.x - v_pos[3 * k], dy = x.y - v_pos[3 * k + 1], dz = x.z - v_pos[3 * k + 2];
+      const float n2 = dx * dx + dy * dy + dz * dz;
+      if (n2 > 0.f) { const float l = sqrtf(n2), inv = 1.f / l; md += l; gx += dx * inv; gy += dy * inv; gz += dz * inv; }
+    }
+    if (d_gpos) { d_gpos[3 * g] = gx; d_gpos[3 * g + 1] = gy; d_gpos[3 * g + 2] = gz; }
+    const float4 s = g_scale_op[g];
+    const float e0 = s.x - s0, e1 = s.y - s0, e2 = s.z - s0;
+    sc = fmaxf(e0, 0.f) + fmaxf(e1, 0.f) + fmaxf(e2, 0.f);
+    if (d_scale) { d_scale[3 * g] = e0 > 0.f ? 1.f : 0.f; d_scale[3 * g + 1] = e1 > 0.f ? 1.f : 0.f; d_scale[3 * g + 2] = e2 > 0.f ? 1.f : 0.f; }
+  }
+  const float t0 = block_sum256(md, s_red), t1 = block_sum256(sc, s_red);
+  if (threadIdx.x == 0) { atomicAdd(sums + 1, (double)t0); atomicAdd(sums + 3, (double)t1); }
+}
+
+__global__ void reg_finish_kernel(const double* __restrict__ sums, float* __restrict__ out) {
+  if (threadIdx.x < 4) out[threadIdx.x] = (float)sums[threadIdx.x];
+}
+
+cudaError_t rga_launch_regularisers(rga_avatar* av, float s0, float* out_losses, float* d_alb, float* d_rough, float* d_spec, float* d_gpos,
+                                    float* d_disp, float* d_scale, cudaStream_t s) {
+  cudaError_t e = cudaMemsetAsync(av->reg_sums, 0, 4 * sizeof(double), s);
+  if (e != cudaSuccess) return e;
+  const size_t nv = av->n_verts;
+  if (d_alb && (e = cudaMemsetAsync(d_alb, 0, 12 * nv, s)) != cudaSuccess) return e;
+  if (d_rough && (e = cudaMemsetAsync(d_rough, 0, 4 * nv, s)) != cudaSuccess) return e;
+  if (d_spec && (e = cudaMemsetAsync(d_spec, 0, 4 * nv, s)) != cudaSuccess) return e;
+  reg_vertex_kernel<<<(av->n_verts + 255) / 256, 256, 0, s>>>(av->n_verts, av->k_v, av->vt_albedo, av->vt_rough, av->vt_spec, av->knn_v,
+      av->disp_is_mlp ? av->v_disp : nullptr, av->disp_is_mlp ? nullptr : av->vt_disp, d_alb, d_rough, d_spec, d_disp, av->reg_sums);
+  rga_prof_mark(av, "reg_vertex", s);
+  reg_gauss_kernel<<<(av->n_gauss + 255) / 256, 256, 0, s>>>(av->n_gauss, av->k_g, s0, av->g_pos, av->vt_pos, av->knn_g, av->g_scale_op,
+      d_gpos, d_scale, av->reg_sums);
+  rga_prof_mark(av, "reg_gauss", s);
+  if (out_losses) reg_finish_kernel<<<1, 32, 0, s>>>(av->reg_sums, out_losses);
+  av->launches += 2 + (out_losses != nullptr);
+  return cudaGetLastError();
+}

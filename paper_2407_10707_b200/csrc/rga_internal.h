@@ -78,6 +78,8 @@ struct rga_avatar {
   int* stop_seg;               // [pixels] segment in which the pixel's blend stops (-1: list exhausted)
   unsigned char* item_flag;    // [items_cap] work item has pixels to replay (cleared by the replay kernel)
   float* t_final; unsigned* n_contrib;
+  double* reg_sums;            // [4] regularisers: sums of Eq.6, 7, 8, 9
+  int disp_is_mlp;             // the current displacement is displacement_mlp's v_disp (else the static vt_disp table)
   float* loss_maps; double* loss_sums;   // image_loss: [max_h][max_w][9] SSIM derivative maps, {sum SSIM, sum |I - J|}
   int* work_counter;           // [1] dynamic work distribution of persistent kernels (zeroed before the launch)
   float* splat_grad;           // [n_gauss][12] splat_backward: d_colour(3), d_opacity, d_mu(2), d_conic(3), pad
@@ -139,6 +141,8 @@ int rga_shade_backward_init_attributes(int max_env);
 // loss_kernels.cu
 cudaError_t rga_launch_image_loss(rga_avatar* av, const float* image, const float* target, int W, int H, float lam, float* out_loss,
                                   float* out_dimage, cudaStream_t s);
+cudaError_t rga_launch_regularisers(rga_avatar* av, float s0, float* out_losses, float* d_alb, float* d_rough, float* d_spec, float* d_gpos,
+                                    float* d_disp, float* d_scale, cudaStream_t s);
 // densify_kernels.cu
 cudaError_t rga_launch_densify(rga_avatar* av, float d0, float p0, const unsigned* rnd, int max_out, float* out_pos, int* out_tri,
                                int* out_count, cudaStream_t s);

@@ -152,3 +152,47 @@ def test_image_loss_matches_oracle(W, H, lam):
     print(W, H, lam, "loss", got, "grad err max/mean rel", err.max() / scale, err.mean() / scale)
     assert np.isfinite(g).all() and err.max() < 2e-4 * scale and err.mean() < 1e-5 * scale
     av.close()
+
+
+@pytest.mark.parametrize("cfg,with_mlp", [(0, False), (1, False), (1, True), (2, False)])
+def test_regularisers_match_oracle(cfg, with_mlp):
+    # Eq.6-9: losses to 1e-5 relative (fp32 terms, double sums); Eq.6 / Eq.9 gradients are sums of +-1 / 0-1 flags: exact;
+    # Eq.7 / Eq.8 gradients are sums of unit vectors: 1e-5 absolute
+    import torch
+    from oracle import backward as bwd
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    inp = workloads.make(cfg, n_gauss=50_000 if cfg == 2 else None)
+    if cfg == 0:                                                         # a static displacement attribute, a few exactly 0
+        inp["vert_disp"] = (np.random.default_rng(12).normal(0.0, 0.004, inp["vert_pos"].shape)).astype(np.float32)
+        inp["vert_disp"][::7] = 0.0
+    cam = inp["camera"]
+    av = rga.Avatar(inp, max_width=cam["width"], max_height=cam["height"], max_vis_dirs=16, max_vis_res=32, max_env_texels=512)
+    orc_av = orc.avatar_load(inp)
+    disp = inp["vert_disp"]
+    if with_mlp:
+        mlp = workloads.make_disp_mlp(seed=2)
+        rga.displacement_mlp(av.h, {k: (torch.as_tensor(v).cuda() if isinstance(v, np.ndarray) else v) for k, v in mlp.items()},
+                             torch.as_tensor(mlp["theta"]).cuda())
+        disp = orc.disp_mlp(inp["vert_pos"], mlp["theta"], mlp)          # fp64; the kernel's TF32 result is within 1e-2 of its scale
+    ref = bwd.regularisers(inp["vert_albedo"], inp["vert_rough"], inp["vert_spec"], orc_av["knn_v"], inp["gauss_pos"], inp["vert_pos"],
+                           orc_av["knn_g"], disp, inp["gauss_scale"])
+    nv, ng = len(inp["vert_pos"]), len(inp["gauss_pos"])
+    nanf = lambda *s: torch.full(s, float("nan"), device="cuda")
+    L = nanf(4); o = dict(out_dalbedo=nanf(nv, 3), out_drough=nanf(nv), out_dspec=nanf(nv), out_dgauss_pos=nanf(ng, 3), out_ddisp=nanf(nv, 3),
+                          out_dscale=nanf(ng, 3))
+    rga.regularisers(av.h, 0.005, L, **o)
+    rga.rga_check(av.h)
+    got = L.cpu().numpy()
+    print(cfg, with_mlp, got, [ref[k] for k in ("smooth", "mdist", "disp", "scale")])
+    for i, k in enumerate(("smooth", "mdist", "disp", "scale")):
+        tol = 2e-2 if (with_mlp and k == "disp") else 1e-5
+        assert abs(got[i] - ref[k]) <= tol * abs(ref[k]) + 1e-7, (k, got[i], ref[k])
+    assert np.array_equal(o["out_dalbedo"].cpu().numpy(), ref["d_albedo"]) and np.array_equal(o["out_drough"].cpu().numpy(), ref["d_rough"])
+    assert np.array_equal(o["out_dspec"].cpu().numpy(), ref["d_spec"]) and np.array_equal(o["out_dscale"].cpu().numpy(), ref["d_scale"])
+    assert np.abs(o["out_dgauss_pos"].cpu().numpy() - ref["d_gauss_pos"]).max() < 1e-5
+    if not with_mlp:
+        assert np.abs(o["out_ddisp"].cpu().numpy() - ref["d_disp"]).max() < 1e-5
+    else:                                                                # unit vectors of nearly equal displacements
+        assert np.abs(o["out_ddisp"].cpu().numpy() - ref["d_disp"]).max() < 5e-2
+    av.close()
