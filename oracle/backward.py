@@ -251,3 +251,50 @@ def regularisers(vert_albedo, vert_rough, vert_spec, knn_v, gauss_pos, vert_pos,
     return {"smooth": float(smooth.detach()), "mdist": float(mdist.detach()), "disp": float(disp.detach()), "scale": float(scale.detach()),
             "d_albedo": a.grad.numpy(), "d_rough": r.grad.numpy(), "d_spec": p.grad.numpy(), "d_gauss_pos": xg.grad.numpy(),
             "d_disp": dx.grad.numpy(), "d_scale": s.grad.numpy()}
+
+
+# ------------------------------------------------------------------------------------------------ H2 + Eq.1 (canonical -> posed)
+def pose_torch(xg, quat, scale, bones, vert_disp, vert_normal, vert_albedo, vert_rough, vert_spec, knn_g, ubar, vert_skin_w):
+    """Canonical Gaussians -> posed space, differentiable (fp64): Eq.1 with the frozen neighbour sets S_g and
+    weights ubar for dx_g, n_g (renormalised), w_g, a_g, gamma_g, p_g; forward LBS (:95) M = sum_b w_gb G_b,
+    xbar = M [x_g + dx_g; 1], nbar = normalize(M3 n_g); covariance Sigma = A A^T, A = M3 R(q / |q|) diag(s)
+    (orc_skin / orc_gauss_cov / orc_interp_attr of rga_oracle.cpp, same formulas).  bones [B,12] row-major 3x4.
+    Returns xbar [N,3], nbar [N,3], cov6 [N,6], a_g [N,3], gamma_g [N], p_g [N]."""
+    u = ubar[:, :, None]
+    interp = lambda t: (u * t[knn_g]).sum(1) if t.dim() == 2 else (ubar * t[knn_g]).sum(1)
+    dx, nraw, w = interp(vert_disp), interp(vert_normal), interp(vert_skin_w)
+    a_g, r_g, p_g = interp(vert_albedo), interp(vert_rough), interp(vert_spec)
+    n_g = nraw / nraw.norm(dim=1, keepdim=True)
+    M = (w @ bones).reshape(-1, 3, 4)
+    M3, tr = M[:, :, :3], M[:, :, 3]
+    p = xg + dx
+    xbar = torch.einsum("nrc,nc->nr", M3, p) + tr
+    t = torch.einsum("nrc,nc->nr", M3, n_g)
+    nbar = t / t.norm(dim=1, keepdim=True)
+    q = quat / quat.norm(dim=1, keepdim=True)
+    qw, qx, qy, qz = q[:, 0], q[:, 1], q[:, 2], q[:, 3]
+    R = torch.stack([1 - 2 * (qy * qy + qz * qz), 2 * (qx * qy - qw * qz), 2 * (qx * qz + qw * qy),
+                     2 * (qx * qy + qw * qz), 1 - 2 * (qx * qx + qz * qz), 2 * (qy * qz - qw * qx),
+                     2 * (qx * qz - qw * qy), 2 * (qy * qz + qw * qx), 1 - 2 * (qx * qx + qy * qy)], 1).reshape(-1, 3, 3)
+    A = M3 @ (R * scale[:, None, :])
+    S = A @ A.transpose(1, 2)
+    cov6 = torch.stack([S[:, 0, 0], S[:, 0, 1], S[:, 0, 2], S[:, 1, 1], S[:, 1, 2], S[:, 2, 2]], 1)
+    return xbar, nbar, cov6, a_g, r_g, p_g
+
+
+def pose_backward(inp, knn_g, ubar, frame, d_mean, d_normal, d_cov6, d_alb_g, d_rough_g, d_spec_g):
+    """Gradient of L = <d_mean, xbar> + <d_normal, nbar> + <d_cov6, cov6> + <d_alb_g, a_g> + <d_rough_g, gamma_g> + <d_spec_g, p_g>
+    w.r.t. the canonical Gaussian position, rotation and scale, the bone transforms of the pose, and the vertex attributes
+    dx, n, a, gamma, p (through Eq.1's transpose; S_g, ubar and the skinning weights are frozen).  inp: the workload dict."""
+    T = lambda a: _t(a).requires_grad_(True)
+    leaves = {"d_gauss_pos": T(inp["gauss_pos"]), "d_gauss_quat": T(inp["gauss_quat"]), "d_gauss_scale": T(inp["gauss_scale"]),
+              "d_bones": T(np.asarray(inp["bone_mats"][frame]).reshape(-1, 12)), "d_vert_disp": T(inp["vert_disp"]),
+              "d_vert_normal": T(inp["vert_normal"]), "d_vert_albedo": T(inp["vert_albedo"]), "d_vert_rough": T(inp["vert_rough"]),
+              "d_vert_spec": T(inp["vert_spec"])}
+    outs = pose_torch(*leaves.values(), torch.as_tensor(np.asarray(knn_g).astype(np.int64)), _t(ubar), _t(inp["vert_skin_w"]))
+    cot = [d_mean, d_normal, d_cov6, d_alb_g, d_rough_g, d_spec_g]
+    sum((o * _t(c)).sum() for o, c in zip(outs, cot)).backward()
+    res = {k: v.grad.numpy() for k, v in leaves.items()}
+    res.update({"xbar": outs[0].detach().numpy(), "nbar": outs[1].detach().numpy(), "cov6": outs[2].detach().numpy(),
+                "a_g": outs[3].detach().numpy()})
+    return res

@@ -352,3 +352,53 @@ def test_regularisers_hand_example_and_finite_differences():
         ap[ai][idx] += 1e-7; am[ai][idx] -= 1e-7
         fd = (tot(bwd.regularisers(*ap)) - tot(bwd.regularisers(*am))) / 2e-7
         assert abs(fd - r[key][idx]) < 1e-5 * (1 + abs(fd)), key
+
+
+# ------------------------------------------------------------------------------------------------ H2 + Eq.1 backward
+def test_pose_backward_forward_equals_cpp_oracle_and_gradcheck():
+    inp = workloads.make(0)
+    av = orc.avatar_load(inp)
+    o = orc.render_frame(av, inp, stop_after="skin")
+    N = len(inp["gauss_pos"])
+    z3, z1, z6 = np.zeros((N, 3)), np.zeros(N), np.zeros((N, 6))
+    r = bwd.pose_backward(inp, av["knn_g"], av["ubar_g"], 0, z3, z3, z6, z3, z1, z1)
+    # same forward as orc_interp_attr + orc_skin + orc_gauss_cov (fp32 there, fp64 here)
+    assert np.abs(r["xbar"] - o["gauss_posed"]).max() < 2e-6 and np.abs(r["nbar"] - o["gauss_normal_posed"]).max() < 2e-6
+    assert np.allclose(r["cov6"], o["cov6"], rtol=2e-5, atol=1e-10) and np.abs(r["a_g"] - av["albedo_g"]).max() < 1e-6
+    # gradcheck on a small random instance (6 Gaussians, 5 vertices, 3 bones)
+    rs = np.random.default_rng(9)
+    t = lambda a: torch.tensor(a, dtype=torch.float64, requires_grad=True)
+    nv, ng, B = 5, 6, 3
+    nn = rs.normal(size=(nv, 3)); nn /= np.linalg.norm(nn, axis=1, keepdims=True)
+    w = rs.uniform(size=(nv, B)); w /= w.sum(1, keepdims=True)
+    u = rs.uniform(0.1, 1, (ng, 3)); u /= u.sum(1, keepdims=True)
+    args = (t(rs.normal(size=(ng, 3))), t(rs.normal(size=(ng, 4))), t(rs.uniform(0.01, 0.1, (ng, 3))), t(rs.normal(size=(B, 12))),
+            t(rs.normal(size=(nv, 3)) * 0.01), t(nn), t(rs.uniform(size=(nv, 3))), t(rs.uniform(size=nv)), t(rs.uniform(size=nv)))
+    knn = torch.tensor(rs.integers(0, nv, (ng, 3)))
+    f = lambda *a: bwd.pose_torch(*a, knn, torch.tensor(u), torch.tensor(w))
+    assert torch.autograd.gradcheck(f, args, eps=1e-7, atol=1e-7, rtol=1e-5)
+
+
+def test_pose_backward_identity_pose_closed_forms():
+    # every bone the identity: xbar = x_g + dx_g, nbar = n_g, Sigma = R diag(s^2) R^T.  Hand derivatives: d<g,xbar>/dx_g = g;
+    # d<g,xbar>/d(dx_v[k]) = sum of ubar over the Gaussians that list k; with only d_cov6 xx = 1 and R = I: d/ds_x = 2 s_x
+    inp = workloads.make(0)
+    B = inp["bone_mats"].shape[1]
+    inp = dict(inp); inp["bone_mats"] = np.tile(np.eye(3, 4, dtype=np.float32)[None, None], (1, B, 1, 1))
+    inp["gauss_quat"] = np.tile(np.array([[1.0, 0, 0, 0]], np.float32), (len(inp["gauss_pos"]), 1))
+    av = orc.avatar_load(inp)
+    N, nv = len(inp["gauss_pos"]), len(inp["vert_pos"])
+    g = np.random.default_rng(10).normal(size=(N, 3))
+    z3, z1, z6 = np.zeros((N, 3)), np.zeros(N), np.zeros((N, 6))
+    r = bwd.pose_backward(inp, av["knn_g"], av["ubar_g"], 0, g, z3, z6, z3, z1, z1)
+    assert np.allclose(r["d_gauss_pos"], g)
+    ref = np.zeros((nv, 3)); np.add.at(ref, av["knn_g"].reshape(-1), (av["ubar_g"][:, :, None] * g[:, None, :]).reshape(-1, 3))
+    assert np.allclose(r["d_vert_disp"], ref, rtol=1e-5, atol=1e-6)       # the fp32 skinning weights sum to 1 within 1e-7
+    c = z6.copy(); c[:, 0] = 1.0
+    r = bwd.pose_backward(inp, av["knn_g"], av["ubar_g"], 0, z3, z3, c, z3, z1, z1)
+    assert np.allclose(r["d_gauss_scale"][:, 0], 2 * inp["gauss_scale"][:, 0], rtol=1e-6) and np.allclose(r["d_gauss_scale"][:, 1:], 0, atol=1e-12)
+    # Eq.1's transpose for a material attribute
+    ga = np.random.default_rng(11).normal(size=(N, 3))
+    r = bwd.pose_backward(inp, av["knn_g"], av["ubar_g"], 0, z3, z3, z6, ga, z1, z1)
+    ref = np.zeros((nv, 3)); np.add.at(ref, av["knn_g"].reshape(-1), (av["ubar_g"][:, :, None] * ga[:, None, :]).reshape(-1, 3))
+    assert np.allclose(r["d_vert_albedo"], ref, rtol=1e-12, atol=1e-12)
