@@ -298,6 +298,30 @@ def main():
         run_rg()
     rg_obj = {"ms": timed(run_rg, 20), "vertices": nv_all, "gaussians": ng_all}
 
+    # ... the pull-back to the canonical parameters (H2 + Eq.1), and the whole backward chain of one training view:
+    # image_loss -> splat_backward -> shade_backward -> pose_backward, each fed by the previous call
+    nb_all = inp["bone_mats"].shape[1]
+    pb_out = {"d_gauss_pos": torch.empty((ng_all, 3), device=dev), "d_gauss_quat": torch.empty((ng_all, 4), device=dev),
+              "d_gauss_scale": torch.empty((ng_all, 3), device=dev), "d_bones": torch.empty((nb_all, 12), device=dev),
+              "d_vert_disp": torch.empty((nv_all, 3), device=dev), "d_vert_normal": torch.empty((nv_all, 3), device=dev),
+              "d_vert_albedo": torch.empty((nv_all, 3), device=dev), "d_vert_rough": torch.empty(nv_all, device=dev),
+              "d_vert_spec": torch.empty(nv_all, device=dev)}
+    pb_in = {"d_mean": d_x, "d_mean2": sb["out_dpos"], "d_normal": sb["out_dnormal"], "d_cov": d_cov, "d_albedo": sb["out_dalbedo"],
+             "d_rough": sb["out_drough"], "d_spec": sb["out_dspec"]}
+    run_pb = lambda: rga.pose_backward(av.h, bones, pb_in, pb_out)
+    for _ in range(3):
+        run_pb()
+    ms_pb = timed(run_pb, 20)
+    def run_chain():
+        run_il(); run_bwd(); run_sb(); run_pb()
+    for _ in range(3):
+        run_chain()
+    l_chain = rga.rga_launch_count(av.h)
+    ms_chain = timed(run_chain, 20)
+    l_chain = (rga.rga_launch_count(av.h) - l_chain) // 20
+    train_obj = {"pose_backward_ms": ms_pb, "backward_chain_ms": ms_chain, "launches": int(l_chain),
+                 "note": "image_loss + splat_backward + shade_backward + pose_backward of the rendered view; forward frame = ms_per_step"}
+
     # algorithmic units of each candidate dominant kernel: counted from the frame that was rendered
     gp = av.read("GAUSS_POSED").reshape(-1, 4)[:, :3]; gn = av.read("GAUSS_NORMAL_POSED").reshape(-1, 4)[:, :3]
     front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
@@ -368,7 +392,7 @@ def main():
                 "pipelined_value": world * 1e3 / ms_e2e_pipe,
                 "pipelined_note": "image read-back of step i on a copy stream beside step i+1; per-step events plus the last copy's tail"},
         "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
-        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj, "shade_backward": sb_obj, "image_loss": il_obj, "regularisers": rg_obj,
+        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj, "shade_backward": sb_obj, "image_loss": il_obj, "regularisers": rg_obj, "train_backward": train_obj,
         "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -181,6 +181,23 @@ RGA_API rga_status image_loss(rga_avatar* av, const float* image, const float* t
 RGA_API rga_status regularisers(rga_avatar* av, float s0, float* out_losses, float* out_dalbedo, float* out_drough, float* out_dspec,
                                 float* out_dgauss_pos, float* out_ddisp, float* out_dscale, void* stream);
 
+/* Backward of pose_skin's Gaussian half (H2) and of Eq.1: pulls a frame's posed-space gradients back to the canonical
+ * parameters the paper optimises.  Inputs (DEVICE, each may be NULL = zero): d_mean [n_gauss][3]
+ * and d_mean2 [n_gauss][3], summed = dL/d xbar_gd (splat_backward's out_dmean and shade_backward's out_dpos), d_normal [n_gauss][3] = dL/d nbar_gd
+ * (shade_backward's out_dnormal), d_cov [n_gauss][6] (splat_backward's out_dcov), and the per-Gaussian material gradients
+ * d_albedo [n_gauss][3], d_rough, d_spec [n_gauss] (shade_backward's).  bone_mats: dev [n_bones][12], the pose of that
+ * frame.  Outputs (DEVICE, each may be NULL): d_gauss_pos [n_gauss][3] (canonical x_g), d_gauss_quat [n_gauss][4] (w,x,y,z;
+ * the forward normalises q, so the gradient is tangent to it), d_gauss_scale [n_gauss][3], d_bones [n_bones][12] (the pose,
+ * :155), and through the transpose of Eq.1 -- S_g and its weights frozen -- the vertex attributes d_vert_disp [n_verts][3]
+ * (dx), d_vert_normal [n_verts][3] (n, incl. the renormalisation of the interpolated normal), d_vert_albedo [n_verts][3],
+ * d_vert_rough, d_vert_spec [n_verts].  The skinning weights are not differentiated.  k_g <= 8.  Enqueue-only. */
+typedef struct { const float *d_mean, *d_mean2, *d_normal, *d_cov, *d_albedo, *d_rough, *d_spec; } rga_posed_grads;
+typedef struct {
+  float *d_gauss_pos, *d_gauss_quat, *d_gauss_scale, *d_bones, *d_vert_disp, *d_vert_normal, *d_vert_albedo, *d_vert_rough, *d_vert_spec;
+} rga_canonical_grads;
+RGA_API rga_status pose_backward(rga_avatar* av, const float* bone_mats, const rga_posed_grads* in, const rga_canonical_grads* out,
+                                 void* stream);
+
 /* Algorithm 1, "Gaussian densification based on density": from the avatar's current
  * S_g (avatar_load / gaussians_update) and its mesh, counts the Gaussians near every vertex (D_v), estimates the Gaussian
  * density of every triangle d_f = sum of its three D_v / (6 K_g), sets P = max(0, d0 - d_f), asks for

@@ -214,6 +214,24 @@ def regularisers(h, s0=0.005, out_losses=None, out_dalbedo=None, out_drough=None
                             _ptr(out_ddisp), _ptr(out_dscale), _stream()))
 
 
+class _PosedGrads(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("d_mean", "d_mean2", "d_normal", "d_cov", "d_albedo", "d_rough", "d_spec")]
+
+
+class _CanonicalGrads(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("d_gauss_pos", "d_gauss_quat", "d_gauss_scale", "d_bones", "d_vert_disp", "d_vert_normal",
+                                          "d_vert_albedo", "d_vert_rough", "d_vert_spec")]
+
+
+def pose_backward(h, bone_mats, posed, canonical):
+    """Backward of H2 + Eq.1 (include/rga.h pose_backward).  posed / canonical: dicts of CUDA float32 tensors keyed by the
+    field names of rga_posed_grads / rga_canonical_grads; missing keys are NULL."""
+    pin = _PosedGrads(*[None if posed.get(n) is None else posed[n].data_ptr() for n, _ in _PosedGrads._fields_])
+    pout = _CanonicalGrads(*[None if canonical.get(n) is None else canonical[n].data_ptr() for n, _ in _CanonicalGrads._fields_])
+    lib().pose_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(_PosedGrads), C.POINTER(_CanonicalGrads), C.c_void_p]
+    _chk(lib().pose_backward(h, _ptr(bone_mats), C.byref(pin), C.byref(pout), _stream()))
+
+
 def densify_density(h, d0, p0, rnd, out_pos, out_tri=None, out_count=None):
     """Algorithm 1, density-based densification (include/rga.h densify_density).  rnd: CUDA int32/uint32 tensor [3 * max_out]
     of raw 32-bit random numbers; out_pos: CUDA float32 [max_out, 3]; out_tri / out_count: CUDA int32 [max_out] / [1] or None."""

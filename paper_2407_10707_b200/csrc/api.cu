@@ -313,6 +313,16 @@ extern "C" rga_status regularisers(rga_avatar* av, float s0, float* out_losses, 
   return RGA_OK;
 }
 
+extern "C" rga_status pose_backward(rga_avatar* av, const float* bone_mats, const rga_posed_grads* in, const rga_canonical_grads* out,
+                                    void* stream) {
+  if (!av || !bone_mats || !in || !out) return fail(RGA_ERR_INVALID_ARG, "pose_backward: null argument");
+  if (av->k_g > 8) return fail(RGA_ERR_INVALID_ARG, "pose_backward: k_g > 8 is not supported");
+  cudaStream_t s = (cudaStream_t)stream;
+  rga_prof_mark(av, "-", s);
+  CU(rga_launch_pose_backward(av, bone_mats, in, out, s));
+  return RGA_OK;
+}
+
 extern "C" rga_status densify_density(rga_avatar* av, float d0, float p0, const uint32_t* rnd, int max_out, float* out_pos,
                                       int32_t* out_tri, int32_t* out_count, void* stream) {
   if (!av) return fail(RGA_ERR_INVALID_ARG, "densify_density: null avatar");

@@ -143,6 +143,8 @@ cudaError_t rga_launch_image_loss(rga_avatar* av, const float* image, const floa
                                   float* out_dimage, cudaStream_t s);
 cudaError_t rga_launch_regularisers(rga_avatar* av, float s0, float* out_losses, float* d_alb, float* d_rough, float* d_spec, float* d_gpos,
                                     float* d_disp, float* d_scale, cudaStream_t s);
+// pose_backward_kernels.cu
+cudaError_t rga_launch_pose_backward(rga_avatar* av, const float* bone_mats, const rga_posed_grads* in, const rga_canonical_grads* out, cudaStream_t s);
 // densify_kernels.cu
 cudaError_t rga_launch_densify(rga_avatar* av, float d0, float p0, const unsigned* rnd, int max_out, float* out_pos, int* out_tri,
                                int* out_count, cudaStream_t s);

@@ -247,3 +247,8 @@ def make_image_pair(seed, width, height):
     img = np.clip(tgt + rs.normal(0.0, 0.05, tgt.shape), 0.0, 1.0)
     img[: height // 4, : width // 4] = 0.0                                # a black corner: zero-variance windows on one side
     return img.astype(np.float32), tgt.astype(np.float32)
+
+
+def make_cotangent(seed, shape):
+    """A seeded standard-normal cotangent (fp32) of any shape, for the backward tests and benches."""
+    return np.random.default_rng(4000 + seed).normal(size=shape).astype(np.float32)
