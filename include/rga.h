@@ -244,7 +244,11 @@ RGA_API rga_status splat_attribute(rga_avatar* av, const rga_camera* cam, const 
  * env->use_visibility == 0), shade_gaussians and splat_render with the same arguments, results and intermediates as the
  * four calls above.  Enqueue-only like them.  The steps that depend neither on visibility nor on shading (H6-H9 and
  * the environment table) are issued on a second stream owned by the avatar and joined before the blend, so `stream`
- * observes the whole frame in order; the call can be captured into a CUDA graph. */
+ * observes the whole frame in order; the call can be captured into a CUDA graph.
+ * One difference in the intermediates: this call knows the camera when it tests visibility, so in mode 0 the depth test
+ * is not run for Gaussians that face away from the camera (their opacity is 0 and shade_gaussians skips
+ * them by the same test); their RGA_BUF_VISBITS words are 0.  Radiance, colour and image are unchanged.  To shade the
+ * same pose from ANOTHER camera afterwards, call visibility_raster first (shade_gaussians returns RGA_ERR_STATE if not). */
 RGA_API rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, const rga_vis_params* vis, const rga_env* env,
                                     const float cam_pos[3], const rga_camera* cam, const float bg[3], float* out_image,
                                     void* stream);

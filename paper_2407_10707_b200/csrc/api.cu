@@ -210,8 +210,9 @@ extern "C" rga_status visibility_raster(rga_avatar* av, const rga_vis_params* p,
   av->have_vis = av->have_shade = av->have_splat = 0;
   rga_prof_mark(av, "-", s);
   CU(rga_launch_vis_raster(av, p, s));
-  if (p->mode == 0) CU(rga_launch_vis_depth_test(av, p, s));
+  if (p->mode == 0) CU(rga_launch_vis_depth_test(av, p, nullptr, s));
   else CU(rga_launch_vis_paper(av, p, s));
+  av->vis_culled = 0;
   av->vis_mode = p->mode; av->vis_dirs = p->n_dirs; av->vis_res = p->res; av->vis_words = (p->n_dirs + 31) / 32;
   av->keep_maps = p->keep_maps || p->mode == 1;
   av->have_vis = 1;
@@ -222,6 +223,10 @@ extern "C" rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const 
   if (!av || !env || !env->radiance || !cam_pos) return fail(RGA_ERR_INVALID_ARG, "shade_gaussians: null argument");
   if (!av->have_skin) return fail(RGA_ERR_STATE, "shade_gaussians: call pose_skin first");
   if (env->use_visibility && !av->have_vis) return fail(RGA_ERR_STATE, "shade_gaussians: call visibility_raster first");
+  if (env->use_visibility && av->vis_mode == 0 && av->vis_culled &&
+      (cam_pos[0] != av->vis_cull_cam[0] || cam_pos[1] != av->vis_cull_cam[1] || cam_pos[2] != av->vis_cull_cam[2]))
+    return fail(RGA_ERR_STATE, "shade_gaussians: rga_render_frame computed this pose's visibility only for Gaussians facing ITS camera; "
+                               "call visibility_raster before shading from another camera");
   if (env->rows < 1 || env->cols < 1 || env->rows * env->cols > av->max_env || !(env->gamma > 0.f))
     return fail(RGA_ERR_INVALID_ARG, "shade_gaussians: env size/gamma out of range");
   if (env->use_visibility && !env->texel_to_dir && env->rows * env->cols != av->vis_dirs)
@@ -281,6 +286,9 @@ extern "C" rga_status shade_backward(rga_avatar* av, const rga_env* env, const f
   if (!av || !env || !env->radiance || !cam_pos || !dL_dcolor) return fail(RGA_ERR_INVALID_ARG, "shade_backward: null argument");
   if (!av->have_shade) return fail(RGA_ERR_STATE, "shade_backward: call shade_gaussians (or rga_render_frame) first");
   if (env->use_visibility && !av->have_vis) return fail(RGA_ERR_STATE, "shade_backward: no visibility for this pose");
+  if (env->use_visibility && av->vis_mode == 0 && av->vis_culled &&
+      (cam_pos[0] != av->vis_cull_cam[0] || cam_pos[1] != av->vis_cull_cam[1] || cam_pos[2] != av->vis_cull_cam[2]))
+    return fail(RGA_ERR_STATE, "shade_backward: this pose's visibility was computed for another camera (rga_render_frame)");
   if (env->rows < 1 || env->cols < 1 || env->rows * env->cols > av->max_env || !(env->gamma > 0.f))
     return fail(RGA_ERR_INVALID_ARG, "shade_backward: env size/gamma out of range");
   if (env->use_visibility && !env->texel_to_dir && env->rows * env->cols != av->vis_dirs)
@@ -411,8 +419,13 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   if (vis) {
     CU(rga_launch_vis_raster(av, vis, s));
     if (overlap) CU(cudaStreamWaitEvent(s, av->ev_gskin, 0));
-    if (vis->mode == 0) CU(rga_launch_vis_depth_test(av, vis, s));
-    else CU(rga_launch_vis_paper(av, vis, s));
+    if (vis->mode == 0) {
+      CU(rga_launch_vis_depth_test(av, vis, cam_pos, s));
+      av->vis_culled = 1; av->vis_cull_cam[0] = cam_pos[0]; av->vis_cull_cam[1] = cam_pos[1]; av->vis_cull_cam[2] = cam_pos[2];
+    } else {
+      CU(rga_launch_vis_paper(av, vis, s));
+      av->vis_culled = 0;
+    }
     av->vis_mode = vis->mode; av->vis_dirs = vis->n_dirs; av->vis_res = vis->res; av->vis_words = (vis->n_dirs + 31) / 32;
     av->keep_maps = vis->keep_maps || vis->mode == 1;
     av->have_vis = 1;

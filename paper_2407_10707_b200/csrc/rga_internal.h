@@ -88,6 +88,7 @@ struct rga_avatar {
   // state of the current pose
   int have_skin, have_vis, have_shade, have_splat;
   int vis_mode, vis_dirs, vis_res, vis_words, keep_maps;
+  int vis_culled; float vis_cull_cam[3];   // mode-0 bits were computed only for Gaussians facing this camera (rga_render_frame)
   int cam_w, cam_h;
   long long launches;
   // rga_render_frame: the splat preparation (H6-H9) runs on a second stream beside visibility and shading
@@ -110,7 +111,7 @@ cudaError_t rga_launch_load_gauss(rga_avatar* av, const float* gauss_pos, const 
 cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, int which, cudaStream_t s);
 // vis_kernels.cu
 cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
-cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
+cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, const float* cull_cam, cudaStream_t s);
 cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
 size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads);
 cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s);

@@ -30,8 +30,19 @@ def run_gpu(inp, vis_mode=0, frame=0, keep_maps=True, use_visibility=True, max_d
     return av, img.cpu().numpy()
 
 
-def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=None):
-    """Assert stage-by-stage parity.  `o` is oracle.render_frame's dict, `orc_av` oracle.avatar_load's."""
+def facing_split(inp, o, cam_pos=None):
+    """(kept, culled) masks of the Gaussians w.r.t. the camera-facing test of rga_render_frame / shade_gaussians
+    (PAPER.md:101), with a guard band around 0 in which neither is asserted."""
+    cp = inp["cam_pos"] if cam_pos is None else cam_pos
+    wo = cp[None, :].astype(np.float64) - o["gauss_posed"]
+    f = (wo * o["gauss_normal_posed"]).sum(1) / np.linalg.norm(wo, axis=1)
+    return f > 1e-3, f < -1e-3
+
+
+def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=None, frame_call=False):
+    """Assert stage-by-stage parity.  `o` is oracle.render_frame's dict, `orc_av` oracle.avatar_load's.
+    frame_call: the frame came from rga_render_frame, whose mode-0 depth test skips Gaussians that face away from the
+    camera (their bits are never read): visibility bits are compared on the kept Gaussians and must be 0 on the culled."""
     rep = report if report is not None else {}
     ng, nv = len(inp["gauss_pos"]), len(inp["vert_pos"])
     K, R = len(inp["vis_dirs"]), inp["vis_res"]
@@ -63,7 +74,13 @@ def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=N
         if ids.size:
             assert eq(ids.reshape(K, R, R), o["idmap"]), "idmap"
         if vis_mode == 0:
-            assert eq(rd("VISBITS").reshape(ng, words), o["visbits"]), "visbits"
+            vb = rd("VISBITS").reshape(ng, words)
+            if frame_call:
+                kept, culled = facing_split(inp, o)
+                assert kept.sum() > 0 and eq(vb[kept], o["visbits"][kept]), "visbits (camera-facing Gaussians)"
+                assert not vb[culled].any(), "visbits of culled Gaussians"
+            else:
+                assert eq(vb, o["visbits"]), "visbits"
         else:
             assert eq(rd("VCOUNT").reshape(nv, K), o["vcount"]), "vcount"
     # H6 (bit-exact)

@@ -63,7 +63,7 @@ def test_cfg3_animation_frames():
     import torch
     from oracle import oracle as orc
     from paper_2407_10707_b200 import binding as rga
-    from parity_util import IMG_MAX
+    from parity_util import IMG_MAX, facing_split
     inp = workloads.make(3, n_gauss=20_000)
     orc_av = orc.avatar_load(inp)
     cam = inp["camera"]; W, H = cam["width"], cam["height"]
@@ -75,7 +75,9 @@ def test_cfg3_animation_frames():
         av.render(bones[t], dirs, 128, envs[int(inp["env_of_frame"][t])], t2d, inp["cam_pos"], cam, inp["bg"], img)
         rga.rga_check(av.h)
         o = orc.render_frame(orc_av, inp, frame=t, vis_mode=0)
-        assert np.array_equal(av.read("VISBITS").reshape(len(inp["gauss_pos"]), -1), o["visbits"])
+        kept, culled = facing_split(inp, o)                             # rga_render_frame tests only camera-facing Gaussians
+        vb = av.read("VISBITS").reshape(len(inp["gauss_pos"]), -1)
+        assert np.array_equal(vb[kept], o["visbits"][kept]) and not vb[culled].any()
         assert np.array_equal(av.read("KEYS_SORTED"), o["keys"]) and np.array_equal(av.read("VALS_SORTED"), o["vals"])
         d = np.abs(img.cpu().numpy().astype(np.float64) - o["image"]).max(-1)
         assert d[o["flags"] == 0].max() <= IMG_MAX
@@ -120,13 +122,18 @@ def test_edge_cases_state_capacity_and_args():
 
 
 def test_render_frame_equals_the_four_calls():
-    # rga_render_frame overlaps H6-H9 with H3-H5 on a second stream: same kernels, so every output must be identical
+    # rga_render_frame overlaps H6-H9 with H3-H5 on a second stream: same kernels, so every output must be identical --
+    # except the visibility words of Gaussians that face away from the camera, which it does not compute (they are 0)
     import torch
+    from oracle import oracle as orc
     from paper_2407_10707_b200 import binding as rga
-    from parity_util import run_gpu
+    from parity_util import facing_split, run_gpu
     inp = workloads.make(1, n_gauss=30_000)
     av, img4 = run_gpu(inp, vis_mode=0, keep_maps=False)
     keys4, vis4, col4 = av.read("KEYS_SORTED"), av.read("VISBITS"), av.read("COLOR")
+    kept, culled = facing_split(inp, orc.render_frame(orc.avatar_load(inp), inp, stop_after="skin"))
+    assert kept.sum() > 5000 and culled.sum() > 5000
+    vis4 = vis4.reshape(len(kept), -1).copy(); vis4[~kept] = 0
     cam = inp["camera"]
     img = torch.empty((cam["height"], cam["width"], 3), dtype=torch.float32, device="cuda")
     bias = (inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
@@ -135,9 +142,18 @@ def test_render_frame_equals_the_four_calls():
                   torch.as_tensor(inp["env"][0]).cuda(), torch.as_tensor(inp["texel_to_dir"]).cuda(), inp["cam_pos"], cam,
                   inp["bg"], img, vis_mode=0, gamma=inp["gamma"], bias=bias)
         rga.rga_check(av.h)
-        assert np.array_equal(av.read("KEYS_SORTED"), keys4) and np.array_equal(av.read("VISBITS"), vis4)
+        vb = av.read("VISBITS").reshape(len(kept), -1).copy()
+        assert not vb[culled].any()
+        vb[~kept] = 0                                                   # guard band around facing = 0: either is fine
+        assert np.array_equal(av.read("KEYS_SORTED"), keys4) and np.array_equal(vb, vis4)
         assert np.array_equal(av.read("COLOR"), col4)
         assert np.array_equal(img.cpu().numpy(), img4)
+    # the visibility of this frame is only valid for its camera: shading from another one is refused, the same one is fine
+    with pytest.raises(RuntimeError):
+        rga.shade_gaussians(av.h, torch.as_tensor(inp["env"][0]).cuda(), inp["cam_pos"] + np.float32(0.5), torch.as_tensor(inp["texel_to_dir"]).cuda(),
+                            inp["gamma"], True)
+    rga.shade_gaussians(av.h, torch.as_tensor(inp["env"][0]).cuda(), inp["cam_pos"], torch.as_tensor(inp["texel_to_dir"]).cuda(), inp["gamma"], True)
+    assert np.array_equal(av.read("COLOR"), col4)
     # the same call inside a CUDA graph (fork / join on the avatar's second stream is capturable)
     bones = torch.as_tensor(inp["bone_mats"][0]).cuda(); dirs = torch.as_tensor(inp["vis_dirs"]).cuda()
     env = torch.as_tensor(inp["env"][0]).cuda(); t2d = torch.as_tensor(inp["texel_to_dir"]).cuda()
@@ -313,7 +329,7 @@ def test_gaussians_update_equals_a_fresh_load():
     rga.rga_check(av.h)
     assert (orc_av["knn_g"] != orc.avatar_load(inp)["knn_g"]).any()          # the move does change neighbour sets
     # keep_maps was off in this frame: compare everything except the triangle-id maps
-    rep = compare_all(inp2, av, img.cpu().numpy(), orc_av, o, 0)
+    rep = compare_all(inp2, av, img.cpu().numpy(), orc_av, o, 0, frame_call=True)
     print(rep)
     av.close()
 
