@@ -89,14 +89,14 @@ def light_frames(dirs):
     return out
 
 
-def vis_raster(xp, faces, dirs, R, c, r, want_ids=True):
+def vis_raster(xp, faces, dirs, R, c, r, want_ids=True, cull=False):
     xp, dirs, c = _f32(xp), _f32(dirs), _f32(c)
     faces = np.ascontiguousarray(faces, np.int32)
     K = len(dirs)
     z = np.empty((K, R, R), np.uint32)
     ids = np.empty((K, R, R), np.int32) if want_ids else None
     lib().orc_vis_raster(_p(xp), C.c_int(len(xp)), _p(faces), C.c_int(len(faces)), _p(dirs), C.c_int(K), C.c_int(R),
-                         _p(c), C.c_float(r), _p(z), _p(ids))
+                         _p(c), C.c_float(r), _p(z), _p(ids), C.c_int(int(cull)))
     return z, ids
 
 
@@ -298,7 +298,8 @@ def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None):
     K = len(dirs)
     bits = vg = None
     if vis_mode in (0, 1):
-        o["zmap"], o["idmap"] = vis_raster(o["vert_posed"], inp["faces"], dirs, R, o["win_c"], o["win_r"], want_ids=True)
+        o["zmap"], o["idmap"] = vis_raster(o["vert_posed"], inp["faces"], dirs, R, o["win_c"], o["win_r"], want_ids=True,
+                                           cull=bool(inp.get("vis_cull_backfaces", False)))
     if vis_mode == 0:
         bits = o["visbits"] = vis_depth_test(o["gauss_posed"], o["gauss_normal_posed"], dirs, R, o["win_c"], o["win_r"],
                                              o["zmap"], inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])

@@ -178,8 +178,10 @@ static inline void light_project(const float* p, const float* c, float r, const 
 // centre covered when the three edge functions share a sign or are zero (two-sided, inclusive), depth
 // z = (z0 + (e1/area)(z1-z0)) + (e2/area)(z2-z0) in fp32, clamped at 0, winner = min (zbits << 32 | tri).
 // zmap: [K][R][R] float bits, 0xFFFFFFFF = empty; idmap: [K][R][R] triangle id, -1 = empty (may be NULL).
+// cull != 0 (reading A36, an option for closed, outward-oriented meshes): a triangle whose snapped area is negative --
+// it faces away from the light -- is skipped like a zero-area one.
 ORC void orc_vis_raster(const float* xp, int nv, const int32_t* f, int nf, const float* dirs, int K, int R,
-                        const float* c, float r, uint32_t* zmap, int32_t* idmap) {
+                        const float* c, float r, uint32_t* zmap, int32_t* idmap, int cull) {
 #pragma omp parallel for schedule(dynamic, 1)
   for (int k = 0; k < K; ++k) {
     float u[3], v[3]; const float* w = dirs + 3 * k;
@@ -195,6 +197,7 @@ ORC void orc_vis_raster(const float* xp, int nv, const int32_t* f, int nf, const
       int64_t x0 = X[i0], y0 = Y[i0], x1 = X[i1], y1 = Y[i1], x2 = X[i2], y2 = Y[i2];
       int64_t area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
       if (area == 0) continue;
+      if (cull && area < 0) continue;
       int64_t mnx = std::min(x0, std::min(x1, x2)), mxx = std::max(x0, std::max(x1, x2));
       int64_t mny = std::min(y0, std::min(y1, y2)), mxy = std::max(y0, std::max(y1, y2));
       // pixel i has centre 256 i + 128: first i with centre >= mnx, last with centre <= mxx

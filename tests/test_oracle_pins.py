@@ -532,3 +532,39 @@ def test_densify_uniform_density_closed_form():
     d_f = 3 * (3 * D) / (6.0 * Kg)
     assert np.allclose(r["P_fix"] / 65536.0, 2.0 - d_f, atol=2.0 ** -16)
     assert r["n_add"] == int(np.floor(len(faces) * (2.0 - d_f) * 0.25))
+
+
+def test_backface_cull_option_of_the_depth_rasteriser(cfg0):
+    # reading A36: cull = the same rasteriser over the mesh WITHOUT the triangles whose snapped light-space area is
+    # negative.  The area is recomputed here in numpy from the light frame (independent of the C++ code path).
+    inp = cfg0
+    av = orc.avatar_load(inp)
+    o = orc.render_frame(av, inp, stop_after="skin")
+    dirs, R = inp["vis_dirs"][:24], 64
+    xp, f = o["vert_posed"], inp["faces"]
+    zc, ic = orc.vis_raster(xp, f, dirs, R, o["win_c"], o["win_r"], cull=True)
+    zn, idn = orc.vis_raster(xp, f, dirs, R, o["win_c"], o["win_r"], cull=False)
+    uvw = orc.light_frames(dirs)                                        # [K, 9]: u, v, w of every direction
+    n_front = 0
+    for k in range(len(dirs)):
+        s = (R / 2.0) / float(o["win_r"])
+        d = (xp - o["win_c"]).astype(np.float64)
+        X = np.rint((d @ uvw[k, 0:3].astype(np.float64) * s + R / 2) * 256); Y = np.rint((d @ uvw[k, 3:6].astype(np.float64) * s + R / 2) * 256)
+        area = (X[f[:, 1]] - X[f[:, 0]]) * (Y[f[:, 2]] - Y[f[:, 0]]) - (Y[f[:, 1]] - Y[f[:, 0]]) * (X[f[:, 2]] - X[f[:, 0]])
+        keep = np.nonzero(area > 0)[0]
+        n_front += len(keep)
+        zk, ik = orc.vis_raster(xp, f[keep], dirs[k:k + 1], R, o["win_c"], o["win_r"], cull=False)
+        assert np.array_equal(zk[0], zc[k])
+        assert np.array_equal(np.where(ik[0] >= 0, keep[np.maximum(ik[0], 0)], -1), ic[k])
+        # outward-oriented closed mesh: a positive snapped area is a triangle that faces the light
+        nrm = np.cross(xp[f[:, 1]] - xp[f[:, 0]], xp[f[:, 2]] - xp[f[:, 0]])
+        front = (nrm @ dirs[k]) > 0
+        big = np.abs(area) > 4 * 256
+        assert (front[big] == (area[big] > 0)).all()
+    assert 0.3 < n_front / (len(dirs) * len(f)) < 0.7
+    # on a closed mesh the nearest surface is a front face: the culled map differs from the full one only where a nearly
+    # edge-on back face extrapolates its plane in front of it (a fraction of a percent of the covered texels)
+    cov = zn != 0xFFFFFFFF
+    assert np.array_equal(cov, zc != 0xFFFFFFFF)
+    assert (zc != zn).sum() < 0.01 * cov.sum()
+    assert (zc.view(np.float32)[cov] >= zn.view(np.float32)[cov]).all()
