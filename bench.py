@@ -84,6 +84,7 @@ def run_reference(args, rank):
     from oracle import oracle as orc
     from synth import workloads
     inp = workloads.make(1)
+    inp["vis_cull_backfaces"] = bool(args.cull_backfaces)
     cores = os.cpu_count()
     av = orc.avatar_load(inp)
     for _ in range(max(args.warmup, 1)):
@@ -96,7 +97,7 @@ def run_reference(args, rank):
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic", "config": {"workload": WORKLOAD, "vis_mode": args.vis_mode},
+        "dtype": "f32", "data": "synthetic", "config": {"workload": WORKLOAD, "vis_mode": args.vis_mode, "vis_cull_backfaces": bool(args.cull_backfaces)},
         "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle",
                          "sample": "%d full frames of configs[1] (every step of the path, OpenMP on outer loops)" % args.steps},
         "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
@@ -109,6 +110,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--vis-mode", type=int, default=0, help="0 = depth test (north_star, default), 1 = paper filters")
+    ap.add_argument("--cull-backfaces", type=int, default=1,
+                    help="1 (default): the workload's body mesh is closed and outward-oriented, so the depth rasteriser skips "
+                         "triangles that face away from the light (rga_vis_params.cull_backfaces, DESIGN.md A36); 0: rasterise all")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -143,8 +147,10 @@ def main():
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)            # > 126 MB L2
     bias = (inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
 
+    cull = bool(args.cull_backfaces)
+
     def frame(b=bones, e=env):
-        av.render(b, dirs, R, e, t2d, inp["cam_pos"], camc, inp["bg"], img, vis_mode=args.vis_mode, bias=bias)
+        av.render(b, dirs, R, e, t2d, inp["cam_pos"], camc, inp["bg"], img, vis_mode=args.vis_mode, bias=bias, cull_backfaces=cull)
 
     def barrier():
         torch.cuda.synchronize()
@@ -170,6 +176,12 @@ def main():
     ms = timed(frame, args.steps)
     launches = rga.rga_launch_count(av.h) - l0
     ms_warm = timed(frame, args.steps, do_flush=False)
+    ms_nocull = None
+    if cull:                                                     # the same frame with every triangle rasterised, for comparison
+        frame_all = lambda: av.render(bones, dirs, R, env, t2d, inp["cam_pos"], camc, inp["bg"], img, vis_mode=args.vis_mode, bias=bias)
+        for _ in range(3):
+            frame_all()
+        ms_nocull = timed(frame_all, max(args.steps // 4, 10))
 
     # end to end: host (pinned) pose + env in, image out, every step, through the same C-ABI calls
     h_bones = torch.as_tensor(inp["bone_mats"][0]).pin_memory(); h_env = torch.as_tensor(inp["env"][0]).pin_memory()
@@ -201,7 +213,7 @@ def main():
             if copied[i & 1] is not None:
                 torch.cuda.current_stream().wait_event(copied[i & 1])     # buffer i&1 has been read back
             d_bones.copy_(h_bones, non_blocking=True); d_env.copy_(h_env, non_blocking=True)
-            av.render(d_bones, dirs, R, d_env, t2d, inp["cam_pos"], camc, inp["bg"], imgs[i & 1], vis_mode=args.vis_mode, bias=bias)
+            av.render(d_bones, dirs, R, d_env, t2d, inp["cam_pos"], camc, inp["bg"], imgs[i & 1], vis_mode=args.vis_mode, bias=bias, cull_backfaces=cull)
             b.record()
             copy_stream.wait_event(b)
             with torch.cuda.stream(copy_stream):
@@ -239,7 +251,7 @@ def main():
     NV = 4
     def pose_with_views():
         rga.pose_skin(av.h, bones)
-        rga.visibility_raster(av.h, dirs, R, args.vis_mode, bias[0], bias[1], bias[2])
+        rga.visibility_raster(av.h, dirs, R, args.vis_mode, bias[0], bias[1], bias[2], cull_backfaces=cull)
         for _ in range(NV):
             rga.shade_gaussians(av.h, env, inp["cam_pos"], t2d, inp["gamma"], True)
             rga.splat_render(av.h, camc, inp["bg"], img)
@@ -326,10 +338,15 @@ def main():
     gp = av.read("GAUSS_POSED").reshape(-1, 4)[:, :3]; gn = av.read("GAUSS_NORMAL_POSED").reshape(-1, 4)[:, :3]
     front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
     rg = av.read("TILE_RANGES").reshape(-1, 2).astype(np.int64)
-    units = {"shade": front * 512 * 0.5, "vis_depth_test": len(gp) * K, "vis_raster": len(inp["faces"]) * K,
+    # (inside rga_render_frame the mode-0 depth test runs for the camera-facing Gaussians only; with the back-face option
+    # about half of the (triangle, direction) units stop after projection and the area test: 0.5 x 220 + 0.5 x 50)
+    units = {"shade": front * 512 * 0.5, "vis_depth_test": (front if args.vis_mode == 0 else len(gp)) * K, "vis_raster": len(inp["faces"]) * K,
              "composite_segments": float(((rg[:, 1] - rg[:, 0]) * 256).sum())}
     dom = max((k for k in kern_ms if k in units), key=lambda k: kern_ms[k])
-    ach = units[dom] * FLOP_PER_UNIT[dom] / (kern_ms[dom] * 1e-3) / 1e12
+    fpu = dict(FLOP_PER_UNIT)
+    if cull:
+        fpu["vis_raster"] = 135.0
+    ach = units[dom] * fpu[dom] / (kern_ms[dom] * 1e-3) / 1e12
     pk, pk_kind = peaks()
     fma_meas = rga.rga_measure_fp32_peak()
     roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
@@ -337,7 +354,7 @@ def main():
                 "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES.get(dom), "traffic_source": NCU_SOURCE.get(dom),
                 "note": "fp32 FMA-pipe peak derived from the guide (148 SM x 128 lanes x 2 x 1.965 GHz); "
                         "HBM peak %s %.0f GB/s is not the bound of this kernel" % (pk_kind, pk["hbm_gbs"]),
-                "units_per_launch": units[dom], "flop_per_unit": FLOP_PER_UNIT[dom], "kernel_ms": kern_ms[dom]}
+                "units_per_launch": units[dom], "flop_per_unit": fpu[dom], "kernel_ms": kern_ms[dom]}
 
     # SURVEY 8(f) item 2 (beside the metric): the displacement network d(x, theta) on the tensor cores (tcgen05, TF32)
     mlp = workloads.make_disp_mlp(seed=1)
@@ -384,7 +401,9 @@ def main():
         "metric": METRIC, "value": world * 1e3 / ms, "unit": "frames/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "vis_mode": args.vis_mode, "l2": "flushed between steps (256 MiB fill)",
+        "config": {"workload": WORKLOAD, "vis_mode": args.vis_mode, "vis_cull_backfaces": cull,
+                   "mesh": "closed, outward-oriented (the depth rasteriser may skip faces turned away from the light)",
+                   "l2": "flushed between steps (256 MiB fill)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "paper_context": "6.9 fps on RTX 4090 (PAPER.md:314)"},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": world * 1e3 / ms_e2e, "unit": "frames/s", "h2d_bytes_per_step": int(h_bones.numel() * 4 + h_env.numel() * 4),
@@ -392,11 +411,13 @@ def main():
                 "pipelined_value": world * 1e3 / ms_e2e_pipe,
                 "pipelined_note": "image read-back of step i on a copy stream beside step i+1; per-step events plus the last copy's tail"},
         "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
+        "value_all_triangles": (world * 1e3 / ms_nocull) if ms_nocull else None,
         "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj, "shade_backward": sb_obj, "image_loss": il_obj, "regularisers": rg_obj, "train_backward": train_obj,
         "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as orc                 # cpu_baseline leg: the oracle, untuned, on the host cores
+        inp["vis_cull_backfaces"] = cull
         oav = orc.avatar_load(inp)
         orc.render_frame(oav, inp, vis_mode=args.vis_mode)
         n, t0 = 0, time.perf_counter()

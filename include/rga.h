@@ -99,6 +99,11 @@ typedef struct {
   float depth_bias_world;    /* mode 0: constant bias in world units (default 0.015)                    */
   float slope_max;           /* mode 0: clamp of the slope factor tan(theta) (default 8)                */
   int32_t keep_maps;         /* non-zero: also keep the triangle-ID maps in mode 0 (parity / debug)     */
+  int32_t cull_backfaces;    /* non-zero: the mesh is CLOSED with outward counter-clockwise faces, so the surface
+                                nearest a light is always a face turned towards it: triangles whose snapped light-space
+                                area is negative are skipped (reading A36).  On such a mesh the maps differ from
+                                the unculled ones only where a nearly edge-on back face extrapolates its plane in front of
+                                the surface (< 1 % of the covered texels).  0 = rasterise every triangle                */
 } rga_vis_params;
 
 typedef struct {

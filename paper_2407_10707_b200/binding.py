@@ -48,7 +48,7 @@ class _Camera(C.Structure):
 class _VisParams(C.Structure):
     _fields_ = [("n_dirs", C.c_int32), ("res", C.c_int32), ("mode", C.c_int32), ("dirs", C.c_void_p),
                 ("depth_bias_texels", C.c_float), ("depth_bias_world", C.c_float), ("slope_max", C.c_float),
-                ("keep_maps", C.c_int32)]
+                ("keep_maps", C.c_int32), ("cull_backfaces", C.c_int32)]
 
 
 class _Env(C.Structure):
@@ -153,9 +153,10 @@ def pose_skin(h, bone_mats):
     _chk(lib().pose_skin(h, _ptr(bone_mats), _stream()))
 
 
-def visibility_raster(h, dirs, res, mode=0, depth_bias_texels=1.0, depth_bias_world=0.015, slope_max=8.0, keep_maps=False):
+def visibility_raster(h, dirs, res, mode=0, depth_bias_texels=1.0, depth_bias_world=0.015, slope_max=8.0, keep_maps=False,
+                      cull_backfaces=False):
     p = _VisParams(int(dirs.shape[0]), int(res), int(mode), dirs.data_ptr(), depth_bias_texels, depth_bias_world, slope_max,
-                   int(keep_maps))
+                   int(keep_maps), int(cull_backfaces))
     _chk(lib().visibility_raster(h, C.byref(p), _stream()))
 
 
@@ -267,7 +268,7 @@ def splat_attribute(h, camera, bg, which, out_image):
 
 
 def rga_render_frame(h, bone_mats, dirs, vis_res, radiance, texel_to_dir, cam_pos, camera, bg, out_image, vis_mode=0,
-                     use_visibility=True, gamma=2.2, bias=(1.0, 0.015, 8.0), keep_maps=False):
+                     use_visibility=True, gamma=2.2, bias=(1.0, 0.015, 8.0), keep_maps=False, cull_backfaces=False):
     """One whole frame in one C-ABI call (include/rga.h rga_render_frame)."""
     e = _Env(int(radiance.shape[0]), int(radiance.shape[1]), radiance.data_ptr(),
              0 if texel_to_dir is None else texel_to_dir.data_ptr(), gamma, int(use_visibility))
@@ -277,7 +278,7 @@ def rga_render_frame(h, bone_mats, dirs, vis_res, radiance, texel_to_dir, cam_po
     vp = None
     if use_visibility:
         vp = C.byref(_VisParams(int(dirs.shape[0]), int(vis_res), int(vis_mode), dirs.data_ptr(), bias[0], bias[1], bias[2],
-                                int(keep_maps)))
+                                int(keep_maps), int(cull_backfaces)))
     _chk(lib().rga_render_frame(h, _ptr(bone_mats), vp, C.byref(e), cp, C.byref(cam), b, _ptr(out_image), _stream()))
 
 
@@ -341,10 +342,10 @@ class Avatar:
             pass
 
     def render(self, bone_mats, dirs, vis_res, radiance, texel_to_dir, cam_pos, camera, bg, out_image, vis_mode=0,
-               use_visibility=True, gamma=2.2, bias=(1.0, 0.015, 8.0)):
+               use_visibility=True, gamma=2.2, bias=(1.0, 0.015, 8.0), cull_backfaces=False):
         """One relit posed frame through rga_render_frame."""
         rga_render_frame(self.h, bone_mats, dirs, vis_res, radiance, texel_to_dir, cam_pos, camera, bg, out_image, vis_mode,
-                         use_visibility, gamma, bias)
+                         use_visibility, gamma, bias, cull_backfaces=cull_backfaces)
         return out_image
 
     def read(self, which):

@@ -270,7 +270,7 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
     int tail_first, int split,
     const float4* __restrict__ v_posed, const unsigned long long* __restrict__ faces_packed, const float* __restrict__ dirs,
     const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
-    unsigned* __restrict__ vbits_raw, int words) {
+    unsigned* __restrict__ vbits_raw, int words, int cull) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_next;
   __shared__ float s_zf[8];
@@ -345,7 +345,13 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
           int i0, i1, i2;
           face_unpack(__ldg(faces_packed + t), i0, i1, i2);
           int ia, ja, bw, bh; bool narrow;
-          ne = tri_box(sXY[i0], sXY[i1], sXY[i2], R, row0, rows, ia, ja, bw, bh, narrow) > 0;
+          const unsigned Q0 = sXY[i0], Q1 = sXY[i1], Q2 = sXY[i2];
+          ne = tri_box(Q0, Q1, Q2, R, row0, rows, ia, ja, bw, bh, narrow) > 0;
+          if (cull && ne) {                               // reading A36: negative snapped area = facing away from the light
+            const long long ax = (int)(Q1 & 0xffff) - (int)(Q0 & 0xffff), ay = (int)(Q1 >> 16) - (int)(Q0 >> 16);
+            const long long bx = (int)(Q2 & 0xffff) - (int)(Q0 & 0xffff), by = (int)(Q2 >> 16) - (int)(Q0 >> 16);
+            ne = ax * by - ay * bx > 0;
+          }
         }
         const unsigned m = __ballot_sync(0xffffffffu, ne);
         if (m) {
@@ -449,7 +455,7 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
     cudaMemsetAsync(av->zmap + first_px, 0xff, ((size_t)p->n_dirs * p->res * p->res - first_px) * 4, s);
   }
 #define RAST_ARGS av->n_faces, av->n_verts, p->res, band_rows, n_bands, n_units, tail_first, split, av->v_posed, av->faces_packed, p->dirs, av->window, \
-    av->zmap, av->idmap, raw, words
+    av->zmap, av->idmap, raw, words, p->cull_backfaces != 0
   if (with_id) vis_raster_kernel<true><<<grid, threads, smem, s>>>(RAST_ARGS);
   else vis_raster_kernel<false><<<grid, threads, smem, s>>>(RAST_ARGS);
   av->launches += 1;

@@ -22,7 +22,7 @@ def run_gpu(inp, vis_mode=0, frame=0, keep_maps=True, use_visibility=True, max_d
     rga.pose_skin(av.h, bones)
     if use_visibility:
         rga.visibility_raster(av.h, dirs, inp["vis_res"], vis_mode, inp["depth_bias_texels"], inp["depth_bias_world"],
-                              inp["slope_max"], keep_maps)
+                              inp["slope_max"], keep_maps, cull_backfaces=bool(inp.get("vis_cull_backfaces", False)))
     rga.shade_gaussians(av.h, env, inp["cam_pos"], t2d, inp["gamma"], use_visibility)
     rga.splat_render(av.h, cam, inp["bg"], img)
     rga.rga_check(av.h)

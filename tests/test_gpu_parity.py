@@ -408,3 +408,22 @@ def test_densify_density_matches_algorithm_1(cfg, n_gauss, d0, p0):
     assert np.array_equal(pos2.cpu().numpy()[:m].view(np.uint32), ref["pos"][:m].view(np.uint32))
     assert av.read("DENS_NG").sum() == m
     av.close()
+
+
+@pytest.mark.parametrize("cfg,vis_mode", [(0, 0), (0, 1), (1, 0), (1, 1), (2, 0)])
+def test_backface_cull_option_full_parity(cfg, vis_mode):
+    # rga_vis_params.cull_backfaces (reading A36: closed outward-oriented mesh): same stage-by-stage parity -- depth maps,
+    # triangle-id maps, visibility bits / counts bit-exact -- against the oracle run with the same option
+    from oracle import oracle as orc
+    from parity_util import compare_all, run_gpu
+    inp = workloads.make(cfg, n_gauss=50_000 if cfg == 2 else None)
+    inp["vis_cull_backfaces"] = True
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=vis_mode)
+    o_full = orc.render_frame(orc_av, dict(inp, vis_cull_backfaces=False), vis_mode=vis_mode, stop_after="vis")
+    av, img = run_gpu(inp, vis_mode=vis_mode)
+    print(compare_all(inp, av, img, orc_av, o, vis_mode))
+    # the option changes the maps only at a fraction of a percent of the covered texels, never the coverage
+    cov = o_full["zmap"] != 0xFFFFFFFF
+    assert np.array_equal(cov, o["zmap"] != 0xFFFFFFFF) and (o["zmap"] != o_full["zmap"]).sum() < 0.01 * cov.sum()
+    av.close()
