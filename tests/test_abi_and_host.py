@@ -30,7 +30,7 @@ def test_every_declared_symbol_is_exported(built_lib):
 def test_binding_struct_layouts_match_header(built_lib):
     from paper_2407_10707_b200 import binding as rga
     assert C.sizeof(rga._Camera) == 9 * 4 + 3 * 4 + 4 * 4 + 2 * 4 + 4
-    assert C.sizeof(rga._VisParams) == 40 and rga._VisParams.dirs.offset == 16
+    assert C.sizeof(rga._VisParams) == 48 and rga._VisParams.dirs.offset == 16 and rga._VisParams.cull_backfaces.offset == 40
     assert C.sizeof(rga._Env) == 32 and rga._Env.radiance.offset == 8
     assert rga._Desc.vert_pos.offset == 24 and rga._Desc.max_width.offset == 24 + 12 * 8
     assert C.sizeof(rga._Desc) == 24 + 12 * 8 + 5 * 4 + 4 + 8
