@@ -296,3 +296,90 @@ def test_training_backward_chain_matches_oracle_chain():
     for k, (emax, emean, scale) in rep.items():
         assert scale > 0 and emax < 1e-3 and emean < 1e-5, (k, emax, emean, scale)     # measured <= 4e-5 / 4.2e-7
     av.close()
+
+
+def _retarget(inp, W, H):
+    cam = dict(inp["camera"])
+    fy = np.float32(0.5 * H / np.tan(np.deg2rad(20.0)))
+    cam.update(width=W, height=H, fx=fy, fy=fy, cx=np.float32(W / 2), cy=np.float32(H / 2))
+    inp["camera"] = cam
+
+
+@pytest.mark.parametrize("n_gauss,W,H", [(777, 70, 50), (12_000, 16, 16), (1, 33, 17)])
+def test_backward_edge_shapes(n_gauss, W, H):
+    # ragged image (partial tile row and column) with a non-black background; ONE tile whose list has ~6k entries (about a
+    # hundred segments fold into each pixel's prefix); a single Gaussian.  Whole chain splat -> shade -> pose.
+    import torch
+    from oracle import backward as bwd
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import run_gpu
+    inp = workloads.make(0, n_gauss=n_gauss)
+    inp["bg"] = np.array([0.1, 0.2, 0.3], np.float32)
+    _retarget(inp, W, H)
+    cam = inp["camera"]
+    env = inp["env"][inp["env_of_frame"][0]]
+    N, nv, B = len(inp["gauss_pos"]), len(inp["vert_pos"]), inp["bone_mats"].shape[1]
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=0)
+    G = workloads.make_image_cotangent(n_gauss, W, H)
+    sp = bwd.splat_backward(o["gauss_posed"], o["cov6"], o["color"], inp["gauss_opacity"], cam, inp["bg"], o["vals"], o["ranges"], o["touched"], G,
+                            mu32=o["mu"], conic32=o["conic_o"])
+    v = bwd.texel_visibility(N, env.shape[0] * env.shape[1], inp["texel_to_dir"], 0, bits=o["visbits"])
+    sh = bwd.shade_backward(o["gauss_posed"], o["gauss_normal_posed"], orc_av["albedo_g"], orc_av["rough_g"], orc_av["spec_g"], inp["cam_pos"],
+                            env, v, inp["gamma"], sp["d_col"])
+    ref = bwd.pose_backward(inp, orc_av["knn_g"], orc_av["ubar_g"], 0, sp["d_x"] + sh["d_x"], sh["d_n"], sp["d_cov6"], sh["d_alb"], sh["d_rough"],
+                            sh["d_spec"])
+    dev = "cuda"
+    av, img = run_gpu(inp, vis_mode=0, keep_maps=False)
+    z = lambda *s: torch.zeros(s, device=dev)
+    img_d = torch.as_tensor(np.ascontiguousarray(img, np.float32)).to(dev)
+    d_col, d_op, d_mean, d_cov = z(N, 3), z(N), z(N, 3), z(N, 6)
+    rga.splat_backward(av.h, cam, inp["bg"], img_d, torch.as_tensor(G).to(dev), d_col, d_op, d_mean, d_cov)
+    s_out = dict(out_dalbedo=z(N, 3), out_drough=z(N), out_dspec=z(N), out_dnormal=z(N, 3), out_dpos=z(N, 3), out_denv=z(env.shape[0], env.shape[1], 3))
+    rga.shade_backward(av.h, torch.as_tensor(env).to(dev), inp["cam_pos"], d_col, texel_to_dir=torch.as_tensor(inp["texel_to_dir"]).to(dev),
+                       gamma=inp["gamma"], use_visibility=True, **s_out)
+    out = {"d_gauss_pos": z(N, 3), "d_gauss_quat": z(N, 4), "d_gauss_scale": z(N, 3), "d_bones": z(B, 12), "d_vert_disp": z(nv, 3),
+           "d_vert_normal": z(nv, 3), "d_vert_albedo": z(nv, 3), "d_vert_rough": z(nv), "d_vert_spec": z(nv)}
+    rga.pose_backward(av.h, torch.as_tensor(inp["bone_mats"][0]).to(dev),
+                      {"d_mean": d_mean, "d_mean2": s_out["out_dpos"], "d_normal": s_out["out_dnormal"], "d_cov": d_cov, "d_albedo": s_out["out_dalbedo"],
+                       "d_rough": s_out["out_drough"], "d_spec": s_out["out_dspec"]}, out)
+    rga.rga_check(av.h)
+    pairs = [("d_col", d_col, sp["d_col"]), ("d_opac", d_op, sp["d_opac"]), ("d_x", d_mean, sp["d_x"]), ("d_cov6", d_cov, sp["d_cov6"]),
+             ("d_env", s_out["out_denv"], sh["d_env"])] + [(k, t, ref[k]) for k, t in out.items()]
+    rep = {}
+    for k, t, r in pairs:
+        g = t.cpu().numpy(); r = np.asarray(r).reshape(g.shape)
+        assert np.isfinite(g).all(), k
+        scale = np.abs(r).max()
+        if scale == 0:                                                    # e.g. the single Gaussian faces away: everything is 0
+            assert not g.any(), k
+            continue
+        rep[k] = (float(np.abs(g - r).max() / scale), float(np.abs(g - r).mean() / scale))
+    print(n_gauss, rep)
+    for k, (emax, emean) in rep.items():
+        assert emax < 2e-3 and emean < 1e-4, (k, emax, emean)
+    av.close()
+
+
+def test_image_loss_tiny_images_and_argument_checks():
+    import torch
+    from oracle import backward as bwd
+    from paper_2407_10707_b200 import binding as rga
+    inp = workloads.make(0)
+    av = rga.Avatar(inp, max_width=64, max_height=64, max_vis_dirs=16, max_vis_res=32, max_env_texels=512)
+    for (W, H) in [(1, 1), (5, 3), (11, 11)]:                             # the window is wider than the image: all border
+        img, tgt = workloads.make_image_pair(W * 31 + H, W, H)
+        img[:] = np.clip(tgt + 0.1, 0, 1)                                # (the generator's black corner would cover a 1x1 image)
+        ref = bwd.image_loss(img, tgt, 0.2)
+        out = torch.zeros(3, device="cuda"); dI = torch.zeros((H, W, 3), device="cuda")
+        rga.image_loss(av.h, torch.as_tensor(img).cuda(), torch.as_tensor(tgt).cuda(), 0.2, out, dI)
+        rga.rga_check(av.h)
+        assert abs(out[0].item() - ref["loss"]) < 1e-5 * max(ref["loss"], 1e-3)
+        assert np.abs(dI.cpu().numpy() - ref["d_image"]).max() < 2e-4 * np.abs(ref["d_image"]).max()
+    big = torch.zeros((65, 64, 3), device="cuda")
+    with pytest.raises(RuntimeError):
+        rga.image_loss(av.h, big, big, 0.2)                              # larger than the avatar's max_height
+    with pytest.raises(RuntimeError):
+        rga.image_loss(av.h, big[:64], big[:64], 1.5)                    # lambda outside [0, 1]
+    av.close()
