@@ -13,6 +13,12 @@
  *                          visibility with the median/median/mean filters (mode 1, Eq.3-4)
  *   shade_gaussians    H5  Eq.2 with the Appendix-A BRDF, then gamma
  *   splat_render       H6-H10 back-face opacity kill and the 3DGS tile rasteriser
+ *   rga_render_frame   the four per-frame calls as one, independent stages overlapped on a second stream
+ *
+ * Beyond the per-frame path (each documented at its declaration): splat_attribute (albedo / normal maps), displacement_mlp
+ * (d(x, theta) on the tensor cores), gaussians_update (per-frame KNN + Eq.1 for moved Gaussians), densify_density
+ * (Algorithm 1), and the training side of one view: image_loss (Eq.5), regularisers (Eq.6-9), splat_backward,
+ * shade_backward, pose_backward (the backward of H10 + H6, of H5, and of H2 + Eq.1).
  *
  * Conventions
  *  - Every pointer marked "dev" is DEVICE memory owned by the caller (row-major, fp32 / int32); pointers marked "host"
