@@ -253,7 +253,7 @@ extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const 
   CU(rga_launch_tile_sort(av, cam, s));
   CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->color, out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
-  av->have_splat = 1;
+  av->have_splat = 1; av->splat_is_attr = 0;
   return RGA_OK;
 }
 
@@ -273,7 +273,7 @@ extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, v
 extern "C" rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* image, const float* dL_dimage,
                                      float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, void* stream) {
   if (!av || !cam || !bg || !image || !dL_dimage) return fail(RGA_ERR_INVALID_ARG, "splat_backward: null argument");
-  if (!av->have_splat) return fail(RGA_ERR_STATE, "splat_backward: call splat_render (or rga_render_frame) first");
+  if (!av->have_splat || av->splat_is_attr) return fail(RGA_ERR_STATE, "splat_backward: call splat_render (or rga_render_frame) first");
   if (cam->width != av->cam_w || cam->height != av->cam_h) return fail(RGA_ERR_INVALID_ARG, "splat_backward: not the camera of the last splat_render");
   cudaStream_t s = (cudaStream_t)stream;
   rga_prof_mark(av, "-", s);
@@ -374,7 +374,7 @@ extern "C" rga_status splat_attribute(rga_avatar* av, const rga_camera* cam, con
   CU(rga_launch_tile_sort(av, cam, s));
   CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->attr_color, out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
-  av->have_splat = 1;
+  av->have_splat = 1; av->splat_is_attr = 1;      // the blend state now belongs to the attribute map, not to the shaded frame
   return RGA_OK;
 }
 
@@ -436,7 +436,7 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   if (overlap) CU(cudaStreamWaitEvent(s, av->ev_join, 0));
   CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->color, out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
-  av->have_splat = 1;
+  av->have_splat = 1; av->splat_is_attr = 0;
   return RGA_OK;
 }
 

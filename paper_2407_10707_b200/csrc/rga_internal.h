@@ -86,7 +86,7 @@ struct rga_avatar {
   int* status;                 // sticky device status
   int sorted_buf;              // which of keys[]/vals[] holds the sorted result
   // state of the current pose
-  int have_skin, have_vis, have_shade, have_splat;
+  int have_skin, have_vis, have_shade, have_splat, splat_is_attr;
   int vis_mode, vis_dirs, vis_res, vis_words, keep_maps;
   int vis_culled; float vis_cull_cam[3];   // mode-0 bits were computed only for Gaussians facing this camera (rga_render_frame)
   int cam_w, cam_h;

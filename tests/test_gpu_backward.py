@@ -69,6 +69,18 @@ def test_splat_backward_argument_checks():
     G = torch.zeros((H, W, 3), device="cuda")
     with pytest.raises(RuntimeError):
         rga.splat_backward(av.h, cam, inp["bg"], G, G)                   # nothing rendered yet
+    # an attribute map overwrites the blend state of the shaded frame: its backward is refused until the frame is splatted again
+    rga.pose_skin(av.h, torch.as_tensor(inp["bone_mats"][0]).cuda())
+    rga.shade_gaussians(av.h, torch.as_tensor(inp["env"][0]).cuda(), inp["cam_pos"], None, inp["gamma"], False)
+    img = torch.zeros((H, W, 3), device="cuda")
+    rga.splat_render(av.h, cam, inp["bg"], img)
+    rga.splat_backward(av.h, cam, inp["bg"], img, G)
+    rga.splat_attribute(av.h, cam, inp["bg"], rga.RGA_ATTR_ALBEDO, img)
+    with pytest.raises(RuntimeError):
+        rga.splat_backward(av.h, cam, inp["bg"], img, G)
+    rga.splat_render(av.h, cam, inp["bg"], img)
+    rga.splat_backward(av.h, cam, inp["bg"], img, G)
+    rga.rga_check(av.h)
     av.close()
 
 
