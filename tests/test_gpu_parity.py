@@ -427,3 +427,27 @@ def test_backface_cull_option_full_parity(cfg, vis_mode):
     cov = o_full["zmap"] != 0xFFFFFFFF
     assert np.array_equal(cov, o["zmap"] != 0xFFFFFFFF) and (o["zmap"] != o_full["zmap"]).sum() < 0.01 * cov.sum()
     av.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_backface_cull_image_stays_within_tolerance_of_the_full_rasterisation(cfg):
+    # the option changes < 1 % of the depth texels (reading A36); the frame rendered WITH it still meets the north_star image
+    # tolerance against the oracle that rasterises every triangle, and only a handful of visibility bits differ
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import IMG_MAX, IMG_MEAN
+    inp = workloads.make(cfg)
+    cam = inp["camera"]; W, H = cam["width"], cam["height"]
+    o_full = orc.render_frame(orc.avatar_load(inp), inp, vis_mode=0)          # no culling anywhere
+    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=len(inp["vis_dirs"]), max_vis_res=inp["vis_res"],
+                    max_env_texels=inp["env_rows"] * inp["env_cols"])
+    img = torch.empty((H, W, 3), dtype=torch.float32, device="cuda")
+    av.render(torch.as_tensor(inp["bone_mats"][0]).cuda(), torch.as_tensor(inp["vis_dirs"]).cuda(), inp["vis_res"],
+              torch.as_tensor(inp["env"][0]).cuda(), torch.as_tensor(inp["texel_to_dir"]).cuda(), inp["cam_pos"], cam, inp["bg"], img,
+              vis_mode=0, gamma=inp["gamma"], bias=(inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"]), cull_backfaces=True)
+    rga.rga_check(av.h)
+    d = np.abs(img.cpu().numpy().astype(np.float64) - o_full["image"]).max(-1)
+    print(cfg, "image max / mean abs diff vs the unculled oracle:", d[o_full["flags"] == 0].max(), d.mean())
+    assert d[o_full["flags"] == 0].max() <= IMG_MAX and d.mean() <= IMG_MEAN
+    av.close()
