@@ -575,9 +575,9 @@ cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, c
   // directions are split over blockIdx.y so that small avatars still fill the machine (100k Gaussians alone give
   // 676 threads per SM); neighbouring threads stay neighbouring Gaussians, whose texel gathers coalesce in L1
   int words = (p->n_dirs + 31) / 32;
-  // (with the camera cull about half of the Gaussians retire at once: 16 parts keep enough warps in flight for the texel
-  // gathers -- 88 us with 4 parts, 73 us with 16 at config 1; without the cull 4 parts measured best)
-  const int maxparts = cull_cam ? 16 : 4;
+  // (16 parts keep enough warps in flight for the texel gathers: with rga_render_frame's camera cull, where about half of
+  // the Gaussians retire at once, 88 us with 4 parts and 73 us with 16 at config 1; without the cull 118 -> 108 us)
+  const int maxparts = 16;
   int parts = words < maxparts ? words : maxparts;
   int wpp = (words + parts - 1) / parts;
   parts = (words + wpp - 1) / wpp;
