@@ -56,7 +56,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
+  void* ptrs[] = {av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
                   av->vt_spec, av->knn_d2, av->grid_start, av->grid_verts, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
@@ -113,7 +113,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   float* d2 = nullptr;
 #define A(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, \
     "avatar_load: %s: %s", #call, cudaGetErrorString(e_)); goto done; } } while (0)
-  A(dalloc(&av->reg_sums, 4)); A(dalloc(&av->loss_maps, 9 * npix)); A(dalloc(&av->loss_sums, 2)); A(dalloc(&av->work_counter, 1)); A(dalloc(&av->splat_grad, 12 * ng)); A(dalloc(&av->dens_dv, nv)); A(dalloc(&av->dens_pfix, (size_t)av->n_faces)); A(dalloc(&av->dens_cdf, (size_t)av->n_faces));
+  A(dalloc(&av->reg_sums, 4)); A(dalloc(&av->loss_maps, 9 * npix)); A(dalloc(&av->loss_sums, 2)); A(dalloc(&av->work_counter, 1)); A(dalloc(&av->shade_counter, 1)); A(cudaMemsetAsync(av->shade_counter, 0, sizeof(unsigned), s)); A(dalloc(&av->splat_grad, 12 * ng)); A(dalloc(&av->dens_dv, nv)); A(dalloc(&av->dens_pfix, (size_t)av->n_faces)); A(dalloc(&av->dens_cdf, (size_t)av->n_faces));
   A(dalloc(&av->dens_ng, (size_t)av->n_faces)); A(dalloc(&av->dens_block, (size_t)av->n_faces / 2048 + 1)); A(dalloc(&av->dens_hdr, 2));
   A(dalloc(&av->v_pos, nv)); A(dalloc(&av->v_disp, nv)); A(dalloc(&av->g_pos, ng)); A(dalloc(&av->mlp_bias1, 256));
   A(dalloc(&av->v_xbar, nv)); A(dalloc(&av->v_normal, nv)); A(dalloc(&av->v_skin_w, nv * B)); A(dalloc(&av->faces, 3 * (size_t)av->n_faces)); A(dalloc(&av->faces_packed, (size_t)av->n_faces));

@@ -82,6 +82,7 @@ struct rga_avatar {
   int disp_is_mlp;             // the current displacement is displacement_mlp's v_disp (else the static vt_disp table)
   float* loss_maps; double* loss_sums;   // image_loss: [max_h][max_w][9] SSIM derivative maps, {sum SSIM, sum |I - J|}
   int* work_counter;           // [1] dynamic work distribution of persistent kernels (zeroed before the launch)
+  unsigned* shade_counter;     // [1] group tickets of shade_kernel (zero between launches: the last CTA re-arms it)
   float* splat_grad;           // [n_gauss][12] splat_backward: d_colour(3), d_opacity, d_mu(2), d_conic(3), pad
   int* status;                 // sticky device status
   int sorted_buf;              // which of keys[]/vals[] holds the sorted result
