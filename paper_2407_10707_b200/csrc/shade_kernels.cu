@@ -2,9 +2,9 @@
 // FAST file (default FMA contraction, MUFU intrinsics): the result is compared with the fp64 oracle under the
 // north_star tolerance (2e-3 max-abs on colour), not bit-exactly.
 //
-// Layout: LANES threads cooperate on one Gaussian; each walks a strided subset of the environment texels.  The env
-// table (w_k, L_k A_k) is staged in shared memory once per CTA; visibility comes as bits (mode 0), as vertex counts
-// gathered through S_g (mode 1) or is 1 (mode 2).
+// Layout: persistent CTAs draw groups of consecutive Gaussians from a ticket counter; one Gaussian per lane, the texel
+// warp-uniform (see the comment above shade_kernel).  The env table (w_k, L_k A_k) is staged in shared memory once per
+// CTA; visibility comes as bits (mode 0), as vertex counts gathered through S_g (mode 1) or is 1 (mode 2).
 #include "rga_internal.h"
 
 #define PI_F 3.14159265358979323846f
@@ -44,9 +44,13 @@ __device__ __forceinline__ float ex2_approx(float x) { float r; asm("ex2.approx.
 // (w_i.n <= 0, visibility bit clear) mostly agree across the warp: a texel that no lane needs costs the test only
 // (the first version gave four lanes to a Gaussian and every lane its own texel, so a warp ran the BRDF block in nearly
 // every trip with half of its lanes idle: 67 us at config 1).  Slice partials are folded in slice order in shared memory.
+#ifndef SH_THREADS
 #define SH_THREADS 256
+#endif
 #define SH_WARPS (SH_THREADS / 32)
+#ifndef SH_GROUP
 #define SH_GROUP 64
+#endif
 
 template <int MODE>
 __global__ void __launch_bounds__(SH_THREADS) shade_kernel(int ng, int ne, int K, int words, int Kg, int Kv,

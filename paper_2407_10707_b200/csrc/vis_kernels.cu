@@ -468,7 +468,12 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
 // directions; neighbouring (Morton-ordered) Gaussians hit neighbouring texels, so the depth-map gathers stay in
 // L1/L2.  32 directions are packed into one output word.  The slope factor tau (sqrt and divide) is only evaluated when
 // the two monotone bounds beta(1) <= beta(tau) <= beta(slope_max) do not already decide the comparison.
+#ifndef DT_THREADS
 #define DT_THREADS 128
+#endif
+#ifndef DT_MAXPARTS
+#define DT_MAXPARTS 16
+#endif
 __global__ void __launch_bounds__(DT_THREADS) vis_depth_test_kernel(int ng, int K, int R, const float4* __restrict__ g_posed,
     const float4* __restrict__ g_nposed, const float* __restrict__ dirs, const float* __restrict__ window,
     const unsigned* __restrict__ zmap, float bias_texels, float bias_world, float slope_max, int words_per_part,
@@ -577,7 +582,7 @@ cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, c
   int words = (p->n_dirs + 31) / 32;
   // (16 parts keep enough warps in flight for the texel gathers: with rga_render_frame's camera cull, where about half of
   // the Gaussians retire at once, 88 us with 4 parts and 73 us with 16 at config 1; without the cull 118 -> 108 us)
-  const int maxparts = 16;
+  const int maxparts = DT_MAXPARTS;
   int parts = words < maxparts ? words : maxparts;
   int wpp = (words + parts - 1) / parts;
   parts = (words + wpp - 1) / wpp;
