@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(BB) composite_backward_kernel(int W, int H, in
         if (fabsf(mm.x - bcx) > ex.x + 3.5f || fabsf(mm.y - bcy) > ex.y + 1.5f) continue;
         const float4 co = st.co[j];
         const float dx = mm.x - fx, dy = mm.y - fy;
-        const float p2 = dx * (co.x * dx + co.y * dy) + co.z * dy * dy;   // log2(e) * power, as in the forward
+        const float p2 = fmaf(dx, fmaf(co.x, dx, co.y * dy), (co.z * dy) * dy);   // log2(e) * power, rounded as in the forward's seg_alpha
         const float raw = co.w * bex2_approx(p2);
         const float a = fminf(0.99f, raw);
         const bool valid = (b0 + j < last) && !(p2 > 0.f || a < 1.f / 255.f);

@@ -156,7 +156,8 @@ __device__ __forceinline__ void stage_segment(SegStage& st, int m, const unsigne
 __device__ __forceinline__ float seg_alpha(const SegStage& st, int j, float fx, float fy) {
   const float2 mm = st.mu[j]; const float4 co = st.co[j];
   const float dx = mm.x - fx, dy = mm.y - fy;
-  const float p2 = dx * (co.x * dx + co.y * dy) + co.z * dy * dy;        // log2(e) * power
+  // log2(e) * power; the contraction is written out so that every inlined copy rounds alike (the replay evaluates an alpha twice)
+  const float p2 = fmaf(dx, fmaf(co.x, dx, co.y * dy), (co.z * dy) * dy);
   const float al = fminf(0.99f, co.w * ex2_approx(p2));
   return (p2 > 0.f || al < 1.f / 255.f) ? 0.f : al;
 }
@@ -270,6 +271,7 @@ __global__ void __launch_bounds__(CB) composite_replay_kernel(int W, int H, int 
   __shared__ SegStage st;
   __shared__ int s_cnt;
   __shared__ unsigned short s_pix[CB];
+  __shared__ unsigned s_mask[CB][RGA_SEG / 32];
   const unsigned n_items = *num_items;
   for (unsigned item = blockIdx.x; item < n_items; item += gridDim.x) {
     if (!item_flag[item]) continue;                        // block-uniform
@@ -289,29 +291,52 @@ __global__ void __launch_bounds__(CB) composite_replay_kernel(int W, int H, int 
       if (qx < W && qy < H && stop_seg[(size_t)qy * W + qx] == seg) s_pix[atomicAdd(&s_cnt, 1)] = (unsigned short)threadIdx.x;
     }
     __syncthreads();
-    if ((int)threadIdx.x >= s_cnt) continue;
+    // few pixels replay, so latency rules.  Phase 1, all warps: a warp takes one stopping pixel at a time and evaluates the
+    // segment's entries one per lane; the ballot of alpha > 0 is the pixel's list of contributing entries (about one in
+    // eight).  Phase 2, one thread per pixel: the sequential rule over the set bits only, four alphas per trip (the same
+    // seg_alpha on the same operands, so the same values as in phase 1).
+    const int cnt = s_cnt;
+    const int tx0 = (int)(tile % TX) * RGA_TILE, ty0 = (int)(tile / TX) * RGA_TILE;
+    for (int i = (int)(threadIdx.x >> 5); i < cnt; i += CB / 32) {
+      const unsigned qq = s_pix[i];
+      const float gx = (float)(tx0 + tile_px(qq)) + 0.5f, gy = (float)(ty0 + tile_py(qq)) + 0.5f;
+#pragma unroll
+      for (int h = 0; h < RGA_SEG / 32; ++h) {
+        const int j = h * 32 + (int)(threadIdx.x & 31u);
+        const float a = j < m ? seg_alpha(st, j, gx, gy) : 0.f;
+        const unsigned mk = __ballot_sync(0xffffffffu, a > 0.f);
+        if ((threadIdx.x & 31u) == 0) s_mask[i][h] = mk;
+      }
+    }
+    __syncthreads();
+    if ((int)threadIdx.x >= cnt) continue;
     const unsigned q = s_pix[threadIdx.x];
-    const int px = (int)(tile % TX) * RGA_TILE + tile_px(q), py = (int)(tile / TX) * RGA_TILE + tile_py(q);
+    const int px = tx0 + tile_px(q), py = ty0 + tile_py(q);
     const size_t p = (size_t)py * W + px;
     const float fx = (float)px + 0.5f, fy = (float)py + 0.5f;
     float T = t_final[p], C0 = image[3 * p], C1 = image[3 * p + 1], C2 = image[3 * p + 2];
     unsigned last = n_contrib[p];
     bool done = false;
-    // few threads replay, so latency rules: eight independent alphas per trip, then the short sequential blend
-    for (int j0 = 0; j0 < m && !done; j0 += 8) {
-      float a[8];
 #pragma unroll
-      for (int u = 0; u < 8; ++u) a[u] = (j0 + u < m) ? seg_alpha(st, j0 + u, fx, fy) : 0.f;
+    for (int h = 0; h < RGA_SEG / 32; ++h) {
+      unsigned mk = s_mask[threadIdx.x][h];
+      while (mk != 0u && !done) {
+        int jj[4]; float a[4];
 #pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        if (!done && a[u] > 0.f) {
-          const float test_T = T * (1.f - a[u]);
-          if (test_T < 1e-4f) done = true;
-          else {
-            const float4 c = st.col[j0 + u];
-            const float w = a[u] * T;
-            C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
-            T = test_T; last = (unsigned)(seg * RGA_SEG + j0 + u + 1);
+        for (int u = 0; u < 4; ++u) { jj[u] = mk ? h * 32 + __ffs((int)mk) - 1 : -1; mk &= mk - 1u; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) a[u] = jj[u] >= 0 ? seg_alpha(st, jj[u], fx, fy) : 0.f;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (!done && a[u] > 0.f) {
+            const float test_T = T * (1.f - a[u]);
+            if (test_T < 1e-4f) done = true;
+            else {
+              const float4 c = st.col[jj[u]];
+              const float w = a[u] * T;
+              C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+              T = test_T; last = (unsigned)(seg * RGA_SEG + jj[u] + 1);
+            }
           }
         }
       }
