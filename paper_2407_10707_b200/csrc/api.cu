@@ -120,7 +120,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->knn_v, nv * av->k_v)); A(dalloc(&av->knn_g, ng * av->k_g)); A(dalloc(&av->ubar_g, ng * av->k_g));
   A(dalloc(&av->g_static, 4 * ng)); A(dalloc(&av->g_skin_w, ng * B)); A(dalloc(&av->g_quat, ng)); A(dalloc(&av->g_scale_op, ng));
   A(dalloc(&av->v_posed, nv)); A(dalloc(&av->v_nposed, nv)); A(dalloc(&av->g_posed, ng)); A(dalloc(&av->g_nposed, ng));
-  A(dalloc(&av->g_cov, 6 * ng)); A(dalloc(&av->window, 4)); A(dalloc(&av->aabb, 6));
+  A(dalloc(&av->g_cov, 6 * ng)); A(dalloc(&av->window, 4)); A(dalloc(&av->aabb, 8));
   A(dalloc(&av->zmap, nmap)); A(dalloc(&av->idmap, nmap)); A(dalloc(&av->visbits, ng * words));
   A(dalloc(&av->vbits_a, nv * words)); A(dalloc(&av->vbits_b, nv * words)); A(dalloc(&av->vbits_raw, nv * words));
   A(dalloc(&av->vcount, nv * (size_t)av->max_dirs + 32)); A(dalloc(&av->env_table, 8 * (size_t)av->max_env));
@@ -143,7 +143,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(cudaEventCreateWithFlags(&av->ev_join, cudaEventDisableTiming));
   A(cudaMemsetAsync(av->status, 0, sizeof(int), s)); A(cudaMemsetAsync(av->num_dup, 0, sizeof(unsigned), s));
   {
-    unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
+    unsigned init[8] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u, 0u, 0u};   // [6] = skin_kernel's block counter
     A(cudaMemcpyAsync(av->aabb, init, sizeof init, cudaMemcpyHostToDevice, s));
     A(cudaStreamSynchronize(s));
   }

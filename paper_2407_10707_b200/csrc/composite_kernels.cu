@@ -21,6 +21,12 @@
 #include "rga_internal.h"
 
 #define CB 256
+#ifndef REPLAY_GRID_MULT
+#define REPLAY_GRID_MULT 16
+#endif
+#ifndef SEGMENT_GRID_MULT
+#define SEGMENT_GRID_MULT 8
+#endif
 #define SCAP_SMALL RGA_SORT_SMALL
 #define SCAP_LARGE 24576
 #define LOG2E_F 1.4426950408889634f
@@ -399,13 +405,13 @@ cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStre
 // H10: blend (needs the sorted lists and the shaded colours)
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, const float4* color, float* out, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
-  composite_segment_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
+  composite_segment_kernel<<<av->num_sms * SEGMENT_GRID_MULT, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
       av->ranges, av->vals[0], av->mu2d, av->conic_o, color, av->part, av->part_last);
   rga_prof_mark(av, "composite_segments", s);
   composite_resolve_kernel<<<dim3(TX, TY), CB, 0, s>>>(cam->width, cam->height, TX, (unsigned)av->max_dup, av->ranges, av->seg_off,
       av->part, av->part_last, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
   rga_prof_mark(av, "composite_resolve", s);
-  composite_replay_kernel<<<av->num_sms * 8, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
+  composite_replay_kernel<<<av->num_sms * REPLAY_GRID_MULT, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
       av->ranges, av->vals[0], av->mu2d, av->conic_o, color, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
   rga_prof_mark(av, "composite_replay", s);
   av->launches += 3;

@@ -47,7 +47,7 @@ struct rga_avatar {
   float4* g_nposed;    // [n_gauss]
   float* g_cov;        // [n_gauss][6]
   float* window;       // [4] centre, radius; [4..9] scratch AABB as ordered ints
-  unsigned* aabb;      // [6] ordered-uint min xyz, max xyz
+  unsigned* aabb;      // [8] ordered-uint min xyz, max xyz; [6] counts skin_kernel's finished vertex blocks
   // visibility
   unsigned* zmap;      // [max_dirs][res*res]
   int* idmap;          // [max_dirs][res*res]  (allocated lazily at load: always, sized like zmap)

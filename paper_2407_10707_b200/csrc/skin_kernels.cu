@@ -36,12 +36,23 @@ __device__ __forceinline__ void blend(const float* __restrict__ w, int B, const 
   }
 }
 
+// window = bounding sphere of the posed AABB, radius padded by 1/64; then re-arm the AABB for the next pose.  Run by one
+// thread of the last vertex block of skin_kernel; the AABB words were written by atomics, so they are read past L1.
+__device__ __forceinline__ void window_from_aabb(unsigned* aabb, float* window) {
+  float mn[3], mx[3], dg[3];
+  for (int c = 0; c < 3; ++c) { mn[c] = ord2f(__ldcg(aabb + c)); mx[c] = ord2f(__ldcg(aabb + 3 + c)); }
+  for (int c = 0; c < 3; ++c) { window[c] = (mn[c] + mx[c]) * 0.5f; dg[c] = mx[c] - mn[c]; }
+  float rr = (0.5f * sqrtf((dg[0] * dg[0] + dg[1] * dg[1]) + dg[2] * dg[2])) * 1.015625f;
+  window[3] = (rr > 0.f) ? rr : 1.0f;
+  for (int c = 0; c < 3; ++c) { aabb[c] = 0xffffffffu; aabb[3 + c] = 0u; }
+}
+
 __global__ void __launch_bounds__(256) skin_kernel(int nv, int ng, int B, int vblocks, int block_base, const float* __restrict__ bone,
     const float4* __restrict__ v_xbar, const float4* __restrict__ v_n, const float* __restrict__ v_w,
     const float4* __restrict__ g_static, const float* __restrict__ g_w, const float4* __restrict__ g_quat,
     const float4* __restrict__ g_scale_op,
     float4* __restrict__ v_posed, float4* __restrict__ v_nposed, float4* __restrict__ g_posed, float4* __restrict__ g_nposed,
-    float* __restrict__ g_cov, unsigned* __restrict__ aabb) {
+    float* __restrict__ g_cov, unsigned* __restrict__ aabb, float* __restrict__ window) {
   extern __shared__ float sG[];
   for (int t = threadIdx.x; t < B * 12; t += blockDim.x) sG[t] = bone[t];
   __syncthreads();
@@ -106,17 +117,19 @@ __global__ void __launch_bounds__(256) skin_kernel(int nv, int ng, int B, int vb
     if ((threadIdx.x & 31) == 0)
 #pragma unroll
       for (int c = 0; c < 3; ++c) { atomicMin(aabb + c, f2ord(mn[c])); atomicMax(aabb + 3 + c, f2ord(mx[c])); }
+    // the vertex block that finishes last turns the AABB into the rasteriser's window (c, r) and re-arms the AABB and the
+    // block counter aabb[6] for the next pose (this was a one-thread kernel of its own on the frame's critical path)
+    __shared__ bool s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(aabb + 6, 1u) == (unsigned)(vblocks - 1);
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+      __threadfence();
+      window_from_aabb(aabb, window);
+      aabb[6] = 0u;
+    }
   }
-}
-
-// window = bounding sphere of the posed AABB, radius padded by 1/64; then re-arm the AABB for the next pose.
-__global__ void window_kernel(unsigned* aabb, float* window) {
-  float mn[3], mx[3], dg[3];
-  for (int c = 0; c < 3; ++c) { mn[c] = ord2f(aabb[c]); mx[c] = ord2f(aabb[3 + c]); }
-  for (int c = 0; c < 3; ++c) { window[c] = (mn[c] + mx[c]) * 0.5f; dg[c] = mx[c] - mn[c]; }
-  float rr = (0.5f * sqrtf((dg[0] * dg[0] + dg[1] * dg[1]) + dg[2] * dg[2])) * 1.015625f;
-  window[3] = (rr > 0.f) ? rr : 1.0f;
-  for (int c = 0; c < 3; ++c) { aabb[c] = 0xffffffffu; aabb[3 + c] = 0u; }
 }
 
 // which: 0 = mesh and Gaussians (pose_skin), 1 = mesh + window only, 2 = Gaussians only.  rga_render_frame issues 1 on
@@ -126,13 +139,8 @@ cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, int which, c
   const int base = which == 2 ? vblocks : 0, nblocks = which == 0 ? vblocks + gblocks : (which == 1 ? vblocks : gblocks);
   skin_kernel<<<nblocks, 256, av->n_bones * 12 * sizeof(float), s>>>(
       av->n_verts, av->n_gauss, av->n_bones, vblocks, base, bone_mats, av->v_xbar, av->v_normal, av->v_skin_w, av->g_static,
-      av->g_skin_w, av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->aabb);
+      av->g_skin_w, av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->aabb, av->window);
   rga_prof_mark(av, which == 2 ? "skin_gauss" : (which == 1 ? "skin_mesh" : "skin"), s);
   av->launches += 1;
-  if (which != 2) {
-    window_kernel<<<1, 1, 0, s>>>(av->aabb, av->window);
-    rga_prof_mark(av, "window", s);
-    av->launches += 1;
-  }
   return cudaGetLastError();
 }
