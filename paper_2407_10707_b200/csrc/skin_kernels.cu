@@ -47,7 +47,10 @@ __device__ __forceinline__ void window_from_aabb(unsigned* aabb, float* window) 
   for (int c = 0; c < 3; ++c) { aabb[c] = 0xffffffffu; aabb[3 + c] = 0u; }
 }
 
-__global__ void __launch_bounds__(256) skin_kernel(int nv, int ng, int B, int vblocks, int block_base, const float* __restrict__ bone,
+#ifndef SKIN_THREADS
+#define SKIN_THREADS 256
+#endif
+__global__ void __launch_bounds__(SKIN_THREADS) skin_kernel(int nv, int ng, int B, int vblocks, int block_base, const float* __restrict__ bone,
     const float4* __restrict__ v_xbar, const float4* __restrict__ v_n, const float* __restrict__ v_w,
     const float4* __restrict__ g_static, const float* __restrict__ g_w, const float4* __restrict__ g_quat,
     const float4* __restrict__ g_scale_op,
@@ -135,9 +138,9 @@ __global__ void __launch_bounds__(256) skin_kernel(int nv, int ng, int B, int vb
 // which: 0 = mesh and Gaussians (pose_skin), 1 = mesh + window only, 2 = Gaussians only.  rga_render_frame issues 1 on
 // the main stream (the rasteriser needs nothing else) and 2 on the second stream.
 cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, int which, cudaStream_t s) {
-  const int vblocks = (av->n_verts + 255) / 256, gblocks = (av->n_gauss + 255) / 256;
+  const int vblocks = (av->n_verts + SKIN_THREADS - 1) / SKIN_THREADS, gblocks = (av->n_gauss + SKIN_THREADS - 1) / SKIN_THREADS;
   const int base = which == 2 ? vblocks : 0, nblocks = which == 0 ? vblocks + gblocks : (which == 1 ? vblocks : gblocks);
-  skin_kernel<<<nblocks, 256, av->n_bones * 12 * sizeof(float), s>>>(
+  skin_kernel<<<nblocks, SKIN_THREADS, av->n_bones * 12 * sizeof(float), s>>>(
       av->n_verts, av->n_gauss, av->n_bones, vblocks, base, bone_mats, av->v_xbar, av->v_normal, av->v_skin_w, av->g_static,
       av->g_skin_w, av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->aabb, av->window);
   rga_prof_mark(av, which == 2 ? "skin_gauss" : (which == 1 ? "skin_mesh" : "skin"), s);

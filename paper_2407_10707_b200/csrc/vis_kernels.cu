@@ -80,6 +80,9 @@ cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s) {
 
 // Per-warp working set in shared memory
 #define RAST_Q 64              // queue entries: < 32 left over + <= 32 pushed
+#ifndef RAST_FETCH
+#define RAST_FETCH 32           // triangles a warp draws from the unit's counter at a time
+#endif
 #define RAST_SEGW 4            // a sampling unit is a run of up to 4 pixel centres of one box row
 struct RasterWarp {
   uint4 tab[4][32];            // round table (component-major: lanes read neighbouring owners without bank conflicts):
@@ -334,11 +337,11 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
     int qn = 0, q2n = 0;                                    // warp-uniform queue fills
     for (;;) {
       int base4 = 0;
-      if (lane == 0) base4 = atomicAdd(&s_next, 128);          // four batches per fetch
+      if (lane == 0) base4 = atomicAdd(&s_next, RAST_FETCH);   // RAST_FETCH / 32 batches per fetch
       base4 = __shfl_sync(0xffffffffu, base4, 0);
       if (base4 >= t_end) break;
 #pragma unroll 1
-      for (int base = base4; base < min(base4 + 128, t_end); base += 32) {
+      for (int base = base4; base < min(base4 + RAST_FETCH, t_end); base += 32) {
         const int t = base + lane;
         bool ne = false;
         if (t < t_end) {
