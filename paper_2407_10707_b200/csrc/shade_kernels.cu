@@ -44,6 +44,11 @@ __device__ __forceinline__ float ex2_approx(float x) { float r; asm("ex2.approx.
 // (w_i.n <= 0, visibility bit clear) mostly agree across the warp: a texel that no lane needs costs the test only
 // (the first version gave four lanes to a Gaussian and every lane its own texel, so a warp ran the BRDF block in nearly
 // every trip with half of its lanes idle: 67 us at config 1).  Slice partials are folded in slice order in shared memory.
+#ifndef SH_UNROLL
+#define SH_UNROLL 8
+#endif
+#define RGA_STR(x) #x
+#define RGA_UNROLL(n) _Pragma(RGA_STR(unroll n))
 #ifndef SH_THREADS
 #define SH_THREADS 256
 #endif
@@ -146,7 +151,7 @@ __global__ void __launch_bounds__(SH_THREADS) shade_kernel(int ng, int ne, int K
         if (!valid) vm = 0u;
         if (!__any_sync(0xffffffffu, vm != 0u)) continue;
         const float4* sEk = sE + 2 * kb;
-#pragma unroll 4
+        RGA_UNROLL(SH_UNROLL)
         for (int j = 0; j < kn; ++j) {
           const float4 wi = sEk[2 * j];
           const float cs = n.x * wi.x + n.y * wi.y + n.z * wi.z;

@@ -83,7 +83,9 @@ cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s) {
 #ifndef RAST_FETCH
 #define RAST_FETCH 32           // triangles a warp draws from the unit's counter at a time
 #endif
+#ifndef RAST_SEGW
 #define RAST_SEGW 4            // a sampling unit is a run of up to 4 pixel centres of one box row
+#endif
 struct RasterWarp {
   uint4 tab[4][32];            // round table (component-major: lanes read neighbouring owners without bank conflicts):
                                // edge-function coefficients and box of the 32 triangles being sampled
@@ -474,6 +476,11 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
 #ifndef DT_THREADS
 #define DT_THREADS 128
 #endif
+#ifndef DT_UNROLL
+#define DT_UNROLL 4
+#endif
+#define RGA_STR(x) #x
+#define RGA_UNROLL(n) _Pragma(RGA_STR(unroll n))
 #ifndef DT_MAXPARTS
 #define DT_MAXPARTS 16
 #endif
@@ -535,7 +542,7 @@ __global__ void __launch_bounds__(DT_THREADS) vis_depth_test_kernel(int ng, int 
     const int kend = min(32, K - wd * 32);
     const unsigned* zk = zmap + (size_t)wd * 32 * RR;
     const float4* fk = sF4 + 3 * (wd * 32 - k0);
-#pragma unroll 4
+    RGA_UNROLL(DT_UNROLL)
     for (int b = 0; b < kend; ++b) {
       const float4 fu = fk[3 * b], fv = fk[3 * b + 1], fw = fk[3 * b + 2];
       const float px = __fmaf_rn(fu.z, dz, __fmaf_rn(fu.y, dy, __fmaf_rn(fu.x, dx, W.hR)));
