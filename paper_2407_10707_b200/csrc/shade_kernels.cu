@@ -4,7 +4,8 @@
 //
 // Layout: persistent CTAs draw groups of consecutive Gaussians from a ticket counter; one Gaussian per lane, the texel
 // warp-uniform (see the comment above shade_kernel).  The env table (w_k, L_k A_k) is staged in shared memory once per
-// CTA; visibility comes as bits (mode 0), as vertex counts gathered through S_g (mode 1) or is 1 (mode 2).
+// CTA; visibility comes as bits (mode 0) or is 1 (mode 2).  Paper mode (mode 1: vertex counts gathered through S_g) runs
+// shade_paper_kernel below, with several lanes per Gaussian.
 #include "rga_internal.h"
 
 #define PI_F 3.14159265358979323846f
@@ -124,13 +125,6 @@ __global__ void __launch_bounds__(SH_THREADS) shade_kernel(int ng, int ne, int K
       // (the direct form 1 - nh^2 cancels badly for alpha^2 ~ 1e-4); this is w_o's
       const float tox = fmaf(-nwo_raw, n.x, wox), toy = fmaf(-nwo_raw, n.y, woy), toz = fmaf(-nwo_raw, n.z, woz);
       const float cS = al2 / (4.f * PI_F * go);                          // D F G /(4 ni no) = cS F / (den^2 gi)
-      float u0 = 0.f, u1 = 0.f, u2 = 0.f; int j0 = 0, j1 = 0, j2 = 0;
-      if (MODE == 1) {
-        const float ikv = 1.0f / (float)Kv;
-        j0 = knn_g[(size_t)g * Kg]; u0 = ubar_g[(size_t)g * Kg] * ikv;
-        if (Kg > 1) { j1 = knn_g[(size_t)g * Kg + 1]; u1 = ubar_g[(size_t)g * Kg + 1] * ikv; }
-        if (Kg > 2) { j2 = knn_g[(size_t)g * Kg + 2]; u2 = ubar_g[(size_t)g * Kg + 2] * ikv; }
-      }
       const unsigned* vb = visbits + (size_t)g * words;
       float d0 = 0.f, d1 = 0.f, d2 = 0.f, s0 = 0.f, s1 = 0.f, s2 = 0.f;
       for (int blk = warp; blk < nblk; blk += SH_WARPS) {
@@ -156,16 +150,6 @@ __global__ void __launch_bounds__(SH_THREADS) shade_kernel(int ng, int ne, int K
           const float4 wi = sEk[2 * j];
           const float cs = n.x * wi.x + n.y * wi.y + n.z * wi.z;
           bool live = (cs > 0.f) && ((vm >> j) & 1u);                    // max(0, w_i . n) and the visibility bit
-          float v = 1.f;
-          if (MODE == 1) {
-            if (live) {
-              const int d = sD[kb + j];
-              v = u0 * (float)__ldg(vcount + (size_t)j0 * K + d);
-              if (Kg > 1) v += u1 * (float)__ldg(vcount + (size_t)j1 * K + d);
-              if (Kg > 2) v += u2 * (float)__ldg(vcount + (size_t)j2 * K + d);
-              live = v != 0.f;
-            }
-          }
           if (!__any_sync(0xffffffffu, live)) continue;
           if (live) {
             const float4 LA = sEk[2 * j + 1];
@@ -179,7 +163,7 @@ __global__ void __launch_bounds__(SH_THREADS) shade_kernel(int ng, int ne, int K
             const float F = fmaf(0.96f, ex2_approx((-5.55473f * oh - 6.98316f) * oh), 0.04f);     // Eq.14
             const float gi = fmaf(cs, omk, kk);
             const float sp = cS * F * rcp_approx(den * den * gi);
-            const float w = v * cs;
+            const float w = cs;                                          // visibility is the mask (modes 0, 2)
             const float ws = w * sp;
             d0 = fmaf(LA.x, w, d0); d1 = fmaf(LA.y, w, d1); d2 = fmaf(LA.z, w, d2);
             s0 = fmaf(LA.x, ws, s0); s1 = fmaf(LA.y, ws, s1); s2 = fmaf(LA.z, ws, s2);
