@@ -54,12 +54,15 @@ __device__ __forceinline__ float ex2_approx(float x) { float r; asm("ex2.approx.
 #define SH_THREADS 256
 #endif
 #define SH_WARPS (SH_THREADS / 32)
+#ifndef SH_MINB
+#define SH_MINB 1             // minimum resident CTAs per SM asked of the compiler (register cap)
+#endif
 #ifndef SH_GROUP
-#define SH_GROUP 64
+#define SH_GROUP 32
 #endif
 
 template <int MODE>
-__global__ void __launch_bounds__(SH_THREADS) shade_kernel(int ng, int ne, int K, int words, int Kg, int Kv,
+__global__ void __launch_bounds__(SH_THREADS, SH_MINB) shade_kernel(int ng, int ne, int K, int words, int Kg, int Kv,
     const float4* __restrict__ g_posed, const float4* __restrict__ g_nposed, const float4* __restrict__ g_static,
     const float* __restrict__ env_table, const int* __restrict__ t2d, const unsigned* __restrict__ visbits,
     const unsigned char* __restrict__ vcount, const int* __restrict__ knn_g, const float* __restrict__ ubar_g,
