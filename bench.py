@@ -28,7 +28,7 @@ WORKLOAD = "configs[1] SMPL-sized: 6,890 v / 13,776 f / 24 bones, 100k Gaussians
 # algorithmic work per unit of each kernel (fp32 flop, FMA = 2)
 FLOP_PER_UNIT = {"shade": 70.0, "vis_depth_test": 40.0, "vis_raster": 220.0, "composite_segments": 30.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
-NCU_DRAM_BYTES = {"vis_raster": 810496, "vis_depth_test": 13461248, "shade": 9607168, "composite_segments": 2555648}
+NCU_DRAM_BYTES = {"vis_raster": 807680, "vis_depth_test": 13460736, "shade": 9606400, "composite_segments": 2554368}
 NCU_SOURCE = {k: "profiles/r01m_full.md" for k in NCU_DRAM_BYTES}
 FP32_PEAK_TFLOPS = 2 * 128 * 148 * 1.965e9 / 1e12          # 74.4: 148 SMs x 128 FP32 lanes x FMA x 1.965 GHz (guide)
 
