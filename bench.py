@@ -30,6 +30,9 @@ FLOP_PER_UNIT = {"shade": 70.0, "vis_depth_test": 40.0, "vis_raster": 220.0, "co
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
 NCU_DRAM_BYTES = {"vis_raster": 807680, "vis_depth_test": 13460736, "shade": 9606400, "composite_segments": 2554368}
 NCU_SOURCE = {k: "profiles/r01m_full.md" for k in NCU_DRAM_BYTES}
+# executed warp instructions per launch in the same capture (default options: depth-test mode, back-face option on)
+NCU_WARP_INST = {"vis_raster": 67621486, "vis_depth_test": 56075028, "shade": 40083311, "composite_segments": 19685208}
+ISSUE_PEAK = 148 * 4 * 1.965e9                             # warp instructions per second: 4 schedulers per SM, one issue per clock
 FP32_PEAK_TFLOPS = 2 * 128 * 148 * 1.965e9 / 1e12          # 74.4: 148 SMs x 128 FP32 lanes x FMA x 1.965 GHz (guide)
 
 
@@ -355,6 +358,9 @@ def main():
                 "note": "fp32 FMA-pipe peak derived from the guide (148 SM x 128 lanes x 2 x 1.965 GHz); "
                         "HBM peak %s %.0f GB/s is not the bound of this kernel" % (pk_kind, pk["hbm_gbs"]),
                 "units_per_launch": units[dom], "flop_per_unit": fpu[dom], "kernel_ms": kern_ms[dom]}
+    if cull and args.vis_mode == 0 and dom in NCU_WARP_INST:      # how busy the issue slots are: EXECUTED instructions, not algorithmic work
+        roofline["issue_slots"] = {"executed_warp_inst": NCU_WARP_INST[dom], "source": NCU_SOURCE[dom],
+                                   "frac_of_issue_peak": NCU_WARP_INST[dom] / (kern_ms[dom] * 1e-3) / ISSUE_PEAK}
 
     # SURVEY 8(f) item 2 (beside the metric): the displacement network d(x, theta) on the tensor cores (tcgen05, TF32)
     mlp = workloads.make_disp_mlp(seed=1)
