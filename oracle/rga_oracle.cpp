@@ -7,8 +7,10 @@
 // IMPLICIT fused multiply-add (build with -ffp-contract=off); only + - * / sqrt and, where written, an explicit
 // std::fma -- all of which IEEE-754 rounds identically on every machine.  Everything compared under a tolerance (shading, compositing) is computed in double.
 //
-// Pins (tests/test_oracle_pins.py): see DESIGN.md "Oracle pins".  "parity unpinned" for: gamma exponent (A9),
-// shadow-map bias constants (A17), 3DGS rasteriser constants (A18) -- PAPER.md prints no value for them.
+// Pins (tests/test_oracle_pins.py, tests/test_oracle_pins2.py): see DESIGN.md "Oracle pins".  "parity unpinned" only for
+// the VALUES of: gamma exponent (A9), shadow-map bias constants (A17), 3DGS rasteriser constants (A18) -- PAPER.md prints
+// no value for them; the RULES that use them (clamp, skip, stop-before, n_contrib; bias monotone in the slope) are pinned.
+// Arithmetic frozen since round 2 (reading A37): a kernel that wants another operation order matches this file.
 //
 // Build: g++ -O2 -ffp-contract=off -fno-fast-math -fopenmp -shared -fPIC (oracle/build.py).
 #include <algorithm>
@@ -160,8 +162,22 @@ ORC void orc_light_frames(const float* dirs, int K, float* uvw) {
 //   py = likewise with v_s
 //   z  = fma(w_n.z, d.z, fma(w_n.y, d.y, fma(w_n.x, d.x, 0.5)))     = (r - w.d) / (2r)
 // std::fma is the correctly rounded fused operation on every IEEE-754 machine, so this stays bit-reproducible.
+// DIAGNOSTIC ONLY (reading A37): the same projection and bias in the spelled-out form of SURVEY.md:371-381,
+//   px = ((u.d)/r * 1/2 + 1/2) R,  z = (r - w.d)/(2r),  beta = ((bias_texels (2r/R)) tau + bias_world)/(2r),
+// selected by orc_set_plain_projection(1).  oracle/a37_projection_forms.py counts the depth texels and visibility bits
+// that differ between the two forms; nothing else ever switches it on.
+static int g_plain_projection = 0;
+ORC void orc_set_plain_projection(int on) { g_plain_projection = on; }
+
 static inline void light_project(const float* p, const float* c, float r, const float* u, const float* v, const float* w,
                                  int R, float* px, float* py, float* z) {
+  if (g_plain_projection) {
+    float d[3] = {p[0] - c[0], p[1] - c[1], p[2] - c[2]};
+    *px = ((dot3(u, d) / r) * 0.5f + 0.5f) * (float)R;
+    *py = ((dot3(v, d) / r) * 0.5f + 0.5f) * (float)R;
+    *z = (r - dot3(w, d)) / (2.0f * r);
+    return;
+  }
   float hR = 0.5f * (float)R, sR = hR / r, inv2r = 1.0f / (2.0f * r);
   float us[3] = {u[0] * sR, u[1] * sR, u[2] * sR}, vs[3] = {v[0] * sR, v[1] * sR, v[2] * sR};
   float wn[3] = {-(w[0] * inv2r), -(w[1] * inv2r), -(w[2] * inv2r)};
@@ -255,6 +271,7 @@ ORC void orc_vis_depth_test(const float* xg, const float* ng_, int ng, const flo
           tau = std::fmin(std::fmax(tau, 1.0f), slope_max);
         } else tau = slope_max;
         float beta = (bias_texels / (float)R) * tau + bias_world * (1.0f / (2.0f * r));   // texel = 1/R in normalised depth
+        if (g_plain_projection) beta = ((bias_texels * ((2.0f * r) / (float)R)) * tau + bias_world) / (2.0f * r);
         vis = z <= bitsf(zb) + beta;
       }
       if (vis) bits[(size_t)g * words + (k >> 5)] |= 1u << (k & 31);
@@ -470,25 +487,37 @@ ORC void orc_tile_ranges(const uint64_t* keys, int64_t D, int ntiles, uint32_t* 
 }
 
 // One pixel's front-to-back blend over an index list (3DGS conventions, reading A18): double precision.
-// flag is set when a threshold decision (power>0, alpha<1/255, T<1e-4) is within fp32 rounding reach of flipping.
+// flag (test bookkeeping, not part of the method; SURVEY.md:224-227, reading A38): set when one of the three
+// threshold decisions lies within the reach of an fp32 evaluation of the same formulas, so that a correct fp32 blend may
+// legitimately take the other branch.  The reach is derived from the arithmetic, with U = 2^-23 (one fp32 ulp, relative):
+//   power: an fp32 evaluation of -0.5(a dx^2 + c dy^2) - b dx dy carries an absolute error of at most 4 U M, where
+//          M = 0.5(|a| dx^2 + |c| dy^2) + |b dx dy| >= |power| is the magnitude of its terms;
+//   alpha: o exp(power) inherits that as a relative error, plus 16 U for the exponential (ex2.approx is good to 2 ulp,
+//          its argument power * log2(e) is rounded twice) and the product:  rel(alpha) <= (16 + 4 M) U;
+//   T:     a product of n fp32 factors (1 - alpha_i) carries the relative error sum_i [U + delta(alpha_i) / (1 - alpha_i)]
+//          (an alpha clamped to 0.99 on both sides contributes no delta).
 static void blend_pixel(double pxc, double pyc, const uint32_t* list, int64_t n, const float* mu, const float* conic_o,
                         const double* col, const float* bg, double* out3, double* Tout, uint32_t* ncontrib, uint8_t* flag) {
-  double T = 1.0, C[3] = {0, 0, 0}; uint32_t cnt = 0, last = 0; uint8_t fl = 0;
+  const double U = 1.1920928955078125e-07;                 // 2^-23
+  double T = 1.0, C[3] = {0, 0, 0}, eT = 0.0; uint32_t cnt = 0, last = 0; uint8_t fl = 0;
   for (int64_t i = 0; i < n; ++i) {
     uint32_t g = list[i]; ++cnt;
     double dx = (double)mu[2 * (size_t)g] - pxc, dy = (double)mu[2 * (size_t)g + 1] - pyc;
     const float* co = conic_o + 4 * (size_t)g;
     double power = -0.5 * ((double)co[0] * dx * dx + (double)co[2] * dy * dy) - (double)co[1] * dx * dy;
-    if (std::fabs(power) < 1e-5) fl = 1;
+    double M = 0.5 * (std::fabs((double)co[0]) * dx * dx + std::fabs((double)co[2]) * dy * dy) + std::fabs((double)co[1] * dx * dy);
+    if (power != 0.0 && std::fabs(power) <= 8.0 * U * M) fl = 1;
     if (power > 0.0) continue;
-    double alpha = std::min(0.99, (double)co[3] * std::exp(power));
-    if (std::fabs(alpha - 1.0 / 255.0) < 2e-6 * (1.0 + std::fabs(power))) fl = 1;
+    double raw = (double)co[3] * std::exp(power), rel = (16.0 + 4.0 * M) * U;
+    double alpha = std::min(0.99, raw);
+    if (std::fabs(alpha - 1.0 / 255.0) <= rel * alpha) fl = 1;
     if (alpha < 1.0 / 255.0) continue;
-    double testT = T * (1.0 - alpha);
-    if (std::fabs(testT - 1e-4) < 1e-8) fl = 1;
+    double dalpha = (raw > 0.99 * (1.0 + rel)) ? 0.0 : rel * alpha;       // clamped on both sides: exact
+    double testT = T * (1.0 - alpha), eTest = eT + 2.0 * U + dalpha / (1.0 - alpha);
+    if (std::fabs(testT - 1e-4) <= eTest * testT) fl = 1;
     if (testT < 1e-4) break;
     for (int c = 0; c < 3; ++c) C[c] += col[3 * (size_t)g + c] * alpha * T;
-    T = testT; last = cnt;
+    T = testT; eT = eTest; last = cnt;
   }
   for (int c = 0; c < 3; ++c) out3[c] = C[c] + T * (double)bg[c];
   *Tout = T; *ncontrib = last; if (flag) *flag = fl;
