@@ -120,6 +120,7 @@ def vis_paper(idmap, faces, nv, knn_v, want_stages=False):
 
 
 def vis_gauss(vcount, knn_g, ubar, Kv):
+    knn_g = np.ascontiguousarray(knn_g, np.int32); ubar = _f32(ubar)
     ng, K = len(knn_g), vcount.shape[1]
     out = np.empty((ng, K), np.float64)
     lib().orc_vis_gauss(_p(vcount), _p(knn_g), _p(ubar), C.c_int(ng), C.c_int(knn_g.shape[1]), C.c_int(K), C.c_int(Kv), _p(out))
@@ -283,8 +284,21 @@ def avatar_load(inp):
     return av
 
 
-def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None):
-    """H1..H10.  vis_mode 0 = depth test (north_star), 1 = paper (Eq.3-4), 2 = no visibility (v = 1)."""
+def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None, gauss_chunk=None, timings=None):
+    """H1..H10.  vis_mode 0 = depth test (north_star), 1 = paper (Eq.3-4), 2 = no visibility (v = 1).
+    gauss_chunk (paper mode only): evaluate Eq.1-of-v and the shading in chunks of that many Gaussians, so that the
+    [N_g, K] double table of v_g is never held whole (8 GB at config 4); the arithmetic per Gaussian is unchanged and
+    o["vis_g"] is then not returned.
+    timings: optional dict; the wall-clock seconds of each stage (skin, visibility, shade, splat) are added to it
+    (bench.py's cpu_baseline leg)."""
+    import time as _time
+    t_prev = [_time.perf_counter()]
+
+    def lap(name):
+        if timings is not None:
+            now = _time.perf_counter()
+            timings[name] = timings.get(name, 0.0) + (now - t_prev[0])
+            t_prev[0] = now
     o = {}
     G = inp["bone_mats"][frame]
     o["vert_posed"], o["vert_normal_posed"], _ = skin(inp["vert_pos"], inp["vert_disp"], inp["vert_normal"],
@@ -292,6 +306,7 @@ def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None):
     o["gauss_posed"], o["gauss_normal_posed"], M = skin(inp["gauss_pos"], av["disp_g"], av["normal_g"], av["skin_w_g"], G)
     o["cov6"] = gauss_cov(M, inp["gauss_quat"], inp["gauss_scale"])
     o["win_c"], o["win_r"] = window(o["vert_posed"])
+    lap("skin")
     if stop_after == "skin":
         return o
     dirs, R = inp["vis_dirs"], inp["vis_res"]
@@ -300,17 +315,32 @@ def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None):
     if vis_mode in (0, 1):
         o["zmap"], o["idmap"] = vis_raster(o["vert_posed"], inp["faces"], dirs, R, o["win_c"], o["win_r"], want_ids=True,
                                            cull=bool(inp.get("vis_cull_backfaces", False)))
+        lap("vis_raster")
     if vis_mode == 0:
         bits = o["visbits"] = vis_depth_test(o["gauss_posed"], o["gauss_normal_posed"], dirs, R, o["win_c"], o["win_r"],
                                              o["zmap"], inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
+        lap("vis_depth_test")
     elif vis_mode == 1:
         o["vcount"] = vis_paper(o["idmap"], inp["faces"], len(inp["vert_pos"]), av["knn_v"])
-        vg = o["vis_g"] = vis_gauss(o["vcount"], av["knn_g"], av["ubar_g"], av["knn_v"].shape[1])
+        if not gauss_chunk:
+            vg = o["vis_g"] = vis_gauss(o["vcount"], av["knn_g"], av["ubar_g"], av["knn_v"].shape[1])
+        lap("vis_paper")
     if stop_after == "vis":
         return o
     env = inp["env"][inp["env_of_frame"][frame]]
-    o["L_o"], o["color"] = shade(o["gauss_posed"], o["gauss_normal_posed"], av["albedo_g"], av["rough_g"], av["spec_g"],
-                                 inp["cam_pos"], env, inp["texel_to_dir"], vis_mode, bits, vg, K, inp["gamma"])
+    if vis_mode == 1 and gauss_chunk:
+        ng = len(o["gauss_posed"])
+        o["L_o"] = np.empty((ng, 3), np.float64); o["color"] = np.empty((ng, 3), np.float64)
+        for a in range(0, ng, gauss_chunk):
+            b = min(ng, a + gauss_chunk)
+            vgc = vis_gauss(o["vcount"], av["knn_g"][a:b], av["ubar_g"][a:b], av["knn_v"].shape[1])
+            o["L_o"][a:b], o["color"][a:b] = shade(o["gauss_posed"][a:b], o["gauss_normal_posed"][a:b], av["albedo_g"][a:b],
+                                                   av["rough_g"][a:b], av["spec_g"][a:b], inp["cam_pos"], env, inp["texel_to_dir"],
+                                                   1, None, vgc, K, inp["gamma"])
+    else:
+        o["L_o"], o["color"] = shade(o["gauss_posed"], o["gauss_normal_posed"], av["albedo_g"], av["rough_g"], av["spec_g"],
+                                     inp["cam_pos"], env, inp["texel_to_dir"], vis_mode, bits, vg, K, inp["gamma"])
+    lap("shade")
     if stop_after == "shade":
         return o
     cam = camera or inp["camera"]
@@ -319,6 +349,14 @@ def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None):
     o.update(project(o["gauss_posed"], o["gauss_normal_posed"], o["cov6"], inp["gauss_opacity"], cam))
     o["keys"], o["vals"] = emit_sort(o["depth"], o["rect"], o["touched"], TX)
     o["ranges"] = tile_ranges(o["keys"], TX * TY)
+    lap("project_sort")
     o["image"], o["T_final"], o["n_contrib"], o["flags"] = composite(o["vals"], o["ranges"], o["mu"], o["conic_o"],
                                                                      o["color"], inp["bg"], W, H)
+    lap("composite")
     return o
+
+
+def set_num_threads(n):
+    """OpenMP thread count of the oracle library from here on (bench.py times it single-threaded and on all cores)."""
+    g = C.CDLL("libgomp.so.1")
+    g.omp_set_num_threads(C.c_int(int(n)))

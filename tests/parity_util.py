@@ -105,18 +105,23 @@ def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=N
     assert eq(rd("KEYS_SORTED"), o["keys"]), "sorted keys"
     assert eq(rd("VALS_SORTED"), o["vals"]), "sorted vals"
     assert eq(rd("TILE_RANGES").reshape(-1, 2), o["ranges"]), "tile ranges"
-    # H10
+    # H10.  Unflagged pixels: north_star bounds on image and T_final, n_contrib exact.  Flagged pixels (A38: one
+    # of the blend's threshold decisions is within fp32 reach of flipping; ~1e-5 of the pixels): one alpha ~ 1/255
+    # contribution may flip, so image and T_final are held to 1/255 + 2e-3 there and n_contrib is not constrained.
     d = np.abs(img.astype(np.float64) - o["image"]).max(-1)
     fl = o["flags"].astype(bool)
     rep["image_max"], rep["image_mean"], rep["flagged"] = d[~fl].max() if (~fl).any() else 0.0, d.mean(), int(fl.sum())
+    assert fl.mean() <= 1e-4 or fl.sum() <= 2, "flag band too wide: %d px" % fl.sum()
     assert rep["image_max"] <= IMG_MAX, "image max %g" % rep["image_max"]
     assert d.mean() <= IMG_MEAN, "image mean %g" % d.mean()
-    if fl.any():
-        assert d[fl].max() <= FLAG_MAX, "flagged pixels max %g" % d[fl].max()
     H, W = img.shape[:2]
     T = rd("T_FINAL").reshape(H, W).astype(np.float64)
-    assert np.abs(T - o["T_final"])[~fl].max() <= IMG_MAX, "T_final"
+    dT = np.abs(T - o["T_final"])
+    if fl.any():
+        assert d[fl].max() <= FLAG_MAX, "flagged pixels max %g" % d[fl].max()
+        assert dT[fl].max() <= FLAG_MAX, "flagged pixels T_final %g" % dT[fl].max()
+    assert dT[~fl].max() <= IMG_MAX, "T_final"
     nc = rd("N_CONTRIB").reshape(H, W)
-    rep["n_contrib_mismatch"] = float((nc != o["n_contrib"])[~fl].mean())
-    assert rep["n_contrib_mismatch"] < 1e-3, "n_contrib"
+    rep["n_contrib_mismatch"] = int((nc != o["n_contrib"])[~fl].sum())
+    assert rep["n_contrib_mismatch"] == 0, "n_contrib differs on %d unflagged pixels" % rep["n_contrib_mismatch"]
     return rep

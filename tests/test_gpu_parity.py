@@ -9,12 +9,12 @@ from synth import workloads
 pytestmark = pytest.mark.gpu
 
 
-def _both(cfg, vis_mode, n_gauss=None, use_visibility=True, **kw):
+def _both(cfg, vis_mode, n_gauss=None, use_visibility=True, morton=True, gauss_chunk=None, **kw):
     from oracle import oracle as orc
     from parity_util import compare_all, run_gpu
-    inp = workloads.make(cfg, n_gauss=n_gauss)
+    inp = workloads.make(cfg, n_gauss=n_gauss, morton=morton)
     orc_av = orc.avatar_load(inp)
-    o = orc.render_frame(orc_av, inp, vis_mode=vis_mode if use_visibility else 2)
+    o = orc.render_frame(orc_av, inp, vis_mode=vis_mode if use_visibility else 2, gauss_chunk=gauss_chunk)
     av, img = run_gpu(inp, vis_mode=vis_mode, use_visibility=use_visibility, **kw)
     rep = compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility)
     av.close()
@@ -58,6 +58,28 @@ def test_cfg4_structure_paper_mode():
     print(rep)
 
 
+def test_cfg2_highres_full_size_paper_mode():
+    # configs[2] at full size in the paper's own visibility: 512 triangle-ID maps of 256^2, Eq.3-4 over the
+    # 27.5k-vertex mesh, v_g gathered for 300k Gaussians x 2,048 texels (SURVEY.md:300-302: H4b is parity-checked on all five)
+    rep = _both(2, 1)
+    print(rep)
+
+
+def test_cfg4_stress_full_size_paper_mode():
+    # configs[4] at full size in paper mode: 1M Gaussians, 1,024 ID maps of 256^2; the oracle shades in chunks of 100k Gaussians
+    # (orchestration only) so that the [N_g, K] table of v_g is never held whole
+    rep = _both(4, 1, gauss_chunk=100_000)
+    print(rep)
+
+
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_cfg1_gaussians_in_caller_order(vis_mode):
+    # BASELINE.json configs[0]: "Gaussians placed on random surface points" -- a trained asset's order is arbitrary
+    # (PAPER.md:88-93 defines none).  Same full-size config 1 with the generator's spatial sort switched off.
+    rep = _both(1, vis_mode, morton=False)
+    print(rep)
+
+
 def test_cfg3_animation_frames():
     # configs[3]: several poses / env maps of the sequence through ONE loaded avatar
     import torch
@@ -81,6 +103,60 @@ def test_cfg3_animation_frames():
         assert np.array_equal(av.read("KEYS_SORTED"), o["keys"]) and np.array_equal(av.read("VALS_SORTED"), o["vals"])
         d = np.abs(img.cpu().numpy().astype(np.float64) - o["image"]).max(-1)
         assert d[o["flags"] == 0].max() <= IMG_MAX
+    av.close()
+
+
+def test_cfg3_animation_100k_gaussians_one_graph_of_eight_poses():
+    # configs[3] at full size (100k Gaussians, 512 directions at 128^2, 512x512): eight poses of the 64-pose sequence, each
+    # lit by its own environment map (visibility is recomputed for every novel pose), captured as ONE CUDA
+    # graph of eight rga_render_frame calls and replayed; every replayed image is compared with the oracle's frame, and the
+    # last pose's visibility bits and sorted lists bit for bit.
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import IMG_MAX, IMG_MEAN, facing_split
+    inp = workloads.make(3)
+    assert len(inp["gauss_pos"]) == 100_000 and len(inp["bone_mats"]) == 64
+    orc_av = orc.avatar_load(inp)
+    cam = inp["camera"]; W, H = cam["width"], cam["height"]
+    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=512, max_vis_res=128, max_env_texels=512)
+    dirs = torch.as_tensor(inp["vis_dirs"]).cuda(); t2d = torch.as_tensor(inp["texel_to_dir"]).cuda()
+    envs = torch.as_tensor(inp["env"]).cuda(); bones = torch.as_tensor(inp["bone_mats"]).cuda()
+    poses = (0, 9, 18, 27, 36, 45, 54, 63)
+    assert len({int(inp["env_of_frame"][t]) for t in poses}) > 1           # the environment map does switch
+    imgs = torch.zeros((len(poses), H, W, 3), dtype=torch.float32, device="cuda")
+    bias = (inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
+
+    def frames():
+        for i, t in enumerate(poses):
+            av.render(bones[t], dirs, 128, envs[int(inp["env_of_frame"][t])], t2d, inp["cam_pos"], cam, inp["bg"], imgs[i],
+                      vis_mode=0, gamma=inp["gamma"], bias=bias)
+    frames()                                                               # warm-up outside the capture
+    rga.rga_check(av.h)
+    imgs.zero_()
+    g = torch.cuda.CUDAGraph()
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(g, stream=st):
+            frames()
+    torch.cuda.current_stream().wait_stream(st)
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    rga.rga_check(av.h)
+    out = imgs.cpu().numpy()
+    for i, t in enumerate(poses):
+        o = orc.render_frame(orc_av, inp, frame=t, vis_mode=0)
+        d = np.abs(out[i].astype(np.float64) - o["image"]).max(-1)
+        fl = o["flags"].astype(bool)
+        assert fl.sum() <= 26 and d[~fl].max() <= IMG_MAX and d.mean() <= IMG_MEAN, (t, int(fl.sum()), d[~fl].max(), d.mean())
+    kept, culled = facing_split(inp, o)                                    # the last pose's intermediates are still there
+    vb = av.read("VISBITS").reshape(len(inp["gauss_pos"]), -1)
+    assert np.array_equal(vb[kept], o["visbits"][kept]) and not vb[culled].any()
+    assert np.array_equal(av.read("ZMAP").reshape(o["zmap"].shape), o["zmap"])
+    assert np.array_equal(av.read("KEYS_SORTED"), o["keys"]) and np.array_equal(av.read("VALS_SORTED"), o["vals"])
+    assert np.array_equal(av.read("N_CONTRIB").reshape(H, W)[~fl], o["n_contrib"][~fl])
     av.close()
 
 
