@@ -2,17 +2,27 @@
 """bench.py -- relit posed frames/sec of the arXiv 2407.10707 forward render on B200 (BASELINE.json metric).
 
 A "step" is one pass of the whole hot path (pose_skin -> visibility_raster -> shade_gaussians -> splat_render, all
-SURVEY.md 8(a) rows H1..H10) for one frame of BASELINE.json configs[1]: 100k Gaussians on the 6,890-vertex body,
-512 light directions at 128^2, 16x32 HDR environment map, 512x512 camera; seeded synthetic inputs (synth/).
+SURVEY.md 8(a) rows H1..H10) for one frame of one BASELINE.json config, through `rga_render_frame`; seeded synthetic
+inputs (synth/).  The contract path is measured: every triangle rasterised (two-sided, no culling),
+Gaussians as the generator stores them.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--vis-mode 0|1]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 0..4] [--vis-mode 0|1]
+                  [--all-configs 0|1] [--next 0|1] [--no-cpu-baseline]
 
-Prints ONE JSON line (rank 0).  `value` = frames/s with inputs resident in HBM; `e2e` = the same through the C-ABI
-calls with host (pinned) pose / env-map buffers copied in and the image copied out inside the timed region;
-`roofline` = the dominant kernel against its bound; `cpu_baseline` = the oracle on this box's host cores.
+Prints ONE JSON line (rank 0):
+  value / ms_per_step   frames/s of --config (default configs[1], the headline) with inputs resident in HBM, L2 flushed
+  e2e                   the same through the C-ABI call with pinned HOST pose / env buffers copied in and the image copied out
+  roofline              LIST, dominant kernel first: one object per kernel of the frame (bound, units, work per unit as
+                        SURVEY 8(d) states it, CUDA-event time, achieved, MEASURED peak, frac, DRAM bytes from the ncu capture)
+  configs               all five configs: ms per frame (L2 flushed) + per-kernel and per-stage ms; configs[3] = the 64-pose
+                        sequence replayed from one CUDA graph, env map switched per pose, fps = 64 / time
+  value_unsorted        the headline frame with the Gaussians in generator (random) order
+  value_cull_backfaces  the headline frame with the rasteriser's closed-mesh option (A36) -- NOT the contract path
+  cpu_baseline          the oracle on this box's host cores: all cores and single thread, per stage
 N > 1: replicas only: every rank renders its own frames, no data-path collective.
 """
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -24,16 +34,40 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "relit posed frames/sec (100k Gaussians, 512x512)"
-WORKLOAD = "configs[1] SMPL-sized: 6,890 v / 13,776 f / 24 bones, 100k Gaussians, 16x32 env, 512 dirs @128^2, 512x512"
-# algorithmic work per unit of each kernel (fp32 flop, FMA = 2)
-FLOP_PER_UNIT = {"shade": 70.0, "vis_depth_test": 40.0, "vis_raster": 220.0, "composite_segments": 30.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/)
-NCU_DRAM_BYTES = {"vis_raster": 807680, "vis_depth_test": 13460736, "shade": 9606400, "composite_segments": 2554368}
-NCU_SOURCE = {k: "profiles/r01m_full.md" for k in NCU_DRAM_BYTES}
-# executed warp instructions per launch in the same capture (default options: depth-test mode, back-face option on)
-NCU_WARP_INST = {"vis_raster": 67621486, "vis_depth_test": 56075028, "shade": 40083311, "composite_segments": 19685208}
-ISSUE_PEAK = 148 * 4 * 1.965e9                             # warp instructions per second: 4 schedulers per SM, one issue per clock
-FP32_PEAK_TFLOPS = 2 * 128 * 148 * 1.965e9 / 1e12          # 74.4: 148 SMs x 128 FP32 lanes x FMA x 1.965 GHz (guide)
+WORKLOADS = {
+    0: "configs[0] tiny: icosphere 642 v / 1,280 f / 2 bones, 2k Gaussians, 8x16 env, 16 dirs @64^2, 64x64",
+    1: "configs[1] SMPL-sized: 6,890 v / 13,776 f / 24 bones, 100k Gaussians, 16x32 env, 512 dirs @128^2, 512x512",
+    2: "configs[2] high-res: 27,554 v / 55,104 f / 24 bones, 300k Gaussians, 32x64 env, 512 dirs @256^2, 1024x1024",
+    3: "configs[3] animation: configs[1] avatar over a 64-pose sequence, 4 env maps switched per pose, 512x512",
+    4: "configs[4] stress: 27,554 v / 55,104 f, 1M Gaussians, 32x64 env, 1,024 dirs @256^2, 1920x1080",
+}
+SM_COUNT, LANES, CLOCK = 148, 128, 1.965e9
+FP32_PEAK_DERIVED = 2 * LANES * SM_COUNT * CLOCK / 1e12      # 74.4 TFLOP/s: guide's unit counts x clock (context only)
+
+# Algorithmic work per unit, SURVEY.md 8(d) (issue slots of the FP32/INT lanes; one slot = one FMA-equivalent = 2 flop-eq):
+#   H3 ~100 slots per (triangle, direction); H4a ~20 slots per (Gaussian, direction); H5 ~70 flop (45 slots) per evaluated
+#   (Gaussian, texel) pair; H10 ~25 slots per evaluated (pixel, list entry).  HBM-bound steps: bytes per unit.
+# kernel -> (stage, bound, unit name, work per unit [flop-eq or bytes])
+KERNELS = {
+    "skin":               ("pose_skin", "hbm", "vertex + Gaussian record", None),
+    "vis_raster":         ("visibility", "alu", "(triangle, direction)", 200.0),
+    "vis_depth_test":     ("visibility", "alu", "(Gaussian, direction) test", 40.0),
+    "vis_median1":        ("visibility", "alu", "(vertex, direction)", None),
+    "vis_median2":        ("visibility", "alu", "(vertex, direction)", None),
+    "vis_mean":           ("visibility", "alu", "(vertex, direction)", None),
+    "env_table":          ("shade", "alu", "texel", None),
+    "shade":              ("shade", "alu", "(camera-facing Gaussian, upper-hemisphere texel)", 70.0),
+    "vis_shade":          ("shade", "alu", "(Gaussian, direction) test + (Gaussian, texel) BRDF", None),
+    "project":            ("splat", "hbm", "Gaussian", 56.0 + 64.0),
+    "tile_scan":          ("splat", "hbm", "tile", None),
+    "tile_scatter":       ("splat", "hbm", "duplicate", 8.0 + 8.0),
+    "tile_sort":          ("splat", "smem", "list entry", None),
+    "tile_sort_long":     ("splat", "smem", "list entry", None),
+    "composite_T":        ("splat", "alu", "(pixel, list entry)", 50.0),
+    "composite_segments": ("splat", "alu", "(pixel, list entry)", 50.0),
+    "composite_resolve":  ("splat", "hbm", "pixel", None),
+    "composite_replay":   ("splat", "alu", "(pixel, list entry)", None),
+}
 
 
 class ClockSampler:
@@ -76,8 +110,49 @@ class ClockSampler:
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
-        return json.load(open(p)), "measured"
-    return {"hbm_gbs": 6650.0}, "fallback"
+        return json.load(open(p)), "MEASURED_PEAKS.json"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}, "B200_PROFILING.md fallback"
+
+
+def csrc_hash():
+    """Hash of the kernel sources: the ncu counters under profiles/ are only quoted for the build they were captured on."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2407_10707_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_counters():
+    """profiles/ncu_counters.json: per-kernel DRAM bytes and executed warp instructions of ONE `ncu --set full` capture of this
+    command (written from the capture's raw page), with the csrc hash of the build it was taken on."""
+    p = os.path.join(ROOT, "profiles", "ncu_counters.json")
+    if not os.path.exists(p):
+        return {}, None, False
+    d = json.load(open(p))
+    return d.get("kernels", {}), d.get("source"), d.get("csrc_hash") == csrc_hash()
+
+
+def oracle_times(inp, vis_mode, budget_s=12.0):
+    """cpu_baseline leg: the oracle as it stands on the host cores -- all cores (OpenMP outer loops) and one thread."""
+    from oracle import oracle as orc
+    cores = os.cpu_count()
+    oav = orc.avatar_load(inp)
+    orc.set_num_threads(cores)
+    orc.render_frame(oav, inp, vis_mode=vis_mode)
+    n, stages, t0 = 0, {}, time.perf_counter()
+    while n < 3 or (time.perf_counter() - t0 < budget_s and n < 50):
+        orc.render_frame(oav, inp, vis_mode=vis_mode, timings=stages); n += 1
+    dt = (time.perf_counter() - t0) / n
+    orc.set_num_threads(1)
+    st1, t1 = {}, time.perf_counter()
+    orc.render_frame(oav, inp, vis_mode=vis_mode, timings=st1)
+    dt1 = time.perf_counter() - t1
+    orc.set_num_threads(cores)
+    return {"value": 1.0 / dt, "unit": "frames/s", "cores": cores, "kind": "oracle",
+            "sample": "%d full frames (every step of the path) on all cores, 1 frame on one thread" % n,
+            "stage_s": {k: v / n for k, v in stages.items()},
+            "single_thread": {"value": 1.0 / dt1, "unit": "frames/s", "cores": 1, "stage_s": st1}}
 
 
 def run_reference(args, rank):
@@ -86,202 +161,231 @@ def run_reference(args, rank):
         return
     from oracle import oracle as orc
     from synth import workloads
-    inp = workloads.make(1)
-    inp["vis_cull_backfaces"] = bool(args.cull_backfaces)
+    inp = workloads.make(args.config, morton=False)
     cores = os.cpu_count()
     av = orc.avatar_load(inp)
-    for _ in range(max(args.warmup, 1)):
-        orc.render_frame(av, inp, vis_mode=args.vis_mode)
+    frames = list(range(len(inp["bone_mats"])))
+    for i in range(max(args.warmup, 1)):
+        orc.render_frame(av, inp, frame=frames[i % len(frames)], vis_mode=args.vis_mode)
     t0 = time.perf_counter()
-    for _ in range(args.steps):
-        orc.render_frame(av, inp, vis_mode=args.vis_mode)
+    for i in range(args.steps):
+        orc.render_frame(av, inp, frame=frames[i % len(frames)], vis_mode=args.vis_mode)
     dt = (time.perf_counter() - t0) / args.steps
     fps = 1.0 / dt
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic", "config": {"workload": WORKLOAD, "vis_mode": args.vis_mode, "vis_cull_backfaces": bool(args.cull_backfaces)},
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config], "vis_mode": args.vis_mode, "vis_cull_backfaces": False},
         "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle",
-                         "sample": "%d full frames of configs[1] (every step of the path, OpenMP on outer loops)" % args.steps},
+                         "sample": "%d full frames of %s (every step of the path, OpenMP on outer loops)" % (args.steps, WORKLOADS[args.config][:10])},
         "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--vis-mode", type=int, default=0, help="0 = depth test (north_star, default), 1 = paper filters")
-    ap.add_argument("--cull-backfaces", type=int, default=1,
-                    help="1 (default): the workload's body mesh is closed and outward-oriented, so the depth rasteriser skips "
-                         "triangles that face away from the light (rga_vis_params.cull_backfaces, DESIGN.md A36); 0: rasterise all")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
-    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
-        if args.steps == 200 and args.warmup == 20:
-            args.steps, args.warmup = 10, 1
-        return run_reference(args, rank)
-    args.warmup = max(args.warmup, 3)
+class Bench:
+    """One loaded avatar of one config + the timing protocol (CUDA events on the launching stream, L2 flushed between steps)."""
 
-    import numpy as np
-    import torch
-    import torch.distributed as dist
-    from paper_2407_10707_b200 import binding as rga
-    from synth import workloads
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl")
-    dev = torch.device("cuda", local)
-    inp = workloads.make(1, seed=1 + 1000 * rank if world > 1 else None)
-    cam = inp["camera"]; W, H = cam["width"], cam["height"]
-    K, R = len(inp["vis_dirs"]), inp["vis_res"]
-    t0 = time.perf_counter()
-    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=K, max_vis_res=R, max_env_texels=512)
-    torch.cuda.synchronize(); load_ms = (time.perf_counter() - t0) * 1e3
-    bones = torch.as_tensor(inp["bone_mats"][0]).to(dev); dirs = torch.as_tensor(inp["vis_dirs"]).to(dev)
-    env = torch.as_tensor(inp["env"][0]).to(dev); t2d = torch.as_tensor(inp["texel_to_dir"]).to(dev)
-    img = torch.empty((H, W, 3), dtype=torch.float32, device=dev)
-    camc = rga.make_camera(cam)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)            # > 126 MB L2
-    bias = (inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
+    def __init__(self, cfg, vis_mode, dev, world=1, rank=0, morton=False, flush=None):
+        import torch
+        from paper_2407_10707_b200 import binding as rga
+        from synth import workloads
+        self.torch, self.rga, self.cfg, self.vis_mode, self.dev, self.world = torch, rga, cfg, vis_mode, dev, world
+        seed = cfg + 1000 * rank if world > 1 else None
+        self.inp = inp = workloads.make(cfg, seed=seed, morton=morton)
+        cam = inp["camera"]; self.W, self.H = cam["width"], cam["height"]
+        self.K, self.R = len(inp["vis_dirs"]), inp["vis_res"]
+        t0 = time.perf_counter()
+        self.av = rga.Avatar(inp, max_width=self.W, max_height=self.H, max_vis_dirs=self.K, max_vis_res=self.R,
+                             max_env_texels=inp["env_rows"] * inp["env_cols"])
+        torch.cuda.synchronize(); self.load_ms = (time.perf_counter() - t0) * 1e3
+        self.bones = torch.as_tensor(inp["bone_mats"]).to(dev)              # [frames, B, 12]
+        self.dirs = torch.as_tensor(inp["vis_dirs"]).to(dev)
+        self.envs = torch.as_tensor(inp["env"]).to(dev)                     # [n_env, R, C, 3]
+        self.t2d = torch.as_tensor(inp["texel_to_dir"]).to(dev)
+        self.img = torch.empty((self.H, self.W, 3), dtype=torch.float32, device=dev)
+        self.camc = rga.make_camera(cam)
+        self.bias = (inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"])
+        self.flush = flush if flush is not None else torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
-    cull = bool(args.cull_backfaces)
+    def frame(self, t=0, bones=None, env=None, img=None, cull=False):
+        inp = self.inp
+        self.av.render(self.bones[t] if bones is None else bones, self.dirs, self.R,
+                       self.envs[int(inp["env_of_frame"][t])] if env is None else env, self.t2d, inp["cam_pos"], self.camc, inp["bg"],
+                       self.img if img is None else img, vis_mode=self.vis_mode, gamma=inp["gamma"], bias=self.bias, cull_backfaces=cull)
 
-    def frame(b=bones, e=env):
-        av.render(b, dirs, R, e, t2d, inp["cam_pos"], camc, inp["bg"], img, vis_mode=args.vis_mode, bias=bias, cull_backfaces=cull)
+    def barrier(self):
+        self.torch.cuda.synchronize()
+        if self.world > 1:
+            self.torch.distributed.barrier()
+        self.torch.cuda.synchronize()
 
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def timed(fn, steps, do_flush=True):
+    def timed(self, fn, steps, do_flush=True):
+        torch = self.torch
         evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-        barrier()
+        self.barrier()
         for a, b in evs:
             if do_flush:
-                flush.fill_(1)
+                self.flush.fill_(1)
             a.record(); fn(); b.record()
-        barrier()
+        self.barrier()
         return sum(a.elapsed_time(b) for a, b in evs) / steps
 
-    for _ in range(args.warmup):
-        frame()
-    rga.rga_check(av.h)
-    l0 = rga.rga_launch_count(av.h)
-    cs = ClockSampler(local); cs.__enter__()                     # sampled through every timed pass below
-    ms = timed(frame, args.steps)
-    launches = rga.rga_launch_count(av.h) - l0
-    ms_warm = timed(frame, args.steps, do_flush=False)
-    ms_nocull = None
-    if cull:                                                     # the same frame with every triangle rasterised, for comparison
-        frame_all = lambda: av.render(bones, dirs, R, env, t2d, inp["cam_pos"], camc, inp["bg"], img, vis_mode=args.vis_mode, bias=bias)
-        for _ in range(3):
-            frame_all()
-        ms_nocull = timed(frame_all, max(args.steps // 4, 10))
+    def kernel_times(self, steps, t=0):
+        """per-kernel CUDA-event means (the library records an event after each of its kernels; one stream, no overlap)."""
+        import numpy as np
+        rga = self.rga
+        rga.rga_profile_enable(self.av.h, True)
+        acc = {}
+        for _ in range(steps):
+            self.flush.fill_(1)
+            self.frame(t)
+            for name, ms in rga.rga_profile_read(self.av.h):
+                acc.setdefault(name, []).append(ms)
+        rga.rga_profile_enable(self.av.h, False)
+        return {k: float(np.mean(v)) for k, v in acc.items()}
 
-    # end to end: host (pinned) pose + env in, image out, every step, through the same C-ABI calls
-    h_bones = torch.as_tensor(inp["bone_mats"][0]).pin_memory(); h_env = torch.as_tensor(inp["env"][0]).pin_memory()
-    h_img = torch.empty((H, W, 3), dtype=torch.float32).pin_memory()
-    d_bones = torch.empty_like(bones); d_env = torch.empty_like(env)
+    def units(self):
+        """algorithmic units of each kernel for the frame that was just rendered (counted from its intermediates)."""
+        import numpy as np
+        inp, av = self.inp, self.av
+        gp = av.read("GAUSS_POSED").reshape(-1, 4)[:, :3]; gn = av.read("GAUSS_NORMAL_POSED").reshape(-1, 4)[:, :3]
+        front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
+        rg = av.read("TILE_RANGES").reshape(-1, 2).astype(np.int64)
+        D = int(av.read("NUM_DUPLICATES")[0])
+        ne = inp["env_rows"] * inp["env_cols"]
+        nv, ng, nb = len(inp["vert_pos"]), len(gp), inp["bone_mats"].shape[1]
+        nc = av.read("N_CONTRIB").astype(np.int64)
+        return {
+            "skin": {"units": nv + ng, "bytes": nv * (132 + 24 + 4 * max(nb - 24, 0)) + ng * (176 + 72 + 4 * max(nb - 24, 0))},
+            "vis_raster": {"units": len(inp["faces"]) * self.K},
+            # inside rga_render_frame the mode-0 depth test runs for the camera-facing Gaussians only
+            "vis_depth_test": {"units": front * self.K},
+            "shade": {"units": front * ne * 0.5},
+            "project": {"units": ng},
+            "tile_scatter": {"units": D},
+            "composite_T": {"units": float(nc.sum())},
+            "composite_segments": {"units": float(nc.sum())},
+            "_front": front, "_D": D, "_active_tiles": int(((rg[:, 1] - rg[:, 0]) > 0).sum()),
+            "_list_max": int((rg[:, 1] - rg[:, 0]).max()), "_pairs_all": float(((rg[:, 1] - rg[:, 0]) * 256).sum()),
+            "_pairs_until_stop": float(nc.sum()),
+        }
 
-    def frame_e2e():
-        d_bones.copy_(h_bones, non_blocking=True); d_env.copy_(h_env, non_blocking=True)
-        frame(d_bones, d_env)
-        h_img.copy_(img, non_blocking=True)
-    for _ in range(3):
-        frame_e2e()
-    ms_e2e = timed(frame_e2e, args.steps)
+    def close(self):
+        self.av.close()
 
-    # the same with the image read-back of step i on a copy stream beside step i+1 (two image buffers): what a viewer
-    # loop does.  Reported as e2e.pipelined_value; e2e.value stays the serial number above.
-    copy_stream = torch.cuda.Stream(device=dev)
-    imgs = [torch.empty_like(img) for _ in range(2)]
-    h_imgs = [torch.empty((H, W, 3), dtype=torch.float32).pin_memory() for _ in range(2)]
-    copied = [None, None]
 
-    def run_pipelined(steps):
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-        last_copy = None
-        barrier()
-        for i, (a, b) in enumerate(evs):
-            flush.fill_(1)
-            a.record()
-            if copied[i & 1] is not None:
-                torch.cuda.current_stream().wait_event(copied[i & 1])     # buffer i&1 has been read back
-            d_bones.copy_(h_bones, non_blocking=True); d_env.copy_(h_env, non_blocking=True)
-            av.render(d_bones, dirs, R, d_env, t2d, inp["cam_pos"], camc, inp["bg"], imgs[i & 1], vis_mode=args.vis_mode, bias=bias, cull_backfaces=cull)
-            b.record()
-            copy_stream.wait_event(b)
-            with torch.cuda.stream(copy_stream):
-                h_imgs[i & 1].copy_(imgs[i & 1], non_blocking=True)
-                copied[i & 1] = torch.cuda.Event(enable_timing=True); copied[i & 1].record()
-                last_copy = copied[i & 1]
-        barrier(); copy_stream.synchronize()
-        tail = max(evs[-1][1].elapsed_time(last_copy), 0.0)                # the last read-back is not hidden by a next step
-        return (sum(a.elapsed_time(b) for a, b in evs) + tail) / steps
-    run_pipelined(3)
-    ms_e2e_pipe = run_pipelined(args.steps)
+def stage_ms(kern_ms):
+    st = {}
+    for k, v in kern_ms.items():
+        s = KERNELS.get(k, ("other",))[0]
+        st[s] = st.get(s, 0.0) + v
+    return st
 
-    # per-kernel times (CUDA events recorded by the library after each of its kernels), same flush protocol
-    rga.rga_profile_enable(av.h, True)
-    acc = {}
-    for _ in range(args.steps):
-        flush.fill_(1)
-        frame()
-        for name, t in rga.rga_profile_read(av.h):
-            acc.setdefault(name, []).append(t)
-    rga.rga_profile_enable(av.h, False)
-    kern_ms = {k: float(np.mean(v)) for k, v in acc.items()}
-    rga.rga_check(av.h)
-    t_end = time.time() + 1.0                                      # at least a second of load for the sampler
-    while time.time() < t_end or len(cs.rows) < 3:
-        for _ in range(50):
-            frame()
-        torch.cuda.synchronize()
-        if time.time() > t_end + 5.0:
-            break
-    cs.__exit__(); clocks = cs.summary()
 
-    # SURVEY 8(f) item 1 (reported beside the metric, not part of it): visibility is view- and light-independent for a
-    # pose, so further views of the same pose cost only shade + splat through the per-stage calls
+def roofline_list(kern_ms, units, fma_meas, hbm_gbs, hbm_src):
+    ncu, ncu_src, ncu_ok = ncu_counters()
+    out = []
+    for k, ms in sorted(kern_ms.items(), key=lambda kv: -kv[1]):
+        stage, bound, unit_name, work = KERNELS.get(k, ("other", "alu", "", None))
+        u = units.get(k)
+        o = {"kernel": k, "stage": stage, "bound": bound, "kernel_ms": ms}
+        if u is not None and bound == "hbm" and ("bytes" in u or work):
+            byts = u.get("bytes", u["units"] * (work or 0))
+            o.update(units_per_launch=u["units"], unit_of_work=unit_name, bytes_per_launch=byts, achieved=byts / (ms * 1e-3) / 1e9,
+                     peak=hbm_gbs, peak_source=hbm_src, unit="GB/s")
+            o["frac"] = o["achieved"] / o["peak"]
+        elif u is not None and work and bound == "alu":
+            ach = u["units"] * work / (ms * 1e-3) / 1e12
+            o.update(units_per_launch=u["units"], unit_of_work=unit_name, flop_eq_per_unit=work, achieved=ach, peak=fma_meas,
+                     peak_source="register-resident FFMA chains measured in this run (rga_measure_fp32_peak)",
+                     peak_derived=FP32_PEAK_DERIVED, unit="TFLOP/s", frac=ach / fma_meas if fma_meas > 0 else None)
+        else:
+            o.update(achieved=None, peak=None, frac=None, unit=None, note="latency / launch bound helper kernel: no work model")
+        c = ncu.get(k)
+        if c and ncu_ok:
+            o["traffic"] = c.get("dram_bytes"); o["traffic_source"] = ncu_src
+            if c.get("warp_inst"):
+                o["issue_slots"] = {"executed_warp_inst": c["warp_inst"],
+                                    "frac_of_issue_peak": c["warp_inst"] / (ms * 1e-3) / (SM_COUNT * 4 * CLOCK)}
+        else:
+            o["traffic"] = None
+            if c and not ncu_ok:
+                o["traffic_note"] = "profiles/ncu_counters.json was captured on another build of csrc/ (hash mismatch): not quoted"
+        out.append(o)
+    return out
+
+
+def bench_config(cfg, vis_mode, dev, steps, warmup, flush):
+    """One entry of `configs`: ms per frame (L2 flushed), per-kernel / per-stage ms; configs[3]: the 64-pose graph replay."""
+    import torch
+    b = Bench(cfg, vis_mode, dev, morton=False, flush=flush)
+    rga = b.rga
+    nfr = len(b.inp["bone_mats"])
+    for i in range(warmup):
+        b.frame(i % nfr)
+    rga.rga_check(b.av.h)
+    out = {"workload": WORKLOADS[cfg], "avatar_load_ms": b.load_ms}
+    if nfr > 1:
+        # SURVEY 8(d) timing protocol: the whole pose sequence captured once as a CUDA graph (re-skinning, re-visibility,
+        # env map switched per pose), replayed; steady-state fps = frames / time
+        g = torch.cuda.CUDAGraph(); st = torch.cuda.Stream(device=dev)
+        st.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(st):
+            with torch.cuda.graph(g, stream=st):
+                for t in range(nfr):
+                    b.frame(t)
+        torch.cuda.current_stream().wait_stream(st)
+        g.replay(); torch.cuda.synchronize()
+        reps = max(2, min(steps, 10))
+        ms_seq = b.timed(g.replay, reps)
+        rga.rga_check(b.av.h)
+        out.update(protocol="%d-pose sequence in ONE CUDA graph, env map switched per pose, L2 flushed between replays" % nfr,
+                   ms_per_sequence=ms_seq, ms_per_frame=ms_seq / nfr, fps=nfr * 1e3 / ms_seq, envs_used=len(set(int(e) for e in b.inp["env_of_frame"])))
+        ms_single = b.timed(lambda: b.frame(7), max(3, min(steps, 20)))
+        out["ms_per_frame_single_call_flushed"] = ms_single
+    else:
+        ms = b.timed(b.frame, steps)
+        out.update(protocol="rga_render_frame per step, L2 flushed between steps", ms_per_frame=ms, fps=1e3 / ms)
+    km = b.kernel_times(max(3, min(steps, 10)))
+    u = b.units()
+    out.update(kernel_ms=km, stage_ms=stage_ms(km), duplicates=u["_D"], camera_facing_gaussians=u["_front"], active_tiles=u["_active_tiles"],
+               longest_tile_list=u["_list_max"], blend_pairs_until_stop=u["_pairs_until_stop"], blend_pairs_all=u["_pairs_all"])
+    rga.rga_check(b.av.h)
+    b.close()
+    del b
+    torch.cuda.empty_cache()
+    return out
+
+
+def next_rows(b, steps):
+    """SURVEY 8(f) rows, reported beside the metric (not part of it); same timing protocol."""
+    import numpy as np
+    import torch
+    from synth import workloads
+    rga, av, inp, dev, camc, img = b.rga, b.av, b.inp, b.dev, b.camc, b.img
+    bones, env, t2d, dirs = b.bones[0], b.envs[0], b.t2d, b.dirs
+    out = {}
     NV = 4
+
     def pose_with_views():
         rga.pose_skin(av.h, bones)
-        rga.visibility_raster(av.h, dirs, R, args.vis_mode, bias[0], bias[1], bias[2], cull_backfaces=cull)
+        rga.visibility_raster(av.h, dirs, b.R, b.vis_mode, b.bias[0], b.bias[1], b.bias[2])
         for _ in range(NV):
             rga.shade_gaussians(av.h, env, inp["cam_pos"], t2d, inp["gamma"], True)
             rga.splat_render(av.h, camc, inp["bg"], img)
     for _ in range(3):
         pose_with_views()
-    ms_views = timed(pose_with_views, max(args.steps // 4, 5))
-
-    # backward of the splat (H10 + H6) for the frame just rendered, seeded dL/dimage
+    ms_views = b.timed(pose_with_views, max(steps // 4, 5))
+    out["amortised"] = {"views_per_pose": NV, "views_per_s": NV * 1e3 / ms_views, "ms_per_pose": ms_views}
+    b.frame()
     dLdI = torch.as_tensor(workloads.make_image_cotangent(1, camc.width, camc.height)).to(dev)
-    ng_all = len(inp["gauss_pos"])
+    ng_all, nv_all, nb_all = len(inp["gauss_pos"]), len(inp["vert_pos"]), inp["bone_mats"].shape[1]
     d_col = torch.empty((ng_all, 3), device=dev); d_op = torch.empty((ng_all,), device=dev)
     d_x = torch.empty((ng_all, 3), device=dev); d_cov = torch.empty((ng_all, 6), device=dev)
     run_bwd = lambda: rga.splat_backward(av.h, camc, inp["bg"], img, dLdI, d_col, d_op, d_x, d_cov)
     for _ in range(3):
         run_bwd()
-    ms_bwd = timed(run_bwd, 20)
-    rga.rga_profile_enable(av.h, True)
-    bwd_k = {}
-    for _ in range(10):
-        run_bwd()
-        for name, t in rga.rga_profile_read(av.h):
-            bwd_k.setdefault(name, []).append(t)
-    rga.rga_profile_enable(av.h, False)
-    bwd_obj = {"ms": ms_bwd, "kernel_ms": {k: float(np.mean(v)) for k, v in bwd_k.items() if k != "-"},
-               "note": "gradients w.r.t. colour, opacity, posed mean and 3D covariance of every Gaussian; L2 flushed between calls"}
-
-    # ... and of the shading step H5, fed with the colour gradient the splat's backward just produced
+    out["splat_backward"] = {"ms": b.timed(run_bwd, 20)}
     ne_all = int(env.shape[0] * env.shape[1])
     sb = dict(out_dalbedo=torch.empty((ng_all, 3), device=dev), out_drough=torch.empty((ng_all,), device=dev),
               out_dspec=torch.empty((ng_all,), device=dev), out_dnormal=torch.empty((ng_all, 3), device=dev),
@@ -289,33 +393,20 @@ def main():
     run_sb = lambda: rga.shade_backward(av.h, env, inp["cam_pos"], d_col, texel_to_dir=t2d, gamma=inp["gamma"], use_visibility=True, **sb)
     for _ in range(3):
         run_sb()
-    ms_sb = timed(run_sb, 20)
-    n_grad = int((d_col.abs().sum(1) > 0).sum().item())
-    sb_obj = {"ms": ms_sb, "gaussians_with_gradient": n_grad, "texels": ne_all,
-              "note": "albedo, roughness, specular, normal, position and environment-map gradients; env table rebuilt inside the call"}
-
-    # ... and Eq.5, the image loss that produces dL/dimage (target: a seeded stand-in image of the same size)
+    out["shade_backward"] = {"ms": b.timed(run_sb, 20), "gaussians_with_gradient": int((d_col.abs().sum(1) > 0).sum().item())}
     _, tgt_np = workloads.make_image_pair(1, camc.width, camc.height)
     tgt_d = torch.as_tensor(tgt_np).to(dev); loss_d = torch.zeros(3, device=dev)
     run_il = lambda: rga.image_loss(av.h, img, tgt_d, 0.2, loss_d, dLdI)
     for _ in range(3):
         run_il()
-    ms_il = timed(run_il, 20)
-    il_obj = {"ms": ms_il, "pixels": int(camc.width * camc.height), "lambda": 0.2}
-
-    # ... and the regularisers Eq.6-9 with their gradients
-    nv_all = len(inp["vert_pos"])
+    out["image_loss"] = {"ms": b.timed(run_il, 20)}
     rg = dict(out_losses=torch.zeros(4, device=dev), out_dalbedo=torch.empty((nv_all, 3), device=dev), out_drough=torch.empty(nv_all, device=dev),
               out_dspec=torch.empty(nv_all, device=dev), out_dgauss_pos=torch.empty((ng_all, 3), device=dev),
               out_ddisp=torch.empty((nv_all, 3), device=dev), out_dscale=torch.empty((ng_all, 3), device=dev))
     run_rg = lambda: rga.regularisers(av.h, 0.005, **rg)
     for _ in range(3):
         run_rg()
-    rg_obj = {"ms": timed(run_rg, 20), "vertices": nv_all, "gaussians": ng_all}
-
-    # ... the pull-back to the canonical parameters (H2 + Eq.1), and the whole backward chain of one training view:
-    # image_loss -> splat_backward -> shade_backward -> pose_backward, each fed by the previous call
-    nb_all = inp["bone_mats"].shape[1]
+    out["regularisers"] = {"ms": b.timed(run_rg, 20)}
     pb_out = {"d_gauss_pos": torch.empty((ng_all, 3), device=dev), "d_gauss_quat": torch.empty((ng_all, 4), device=dev),
               "d_gauss_scale": torch.empty((ng_all, 3), device=dev), "d_bones": torch.empty((nb_all, 12), device=dev),
               "d_vert_disp": torch.empty((nv_all, 3), device=dev), "d_vert_normal": torch.empty((nv_all, 3), device=dev),
@@ -326,47 +417,17 @@ def main():
     run_pb = lambda: rga.pose_backward(av.h, bones, pb_in, pb_out)
     for _ in range(3):
         run_pb()
-    ms_pb = timed(run_pb, 20)
+    ms_pb = b.timed(run_pb, 20)
+
     def run_chain():
         run_il(); run_bwd(); run_sb(); run_pb()
     for _ in range(3):
         run_chain()
-    l_chain = rga.rga_launch_count(av.h)
-    ms_chain = timed(run_chain, 20)
-    l_chain = (rga.rga_launch_count(av.h) - l_chain) // 20
-    train_obj = {"pose_backward_ms": ms_pb, "backward_chain_ms": ms_chain, "launches": int(l_chain),
-                 "note": "image_loss + splat_backward + shade_backward + pose_backward of the rendered view; forward frame = ms_per_step"}
-
-    # algorithmic units of each candidate dominant kernel: counted from the frame that was rendered
-    gp = av.read("GAUSS_POSED").reshape(-1, 4)[:, :3]; gn = av.read("GAUSS_NORMAL_POSED").reshape(-1, 4)[:, :3]
-    front = int((((inp["cam_pos"][None, :] - gp) * gn).sum(1) >= 0).sum())
-    rg = av.read("TILE_RANGES").reshape(-1, 2).astype(np.int64)
-    # (inside rga_render_frame the mode-0 depth test runs for the camera-facing Gaussians only; with the back-face option
-    # about half of the (triangle, direction) units stop after projection and the area test: 0.5 x 220 + 0.5 x 50)
-    units = {"shade": front * 512 * 0.5, "vis_depth_test": (front if args.vis_mode == 0 else len(gp)) * K, "vis_raster": len(inp["faces"]) * K,
-             "composite_segments": float(((rg[:, 1] - rg[:, 0]) * 256).sum())}
-    dom = max((k for k in kern_ms if k in units), key=lambda k: kern_ms[k])
-    fpu = dict(FLOP_PER_UNIT)
-    if cull:
-        fpu["vis_raster"] = 135.0
-    ach = units[dom] * fpu[dom] / (kern_ms[dom] * 1e-3) / 1e12
-    pk, pk_kind = peaks()
-    fma_meas = rga.rga_measure_fp32_peak()
-    roofline = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "peak_fma_measured": fma_meas, "frac_of_measured": ach / fma_meas if fma_meas > 0 else None,
-                "frac": ach / FP32_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES.get(dom), "traffic_source": NCU_SOURCE.get(dom),
-                "note": "fp32 FMA-pipe peak derived from the guide (148 SM x 128 lanes x 2 x 1.965 GHz); "
-                        "HBM peak %s %.0f GB/s is not the bound of this kernel" % (pk_kind, pk["hbm_gbs"]),
-                "units_per_launch": units[dom], "flop_per_unit": fpu[dom], "kernel_ms": kern_ms[dom]}
-    if cull and args.vis_mode == 0 and dom in NCU_WARP_INST:      # how busy the issue slots are: EXECUTED instructions, not algorithmic work
-        roofline["issue_slots"] = {"executed_warp_inst": NCU_WARP_INST[dom], "source": NCU_SOURCE[dom],
-                                   "frac_of_issue_peak": NCU_WARP_INST[dom] / (kern_ms[dom] * 1e-3) / ISSUE_PEAK}
-
-    # SURVEY 8(f) item 2 (beside the metric): the displacement network d(x, theta) on the tensor cores (tcgen05, TF32)
+    out["train_backward"] = {"pose_backward_ms": ms_pb, "backward_chain_ms": b.timed(run_chain, 20),
+                             "note": "image_loss + splat_backward + shade_backward + pose_backward of the rendered view"}
     mlp = workloads.make_disp_mlp(seed=1)
     mlp_d = {k: (torch.as_tensor(v).to(dev) if isinstance(v, np.ndarray) else v) for k, v in mlp.items()}
-    def run_mlp():
-        rga.displacement_mlp(av.h, mlp_d, mlp_d["theta"])
+    run_mlp = lambda: rga.displacement_mlp(av.h, mlp_d, mlp_d["theta"])
     for _ in range(3):
         run_mlp()
     rga.rga_profile_enable(av.h, True)
@@ -375,66 +436,179 @@ def main():
         run_mlp()
         mlp_t += [t for name, t in rga.rga_profile_read(av.h) if name == "disp_mlp"]
     rga.rga_profile_enable(av.h, False)
-    nvv = len(inp["vert_pos"])
-    mlp_flop = 2.0 * nvv * (2 * mlp["n_freq"] * 256 + 3 * 256 * 256 + 3 * 256)
+    mlp_flop = 2.0 * nv_all * (2 * mlp["n_freq"] * 256 + 3 * 256 * 256 + 3 * 256)
     mlp_ms = float(np.mean(mlp_t))
+    pk, _ = peaks()
     tf32_peak = pk.get("bf16_tflops", 1590.0) * (1.1 / 2.25)          # measured bf16 peak x the guide's nominal tf32 : bf16 ratio
-    mlp_obj = {"kernel": "disp_mlp", "bound": "tensor", "ms": mlp_ms, "achieved": mlp_flop / (mlp_ms * 1e-3) / 1e12, "peak": tf32_peak,
-               "unit": "TFLOP/s", "frac": mlp_flop / (mlp_ms * 1e-3) / 1e12 / tf32_peak, "dtype": "tf32 operands, f32 accumulate",
-               "vertices": nvv, "note": "one CTA per 128 vertices (54 CTAs at config 1), all four layers and the head fused; profiles/r01g_mlp.md"}
-    # (the avatar now carries the network's displacement; it is not rendered again and is closed below)
-
-    # per-frame KNN + Eq.1 re-interpolation for moved Gaussians (the paper's KNN step: 0.93 ms per frame
-    # on an RTX 4090), exact uniform-grid search
+    out["disp_mlp"] = {"kernel": "disp_mlp", "bound": "tensor", "ms": mlp_ms, "achieved": mlp_flop / (mlp_ms * 1e-3) / 1e12, "peak": tf32_peak,
+                       "unit": "TFLOP/s", "frac": mlp_flop / (mlp_ms * 1e-3) / 1e12 / tf32_peak, "dtype": "tf32 operands, f32 accumulate"}
     gp = torch.as_tensor(inp["gauss_pos"]).to(dev)
     for _ in range(3):
         rga.gaussians_update(av.h, gp)
-    ms_knn = timed(lambda: rga.gaussians_update(av.h, gp), 20)
-
-    # Algorithm 1 (density-based densification) over the same avatar; a density
-    # threshold of 12 makes ~45k draws on this (densely covered) synthetic body, the paper's d0 = 1 asks for ~15
+    out["gaussians_update_ms"] = b.timed(lambda: rga.gaussians_update(av.h, gp), 20)
     n_dens = 65536
     d_rnd = torch.randint(-2 ** 31, 2 ** 31 - 1, (3 * n_dens,), dtype=torch.int32, device=dev, generator=torch.Generator(dev).manual_seed(5))
     d_pos = torch.empty((n_dens, 3), dtype=torch.float32, device=dev); d_cnt = torch.zeros(1, dtype=torch.int32, device=dev)
     for _ in range(3):
         rga.densify_density(av.h, 12.0, 0.25, d_rnd, d_pos, None, d_cnt)
-    ms_dens = timed(lambda: rga.densify_density(av.h, 12.0, 0.25, d_rnd, d_pos, None, d_cnt), 20)
-    dens_obj = {"ms": ms_dens, "d0": 12.0, "p0": 0.25, "added": int(d_cnt.item()), "launches": 7}
+    out["densify_density"] = {"ms": b.timed(lambda: rga.densify_density(av.h, 12.0, 0.25, d_rnd, d_pos, None, d_cnt), 20),
+                              "d0": 12.0, "p0": 0.25, "added": int(d_cnt.item())}
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4], help="BASELINE.json config of the main line (default 1, the headline)")
+    ap.add_argument("--vis-mode", type=int, default=0, help="0 = depth test (north_star, default), 1 = paper filters")
+    ap.add_argument("--all-configs", type=int, default=1, help="1 (default): also time all five configs -> `configs`")
+    ap.add_argument("--next", type=int, default=1, help="1 (default): also time the SURVEY 8(f) rows")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        if args.steps == 200 and args.warmup == 20:
+            args.steps, args.warmup = 10, 1
+        return run_reference(args, rank)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2407_10707_b200 import binding as rga
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    dev = torch.device("cuda", local)
+    cfg = args.config
+    b = Bench(cfg, args.vis_mode, dev, world=world, rank=rank, morton=False)
+    inp, av, W, H = b.inp, b.av, b.W, b.H
+    nfr = len(inp["bone_mats"])
+    steps = args.steps if cfg in (0, 1, 3) else max(10, min(args.steps, 40))
+    it = [0]
+
+    def frame():                                                # config 3 walks its pose sequence; the others have one pose
+        b.frame(it[0] % nfr); it[0] += 1
+
+    for _ in range(args.warmup):
+        frame()
+    rga.rga_check(av.h)
+    l0 = rga.rga_launch_count(av.h)
+    cs = ClockSampler(local); cs.__enter__()                     # sampled through every timed pass below
+    ms = b.timed(frame, steps)
+    launches = (rga.rga_launch_count(av.h) - l0) / steps
+    ms_warm = b.timed(frame, steps, do_flush=False)
+
+    # end to end: host (pinned) pose + env in, image out, every step, through the same C-ABI call
+    h_bones = torch.as_tensor(inp["bone_mats"][0]).pin_memory(); h_env = torch.as_tensor(inp["env"][0]).pin_memory()
+    h_img = torch.empty((H, W, 3), dtype=torch.float32).pin_memory()
+    d_bones = torch.empty_like(b.bones[0]); d_env = torch.empty_like(b.envs[0])
+
+    def frame_e2e():
+        d_bones.copy_(h_bones, non_blocking=True); d_env.copy_(h_env, non_blocking=True)
+        b.frame(0, bones=d_bones, env=d_env)
+        h_img.copy_(b.img, non_blocking=True)
+    for _ in range(3):
+        frame_e2e()
+    ms_e2e = b.timed(frame_e2e, steps)
+
+    # the documented viewer loop: the image read-back of step i on a copy stream beside step i+1 (two image buffers).
+    # Reported as e2e.pipelined_value; e2e.value stays the serial number above.
+    copy_stream = torch.cuda.Stream(device=dev)
+    imgs = [torch.empty_like(b.img) for _ in range(2)]
+    h_imgs = [torch.empty((H, W, 3), dtype=torch.float32).pin_memory() for _ in range(2)]
+    copied = [None, None]
+
+    def run_pipelined(n):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        last_copy = None
+        b.barrier()
+        for i, (a, e) in enumerate(evs):
+            b.flush.fill_(1)
+            a.record()
+            if copied[i & 1] is not None:
+                torch.cuda.current_stream().wait_event(copied[i & 1])     # buffer i&1 has been read back
+            d_bones.copy_(h_bones, non_blocking=True); d_env.copy_(h_env, non_blocking=True)
+            b.frame(0, bones=d_bones, env=d_env, img=imgs[i & 1])
+            e.record()
+            copy_stream.wait_event(e)
+            with torch.cuda.stream(copy_stream):
+                h_imgs[i & 1].copy_(imgs[i & 1], non_blocking=True)
+                copied[i & 1] = torch.cuda.Event(enable_timing=True); copied[i & 1].record()
+                last_copy = copied[i & 1]
+        b.barrier(); copy_stream.synchronize()
+        tail = max(evs[-1][1].elapsed_time(last_copy), 0.0)                # the last read-back is not hidden by a next step
+        return (sum(a.elapsed_time(e) for a, e in evs) + tail) / n
+    run_pipelined(3)
+    ms_e2e_pipe = run_pipelined(steps)
+
+    kern_ms = b.kernel_times(steps)
+    rga.rga_check(av.h)
+    t_end = time.time() + 1.0                                      # at least a second of load for the sampler
+    while time.time() < t_end or len(cs.rows) < 3:
+        for _ in range(50):
+            frame()
+        torch.cuda.synchronize()
+        if time.time() > t_end + 5.0:
+            break
+    cs.__exit__(); clocks = cs.summary()
+    b.frame(0)
+    units = b.units()
+    pk, pk_src = peaks()
+    fma_meas = rga.rga_measure_fp32_peak()
+    roofline = roofline_list(kern_ms, units, fma_meas, pk["hbm_gbs"], pk_src)
+
+    # the rasteriser's closed-mesh option (reading A36) -- NOT the contract path, reported beside it
+    for _ in range(3):
+        b.frame(0, cull=True)
+    ms_cull = b.timed(lambda: b.frame(0, cull=True), max(steps // 4, 10))
+    extra = next_rows(b, steps) if (args.next and world == 1 and cfg == 1) else {}
+    b.close()
+
+    ms_sorted = None
+    if world == 1:                                                 # the same frame with the Gaussians in spatial (Morton) order
+        bs = Bench(cfg, args.vis_mode, dev, morton=True, flush=b.flush)
+        for _ in range(args.warmup):
+            bs.frame(0)
+        ms_sorted = bs.timed(lambda: bs.frame(0), max(steps // 2, 10))
+        bs.close()
 
     from paper_2407_10707_b200 import replica
     ms, ms_e2e, ms_warm = replica.max_over_ranks([ms, ms_e2e, ms_warm], device=dev)      # slowest rank sets the job time
     out = {
-        "metric": METRIC, "value": world * 1e3 / ms, "unit": "frames/s", "n_gpus": world, "steps": args.steps,
+        "metric": METRIC, "value": world * 1e3 / ms, "unit": "frames/s", "n_gpus": world, "steps": steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "vis_mode": args.vis_mode, "vis_cull_backfaces": cull,
-                   "mesh": "closed, outward-oriented (the depth rasteriser may skip faces turned away from the light)",
+        "config": {"workload": WORKLOADS[cfg], "vis_mode": args.vis_mode, "vis_cull_backfaces": False,
+                   "gaussian_order": "generator order (random surface points, unsorted)",
                    "l2": "flushed between steps (256 MiB fill)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU", "paper_context": "6.9 fps on RTX 4090 (PAPER.md:314)"},
-        "clocks": clocks, "gpu_launches": int(launches),
+        "clocks": clocks, "gpu_launches": int(round(launches * steps)), "gpu_launches_per_step": launches,
         "e2e": {"value": world * 1e3 / ms_e2e, "unit": "frames/s", "h2d_bytes_per_step": int(h_bones.numel() * 4 + h_env.numel() * 4),
                 "d2h_bytes_per_step": int(h_img.numel() * 4),
                 "pipelined_value": world * 1e3 / ms_e2e_pipe,
-                "pipelined_note": "image read-back of step i on a copy stream beside step i+1; per-step events plus the last copy's tail"},
-        "roofline": roofline, "kernel_ms": kern_ms, "warm_l2_fps": world * 1e3 / ms_warm, "avatar_load_ms": load_ms,
-        "value_all_triangles": (world * 1e3 / ms_nocull) if ms_nocull else None,
-        "disp_mlp": mlp_obj, "gaussians_update_ms": ms_knn, "densify_density": dens_obj, "splat_backward": bwd_obj, "shade_backward": sb_obj, "image_loss": il_obj, "regularisers": rg_obj, "train_backward": train_obj,
-        "amortised": {"views_per_pose": NV, "views_per_s": world * NV * 1e3 / ms_views, "ms_per_pose": ms_views},
+                "pipelined_note": "the documented viewer loop: image read-back of step i on a copy stream beside step i+1"},
+        "roofline": roofline, "kernel_ms": kern_ms, "stage_ms": stage_ms(kern_ms), "warm_l2_fps": world * 1e3 / ms_warm,
+        "avatar_load_ms": b.load_ms,
+        "value_unsorted": world * 1e3 / ms, "value_spatially_sorted_input": (1e3 / ms_sorted) if ms_sorted else None,
+        "value_cull_backfaces": world * 1e3 / ms_cull,
+        "workload_stats": {k[1:]: v for k, v in units.items() if k.startswith("_")},
     }
+    out.update(extra)
+    if rank == 0 and world == 1 and args.all_configs:
+        flush = b.flush
+        out["configs"] = {}
+        for c in range(5):
+            out["configs"][str(c)] = bench_config(c, args.vis_mode, dev, max(5, min(args.steps, 20 if c in (2, 4) else 50)), 3, flush)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        from oracle import oracle as orc                 # cpu_baseline leg: the oracle, untuned, on the host cores
-        inp["vis_cull_backfaces"] = cull
-        oav = orc.avatar_load(inp)
-        orc.render_frame(oav, inp, vis_mode=args.vis_mode)
-        n, t0 = 0, time.perf_counter()
-        while n < 3 or (time.perf_counter() - t0 < 10.0 and n < 50):
-            orc.render_frame(oav, inp, vis_mode=args.vis_mode); n += 1
-        dt = (time.perf_counter() - t0) / n
-        out["cpu_baseline"] = {"value": 1.0 / dt, "unit": "frames/s", "cores": os.cpu_count(), "kind": "oracle",
-                               "sample": "%d full frames of configs[1], all steps, OpenMP outer loops" % n}
+        out["cpu_baseline"] = oracle_times(inp, args.vis_mode)     # the oracle is imported only here, after every timed region
     if rank == 0:
         print(json.dumps(out))
-    av.close()
     if world > 1:
         dist.destroy_process_group()
 

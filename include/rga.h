@@ -301,14 +301,24 @@ typedef enum {
   RGA_BUF_DENS_NG = 32,       /* i32 [n_faces]  Gaussians added per triangle by the last call          */
   RGA_BUF_DENS_HDR = 33,      /* u64 [2]        sum of the fixed-point P, N'                            */
   RGA_BUF_SPLAT_GRAD = 34,    /* f32 [n_gauss][12] splat_backward: d_colour(3), d_opacity, d_mu2D(2), d_conic(3), pad(3) */
-  RGA_BUF_COUNT_ = 35
+  RGA_BUF_GAUSS_ORDER = 35,   /* i32 [n_gauss] caller index of the i-th Gaussian in the library's internal (spatial) order */
+  RGA_BUF_COUNT_ = 36
 } rga_buffer_id;
 
-/* Returns the device pointer and current size in bytes of an internal buffer (valid until the next call that
+/* Gaussian order.  PAPER.md:88-93 defines no order of the Gaussians and a trained asset's is arbitrary, so avatar_load sorts
+ * them ONCE by the Morton code of their canonical position and keeps the permutation (RGA_BUF_GAUSS_ORDER); gaussians_update
+ * keeps it.  Every array the CALLER passes or receives is in the caller's order: the rga_avatar_desc tables, gaussians_update's
+ * positions, every [n_gauss] gradient input / output of the backward calls, the Gaussian indices in RGA_BUF_VALS_SORTED
+ * (equal (tile, depth) keys order by the caller's index) and whatever rga_read_buffer copies to the host.  Only the DEVICE
+ * pointers rga_get_buffer returns for the per-Gaussian buffers ([n_gauss][...] rows above) address the library's internal
+ * order: row i belongs to the caller's Gaussian RGA_BUF_GAUSS_ORDER[i].
+ *
+ * Returns the device pointer and current size in bytes of an internal buffer (valid until the next call that
  * rewrites it).  For data-dependent sizes (KEYS/VALS) this synchronises `stream` to read D. */
 RGA_API rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, const void** dev_ptr, size_t* bytes);
 
-/* Copies an internal buffer to HOST memory `host_dst` (capacity bytes); *bytes = size copied.  Synchronises `stream`.
+/* Copies an internal buffer to HOST memory `host_dst` (capacity bytes), per-Gaussian rows put back into the caller's order;
+ * *bytes = size copied.  Synchronises `stream`.
  * RGA_ERR_INVALID_ARG if capacity is too small (then *bytes holds the required size). */
 RGA_API rga_status rga_read_buffer(rga_avatar* av, int which, void* stream, void* host_dst, size_t capacity, size_t* bytes);
 

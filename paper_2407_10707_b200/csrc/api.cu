@@ -56,7 +56,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
+  void* ptrs[] = {av->g_order, av->g_inv, av->gi_pos, av->bb_scratch, av->bb_dev, av->vals[1], av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
                   av->vt_spec, av->knn_d2, av->grid_start, av->grid_verts, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
@@ -128,7 +128,8 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->mu2d, ng)); A(dalloc(&av->depth, ng)); A(dalloc(&av->conic_o, ng)); A(dalloc(&av->rect, ng)); A(dalloc(&av->touched, ng));
   A(dalloc(&av->tile_count, ntiles)); A(dalloc(&av->cursor, ntiles));
   A(dalloc(&av->keys[0], (size_t)av->max_dup)); A(dalloc(&av->keys[1], (size_t)av->max_dup));
-  A(dalloc(&av->vals[0], (size_t)av->max_dup));
+  A(dalloc(&av->vals[0], (size_t)av->max_dup)); A(dalloc(&av->vals[1], (size_t)av->max_dup));
+  A(dalloc(&av->g_order, ng)); A(dalloc(&av->g_inv, ng)); A(dalloc(&av->gi_pos, 3 * ng)); A(dalloc(&av->bb_scratch, 8)); A(dalloc(&av->bb_dev, 8));
   A(dalloc(&av->num_dup, 1)); A(dalloc(&av->ranges, ntiles));
   av->items_cap = av->max_dup / RGA_SEG + (long long)ntiles + 1;
   A(dalloc(&av->seg_off, ntiles + 1)); A(dalloc(&av->num_items, 1)); A(dalloc(&av->item_tab, (size_t)av->items_cap));
@@ -165,22 +166,34 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   // KNN: S_v = K_v nearest vertices of each vertex (self included), S_g = K_g nearest of each Gaussian
   A(dalloc(&d2, nv * av->k_v));
   {
-    // canonical-vertex AABB for the KNN grid: one pass over a host copy (load time)
-    float* hv = (float*)malloc(3 * nv * sizeof(float));
-    if (!hv) { st = fail(RGA_ERR_OOM, "avatar_load: host allocation"); goto done; }
-    cudaError_t ce = cudaMemcpyAsync(hv, av->vt_pos, 3 * nv * sizeof(float), cudaMemcpyDeviceToHost, s);
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
-    float bb[6] = {1e30f, 1e30f, 1e30f, -1e30f, -1e30f, -1e30f};
-    if (ce == cudaSuccess)
-      for (size_t i = 0; i < nv; ++i)
-        for (int c = 0; c < 3; ++c) { float x = hv[3 * i + c]; if (x < bb[c]) bb[c] = x; if (x > bb[3 + c]) bb[3 + c] = x; }
-    free(hv);
-    if (ce != cudaSuccess) { st = fail(RGA_ERR_CUDA, "avatar_load: %s", cudaGetErrorString(ce)); goto done; }
+    // canonical-vertex AABB for the KNN grid: device reduction, six floats read back (load time)
+    float bb[6];
+    A(rga_points_aabb(av->vt_pos, av->n_verts, av->bb_scratch, av->bb_dev, s));
+    A(cudaMemcpyAsync(bb, av->bb_dev, sizeof bb, cudaMemcpyDeviceToHost, s));
+    A(cudaStreamSynchronize(s));
     A(rga_build_knn_grid(av, bb, s));
   }
   A(rga_launch_knn_verts(av, d2, s));
-  A(rga_launch_knn_gauss(av, d->gauss_pos, s));
-  A(rga_launch_load_gauss(av, d->gauss_pos, d->gauss_quat, d->gauss_scale, d->gauss_opacity, av->knn_d2, s));
+  {
+    // Gaussian order (order_kernels.cu): sort once by the Morton code of the canonical position; the caller's per-Gaussian
+    // arrays are gathered into library order and every table below is built from those copies
+    int npad = 2048; while (npad < av->n_gauss) npad <<= 1;
+    unsigned long long* okeys = nullptr; float *pq = nullptr, *ps = nullptr, *po = nullptr;
+    cudaError_t e_ = dalloc(&okeys, (size_t)npad);
+    if (e_ == cudaSuccess) e_ = dalloc(&pq, 4 * ng);
+    if (e_ == cudaSuccess) e_ = dalloc(&ps, 3 * ng);
+    if (e_ == cudaSuccess && d->gauss_opacity) e_ = dalloc(&po, ng);
+    if (e_ == cudaSuccess) e_ = rga_build_gauss_order(d->gauss_pos, av->n_gauss, okeys, npad, av->bb_scratch, av->bb_dev, av->g_order, av->g_inv, s);
+    if (e_ == cudaSuccess) e_ = rga_gather_rows(av->n_gauss, 3, d->gauss_pos, av->g_order, av->gi_pos, s);
+    if (e_ == cudaSuccess) e_ = rga_gather_rows(av->n_gauss, 4, d->gauss_quat, av->g_order, pq, s);
+    if (e_ == cudaSuccess) e_ = rga_gather_rows(av->n_gauss, 3, d->gauss_scale, av->g_order, ps, s);
+    if (e_ == cudaSuccess && po) e_ = rga_gather_rows(av->n_gauss, 1, d->gauss_opacity, av->g_order, po, s);
+    if (e_ == cudaSuccess) e_ = rga_launch_knn_gauss(av, av->gi_pos, s);
+    if (e_ == cudaSuccess) e_ = rga_launch_load_gauss(av, av->gi_pos, pq, ps, po, av->knn_d2, s);
+    if (e_ == cudaSuccess) e_ = cudaStreamSynchronize(s);
+    cudaFree(okeys); cudaFree(pq); cudaFree(ps); cudaFree(po);
+    if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, "avatar_load: Gaussian order / tables: %s", cudaGetErrorString(e_)); goto done; }
+  }
   av->launches += 5;
   if (rga_shade_init_attributes(av->max_env) != 0 || rga_shade_backward_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_composite_init_attributes() != 0 || rga_mlp_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
   A(cudaStreamSynchronize(s));
@@ -262,11 +275,14 @@ extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, v
   cudaStream_t s = (cudaStream_t)stream;
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
   rga_prof_mark(av, "-", s);
-  CU(rga_launch_knn_gauss(av, gauss_pos, s));
+  CU(rga_gather_rows(av->n_gauss, 3, gauss_pos, av->g_order, av->gi_pos, s));      // caller order -> library order (kept from the load)
+  CU(rga_launch_knn_gauss(av, av->gi_pos, s));
   rga_prof_mark(av, "knn_g", s);
-  CU(rga_launch_load_gauss(av, gauss_pos, nullptr, nullptr, nullptr, av->knn_d2, s));
+  CU(rga_launch_load_gauss(av, av->gi_pos, nullptr, nullptr, nullptr, av->knn_d2, s));
   rga_prof_mark(av, "load_gauss", s);
-  av->launches += 2;
+  av->launches += 3;
+  // the displacement network's per-pose dx (if it is the current displacement) is re-interpolated over the new S_g
+  if (av->disp_is_mlp) CU(rga_launch_disp_apply(av, s));
   return RGA_OK;
 }
 
@@ -497,10 +513,21 @@ extern "C" rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, co
     case RGA_BUF_DENS_P: p = av->dens_pfix; n = (size_t)av->n_faces * 4; break;
     case RGA_BUF_DENS_NG: p = av->dens_ng; n = (size_t)av->n_faces * 4; break;
     case RGA_BUF_DENS_HDR: p = av->dens_hdr; n = 16; break;
+    case RGA_BUF_GAUSS_ORDER: p = av->g_order; n = ng * 4; break;
     default: return fail(RGA_ERR_INVALID_ARG, "rga_get_buffer: unknown id %d", which);
   }
   *dev_ptr = p; *bytes = n;
   return RGA_OK;
+}
+
+static bool per_gaussian_buffer(int which) {
+  switch (which) {
+    case RGA_BUF_KNN_G: case RGA_BUF_UBAR_G: case RGA_BUF_GAUSS_STATIC: case RGA_BUF_GAUSS_SKIN_W: case RGA_BUF_GAUSS_POSED:
+    case RGA_BUF_GAUSS_NORMAL_POSED: case RGA_BUF_GAUSS_COV: case RGA_BUF_VISBITS: case RGA_BUF_RADIANCE: case RGA_BUF_COLOR:
+    case RGA_BUF_MU2D: case RGA_BUF_DEPTH: case RGA_BUF_CONIC_OPACITY: case RGA_BUF_RECT: case RGA_BUF_TOUCHED: case RGA_BUF_SPLAT_GRAD:
+      return true;
+    default: return false;
+  }
 }
 
 extern "C" rga_status rga_read_buffer(rga_avatar* av, int which, void* stream, void* host_dst, size_t capacity, size_t* bytes) {
@@ -509,7 +536,19 @@ extern "C" rga_status rga_read_buffer(rga_avatar* av, int which, void* stream, v
   if (st != RGA_OK) return st;
   if (bytes) *bytes = n;
   if (!host_dst || capacity < n) return fail(RGA_ERR_INVALID_ARG, "rga_read_buffer: need %zu bytes", n);
-  if (n) CU(cudaMemcpyAsync(host_dst, p, n, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
-  CU(cudaStreamSynchronize((cudaStream_t)stream));
+  cudaStream_t s = (cudaStream_t)stream;
+  if (n && per_gaussian_buffer(which)) {
+    // per-Gaussian tables live in the library's spatial order: rows are put back into the CALLER's order on the way out
+    void* tmp = nullptr;
+    CU(cudaMalloc(&tmp, n));
+    cudaError_t e = rga_scatter_rows(av->n_gauss, (int)(n / 4 / (size_t)av->n_gauss), p, av->g_order, tmp, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(host_dst, tmp, n, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return fail(RGA_ERR_CUDA, "rga_read_buffer: %s", cudaGetErrorString(e));
+    return RGA_OK;
+  }
+  if (n) CU(cudaMemcpyAsync(host_dst, p, n, cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
   return RGA_OK;
 }

@@ -160,9 +160,11 @@ struct CamB { float R[9], t[3], fx, fy, limx, limy; };
 
 __global__ void __launch_bounds__(256) project_backward_kernel(int ng, CamB cam, const float4* __restrict__ g_posed,
     const float* __restrict__ g_cov, const float4* __restrict__ conic_o, const unsigned* __restrict__ touched, float* __restrict__ grad,
-    float* __restrict__ out_dcolor, float* __restrict__ out_dopacity, float* __restrict__ out_dmean, float* __restrict__ out_dcov) {
+    float* __restrict__ out_dcolor, float* __restrict__ out_dopacity, float* __restrict__ out_dmean, float* __restrict__ out_dcov,
+    const int* __restrict__ order) {
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= ng) return;
+  const int gc = order[g];                 // the caller's index: [n_gauss] outputs are written in the caller's order
   float* gr = grad + 12 * (size_t)g;
   float dcol[3] = {gr[0], gr[1], gr[2]}, dop = 0.f, dmean[3] = {0.f, 0.f, 0.f}, dcov[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   float dmx = 0.f, dmy = 0.f, dA = 0.f, dB = 0.f, dC = 0.f;
@@ -219,12 +221,12 @@ __global__ void __launch_bounds__(256) project_backward_kernel(int ng, CamB cam,
     dcol[0] = dcol[1] = dcol[2] = 0.f;
   }
   gr[3] = dop; gr[4] = dmx; gr[5] = dmy; gr[6] = dA; gr[7] = dB; gr[8] = dC;      // the buffer now holds d_opacity, d_mu, d_conic
-  if (out_dcolor) { out_dcolor[3 * (size_t)g] = dcol[0]; out_dcolor[3 * (size_t)g + 1] = dcol[1]; out_dcolor[3 * (size_t)g + 2] = dcol[2]; }
-  if (out_dopacity) out_dopacity[g] = dop;
-  if (out_dmean) { out_dmean[3 * (size_t)g] = dmean[0]; out_dmean[3 * (size_t)g + 1] = dmean[1]; out_dmean[3 * (size_t)g + 2] = dmean[2]; }
+  if (out_dcolor) { out_dcolor[3 * (size_t)gc] = dcol[0]; out_dcolor[3 * (size_t)gc + 1] = dcol[1]; out_dcolor[3 * (size_t)gc + 2] = dcol[2]; }
+  if (out_dopacity) out_dopacity[gc] = dop;
+  if (out_dmean) { out_dmean[3 * (size_t)gc] = dmean[0]; out_dmean[3 * (size_t)gc + 1] = dmean[1]; out_dmean[3 * (size_t)gc + 2] = dmean[2]; }
   if (out_dcov) {
 #pragma unroll
-    for (int k = 0; k < 6; ++k) out_dcov[6 * (size_t)g + k] = dcov[k];
+    for (int k = 0; k < 6; ++k) out_dcov[6 * (size_t)gc + k] = dcov[k];
   }
 }
 
@@ -234,7 +236,7 @@ cudaError_t rga_launch_splat_backward(rga_avatar* av, const rga_camera* cam, flo
   cudaError_t e = cudaMemsetAsync(av->splat_grad, 0, sizeof(float) * 12 * (size_t)av->n_gauss, s);
   if (e != cudaSuccess) return e;
   composite_backward_kernel<<<av->num_sms * 4, BB, 0, s>>>(cam->width, cam->height, TX, bg, av->num_items, av->item_tab, av->seg_off,
-                                                           av->ranges, av->vals[0], av->mu2d, av->conic_o, av->color, av->part,
+                                                           av->ranges, av->vals[1], av->mu2d, av->conic_o, av->color, av->part,
                                                            av->n_contrib, image, dL_dimage, av->splat_grad);
   rga_prof_mark(av, "composite_backward", s);
   CamB k;
@@ -243,7 +245,7 @@ cudaError_t rga_launch_splat_backward(rga_avatar* av, const rga_camera* cam, flo
   k.fx = cam->fx; k.fy = cam->fy;
   k.limx = 1.3f * ((float)cam->width / (2.0f * cam->fx)); k.limy = 1.3f * ((float)cam->height / (2.0f * cam->fy));
   project_backward_kernel<<<(av->n_gauss + 255) / 256, 256, 0, s>>>(av->n_gauss, k, av->g_posed, av->g_cov, av->conic_o, av->touched,
-                                                                    av->splat_grad, out_dcolor, out_dopacity, out_dmean, out_dcov);
+                                                                    av->splat_grad, out_dcolor, out_dopacity, out_dmean, out_dcov, av->g_order);
   rga_prof_mark(av, "project_backward", s);
   av->launches += 2;
   return cudaGetLastError();

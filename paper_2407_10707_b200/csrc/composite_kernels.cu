@@ -87,7 +87,8 @@ __device__ __forceinline__ void bitonic_sort(unsigned long long* buf, int n) {
 
 __device__ __forceinline__ void sort_tile(int tile, unsigned capacity, int scap, unsigned long long* s_keys,
     const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, unsigned long long* __restrict__ lkeys,
-    unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ item_tab) {
+    unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ vals_int,
+    const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
   uint2 rg = ranges[tile];
   rg.x = min(rg.x, capacity); rg.y = min(rg.y, capacity);
   const int n = (int)(rg.y - rg.x);
@@ -103,7 +104,8 @@ __device__ __forceinline__ void sort_tile(int tile, unsigned capacity, int scap,
   for (int i = threadIdx.x; i < n; i += SORT_THREADS) {      // the sorted (tile, depth) keys and values (H8 output)
     const unsigned long long k = buf[i];
     keys_out[rg.x + i] = ((unsigned long long)(unsigned)tile << 32) | (k >> 32);
-    vals_out[rg.x + i] = (unsigned)k;
+    vals_out[rg.x + i] = (unsigned)k;                               // caller's index (H8 output)
+    vals_int[rg.x + i] = (unsigned)inv[(unsigned)k];                // the same Gaussian in library order (what the blend reads)
   }
   __syncthreads();
 }
@@ -111,12 +113,13 @@ __device__ __forceinline__ void sort_tile(int tile, unsigned capacity, int scap,
 // one CTA per tile; tiles with more than SCAP_SMALL entries are left to tile_sort_long_kernel
 __global__ void __launch_bounds__(SORT_THREADS) tile_sort_kernel(unsigned capacity, int scap,
     const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, unsigned long long* __restrict__ lkeys,
-    unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ item_tab) {
+    unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ vals_int,
+    const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
   extern __shared__ __align__(16) unsigned long long s_keys[];
   const uint2 rg = ranges[blockIdx.x];
   const unsigned n = min(rg.y, capacity) - min(rg.x, capacity);
   if (n == 0 || n > (unsigned)scap) return;
-  sort_tile(blockIdx.x, capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, item_tab);
+  sort_tile(blockIdx.x, capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, vals_int, inv, item_tab);
 }
 
 // the tiles listed by tile_scan_kernel as long (usually none): persistent CTAs with the large shared-memory buffer;
@@ -124,11 +127,11 @@ __global__ void __launch_bounds__(SORT_THREADS) tile_sort_kernel(unsigned capaci
 __global__ void __launch_bounds__(SORT_THREADS) tile_sort_long_kernel(unsigned capacity, int scap, const unsigned* __restrict__ num_long,
     const unsigned* __restrict__ long_list, const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off,
     unsigned long long* __restrict__ lkeys, unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out,
-    unsigned* __restrict__ item_tab) {
+    unsigned* __restrict__ vals_int, const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
   extern __shared__ __align__(16) unsigned long long s_keys[];
   const unsigned nl = *num_long;
   for (unsigned q = blockIdx.x; q < nl; q += gridDim.x)
-    sort_tile((int)long_list[q], capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, item_tab);
+    sort_tile((int)long_list[q], capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, vals_int, inv, item_tab);
 }
 
 // Thread -> pixel of the 16x16 tile: a warp owns an 8x4 block of pixels (2 x 4 blocks per tile), so that a Gaussian
@@ -397,10 +400,10 @@ cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStre
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
   const int ntiles = TX * TY;
   tile_sort_kernel<<<ntiles, SORT_THREADS, SCAP_SMALL * 8, s>>>((unsigned)av->max_dup, SCAP_SMALL, av->ranges, av->seg_off, av->keys[0],
-                                                           av->keys[1], av->vals[0], av->item_tab);
+                                                           av->keys[1], av->vals[0], av->vals[1], av->g_inv, av->item_tab);
   rga_prof_mark(av, "tile_sort", s);
   tile_sort_long_kernel<<<av->num_sms, SORT_THREADS, SCAP_LARGE * 8, s>>>((unsigned)av->max_dup, SCAP_LARGE, av->num_long, av->long_list,
-      av->ranges, av->seg_off, av->keys[0], av->keys[1], av->vals[0], av->item_tab);
+      av->ranges, av->seg_off, av->keys[0], av->keys[1], av->vals[0], av->vals[1], av->g_inv, av->item_tab);
   rga_prof_mark(av, "tile_sort_long", s);
   av->launches += 2;
   return cudaGetLastError();
@@ -410,13 +413,13 @@ cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStre
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, const float4* color, float* out, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
   composite_segment_kernel<<<av->num_sms * SEGMENT_GRID_MULT, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
-      av->ranges, av->vals[0], av->mu2d, av->conic_o, color, av->part, av->part_last);
+      av->ranges, av->vals[1], av->mu2d, av->conic_o, color, av->part, av->part_last);
   rga_prof_mark(av, "composite_segments", s);
   composite_resolve_kernel<<<dim3(TX, TY), CB, 0, s>>>(cam->width, cam->height, TX, (unsigned)av->max_dup, av->ranges, av->seg_off,
       av->part, av->part_last, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
   rga_prof_mark(av, "composite_resolve", s);
   composite_replay_kernel<<<av->num_sms * REPLAY_GRID_MULT, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
-      av->ranges, av->vals[0], av->mu2d, av->conic_o, color, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
+      av->ranges, av->vals[1], av->mu2d, av->conic_o, color, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);
   rga_prof_mark(av, "composite_replay", s);
   av->launches += 3;
   return cudaGetLastError();

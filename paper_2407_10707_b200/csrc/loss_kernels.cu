@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(256) reg_vertex_kernel(int nv, int Kv, const f
 
 __global__ void __launch_bounds__(256) reg_gauss_kernel(int ng, int Kg, float s0, const float4* __restrict__ g_pos, const float* __restrict__ v_pos,
     const int* __restrict__ knn_g, const float4* __restrict__ g_scale_op, float* __restrict__ d_gpos, float* __restrict__ d_scale,
-    double* __restrict__ sums) {
+    double* __restrict__ sums, const int* __restrict__ order) {
   __shared__ float s_red[8];
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   float md = 0.f, sc = 0.f;
@@ -216,11 +216,12 @@ __global__ void __launch_bounds__(256) reg_gauss_kernel(int ng, int Kg, float s0
       const float n2 = dx * dx + dy * dy + dz * dz;
       if (n2 > 0.f) { const float l = sqrtf(n2), inv = 1.f / l; md += l; gx += dx * inv; gy += dy * inv; gz += dz * inv; }
     }
-    if (d_gpos) { d_gpos[3 * g] = gx; d_gpos[3 * g + 1] = gy; d_gpos[3 * g + 2] = gz; }
+    const size_t gc = (size_t)order[g];        // gradients go out in the caller's order
+    if (d_gpos) { d_gpos[3 * gc] = gx; d_gpos[3 * gc + 1] = gy; d_gpos[3 * gc + 2] = gz; }
     const float4 s = g_scale_op[g];
     const float e0 = s.x - s0, e1 = s.y - s0, e2 = s.z - s0;
     sc = fmaxf(e0, 0.f) + fmaxf(e1, 0.f) + fmaxf(e2, 0.f);
-    if (d_scale) { d_scale[3 * g] = e0 > 0.f ? 1.f : 0.f; d_scale[3 * g + 1] = e1 > 0.f ? 1.f : 0.f; d_scale[3 * g + 2] = e2 > 0.f ? 1.f : 0.f; }
+    if (d_scale) { d_scale[3 * gc] = e0 > 0.f ? 1.f : 0.f; d_scale[3 * gc + 1] = e1 > 0.f ? 1.f : 0.f; d_scale[3 * gc + 2] = e2 > 0.f ? 1.f : 0.f; }
   }
   const float t0 = block_sum256(md, s_red), t1 = block_sum256(sc, s_red);
   if (threadIdx.x == 0) { atomicAdd(sums + 1, (double)t0); atomicAdd(sums + 3, (double)t1); }
@@ -242,7 +243,7 @@ cudaError_t rga_launch_regularisers(rga_avatar* av, float s0, float* out_losses,
       av->disp_is_mlp ? av->v_disp : nullptr, av->disp_is_mlp ? nullptr : av->vt_disp, d_alb, d_rough, d_spec, d_disp, av->reg_sums);
   rga_prof_mark(av, "reg_vertex", s);
   reg_gauss_kernel<<<(av->n_gauss + 255) / 256, 256, 0, s>>>(av->n_gauss, av->k_g, s0, av->g_pos, av->vt_pos, av->knn_g, av->g_scale_op,
-      d_gpos, d_scale, av->reg_sums);
+      d_gpos, d_scale, av->reg_sums, av->g_order);
   rga_prof_mark(av, "reg_gauss", s);
   if (out_losses) reg_finish_kernel<<<1, 32, 0, s>>>(av->reg_sums, out_losses);
   av->launches += 2 + (out_losses != nullptr);

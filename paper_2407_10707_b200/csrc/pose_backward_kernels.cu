@@ -34,7 +34,8 @@ __global__ void __launch_bounds__(256) pose_backward_kernel(int ng, int B, int K
     const float* __restrict__ d_mean, const float* __restrict__ d_mean2, const float* __restrict__ d_normal, const float* __restrict__ d_cov, const float* __restrict__ d_alb,
     const float* __restrict__ d_rough, const float* __restrict__ d_spec,
     float* __restrict__ o_gpos, float* __restrict__ o_gquat, float* __restrict__ o_gscale, float* __restrict__ o_bones,
-    float* __restrict__ o_vdisp, float* __restrict__ o_vnormal, float* __restrict__ o_valb, float* __restrict__ o_vrough, float* __restrict__ o_vspec) {
+    float* __restrict__ o_vdisp, float* __restrict__ o_vnormal, float* __restrict__ o_valb, float* __restrict__ o_vrough, float* __restrict__ o_vspec,
+    const int* __restrict__ order) {
   extern __shared__ float smem[];
   float* sG = smem;                 // [B][12] bone transforms
   float* sB = smem + 12 * B;        // [B][12] their gradient, this CTA's share
@@ -45,6 +46,7 @@ __global__ void __launch_bounds__(256) pose_backward_kernel(int ng, int B, int K
 #pragma unroll
   for (int e = 0; e < 12; ++e) gM[e] = 0.f;
   if (g < ng) {
+    const int gc = order[g];          // the caller's index: [n_gauss] gradient arrays come and go in the caller's order
     const float* w = g_w + (size_t)g * B;
     float M[12];
 #pragma unroll
@@ -62,21 +64,21 @@ __global__ void __launch_bounds__(256) pose_backward_kernel(int ng, int B, int K
     for (int j = 0; j < Kg; ++j) { kk[j] = knn_g[(size_t)g * Kg + j]; uu[j] = ubar_g[(size_t)g * Kg + j]; }
     // ---- position: xbar = M3 p + t
     float gx[3] = {0.f, 0.f, 0.f};
-    if (d_mean) { gx[0] = d_mean[3 * (size_t)g]; gx[1] = d_mean[3 * (size_t)g + 1]; gx[2] = d_mean[3 * (size_t)g + 2]; }
-    if (d_mean2) { gx[0] += d_mean2[3 * (size_t)g]; gx[1] += d_mean2[3 * (size_t)g + 1]; gx[2] += d_mean2[3 * (size_t)g + 2]; }
+    if (d_mean) { gx[0] = d_mean[3 * (size_t)gc]; gx[1] = d_mean[3 * (size_t)gc + 1]; gx[2] = d_mean[3 * (size_t)gc + 2]; }
+    if (d_mean2) { gx[0] += d_mean2[3 * (size_t)gc]; gx[1] += d_mean2[3 * (size_t)gc + 1]; gx[2] += d_mean2[3 * (size_t)gc + 2]; }
     float gp[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) gp[c] = M[c] * gx[0] + M[4 + c] * gx[1] + M[8 + c] * gx[2];
 #pragma unroll
     for (int r = 0; r < 3; ++r) { gM[4 * r] = gx[r] * p[0]; gM[4 * r + 1] = gx[r] * p[1]; gM[4 * r + 2] = gx[r] * p[2]; gM[4 * r + 3] = gx[r]; }
-    if (o_gpos) { o_gpos[3 * (size_t)g] = gp[0]; o_gpos[3 * (size_t)g + 1] = gp[1]; o_gpos[3 * (size_t)g + 2] = gp[2]; }
+    if (o_gpos) { o_gpos[3 * (size_t)gc] = gp[0]; o_gpos[3 * (size_t)gc + 1] = gp[1]; o_gpos[3 * (size_t)gc + 2] = gp[2]; }
     if (o_vdisp && (d_mean || d_mean2))
       for (int j = 0; j < Kg; ++j)
 #pragma unroll
         for (int c = 0; c < 3; ++c) { const float v = uu[j] * gp[c]; if (v != 0.f) atomicAdd(o_vdisp + 3 * (size_t)kk[j] + c, v); }
     // ---- normal: nbar = t / |t|, t = M3 n_g, n_g = nraw / |nraw|, nraw = Eq.1(n_v)
     if (d_normal) {
-      const float gn[3] = {d_normal[3 * (size_t)g], d_normal[3 * (size_t)g + 1], d_normal[3 * (size_t)g + 2]};
+      const float gn[3] = {d_normal[3 * (size_t)gc], d_normal[3 * (size_t)gc + 1], d_normal[3 * (size_t)gc + 2]};
       if (gn[0] != 0.f || gn[1] != 0.f || gn[2] != 0.f) {
         float t[3];
 #pragma unroll
@@ -110,7 +112,7 @@ __global__ void __launch_bounds__(256) pose_backward_kernel(int ng, int B, int K
     // ---- covariance: Sigma = A A^T, A = M3 R diag(s)
     float gq[4] = {0.f, 0.f, 0.f, 0.f}, gs[3] = {0.f, 0.f, 0.f};
     if (d_cov) {
-      const float* c6 = d_cov + 6 * (size_t)g;
+      const float* c6 = d_cov + 6 * (size_t)gc;
       const float G[9] = {c6[0], 0.5f * c6[1], 0.5f * c6[2], 0.5f * c6[1], c6[3], 0.5f * c6[4], 0.5f * c6[2], 0.5f * c6[4], c6[5]};
       const float4 q4 = g_quat[g]; const float4 so = g_scale_op[g];
       const float ql = sqrtf(q4.x * q4.x + q4.y * q4.y + q4.z * q4.z + q4.w * q4.w), iq = 1.f / ql;
@@ -151,16 +153,16 @@ __global__ void __launch_bounds__(256) pose_backward_kernel(int ng, int B, int K
       const float dq = hw * qw + hx * qx + hy * qy + hz * qz;                 // q / |q|: remove the radial part, divide by |q|
       gq[0] = (hw - dq * qw) * iq; gq[1] = (hx - dq * qx) * iq; gq[2] = (hy - dq * qy) * iq; gq[3] = (hz - dq * qz) * iq;
     }
-    if (o_gquat) { o_gquat[4 * (size_t)g] = gq[0]; o_gquat[4 * (size_t)g + 1] = gq[1]; o_gquat[4 * (size_t)g + 2] = gq[2]; o_gquat[4 * (size_t)g + 3] = gq[3]; }
-    if (o_gscale) { o_gscale[3 * (size_t)g] = gs[0]; o_gscale[3 * (size_t)g + 1] = gs[1]; o_gscale[3 * (size_t)g + 2] = gs[2]; }
+    if (o_gquat) { o_gquat[4 * (size_t)gc] = gq[0]; o_gquat[4 * (size_t)gc + 1] = gq[1]; o_gquat[4 * (size_t)gc + 2] = gq[2]; o_gquat[4 * (size_t)gc + 3] = gq[3]; }
+    if (o_gscale) { o_gscale[3 * (size_t)gc] = gs[0]; o_gscale[3 * (size_t)gc + 1] = gs[1]; o_gscale[3 * (size_t)gc + 2] = gs[2]; }
     // ---- materials: transpose of Eq.1
     for (int j = 0; j < Kg; ++j) {
       const size_t k = (size_t)kk[j];
       if (o_valb && d_alb)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) { const float v = uu[j] * d_alb[3 * (size_t)g + c]; if (v != 0.f) atomicAdd(o_valb + 3 * k + c, v); }
-      if (o_vrough && d_rough) { const float v = uu[j] * d_rough[g]; if (v != 0.f) atomicAdd(o_vrough + k, v); }
-      if (o_vspec && d_spec) { const float v = uu[j] * d_spec[g]; if (v != 0.f) atomicAdd(o_vspec + k, v); }
+        for (int c = 0; c < 3; ++c) { const float v = uu[j] * d_alb[3 * (size_t)gc + c]; if (v != 0.f) atomicAdd(o_valb + 3 * k + c, v); }
+      if (o_vrough && d_rough) { const float v = uu[j] * d_rough[gc]; if (v != 0.f) atomicAdd(o_vrough + k, v); }
+      if (o_vspec && d_spec) { const float v = uu[j] * d_spec[gc]; if (v != 0.f) atomicAdd(o_vspec + k, v); }
     }
   }
   // ---- pose: dL/dG_b = sum_g w_gb dL/dM_g.  Neighbouring Gaussians share their bones: per bone the warp reduces its 12
@@ -198,7 +200,7 @@ cudaError_t rga_launch_pose_backward(rga_avatar* av, const float* bone_mats, con
   pose_backward_kernel<<<(av->n_gauss + 255) / 256, 256, smem, s>>>(av->n_gauss, av->n_bones, av->k_g, bone_mats, av->g_static, av->g_skin_w,
       av->g_quat, av->g_scale_op, av->knn_g, av->ubar_g, av->vt_normal, in->d_mean, in->d_mean2, in->d_normal, in->d_cov, in->d_albedo, in->d_rough, in->d_spec,
       out->d_gauss_pos, out->d_gauss_quat, out->d_gauss_scale, out->d_bones, out->d_vert_disp, out->d_vert_normal, out->d_vert_albedo,
-      out->d_vert_rough, out->d_vert_spec);
+      out->d_vert_rough, out->d_vert_spec, av->g_order);
   rga_prof_mark(av, "pose_backward", s);
   av->launches += 1;
   return cudaGetLastError();

@@ -20,6 +20,9 @@ struct rga_avatar {
   float4* v_pos;       // [n_verts]  canonical x (displacement_mlp re-derives x + dx from it)
   float4* v_disp;      // [n_verts]  per-pose displacement written by displacement_mlp
   float4* g_pos;       // [n_gauss]  canonical x_g
+  // Gaussian order (order_kernels.cu): every per-Gaussian table below is stored in the library's spatial order;
+  // g_order[i] = caller index of the i-th Gaussian, g_inv = its inverse; gi_pos = the caller's positions in library order
+  int *g_order, *g_inv; float* gi_pos; unsigned* bb_scratch; float* bb_dev;
   // the library's copies of the vertex tables Eq.1 reads (gaussians_update re-interpolates from them)
   float *vt_pos, *vt_disp, *vt_normal, *vt_albedo, *vt_rough, *vt_spec;   // [n_verts][3] x4 (disp NULL = 0), [n_verts] x2
   float* knn_d2;       // [n_gauss][k_g] squared distances of the last Gaussian KNN
@@ -64,7 +67,7 @@ struct rga_avatar {
   // splat
   float2* mu2d; float* depth; float4* conic_o; int4* rect; unsigned* touched;
   unsigned* tile_count; unsigned* cursor;   // [tiles] histogram of the tile digit, scatter cursors
-  unsigned long long* keys[2]; unsigned* vals[2];   // keys[0]: binned local keys (depth<<32|g); keys[1]/vals[0]: sorted output
+  unsigned long long* keys[2]; unsigned* vals[2];   // keys[0]: binned local keys (depth<<32|caller index); keys[1]/vals[0]: sorted output (caller indices); vals[1]: the same list as library indices
   unsigned* num_dup;           // [1] D (device)
   uint2* ranges;               // [tiles]
   unsigned* seg_off;           // [tiles + 1] exclusive scan of ceil(n_t / RGA_SEG)
@@ -108,6 +111,12 @@ cudaError_t rga_launch_knn(const float* q, int nq, const float* v, int nv, int K
 cudaError_t rga_launch_load_verts(rga_avatar* av, const float* pos, const float* disp, const float* nrm, cudaStream_t s);
 cudaError_t rga_launch_load_gauss(rga_avatar* av, const float* gauss_pos, const float* gauss_quat, const float* gauss_scale,
                                   const float* gauss_opacity, const float* d2, cudaStream_t s);
+// order_kernels.cu
+cudaError_t rga_points_aabb(const float* pos, int n, unsigned* scratch6, float* out6_dev, cudaStream_t s);
+cudaError_t rga_build_gauss_order(const float* pos, int n, unsigned long long* keys, int npad, unsigned* bb_u, float* bb_dev,
+                                  int* order, int* inv, cudaStream_t s);
+cudaError_t rga_gather_rows(int n, int words_per_row, const void* src, const int* order, void* dst, cudaStream_t s);
+cudaError_t rga_scatter_rows(int n, int words_per_row, const void* src, const int* order, void* dst, cudaStream_t s);
 // skin_kernels.cu
 cudaError_t rga_launch_skin(rga_avatar* av, const float* bone_mats, int which, cudaStream_t s);
 // vis_kernels.cu

@@ -28,7 +28,7 @@ __global__ void __launch_bounds__(SB_THREADS) shade_backward_kernel(int ng, int 
     const unsigned char* __restrict__ vcount, const int* __restrict__ knn_g, const float* __restrict__ ubar_g,
     float3 cam, float inv_gamma, const float4* __restrict__ radiance, const float* __restrict__ dL_dcolor,
     float* __restrict__ out_dalbedo, float* __restrict__ out_drough, float* __restrict__ out_dspec, float* __restrict__ out_dnormal,
-    float* __restrict__ out_dpos, float* __restrict__ out_denv, int* __restrict__ work) {
+    float* __restrict__ out_dpos, float* __restrict__ out_denv, int* __restrict__ work, const int* __restrict__ order) {
   extern __shared__ __align__(16) float smem[];
   float4* sE = reinterpret_cast<float4*>(smem);                          // [ne][2]: (w, A), (L A, 0)
   float* sG = reinterpret_cast<float*>(sE + 2 * ne);                     // [ne][3] environment gradient of this CTA
@@ -50,11 +50,12 @@ __global__ void __launch_bounds__(SB_THREADS) shade_backward_kernel(int ng, int 
     if (gbase >= ng) break;
     const int g = gbase + threadIdx.x / SB_LANES;
     bool active = g < ng;
+    const int gc = active ? order[g] : 0;           // the caller's index: dL_dcolor and the [n_gauss] outputs are in the caller's order
     float4 x = make_float4(0.f, 0.f, 0.f, 0.f), n = x, ar = x;
     float gL0 = 0.f, gL1 = 0.f, gL2 = 0.f, spec = 0.f;
     if (active) {
       const float4 Lo = radiance[g];
-      const float c0 = dL_dcolor[3 * (size_t)g], c1 = dL_dcolor[3 * (size_t)g + 1], c2 = dL_dcolor[3 * (size_t)g + 2];
+      const float c0 = dL_dcolor[3 * (size_t)gc], c1 = dL_dcolor[3 * (size_t)gc + 1], c2 = dL_dcolor[3 * (size_t)gc + 2];
       // colour = clamp(L_o, 0, 1)^(1/gamma): slope (1/gamma) L_o^(1/gamma - 1) strictly inside the limits, 0 otherwise
       if (Lo.x > 0.f && Lo.x < 1.f) gL0 = c0 * inv_gamma * exp2f((inv_gamma - 1.f) * log2f(Lo.x));
       if (Lo.y > 0.f && Lo.y < 1.f) gL1 = c1 * inv_gamma * exp2f((inv_gamma - 1.f) * log2f(Lo.y));
@@ -184,11 +185,11 @@ __global__ void __launch_bounds__(SB_THREADS) shade_backward_kernel(int ng, int 
         const float dt = gwx * wox + gwy * woy + gwz * woz;               // w_o = (cam - x) / |cam - x|
         o_x[0] = -(gwx - dt * wox) * winv; o_x[1] = -(gwy - dt * woy) * winv; o_x[2] = -(gwz - dt * woz) * winv;
       }
-      if (out_dalbedo) { out_dalbedo[3 * (size_t)g] = gL0 * d0 * ip; out_dalbedo[3 * (size_t)g + 1] = gL1 * d1 * ip; out_dalbedo[3 * (size_t)g + 2] = gL2 * d2 * ip; }
-      if (out_dspec) out_dspec[g] = gp;
-      if (out_drough) out_drough[g] = gr;
-      if (out_dnormal) { out_dnormal[3 * (size_t)g] = o_n[0]; out_dnormal[3 * (size_t)g + 1] = o_n[1]; out_dnormal[3 * (size_t)g + 2] = o_n[2]; }
-      if (out_dpos) { out_dpos[3 * (size_t)g] = o_x[0]; out_dpos[3 * (size_t)g + 1] = o_x[1]; out_dpos[3 * (size_t)g + 2] = o_x[2]; }
+      if (out_dalbedo) { out_dalbedo[3 * (size_t)gc] = gL0 * d0 * ip; out_dalbedo[3 * (size_t)gc + 1] = gL1 * d1 * ip; out_dalbedo[3 * (size_t)gc + 2] = gL2 * d2 * ip; }
+      if (out_dspec) out_dspec[gc] = gp;
+      if (out_drough) out_drough[gc] = gr;
+      if (out_dnormal) { out_dnormal[3 * (size_t)gc] = o_n[0]; out_dnormal[3 * (size_t)gc + 1] = o_n[1]; out_dnormal[3 * (size_t)gc + 2] = o_n[2]; }
+      if (out_dpos) { out_dpos[3 * (size_t)gc] = o_x[0]; out_dpos[3 * (size_t)gc + 1] = o_x[1]; out_dpos[3 * (size_t)gc + 2] = o_x[2]; }
     }
   }
   __syncthreads();
@@ -208,7 +209,7 @@ cudaError_t rga_launch_shade_backward(rga_avatar* av, const rga_env* env, float3
   const int grid = min((av->n_gauss + gpb - 1) / gpb, av->num_sms * 8);
 #define SB_ARGS av->n_gauss, ne, av->vis_dirs, av->vis_words, av->k_g, av->k_v, av->g_posed, av->g_nposed, av->g_static, av->env_table, \
     env->texel_to_dir, av->visbits, av->vcount, av->knn_g, av->ubar_g, cam, ig, av->radiance, dL_dcolor, out_dalbedo, out_drough, out_dspec, \
-    out_dnormal, out_dpos, out_denv, av->work_counter
+    out_dnormal, out_dpos, out_denv, av->work_counter, av->g_order
   if (vis_mode == 0) shade_backward_kernel<0><<<grid, SB_THREADS, smem, s>>>(SB_ARGS);
   else if (vis_mode == 1) shade_backward_kernel<1><<<grid, SB_THREADS, smem, s>>>(SB_ARGS);
   else shade_backward_kernel<2><<<grid, SB_THREADS, smem, s>>>(SB_ARGS);

@@ -66,14 +66,15 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int ntiles, long long c
 }
 
 // scatter: every (Gaussian, tile) duplicate takes the next slot of its tile's bucket; the order inside a bucket is
-// arbitrary here and fixed by the per-tile sort.  local key = depth bits << 32 | Gaussian index.
+// arbitrary here and fixed by the per-tile sort.  local key = depth bits << 32 | Gaussian index (the caller's).
 __global__ void __launch_bounds__(256) tile_scatter_kernel(int ng, int TX, long long capacity, const unsigned* __restrict__ touched,
-    const int4* __restrict__ rect, const float* __restrict__ depth, unsigned* __restrict__ cursor,
+    const int4* __restrict__ rect, const float* __restrict__ depth, const int* __restrict__ order, unsigned* __restrict__ cursor,
     unsigned long long* __restrict__ lkeys) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= ng || touched[g] == 0) return;
   int4 r = rect[g];
-  unsigned long long key = ((unsigned long long)__float_as_uint(depth[g]) << 32) | (unsigned)g;
+  // the low word is the CALLER's index of the Gaussian: equal (tile, depth) keys order by it (A22)
+  unsigned long long key = ((unsigned long long)__float_as_uint(depth[g]) << 32) | (unsigned)order[g];
   const unsigned lane = threadIdx.x & 31;
   for (int y = r.y; y < r.w; ++y)
     for (int x = r.x; x < r.z; ++x) {
@@ -94,7 +95,7 @@ cudaError_t rga_launch_bin(rga_avatar* av, int TX, int ntiles, cudaStream_t s) {
                                       av->num_items, av->num_long, av->long_list, av->status);
   rga_prof_mark(av, "tile_scan", s);
   tile_scatter_kernel<<<(av->n_gauss + 255) / 256, 256, 0, s>>>(av->n_gauss, TX, av->max_dup, av->touched, av->rect, av->depth,
-                                                               av->cursor, av->keys[0]);
+                                                               av->g_order, av->cursor, av->keys[0]);
   rga_prof_mark(av, "tile_scatter", s);
   av->launches += 2;
   return cudaGetLastError();

@@ -104,9 +104,11 @@ def _base_mesh(kind):
     return v, f, J, _mesh.PARENTS.copy(), _mesh.two_nearest_joint_weights(v, J)
 
 
-def make(cfg_id, seed=None, n_gauss=None, morton=True):
+def make(cfg_id, seed=None, n_gauss=None, morton=False):
     """Return a dict of contiguous numpy arrays for config `cfg_id` (0..4).  `n_gauss` overrides the count
-    (used by tests to shrink a config while keeping its structure)."""
+    (used by tests to shrink a config while keeping its structure).  Gaussians come in the order they were drawn
+    ("random surface points", BASELINE.json); `morton=True` stores them in Morton order of their canonical position
+    instead (bench.py reports that variant beside the metric)."""
     c = dict(_CFG[cfg_id])
     seed = cfg_id if seed is None else seed
     if n_gauss is not None:
