@@ -14,7 +14,7 @@ OBJ = os.path.join(HERE, "build")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC,-fvisibility=hidden", "-Xptxas", "-v"]
 EXACT = ["load_kernels.cu", "skin_kernels.cu", "vis_kernels.cu", "project_kernels.cu", "densify_kernels.cu"]
-FAST = ["order_kernels.cu", "shade_kernels.cu", "composite_kernels.cu", "sort_kernels.cu", "api.cu", "peak_kernels.cu", "mlp_kernels.cu", "backward_kernels.cu", "shade_backward_kernels.cu", "loss_kernels.cu", "pose_backward_kernels.cu"]
+FAST = ["vis_shade_kernels.cu", "order_kernels.cu", "shade_kernels.cu", "composite_kernels.cu", "sort_kernels.cu", "api.cu", "peak_kernels.cu", "mlp_kernels.cu", "backward_kernels.cu", "shade_backward_kernels.cu", "loss_kernels.cu", "pose_backward_kernels.cu"]
 
 
 def _stale():

@@ -56,7 +56,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->g_order, av->g_inv, av->gi_pos, av->bb_scratch, av->bb_dev, av->vals[1], av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
+  void* ptrs[] = {av->rast_bins, av->frames, av->front_list, av->n_front, av->vs_counter, av->dir_start, av->tex_list, av->tex_dir, av->dir_eps, av->g_order, av->g_inv, av->gi_pos, av->bb_scratch, av->bb_dev, av->vals[1], av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
                   av->vt_spec, av->knn_d2, av->grid_start, av->grid_verts, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
@@ -121,6 +121,8 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->g_static, 4 * ng)); A(dalloc(&av->g_skin_w, ng * B)); A(dalloc(&av->g_quat, ng)); A(dalloc(&av->g_scale_op, ng));
   A(dalloc(&av->v_posed, nv)); A(dalloc(&av->v_nposed, nv)); A(dalloc(&av->g_posed, ng)); A(dalloc(&av->g_nposed, ng));
   A(dalloc(&av->g_cov, 6 * ng)); A(dalloc(&av->window, 4)); A(dalloc(&av->aabb, 8));
+  av->rast_bins_bands = rga_vis_raster_max_bands(av->max_res, av->n_verts);
+  if (av->rast_bins_bands > 0) A(dalloc(&av->rast_bins, (size_t)av->num_sms * av->rast_bins_bands * (size_t)av->n_faces));
   A(dalloc(&av->zmap, nmap)); A(dalloc(&av->idmap, nmap)); A(dalloc(&av->visbits, ng * words));
   A(dalloc(&av->vbits_a, nv * words)); A(dalloc(&av->vbits_b, nv * words)); A(dalloc(&av->vbits_raw, nv * words));
   A(dalloc(&av->vcount, nv * (size_t)av->max_dirs + 32)); A(dalloc(&av->env_table, 8 * (size_t)av->max_env));
@@ -129,6 +131,8 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->tile_count, ntiles)); A(dalloc(&av->cursor, ntiles));
   A(dalloc(&av->keys[0], (size_t)av->max_dup)); A(dalloc(&av->keys[1], (size_t)av->max_dup));
   A(dalloc(&av->vals[0], (size_t)av->max_dup)); A(dalloc(&av->vals[1], (size_t)av->max_dup));
+  A(dalloc(&av->frames, 4 * (2 + 3 * (size_t)av->max_dirs))); A(dalloc(&av->front_list, ng)); A(dalloc(&av->n_front, 1)); A(dalloc(&av->vs_counter, 1));
+  A(cudaMemsetAsync(av->vs_counter, 0, sizeof(unsigned), s)); A(dalloc(&av->dir_start, (size_t)av->max_dirs + 2)); A(dalloc(&av->tex_list, (size_t)av->max_env + 1)); A(dalloc(&av->tex_dir, (size_t)av->max_env + 1)); A(dalloc(&av->dir_eps, (size_t)av->max_dirs));
   A(dalloc(&av->g_order, ng)); A(dalloc(&av->g_inv, ng)); A(dalloc(&av->gi_pos, 3 * ng)); A(dalloc(&av->bb_scratch, 8)); A(dalloc(&av->bb_dev, 8));
   A(dalloc(&av->num_dup, 1)); A(dalloc(&av->ranges, ntiles));
   av->items_cap = av->max_dup / RGA_SEG + (long long)ntiles + 1;
@@ -195,7 +199,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
     if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, "avatar_load: Gaussian order / tables: %s", cudaGetErrorString(e_)); goto done; }
   }
   av->launches += 5;
-  if (rga_shade_init_attributes(av->max_env) != 0 || rga_shade_backward_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_composite_init_attributes() != 0 || rga_mlp_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
+  if (rga_shade_init_attributes(av->max_env) != 0 || rga_shade_backward_init_attributes(av->max_env) != 0 || rga_vis_init_attributes() != 0 || rga_vis_shade_init_attributes() != 0 || rga_composite_init_attributes() != 0 || rga_mlp_init_attributes() != 0) { st = fail(RGA_ERR_CUDA, "avatar_load: cudaFuncSetAttribute failed"); goto done; }
   A(cudaStreamSynchronize(s));
 done:
   if (d2) cudaFree(d2);
@@ -225,7 +229,7 @@ extern "C" rga_status visibility_raster(rga_avatar* av, const rga_vis_params* p,
   CU(rga_launch_vis_raster(av, p, s));
   if (p->mode == 0) CU(rga_launch_vis_depth_test(av, p, nullptr, s));
   else CU(rga_launch_vis_paper(av, p, s));
-  av->vis_culled = 0;
+  av->vis_culled = 0; av->vis_partial = 0;
   av->vis_mode = p->mode; av->vis_dirs = p->n_dirs; av->vis_res = p->res; av->vis_words = (p->n_dirs + 31) / 32;
   av->keep_maps = p->keep_maps || p->mode == 1;
   av->have_vis = 1;
@@ -240,6 +244,10 @@ extern "C" rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const 
       (cam_pos[0] != av->vis_cull_cam[0] || cam_pos[1] != av->vis_cull_cam[1] || cam_pos[2] != av->vis_cull_cam[2]))
     return fail(RGA_ERR_STATE, "shade_gaussians: rga_render_frame computed this pose's visibility only for Gaussians facing ITS camera; "
                                "call visibility_raster before shading from another camera");
+  if (env->use_visibility && av->vis_mode == 0 && av->vis_partial &&
+      ((env->texel_to_dir == nullptr) != (av->vs_t2d == nullptr) || env->rows != av->vs_rows || env->cols != av->vs_cols))
+    return fail(RGA_ERR_STATE, "shade_gaussians: rga_render_frame tested only the directions ITS environment map reads; "
+                               "call visibility_raster before shading with another map layout");
   if (env->rows < 1 || env->cols < 1 || env->rows * env->cols > av->max_env || !(env->gamma > 0.f))
     return fail(RGA_ERR_INVALID_ARG, "shade_gaussians: env size/gamma out of range");
   if (env->use_visibility && !env->texel_to_dir && env->rows * env->cols != av->vis_dirs)
@@ -305,6 +313,9 @@ extern "C" rga_status shade_backward(rga_avatar* av, const rga_env* env, const f
   if (env->use_visibility && av->vis_mode == 0 && av->vis_culled &&
       (cam_pos[0] != av->vis_cull_cam[0] || cam_pos[1] != av->vis_cull_cam[1] || cam_pos[2] != av->vis_cull_cam[2]))
     return fail(RGA_ERR_STATE, "shade_backward: this pose's visibility was computed for another camera (rga_render_frame)");
+  if (env->use_visibility && av->vis_mode == 0 && av->vis_partial &&
+      ((env->texel_to_dir == nullptr) != (av->vs_t2d == nullptr) || env->rows != av->vs_rows || env->cols != av->vs_cols))
+    return fail(RGA_ERR_STATE, "shade_backward: this pose's visibility was computed for another environment-map layout (rga_render_frame)");
   if (env->rows < 1 || env->cols < 1 || env->rows * env->cols > av->max_env || !(env->gamma > 0.f))
     return fail(RGA_ERR_INVALID_ARG, "shade_backward: env size/gamma out of range");
   if (env->use_visibility && !env->texel_to_dir && env->rows * env->cols != av->vis_dirs)
@@ -418,24 +429,36 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   const int TX = (cam->width + 15) / 16, TY = (cam->height + 15) / 16, ntiles = TX * TY;
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
   rga_prof_mark(av, "-", s);
+  const float3 cam3 = make_float3(cam_pos[0], cam_pos[1], cam_pos[2]);
+  // mode 0 inside one frame: camera, environment map and texel -> direction map are known when visibility is tested, so the
+  // depth test and the shading run as ONE kernel over the camera-facing Gaussians (vis_shade_kernels.cu)
+  const bool fused = vis && vis->mode == 0 && env->use_visibility && rga_vis_shade_teams(vis->n_dirs, env->rows * env->cols) > 0;
   if (overlap) {
     // the rasteriser only needs the posed mesh and the window: the Gaussians are skinned on the second stream
     CU(cudaEventRecord(av->ev_fork, s)); CU(cudaStreamWaitEvent(s2, av->ev_fork, 0));
     CU(rga_launch_skin(av, bone_mats, 1, s));
     CU(rga_launch_skin(av, bone_mats, 2, s2));
-    CU(cudaEventRecord(av->ev_gskin, s2));
   } else CU(rga_launch_skin(av, bone_mats, 0, s));
   av->have_skin = 1;
+  if (fused) CU(rga_launch_front_compact(av, (vis->n_dirs + 31) / 32, cam3, s2));
+  if (overlap) CU(cudaEventRecord(av->ev_gskin, s2));
   CU(rga_launch_env_table(av, env, s2));
+  if (fused) CU(rga_launch_texel_csr(av, env, vis, s2));
   if (overlap) CU(cudaEventRecord(av->ev_env, s2));
   CU(rga_launch_project(av, cam, s2));
   CU(rga_launch_bin(av, TX, ntiles, s2));
   CU(rga_launch_tile_sort(av, cam, s2));
   if (overlap) CU(cudaEventRecord(av->ev_join, s2));
+  av->vis_partial = 0;
   if (vis) {
     CU(rga_launch_vis_raster(av, vis, s));
     if (overlap) CU(cudaStreamWaitEvent(s, av->ev_gskin, 0));
-    if (vis->mode == 0) {
+    if (fused) {
+      if (overlap) CU(cudaStreamWaitEvent(s, av->ev_env, 0));
+      CU(rga_launch_vis_shade(av, vis, env, cam3, s));
+      av->vis_culled = 1; av->vis_cull_cam[0] = cam_pos[0]; av->vis_cull_cam[1] = cam_pos[1]; av->vis_cull_cam[2] = cam_pos[2];
+      av->vis_partial = 1; av->vs_t2d = env->texel_to_dir; av->vs_rows = env->rows; av->vs_cols = env->cols;
+    } else if (vis->mode == 0) {
       CU(rga_launch_vis_depth_test(av, vis, cam_pos, s));
       av->vis_culled = 1; av->vis_cull_cam[0] = cam_pos[0]; av->vis_cull_cam[1] = cam_pos[1]; av->vis_cull_cam[2] = cam_pos[2];
     } else {
@@ -446,8 +469,10 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
     av->keep_maps = vis->keep_maps || vis->mode == 1;
     av->have_vis = 1;
   }
-  if (overlap) { if (!vis) CU(cudaStreamWaitEvent(s, av->ev_gskin, 0)); CU(cudaStreamWaitEvent(s, av->ev_env, 0)); }
-  CU(rga_launch_shade(av, env, make_float3(cam_pos[0], cam_pos[1], cam_pos[2]), env->use_visibility ? av->vis_mode : 2, s));
+  if (!fused) {
+    if (overlap) { if (!vis) CU(cudaStreamWaitEvent(s, av->ev_gskin, 0)); CU(cudaStreamWaitEvent(s, av->ev_env, 0)); }
+    CU(rga_launch_shade(av, env, cam3, env->use_visibility ? av->vis_mode : 2, s));
+  }
   av->have_shade = 1;
   if (overlap) CU(cudaStreamWaitEvent(s, av->ev_join, 0));
   CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->color, out_image, s));

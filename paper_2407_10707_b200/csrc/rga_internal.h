@@ -52,6 +52,7 @@ struct rga_avatar {
   float* window;       // [4] centre, radius; [4..9] scratch AABB as ordered ints
   unsigned* aabb;      // [8] ordered-uint min xyz, max xyz; [6] counts skin_kernel's finished vertex blocks
   // visibility
+  unsigned* rast_bins; int rast_bins_bands;   // [num_sms][bands][n_faces] triangle lists of banded depth maps (vis_raster)
   unsigned* zmap;      // [max_dirs][res*res]
   int* idmap;          // [max_dirs][res*res]  (allocated lazily at load: always, sized like zmap)
   unsigned* visbits;   // [n_gauss][words]
@@ -84,6 +85,9 @@ struct rga_avatar {
   double* reg_sums;            // [4] regularisers: sums of Eq.6, 7, 8, 9
   int disp_is_mlp;             // the current displacement is displacement_mlp's v_disp (else the static vt_disp table)
   float* loss_maps; double* loss_sums;   // image_loss: [max_h][max_w][9] SSIM derivative maps, {sum SSIM, sum |I - J|}
+  // fused depth test + shading of rga_render_frame (vis_shade_kernels.cu)
+  float* frames; int* front_list; unsigned* n_front; unsigned* vs_counter; unsigned short* dir_start; unsigned short* tex_list; unsigned short* tex_dir; float* dir_eps;
+  int vis_partial; const int* vs_t2d; int vs_rows, vs_cols;   // the frame's visibility words hold only the directions its env map could read
   int* work_counter;           // [1] dynamic work distribution of persistent kernels (zeroed before the launch)
   unsigned* shade_counter;     // [1] group tickets of shade_kernel (zero between launches: the last CTA re-arms it)
   float* splat_grad;           // [n_gauss][12] splat_backward: d_colour(3), d_opacity, d_mu(2), d_conic(3), pad
@@ -124,7 +128,15 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
 cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, const float* cull_cam, cudaStream_t s);
 cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
 size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads);
+int rga_vis_raster_max_bands(int max_res, int n_verts);
 cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s);
+// vis_shade_kernels.cu
+int rga_vis_shade_teams(int K, int ne);
+int rga_vis_shade_init_attributes();
+cudaError_t rga_launch_light_frames(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
+cudaError_t rga_launch_front_compact(rga_avatar* av, int words, float3 cam, cudaStream_t s);
+cudaError_t rga_launch_texel_csr(rga_avatar* av, const rga_env* env, const rga_vis_params* vis, cudaStream_t s);
+cudaError_t rga_launch_vis_shade(rga_avatar* av, const rga_vis_params* vis, const rga_env* env, float3 cam, cudaStream_t s);
 // shade_kernels.cu
 cudaError_t rga_launch_env_table(rga_avatar* av, const rga_env* env, cudaStream_t s);
 cudaError_t rga_launch_shade(rga_avatar* av, const rga_env* env, float3 cam, int vis_mode, cudaStream_t s);

@@ -61,6 +61,7 @@ __device__ __forceinline__ float light_project_z(float dx, float dy, float dz, c
 // functions (inclusive, two-sided; int32 when the triangle spans < 64 pixels, else int64), area = e0+e1+e2 (exact
 // identity), z = (z0 + (e1/area)(z1-z0)) + (e2/area)(z2-z0) in fp32, clamped at 0.
 #define RAST_MAX_RES 256       // snapped coordinates must fit 16 bits
+#define RAST_MAX_BANDS 64      // bands of a map that does not fit shared memory whole
 
 __device__ __forceinline__ void face_unpack(unsigned long long f, int& i0, int& i1, int& i2) {
   i0 = (int)(f & 0x1fffffull); i1 = (int)((f >> 21) & 0x1fffffull); i2 = (int)((f >> 42) & 0x1fffffull);
@@ -270,14 +271,16 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
   return q2n;
 }
 
-template <bool WITH_ID>
+template <bool WITH_ID, bool BINNED>
 __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
     int tail_first, int split,
     const float4* __restrict__ v_posed, const unsigned long long* __restrict__ faces_packed, const float* __restrict__ dirs,
     const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
-    unsigned* __restrict__ vbits_raw, int words, int cull) {
+    unsigned* __restrict__ vbits_raw, int words, int cull, float4* __restrict__ frames_out, float bias_texels, float bias_world,
+    float slope_max, unsigned* __restrict__ bins, int band_magic) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_next;
+  __shared__ unsigned s_bin_cnt[RAST_MAX_BANDS];
   __shared__ float s_zf[8];
   // layout: [RasterWarp x warps][map band_rows*R*(4|8)][sXY nv*4][svert (WITH_ID)]
   const int nthreads = blockDim.x, nwarps = nthreads >> 5;
@@ -303,15 +306,33 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
       unit = tail_first + q / split;
       t_begin = (int)((long long)nf * part / split); t_end = (int)((long long)nf * (part + 1) / split);
     }
-    const int k = unit / n_bands, band = unit - k * n_bands;
-    const int row0 = band * band_rows, rows = min(band_rows, R - row0);
-    const int npix = rows * R;
+    // Maps that fit shared memory whole: a unit is a direction.  Larger maps (256^2) are cut into bands of rows, and a
+    // unit is still ONE direction: its triangles are walked and boxed once and BINNED by band (triangle ids in an
+    // L2-resident scratch list per band), then the bands are rasterised one after the other from their lists -- the
+    // fetch / gather / box work is not repeated per band (it was: 7x the time for 4x the work at config 2).
+    const bool binned = BINNED;
+    const int k = binned ? unit : unit / n_bands;
+    int band = binned ? 0 : unit - k * n_bands;
+    int row0 = band * band_rows, rows = binned ? R : min(band_rows, R - row0);
+    int npix = min(band_rows, R - row0) * R;
     {                                                       // frame and window live only through phase A
     const WinConst W = make_win(window, R);
     const LightFrame F = make_frame(dirs + 3 * k, W);
+    if (binned && threadIdx.x < n_bands) s_bin_cnt[threadIdx.x] = 0u;
     if (threadIdx.x == 0) {
       s_next = t_begin;
       s_zf[0] = W.cx; s_zf[1] = W.cy; s_zf[2] = W.cz; s_zf[3] = F.wn[0]; s_zf[4] = F.wn[1]; s_zf[5] = F.wn[2];
+      // the pre-scaled frame and the depth-test constants for the fused depth-test + shading kernel (vis_shade_kernels.cu,
+      // a FAST file): written HERE, by the EXACT file's make_win / make_frame -- layout as light_frames_kernel below
+      if (frames_out && band == 0 && t_begin == 0) {
+        frames_out[2 + 3 * k] = make_float4(F.us[0], F.us[1], F.us[2], F.w[0]);
+        frames_out[2 + 3 * k + 1] = make_float4(F.vs[0], F.vs[1], F.vs[2], F.w[1]);
+        frames_out[2 + 3 * k + 2] = make_float4(F.wn[0], F.wn[1], F.wn[2], F.w[2]);
+        if (k == 0) {
+          frames_out[0] = make_float4(W.cx, W.cy, W.cz, W.hR);
+          frames_out[1] = make_float4(bias_texels / (float)R, bias_world * W.inv2r, slope_max, (float)R);
+        }
+      }
     }
     // clear the band
     if (WITH_ID) { for (int p = threadIdx.x; p < npix; p += nthreads) sz64[p] = ~0ull; }
@@ -346,10 +367,11 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
       for (int base = base4; base < min(base4 + RAST_FETCH, t_end); base += 32) {
         const int t = base + lane;
         bool ne = false;
+        int ia = 0, ja = 0, bw = 0, bh = 0;
         if (t < t_end) {
           int i0, i1, i2;
           face_unpack(__ldg(faces_packed + t), i0, i1, i2);
-          int ia, ja, bw, bh; bool narrow;
+          bool narrow;
           const unsigned Q0 = sXY[i0], Q1 = sXY[i1], Q2 = sXY[i2];
           ne = tri_box(Q0, Q1, Q2, R, row0, rows, ia, ja, bw, bh, narrow) > 0;
           if (cull && ne) {                               // reading A36: negative snapped area = facing away from the light
@@ -357,6 +379,14 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
             const long long bx = (int)(Q2 & 0xffff) - (int)(Q0 & 0xffff), by = (int)(Q2 >> 16) - (int)(Q0 >> 16);
             ne = ax * by - ay * bx > 0;
           }
+        }
+        if (binned) {                                     // push the triangle into the list of every band its box touches
+          if (ne) {
+            const int jb2 = ja + bh - 1;
+            const int blo = (ja * band_magic) >> 16, bhi = (jb2 * band_magic) >> 16;
+            for (int b = blo; b <= bhi; ++b) bins[((size_t)blockIdx.x * n_bands + b) * (size_t)nf + atomicAdd(&s_bin_cnt[b], 1u)] = (unsigned)t;
+          }
+          continue;
         }
         const unsigned m = __ballot_sync(0xffffffffu, ne);
         if (m) {
@@ -375,6 +405,39 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
     if (q2n) raster_depth<WITH_ID>(c, w, 0, q2n, lane);
     __syncthreads();
 
+    for (band = 0; band < (binned ? n_bands : 1); ++band) {
+    if (binned) {
+      // rasterise band `band` from its triangle list: 32 listed triangles per round, every lane busy from the start
+      row0 = band * band_rows; rows = min(band_rows, R - row0); npix = rows * R;
+      c.row0 = row0; c.rows = rows;
+      if (band > 0) {                                        // band 0 was cleared before phase A
+        if (WITH_ID) { for (int p = threadIdx.x; p < npix; p += nthreads) sz64[p] = ~0ull; }
+        else {
+          uint4* m4 = reinterpret_cast<uint4*>(sz32);
+          const uint4 ones = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
+          for (int p = threadIdx.x; p < (npix + 3) >> 2; p += nthreads) m4[p] = ones;
+        }
+      }
+      if (threadIdx.x == 0) s_next = 0;
+      __syncthreads();
+      const int nlist = (int)s_bin_cnt[band];
+      const unsigned* list = bins + ((size_t)blockIdx.x * n_bands + band) * (size_t)nf;
+      int q2b = 0;
+      for (;;) {
+        int base = 0;
+        if (lane == 0) base = atomicAdd(&s_next, 32);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base >= nlist) break;
+        const int cnt = min(32, nlist - base);
+        if (lane < cnt) w->q1[lane] = (int)__ldcg(list + base + lane);
+        __syncwarp();
+        q2b = raster_round<WITH_ID>(c, w, 0, cnt, lane, q2b);
+        __syncwarp();
+      }
+      if (q2b) raster_depth<WITH_ID>(c, w, 0, q2b, lane);
+      __syncthreads();
+    }
+
     // write the band out
     const size_t gbase = ((size_t)k * R + row0) * R;
     if (WITH_ID) {
@@ -391,7 +454,7 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
           atomicOr(svert + (v2 >> 5), 1u << (v2 & 31));
         }
       }
-      if (vbits_raw) {
+      if (vbits_raw && (!binned || band == n_bands - 1)) {
         __syncthreads();
         const unsigned bit = 1u << (k & 31);
         for (int wd = threadIdx.x; wd < nv_words; wd += nthreads) {
@@ -412,13 +475,14 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
     } else {
       for (int p = threadIdx.x; p < npix; p += nthreads) zmap[gbase + p] = sz32[p];
     }
-    __syncthreads();                                      // the map and the vertex table are reused by the next unit
+    __syncthreads();                                      // the map and the vertex table are reused by the next band / unit
+    }
   }
 }
 
 // shared-memory plan: picks the CTA size (1024 / 512 / 256 threads) that minimises bands / warps; returns bytes
 size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads) {
-  const size_t budget = 227 * 1024 - 256;
+  const size_t budget = 227 * 1024 - 512;               // static shared memory (counters, band list sizes) counts against the 227 KB
   const size_t per_row = (size_t)res * (with_id ? 8 : 4);
   size_t best = 0; double best_score = 1e30;
   *band_rows = 0; *threads = 0;
@@ -445,26 +509,71 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
   if (band_rows < 1) return cudaErrorInvalidConfiguration;
   const int n_bands = (p->res + band_rows - 1) / band_rows;
   const int words = (p->n_dirs + 31) / 32;
-  const int n_units = p->n_dirs * n_bands;
+  // a map cut into bands: one unit per direction, triangles binned by band (needs the scratch lists sized at load)
+  const bool binned = n_bands > 1;
+  if (binned && (n_bands > RAST_MAX_BANDS || !av->rast_bins || n_bands > av->rast_bins_bands)) return cudaErrorInvalidConfiguration;
+  const int n_units = binned ? p->n_dirs : p->n_dirs * n_bands;
   const int grid = n_units < av->num_sms ? n_units : av->num_sms;
   unsigned* raw = (with_id && p->mode == 1) ? av->vbits_raw : nullptr;
   if (raw) cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s);
   // last, partial round of the persistent grid: cut its units into triangle ranges (depth-only maps merge with atomicMin)
   int tail_first = n_units, split = 1;
   const int rem = n_units > grid ? n_units % grid : 0;
-  if (rem > 0 && !with_id && grid / rem >= 2) {
+  if (rem > 0 && !with_id && !binned && grid / rem >= 2) {
     split = grid / rem > 4 ? 4 : grid / rem;
     tail_first = n_units - rem;
     const size_t unit_px = (size_t)band_rows * p->res;       // bands are even; the last may be shorter (covered anyway)
     const size_t first_px = (size_t)(tail_first / n_bands) * p->res * p->res + (size_t)(tail_first % n_bands) * unit_px;
     cudaMemsetAsync(av->zmap + first_px, 0xff, ((size_t)p->n_dirs * p->res * p->res - first_px) * 4, s);
   }
+  const int band_magic = (65536 + band_rows - 1) / band_rows;   // (row * magic) >> 16 == row / band_rows for row < 256
 #define RAST_ARGS av->n_faces, av->n_verts, p->res, band_rows, n_bands, n_units, tail_first, split, av->v_posed, av->faces_packed, p->dirs, av->window, \
-    av->zmap, av->idmap, raw, words, p->cull_backfaces != 0
-  if (with_id) vis_raster_kernel<true><<<grid, threads, smem, s>>>(RAST_ARGS);
-  else vis_raster_kernel<false><<<grid, threads, smem, s>>>(RAST_ARGS);
+    av->zmap, av->idmap, raw, words, p->cull_backfaces != 0, reinterpret_cast<float4*>(av->frames), p->depth_bias_texels, p->depth_bias_world, \
+    p->slope_max, binned ? av->rast_bins : nullptr, band_magic
+  if (with_id) { if (binned) vis_raster_kernel<true, true><<<grid, threads, smem, s>>>(RAST_ARGS); else vis_raster_kernel<true, false><<<grid, threads, smem, s>>>(RAST_ARGS); }
+  else { if (binned) vis_raster_kernel<false, true><<<grid, threads, smem, s>>>(RAST_ARGS); else vis_raster_kernel<false, false><<<grid, threads, smem, s>>>(RAST_ARGS); }
   av->launches += 1;
   rga_prof_mark(av, "vis_raster", s);
+  return cudaGetLastError();
+}
+
+// scratch for the triangle lists of banded maps: bands needed at the declared maximum resolution (0: the map fits whole)
+int rga_vis_raster_max_bands(int max_res, int n_verts) {
+  int rows = 0, th = 0, worst = 1;
+  for (int with_id = 0; with_id < 2; ++with_id)
+    for (int res = 1; res <= max_res; ++res) {               // the planner is cheap; band counts are not monotone in res
+      rga_vis_raster_smem(res, with_id, n_verts, &rows, &th);
+      if (rows < 1) continue;
+      const int b = (res + rows - 1) / rows;
+      if (b > worst) worst = b;
+    }
+  return worst > 1 ? worst : 0;
+}
+
+// Pre-scaled light frames and depth-test constants for the fused depth-test + shading kernel (vis_shade_kernels.cu, a FAST
+// file): computed HERE, in the EXACT file, by the same make_win / make_frame as every other visibility kernel.
+// out: float4[2 + 3K]: (cx, cy, cz, hR) (bias_texels / R, bias_world * inv2r, slope_max, R) then per direction
+// (us, w.x) (vs, w.y) (wn, w.z).
+__global__ void light_frames_kernel(int K, int R, const float* __restrict__ dirs, const float* __restrict__ window, float bias_texels,
+                                    float bias_world, float slope_max, float4* __restrict__ out) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const WinConst W = make_win(window, R);
+  if (k == 0) {
+    out[0] = make_float4(W.cx, W.cy, W.cz, W.hR);
+    out[1] = make_float4(bias_texels / (float)R, bias_world * W.inv2r, slope_max, (float)R);
+  }
+  if (k >= K) return;
+  const LightFrame f = make_frame(dirs + 3 * k, W);
+  out[2 + 3 * k] = make_float4(f.us[0], f.us[1], f.us[2], f.w[0]);
+  out[2 + 3 * k + 1] = make_float4(f.vs[0], f.vs[1], f.vs[2], f.w[1]);
+  out[2 + 3 * k + 2] = make_float4(f.wn[0], f.wn[1], f.wn[2], f.w[2]);
+}
+
+cudaError_t rga_launch_light_frames(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {
+  light_frames_kernel<<<(p->n_dirs + 127) / 128, 128, 0, s>>>(p->n_dirs, p->res, p->dirs, av->window, p->depth_bias_texels, p->depth_bias_world,
+                                                             p->slope_max, reinterpret_cast<float4*>(av->frames));
+  rga_prof_mark(av, "light_frames", s);
+  av->launches += 1;
   return cudaGetLastError();
 }
 
@@ -685,9 +794,11 @@ cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaSt
 }
 
 int rga_vis_init_attributes() {
-  const int mx = 227 * 1024 - 256;            // the static s_next counts against the 227 KB block limit
-  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  const int mx = 227 * 1024 - 512;            // the static counters count against the 227 KB block limit
+  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_depth_test_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   return (int)e;
 }
