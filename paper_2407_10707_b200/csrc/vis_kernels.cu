@@ -90,7 +90,7 @@ cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s) {
 struct RasterWarp {
   uint4 tab[4][32];            // round table (component-major: lanes read neighbouring owners without bank conflicts):
                                // edge-function coefficients and box of the 32 triangles being sampled
-  uint4 q2[RAST_Q];            // row segments with covered samples: {triangle | mask << 24 | wide << 31, pixel, e1, e2}
+  uint4 q2[RAST_Q];            // runs with covered samples: {triangle | mask << 24 | tall << 28 | wide << 31, first pixel, e1, e2}
   int q1[RAST_Q];              // triangles whose pixel box is not empty
 };
 
@@ -137,7 +137,12 @@ __device__ __forceinline__ void raster_depth(const RasterCtx& c, const RasterWar
   int i0, i1, i2;
   face_unpack(__ldg(c.faces_packed + t), i0, i1, i2);
   const float4 a = __ldg(c.v_posed + i0), b = __ldg(c.v_posed + i1), e = __ldg(c.v_posed + i2);
-  const unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
+  // a tall run (down a column) was sampled with x and y exchanged: exchange them here too (a 16-bit rotation of the packed
+  // corner); edge functions and area both change sign under the exchange, so e1 / area and e2 / area are unchanged
+  const bool tall = (q.x >> 28) & 1u;
+  const int rot = tall ? 16 : 0;
+  const unsigned P0 = __funnelshift_l(c.sXY[i0], c.sXY[i0], rot), P1 = __funnelshift_l(c.sXY[i1], c.sXY[i1], rot),
+                 P2 = __funnelshift_l(c.sXY[i2], c.sXY[i2], rot);
   const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
   // z = fma(wn.z, d.z, fma(wn.y, d.y, fma(wn.x, d.x, 0.5))): the frame is read from shared memory (kept in registers it
   // cost the sampling loop 20 registers it never uses)
@@ -145,25 +150,27 @@ __device__ __forceinline__ void raster_depth(const RasterCtx& c, const RasterWar
   const float z0 = __fmaf_rn(wnz, a.z - cz, __fmaf_rn(wny, a.y - cy, __fmaf_rn(wnx, a.x - cx, 0.5f)));
   const float z1 = __fmaf_rn(wnz, b.z - cz, __fmaf_rn(wny, b.y - cy, __fmaf_rn(wnx, b.x - cx, 0.5f)));
   const float z2 = __fmaf_rn(wnz, e.z - cz, __fmaf_rn(wny, e.y - cy, __fmaf_rn(wnx, e.x - cx, 0.5f)));
+  const int pstep = tall ? c.R : 1;                                 // the run goes down a column (pixel stride R) or along a row
   if (!(q.x >> 31)) {
     const int area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
     const int ax1 = -256 * (y0 - y2), ax2 = -256 * (y1 - y0);
     const float fa = (float)area;
     for (unsigned m = mask; m; m &= m - 1u) {                         // usually one covered sample per run
       const int u = __ffs(m) - 1;
-      put_depth<WITH_ID>(c, (int)q.y + u, t, (float)((int)q.z + u * ax1), (float)((int)q.w + u * ax2), fa, z0, z1, z2);
+      put_depth<WITH_ID>(c, (int)q.y + u * pstep, t, (float)((int)q.z + u * ax1), (float)((int)q.w + u * ax2), fa, z0, z1, z2);
     }
   } else {                                                          // triangle spanning >= 64 pixels: int64 edge functions
-    const int prow = (int)q.y / c.R, pcol = (int)q.y - prow * c.R;
+    const int prow = (int)q.y / c.R + c.row0, pcol = (int)q.y % c.R;
     const long long X0 = x0, Y0 = y0, X1 = x1, Y1 = y1, X2 = x2, Y2 = y2;
     const long long area = (X1 - X0) * (Y2 - Y0) - (Y1 - Y0) * (X2 - X0);
-    const long long qy = 256ll * (prow + c.row0) + 128;
     for (int u = 0; u < RAST_SEGW; ++u) {
       if ((mask >> u) & 1u) {
-        const long long qx = 256ll * (pcol + u) + 128;
+        // sample (column, row) of the map; in the exchanged space of a tall run its coordinates are (row, column)
+        const int sc = pcol + (tall ? 0 : u), sr = prow + (tall ? u : 0);
+        const long long qx = 256ll * (tall ? sr : sc) + 128, qy = 256ll * (tall ? sc : sr) + 128;
         const long long e1 = (X0 - X2) * (qy - Y2) - (Y0 - Y2) * (qx - X2);
         const long long e2 = (X1 - X0) * (qy - Y0) - (Y1 - Y0) * (qx - X0);
-        put_depth<WITH_ID>(c, (int)q.y + u, t, (float)e1, (float)e2, (float)area, z0, z1, z2);
+        put_depth<WITH_ID>(c, (int)q.y + u * pstep, t, (float)e1, (float)e2, (float)area, z0, z1, z2);
       }
     }
   }
@@ -180,10 +187,20 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
     const int t = w->q1[qbase + lane];
     int i0, i1, i2;
     face_unpack(__ldg(c.faces_packed + t), i0, i1, i2);
-    const unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
+    unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
     int ia, ja, bw, bh; bool narrow;
     tri_box(P0, P1, P2, c.R, c.row0, c.rows, ia, ja, bw, bh, narrow);
-    const int nsr = (bw + RAST_SEGW - 1) / RAST_SEGW;                 // segments per row
+    // runs go along the LONGER side of the box (the body's limbs make most boxes taller than wide: with runs along x only a
+    // 1 x 3 box was three runs of one sample).  A tall box is sampled with x and y EXCHANGED -- a 16-bit rotation of the
+    // packed corners and a swap of the box -- so the code below only knows runs along x; all three edge functions change sign
+    // together under the exchange, which the two-sided inside test does not see.
+    const bool tall = bh > bw;
+    const unsigned origin = (unsigned)((ja - c.row0) * c.R + ia);
+    if (tall) {
+      P0 = __funnelshift_l(P0, P0, 16); P1 = __funnelshift_l(P1, P1, 16); P2 = __funnelshift_l(P2, P2, 16);
+      int tmp = ia; ia = ja; ja = tmp; tmp = bw; bw = bh; bh = tmp;
+    }
+    const int nsr = (bw + RAST_SEGW - 1) / RAST_SEGW;                 // runs per line
     cnt = bh * nsr;
     const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
     const int qx = 256 * ia + 128, qy = 256 * ja + 128;
@@ -199,7 +216,7 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
         ay0 = 256 * (x2 - x1); ay1 = 256 * (x0 - x2); ay2 = 256 * (x1 - x0);
       }
     }
-    boxw = (unsigned)((ja - c.row0) * c.R + ia) | ((unsigned)(bw - 1) << 16) | (narrow ? (1u << 24) : 0u);
+    boxw = origin | ((unsigned)(bw - 1) << 16) | (narrow ? (1u << 24) : 0u) | (tall ? (1u << 25) : 0u);
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"((float)nsr));       // only splits an index (error analysis below)
     ay2u = (unsigned)ay2;
     w->tab[0][lane] = make_uint4((unsigned)C0, (unsigned)ax0, (unsigned)ay0, (unsigned)C1);
@@ -229,8 +246,10 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
       const int li = s - (int)d.y, obw = (int)((d.z >> 16) & 0xffu) + 1, nsr = (obw + RAST_SEGW - 1) / RAST_SEGW;
       // li / nsr: (li + 0.5) / nsr is >= 1/128 away from an integer, the approximate reciprocal is within 2^-22
       const int row = (int)(((float)li + 0.5f) * __uint_as_float(d.w));
-      const int col0 = (li - row * nsr) * RAST_SEGW, ncol = min(RAST_SEGW, obw - col0);
-      out.y = (d.z & 0xffffu) + (unsigned)(row * c.R + col0);
+      const int col0 = (li - row * nsr) * RAST_SEGW, ncol = min(RAST_SEGW, obw - col0);      // row = line, col0 = offset along the run
+      const bool tall = d.z & (1u << 25);
+      out.y = (d.z & 0xffffu) + (unsigned)(tall ? col0 * c.R + row : row * c.R + col0);
+      if (tall) out.x = 1u << 28;
       if (d.z & (1u << 24)) {
         int e0 = (int)a.x + (int)a.y * col0 + (int)a.z * row;
         int e1 = (int)a.w + (int)b.x * col0 + (int)b.y * row;
@@ -245,10 +264,12 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
         const uint4 e = w->tab[3][owner];
         int i0, i1, i2;
         face_unpack(__ldg(c.faces_packed + e.x), i0, i1, i2);
-        const unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
+        const int rot = tall ? 16 : 0;                              // the same exchanged space as the setup
+        const unsigned P0 = __funnelshift_l(c.sXY[i0], c.sXY[i0], rot), P1 = __funnelshift_l(c.sXY[i1], c.sXY[i1], rot),
+                       P2 = __funnelshift_l(c.sXY[i2], c.sXY[i2], rot);
         const long long x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
-        const long long qy = 256ll * ((int)(e.y >> 16) + row) + 128;
         const long long area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
+        const long long qy = 256ll * ((int)(e.y >> 16) + row) + 128;
         for (int u = 0; u < ncol; ++u) {
           const long long qx = 256ll * ((int)(e.y & 0xffffu) + col0 + u) + 128;
           const long long e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
@@ -256,7 +277,7 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
           const long long e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
           if (((e0 >= 0 && e1 >= 0 && e2 >= 0) || (e0 <= 0 && e1 <= 0 && e2 <= 0)) && area != 0) mask |= 1u << u;
         }
-        out.x = 1u << 31;
+        out.x |= 1u << 31;
       }
       if (mask) out.x |= w->tab[3][owner].x | (mask << 24);
     }
