@@ -65,8 +65,9 @@ typedef enum {
 
 /* avatar_load input.  PAPER.md:86 lists the vertex attributes {r,s,a,gamma,p,w,n,dx}; PAPER.md:88 the Gaussians. */
 typedef struct {
-  int32_t n_verts, n_faces, n_bones, n_gauss;   /* n_verts < 2^21 and small enough for the rasteriser's shared-memory
-                                                    vertex table (about 49k), n_faces < 2^24                           */
+  int32_t n_verts, n_faces, n_bones, n_gauss;   /* n_verts < 2^21, n_faces < 2^24 (packed faces).  Beyond about 45k vertices the
+                                                    rasteriser's table of snapped coordinates moves from shared memory to an
+                                                    L2-resident scratch buffer (slower, same results)                    */
   int32_t k_g;                 /* neighbours per Gaussian, 1..3 (paper: 3)          */
   int32_t k_v;                 /* neighbours per vertex, odd, 1..31 (paper: 19); clamped to n_verts */
   const float*   vert_pos;     /* dev [n_verts][3]  canonical x                                      */
@@ -78,14 +79,20 @@ typedef struct {
   const float*   vert_rough;   /* dev [n_verts]     gamma                                            */
   const float*   vert_spec;    /* dev [n_verts]     specular tint p                                  */
   const float*   gauss_pos;    /* dev [n_gauss][3]  canonical x_g                                    */
-  const float*   gauss_quat;   /* dev [n_gauss][4]  (w,x,y,z), any non-zero norm                      */
-  const float*   gauss_scale;  /* dev [n_gauss][3]                                                   */
+  const float*   gauss_quat;   /* dev [n_gauss][4]  (w,x,y,z), any non-zero norm; NULL = interpolate vert_quat  */
+  const float*   gauss_scale;  /* dev [n_gauss][3]; NULL = interpolate vert_scale                        */
   const float*   gauss_opacity;/* dev [n_gauss] or NULL = 1 ("always set the opacity ... to 1") */
   int32_t max_width, max_height;   /* largest camera this avatar will be rendered with                 */
   int32_t max_vis_dirs;            /* largest K_vis (multiple of 32 not required)                      */
   int32_t max_vis_res;             /* largest depth-map side R_v, <= 256 (snapped raster coordinates are 16-bit) */
   int32_t max_env_texels;          /* largest rows*cols of an environment map                           */
   int64_t max_duplicates;          /* capacity of the (tile,depth) key buffers; 0 = library picks       */
+  /* The paper's own layout: rotation r and scale s are VERTEX attributes interpolated to the Gaussians
+   * by Eq.1 like every other attribute.  Used when gauss_quat / gauss_scale is NULL (reading A2): neighbour
+   * quaternions are first given the sign of the nearest neighbour's (q and -q are the same rotation), then averaged with the
+   * Eq.1 weights; the result is normalised where it is used (H2). */
+  const float*   vert_quat;    /* dev [n_verts][4] (w,x,y,z) or NULL                                  */
+  const float*   vert_scale;   /* dev [n_verts][3] or NULL                                            */
 } rga_avatar_desc;
 
 typedef struct {
@@ -241,6 +248,12 @@ typedef struct {
   const float* bo;            /* dev [3]                                                              */
 } rga_disp_mlp;
 RGA_API rga_status displacement_mlp(rga_avatar* av, const rga_disp_mlp* mlp, const float* theta, void* stream);
+
+/* Back to the static per-vertex displacement given to avatar_load (NULL = 0) after displacement_mlp: x + dx for
+ * the mesh and Eq.1 of dx over the current S_g for the Gaussians, bit-identical to a fresh load.  Enqueue-only; call pose_skin
+ * afterwards.  (gaussians_update keeps whichever displacement is current: after displacement_mlp it re-interpolates the
+ * network's dx over the new neighbour sets.) */
+RGA_API rga_status displacement_static(rga_avatar* av, void* stream);
 
 /* Attribute maps: the same splat (H6-H10, incl. the back-face opacity kill) with the Gaussian's albedo a_g
  * (RGA_ATTR_ALBEDO; the albedo map of PAPER.md:177 and :239) or its posed normal n_gd, signed components

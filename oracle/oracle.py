@@ -56,6 +56,12 @@ def interp_attr(idx, ubar, attr):
     return out.reshape((len(idx),) + attr.shape[1:])
 
 
+def interp_quat(idx, ubar, vq):
+    vq = _f32(vq); out = np.empty((len(idx), 4), np.float32)
+    lib().orc_interp_quat(_p(idx), _p(ubar), C.c_int(len(idx)), C.c_int(idx.shape[1]), _p(vq), _p(out))
+    return out
+
+
 def normalize_rows3(v):
     v = _f32(v).copy()
     lib().orc_normalize_rows3(_p(v), C.c_int(len(v)))
@@ -281,6 +287,11 @@ def avatar_load(inp):
     av["spec_g"] = interp_attr(i, u, inp["vert_spec"])
     av["skin_w_g"] = interp_attr(i, u, inp["vert_skin_w"])
     av["disp_g"] = interp_attr(i, u, inp["vert_disp"])
+    # the paper's layout: rotation and scale as vertex attributes, used when no per-Gaussian array is given
+    if inp.get("gauss_quat") is None and inp.get("vert_quat") is not None:
+        av["quat_g"] = interp_quat(i, u, inp["vert_quat"])
+    if inp.get("gauss_scale") is None and inp.get("vert_scale") is not None:
+        av["scale_g"] = interp_attr(i, u, inp["vert_scale"])
     return av
 
 
@@ -304,7 +315,7 @@ def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None, gau
     o["vert_posed"], o["vert_normal_posed"], _ = skin(inp["vert_pos"], inp["vert_disp"], inp["vert_normal"],
                                                       inp["vert_skin_w"], G)
     o["gauss_posed"], o["gauss_normal_posed"], M = skin(inp["gauss_pos"], av["disp_g"], av["normal_g"], av["skin_w_g"], G)
-    o["cov6"] = gauss_cov(M, inp["gauss_quat"], inp["gauss_scale"])
+    o["cov6"] = gauss_cov(M, av["quat_g"] if "quat_g" in av else inp["gauss_quat"], av["scale_g"] if "scale_g" in av else inp["gauss_scale"])
     o["win_c"], o["win_r"] = window(o["vert_posed"])
     lap("skin")
     if stop_after == "skin":

@@ -71,6 +71,24 @@ ORC void orc_interp_attr(const int32_t* idx, const float* ubar, int n, int K, co
     }
 }
 
+// Eq.1 for the rotation attribute r (reading A2): q and -q are the same rotation, so every neighbour's
+// quaternion first takes the sign of neighbour 0's (dot4 < 0 -> negated); then the weighted sum in neighbour order, fp32,
+// no FMA.  The result is NOT normalised here: orc_gauss_cov normalises the quaternion it is given.
+ORC void orc_interp_quat(const int32_t* idx, const float* ubar, int n, int K, const float* vq, float* out) {
+  for (int i = 0; i < n; ++i) {
+    const float* q0 = vq + 4 * (size_t)idx[(size_t)i * K];
+    float acc[4];
+    for (int c = 0; c < 4; ++c) acc[c] = ubar[(size_t)i * K] * q0[c];
+    for (int k = 1; k < K; ++k) {
+      const float* qk = vq + 4 * (size_t)idx[(size_t)i * K + k];
+      float dt = ((qk[0] * q0[0] + qk[1] * q0[1]) + qk[2] * q0[2]) + qk[3] * q0[3];
+      float sg = dt < 0.0f ? -1.0f : 1.0f;
+      for (int c = 0; c < 4; ++c) acc[c] = acc[c] + ubar[(size_t)i * K + k] * (sg * qk[c]);
+    }
+    for (int c = 0; c < 4; ++c) out[4 * (size_t)i + c] = acc[c];
+  }
+}
+
 ORC void orc_normalize_rows3(float* v, int n) {
   for (int i = 0; i < n; ++i) {
     float* p = v + 3 * (size_t)i;

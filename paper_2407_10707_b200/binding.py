@@ -37,7 +37,7 @@ class _Desc(C.Structure):
                 ("vert_disp", C.c_void_p), ("vert_albedo", C.c_void_p), ("vert_rough", C.c_void_p), ("vert_spec", C.c_void_p),
                 ("gauss_pos", C.c_void_p), ("gauss_quat", C.c_void_p), ("gauss_scale", C.c_void_p), ("gauss_opacity", C.c_void_p),
                 ("max_width", C.c_int32), ("max_height", C.c_int32), ("max_vis_dirs", C.c_int32), ("max_vis_res", C.c_int32),
-                ("max_env_texels", C.c_int32), ("max_duplicates", C.c_int64)]
+                ("max_env_texels", C.c_int32), ("max_duplicates", C.c_int64), ("vert_quat", C.c_void_p), ("vert_scale", C.c_void_p)]
 
 
 class _Camera(C.Structure):
@@ -129,8 +129,9 @@ def avatar_load(inp, max_width, max_height, max_vis_dirs, max_vis_res, max_env_t
                 vert_skin_w=_dev(inp["vert_skin_w"], f32), vert_disp=_dev(inp.get("vert_disp"), f32),
                 vert_albedo=_dev(inp["vert_albedo"], f32), vert_rough=_dev(inp["vert_rough"], f32),
                 vert_spec=_dev(inp["vert_spec"], f32), gauss_pos=_dev(inp["gauss_pos"], f32),
-                gauss_quat=_dev(inp["gauss_quat"], f32), gauss_scale=_dev(inp["gauss_scale"], f32),
-                gauss_opacity=_dev(inp.get("gauss_opacity"), f32))
+                gauss_quat=_dev(inp.get("gauss_quat"), f32), gauss_scale=_dev(inp.get("gauss_scale"), f32),
+                gauss_opacity=_dev(inp.get("gauss_opacity"), f32), vert_quat=_dev(inp.get("vert_quat"), f32),
+                vert_scale=_dev(inp.get("vert_scale"), f32))
     d = _Desc()
     d.n_verts, d.n_faces = keep["vert_pos"].shape[0], keep["faces"].shape[0]
     d.n_bones, d.n_gauss = keep["vert_skin_w"].shape[1], keep["gauss_pos"].shape[0]
@@ -255,6 +256,12 @@ def displacement_mlp(h, mlp, theta):
     m = _DispMlp(int(mlp["n_freq"]), int(mlp["n_pose"]), *[mlp[k].data_ptr() for k in ("rff", "W1", "b1", "Wh", "bh", "Wo", "bo")])
     lib().displacement_mlp.argtypes = [C.c_void_p, C.POINTER(_DispMlp), C.c_void_p, C.c_void_p]
     _chk(lib().displacement_mlp(h, C.byref(m), _ptr(theta), _stream()))
+
+
+def displacement_static(h):
+    """Back to avatar_load's static displacement (include/rga.h displacement_static)."""
+    lib().displacement_static.argtypes = [C.c_void_p, C.c_void_p]
+    _chk(lib().displacement_static(h, _stream()))
 
 
 RGA_ATTR_ALBEDO, RGA_ATTR_NORMAL = 1, 2

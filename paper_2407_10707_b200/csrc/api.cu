@@ -56,7 +56,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->rast_bins, av->frames, av->front_list, av->n_front, av->vs_counter, av->dir_start, av->tex_list, av->tex_dir, av->dir_eps, av->g_order, av->g_inv, av->gi_pos, av->bb_scratch, av->bb_dev, av->vals[1], av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
+  void* ptrs[] = {av->vt_quat, av->vt_scale, av->rast_sxy, av->rast_bins, av->frames, av->front_list, av->n_front, av->vs_counter, av->dir_start, av->tex_list, av->tex_dir, av->dir_eps, av->g_order, av->g_inv, av->gi_pos, av->bb_scratch, av->bb_dev, av->vals[1], av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
                   av->vt_spec, av->knn_d2, av->grid_start, av->grid_verts, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
@@ -81,16 +81,15 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   if (d->k_g < 1 || d->k_g > 3) return fail(RGA_ERR_INVALID_ARG, "avatar_load: k_g must be 1..3");
   if (d->k_v < 1 || d->k_v > 31 || !(d->k_v & 1)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: k_v must be odd, 1..31");
   if (!d->vert_pos || !d->faces || !d->vert_normal || !d->vert_skin_w || !d->vert_albedo || !d->vert_rough || !d->vert_spec ||
-      !d->gauss_pos || !d->gauss_quat || !d->gauss_scale) return fail(RGA_ERR_INVALID_ARG, "avatar_load: missing table");
+      !d->gauss_pos || (!d->gauss_quat && !d->vert_quat) || (!d->gauss_scale && !d->vert_scale))
+    return fail(RGA_ERR_INVALID_ARG, "avatar_load: missing table (rotation and scale are needed per Gaussian or per vertex)");
   if (d->max_width < 1 || d->max_height < 1 || d->max_vis_dirs < 1 || d->max_vis_res < 1 || d->max_vis_res > 256 ||
-      d->max_env_texels < 1 || d->max_env_texels > 65535) return fail(RGA_ERR_INVALID_ARG, "avatar_load: bad maxima");
+      d->max_env_texels < 1) return fail(RGA_ERR_INVALID_ARG, "avatar_load: bad maxima");
+  if ((size_t)d->max_env_texels * 34 + 8 * 1024 > 227 * 1024)
+    return fail(RGA_ERR_INVALID_ARG, "avatar_load: max_env_texels = %d is above %d: the shading kernels stage the whole environment table "
+                "(34 bytes per texel) in shared memory", d->max_env_texels, (int)((227 * 1024 - 8 * 1024) / 34));
   if (d->n_verts >= (1 << 21)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: n_verts must be below 2^21 (packed faces)");
   if (d->n_faces >= (1 << 24)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: n_faces must be below 2^24 (rasteriser queue entries)");
-  {
-    int rows = 0, th = 0;
-    rga_vis_raster_smem(d->max_vis_res, 1, d->n_verts, &rows, &th);
-    if (rows < 1) return fail(RGA_ERR_INVALID_ARG, "avatar_load: mesh too large for the shared-memory vertex table of the rasteriser");
-  }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(RGA_ERR_CUDA, "avatar_load: no CUDA device (there is no CPU fallback)");
   cudaStream_t s = (cudaStream_t)stream;
@@ -121,6 +120,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->g_static, 4 * ng)); A(dalloc(&av->g_skin_w, ng * B)); A(dalloc(&av->g_quat, ng)); A(dalloc(&av->g_scale_op, ng));
   A(dalloc(&av->v_posed, nv)); A(dalloc(&av->v_nposed, nv)); A(dalloc(&av->g_posed, ng)); A(dalloc(&av->g_nposed, ng));
   A(dalloc(&av->g_cov, 6 * ng)); A(dalloc(&av->window, 4)); A(dalloc(&av->aabb, 8));
+  if (rga_vis_raster_needs_global_table(av->max_res, av->n_verts)) A(dalloc(&av->rast_sxy, (size_t)av->num_sms * nv));
   av->rast_bins_bands = rga_vis_raster_max_bands(av->max_res, av->n_verts);
   if (av->rast_bins_bands > 0) A(dalloc(&av->rast_bins, (size_t)av->num_sms * av->rast_bins_bands * (size_t)av->n_faces));
   A(dalloc(&av->zmap, nmap)); A(dalloc(&av->idmap, nmap)); A(dalloc(&av->visbits, ng * words));
@@ -161,6 +161,8 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(cudaMemcpyAsync(av->vt_albedo, d->vert_albedo, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
   A(cudaMemcpyAsync(av->vt_rough, d->vert_rough, nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
   A(cudaMemcpyAsync(av->vt_spec, d->vert_spec, nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  if (d->vert_quat && !d->gauss_quat) { A(dalloc(&av->vt_quat, 4 * nv)); A(cudaMemcpyAsync(av->vt_quat, d->vert_quat, 4 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s)); }
+  if (d->vert_scale && !d->gauss_scale) { A(dalloc(&av->vt_scale, 3 * nv)); A(cudaMemcpyAsync(av->vt_scale, d->vert_scale, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s)); }
   if (d->vert_disp) {
     A(dalloc(&av->vt_disp, 3 * nv));
     A(cudaMemcpyAsync(av->vt_disp, d->vert_disp, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
@@ -184,16 +186,16 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
     int npad = 2048; while (npad < av->n_gauss) npad <<= 1;
     unsigned long long* okeys = nullptr; float *pq = nullptr, *ps = nullptr, *po = nullptr;
     cudaError_t e_ = dalloc(&okeys, (size_t)npad);
-    if (e_ == cudaSuccess) e_ = dalloc(&pq, 4 * ng);
-    if (e_ == cudaSuccess) e_ = dalloc(&ps, 3 * ng);
+    if (e_ == cudaSuccess && d->gauss_quat) e_ = dalloc(&pq, 4 * ng);
+    if (e_ == cudaSuccess && d->gauss_scale) e_ = dalloc(&ps, 3 * ng);
     if (e_ == cudaSuccess && d->gauss_opacity) e_ = dalloc(&po, ng);
     if (e_ == cudaSuccess) e_ = rga_build_gauss_order(d->gauss_pos, av->n_gauss, okeys, npad, av->bb_scratch, av->bb_dev, av->g_order, av->g_inv, s);
     if (e_ == cudaSuccess) e_ = rga_gather_rows(av->n_gauss, 3, d->gauss_pos, av->g_order, av->gi_pos, s);
-    if (e_ == cudaSuccess) e_ = rga_gather_rows(av->n_gauss, 4, d->gauss_quat, av->g_order, pq, s);
-    if (e_ == cudaSuccess) e_ = rga_gather_rows(av->n_gauss, 3, d->gauss_scale, av->g_order, ps, s);
+    if (e_ == cudaSuccess && pq) e_ = rga_gather_rows(av->n_gauss, 4, d->gauss_quat, av->g_order, pq, s);
+    if (e_ == cudaSuccess && ps) e_ = rga_gather_rows(av->n_gauss, 3, d->gauss_scale, av->g_order, ps, s);
     if (e_ == cudaSuccess && po) e_ = rga_gather_rows(av->n_gauss, 1, d->gauss_opacity, av->g_order, po, s);
     if (e_ == cudaSuccess) e_ = rga_launch_knn_gauss(av, av->gi_pos, s);
-    if (e_ == cudaSuccess) e_ = rga_launch_load_gauss(av, av->gi_pos, pq, ps, po, av->knn_d2, s);
+    if (e_ == cudaSuccess) e_ = rga_launch_load_gauss(av, av->gi_pos, pq, ps, po, av->knn_d2, s, pq ? nullptr : d->vert_quat, ps ? nullptr : d->vert_scale, 1);
     if (e_ == cudaSuccess) e_ = cudaStreamSynchronize(s);
     cudaFree(okeys); cudaFree(pq); cudaFree(ps); cudaFree(po);
     if (e_ != cudaSuccess) { st = fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, "avatar_load: Gaussian order / tables: %s", cudaGetErrorString(e_)); goto done; }
@@ -286,7 +288,7 @@ extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, v
   CU(rga_gather_rows(av->n_gauss, 3, gauss_pos, av->g_order, av->gi_pos, s));      // caller order -> library order (kept from the load)
   CU(rga_launch_knn_gauss(av, av->gi_pos, s));
   rga_prof_mark(av, "knn_g", s);
-  CU(rga_launch_load_gauss(av, av->gi_pos, nullptr, nullptr, nullptr, av->knn_d2, s));
+  CU(rga_launch_load_gauss(av, av->gi_pos, nullptr, nullptr, nullptr, av->knn_d2, s, av->vt_quat, av->vt_scale, 0));
   rga_prof_mark(av, "load_gauss", s);
   av->launches += 3;
   // the displacement network's per-pose dx (if it is the current displacement) is re-interpolated over the new S_g
@@ -385,6 +387,18 @@ extern "C" rga_status displacement_mlp(rga_avatar* av, const rga_disp_mlp* mlp, 
   return RGA_OK;
 }
 
+// back to the static per-vertex displacement of avatar_load after displacement_mlp
+extern "C" rga_status displacement_static(rga_avatar* av, void* stream) {
+  if (!av) return fail(RGA_ERR_INVALID_ARG, "displacement_static: null avatar");
+  cudaStream_t s = (cudaStream_t)stream;
+  av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
+  rga_prof_mark(av, "-", s);
+  CU(rga_launch_disp_static(av, s));
+  CU(rga_launch_disp_apply(av, s));
+  av->disp_is_mlp = 0;
+  return RGA_OK;
+}
+
 extern "C" rga_status splat_attribute(rga_avatar* av, const rga_camera* cam, const float bg[3], int which, float* out_image,
                                       void* stream) {
   if (!av || !cam || !bg || !out_image) return fail(RGA_ERR_INVALID_ARG, "splat_attribute: null argument");
@@ -426,6 +440,13 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   cudaStream_t s = (cudaStream_t)stream;
   const bool overlap = !av->prof_on;                       // per-kernel events need one stream
   cudaStream_t s2 = overlap ? av->side : s;
+  // a failure after the fork must not leave the second stream un-joined (inside a CUDA-graph capture that would invalidate
+  // the capture): join it, forget the half-built pose state, then report
+  bool forked = false;
+#define CUF(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { \
+    if (forked) { cudaEventRecord(av->ev_join, s2); cudaStreamWaitEvent(s, av->ev_join, 0); } \
+    av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0; \
+    return fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, "rga_render_frame: %s: %s", #expr, cudaGetErrorString(e_)); } } while (0)
   const int TX = (cam->width + 15) / 16, TY = (cam->height + 15) / 16, ntiles = TX * TY;
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
   rga_prof_mark(av, "-", s);
@@ -435,34 +456,34 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   const bool fused = vis && vis->mode == 0 && env->use_visibility && rga_vis_shade_teams(vis->n_dirs, env->rows * env->cols) > 0;
   if (overlap) {
     // the rasteriser only needs the posed mesh and the window: the Gaussians are skinned on the second stream
-    CU(cudaEventRecord(av->ev_fork, s)); CU(cudaStreamWaitEvent(s2, av->ev_fork, 0));
-    CU(rga_launch_skin(av, bone_mats, 1, s));
-    CU(rga_launch_skin(av, bone_mats, 2, s2));
-  } else CU(rga_launch_skin(av, bone_mats, 0, s));
+    CUF(cudaEventRecord(av->ev_fork, s)); CUF(cudaStreamWaitEvent(s2, av->ev_fork, 0)); forked = true;
+    CUF(rga_launch_skin(av, bone_mats, 1, s));
+    CUF(rga_launch_skin(av, bone_mats, 2, s2));
+  } else CUF(rga_launch_skin(av, bone_mats, 0, s));
   av->have_skin = 1;
-  if (fused) CU(rga_launch_front_compact(av, (vis->n_dirs + 31) / 32, cam3, s2));
-  if (overlap) CU(cudaEventRecord(av->ev_gskin, s2));
-  CU(rga_launch_env_table(av, env, s2));
-  if (fused) CU(rga_launch_texel_csr(av, env, vis, s2));
-  if (overlap) CU(cudaEventRecord(av->ev_env, s2));
-  CU(rga_launch_project(av, cam, s2));
-  CU(rga_launch_bin(av, TX, ntiles, s2));
-  CU(rga_launch_tile_sort(av, cam, s2));
-  if (overlap) CU(cudaEventRecord(av->ev_join, s2));
+  if (fused) CUF(rga_launch_front_compact(av, (vis->n_dirs + 31) / 32, cam3, s2));
+  if (overlap) CUF(cudaEventRecord(av->ev_gskin, s2));
+  CUF(rga_launch_env_table(av, env, s2));
+  if (fused) CUF(rga_launch_texel_csr(av, env, vis, s2));
+  if (overlap) CUF(cudaEventRecord(av->ev_env, s2));
+  CUF(rga_launch_project(av, cam, s2));
+  CUF(rga_launch_bin(av, TX, ntiles, s2));
+  CUF(rga_launch_tile_sort(av, cam, s2));
+  if (overlap) CUF(cudaEventRecord(av->ev_join, s2));
   av->vis_partial = 0;
   if (vis) {
-    CU(rga_launch_vis_raster(av, vis, s));
-    if (overlap) CU(cudaStreamWaitEvent(s, av->ev_gskin, 0));
+    CUF(rga_launch_vis_raster(av, vis, s));
+    if (overlap) CUF(cudaStreamWaitEvent(s, av->ev_gskin, 0));
     if (fused) {
-      if (overlap) CU(cudaStreamWaitEvent(s, av->ev_env, 0));
-      CU(rga_launch_vis_shade(av, vis, env, cam3, s));
+      if (overlap) CUF(cudaStreamWaitEvent(s, av->ev_env, 0));
+      CUF(rga_launch_vis_shade(av, vis, env, cam3, s));
       av->vis_culled = 1; av->vis_cull_cam[0] = cam_pos[0]; av->vis_cull_cam[1] = cam_pos[1]; av->vis_cull_cam[2] = cam_pos[2];
       av->vis_partial = 1; av->vs_t2d = env->texel_to_dir; av->vs_rows = env->rows; av->vs_cols = env->cols;
     } else if (vis->mode == 0) {
-      CU(rga_launch_vis_depth_test(av, vis, cam_pos, s));
+      CUF(rga_launch_vis_depth_test(av, vis, cam_pos, s));
       av->vis_culled = 1; av->vis_cull_cam[0] = cam_pos[0]; av->vis_cull_cam[1] = cam_pos[1]; av->vis_cull_cam[2] = cam_pos[2];
     } else {
-      CU(rga_launch_vis_paper(av, vis, s));
+      CUF(rga_launch_vis_paper(av, vis, s));
       av->vis_culled = 0;
     }
     av->vis_mode = vis->mode; av->vis_dirs = vis->n_dirs; av->vis_res = vis->res; av->vis_words = (vis->n_dirs + 31) / 32;
@@ -470,15 +491,16 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
     av->have_vis = 1;
   }
   if (!fused) {
-    if (overlap) { if (!vis) CU(cudaStreamWaitEvent(s, av->ev_gskin, 0)); CU(cudaStreamWaitEvent(s, av->ev_env, 0)); }
-    CU(rga_launch_shade(av, env, cam3, env->use_visibility ? av->vis_mode : 2, s));
+    if (overlap) { if (!vis) CUF(cudaStreamWaitEvent(s, av->ev_gskin, 0)); CUF(cudaStreamWaitEvent(s, av->ev_env, 0)); }
+    CUF(rga_launch_shade(av, env, cam3, env->use_visibility ? av->vis_mode : 2, s));
   }
   av->have_shade = 1;
-  if (overlap) CU(cudaStreamWaitEvent(s, av->ev_join, 0));
-  CU(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->color, out_image, s));
+  if (overlap) CUF(cudaStreamWaitEvent(s, av->ev_join, 0));
+  CUF(rga_launch_composite(av, cam, make_float3(bg[0], bg[1], bg[2]), av->color, out_image, s));
   av->cam_w = cam->width; av->cam_h = cam->height;
   av->have_splat = 1; av->splat_is_attr = 0;
   return RGA_OK;
+#undef CUF
 }
 
 extern "C" rga_status rga_check(rga_avatar* av, void* stream) {

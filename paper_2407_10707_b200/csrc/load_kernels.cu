@@ -81,7 +81,8 @@ __global__ void __launch_bounds__(128) load_gauss_kernel(int n, int K, int B, co
                                   const float* __restrict__ vw, const float* __restrict__ gquat,
                                   const float* __restrict__ gscale, const float* __restrict__ gop,
                                   float* __restrict__ ubar, float4* __restrict__ gst, float* __restrict__ gw,
-                                  float4* __restrict__ quat, float4* __restrict__ scale_op, float4* __restrict__ gpos4) {
+                                  float4* __restrict__ quat, float4* __restrict__ scale_op, float4* __restrict__ gpos4,
+                                  const float* __restrict__ vquat, const float* __restrict__ vscale, int set_opacity) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n) return;
   float u[4]; int id[4];
@@ -108,20 +109,40 @@ __global__ void __launch_bounds__(128) load_gauss_kernel(int n, int K, int B, co
   gst[4 * (size_t)g + 2] = make_float4(interp(valb, 3, 0), interp(valb, 3, 1), interp(valb, 3, 2), interp(vrough, 1, 0));
   gst[4 * (size_t)g + 3] = make_float4(interp(vspec, 1, 0), 0.f, 0.f, 0.f);
   for (int b = 0; b < B; ++b) gw[(size_t)g * B + b] = interp(vw, B, b);
-  if (gquat) {                                               // NULL on gaussians_update: rotation, scale and opacity stay
-    quat[g] = make_float4(gquat[4 * (size_t)g], gquat[4 * (size_t)g + 1], gquat[4 * (size_t)g + 2], gquat[4 * (size_t)g + 3]);
-    scale_op[g] = make_float4(gscale[3 * (size_t)g], gscale[3 * (size_t)g + 1], gscale[3 * (size_t)g + 2], gop ? gop[g] : 1.0f);
+  // rotation and scale: the caller's per-Gaussian arrays, or (the paper's layout; reading A2) Eq.1 of the
+  // vertex attributes -- neighbour quaternions take the sign of neighbour 0's first (dot4 < 0 -> negated), then the
+  // weighted sum in neighbour order; it is normalised where it is used (H2).  Both NULL (gaussians_update with per-Gaussian
+  // rotations): kept as they are.
+  if (gquat) quat[g] = make_float4(gquat[4 * (size_t)g], gquat[4 * (size_t)g + 1], gquat[4 * (size_t)g + 2], gquat[4 * (size_t)g + 3]);
+  else if (vquat) {
+    const float* q0 = vquat + 4 * (size_t)id[0];
+    float acc[4] = {u[0] * q0[0], u[0] * q0[1], u[0] * q0[2], u[0] * q0[3]};
+    for (int k = 1; k < K; ++k) {
+      const float* qk = vquat + 4 * (size_t)id[k];
+      const float dt = ((qk[0] * q0[0] + qk[1] * q0[1]) + qk[2] * q0[2]) + qk[3] * q0[3];
+      const float sg = dt < 0.f ? -1.0f : 1.0f;
+      for (int c = 0; c < 4; ++c) acc[c] = acc[c] + u[k] * (sg * qk[c]);
+    }
+    quat[g] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+  }
+  if (gscale || vscale || set_opacity) {
+    float4 so = scale_op[g];
+    if (gscale) { so.x = gscale[3 * (size_t)g]; so.y = gscale[3 * (size_t)g + 1]; so.z = gscale[3 * (size_t)g + 2]; }
+    else if (vscale) { so.x = interp(vscale, 3, 0); so.y = interp(vscale, 3, 1); so.z = interp(vscale, 3, 2); }
+    if (set_opacity) so.w = gop ? gop[g] : 1.0f;
+    scale_op[g] = so;
   }
 }
 
 // Eq.1 of every static attribute from the library's own copies of the vertex tables (so that gaussians_update can run
 // after the caller's arrays are gone); gauss_quat == NULL keeps rotation / scale / opacity.
 cudaError_t rga_launch_load_gauss(rga_avatar* av, const float* gauss_pos, const float* gauss_quat, const float* gauss_scale,
-                                  const float* gauss_opacity, const float* d2, cudaStream_t s) {
+                                  const float* gauss_opacity, const float* d2, cudaStream_t s, const float* vert_quat, const float* vert_scale,
+                                  int set_opacity) {
   load_gauss_kernel<<<(av->n_gauss + 127) / 128, 128, 0, s>>>(
       av->n_gauss, av->k_g, av->n_bones, av->knn_g, d2, gauss_pos, av->vt_disp, av->vt_normal, av->vt_albedo,
       av->vt_rough, av->vt_spec, av->v_skin_w, gauss_quat, gauss_scale, gauss_opacity, av->ubar_g,
-      av->g_static, av->g_skin_w, av->g_quat, av->g_scale_op, av->g_pos);
+      av->g_static, av->g_skin_w, av->g_quat, av->g_scale_op, av->g_pos, vert_quat, vert_scale, set_opacity);
   return cudaGetLastError();
 }
 
@@ -146,6 +167,19 @@ __global__ void __launch_bounds__(256) disp_apply_kernel(int nv, int ng, int K, 
     const float4 p = g_pos[g];
     g_static[4 * (size_t)g] = make_float4(p.x + ax, p.y + ay, p.z + az, 0.f);
   }
+}
+
+// the static per-vertex displacement table of avatar_load (or zero) back into the per-pose displacement buffer
+__global__ void disp_static_kernel(int nv, const float* __restrict__ vt_disp, float4* __restrict__ v_disp) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= nv) return;
+  v_disp[i] = vt_disp ? make_float4(vt_disp[3 * (size_t)i], vt_disp[3 * (size_t)i + 1], vt_disp[3 * (size_t)i + 2], 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+cudaError_t rga_launch_disp_static(rga_avatar* av, cudaStream_t s) {
+  disp_static_kernel<<<(av->n_verts + 255) / 256, 256, 0, s>>>(av->n_verts, av->vt_disp, av->v_disp);
+  av->launches += 1;
+  return cudaGetLastError();
 }
 
 cudaError_t rga_launch_disp_apply(rga_avatar* av, cudaStream_t s) {

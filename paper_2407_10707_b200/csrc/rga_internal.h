@@ -25,6 +25,7 @@ struct rga_avatar {
   int *g_order, *g_inv; float* gi_pos; unsigned* bb_scratch; float* bb_dev;
   // the library's copies of the vertex tables Eq.1 reads (gaussians_update re-interpolates from them)
   float *vt_pos, *vt_disp, *vt_normal, *vt_albedo, *vt_rough, *vt_spec;   // [n_verts][3] x4 (disp NULL = 0), [n_verts] x2
+  float *vt_quat, *vt_scale;   // [n_verts][4], [n_verts][3]: the paper's per-vertex rotation / scale when they are interpolated (else NULL)
   float* knn_d2;       // [n_gauss][k_g] squared distances of the last Gaussian KNN
   // uniform grid over the canonical vertices (exact KNN of the Gaussians); grid_G == 0: brute force
   int grid_G; float grid_h, grid_o[3]; unsigned* grid_start; int* grid_verts;
@@ -52,6 +53,7 @@ struct rga_avatar {
   float* window;       // [4] centre, radius; [4..9] scratch AABB as ordered ints
   unsigned* aabb;      // [8] ordered-uint min xyz, max xyz; [6] counts skin_kernel's finished vertex blocks
   // visibility
+  unsigned* rast_sxy;  // [num_sms][n_verts] snapped vertex coordinates of meshes whose table does not fit shared memory
   unsigned* rast_bins; int rast_bins_bands;   // [num_sms][bands][n_faces] triangle lists of banded depth maps (vis_raster)
   unsigned* zmap;      // [max_dirs][res*res]
   int* idmap;          // [max_dirs][res*res]  (allocated lazily at load: always, sized like zmap)
@@ -114,7 +116,8 @@ void rga_prof_mark(rga_avatar* av, const char* name, cudaStream_t s);
 cudaError_t rga_launch_knn(const float* q, int nq, const float* v, int nv, int K, int* idx, float* d2, cudaStream_t s);
 cudaError_t rga_launch_load_verts(rga_avatar* av, const float* pos, const float* disp, const float* nrm, cudaStream_t s);
 cudaError_t rga_launch_load_gauss(rga_avatar* av, const float* gauss_pos, const float* gauss_quat, const float* gauss_scale,
-                                  const float* gauss_opacity, const float* d2, cudaStream_t s);
+                                  const float* gauss_opacity, const float* d2, cudaStream_t s, const float* vert_quat = nullptr,
+                                  const float* vert_scale = nullptr, int set_opacity = 0);
 // order_kernels.cu
 cudaError_t rga_points_aabb(const float* pos, int n, unsigned* scratch6, float* out6_dev, cudaStream_t s);
 cudaError_t rga_build_gauss_order(const float* pos, int n, unsigned long long* keys, int npad, unsigned* bb_u, float* bb_dev,
@@ -129,6 +132,8 @@ cudaError_t rga_launch_vis_depth_test(rga_avatar* av, const rga_vis_params* p, c
 cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaStream_t s);
 size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads);
 int rga_vis_raster_max_bands(int max_res, int n_verts);
+int rga_vis_raster_needs_global_table(int max_res, int n_verts);
+size_t rga_vis_raster_plan(int res, int with_id, int n_verts, int* band_rows, int* threads, int* sxy_global);
 cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s);
 // vis_shade_kernels.cu
 int rga_vis_shade_teams(int K, int ne);
@@ -150,6 +155,7 @@ int rga_init_kernel_attributes();
 // mlp_kernels.cu / load_kernels.cu
 cudaError_t rga_launch_disp_mlp(rga_avatar* av, const rga_disp_mlp* m, const float* theta, cudaStream_t s);
 cudaError_t rga_launch_disp_apply(rga_avatar* av, cudaStream_t s);
+cudaError_t rga_launch_disp_static(rga_avatar* av, cudaStream_t s);
 cudaError_t rga_build_knn_grid(rga_avatar* av, const float* aabb_host, cudaStream_t s);
 cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s);
 cudaError_t rga_launch_knn_verts(rga_avatar* av, float* d2, cudaStream_t s);

@@ -18,7 +18,8 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int ntiles, long long c
     int* __restrict__ status) {
   __shared__ unsigned wsum[32], wseg[32];
   __shared__ unsigned carry, carry_seg, nlong;
-  if (threadIdx.x == 0) { carry = 0; carry_seg = 0; nlong = 0; }
+  __shared__ unsigned long long total64;                  // D in 64 bits: the 32-bit running sum may wrap before the capacity check
+  if (threadIdx.x == 0) { carry = 0; carry_seg = 0; nlong = 0; total64 = 0ull; }
   __syncthreads();
   for (int base = 0; base < ntiles; base += 1024) {
     int i = base + threadIdx.x;
@@ -28,6 +29,12 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int ntiles, long long c
     for (int o = 1; o < 32; o <<= 1) {
       unsigned t = __shfl_up_sync(0xffffffffu, incl, o), tg = __shfl_up_sync(0xffffffffu, gincl, o);
       if ((threadIdx.x & 31) >= o) { incl += t; gincl += tg; }
+    }
+    {
+      unsigned long long v64 = v;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v64 += __shfl_xor_sync(0xffffffffu, v64, o);
+      if ((threadIdx.x & 31) == 0 && v64) atomicAdd(&total64, v64);
     }
     if ((threadIdx.x & 31) == 31) { wsum[threadIdx.x >> 5] = incl; wseg[threadIdx.x >> 5] = gincl; }
     __syncthreads();
@@ -53,12 +60,13 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int ntiles, long long c
     if (threadIdx.x == 1023) { carry = excl + v; carry_seg = gexcl + g; }
     __syncthreads();
   }
-  const bool overflow = (long long)carry > capacity;
+  __syncthreads();
+  const bool overflow = total64 > (unsigned long long)capacity;
   if (overflow)                       // the key buffers cannot hold this frame: report it, render the background only
     for (int i = threadIdx.x; i < ntiles; i += 1024) { ranges[i] = make_uint2(0u, 0u); seg_off[i] = 0u; }
   if (threadIdx.x == 0) {
     if (overflow) atomicExch(status, RGA_ERR_CAPACITY);
-    *num_dup = carry;
+    *num_dup = total64 > 0xffffffffull ? 0xffffffffu : carry;
     seg_off[ntiles] = overflow ? 0u : carry_seg;
     *num_items = overflow ? 0u : carry_seg;
     *num_long = overflow ? 0u : nlong;

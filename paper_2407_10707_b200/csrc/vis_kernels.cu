@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
     const float4* __restrict__ v_posed, const unsigned long long* __restrict__ faces_packed, const float* __restrict__ dirs,
     const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
     unsigned* __restrict__ vbits_raw, int words, int cull, float4* __restrict__ frames_out, float bias_texels, float bias_world,
-    float slope_max, unsigned* __restrict__ bins, int band_magic) {
+    float slope_max, unsigned* __restrict__ bins, int band_magic, unsigned* __restrict__ sxy_scratch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int s_next;
   __shared__ unsigned s_bin_cnt[RAST_MAX_BANDS];
@@ -311,8 +311,9 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
   unsigned* sz32 = reinterpret_cast<unsigned*>(mp);
   unsigned long long* sz64 = reinterpret_cast<unsigned long long*>(mp);
   const size_t map_bytes = (((size_t)band_rows * R * (WITH_ID ? 8 : 4)) + 15) & ~(size_t)15;
-  unsigned* sXY = reinterpret_cast<unsigned*>(mp + map_bytes);
-  unsigned* svert = sXY + nv;
+  // snapped vertex coordinates: shared memory, or (large meshes) this CTA's slice of an L2-resident scratch buffer
+  unsigned* sXY = sxy_scratch ? sxy_scratch + (size_t)blockIdx.x * nv : reinterpret_cast<unsigned*>(mp + map_bytes);
+  unsigned* svert = reinterpret_cast<unsigned*>(mp + map_bytes) + (sxy_scratch ? 0 : nv);
   const int nv_words = (nv + 31) >> 5;
 
   // Work slots: units [0, tail_first) one CTA each; the units of the last, partial round of the persistent grid are cut
@@ -501,14 +502,17 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
   }
 }
 
-// shared-memory plan: picks the CTA size (1024 / 512 / 256 threads) that minimises bands / warps; returns bytes
-size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads) {
+// shared-memory plan: picks the CTA size (1024 / 512 / 256 threads) that minimises bands / warps; returns bytes.
+// *sxy_global = 1: the 4-byte-per-vertex table of snapped coordinates does not fit beside a useful band of the map (meshes
+// beyond about 45k vertices) and lives in an L2-resident scratch buffer instead -- same kernel, slower gathers.
+static size_t raster_plan(int res, int with_id, int n_verts, bool table_in_smem, int* band_rows, int* threads) {
   const size_t budget = 227 * 1024 - 512;               // static shared memory (counters, band list sizes) counts against the 227 KB
   const size_t per_row = (size_t)res * (with_id ? 8 : 4);
   size_t best = 0; double best_score = 1e30;
   *band_rows = 0; *threads = 0;
   for (int th = 1024; th >= 256; th >>= 1) {
-    const size_t fixed = (size_t)(th / 32) * sizeof(RasterWarp) + (size_t)n_verts * 4 + (with_id ? (size_t)((n_verts + 31) / 32) * 4 : 0) + 32;
+    const size_t fixed = (size_t)(th / 32) * sizeof(RasterWarp) + (table_in_smem ? (size_t)n_verts * 4 : 0) +
+                         (with_id ? (size_t)((n_verts + 31) / 32) * 4 : 0) + 32;
     if (fixed + per_row > budget) continue;
     int rows = (int)((budget - fixed) / per_row);
     if (rows > res) rows = res;
@@ -520,14 +524,27 @@ size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, in
       best = fixed + ((per_row * rows + 15) & ~(size_t)15);
     }
   }
-  return best;                                                        // 0: mesh too large for the shared-memory vertex table
+  return best;
+}
+
+size_t rga_vis_raster_plan(int res, int with_id, int n_verts, int* band_rows, int* threads, int* sxy_global) {
+  *sxy_global = 0;
+  size_t b = raster_plan(res, with_id, n_verts, true, band_rows, threads);
+  if (b != 0 && (res + *band_rows - 1) / *band_rows <= 16) return b;
+  *sxy_global = 1;
+  return raster_plan(res, with_id, n_verts, false, band_rows, threads);
+}
+
+size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads) {
+  int g = 0;
+  return rga_vis_raster_plan(res, with_id, n_verts, band_rows, threads, &g);
 }
 
 cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {
   const bool with_id = p->mode == 1 || p->keep_maps;
-  int band_rows = 0, threads = 0;
-  const size_t smem = rga_vis_raster_smem(p->res, with_id, av->n_verts, &band_rows, &threads);
-  if (band_rows < 1) return cudaErrorInvalidConfiguration;
+  int band_rows = 0, threads = 0, sxy_global = 0;
+  const size_t smem = rga_vis_raster_plan(p->res, with_id, av->n_verts, &band_rows, &threads, &sxy_global);
+  if (band_rows < 1 || (sxy_global && !av->rast_sxy)) return cudaErrorInvalidConfiguration;
   const int n_bands = (p->res + band_rows - 1) / band_rows;
   const int words = (p->n_dirs + 31) / 32;
   // a map cut into bands: one unit per direction, triangles binned by band (needs the scratch lists sized at load)
@@ -550,7 +567,7 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
   const int band_magic = (65536 + band_rows - 1) / band_rows;   // (row * magic) >> 16 == row / band_rows for row < 256
 #define RAST_ARGS av->n_faces, av->n_verts, p->res, band_rows, n_bands, n_units, tail_first, split, av->v_posed, av->faces_packed, p->dirs, av->window, \
     av->zmap, av->idmap, raw, words, p->cull_backfaces != 0, reinterpret_cast<float4*>(av->frames), p->depth_bias_texels, p->depth_bias_world, \
-    p->slope_max, binned ? av->rast_bins : nullptr, band_magic
+    p->slope_max, binned ? av->rast_bins : nullptr, band_magic, sxy_global ? av->rast_sxy : nullptr
   if (with_id) { if (binned) vis_raster_kernel<true, true><<<grid, threads, smem, s>>>(RAST_ARGS); else vis_raster_kernel<true, false><<<grid, threads, smem, s>>>(RAST_ARGS); }
   else { if (binned) vis_raster_kernel<false, true><<<grid, threads, smem, s>>>(RAST_ARGS); else vis_raster_kernel<false, false><<<grid, threads, smem, s>>>(RAST_ARGS); }
   av->launches += 1;
@@ -569,6 +586,14 @@ int rga_vis_raster_max_bands(int max_res, int n_verts) {
       if (b > worst) worst = b;
     }
   return worst > 1 ? worst : 0;
+}
+
+// does any map size up to max_res need the vertex table in global memory?
+int rga_vis_raster_needs_global_table(int max_res, int n_verts) {
+  int rows = 0, th = 0, g = 0;
+  for (int with_id = 0; with_id < 2; ++with_id)
+    for (int res = 1; res <= max_res; ++res) { rga_vis_raster_plan(res, with_id, n_verts, &rows, &th, &g); if (g) return 1; }
+  return 0;
 }
 
 // Pre-scaled light frames and depth-test constants for the fused depth-test + shading kernel (vis_shade_kernels.cu, a FAST

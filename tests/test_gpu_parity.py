@@ -533,3 +533,98 @@ def test_backface_cull_image_stays_within_tolerance_of_the_full_rasterisation(cf
     print(cfg, "image max / mean abs diff vs the unculled oracle:", d[o_full["flags"] == 0].max(), d.mean())
     assert d[o_full["flags"] == 0].max() <= IMG_MAX and d.mean() <= IMG_MEAN
     av.close()
+
+
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_mesh_larger_than_the_shared_memory_vertex_table(vis_mode):
+    # the paper's mesh has ~40K vertices; a denser one must still work.  The config-1 body subdivided twice
+    # (110,210 vertices / 220,416 faces) no longer fits the rasteriser's shared-memory table of snapped coordinates (4 B per
+    # vertex): the table then lives in an L2-resident scratch buffer.  Depth maps, ids, bits and counts stay bit-exact.
+    from oracle import oracle as orc
+    from parity_util import compare_all, run_gpu
+    from synth import mesh as smesh
+    inp = workloads.make(1, n_gauss=5_000)
+    v, f, J, _, _ = workloads._base_mesh("body0")
+    for _ in range(2):                                                      # two midpoint subdivisions of the 6,890-vertex body
+        v, f = smesh.subdivide(v, f)
+    w = smesh.two_nearest_joint_weights(v, J)                               # skinning weights by the generator's rule
+    rs = np.random.default_rng(42)
+    nv = len(v)
+    assert nv > 100_000
+    inp["vert_pos"] = np.ascontiguousarray(v, np.float32); inp["faces"] = np.ascontiguousarray(f, np.int32)
+    inp["vert_normal"] = np.ascontiguousarray(smesh.vertex_normals(v, f), np.float32)
+    inp["vert_skin_w"] = np.ascontiguousarray(w, np.float32)
+    inp["vert_disp"] = np.zeros((nv, 3), np.float32)
+    inp["vert_albedo"] = rs.uniform(0, 1, (nv, 3)).astype(np.float32)
+    inp["vert_rough"] = rs.uniform(0.1, 1, nv).astype(np.float32); inp["vert_spec"] = rs.uniform(0, 1, nv).astype(np.float32)
+    inp["vis_dirs"] = workloads.latlong_dirs(2, 8); inp["vis_res"] = 64
+    inp["texel_to_dir"] = workloads.texel_to_dir((inp["env_rows"], inp["env_cols"]), (2, 8))
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=vis_mode)
+    av, img = run_gpu(inp, vis_mode=vis_mode)
+    print(compare_all(inp, av, img, orc_av, o, vis_mode))
+    av.close()
+
+
+def test_rotation_and_scale_as_vertex_attributes():
+    # the paper's own layout: r and s are vertex attributes interpolated to the Gaussians by Eq.1 (reading
+    # A2: neighbour quaternions take the sign of the nearest neighbour's first).  No per-Gaussian rotation / scale is passed;
+    # covariances, tile rects, sorted lists must equal the oracle's bit for bit.  gaussians_update re-interpolates them too.
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import compare_all, run_gpu
+    inp = workloads.make(1, n_gauss=20_000)
+    rs = np.random.default_rng(3)
+    nv = len(inp["vert_pos"])
+    q = rs.normal(size=(nv, 4)); q /= np.linalg.norm(q, axis=1, keepdims=True)
+    inp["vert_quat"] = (q * rs.choice([-1.0, 1.0], size=(nv, 1))).astype(np.float32)      # random signs: the alignment matters
+    inp["vert_scale"] = np.exp(rs.uniform(np.log(2e-3), np.log(1e-2), (nv, 3))).astype(np.float32)
+    inp["gauss_quat"] = None; inp["gauss_scale"] = None
+    orc_av = orc.avatar_load(inp)
+    assert "quat_g" in orc_av and "scale_g" in orc_av
+    o = orc.render_frame(orc_av, inp, vis_mode=0)
+    av, img = run_gpu(inp, vis_mode=0)
+    print(compare_all(inp, av, img, orc_av, o, 0))
+    # moved Gaussians: rotation and scale follow the new neighbour sets
+    inp2 = dict(inp)
+    inp2["gauss_pos"] = (inp["gauss_pos"] + rs.normal(0.0, 0.01, inp["gauss_pos"].shape)).astype(np.float32)
+    rga.gaussians_update(av.h, torch.as_tensor(inp2["gauss_pos"]).cuda())
+    orc_av2 = orc.avatar_load(inp2)
+    o2 = orc.render_frame(orc_av2, inp2, vis_mode=0, stop_after="skin")
+    rga.pose_skin(av.h, torch.as_tensor(inp["bone_mats"][0]).cuda())
+    assert np.array_equal(av.read("GAUSS_COV").reshape(-1, 6), o2["cov6"])
+    av.close()
+
+
+def test_displacement_mlp_then_gaussians_update_then_static():
+    # gaussians_update after displacement_mlp must keep the network's displacement (re-interpolated over the NEW
+    # neighbour sets), and displacement_static must restore the load-time table -- each state equals a fresh oracle load
+    # with that displacement as the vertex attribute, bit for bit on the posed Gaussians.
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    inp = workloads.make(1, n_gauss=8_000)
+    rs = np.random.default_rng(8)
+    inp["vert_disp"] = (0.01 * rs.standard_normal(inp["vert_pos"].shape)).astype(np.float32)       # a non-zero static table
+    cam = inp["camera"]
+    av = rga.Avatar(inp, max_width=cam["width"], max_height=cam["height"], max_vis_dirs=16, max_vis_res=32, max_env_texels=512)
+    m = workloads.make_disp_mlp(seed=3)
+    md = {k: (torch.as_tensor(v).cuda() if isinstance(v, np.ndarray) else v) for k, v in m.items()}
+    bones = torch.as_tensor(inp["bone_mats"][0]).cuda()
+    rga.displacement_mlp(av.h, md, md["theta"])
+    dx = np.ascontiguousarray(av.read("VERT_DISP").reshape(-1, 4)[:, :3], np.float32)
+    moved = (inp["gauss_pos"] + rs.normal(0.0, 0.01, inp["gauss_pos"].shape)).astype(np.float32)
+    rga.gaussians_update(av.h, torch.as_tensor(moved).cuda())
+    rga.pose_skin(av.h, bones)
+    inp_mlp = dict(inp, vert_disp=dx, gauss_pos=moved)
+    o = orc.render_frame(orc.avatar_load(inp_mlp), inp_mlp, stop_after="skin")
+    assert np.array_equal(av.read("GAUSS_POSED").reshape(-1, 4)[:, :3], o["gauss_posed"])           # the MLP's dx over the NEW S_g
+    assert np.array_equal(av.read("VERT_POSED").reshape(-1, 4)[:, :3], o["vert_posed"])
+    rga.displacement_static(av.h)
+    rga.pose_skin(av.h, bones)
+    inp_st = dict(inp, gauss_pos=moved)
+    o = orc.render_frame(orc.avatar_load(inp_st), inp_st, stop_after="skin")
+    assert np.array_equal(av.read("GAUSS_POSED").reshape(-1, 4)[:, :3], o["gauss_posed"])           # back to the static table
+    assert np.array_equal(av.read("VERT_POSED").reshape(-1, 4)[:, :3], o["vert_posed"])
+    av.close()

@@ -31,6 +31,29 @@ def test_vis_gauss_hand_example():
     np.testing.assert_allclose(vg, [[9.75 / 19, 7.25 / 19], [4.375 / 19, 9.0 / 19]], rtol=1e-14)
 
 
+def test_interp_quat_sign_alignment_hand_example():
+    # reading A2 (the rotation r is a vertex attribute interpolated by Eq.1): q and -q are the same
+    # rotation.  Three neighbours q, -q, q with weights 1/2, 1/4, 1/4 must give q back (a plain average gives q/2, and
+    # aligning to the wrong reference or dropping the sign gives something else); the result is not normalised here.
+    q = np.array([0.5, -0.5, 0.5, 0.5], np.float32)                    # a unit quaternion
+    r = np.array([np.sqrt(0.5), 0, np.sqrt(0.5), 0], np.float32)       # another one, 60 degrees from q (dot = 0.7071 > 0)
+    vq = np.stack([q, -q, q, r, -r]).astype(np.float32)
+    idx = np.array([[0, 1, 2], [1, 0, 3], [3, 4, 1]], np.int32)
+    ub = np.array([[0.5, 0.25, 0.25], [0.5, 0.25, 0.25], [0.5, 0.25, 0.25]], np.float32)
+    out = orc.interp_quat(idx, ub, vq)
+    np.testing.assert_allclose(out[0], q, rtol=1e-7)                   # q/2 + q/4 + q/4
+    # reference = neighbour 0 = -q: 0.5(-q) + 0.25(-q) [q flipped] + 0.25(-r) [r.(-q) < 0: flipped]
+    np.testing.assert_allclose(out[1], -0.75 * q - 0.25 * r, rtol=1e-6, atol=1e-7)
+    # reference r: -r flipped to r; -q has dot(-q, r) < 0: flipped to q
+    np.testing.assert_allclose(out[2], 0.75 * r + 0.25 * q, rtol=1e-6, atol=1e-7)
+    # used through the pipeline: per-vertex quats that are all the same rotation (random signs) give that rotation's covariance
+    M = np.eye(3, 4, dtype=np.float32).reshape(1, 12)
+    sgn = np.array([1, -1, 1], np.float32)[:, None]
+    out = orc.interp_quat(np.array([[0, 1, 2]], np.int32), np.array([[0.2, 0.3, 0.5]], np.float32), (sgn * q[None]).astype(np.float32))
+    c_ref = orc.gauss_cov(M, q[None], np.array([[1.0, 2.0, 3.0]], np.float32))
+    np.testing.assert_allclose(orc.gauss_cov(M, out, np.array([[1.0, 2.0, 3.0]], np.float32)), c_ref, rtol=1e-5, atol=1e-6)
+
+
 # ------------------------------------------------------------------ Eq.2 with v_g and the texel -> direction map
 def _one_texel_setup():
     R_, C_ = 8, 16
