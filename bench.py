@@ -22,7 +22,6 @@ Prints ONE JSON line (rank 0):
 N > 1: replicas only: every rank renders its own frames, no data-path collective.
 """
 import argparse
-import hashlib
 import json
 import os
 import subprocess
@@ -115,12 +114,8 @@ def peaks():
 
 
 def csrc_hash():
-    """Hash of the kernel sources: the ncu counters under profiles/ are only quoted for the build they were captured on."""
-    h = hashlib.sha256()
-    d = os.path.join(ROOT, "paper_2407_10707_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        h.update(open(os.path.join(d, f), "rb").read())
-    return h.hexdigest()[:16]
+    from paper_2407_10707_b200 import build
+    return build.csrc_hash()
 
 
 def ncu_counters():
@@ -261,6 +256,9 @@ class Bench:
             # inside rga_render_frame the mode-0 depth test runs for the camera-facing Gaussians only
             "vis_depth_test": {"units": front * self.K},
             "shade": {"units": front * ne * 0.5},
+            # fused kernel: the depth tests Eq.2 can read (camera-facing Gaussian, direction in its upper hemisphere: 40 flop-eq
+            # each) + the BRDF terms (camera-facing Gaussian, upper-hemisphere texel: 70 flop each)
+            "vis_shade": {"units": front * self.K * 0.5 + front * ne * 0.5, "flop_eq": front * self.K * 0.5 * 40.0 + front * ne * 0.5 * 70.0},
             "project": {"units": ng},
             "tile_scatter": {"units": D},
             "composite_T": {"units": float(nc.sum())},
@@ -294,9 +292,11 @@ def roofline_list(kern_ms, units, fma_meas, hbm_gbs, hbm_src):
             o.update(units_per_launch=u["units"], unit_of_work=unit_name, bytes_per_launch=byts, achieved=byts / (ms * 1e-3) / 1e9,
                      peak=hbm_gbs, peak_source=hbm_src, unit="GB/s")
             o["frac"] = o["achieved"] / o["peak"]
-        elif u is not None and work and bound == "alu":
-            ach = u["units"] * work / (ms * 1e-3) / 1e12
-            o.update(units_per_launch=u["units"], unit_of_work=unit_name, flop_eq_per_unit=work, achieved=ach, peak=fma_meas,
+        elif u is not None and (work or "flop_eq" in u) and bound == "alu":
+            flop_eq = u.get("flop_eq", u["units"] * (work or 0.0))
+            ach = flop_eq / (ms * 1e-3) / 1e12
+            o.update(units_per_launch=u["units"], unit_of_work=unit_name, flop_eq_per_unit=flop_eq / u["units"], flop_eq_per_launch=flop_eq,
+                     achieved=ach, peak=fma_meas,
                      peak_source="register-resident FFMA chains measured in this run (rga_measure_fp32_peak)",
                      peak_derived=FP32_PEAK_DERIVED, unit="TFLOP/s", frac=ach / fma_meas if fma_meas > 0 else None)
         else:

@@ -17,6 +17,15 @@ EXACT = ["load_kernels.cu", "skin_kernels.cu", "vis_kernels.cu", "project_kernel
 FAST = ["vis_shade_kernels.cu", "order_kernels.cu", "shade_kernels.cu", "composite_kernels.cu", "sort_kernels.cu", "api.cu", "peak_kernels.cu", "mlp_kernels.cu", "backward_kernels.cu", "shade_backward_kernels.cu", "loss_kernels.cu", "pose_backward_kernels.cu"]
 
 
+def csrc_hash():
+    """Hash of the kernel sources: ncu counters under profiles/ are only quoted by bench.py for the build they were taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(CSRC)):
+        h.update(open(os.path.join(CSRC, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def _stale():
     if not os.path.exists(LIB):
         return True

@@ -3,6 +3,7 @@
 // (mode 0; BASELINE.json north_star (b)) or the paper's triangle-ID visibility with the
 // median/median/mean vertex filters (mode 1; Eq.3-4).
 // EXACT file: -fmad=false; + - * / sqrt and integer arithmetic only.
+#include <cstdlib>
 #include "rga_internal.h"
 
 // DESIGN.md A13: w = direction toward the light; u = normalize(e x w), e = z unless |w_z| > 0.999 then x; v = w x u.
@@ -292,7 +293,7 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
   return q2n;
 }
 
-template <bool WITH_ID, bool BINNED>
+template <bool WITH_ID, bool BINNED, bool GTAB>
 __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
     int tail_first, int split,
     const float4* __restrict__ v_posed, const unsigned long long* __restrict__ faces_packed, const float* __restrict__ dirs,
@@ -312,8 +313,9 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
   unsigned long long* sz64 = reinterpret_cast<unsigned long long*>(mp);
   const size_t map_bytes = (((size_t)band_rows * R * (WITH_ID ? 8 : 4)) + 15) & ~(size_t)15;
   // snapped vertex coordinates: shared memory, or (large meshes) this CTA's slice of an L2-resident scratch buffer
-  unsigned* sXY = sxy_scratch ? sxy_scratch + (size_t)blockIdx.x * nv : reinterpret_cast<unsigned*>(mp + map_bytes);
-  unsigned* svert = reinterpret_cast<unsigned*>(mp + map_bytes) + (sxy_scratch ? 0 : nv);
+  // (a compile-time choice: with a run-time one every gather of the common shared-memory case becomes a generic load)
+  unsigned* sXY = GTAB ? sxy_scratch + (size_t)blockIdx.x * nv : reinterpret_cast<unsigned*>(mp + map_bytes);
+  unsigned* svert = reinterpret_cast<unsigned*>(mp + map_bytes) + (GTAB ? 0 : nv);
   const int nv_words = (nv + 31) >> 5;
 
   // Work slots: units [0, tail_first) one CTA each; the units of the last, partial round of the persistent grid are cut
@@ -528,11 +530,18 @@ static size_t raster_plan(int res, int with_id, int n_verts, bool table_in_smem,
 }
 
 size_t rga_vis_raster_plan(int res, int with_id, int n_verts, int* band_rows, int* threads, int* sxy_global) {
-  *sxy_global = 0;
-  size_t b = raster_plan(res, with_id, n_verts, true, band_rows, threads);
-  if (b != 0 && (res + *band_rows - 1) / *band_rows <= 16) return b;
-  *sxy_global = 1;
-  return raster_plan(res, with_id, n_verts, false, band_rows, threads);
+  // Two places for the table of snapped vertex coordinates: shared memory (fast gathers, but it competes with the map and the
+  // warps' working sets) or an L2-resident scratch slice per CTA.  More warps win: at config 2 (27.5k vertices, 110 KB table)
+  // the shared-memory plan leaves room for 16 warps only and the rasteriser idles on latency -- 860 us; with the table in L2
+  // and 32 warps 615 us (profiles/r02_raster.md).  Equal warps: shared memory.
+  int rows_s = 0, th_s = 0, rows_g = 0, th_g = 0;
+  const size_t b_s = raster_plan(res, with_id, n_verts, true, &rows_s, &th_s);
+  const size_t b_g = raster_plan(res, with_id, n_verts, false, &rows_g, &th_g);
+  const int bands_s = rows_s > 0 ? (res + rows_s - 1) / rows_s : 1 << 30;
+  const bool use_global = b_s == 0 || bands_s > 16 || th_g > th_s;
+  *sxy_global = use_global ? 1 : 0;
+  *band_rows = use_global ? rows_g : rows_s; *threads = use_global ? th_g : th_s;
+  return use_global ? b_g : b_s;
 }
 
 size_t rga_vis_raster_smem(int res, int with_id, int n_verts, int* band_rows, int* threads) {
@@ -557,19 +566,26 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
   // last, partial round of the persistent grid: cut its units into triangle ranges (depth-only maps merge with atomicMin)
   int tail_first = n_units, split = 1;
   const int rem = n_units > grid ? n_units % grid : 0;
-  if (rem > 0 && !with_id && !binned && grid / rem >= 2) {
+  if (rem > 0 && !with_id && grid / rem >= 2) {
     split = grid / rem > 4 ? 4 : grid / rem;
     tail_first = n_units - rem;
     const size_t unit_px = (size_t)band_rows * p->res;       // bands are even; the last may be shorter (covered anyway)
-    const size_t first_px = (size_t)(tail_first / n_bands) * p->res * p->res + (size_t)(tail_first % n_bands) * unit_px;
+    const size_t first_px = binned ? (size_t)tail_first * p->res * p->res      // a binned unit is a whole direction
+                                   : (size_t)(tail_first / n_bands) * p->res * p->res + (size_t)(tail_first % n_bands) * unit_px;
     cudaMemsetAsync(av->zmap + first_px, 0xff, ((size_t)p->n_dirs * p->res * p->res - first_px) * 4, s);
   }
   const int band_magic = (65536 + band_rows - 1) / band_rows;   // (row * magic) >> 16 == row / band_rows for row < 256
 #define RAST_ARGS av->n_faces, av->n_verts, p->res, band_rows, n_bands, n_units, tail_first, split, av->v_posed, av->faces_packed, p->dirs, av->window, \
     av->zmap, av->idmap, raw, words, p->cull_backfaces != 0, reinterpret_cast<float4*>(av->frames), p->depth_bias_texels, p->depth_bias_world, \
     p->slope_max, binned ? av->rast_bins : nullptr, band_magic, sxy_global ? av->rast_sxy : nullptr
-  if (with_id) { if (binned) vis_raster_kernel<true, true><<<grid, threads, smem, s>>>(RAST_ARGS); else vis_raster_kernel<true, false><<<grid, threads, smem, s>>>(RAST_ARGS); }
-  else { if (binned) vis_raster_kernel<false, true><<<grid, threads, smem, s>>>(RAST_ARGS); else vis_raster_kernel<false, false><<<grid, threads, smem, s>>>(RAST_ARGS); }
+#define RAST_LAUNCH(ID, BIN, GT) vis_raster_kernel<ID, BIN, GT><<<grid, threads, smem, s>>>(RAST_ARGS)
+  if (sxy_global) {
+    if (with_id) { if (binned) RAST_LAUNCH(true, true, true); else RAST_LAUNCH(true, false, true); }
+    else { if (binned) RAST_LAUNCH(false, true, true); else RAST_LAUNCH(false, false, true); }
+  } else {
+    if (with_id) { if (binned) RAST_LAUNCH(true, true, false); else RAST_LAUNCH(true, false, false); }
+    else { if (binned) RAST_LAUNCH(false, true, false); else RAST_LAUNCH(false, false, false); }
+  }
   av->launches += 1;
   rga_prof_mark(av, "vis_raster", s);
   return cudaGetLastError();
@@ -841,10 +857,10 @@ cudaError_t rga_launch_vis_paper(rga_avatar* av, const rga_vis_params* p, cudaSt
 
 int rga_vis_init_attributes() {
   const int mx = 227 * 1024 - 512;            // the static counters count against the 227 KB block limit
-  cudaError_t e = cudaFuncSetAttribute(vis_raster_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  cudaError_t e = cudaSuccess;
+#define RAST_ATTR(ID, BIN, GT) if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_raster_kernel<ID, BIN, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx)
+  RAST_ATTR(true, false, false); RAST_ATTR(false, false, false); RAST_ATTR(true, true, false); RAST_ATTR(false, true, false);
+  RAST_ATTR(true, false, true); RAST_ATTR(false, false, true); RAST_ATTR(true, true, true); RAST_ATTR(false, true, true);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_depth_test_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
   return (int)e;
 }
