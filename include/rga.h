@@ -343,7 +343,9 @@ RGA_API int64_t rga_launch_count(const rga_avatar* av);
 
 /* Optional per-kernel timing.  While enabled, the library records a CUDA event on `stream` after each of its kernels.
  * rga_profile_read synchronises `stream`, writes up to `capacity` entries (names: capacity x 32 chars, ms: elapsed
- * milliseconds of each kernel since the previous event) and clears the log.  Not graph-capturable while enabled. */
+ * milliseconds of each kernel since the previous event) and clears the log.  Not graph-capturable while enabled.
+ * on == 2 (timeline): rga_render_frame keeps its second stream and every entry is the completion time of that kernel since
+ * the call began -- how the two streams actually interleave. */
 RGA_API rga_status rga_profile_enable(rga_avatar* av, int on);
 RGA_API rga_status rga_profile_read(rga_avatar* av, void* stream, char* names, float* ms, int capacity, int* count);
 

@@ -41,10 +41,12 @@ extern "C" rga_status rga_profile_read(rga_avatar* av, void* stream, char* names
   if (!av || !names || !ms || !count) return fail(RGA_ERR_INVALID_ARG, "rga_profile_read: null argument");
   CU(cudaStreamSynchronize((cudaStream_t)stream));
   int n = 0;
+  if (av->prof_on == 2) CU(cudaStreamSynchronize(av->side));
   for (int i = 1; i < av->prof_n && n < capacity; ++i) {
     if (av->prof_name[i][0] == '-') continue;                      // API-entry boundary marks carry no kernel
     float t = 0.f;
-    CU(cudaEventElapsedTime(&t, av->prof_ev[i - 1], av->prof_ev[i]));
+    // mode 2 (timeline): both streams stay in use and every mark reports its completion time since the call's entry mark
+    CU(cudaEventElapsedTime(&t, av->prof_ev[av->prof_on == 2 ? 0 : i - 1], av->prof_ev[i]));
     snprintf(names + 32 * n, 32, "%s", av->prof_name[i]);
     ms[n++] = t;
   }
@@ -142,7 +144,13 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->stop_seg, npix)); A(dalloc(&av->item_flag, (size_t)av->items_cap));
   A(cudaMemsetAsync(av->item_flag, 0, (size_t)av->items_cap, s));
   A(dalloc(&av->t_final, npix)); A(dalloc(&av->n_contrib, npix)); A(dalloc(&av->status, 1));
-  A(cudaStreamCreateWithFlags(&av->side, cudaStreamNonBlocking));
+  {
+    // the second stream of rga_render_frame carries small, latency-bound kernels: highest priority, so that its CTAs are
+    // placed as soon as a CTA of the big kernels on the caller's stream retires
+    int prio_lo = 0, prio_hi = 0;
+    A(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    A(cudaStreamCreateWithPriority(&av->side, cudaStreamNonBlocking, prio_hi));
+  }
   A(cudaEventCreateWithFlags(&av->ev_fork, cudaEventDisableTiming)); A(cudaEventCreateWithFlags(&av->ev_env, cudaEventDisableTiming));
   A(cudaEventCreateWithFlags(&av->ev_gskin, cudaEventDisableTiming));
   A(cudaEventCreateWithFlags(&av->ev_join, cudaEventDisableTiming));
@@ -438,7 +446,7 @@ extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, c
   if (cam->width < 1 || cam->height < 1 || cam->width > av->max_w || cam->height > av->max_h)
     return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: camera larger than max_width/max_height");
   cudaStream_t s = (cudaStream_t)stream;
-  const bool overlap = !av->prof_on;                       // per-kernel events need one stream
+  const bool overlap = av->prof_on != 1;                   // per-kernel events need one stream (mode 2 = timeline keeps both)
   cudaStream_t s2 = overlap ? av->side : s;
   // a failure after the fork must not leave the second stream un-joined (inside a CUDA-graph capture that would invalidate
   // the capture): join it, forget the half-built pose state, then report
