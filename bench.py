@@ -280,8 +280,8 @@ def stage_ms(kern_ms):
     return st
 
 
-def roofline_list(kern_ms, units, fma_meas, hbm_gbs, hbm_src):
-    ncu, ncu_src, ncu_ok = ncu_counters()
+def roofline_list(kern_ms, units, fma_meas, hbm_gbs, hbm_src, with_ncu=True):
+    ncu, ncu_src, ncu_ok = ncu_counters() if with_ncu else ({}, None, False)
     out = []
     for k, ms in sorted(kern_ms.items(), key=lambda kv: -kv[1]):
         stage, bound, unit_name, work = KERNELS.get(k, ("other", "alu", "", None))
@@ -315,7 +315,7 @@ def roofline_list(kern_ms, units, fma_meas, hbm_gbs, hbm_src):
     return out
 
 
-def bench_config(cfg, vis_mode, dev, steps, warmup, flush):
+def bench_config(cfg, vis_mode, dev, steps, warmup, flush, fma_meas):
     """One entry of `configs`: ms per frame (L2 flushed), per-kernel / per-stage ms; configs[3]: the 64-pose graph replay."""
     import torch
     b = Bench(cfg, vis_mode, dev, morton=False, flush=flush)
@@ -348,6 +348,10 @@ def bench_config(cfg, vis_mode, dev, steps, warmup, flush):
         out.update(protocol="rga_render_frame per step, L2 flushed between steps", ms_per_frame=ms, fps=1e3 / ms)
     km = b.kernel_times(max(3, min(steps, 10)))
     u = b.units()
+    pk, pk_src = peaks()
+    rl = roofline_list(km, u, fma_meas, pk["hbm_gbs"], pk_src, with_ncu=False)
+    out["roofline"] = [{k: r.get(k) for k in ("kernel", "bound", "kernel_ms", "units_per_launch", "flop_eq_per_unit", "bytes_per_launch", "achieved",
+                                            "peak", "unit", "frac")} for r in rl if r.get("frac") is not None]
     out.update(kernel_ms=km, stage_ms=stage_ms(km), duplicates=u["_D"], camera_facing_gaussians=u["_front"], active_tiles=u["_active_tiles"],
                longest_tile_list=u["_list_max"], blend_pairs_until_stop=u["_pairs_until_stop"], blend_pairs_all=u["_pairs_all"])
     rga.rga_check(b.av.h)
@@ -604,7 +608,7 @@ def main():
         flush = b.flush
         out["configs"] = {}
         for c in range(5):
-            out["configs"][str(c)] = bench_config(c, args.vis_mode, dev, max(5, min(args.steps, 20 if c in (2, 4) else 50)), 3, flush)
+            out["configs"][str(c)] = bench_config(c, args.vis_mode, dev, max(5, min(args.steps, 20 if c in (2, 4) else 50)), 3, flush, fma_meas)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = oracle_times(inp, args.vis_mode)     # the oracle is imported only here, after every timed region
     if rank == 0:

@@ -74,6 +74,22 @@ def main():
         print("|---|" + "---|" * len(d["configs"]))
         for k in names:
             print("| %s | %s |" % (k, " | ".join("%.1f" % (v["kernel_ms"].get(k, 0.0) * 1e3) for v in d["configs"].values())))
+        print()
+        print("Per-kernel roofline fraction per config (achieved / measured peak; work per unit as in the headline table):")
+        print()
+        kn = []
+        for v in d["configs"].values():
+            for r in v.get("roofline", []):
+                if r["kernel"] not in kn:
+                    kn.append(r["kernel"])
+        print("| kernel | " + " | ".join("cfg%s" % c for c in d["configs"]) + " |")
+        print("|---|" + "---|" * len(d["configs"]))
+        for k in kn:
+            cells = []
+            for v in d["configs"].values():
+                r = next((r for r in v.get("roofline", []) if r["kernel"] == k), None)
+                cells.append("-" if r is None else "%.3f (%.1f %s)" % (r["frac"], r["achieved"], r["unit"]))
+            print("| %s | %s |" % (k, " | ".join(cells)))
     nx = [k for k in ("amortised", "disp_mlp", "gaussians_update_ms", "densify_density", "image_loss", "splat_backward", "shade_backward",
                       "regularisers", "train_backward") if k in d]
     if nx:
