@@ -68,6 +68,14 @@ def normalize_rows3(v):
     return v
 
 
+def vertex_normals(x, faces):
+    """Area-weighted vertex normals of the canonical mesh (reading A40): what `vert_normal = None` means."""
+    x = _f32(x); faces = np.ascontiguousarray(faces, np.int32)
+    out = np.empty_like(x)
+    lib().orc_vertex_normals(_p(x), _p(faces), C.c_int(len(x)), C.c_int(len(faces)), _p(out))
+    return out
+
+
 def skin(x, dx, n, w, G):
     x, n, w, G = _f32(x), _f32(n), _f32(w), _f32(G)
     dx = None if dx is None else _f32(dx)
@@ -281,7 +289,8 @@ def avatar_load(inp):
     kv = min(K_V, len(inp["vert_pos"]))
     av["knn_v"], _ = knn(inp["vert_pos"], inp["vert_pos"], kv)
     i, u = av["knn_g"], av["ubar_g"]
-    av["normal_g"] = normalize_rows3(interp_attr(i, u, inp["vert_normal"]))
+    av["vert_normal"] = _f32(inp["vert_normal"]) if inp.get("vert_normal") is not None else vertex_normals(inp["vert_pos"], inp["faces"])
+    av["normal_g"] = normalize_rows3(interp_attr(i, u, av["vert_normal"]))
     av["albedo_g"] = interp_attr(i, u, inp["vert_albedo"])
     av["rough_g"] = interp_attr(i, u, inp["vert_rough"])
     av["spec_g"] = interp_attr(i, u, inp["vert_spec"])
@@ -312,7 +321,7 @@ def render_frame(av, inp, frame=0, vis_mode=0, camera=None, stop_after=None, gau
             t_prev[0] = now
     o = {}
     G = inp["bone_mats"][frame]
-    o["vert_posed"], o["vert_normal_posed"], _ = skin(inp["vert_pos"], inp["vert_disp"], inp["vert_normal"],
+    o["vert_posed"], o["vert_normal_posed"], _ = skin(inp["vert_pos"], inp["vert_disp"], av["vert_normal"],
                                                       inp["vert_skin_w"], G)
     o["gauss_posed"], o["gauss_normal_posed"], M = skin(inp["gauss_pos"], av["disp_g"], av["normal_g"], av["skin_w_g"], G)
     o["cov6"] = gauss_cov(M, av["quat_g"] if "quat_g" in av else inp["gauss_quat"], av["scale_g"] if "scale_g" in av else inp["gauss_scale"])

@@ -97,6 +97,26 @@ ORC void orc_normalize_rows3(float* v, int n) {
   }
 }
 
+// L0, vertex normals when the caller stores nothing but geometry (PAPER.md:86 lists n among the vertex attributes and does
+// not say where it comes from; NULL = area-weighted normals of the canonical mesh; reading A40).
+// n_v = normalize( sum over the faces f = 0..nf-1 in ascending order, corners k = 0..2, that touch v, of
+// (x_b - x_a) x (x_c - x_a) ): the cross product's length is twice the face area, so the sum is area-weighted.  fp32, one
+// rounding per operation, in this order (the normal decides visibility bits downstream); a vertex without a face keeps 0.
+ORC void orc_vertex_normals(const float* x, const int* faces, int nv, int nf, float* out) {
+  for (size_t i = 0; i < 3 * (size_t)nv; ++i) out[i] = 0.0f;
+  for (int f = 0; f < nf; ++f) {
+    const int* t = faces + 3 * (size_t)f;
+    const float *a = x + 3 * (size_t)t[0], *b = x + 3 * (size_t)t[1], *c = x + 3 * (size_t)t[2];
+    float e1[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]}, e2[3] = {c[0] - a[0], c[1] - a[1], c[2] - a[2]};
+    float cr[3] = {e1[1] * e2[2] - e1[2] * e2[1], e1[2] * e2[0] - e1[0] * e2[2], e1[0] * e2[1] - e1[1] * e2[0]};
+    for (int k = 0; k < 3; ++k) {
+      float* o = out + 3 * (size_t)t[k];
+      o[0] = o[0] + cr[0]; o[1] = o[1] + cr[1]; o[2] = o[2] + cr[2];
+    }
+  }
+  orc_normalize_rows3(out, nv);
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // H1/H2 forward LBS (reading A3).  M = sum_b w_b G_b accumulated b = 0..B-1 from +0;
 // x' = M [x + dx; 1];  n' = normalize(M3x3 n).  Also returns M (12 floats per point) for the covariance step.

@@ -322,3 +322,47 @@ def test_a37_fused_vs_plain_projection_counts():
     assert r["max_abs_depth_diff"] < 2e-7                                  # one or two fp32 ulps of a depth in [0,1]
     g1 = [x for x in rows if x[0] == "1"][0]
     assert int(g1[3]) == 0 and int(g1[8]) <= 1e-6 * int(g1[7])            # config 1: same coverage, < 1e-6 of the bits move
+
+
+# ------------------------------------------------------------------ reading A40: vertex normals from the geometry
+def test_vertex_normals_closed_forms_and_hand_example():
+    # (1) regular octahedron, faces counter-clockwise seen from outside: by symmetry the area-weighted sum at +e_i is
+    # (s, 0, 0) with the other components cancelling EXACTLY, so the normal is the vertex position itself
+    v = np.array([[1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1]], np.float32)
+    f = np.array([[0, 2, 4], [2, 1, 4], [1, 3, 4], [3, 0, 4], [2, 0, 5], [1, 2, 5], [3, 1, 5], [0, 3, 5]], np.int32)
+    assert np.array_equal(orc.vertex_normals(v, f), v)
+    # (2) winding decides the sign
+    assert np.array_equal(orc.vertex_normals(v, f[:, [0, 2, 1]]), -v)
+    # (3) area weighting, by hand.  O=(0,0,0) A=(2,0,0) B=(0,2,0) C=(0,0,1) and an isolated vertex D.
+    #   face (O,A,B): (A-O) x (B-O) = (2,0,0) x (0,2,0) = (0,0,4)      (area 2)
+    #   face (O,C,A): (C-O) x (A-O) = (0,0,1) x (2,0,0) = (0,2,0)      (area 1)
+    #   O and A touch both: (0,2,4)/sqrt(20);  B only the first: (0,0,1);  C only the second: (0,1,0);  D: no face, stays 0.
+    #   An unweighted mean of the two face normals would give (0,1,1)/sqrt(2) at O instead.
+    v = np.array([[0, 0, 0], [2, 0, 0], [0, 2, 0], [0, 0, 1], [5, 5, 5]], np.float32)
+    f = np.array([[0, 1, 2], [0, 3, 1]], np.int32)
+    n = orc.vertex_normals(v, f).astype(np.float64)
+    s5 = np.sqrt(5.0)
+    exp = np.array([[0, 1 / s5, 2 / s5], [0, 1 / s5, 2 / s5], [0, 0, 1], [0, 1, 0], [0, 0, 0]])
+    np.testing.assert_allclose(n, exp, atol=1e-7)
+    # (4) a flat grid in the plane z = 3 x (not axis-aligned): every vertex normal is (-3,0,1)/sqrt(10)
+    gx, gy = np.meshgrid(np.arange(5, dtype=np.float64), np.arange(4, dtype=np.float64))
+    v = np.stack([gx.ravel(), gy.ravel(), 3.0 * gx.ravel()], 1).astype(np.float32)
+    idx = lambda i, j: j * 5 + i
+    f = np.array([t for j in range(3) for i in range(4) for t in ([idx(i, j), idx(i + 1, j), idx(i + 1, j + 1)],
+                                                                 [idx(i, j), idx(i + 1, j + 1), idx(i, j + 1)])], np.int32)
+    np.testing.assert_allclose(orc.vertex_normals(v, f), np.tile(np.array([-3.0, 0.0, 1.0]) / np.sqrt(10.0), (20, 1)), atol=2e-7)
+
+
+def test_vertex_normals_against_fp64_on_the_body_mesh():
+    # the synthetic body: the fp32 fixed-order sum agrees with an fp64 accumulation (numpy, written independently in the input
+    # generator) to fp32 rounding, and a frame rendered with vert_normal = None equals one rendered with these normals passed in
+    inp = workloads.make(0)
+    n32 = orc.vertex_normals(inp["vert_pos"], inp["faces"])
+    n64 = smesh.vertex_normals(inp["vert_pos"].astype(np.float64), inp["faces"])
+    assert np.abs(n32 - n64).max() < 2e-6
+    np.testing.assert_allclose(np.linalg.norm(n32.astype(np.float64), axis=1), 1.0, atol=2e-7)
+    a = dict(inp); a["vert_normal"] = None
+    b = dict(inp); b["vert_normal"] = n32
+    oa = orc.render_frame(orc.avatar_load(a), a, stop_after="skin")
+    ob = orc.render_frame(orc.avatar_load(b), b, stop_after="skin")
+    assert np.array_equal(oa["gauss_normal_posed"], ob["gauss_normal_posed"]) and np.array_equal(oa["vert_normal_posed"], ob["vert_normal_posed"])
