@@ -72,7 +72,10 @@ typedef struct {
   int32_t k_v;                 /* neighbours per vertex, odd, 1..31 (paper: 19); clamped to n_verts */
   const float*   vert_pos;     /* dev [n_verts][3]  canonical x                                      */
   const int32_t* faces;        /* dev [n_faces][3]                                                   */
-  const float*   vert_normal;  /* dev [n_verts][3]  unit normals n                                   */
+  const float*   vert_normal;  /* dev [n_verts][3]  unit normals n, or NULL = area-weighted normals of the canonical mesh,
+                                  computed once here (sum of (x_b-x_a) x (x_c-x_a) over a vertex's faces in ascending face
+                                  order, normalised; a vertex without a face gets 0; readable as RGA_BUF_VERT_NORMAL;
+                                  DESIGN.md reading A40)                                              */
   const float*   vert_skin_w;  /* dev [n_verts][n_bones] LBS weights w, rows sum to 1                */
   const float*   vert_disp;    /* dev [n_verts][3]  static average displacement or NULL = 0 */
   const float*   vert_albedo;  /* dev [n_verts][3]  a                                                */
@@ -315,7 +318,8 @@ typedef enum {
   RGA_BUF_DENS_HDR = 33,      /* u64 [2]        sum of the fixed-point P, N'                            */
   RGA_BUF_SPLAT_GRAD = 34,    /* f32 [n_gauss][12] splat_backward: d_colour(3), d_opacity, d_mu2D(2), d_conic(3), pad(3) */
   RGA_BUF_GAUSS_ORDER = 35,   /* i32 [n_gauss] caller index of the i-th Gaussian in the library's internal (spatial) order */
-  RGA_BUF_COUNT_ = 36
+  RGA_BUF_VERT_NORMAL = 36,   /* f32 [n_verts][3] canonical vertex normals as used (the caller's, or the computed ones) */
+  RGA_BUF_COUNT_ = 37
 } rga_buffer_id;
 
 /* Gaussian order.  PAPER.md:88-93 defines no order of the Gaussians and a trained asset's is arbitrary, so avatar_load sorts

@@ -16,12 +16,12 @@ BUF = dict(KNN_G=0, UBAR_G=1, KNN_V=2, GAUSS_STATIC=3, GAUSS_SKIN_W=4, VERT_POSE
            GAUSS_NORMAL_POSED=8, GAUSS_COV=9, WINDOW=10, ZMAP=11, IDMAP=12, VISBITS=13, VCOUNT=14, RADIANCE=15, COLOR=16,
            MU2D=17, DEPTH=18, CONIC_OPACITY=19, RECT=20, TOUCHED=21, NUM_DUPLICATES=22, KEYS_SORTED=23, VALS_SORTED=24,
            TILE_RANGES=25, T_FINAL=26, N_CONTRIB=27, VERT_BITS_RAW=28, VERT_DISP=29,
-           DENS_DV=30, DENS_P=31, DENS_NG=32, DENS_HDR=33, SPLAT_GRAD=34, GAUSS_ORDER=35)
+           DENS_DV=30, DENS_P=31, DENS_NG=32, DENS_HDR=33, SPLAT_GRAD=34, GAUSS_ORDER=35, VERT_NORMAL=36)
 _BUF_DTYPE = {0: np.int32, 1: np.float32, 2: np.int32, 3: np.float32, 4: np.float32, 5: np.float32, 6: np.float32,
               7: np.float32, 8: np.float32, 9: np.float32, 10: np.float32, 11: np.uint32, 12: np.int32, 13: np.uint32,
               14: np.uint8, 15: np.float32, 16: np.float32, 17: np.float32, 18: np.float32, 19: np.float32, 20: np.int32,
               21: np.uint32, 22: np.uint32, 23: np.uint64, 24: np.uint32, 25: np.uint32, 26: np.float32, 27: np.uint32,
-              28: np.uint32, 29: np.float32, 30: np.int32, 31: np.uint32, 32: np.int32, 33: np.uint64, 34: np.float32, 35: np.int32}
+              28: np.uint32, 29: np.float32, 30: np.int32, 31: np.uint32, 32: np.int32, 33: np.uint64, 34: np.float32, 35: np.int32, 36: np.float32}
 
 
 class RgaError(RuntimeError):
@@ -125,7 +125,7 @@ def avatar_load(inp, max_width, max_height, max_vis_dirs, max_vis_res, max_env_t
     if not torch.cuda.is_available():
         raise RgaError(RGA_ERR_CUDA, "no CUDA device (there is no CPU fallback)")
     f32, i32 = torch.float32, torch.int32
-    keep = dict(vert_pos=_dev(inp["vert_pos"], f32), faces=_dev(inp["faces"], i32), vert_normal=_dev(inp["vert_normal"], f32),
+    keep = dict(vert_pos=_dev(inp["vert_pos"], f32), faces=_dev(inp["faces"], i32), vert_normal=_dev(inp.get("vert_normal"), f32),
                 vert_skin_w=_dev(inp["vert_skin_w"], f32), vert_disp=_dev(inp.get("vert_disp"), f32),
                 vert_albedo=_dev(inp["vert_albedo"], f32), vert_rough=_dev(inp["vert_rough"], f32),
                 vert_spec=_dev(inp["vert_spec"], f32), gauss_pos=_dev(inp["gauss_pos"], f32),

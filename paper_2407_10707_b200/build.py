@@ -52,7 +52,7 @@ def build(force=False, verbose=False):
     jobs = [(s, ["-fmad=false"]) for s in EXACT] + [(s, []) for s in FAST]
     with ThreadPoolExecutor(max_workers=8) as ex:
         objs = list(ex.map(lambda j: _compile(j[0], j[1], verbose), jobs))
-    cmd = ["nvcc"] + ARCH + ["-shared", "-o", LIB] + objs + ["-lcudart"]
+    cmd = ["nvcc"] + ARCH + ["-shared", "-o", LIB] + objs + ["-lcudart", "-ldl"]
     subprocess.check_call(cmd)
     return LIB
 

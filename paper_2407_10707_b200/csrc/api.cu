@@ -4,6 +4,14 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <nvtx3/nvToolsExt.h>
+
+// NVTX range per C-ABI call (header-only NVTX 3: a no-op unless a profiler injects itself), so that an Nsight timeline shows
+// the path's stages by name (tracing)
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
 
 #include "rga_internal.h"
 
@@ -77,12 +85,13 @@ extern "C" rga_status avatar_free(rga_avatar* av) {
 }
 
 extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_avatar** out) {
+  NvtxRange nvtx_("rga::avatar_load");
   if (out) *out = nullptr;
   if (!d || !out) return fail(RGA_ERR_INVALID_ARG, "avatar_load: null argument");
   if (d->n_verts < 1 || d->n_faces < 1 || d->n_bones < 1 || d->n_gauss < 1) return fail(RGA_ERR_INVALID_ARG, "avatar_load: empty avatar");
   if (d->k_g < 1 || d->k_g > 3) return fail(RGA_ERR_INVALID_ARG, "avatar_load: k_g must be 1..3");
   if (d->k_v < 1 || d->k_v > 31 || !(d->k_v & 1)) return fail(RGA_ERR_INVALID_ARG, "avatar_load: k_v must be odd, 1..31");
-  if (!d->vert_pos || !d->faces || !d->vert_normal || !d->vert_skin_w || !d->vert_albedo || !d->vert_rough || !d->vert_spec ||
+  if (!d->vert_pos || !d->faces || !d->vert_skin_w || !d->vert_albedo || !d->vert_rough || !d->vert_spec ||
       !d->gauss_pos || (!d->gauss_quat && !d->vert_quat) || (!d->gauss_scale && !d->vert_scale))
     return fail(RGA_ERR_INVALID_ARG, "avatar_load: missing table (rotation and scale are needed per Gaussian or per vertex)");
   if (d->max_width < 1 || d->max_height < 1 || d->max_vis_dirs < 1 || d->max_vis_res < 1 || d->max_vis_res > 256 ||
@@ -165,7 +174,8 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->vt_pos, 3 * nv)); A(dalloc(&av->vt_normal, 3 * nv)); A(dalloc(&av->vt_albedo, 3 * nv));
   A(dalloc(&av->vt_rough, nv)); A(dalloc(&av->vt_spec, nv)); A(dalloc(&av->knn_d2, ng * av->k_g));
   A(cudaMemcpyAsync(av->vt_pos, d->vert_pos, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
-  A(cudaMemcpyAsync(av->vt_normal, d->vert_normal, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  if (d->vert_normal) A(cudaMemcpyAsync(av->vt_normal, d->vert_normal, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  else A(rga_launch_vertex_normals(av->vt_pos, av->faces, av->n_verts, av->n_faces, av->vt_normal, s));   // reading A40
   A(cudaMemcpyAsync(av->vt_albedo, d->vert_albedo, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
   A(cudaMemcpyAsync(av->vt_rough, d->vert_rough, nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
   A(cudaMemcpyAsync(av->vt_spec, d->vert_spec, nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
@@ -176,7 +186,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
     A(cudaMemcpyAsync(av->vt_disp, d->vert_disp, 3 * nv * sizeof(float), cudaMemcpyDeviceToDevice, s));
   }
   A(rga_launch_pack_faces(av, s));
-  A(rga_launch_load_verts(av, d->vert_pos, d->vert_disp, d->vert_normal, s));
+  A(rga_launch_load_verts(av, d->vert_pos, d->vert_disp, av->vt_normal, s));
   // KNN: S_v = K_v nearest vertices of each vertex (self included), S_g = K_g nearest of each Gaussian
   A(dalloc(&d2, nv * av->k_v));
   {
@@ -220,6 +230,7 @@ done:
 }
 
 extern "C" rga_status pose_skin(rga_avatar* av, const float* bone_mats, void* stream) {
+  NvtxRange nvtx_("rga::pose_skin");
   if (!av || !bone_mats) return fail(RGA_ERR_INVALID_ARG, "pose_skin: null argument");
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
   rga_prof_mark(av, "-", (cudaStream_t)stream);
@@ -229,6 +240,7 @@ extern "C" rga_status pose_skin(rga_avatar* av, const float* bone_mats, void* st
 }
 
 extern "C" rga_status visibility_raster(rga_avatar* av, const rga_vis_params* p, void* stream) {
+  NvtxRange nvtx_("rga::visibility_raster");
   if (!av || !p || !p->dirs) return fail(RGA_ERR_INVALID_ARG, "visibility_raster: null argument");
   if (!av->have_skin) return fail(RGA_ERR_STATE, "visibility_raster: call pose_skin first");
   if (p->n_dirs < 1 || p->n_dirs > av->max_dirs || p->res < 1 || p->res > av->max_res || (p->mode != 0 && p->mode != 1))
@@ -247,6 +259,7 @@ extern "C" rga_status visibility_raster(rga_avatar* av, const rga_vis_params* p,
 }
 
 extern "C" rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const float cam_pos[3], void* stream) {
+  NvtxRange nvtx_("rga::shade_gaussians");
   if (!av || !env || !env->radiance || !cam_pos) return fail(RGA_ERR_INVALID_ARG, "shade_gaussians: null argument");
   if (!av->have_skin) return fail(RGA_ERR_STATE, "shade_gaussians: call pose_skin first");
   if (env->use_visibility && !av->have_vis) return fail(RGA_ERR_STATE, "shade_gaussians: call visibility_raster first");
@@ -272,6 +285,7 @@ extern "C" rga_status shade_gaussians(rga_avatar* av, const rga_env* env, const 
 }
 
 extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const float bg[3], float* out_image, void* stream) {
+  NvtxRange nvtx_("rga::splat_render");
   if (!av || !cam || !bg || !out_image) return fail(RGA_ERR_INVALID_ARG, "splat_render: null argument");
   if (!av->have_shade) return fail(RGA_ERR_STATE, "splat_render: call shade_gaussians first");
   if (cam->width < 1 || cam->height < 1 || cam->width > av->max_w || cam->height > av->max_h)
@@ -289,6 +303,7 @@ extern "C" rga_status splat_render(rga_avatar* av, const rga_camera* cam, const 
 }
 
 extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, void* stream) {
+  NvtxRange nvtx_("rga::gaussians_update");
   if (!av || !gauss_pos) return fail(RGA_ERR_INVALID_ARG, "gaussians_update: null argument");
   cudaStream_t s = (cudaStream_t)stream;
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
@@ -306,6 +321,7 @@ extern "C" rga_status gaussians_update(rga_avatar* av, const float* gauss_pos, v
 
 extern "C" rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const float bg[3], const float* image, const float* dL_dimage,
                                      float* out_dcolor, float* out_dopacity, float* out_dmean, float* out_dcov, void* stream) {
+  NvtxRange nvtx_("rga::splat_backward");
   if (!av || !cam || !bg || !image || !dL_dimage) return fail(RGA_ERR_INVALID_ARG, "splat_backward: null argument");
   if (!av->have_splat || av->splat_is_attr) return fail(RGA_ERR_STATE, "splat_backward: call splat_render (or rga_render_frame) first");
   if (cam->width != av->cam_w || cam->height != av->cam_h) return fail(RGA_ERR_INVALID_ARG, "splat_backward: not the camera of the last splat_render");
@@ -317,6 +333,7 @@ extern "C" rga_status splat_backward(rga_avatar* av, const rga_camera* cam, cons
 
 extern "C" rga_status shade_backward(rga_avatar* av, const rga_env* env, const float cam_pos[3], const float* dL_dcolor, float* out_dalbedo,
                                      float* out_drough, float* out_dspec, float* out_dnormal, float* out_dpos, float* out_denv, void* stream) {
+  NvtxRange nvtx_("rga::shade_backward");
   if (!av || !env || !env->radiance || !cam_pos || !dL_dcolor) return fail(RGA_ERR_INVALID_ARG, "shade_backward: null argument");
   if (!av->have_shade) return fail(RGA_ERR_STATE, "shade_backward: call shade_gaussians (or rga_render_frame) first");
   if (env->use_visibility && !av->have_vis) return fail(RGA_ERR_STATE, "shade_backward: no visibility for this pose");
@@ -340,6 +357,7 @@ extern "C" rga_status shade_backward(rga_avatar* av, const rga_env* env, const f
 
 extern "C" rga_status image_loss(rga_avatar* av, const float* image, const float* target, int width, int height, float lambda,
                                  float* out_loss, float* out_dL_dimage, void* stream) {
+  NvtxRange nvtx_("rga::image_loss");
   if (!av || !image || !target) return fail(RGA_ERR_INVALID_ARG, "image_loss: null argument");
   if (width < 1 || height < 1 || width > av->max_w || height > av->max_h) return fail(RGA_ERR_INVALID_ARG, "image_loss: image larger than max_width/max_height");
   if (!(lambda >= 0.f && lambda <= 1.f)) return fail(RGA_ERR_INVALID_ARG, "image_loss: lambda must be in [0, 1]");
@@ -351,6 +369,7 @@ extern "C" rga_status image_loss(rga_avatar* av, const float* image, const float
 
 extern "C" rga_status regularisers(rga_avatar* av, float s0, float* out_losses, float* out_dalbedo, float* out_drough, float* out_dspec,
                                    float* out_dgauss_pos, float* out_ddisp, float* out_dscale, void* stream) {
+  NvtxRange nvtx_("rga::regularisers");
   if (!av) return fail(RGA_ERR_INVALID_ARG, "regularisers: null avatar");
   cudaStream_t s = (cudaStream_t)stream;
   rga_prof_mark(av, "-", s);
@@ -360,6 +379,7 @@ extern "C" rga_status regularisers(rga_avatar* av, float s0, float* out_losses, 
 
 extern "C" rga_status pose_backward(rga_avatar* av, const float* bone_mats, const rga_posed_grads* in, const rga_canonical_grads* out,
                                     void* stream) {
+  NvtxRange nvtx_("rga::pose_backward");
   if (!av || !bone_mats || !in || !out) return fail(RGA_ERR_INVALID_ARG, "pose_backward: null argument");
   if (av->k_g > 8) return fail(RGA_ERR_INVALID_ARG, "pose_backward: k_g > 8 is not supported");
   cudaStream_t s = (cudaStream_t)stream;
@@ -370,6 +390,7 @@ extern "C" rga_status pose_backward(rga_avatar* av, const float* bone_mats, cons
 
 extern "C" rga_status densify_density(rga_avatar* av, float d0, float p0, const uint32_t* rnd, int max_out, float* out_pos,
                                       int32_t* out_tri, int32_t* out_count, void* stream) {
+  NvtxRange nvtx_("rga::densify_density");
   if (!av) return fail(RGA_ERR_INVALID_ARG, "densify_density: null avatar");
   if (!(d0 > 0.0f) || d0 > 32768.0f || !(p0 >= 0.0f)) return fail(RGA_ERR_INVALID_ARG, "densify_density: need 0 < d0 <= 32768 and p0 >= 0");
   if (max_out < 0 || (max_out > 0 && (!rnd || !out_pos))) return fail(RGA_ERR_INVALID_ARG, "densify_density: max_out > 0 needs rnd and out_pos");
@@ -381,6 +402,7 @@ extern "C" rga_status densify_density(rga_avatar* av, float d0, float p0, const 
 }
 
 extern "C" rga_status displacement_mlp(rga_avatar* av, const rga_disp_mlp* mlp, const float* theta, void* stream) {
+  NvtxRange nvtx_("rga::displacement_mlp");
   if (!av || !mlp || !theta || !mlp->rff || !mlp->W1 || !mlp->b1 || !mlp->Wh || !mlp->bh || !mlp->Wo || !mlp->bo)
     return fail(RGA_ERR_INVALID_ARG, "displacement_mlp: null argument");
   if (mlp->n_freq < 16 || mlp->n_freq > 128 || (mlp->n_freq & 15) || mlp->n_pose < 0 || mlp->n_pose > 1024)
@@ -397,6 +419,7 @@ extern "C" rga_status displacement_mlp(rga_avatar* av, const rga_disp_mlp* mlp, 
 
 // back to the static per-vertex displacement of avatar_load after displacement_mlp
 extern "C" rga_status displacement_static(rga_avatar* av, void* stream) {
+  NvtxRange nvtx_("rga::displacement_static");
   if (!av) return fail(RGA_ERR_INVALID_ARG, "displacement_static: null avatar");
   cudaStream_t s = (cudaStream_t)stream;
   av->have_skin = av->have_vis = av->have_shade = av->have_splat = 0;
@@ -409,6 +432,7 @@ extern "C" rga_status displacement_static(rga_avatar* av, void* stream) {
 
 extern "C" rga_status splat_attribute(rga_avatar* av, const rga_camera* cam, const float bg[3], int which, float* out_image,
                                       void* stream) {
+  NvtxRange nvtx_("rga::splat_attribute");
   if (!av || !cam || !bg || !out_image) return fail(RGA_ERR_INVALID_ARG, "splat_attribute: null argument");
   if (which != RGA_ATTR_ALBEDO && which != RGA_ATTR_NORMAL) return fail(RGA_ERR_INVALID_ARG, "splat_attribute: unknown attribute %d", which);
   if (!av->have_skin) return fail(RGA_ERR_STATE, "splat_attribute: call pose_skin first");
@@ -433,6 +457,7 @@ extern "C" rga_status splat_attribute(rga_avatar* av, const rga_camera* cam, con
 extern "C" rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, const rga_vis_params* vis, const rga_env* env,
                                        const float cam_pos[3], const rga_camera* cam, const float bg[3], float* out_image,
                                        void* stream) {
+  NvtxRange nvtx_("rga::rga_render_frame");
   if (!av || !bone_mats || !env || !env->radiance || !cam_pos || !cam || !bg || !out_image)
     return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: null argument");
   if (env->use_visibility && !vis) return fail(RGA_ERR_INVALID_ARG, "rga_render_frame: use_visibility needs vis params");
@@ -569,6 +594,7 @@ extern "C" rga_status rga_get_buffer(rga_avatar* av, int which, void* stream, co
     case RGA_BUF_DENS_NG: p = av->dens_ng; n = (size_t)av->n_faces * 4; break;
     case RGA_BUF_DENS_HDR: p = av->dens_hdr; n = 16; break;
     case RGA_BUF_GAUSS_ORDER: p = av->g_order; n = ng * 4; break;
+    case RGA_BUF_VERT_NORMAL: p = av->vt_normal; n = nv * 12; break;
     default: return fail(RGA_ERR_INVALID_ARG, "rga_get_buffer: unknown id %d", which);
   }
   *dev_ptr = p; *bytes = n;

@@ -323,3 +323,68 @@ cudaError_t rga_launch_knn_gauss(rga_avatar* av, const float* q, cudaStream_t s)
                                                                 av->knn_d2);
   return cudaGetLastError();
 }
+
+// ------------------------------------------------------------------------------------------------------------------
+// vert_normal == NULL (include/rga.h; reading A40): area-weighted vertex normals of the canonical mesh,
+// n_v = normalize(sum over the faces that touch v, in ASCENDING face order, of (x_b - x_a) x (x_c - x_a)), one fp32 rounding per
+// operation (this file is compiled with -fmad=false).  The order is fixed because the normal feeds the bit-exact chain
+// (front-facing tests, visibility bits): a vertex -> face adjacency is built with atomics (any order) and each vertex then walks
+// its list by repeated selection of the next larger face index.  Load time only.
+__global__ void vn_count_kernel(int n3, const int* __restrict__ faces, unsigned* __restrict__ deg) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n3) atomicAdd(deg + faces[i], 1u);
+}
+
+__global__ void vn_fill_kernel(int n3, const int* __restrict__ faces, unsigned* __restrict__ cursor, int* __restrict__ adj) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n3) adj[atomicAdd(cursor + faces[i], 1u)] = i / 3;
+}
+
+__global__ void __launch_bounds__(128) vn_accum_kernel(int nv, const float* __restrict__ x, const int* __restrict__ faces,
+                                                       const unsigned* __restrict__ start, const int* __restrict__ adj,
+                                                       float* __restrict__ out) {
+  int v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= nv) return;
+  const unsigned lo = start[v], hi = start[v + 1];
+  float sx = 0.f, sy = 0.f, sz = 0.f;
+  int last = -1;
+  for (;;) {
+    int m = 0x7fffffff, cnt = 0;
+    for (unsigned j = lo; j < hi; ++j) {
+      int e = adj[j];
+      if (e > last && e < m) { m = e; cnt = 1; }
+      else if (e == m) ++cnt;                                    // a face that names v twice adds twice, as the plain loop does
+    }
+    if (cnt == 0) break;
+    const int a = faces[3 * m], b = faces[3 * m + 1], c = faces[3 * m + 2];
+    const float e1x = x[3 * b] - x[3 * a], e1y = x[3 * b + 1] - x[3 * a + 1], e1z = x[3 * b + 2] - x[3 * a + 2];
+    const float e2x = x[3 * c] - x[3 * a], e2y = x[3 * c + 1] - x[3 * a + 1], e2z = x[3 * c + 2] - x[3 * a + 2];
+    const float cx = e1y * e2z - e1z * e2y, cy = e1z * e2x - e1x * e2z, cz = e1x * e2y - e1y * e2x;
+    for (int r = 0; r < cnt; ++r) { sx = sx + cx; sy = sy + cy; sz = sz + cz; }
+    last = m;
+  }
+  const float len = sqrtf((sx * sx + sy * sy) + sz * sz);
+  if (len > 0.f) { sx = sx / len; sy = sy / len; sz = sz / len; }
+  out[3 * v] = sx; out[3 * v + 1] = sy; out[3 * v + 2] = sz;
+}
+
+// faces: device [n_faces][3] (indices already checked by the caller's contract), x: device [n_verts][3]; out: device [n_verts][3]
+cudaError_t rga_launch_vertex_normals(const float* x, const int* faces, int nv, int nf, float* out, cudaStream_t s) {
+  unsigned *deg = nullptr, *start = nullptr, *cursor = nullptr; int* adj = nullptr;
+  const int n3 = 3 * nf;
+  cudaError_t e = cudaMalloc(&deg, sizeof(unsigned) * ((size_t)nv + 1));
+  if (e == cudaSuccess) e = cudaMalloc(&start, sizeof(unsigned) * ((size_t)nv + 1));
+  if (e == cudaSuccess) e = cudaMalloc(&cursor, sizeof(unsigned) * ((size_t)nv + 1));
+  if (e == cudaSuccess) e = cudaMalloc(&adj, sizeof(int) * (size_t)n3);
+  if (e == cudaSuccess) e = cudaMemsetAsync(deg, 0, sizeof(unsigned) * ((size_t)nv + 1), s);
+  if (e == cudaSuccess) {
+    vn_count_kernel<<<(n3 + 255) / 256, 256, 0, s>>>(n3, faces, deg);
+    grid_scan_kernel<<<1, 1024, 0, s>>>(nv, deg, start, cursor);
+    vn_fill_kernel<<<(n3 + 255) / 256, 256, 0, s>>>(n3, faces, cursor, adj);
+    vn_accum_kernel<<<(nv + 127) / 128, 128, 0, s>>>(nv, x, faces, start, adj, out);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  }
+  cudaFree(deg); cudaFree(start); cudaFree(cursor); cudaFree(adj);
+  return e;
+}

@@ -135,6 +135,7 @@ int rga_vis_raster_max_bands(int max_res, int n_verts);
 int rga_vis_raster_needs_global_table(int max_res, int n_verts);
 size_t rga_vis_raster_plan(int res, int with_id, int n_verts, int* band_rows, int* threads, int* sxy_global);
 cudaError_t rga_launch_pack_faces(rga_avatar* av, cudaStream_t s);
+cudaError_t rga_launch_vertex_normals(const float* x, const int* faces, int nv, int nf, float* out, cudaStream_t s);
 // vis_shade_kernels.cu
 int rga_vis_shade_teams(int K, int ne);
 int rga_vis_shade_init_attributes();

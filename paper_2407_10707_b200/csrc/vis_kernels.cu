@@ -569,8 +569,17 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
   // last, partial round of the persistent grid: cut its units into triangle ranges (depth-only maps merge with atomicMin)
   int tail_first = n_units, split = 1;
   const int rem = n_units > grid_sm ? n_units % grid_sm : 0;
-  if (rem > 0 && !with_id && grid_sm / rem >= 2) {
-    split = grid_sm / rem > 4 ? 4 : grid_sm / rem;
+  int best_split = 1;
+  {
+    // the split (1..4) that leaves the shortest last round: ceil(rem * s / grid) / s
+    double best = 1.0;
+    for (int sp = 2; sp <= 4; ++sp) {
+      const double t = (double)((rem * sp + grid_sm - 1) / grid_sm) / sp;
+      if (t < best - 1e-9) { best = t; best_split = sp; }
+    }
+  }
+  if (rem > 0 && !with_id && best_split >= 2) {
+    split = best_split;
     tail_first = n_units - rem;
     const size_t unit_px = (size_t)band_rows * p->res;       // bands are even; the last may be shorter (covered anyway)
     const size_t first_px = binned ? (size_t)tail_first * p->res * p->res      // a binned unit is a whole direction

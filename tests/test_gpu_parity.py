@@ -597,6 +597,43 @@ def test_rotation_and_scale_as_vertex_attributes():
     av.close()
 
 
+def test_vertex_normals_from_the_geometry_when_none_are_passed():
+    # include/rga.h: vert_normal = NULL -> area-weighted normals of the canonical mesh in a fixed face order (reading A40).
+    # The computed table equals the oracle's bit for bit, and so does everything downstream (the whole frame compare);
+    # a mesh with a degree-200 fan vertex and an unreferenced vertex covers the long adjacency list and the zero normal.
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import compare_all, run_gpu
+    inp = workloads.make(1, n_gauss=20_000)
+    inp["vert_normal"] = None
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=0)
+    av, img = run_gpu(inp, vis_mode=0)
+    assert np.array_equal(av.read("VERT_NORMAL").reshape(-1, 3), orc_av["vert_normal"])
+    print(compare_all(inp, av, img, orc_av, o, 0))
+    av.close()
+    # fan: centre vertex 0, 200 rim vertices on a wobbling circle, one vertex no face names
+    rs = np.random.default_rng(5)
+    m = 200
+    ang = np.linspace(0.0, 2 * np.pi, m, endpoint=False)
+    rim = np.stack([np.cos(ang), np.sin(ang), 0.2 * rs.standard_normal(m)], 1)
+    v = np.concatenate([[[0.0, 0.0, 0.3]], rim, [[3.0, 3.0, 3.0]]]).astype(np.float32)
+    f = np.array([[0, 1 + i, 1 + (i + 1) % m] for i in range(m)], np.int32)[rs.permutation(m)]
+    exp = orc.vertex_normals(v, f)
+    assert np.all(exp[-1] == 0) and exp[0, 2] > 0.9
+    small = workloads.make(0)
+    nv = len(v)
+    inp2 = dict(small)
+    inp2.update(vert_pos=v, faces=f, vert_normal=None, vert_disp=None,
+                vert_skin_w=np.ascontiguousarray(np.tile(small["vert_skin_w"][:1], (nv, 1))),
+                vert_albedo=np.full((nv, 3), 0.5, np.float32), vert_rough=np.full(nv, 0.5, np.float32),
+                vert_spec=np.full(nv, 0.5, np.float32))
+    h = rga.avatar_load(inp2, 64, 64, 16, 64, 128)
+    assert np.array_equal(rga.rga_read_buffer(h, "VERT_NORMAL").reshape(-1, 3), exp)
+    rga.avatar_free(h)
+
+
 def test_displacement_mlp_then_gaussians_update_then_static():
     # gaussians_update after displacement_mlp must keep the network's displacement (re-interpolated over the NEW
     # neighbour sets), and displacement_static must restore the load-time table -- each state equals a fresh oracle load
