@@ -208,6 +208,58 @@ def make(cfg_id, seed=None, n_gauss=None, morton=False):
     return out
 
 
+def make_random(seed):
+    """A small RANDOM configuration for the randomised parity sweep (tests/test_gpu_random_configs.py): config 0 or 1 with
+    500..9000 Gaussians and everything the hot path is parameterised by drawn at random -- direction grid (K not a multiple
+    of 32), environment map (1..6 texels per direction), depth-map side (8..256, odd sizes), bias constants, Gaussian scale
+    and opacity ranges, image size (not a multiple of the 16-pixel tile), camera position / orientation / focal lengths /
+    principal point / near plane (close-ups give long tile lists), background, gamma, and in a third of the cases no vertex
+    normals (the library computes them).  Returns (inputs, description).  Inputs only."""
+    rs = np.random.default_rng(10_000 + seed)
+    base = int(rs.choice([0, 1, 1]))
+    ng = int(rs.integers(500, 9000))
+    inp = make(base, seed=seed, n_gauss=ng)
+    Rd, Cd = int(rs.integers(1, 7)), int(rs.integers(1, 13))
+    mr, mc = int(rs.choice([1, 1, 2, 3])), int(rs.choice([1, 1, 2]))
+    R, C = Rd * mr, Cd * mc
+    inp["vis_dirs"] = latlong_dirs(Rd, Cd)
+    inp["texel_to_dir"] = texel_to_dir((R, C), (Rd, Cd))
+    env = rs.uniform(0, 2, (1, R, C, 3)) if rs.integers(0, 2) == 0 else np.exp(rs.normal(0, 1, (1, R, C, 3)))
+    inp["env"] = np.ascontiguousarray(env, np.float32)
+    inp["env_rows"], inp["env_cols"] = R, C
+    inp["env_of_frame"] = np.zeros(len(inp["bone_mats"]), np.int32)
+    inp["vis_res"] = int(rs.choice([8, 17, 33, 64, 100, 128, 129, 200, 256]))
+    inp["depth_bias_texels"] = float(rs.choice([0.0, 0.5, 1.0, 2.0]))
+    inp["depth_bias_world"] = float(rs.choice([0.0, 0.005, 0.015, 0.05]))
+    inp["slope_max"] = float(rs.choice([1.0, 2.0, 8.0, 50.0]))
+    smax = float(rs.choice([5e-3, 1e-2, 3e-2, 8e-2]))
+    inp["gauss_scale"] = np.exp(rs.uniform(np.log(1e-3), np.log(smax), (ng, 3))).astype(np.float32)
+    inp["gauss_opacity"] = rs.uniform(float(rs.choice([0.05, 0.3, 0.9])), 1.0, ng).astype(np.float32)
+    v = inp["vert_pos"]
+    lo3, hi3 = v.min(0), v.max(0)
+    ctr = 0.5 * (lo3 + hi3)
+    rb = 0.5 * np.linalg.norm(hi3 - lo3)
+    W, H = int(rs.integers(20, 400)), int(rs.integers(20, 400))
+    az, el = rs.uniform(0, 2 * np.pi), rs.uniform(-1.2, 1.2)
+    dist = rb * float(rs.choice([0.6, 1.0, 2.0, 3.5]) if base == 1 else rs.choice([2.0, 3.5]))   # config 0 is a ball: stay outside
+    fwd = -np.array([np.cos(el) * np.cos(az), np.cos(el) * np.sin(az), np.sin(el)])
+    cam_pos = ctr - fwd * dist + rs.normal(0, 0.05, 3)
+    right = np.cross(fwd, np.array([0, 0, 1.0])); right /= np.linalg.norm(right)
+    R_wc = np.stack([right, np.cross(fwd, right), fwd])
+    fy = 0.5 * H / np.tan(0.5 * np.deg2rad(float(rs.choice([25, 40, 70]))))
+    inp["camera"] = dict(R_wc=R_wc.astype(np.float32).reshape(9), t_wc=(-R_wc @ cam_pos).astype(np.float32),
+                         fx=np.float32(fy * rs.uniform(0.8, 1.2)), fy=np.float32(fy), cx=np.float32(W / 2 + rs.uniform(-5, 5)),
+                         cy=np.float32(H / 2 + rs.uniform(-5, 5)), width=W, height=H, z_near=np.float32(rs.choice([0.05, 0.2, 0.8])))
+    inp["cam_pos"] = cam_pos.astype(np.float32)
+    inp["bg"] = rs.uniform(0, 1, 3).astype(np.float32)
+    inp["gamma"] = float(rs.choice([1.0, 2.2]))
+    if rs.uniform() < 0.3:
+        inp["vert_normal"] = None
+    desc = dict(seed=seed, base=base, n_gauss=ng, dirs=(Rd, Cd), env=(R, C), vis_res=inp["vis_res"], image=(W, H),
+                dist=round(float(dist), 2), scale_max=smax, normals=inp["vert_normal"] is not None)
+    return inp, desc
+
+
 def make_disp_mlp(seed=0, n_freq=64, n_pose=72, width=256, n_hidden=4, rff_sigma=1.0, out_scale=0.01):
     """Random weights of the displacement network d(x, theta): the trained weights are not
     available, so these are seeded stand-ins with the architecture of DESIGN.md readings A26-A28 (He-initialised hidden

@@ -70,7 +70,7 @@ def check_frame_visbits(inp, o, vb, cam_pos=None):
     return n_checked
 
 
-def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=None, frame_call=False):
+def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=None, frame_call=False, flag_per_pair=None):
     """Assert stage-by-stage parity.  `o` is oracle.render_frame's dict, `orc_av` oracle.avatar_load's.
     frame_call: the frame came from rga_render_frame, whose mode-0 depth test skips Gaussians that face away from the
     camera (their bits are never read): visibility bits are compared on the kept Gaussians and must be 0 on the culled."""
@@ -140,7 +140,11 @@ def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=N
     d = np.abs(img.astype(np.float64) - o["image"]).max(-1)
     fl = o["flags"].astype(bool)
     rep["image_max"], rep["image_mean"], rep["flagged"] = d[~fl].max() if (~fl).any() else 0.0, d.mean(), int(fl.sum())
-    assert fl.mean() <= 1e-4 or fl.sum() <= 2, "flag band too wide: %d px" % fl.sum()
+    # how many pixels may be flagged: 1e-4 of them on the configs; the band has a fixed RELATIVE width (A38), so the count really
+    # scales with the blended (pixel, entry) pairs -- the randomised sweep (large Gaussians seen close up) bounds it per pair
+    pairs = float(o["n_contrib"].astype(np.int64).sum())
+    allowed = max(2.0, 1e-4 * fl.size) if flag_per_pair is None else max(2.0, flag_per_pair * pairs)
+    assert fl.sum() <= allowed, "flag band too wide: %d px (allowed %.0f)" % (fl.sum(), allowed)
     assert rep["image_max"] <= IMG_MAX, "image max %g" % rep["image_max"]
     assert d.mean() <= IMG_MEAN, "image mean %g" % d.mean()
     H, W = img.shape[:2]
