@@ -61,7 +61,6 @@ KERNELS = {
     "tile_scan":          ("splat", "hbm", "tile", None),
     "tile_scatter":       ("splat", "hbm", "duplicate", 8.0 + 8.0),
     "tile_sort":          ("splat", "smem", "list entry", None),
-    "tile_sort_long":     ("splat", "smem", "list entry", None),
     "composite_T":        ("splat", "alu", "(pixel, list entry)", 50.0),
     "composite_segments": ("splat", "alu", "(pixel, list entry)", 50.0),
     "composite_resolve":  ("splat", "hbm", "pixel", None),

@@ -1,12 +1,13 @@
 // H8 (depth digit) + H10: per-tile sort and front-to-back alpha compositing (PAPER.md:103 -> 3DGS rasteriser, DESIGN.md
 // A18; black background PAPER.md:239-241 is the default of the bg parameter).
 //
-// Three kernels (the first version did all of this in one CTA per tile and left the SMs 63 % idle: 208 active tiles on
+// The kernels (the first version did all of this in one CTA per tile and left the SMs 63 % idle: 208 active tiles on
 // 148 SMs, each walking up to 1,304 entries serially -- profiles/r01a_ncu_full.md):
 //   tile_sort_kernel        one CTA per tile: the tile's bucket of (depth bits << 32 | Gaussian) keys (binned by
 //                           sort_kernels.cu) is sorted in shared memory by an ascending-only bitonic network (exact
 //                           integer compare, so the order equals the stable (tile, depth) sort of the emission order)
 //                           and written out as the sorted key/value lists; it also lists the tile's work items.
+//                           Buckets beyond 2,048 entries: a per-tile LSD radix sort in L2 (radix_sort_tile), same launch.
 //   composite_segment_kernel  front-to-back "over" is associative: (C,T) o (C',T') = (C + T C', T T').  A work item is
 //                           one segment of RGA_SEG consecutive list entries of one tile; persistent CTAs blend every
 //                           segment from T = 1 for the tile's 256 pixels, in parallel over all segments of all tiles.
@@ -29,7 +30,6 @@
 #define SEGMENT_GRID_MULT 8
 #endif
 #define SCAP_SMALL RGA_SORT_SMALL
-#define SCAP_LARGE 24576
 #define LOG2E_F 1.4426950408889634f
 
 // Ascending-only bitonic network on buf[0..n): every compare-exchange puts the minimum at the lower index, so virtual
@@ -110,28 +110,133 @@ __device__ __forceinline__ void sort_tile(int tile, unsigned capacity, int scap,
   __syncthreads();
 }
 
-// one CTA per tile; tiles with more than SCAP_SMALL entries are left to tile_sort_long_kernel
-__global__ void __launch_bounds__(SORT_THREADS) tile_sort_kernel(unsigned capacity, int scap,
+// Tiles with more than SCAP_SMALL entries (none at config 1, lists up to 8,688 at config 4):
+// LSD radix sort of the tile's 64-bit keys, 8 bits per pass, by one CTA per tile, ping-ponging between the bucket buffer and
+// the tile's own slice of keys_out (both in L2).  The list is cut into one contiguous part per warp; a pass is (1) per-warp
+// digit histograms, (2) a scan in (digit, warp) order, (3) a stable scatter in which every warp walks its part in order and
+// ranks equal digits inside a 32-key batch with match.any.  A pass whose digit is the same for every key (the upper index
+// bytes, the exponent byte of the depth) is skipped after its histogram.  The histograms live in the 16 KB the short tiles
+// use for their keys, so one launch sorts every tile (a separate long-list kernel with 192 KB of shared memory came before:
+// it had to wait for an empty SM even with nothing to sort, at the end of the chain the blend waits for).
+// Keys are distinct (the low word is the Gaussian's index), so the result is THE ascending order, as the bitonic network's.
+#define RADIX_WARPS (SORT_THREADS / 32)
+#ifndef RADIX_UNROLL
+#define RADIX_UNROLL 4
+#endif
+__device__ __forceinline__ void radix_sort_tile(int tile, unsigned capacity, int idx_bits, unsigned* s_hist /*[RADIX_WARPS][256]*/,
+    unsigned* s_base /*[256]*/, int* s_flag, const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off,
+    unsigned long long* __restrict__ lkeys, unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out,
+    unsigned* __restrict__ vals_int, const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
+  uint2 rg = ranges[tile];
+  rg.x = min(rg.x, capacity); rg.y = min(rg.y, capacity);
+  const int n = (int)(rg.y - rg.x);
+  const unsigned so = seg_off[tile];
+  for (int j = threadIdx.x; j < (n + RGA_SEG - 1) / RGA_SEG; j += SORT_THREADS) item_tab[so + j] = (unsigned)tile;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  const int per = (((n + RADIX_WARPS - 1) / RADIX_WARPS) + 31) & ~31;          // whole batches per warp
+  const int lo = min(n, warp * per), hi = min(n, lo + per);
+  unsigned long long* src = lkeys + rg.x;
+  unsigned long long* dst = keys_out + rg.x;
+  unsigned* hist = s_hist + warp * 256;
+  const int idx_passes = (idx_bits + 7) >> 3;
+  for (int pass = 0; pass < idx_passes + 4; ++pass) {
+    const int shift = pass < idx_passes ? 8 * pass : 32 + 8 * (pass - idx_passes);
+    for (int t = threadIdx.x; t < RADIX_WARPS * 256; t += SORT_THREADS) s_hist[t] = 0u;
+    if (threadIdx.x == 0) *s_flag = 0;
+    __syncthreads();
+    // (1) histogram of my part; RADIX_UNROLL batches are requested before the first is used (the loop is a chain of L2 trips)
+    for (int b = lo; b < hi; b += 32 * RADIX_UNROLL) {
+      unsigned long long kk[RADIX_UNROLL];
+#pragma unroll
+      for (int u = 0; u < RADIX_UNROLL; ++u) { const int i = b + 32 * u + lane; kk[u] = i < hi ? src[i] : 0ull; }
+#pragma unroll
+      for (int u = 0; u < RADIX_UNROLL; ++u) {
+        const bool act = b + 32 * u + lane < hi;
+        const unsigned am = __ballot_sync(0xffffffffu, act);
+        if (act) {
+          const unsigned d = (unsigned)(kk[u] >> shift) & 255u;
+          const unsigned m = __match_any_sync(am, d);
+          if ((m & lt) == 0u) hist[d] += (unsigned)__popc(m);                   // lowest lane of each digit group; one warp per row
+        }
+        __syncwarp();
+      }
+    }
+    __syncthreads();
+    // (2) exclusive scan in (digit, warp) order: s_hist[w][d] <- keys of digit d in warps before w; s_base[d] <- keys of digits < d
+    if (threadIdx.x < 256) {
+      unsigned run = 0u;
+      for (int w = 0; w < RADIX_WARPS; ++w) { const unsigned c = s_hist[w * 256 + threadIdx.x]; s_hist[w * 256 + threadIdx.x] = run; run += c; }
+      s_base[threadIdx.x] = run;
+      if (run == (unsigned)n) *s_flag = 1;                                       // every key has this digit: nothing to move
+    }
+    __syncthreads();
+    if (*s_flag) { __syncthreads(); continue; }
+    if (warp == 0) {
+      unsigned v[8], sum = 0u;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { v[e] = s_base[lane * 8 + e]; sum += v[e]; }
+      unsigned inc = sum;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const unsigned u = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += u; }
+      unsigned ex = inc - sum;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { s_base[lane * 8 + e] = ex; ex += v[e]; }
+    }
+    __syncthreads();
+    // (3) stable scatter
+    for (int b = lo; b < hi; b += 32 * RADIX_UNROLL) {
+      unsigned long long kk[RADIX_UNROLL];
+#pragma unroll
+      for (int u = 0; u < RADIX_UNROLL; ++u) { const int i = b + 32 * u + lane; kk[u] = i < hi ? src[i] : 0ull; }
+#pragma unroll
+      for (int u = 0; u < RADIX_UNROLL; ++u) {
+        const bool act = b + 32 * u + lane < hi;
+        const unsigned am = __ballot_sync(0xffffffffu, act);
+        const unsigned long long k = kk[u];
+        unsigned d = 0u, m = 0u, off = 0u;
+        if (act) {
+          d = (unsigned)(k >> shift) & 255u;
+          m = __match_any_sync(am, d);
+          off = hist[d];
+        }
+        __syncwarp();
+        if (act) {
+          if ((m & lt) == 0u) hist[d] = off + (unsigned)__popc(m);
+          dst[s_base[d] + off + (unsigned)__popc(m & lt)] = k;
+        }
+        __syncwarp();
+      }
+    }
+    __syncthreads();
+    unsigned long long* t = src; src = dst; dst = t;
+  }
+  // H8 output from the sorted keys (in place when they ended in the tile's slice of keys_out: one element per thread)
+  for (int i = threadIdx.x; i < n; i += SORT_THREADS) {
+    const unsigned long long k = src[i];
+    keys_out[rg.x + i] = ((unsigned long long)(unsigned)tile << 32) | (k >> 32);
+    vals_out[rg.x + i] = (unsigned)k;
+    vals_int[rg.x + i] = (unsigned)inv[(unsigned)k];
+  }
+  __syncthreads();
+}
+
+// one CTA per tile: bitonic in shared memory up to SCAP_SMALL entries, the radix sort above beyond
+__global__ void __launch_bounds__(SORT_THREADS) tile_sort_kernel(unsigned capacity, int scap, int idx_bits,
     const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, unsigned long long* __restrict__ lkeys,
     unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ vals_int,
     const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
-  extern __shared__ __align__(16) unsigned long long s_keys[];
+  extern __shared__ __align__(16) unsigned long long s_keys[];                   // scap keys, or RADIX_WARPS x 256 counters
+  __shared__ unsigned s_base[256];
+  __shared__ int s_flag;
   const uint2 rg = ranges[blockIdx.x];
   const unsigned n = min(rg.y, capacity) - min(rg.x, capacity);
-  if (n == 0 || n > (unsigned)scap) return;
-  sort_tile(blockIdx.x, capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, vals_int, inv, item_tab);
-}
-
-// the tiles listed by tile_scan_kernel as long (usually none): persistent CTAs with the large shared-memory buffer;
-// buckets beyond it are sorted in place in global memory by the same network
-__global__ void __launch_bounds__(SORT_THREADS) tile_sort_long_kernel(unsigned capacity, int scap, const unsigned* __restrict__ num_long,
-    const unsigned* __restrict__ long_list, const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off,
-    unsigned long long* __restrict__ lkeys, unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out,
-    unsigned* __restrict__ vals_int, const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
-  extern __shared__ __align__(16) unsigned long long s_keys[];
-  const unsigned nl = *num_long;
-  for (unsigned q = blockIdx.x; q < nl; q += gridDim.x)
-    sort_tile((int)long_list[q], capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, vals_int, inv, item_tab);
+  if (n == 0) return;
+  if (n > (unsigned)scap)
+    radix_sort_tile(blockIdx.x, capacity, idx_bits, reinterpret_cast<unsigned*>(s_keys), s_base, &s_flag, ranges, seg_off, lkeys, keys_out,
+                    vals_out, vals_int, inv, item_tab);
+  else
+    sort_tile(blockIdx.x, capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, vals_int, inv, item_tab);
 }
 
 // Thread -> pixel of the 16x16 tile: a warp owns an 8x4 block of pixels (2 x 4 blocks per tile), so that a Gaussian
@@ -375,7 +480,7 @@ __global__ void __launch_bounds__(CB) composite_replay_kernel(int W, int H, int 
 
 
 int rga_composite_init_attributes() {
-  return (int)cudaFuncSetAttribute(tile_sort_long_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SCAP_LARGE * 8);
+  return 0;                                                      // no kernel here needs more than the default 48 KB
 }
 
 // Attribute maps (PAPER.md:177 albedo map for editing; PAPER.md:239 albedo and normal maps for the metrics): the colour
@@ -399,13 +504,12 @@ cudaError_t rga_launch_attr_color(rga_avatar* av, int which, cudaStream_t s) {
 cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
   const int ntiles = TX * TY;
-  tile_sort_kernel<<<ntiles, SORT_THREADS, SCAP_SMALL * 8, s>>>((unsigned)av->max_dup, SCAP_SMALL, av->ranges, av->seg_off, av->keys[0],
+  static_assert(SCAP_SMALL * 8 >= RADIX_WARPS * 256 * 4, "the radix histograms reuse the key buffer");
+  int idx_bits = 1; while (idx_bits < 32 && (1ll << idx_bits) < (long long)av->n_gauss) ++idx_bits;
+  tile_sort_kernel<<<ntiles, SORT_THREADS, SCAP_SMALL * 8, s>>>((unsigned)av->max_dup, SCAP_SMALL, idx_bits, av->ranges, av->seg_off, av->keys[0],
                                                            av->keys[1], av->vals[0], av->vals[1], av->g_inv, av->item_tab);
   rga_prof_mark(av, "tile_sort", s);
-  tile_sort_long_kernel<<<av->num_sms, SORT_THREADS, SCAP_LARGE * 8, s>>>((unsigned)av->max_dup, SCAP_LARGE, av->num_long, av->long_list,
-      av->ranges, av->seg_off, av->keys[0], av->keys[1], av->vals[0], av->vals[1], av->g_inv, av->item_tab);
-  rga_prof_mark(av, "tile_sort_long", s);
-  av->launches += 2;
+  av->launches += 1;
   return cudaGetLastError();
 }
 

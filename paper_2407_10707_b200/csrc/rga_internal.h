@@ -7,7 +7,7 @@
 
 #define RGA_TILE 16
 #define RGA_MAX_PROF 96
-#define RGA_SORT_SMALL 2048      // tiles up to this many entries are sorted by the one-CTA-per-tile kernel
+#define RGA_SORT_SMALL 2048      // tiles up to this many entries are sorted in shared memory (bitonic), longer ones by the radix path of the same kernel
 #define RGA_SEG 64               // compositing segment: list entries blended by one work item
 
 struct rga_avatar {
@@ -79,8 +79,6 @@ struct rga_avatar {
   float4* part;                // [items_cap][256] per-pixel partial (C, T) of each segment
   unsigned* part_last;         // [items_cap][256] last contributing entry of the segment (1-based, 0 = none)
   long long items_cap;
-  unsigned* num_long;          // [1] tiles with more than RGA_SORT_SMALL entries
-  unsigned* long_list;         // [tiles] their ids
   int* stop_seg;               // [pixels] segment in which the pixel's blend stops (-1: list exhausted)
   unsigned char* item_flag;    // [items_cap] work item has pixels to replay (cleared by the replay kernel)
   float* t_final; unsigned* n_contrib;

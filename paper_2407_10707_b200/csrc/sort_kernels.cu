@@ -14,12 +14,12 @@
 // threads): ranges, scatter cursors, D, capacity check; segment offsets and the number of compositing work items
 __global__ void __launch_bounds__(1024) tile_scan_kernel(int ntiles, long long capacity, const unsigned* __restrict__ tile_count,
     uint2* __restrict__ ranges, unsigned* __restrict__ cursor, unsigned* __restrict__ num_dup, unsigned* __restrict__ seg_off,
-    unsigned* __restrict__ num_items, unsigned* __restrict__ num_long, unsigned* __restrict__ long_list,
+    unsigned* __restrict__ num_items,
     int* __restrict__ status) {
   __shared__ unsigned wsum[32], wseg[32];
-  __shared__ unsigned carry, carry_seg, nlong;
+  __shared__ unsigned carry, carry_seg;
   __shared__ unsigned long long total64;                  // D in 64 bits: the 32-bit running sum may wrap before the capacity check
-  if (threadIdx.x == 0) { carry = 0; carry_seg = 0; nlong = 0; total64 = 0ull; }
+  if (threadIdx.x == 0) { carry = 0; carry_seg = 0; total64 = 0ull; }
   __syncthreads();
   for (int base = 0; base < ntiles; base += 1024) {
     int i = base + threadIdx.x;
@@ -54,7 +54,6 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int ntiles, long long c
       ranges[i] = v ? make_uint2(excl, excl + v) : make_uint2(0u, 0u);     // empty tiles report (0,0)
       cursor[i] = excl;
       seg_off[i] = gexcl;
-      if (v > RGA_SORT_SMALL) long_list[atomicAdd(&nlong, 1u)] = (unsigned)i;      // sorted by tile_sort_long_kernel
     }
     __syncthreads();
     if (threadIdx.x == 1023) { carry = excl + v; carry_seg = gexcl + g; }
@@ -69,7 +68,6 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int ntiles, long long c
     *num_dup = total64 > 0xffffffffull ? 0xffffffffu : carry;
     seg_off[ntiles] = overflow ? 0u : carry_seg;
     *num_items = overflow ? 0u : carry_seg;
-    *num_long = overflow ? 0u : nlong;
   }
 }
 
@@ -100,7 +98,7 @@ __global__ void __launch_bounds__(256) tile_scatter_kernel(int ng, int TX, long 
 
 cudaError_t rga_launch_bin(rga_avatar* av, int TX, int ntiles, cudaStream_t s) {
   tile_scan_kernel<<<1, 1024, 0, s>>>(ntiles, av->max_dup, av->tile_count, av->ranges, av->cursor, av->num_dup, av->seg_off,
-                                      av->num_items, av->num_long, av->long_list, av->status);
+                                      av->num_items, av->status);
   rga_prof_mark(av, "tile_scan", s);
   tile_scatter_kernel<<<(av->n_gauss + 255) / 256, 256, 0, s>>>(av->n_gauss, TX, av->max_dup, av->touched, av->rect, av->depth,
                                                                av->g_order, av->cursor, av->keys[0]);
