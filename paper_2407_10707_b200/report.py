@@ -22,6 +22,9 @@ def main():
     print("| `e2e.pipelined_value` (read-back on a copy stream) | %.1f |" % d["e2e"]["pipelined_value"])
     print("| `warm_l2_fps` (no L2 flush) | %.1f |" % d["warm_l2_fps"])
     print("| `value_spatially_sorted_input` (same frame, Gaussians pre-sorted) | %s |" % _f(d.get("value_spatially_sorted_input"), 1))
+    fl = d.get("frames_in_flight_fps")
+    if fl:
+        print("| `frames_in_flight_fps` (1 / 2 / 3 avatar handles on their own streams, warm L2; not the metric) | %.1f / %.1f / %.1f |" % (fl["1"], fl["2"], fl["3"]))
     print("| `value_cull_backfaces` (closed-mesh option, NOT the contract path) | %.1f |" % d["value_cull_backfaces"])
     print("| kernels launched per frame | %s |" % _f(d.get("gpu_launches_per_step"), 0))
     print("| `avatar_load` (once) | %.1f ms |" % d["avatar_load_ms"])
