@@ -189,6 +189,21 @@ RGA_API rga_status shade_backward(rga_avatar* av, const rga_env* env, const floa
 RGA_API rga_status image_loss(rga_avatar* av, const float* image, const float* target, int width, int height, float lambda,
                               float* out_loss, float* out_dL_dimage, void* stream);
 
+/* image_loss without an avatar handle and WITHOUT ANY ALLOCATION (Eq.5; same kernels, same arithmetic, same
+ * arguments as image_loss): for callers that cannot call cudaMalloc -- code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid it.  Its scratch (nine floats per pixel + two accumulators) is a fixed device array inside the
+ * library: width * height <= RGA_IMAGE_LOSS_STATIC_MAX_PIXELS (262,144 = 512 x 512), larger images are refused with
+ * RGA_ERR_INVALID_ARG and a message; every GPU that loads the library holds the array's 9.0 MiB until the process exits.
+ * The call makes no cudaMalloc / cudaFree and calls no allocating library routine; it enqueues one 16-byte memset and up
+ * to three kernels on `stream` (device of the current context).  ALL calls share the one array, which keeps the last call's
+ * contents (everything a call reads is rewritten by that call first): calls on the same stream are ordered and safe; calls
+ * that overlap on the GPU (different streams, or several host threads on different streams) RACE -- serialise them.
+ * image, target: dev [height][width][3]; out_loss: dev f32 [3] = {L_img, L_1, SSIM} or NULL; out_dL_dimage: dev
+ * [height][width][3] or NULL.  Enqueue-only. */
+#define RGA_IMAGE_LOSS_STATIC_MAX_PIXELS 262144
+RGA_API rga_status rga_image_loss_static(const float* image, const float* target, int width, int height, float lambda,
+                                         float* out_loss, float* out_dL_dimage, void* stream);
+
 /* Regularisers of the training objective Eq.10, evaluated on the avatar's own tables, each as the plain
  * sum the paper writes (the lambdas of Eq.10 are the caller's), with gradients:
  *   Eq.6 L_smooth = sum_i sum_{k in S_v^i} ||*^i - *^k||_1 over the vertex attributes * in {albedo, roughness, specular};

@@ -208,6 +208,17 @@ def image_loss(h, image, target, lam=0.2, out_loss=None, out_dL_dimage=None):
                           _ptr(out_dL_dimage), _stream()))
 
 
+IMAGE_LOSS_STATIC_MAX_PIXELS = 262144
+
+
+def rga_image_loss_static(image, target, lam=0.2, out_loss=None, out_dL_dimage=None):
+    """Eq.5 image loss and its gradient with the library's fixed scratch array: no avatar handle, no allocation
+    (include/rga.h rga_image_loss_static; width * height <= IMAGE_LOSS_STATIC_MAX_PIXELS).  image, target: CUDA float32 [H, W, 3]."""
+    lib().rga_image_loss_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
+    _chk(lib().rga_image_loss_static(_ptr(image), _ptr(target), int(image.shape[1]), int(image.shape[0]), float(lam), _ptr(out_loss),
+                                     _ptr(out_dL_dimage), _stream()))
+
+
 def regularisers(h, s0=0.005, out_losses=None, out_dalbedo=None, out_drough=None, out_dspec=None, out_dgauss_pos=None, out_ddisp=None,
                  out_dscale=None):
     """Eq.6-9 and their gradients on the avatar's own tables (include/rga.h regularisers)."""

@@ -366,6 +366,20 @@ extern "C" rga_status image_loss(rga_avatar* av, const float* image, const float
   return RGA_OK;
 }
 
+extern "C" rga_status rga_image_loss_static(const float* image, const float* target, int width, int height, float lambda,
+                                            float* out_loss, float* out_dL_dimage, void* stream) {
+  NvtxRange nvtx_("rga::rga_image_loss_static");
+  if (!image || !target) return fail(RGA_ERR_INVALID_ARG, "rga_image_loss_static: null argument");
+  if (width < 1 || height < 1) return fail(RGA_ERR_INVALID_ARG, "rga_image_loss_static: empty image");
+  if ((long long)width * (long long)height > (long long)RGA_IMAGE_LOSS_STATIC_MAX_PIXELS)
+    return fail(RGA_ERR_INVALID_ARG, "rga_image_loss_static: %d x %d = %lld pixels is above the static scratch of %d pixels "
+                "(RGA_IMAGE_LOSS_STATIC_MAX_PIXELS); use image_loss with an avatar handle for larger images",
+                width, height, (long long)width * height, (int)RGA_IMAGE_LOSS_STATIC_MAX_PIXELS);
+  if (!(lambda >= 0.f && lambda <= 1.f)) return fail(RGA_ERR_INVALID_ARG, "rga_image_loss_static: lambda must be in [0, 1]");
+  CU(rga_launch_image_loss_static(image, target, width, height, lambda, out_loss, out_dL_dimage, (cudaStream_t)stream));
+  return RGA_OK;
+}
+
 extern "C" rga_status regularisers(rga_avatar* av, float s0, float* out_losses, float* out_dalbedo, float* out_drough, float* out_dspec,
                                    float* out_dgauss_pos, float* out_ddisp, float* out_dscale, void* stream) {
   NvtxRange nvtx_("rga::regularisers");

@@ -249,3 +249,57 @@ cudaError_t rga_launch_regularisers(rga_avatar* av, float s0, float* out_losses,
   av->launches += 2 + (out_losses != nullptr);
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// rga_image_loss_static (include/rga.h): Eq.5 and its gradient WITHOUT an avatar handle and without any allocation -- for
+// callers that cannot reach cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it).
+// The scratch the two kernels above need (nine floats per pixel between them, two double accumulators) lives in ONE
+// file-scope device array of a fixed size: every GPU that loads librga.so holds these 9.0 MiB until the process exits.
+// In HOST code the array's name is only a stand-in for the symbol, not a device address; the address is asked for once per
+// device with cudaGetSymbolAddress, with that device current, and the kernels get that pointer.
+// The array is shared by every call and keeps the last call's contents: the accumulators are cleared on the stream at the
+// start of each call, the per-pixel maps are written for every pixel of the image before the gradient kernel reads them (it
+// reads no pixel outside the image), so nothing stale is used.  Two calls that overlap on the GPU (different streams) race.
+#include <mutex>
+
+#define RGA_STATIC_LOSS_HEAD 256                      /* bytes in front of the maps: the two double accumulators */
+static __device__ __align__(256) unsigned char g_static_loss_scratch[RGA_STATIC_LOSS_HEAD + (size_t)RGA_IMAGE_LOSS_STATIC_MAX_PIXELS * 9 * sizeof(float)];
+
+static std::mutex g_static_loss_mutex;
+static unsigned char* g_static_loss_ptr[RGA_STATIC_MAX_DEVICES];       // per device: the array's DEVICE address, once known
+
+// device address of the scratch array on the CURRENT device (looked up once per device); nullptr + *err on failure
+static unsigned char* static_loss_scratch(cudaError_t* err) {
+  int dev = -1;
+  *err = cudaGetDevice(&dev);
+  if (*err != cudaSuccess) return nullptr;
+  if (dev < 0 || dev >= RGA_STATIC_MAX_DEVICES) { *err = cudaErrorInvalidDevice; return nullptr; }
+  std::lock_guard<std::mutex> lock(g_static_loss_mutex);
+  if (!g_static_loss_ptr[dev]) {
+    void* p = nullptr;
+    *err = cudaGetSymbolAddress(&p, g_static_loss_scratch);
+    if (*err != cudaSuccess) return nullptr;
+    g_static_loss_ptr[dev] = static_cast<unsigned char*>(p);
+  }
+  return g_static_loss_ptr[dev];
+}
+
+// W * H <= RGA_IMAGE_LOSS_STATIC_MAX_PIXELS is the caller's check (api.cu).  No cudaMalloc / cudaFree here or below.
+cudaError_t rga_launch_image_loss_static(const float* image, const float* target, int W, int H, float lam, float* out_loss,
+                                         float* out_dimage, cudaStream_t s) {
+  cudaError_t e = cudaSuccess;
+  unsigned char* base = static_loss_scratch(&e);
+  if (!base) return e;
+  double* sums = reinterpret_cast<double*>(base);
+  float* maps = reinterpret_cast<float*>(base + RGA_STATIC_LOSS_HEAD);
+  SsimWin win; double g[11], tot = 0.0;
+  for (int k = 0; k < 11; ++k) { g[k] = exp(-(double)((k - 5) * (k - 5)) / (2.0 * 1.5 * 1.5)); tot += g[k]; }
+  for (int k = 0; k < 11; ++k) win.w[k] = (float)(g[k] / tot);
+  e = cudaMemsetAsync(sums, 0, 2 * sizeof(double), s);                 // the accumulators must start at zero
+  if (e != cudaSuccess) return e;
+  const dim3 grid((W + LT - 1) / LT, (H + LT - 1) / LT);
+  ssim_maps_kernel<<<grid, 256, 0, s>>>(W, H, win, image, target, maps, sums);
+  if (out_dimage) ssim_grad_kernel<<<grid, 256, 0, s>>>(W, H, win, lam, image, target, maps, out_dimage);
+  if (out_loss) image_loss_finish_kernel<<<1, 1, 0, s>>>(W, H, lam, sums, out_loss);
+  return cudaGetLastError();
+}

@@ -7,6 +7,7 @@
 
 #define RGA_TILE 16
 #define RGA_MAX_PROF 96
+#define RGA_STATIC_MAX_DEVICES 64   // devices whose static-scratch address rga_image_loss_static remembers
 #define RGA_SORT_SMALL 2048      // tiles up to this many entries are sorted in shared memory (bitonic), longer ones by the radix path of the same kernel
 #define RGA_SEG 64               // compositing segment: list entries blended by one work item
 
@@ -167,6 +168,8 @@ cudaError_t rga_launch_shade_backward(rga_avatar* av, const rga_env* env, float3
                                       float* out_drough, float* out_dspec, float* out_dnormal, float* out_dpos, float* out_denv, cudaStream_t s);
 int rga_shade_backward_init_attributes(int max_env);
 // loss_kernels.cu
+cudaError_t rga_launch_image_loss_static(const float* image, const float* target, int W, int H, float lam, float* out_loss,
+                                         float* out_dimage, cudaStream_t s);
 cudaError_t rga_launch_image_loss(rga_avatar* av, const float* image, const float* target, int W, int H, float lam, float* out_loss,
                                   float* out_dimage, cudaStream_t s);
 cudaError_t rga_launch_regularisers(rga_avatar* av, float s0, float* out_losses, float* d_alb, float* d_rough, float* d_spec, float* d_gpos,
