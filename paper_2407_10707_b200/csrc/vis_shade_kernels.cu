@@ -19,7 +19,10 @@
 #include "rga_internal.h"
 
 #define PI_F 3.14159265358979323846f
-#define VS_TEAM_WARPS 8
+#ifndef VS_TEAM_WARPS
+#define VS_TEAM_WARPS 8        /* measured: teams of 4 / 16 warps give 177 / 151 us at config 1 against 118 us */
+#endif
+#define VS_CTAS_PER_SM(T) (32 / (VS_TEAM_WARPS * (T)) > 0 ? 32 / (VS_TEAM_WARPS * (T)) : 1)
 #define VS_TEAM_THREADS (VS_TEAM_WARPS * 32)
 
 __device__ __forceinline__ float vs_rsq(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
@@ -114,38 +117,75 @@ struct VsArgs {
 };
 
 static size_t vs_smem_bytes(int K, int ne, int teams) {
-  return (size_t)K * 48 + (size_t)ne * 32 + (size_t)K * 4 + (size_t)(K + 2) * 2 + (size_t)(ne + 2) * 4 + 16 +
-         (size_t)teams * VS_TEAM_WARPS * 6 * 32 * 4;
+  return (size_t)K * 48 + (size_t)((ne + 1) / 2) * 48 + (size_t)K * 4 + (size_t)(K + 2) * 2 + (size_t)(ne + 4) * 4 + 16 +
+         (size_t)2 * teams * VS_TEAM_WARPS * 6 * 32 * 4;
 }
 
 // One BRDF term of Eq.2 (Eq.12-15) for the lanes whose weight c = max(0, w_i . n) v is positive; accumulates diffuse (d) and
 // specular (s) sums per channel.
 struct VsBrdf { float wox, woy, woz, nwo_raw, al2, omk, kk, cS, tox, toy, toz; };
 
+// Packed fp32 (sm_100 FFMA2 / FMUL2 / FADD2: one issue slot, two IEEE operations): the BRDF loop takes the texels of a
+// direction unit TWO at a time, the pair's values side by side in 64-bit registers.  The kernel is bound by issue slots, not
+// by the FMA pipe (profiles/r02_vis_shade.md), so halving the count of its fp32 instructions is what pays.
+__device__ __forceinline__ float2 vs_bc(float a) { return make_float2(a, a); }
+#define VS_FMA2 __ffma2_rn
+#define VS_MUL2 __fmul2_rn
+#define VS_ADD2 __fadd2_rn
+
+// The rare middle case of a depth test: z lies between the two ends of the bias beta(tau).  An approximate tau decides unless z
+// is within `margin` of the threshold; only then the exact IEEE sqrt and divide of the contract are evaluated -- the bit is the
+// same.  Out of line: inlined into every one of the sixteen unrolled tests it made the loop larger than the instruction cache.
+__device__ __noinline__ bool vs_slope_test(float z, float zm, float c, float bt, float bw, float slope_max, float margin) {
+  float tau = slope_max;
+  if (c > 0.0f) {
+    const float s2 = fmaxf(__fmaf_rn(-c, c, 1.0f), 0.0f);
+    tau = fminf(fmaxf(__fmul_rn(vs_sqrt(s2), vs_rcp(c)), 1.0f), slope_max);
+  }
+  const float dlt = __fadd_rn(z, -__fadd_rn(zm, __fmaf_rn(bt, tau, bw)));
+  if (fabsf(dlt) > margin) return dlt < 0.0f;
+  float te = slope_max;
+  if (c > 0.0f) {
+    const float s2 = fmaxf(__fsub_rn(1.0f, __fmul_rn(c, c)), 0.0f);
+    te = fminf(fmaxf(__fdiv_rn(__fsqrt_rn(s2), c), 1.0f), slope_max);
+  }
+  return z <= __fadd_rn(zm, __fadd_rn(__fmul_rn(bt, te), bw));
+}
+
 template <int TEAMS, bool IDENT>
-__global__ void __launch_bounds__(VS_TEAM_THREADS * TEAMS, (TEAMS == 1 ? 4 : (TEAMS == 2 ? 2 : 1))) vis_shade_kernel(const VsArgs a) {
+__global__ void __launch_bounds__(VS_TEAM_THREADS * TEAMS, VS_CTAS_PER_SM(TEAMS)) vis_shade_kernel(const VsArgs a) {
   extern __shared__ __align__(16) unsigned char vs_raw[];
   const int K = a.K, ne = a.ne, R = a.R, words = a.words;
   // per direction three float4: A = (us.xyz, vs.x)  B = (vs.yz, wn.xy)  C = (wn.z, w.xyz)
   float4* sF = reinterpret_cast<float4*>(vs_raw);                                  // [3K]
-  float4* sE = sF + 3 * K;                                                        // [2 ne]
-  float* sPart = reinterpret_cast<float*>(sE + 2 * ne);                           // [TEAMS][8][6][32]
-  float* sEps = sPart + TEAMS * VS_TEAM_WARPS * 6 * 32;                           // [K]
+  // environment rows in LIST order (texels sorted by the direction they read), two texels side by side: per pair three float4
+  // (wi.x0 wi.x1 wi.y0 wi.y1) (wi.z0 wi.z1 LA.r0 LA.r1) (LA.g0 LA.g1 LA.b0 LA.b1)
+  float4* sE = sF + 3 * K;                                                        // [3 ceil(ne / 2)]
+  float* sPart = reinterpret_cast<float*>(sE + 3 * ((ne + 1) >> 1));              // [2][TEAMS][8][6][32] (two groups in flight)
+  float* sEps = sPart + 2 * TEAMS * VS_TEAM_WARPS * 6 * 32;                       // [K]
   unsigned short* sStart = reinterpret_cast<unsigned short*>(sEps + K);           // [K + 1]
-  unsigned short* sTex = sStart + ((K + 2) & ~1);                                 // [ne] texels sorted by direction
-  unsigned short* sTexD = sTex + ((ne + 1) & ~1);                                 // [ne] their directions
-  __shared__ unsigned s_ticket[TEAMS];
+  unsigned short* sTexD = sStart + ((K + 2) & ~1);                                // [ne + 2] direction of the texel at each list position
+  __shared__ unsigned s_ticket[2][TEAMS];
   for (int t = threadIdx.x; t < K; t += blockDim.x) {
     const float4 u = a.frames[2 + 3 * t], v = a.frames[3 + 3 * t], w = a.frames[4 + 3 * t];
     sF[3 * t] = make_float4(u.x, u.y, u.z, v.x); sF[3 * t + 1] = make_float4(v.y, v.z, w.x, w.y); sF[3 * t + 2] = make_float4(w.z, u.w, v.w, w.w);
     sEps[t] = a.dir_eps[t];
   }
-  for (int t = threadIdx.x; t < 2 * ne; t += blockDim.x) sE[t] = reinterpret_cast<const float4*>(a.env_table)[t];
+  for (int t = threadIdx.x; t < ((ne + 1) & ~1); t += blockDim.x) {
+    float4 wi = make_float4(0.f, 0.f, 1.f, 0.f), LA = make_float4(0.f, 0.f, 0.f, 0.f);       // padding of an odd list: adds nothing
+    if (t < ne) {
+      const int k = IDENT ? t : (int)a.tex_list[t];
+      wi = reinterpret_cast<const float4*>(a.env_table)[2 * k]; LA = reinterpret_cast<const float4*>(a.env_table)[2 * k + 1];
+    }
+    float* e = reinterpret_cast<float*>(sE + 3 * (t >> 1)) + (t & 1);
+    e[0] = wi.x; e[2] = wi.y; e[4] = wi.z; e[6] = LA.x; e[8] = LA.y; e[10] = LA.z;
+  }
   if (!IDENT) {
     for (int t = threadIdx.x; t <= K; t += blockDim.x) sStart[t] = a.dir_start[t];
-    for (int t = threadIdx.x; t < ne; t += blockDim.x) { sTex[t] = a.tex_list[t]; sTexD[t] = a.tex_dir[t]; }
+    for (int t = threadIdx.x; t < ne + 2; t += blockDim.x) sTexD[t] = t < ne ? a.tex_dir[t] : (unsigned short)0;
   }
   const float4 h0 = a.frames[0], h1 = a.frames[1];
+  if ((threadIdx.x & (VS_TEAM_THREADS - 1)) == 0) s_ticket[0][threadIdx.x / VS_TEAM_THREADS] = atomicAdd(a.counter, 1u);   // the team's first group
   __syncthreads();
   const float cx = h0.x, cy = h0.y, cz = h0.z, hR = h0.w, bt = h1.x, bw = h1.y, slope_max = h1.z;
   const int lane = threadIdx.x & 31, team = threadIdx.x / VS_TEAM_THREADS, tw = (threadIdx.x >> 5) & (VS_TEAM_WARPS - 1);
@@ -160,18 +200,21 @@ __global__ void __launch_bounds__(VS_TEAM_THREADS * TEAMS, (TEAMS == 1 ? 4 : (TE
   const float Rm1 = (float)(R - 1), Rf = (float)R;
   const size_t RR = (size_t)R * R;
   const int nunits = 2 * words;                                                   // a unit = 16 directions (half a visibility word)
-  float* myPart = sPart + ((size_t)team * VS_TEAM_WARPS + tw) * 6 * 32;
+  // ONE barrier per group: the team's lead draws the NEXT ticket while the group is computed (the atomic's round trip hides
+  // behind the work) and publishes it, with the warps' partial sums, at the barrier that ends the group; tickets and partial
+  // sums are double-buffered, so the first warp folds group i while the others are already in group i + 1.
+  const unsigned beyond_last = ngroups + gridDim.x * TEAMS - 1u;
   unsigned short* vis16 = reinterpret_cast<unsigned short*>(a.visbits);
-  for (;;) {
-    team_sync(team);                                                              // s_ticket and sPart are reused
-    if (team_lead) s_ticket[team] = atomicAdd(a.counter, 1u);
-    team_sync(team);
-    const unsigned group = s_ticket[team];
+  for (int it = 0;; ++it) {
+    const unsigned group = s_ticket[it & 1][team];
     if (group >= ngroups) {
       // every team draws exactly one ticket beyond the groups: the last of them re-arms the counter for the next launch
-      if (team_lead && group == ngroups + gridDim.x * TEAMS - 1u) *a.counter = 0u;
+      if (team_lead && group == beyond_last) *a.counter = 0u;
       break;
     }
+    unsigned next_ticket = 0u;
+    if (team_lead) next_ticket = atomicAdd(a.counter, 1u);
+    float* myPart = sPart + (((size_t)(it & 1) * TEAMS + team) * VS_TEAM_WARPS + tw) * 6 * 32;
     const unsigned li = group * 32u + (unsigned)lane;
     const bool valid = li < nfront;
     const int g = a.front_list[valid ? li : group * 32u];                         // idle lanes shadow the group's first Gaussian
@@ -190,7 +233,11 @@ __global__ void __launch_bounds__(VS_TEAM_THREADS * TEAMS, (TEAMS == 1 ? 4 : (TE
       q.cS = q.al2 / (4.f * PI_F * (fmaxf(q.nwo_raw, 0.f) * q.omk + q.kk));         // D F G /(4 ni no) = cS F / (den^2 gi)
     }
     const float dx = __fsub_rn(x.x, cx), dy = __fsub_rn(x.y, cy), dz = __fsub_rn(x.z, cz);
-    float d0 = 0.f, d1 = 0.f, d2 = 0.f, s0 = 0.f, s1 = 0.f, s2 = 0.f;
+    // the pair's constants: the same value in both halves
+    const float2 nx2 = vs_bc(n.x), ny2 = vs_bc(n.y), nz2 = vs_bc(n.z), mnx2 = vs_bc(-n.x), mny2 = vs_bc(-n.y), mnz2 = vs_bc(-n.z);
+    const float2 wox2 = vs_bc(q.wox), woy2 = vs_bc(q.woy), woz2 = vs_bc(q.woz), nwo2 = vs_bc(q.nwo_raw), al22 = vs_bc(q.al2),
+                 omk2 = vs_bc(q.omk), kk2 = vs_bc(q.kk), cS2 = vs_bc(q.cS);
+    float2 d0 = vs_bc(0.f), d1 = vs_bc(0.f), d2 = vs_bc(0.f), s0 = vs_bc(0.f), s1 = vs_bc(0.f), s2 = vs_bc(0.f);   // (even, odd) list positions
     // units are dealt to the team's warps round robin (static, so that every sum has one fixed order): warp w takes the
     // half-words w, w + 8, ... -- the rows of a lat-long direction grid are spread evenly over the warps
     for (int unit = tw; unit < nunits; unit += VS_TEAM_WARPS) {
@@ -233,25 +280,9 @@ __global__ void __launch_bounds__(VS_TEAM_THREADS * TEAMS, (TEAMS == 1 ? 4 : (TE
           // visible iff z <= zm + beta(tau); NaN compares false, so "not (z > ...)" also covers the empty texel
           bool vis = !(z[u] > __fadd_rn(zm[u], blo));
           if (!vis && !(z[u] > __fadd_rn(zm[u], bhi))) {
-            // in between: an approximate tau decides unless z is within `margin` of the threshold; only then the exact
-            // IEEE sqrt and divide of the contract are evaluated -- the bit is the same
             const float4 C = sF[3 * (k0 + min(b0 + u, kend - 1)) + 2];
             const float c = __fadd_rn(__fadd_rn(__fmul_rn(n.x, C.y), __fmul_rn(n.y, C.z)), __fmul_rn(n.z, C.w));   // dot3(n_gd, w)
-            float tau = slope_max;
-            if (c > 0.0f) {
-              const float s2 = fmaxf(__fmaf_rn(-c, c, 1.0f), 0.0f);
-              tau = fminf(fmaxf(__fmul_rn(vs_sqrt(s2), vs_rcp(c)), 1.0f), slope_max);
-            }
-            const float dlt = __fadd_rn(z[u], -__fadd_rn(zm[u], __fmaf_rn(bt, tau, bw)));
-            if (fabsf(dlt) > margin) vis = dlt < 0.0f;
-            else {
-              float te = slope_max;
-              if (c > 0.0f) {
-                const float s2 = fmaxf(__fsub_rn(1.0f, __fmul_rn(c, c)), 0.0f);
-                te = fminf(fmaxf(__fdiv_rn(__fsqrt_rn(s2), c), 1.0f), slope_max);
-              }
-              vis = z[u] <= __fadd_rn(zm[u], __fadd_rn(__fmul_rn(bt, te), bw));
-            }
+            vis = vs_slope_test(z[u], zm[u], c, bt, bw, slope_max, margin);
           }
           bits |= (vis ? 1u : 0u) << (b0 + u);
         }
@@ -262,41 +293,52 @@ __global__ void __launch_bounds__(VS_TEAM_THREADS * TEAMS, (TEAMS == 1 ? 4 : (TE
       const unsigned anyb = __reduce_or_sync(0xffffffffu, bits);
       if (anyb == 0u) continue;
       const int t0 = IDENT ? k0 : sStart[k0], t1 = IDENT ? k0 + kend : sStart[k0 + kend];
-#pragma unroll 4
-      for (int t = t0; t < t1; ++t) {
-        const int k = IDENT ? t : sTex[t];
-        const int j = (IDENT ? t : (int)sTexD[t]) - k0;
-        const float4 wi = sE[2 * k];
-        const float c = n.x * wi.x + n.y * wi.y + n.z * wi.z;
-        const bool live = ((bits >> j) & 1u) && (c > 0.f);                       // max(0, w_i . n) and the visibility bit
-        if (!__any_sync(0xffffffffu, live)) continue;
-        const float4 LA = sE[2 * k + 1];
-        const float ow = q.wox * wi.x + q.woy * wi.y + q.woz * wi.z;
-        const float hl2 = fmaxf(2.f + 2.f * ow, 1e-12f);                         // |w_i + w_o|^2
-        const float hinv = vs_rsq(hl2);
-        const float nh = (c + q.nwo_raw) * hinv;
-        const float oh = (0.5f * hl2) * hinv;                                    // w_o . h
-        const float tx = fmaf(-c, n.x, wi.x) + q.tox, ty = fmaf(-c, n.y, wi.y) + q.toy, tz = fmaf(-c, n.z, wi.z) + q.toz;
-        const float den = fmaf(q.al2 * nh, nh, (tx * tx + ty * ty + tz * tz) * (hinv * hinv));   // (n.h)^2 (a^2 - 1) + 1, Eq.13
-        const float F = fmaf(0.96f, vs_ex2((-5.55473f * oh - 6.98316f) * oh), 0.04f);           // Eq.14
-        const float gi = fmaf(c, q.omk, q.kk);
-        const float sp = q.cS * F * vs_rcp(den * den * gi);
-        const float w = live ? c : 0.f;                                          // branch-free: dead lanes add zero
-        const float ws = w * sp;
-        d0 = fmaf(LA.x, w, d0); d1 = fmaf(LA.y, w, d1); d2 = fmaf(LA.z, w, d2);
-        s0 = fmaf(LA.x, ws, s0); s1 = fmaf(LA.y, ws, s1); s2 = fmaf(LA.z, ws, s2);
+#pragma unroll 2
+      for (int t = t0 & ~1; t < t1; t += 2) {                                     // list positions t (even) and t + 1
+        const float4* ep = sE + 3 * (t >> 1);
+        const float4 Wa = ep[0], Wb = ep[1];
+        const float2 wix = make_float2(Wa.x, Wa.y), wiy = make_float2(Wa.z, Wa.w), wiz = make_float2(Wb.x, Wb.y), LAx = make_float2(Wb.z, Wb.w);
+        const float2 c = VS_FMA2(nz2, wiz, VS_FMA2(ny2, wiy, VS_MUL2(nx2, wix)));      // w_i . n
+        const int j0 = ((IDENT ? t : (int)sTexD[t]) - k0) & 31, j1 = ((IDENT ? t + 1 : (int)sTexD[t + 1]) - k0) & 31;
+        const bool live0 = t >= t0 && ((bits >> j0) & 1u) && c.x > 0.f;             // max(0, w_i . n) and the visibility bit
+        const bool live1 = t + 1 < t1 && ((bits >> j1) & 1u) && c.y > 0.f;
+        if (!__any_sync(0xffffffffu, live0 || live1)) continue;
+        const float4 Wc = ep[2];
+        const float2 LAy = make_float2(Wc.x, Wc.y), LAz = make_float2(Wc.z, Wc.w);
+        const float2 sx = VS_ADD2(wix, wox2), sy = VS_ADD2(wiy, woy2), sz = VS_ADD2(wiz, woz2);     // w_i + w_o
+        float2 hl2 = VS_FMA2(sz, sz, VS_FMA2(sy, sy, VS_MUL2(sx, sx)));                  // |w_i + w_o|^2
+        hl2.x = fmaxf(hl2.x, 1e-12f); hl2.y = fmaxf(hl2.y, 1e-12f);
+        const float2 hinv = make_float2(vs_rsq(hl2.x), vs_rsq(hl2.y));
+        const float2 ns = VS_ADD2(c, nwo2);                                              // n . (w_i + w_o)
+        const float2 nh = VS_MUL2(ns, hinv);
+        const float2 oh = VS_MUL2(VS_MUL2(vs_bc(0.5f), hl2), hinv);                      // w_o . h
+        // 1 - (n.h)^2 = |t|^2 / |w_i + w_o|^2 with t the tangential part of w_i + w_o (the direct form cancels for small alpha)
+        const float2 tx = VS_FMA2(ns, mnx2, sx), ty = VS_FMA2(ns, mny2, sy), tz = VS_FMA2(ns, mnz2, sz);
+        const float2 tt = VS_FMA2(tz, tz, VS_FMA2(ty, ty, VS_MUL2(tx, tx)));
+        const float2 den = VS_FMA2(VS_MUL2(al22, nh), nh, VS_MUL2(tt, VS_MUL2(hinv, hinv)));   // (n.h)^2 (a^2 - 1) + 1, Eq.13
+        const float2 u = VS_MUL2(VS_FMA2(vs_bc(-5.55473f), oh, vs_bc(-6.98316f)), oh);
+        const float2 F = VS_FMA2(vs_bc(0.96f), make_float2(vs_ex2(u.x), vs_ex2(u.y)), vs_bc(0.04f));        // Eq.14
+        const float2 gi = VS_FMA2(c, omk2, kk2);
+        const float2 qd = VS_MUL2(VS_MUL2(den, den), gi);
+        const float2 sp = VS_MUL2(VS_MUL2(cS2, F), make_float2(vs_rcp(qd.x), vs_rcp(qd.y)));
+        const float2 w = make_float2(live0 ? c.x : 0.f, live1 ? c.y : 0.f);               // branch-free: dead entries add zero
+        const float2 ws = VS_MUL2(w, sp);
+        d0 = VS_FMA2(LAx, w, d0); d1 = VS_FMA2(LAy, w, d1); d2 = VS_FMA2(LAz, w, d2);
+        s0 = VS_FMA2(LAx, ws, s0); s1 = VS_FMA2(LAy, ws, s1); s2 = VS_FMA2(LAz, ws, s2);
       }
     }
-    // ---- the warps' partial sums are folded in warp order by the team's first warp, which finishes Eq.12 and the gamma curve
-    myPart[lane] = d0; myPart[32 + lane] = d1; myPart[64 + lane] = d2; myPart[96 + lane] = s0; myPart[128 + lane] = s1; myPart[160 + lane] = s2;
+    // ---- the warps' partial sums are folded in warp order by one warp of the team (the duty rotates), which finishes Eq.12 and the gamma curve
+    myPart[lane] = d0.x + d0.y; myPart[32 + lane] = d1.x + d1.y; myPart[64 + lane] = d2.x + d2.y;
+    myPart[96 + lane] = s0.x + s0.y; myPart[128 + lane] = s1.x + s1.y; myPart[160 + lane] = s2.x + s2.y;
+    if (team_lead) s_ticket[(it + 1) & 1][team] = next_ticket;
     team_sync(team);
-    if (tw != 0) continue;
+    if (tw != (it & (VS_TEAM_WARPS - 1))) continue;                               // the fold duty goes round the team's warps
     float acc[6];
 #pragma unroll
     for (int c = 0; c < 6; ++c) {
       float sum = 0.f;
 #pragma unroll
-      for (int w = 0; w < VS_TEAM_WARPS; ++w) sum += sPart[(((size_t)team * VS_TEAM_WARPS + w) * 6 + c) * 32 + lane];
+      for (int w = 0; w < VS_TEAM_WARPS; ++w) sum += sPart[((((size_t)(it & 1) * TEAMS + team) * VS_TEAM_WARPS + w) * 6 + c) * 32 + lane];
       acc[c] = sum;
     }
     if (valid) {
@@ -315,9 +357,9 @@ __global__ void __launch_bounds__(VS_TEAM_THREADS * TEAMS, (TEAMS == 1 ? 4 : (TE
 int rga_vis_shade_teams(int K, int ne) {
   if (K < 1 || K > 2048 || ne < 1 || ne > 4096) return 0;
   const size_t lim = 227 * 1024 - 1024;
-  if (vs_smem_bytes(K, ne, 1) <= 56 * 1024) return 1;                              // four CTAs of one team per SM
-  if (vs_smem_bytes(K, ne, 2) <= 113 * 1024) return 2;
-  if (vs_smem_bytes(K, ne, 4) <= lim) return 4;
+  // as many CTAs per SM as fill its 32 warp slots at 64 registers; more teams per CTA when the tables are too large for that
+  for (int t = 1; t * VS_TEAM_WARPS <= 32; t *= 2)
+    if (vs_smem_bytes(K, ne, t) <= lim / (size_t)VS_CTAS_PER_SM(t) - 1024) return t;
   return 0;
 }
 
@@ -325,10 +367,12 @@ int rga_vis_shade_init_attributes() {
   const int mx = 227 * 1024 - 1024;
   cudaError_t e = cudaFuncSetAttribute(vis_shade_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_shade_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+#if VS_TEAM_WARPS * 4 <= 32
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_shade_kernel<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_shade_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+#endif
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_shade_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_shade_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(vis_shade_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
   return (int)e;
 }
 
@@ -366,7 +410,7 @@ cudaError_t rga_launch_vis_shade(rga_avatar* av, const rga_vis_params* vis, cons
   a.cam = cam; a.inv_gamma = 1.0f / env->gamma;
   a.radiance = av->radiance; a.color = av->color; a.visbits = av->visbits; a.counter = av->vs_counter;
   const size_t smem = vs_smem_bytes(K, ne, teams);
-  const int per_sm = teams == 1 ? 4 : (teams == 2 ? 2 : 1);
+  const int per_sm = VS_CTAS_PER_SM(teams);
   int grid = av->num_sms * per_sm;
   const int max_groups = (av->n_gauss + 31) / 32;
   if (grid * teams > max_groups) grid = (max_groups + teams - 1) / teams;
@@ -374,7 +418,11 @@ cudaError_t rga_launch_vis_shade(rga_avatar* av, const rga_vis_params* vis, cons
   const bool ident = env->texel_to_dir == nullptr && ne == K;              // texel k reads direction k: no texel lists
   if (teams == 1) { if (ident) vis_shade_kernel<1, true><<<grid, VS_TEAM_THREADS, smem, s>>>(a); else vis_shade_kernel<1, false><<<grid, VS_TEAM_THREADS, smem, s>>>(a); }
   else if (teams == 2) { if (ident) vis_shade_kernel<2, true><<<grid, 2 * VS_TEAM_THREADS, smem, s>>>(a); else vis_shade_kernel<2, false><<<grid, 2 * VS_TEAM_THREADS, smem, s>>>(a); }
+#if VS_TEAM_WARPS * 4 <= 32
   else { if (ident) vis_shade_kernel<4, true><<<grid, 4 * VS_TEAM_THREADS, smem, s>>>(a); else vis_shade_kernel<4, false><<<grid, 4 * VS_TEAM_THREADS, smem, s>>>(a); }
+#else
+  else return cudaErrorInvalidConfiguration;
+#endif
   rga_prof_mark(av, "vis_shade", s);
   av->launches += 1;
   return cudaGetLastError();
