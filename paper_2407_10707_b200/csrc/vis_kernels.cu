@@ -93,6 +93,7 @@ struct RasterWarp {
                                // edge-function coefficients and box of the 32 triangles being sampled
   uint4 q2[RAST_Q];            // runs with covered samples: {triangle | mask << 24 | tall << 28 | wide << 31, first pixel, e1, e2}
   int q1[RAST_Q];              // triangles whose pixel box is not empty
+  int q1s[RAST_Q];             // ... of which the box is ONE run (one line of up to RAST_SEGW pixel centres, int32 edge functions)
 };
 
 struct RasterCtx {
@@ -293,6 +294,54 @@ __device__ __forceinline__ int raster_round(const RasterCtx& c, RasterWarp* w, i
   return q2n;
 }
 
+// B2s. a round of SINGLE-RUN triangles (three quarters of the non-empty boxes at config 1: 1 x 1 .. 1 x 4 and their transposes):
+// lane l samples its own triangle's one run -- no scan over run counts, no round table, no owner search.  It builds exactly
+// the q2 entry raster_round would build for that run (same exchanged space for a tall run, same e1 / e2 at the first sample,
+// same mask), so the depth stage and the result are the same.
+template <bool WITH_ID>
+__device__ __forceinline__ int raster_single(const RasterCtx& c, RasterWarp* w, int qbase, int n, int lane, int q2n) {
+  unsigned mask = 0u;
+  uint4 out = make_uint4(0u, 0u, 0u, 0u);
+  if (lane < n) {
+    const int t = w->q1s[qbase + lane];
+    int i0, i1, i2;
+    face_unpack(__ldg(c.faces_packed + t), i0, i1, i2);
+    unsigned P0 = c.sXY[i0], P1 = c.sXY[i1], P2 = c.sXY[i2];
+    int ia, ja, bw, bh; bool narrow;
+    tri_box(P0, P1, P2, c.R, c.row0, c.rows, ia, ja, bw, bh, narrow);
+    const bool tall = bh > bw;
+    out.y = (unsigned)((ja - c.row0) * c.R + ia);
+    if (tall) {
+      P0 = __funnelshift_l(P0, P0, 16); P1 = __funnelshift_l(P1, P1, 16); P2 = __funnelshift_l(P2, P2, 16);
+      int tmp = ia; ia = ja; ja = tmp; bw = bh;
+      out.x = 1u << 28;
+    }
+    const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
+    const int qx = 256 * ia + 128, qy = 256 * ja + 128;
+    int e0 = (x2 - x1) * (qy - y1) - (y2 - y1) * (qx - x1);
+    int e1 = (x0 - x2) * (qy - y2) - (y0 - y2) * (qx - x2);
+    int e2 = (x1 - x0) * (qy - y0) - (y1 - y0) * (qx - x0);
+    if (e0 + e1 + e2 != 0) {                                            // area == 0: skipped (contract)
+      const int ax0 = -256 * (y2 - y1), ax1 = -256 * (y0 - y2), ax2 = -256 * (y1 - y0);
+      out.z = (unsigned)e1; out.w = (unsigned)e2;
+#pragma unroll
+      for (int u = 0; u < RAST_SEGW; ++u) {
+        if (u < bw && (min(e0, min(e1, e2)) >= 0 || max(e0, max(e1, e2)) <= 0)) mask |= 1u << u;
+        e0 += ax0; e1 += ax1; e2 += ax2;
+      }
+    }
+    if (mask) out.x |= (unsigned)t | (mask << 24);
+  }
+  const unsigned cm = __ballot_sync(0xffffffffu, mask != 0u);
+  if (cm) {
+    if (mask) w->q2[q2n + __popc(cm & ((1u << lane) - 1u))] = out;
+    q2n += __popc(cm);
+    __syncwarp();
+    if (q2n >= 32) { q2n -= 32; raster_depth<WITH_ID>(c, w, q2n, 32, lane); __syncwarp(); }
+  }
+  return q2n;
+}
+
 template <bool WITH_ID, bool BINNED, bool GTAB>
 __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
     int tail_first, int split,
@@ -381,7 +430,7 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
     c.R = R; c.row0 = row0; c.rows = rows; c.sXY = sXY; c.v_posed = v_posed; c.faces_packed = faces_packed;
     c.sz32 = sz32; c.sz64 = sz64; c.zf = s_zf;
     // B1. triangles: one per lane, 32 per warp fetched dynamically; non-empty boxes queued
-    int qn = 0, q2n = 0;                                    // warp-uniform queue fills
+    int qn = 0, qsn = 0, q2n = 0;                           // warp-uniform queue fills
     for (;;) {
       int base4 = 0;
       if (lane == 0) base4 = atomicAdd(&s_next, RAST_FETCH);   // RAST_FETCH / 32 batches per fetch
@@ -390,12 +439,11 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
 #pragma unroll 1
       for (int base = base4; base < min(base4 + RAST_FETCH, t_end); base += 32) {
         const int t = base + lane;
-        bool ne = false;
+        bool ne = false, narrow = false;
         int ia = 0, ja = 0, bw = 0, bh = 0;
         if (t < t_end) {
           int i0, i1, i2;
           face_unpack(__ldg(faces_packed + t), i0, i1, i2);
-          bool narrow;
           const unsigned Q0 = sXY[i0], Q1 = sXY[i1], Q2 = sXY[i2];
           ne = tri_box(Q0, Q1, Q2, R, row0, rows, ia, ja, bw, bh, narrow) > 0;
           if (cull && ne) {                               // reading A36: negative snapped area = facing away from the light
@@ -408,13 +456,27 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
           if (ne) {
             const int jb2 = ja + bh - 1;
             const int blo = (ja * band_magic) >> 16, bhi = (jb2 * band_magic) >> 16;
-            for (int b = blo; b <= bhi; ++b) bins[((size_t)blockIdx.x * n_bands + b) * (size_t)nf + atomicAdd(&s_bin_cnt[b], 1u)] = (unsigned)t;
+            // bit 31: the whole box is one run (then so is its part in any band)
+            const unsigned entry = (unsigned)t | ((narrow && min(bw, bh) == 1 && max(bw, bh) <= RAST_SEGW) ? 0x80000000u : 0u);
+            for (int b = blo; b <= bhi; ++b) bins[((size_t)blockIdx.x * n_bands + b) * (size_t)nf + atomicAdd(&s_bin_cnt[b], 1u)] = entry;
           }
           continue;
         }
-        const unsigned m = __ballot_sync(0xffffffffu, ne);
+        // two queues: boxes that are one run (sampled by their own lane, raster_single) and the rest (runs dealt out, raster_round)
+        const bool single = ne && narrow && min(bw, bh) == 1 && max(bw, bh) <= RAST_SEGW;
+        const unsigned ms = __ballot_sync(0xffffffffu, single), m = __ballot_sync(0xffffffffu, ne && !single);
+        if (ms) {
+          if (single) w->q1s[qsn + __popc(ms & ((1u << lane) - 1u))] = t;
+          qsn += __popc(ms);
+          __syncwarp();
+          if (qsn >= 32) {
+            qsn -= 32;
+            q2n = raster_single<WITH_ID>(c, w, qsn, 32, lane, q2n);
+            __syncwarp();
+          }
+        }
         if (m) {
-          if (ne) w->q1[qn + __popc(m & ((1u << lane) - 1u))] = t;
+          if (ne && !single) w->q1[qn + __popc(m & ((1u << lane) - 1u))] = t;
           qn += __popc(m);
           __syncwarp();
           if (qn >= 32) {
@@ -425,6 +487,7 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
         }
       }
     }
+    if (qsn) { q2n = raster_single<WITH_ID>(c, w, 0, qsn, lane, q2n); __syncwarp(); }
     if (qn) { q2n = raster_round<WITH_ID>(c, w, 0, qn, lane, q2n); __syncwarp(); }
     if (q2n) raster_depth<WITH_ID>(c, w, 0, q2n, lane);
     __syncthreads();
@@ -446,18 +509,25 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
       __syncthreads();
       const int nlist = (int)s_bin_cnt[band];
       const unsigned* list = bins + ((size_t)blockIdx.x * n_bands + band) * (size_t)nf;
-      int q2b = 0;
+      int q2b = 0, qb = 0, qsb = 0;
       for (;;) {
         int base = 0;
         if (lane == 0) base = atomicAdd(&s_next, 32);
         base = __shfl_sync(0xffffffffu, base, 0);
         if (base >= nlist) break;
         const int cnt = min(32, nlist - base);
-        if (lane < cnt) w->q1[lane] = (int)__ldcg(list + base + lane);
+        const unsigned entry = lane < cnt ? __ldcg(list + base + lane) : 0u;
+        const bool single = lane < cnt && (entry >> 31), multi = lane < cnt && !(entry >> 31);
+        const unsigned ms = __ballot_sync(0xffffffffu, single), mm = __ballot_sync(0xffffffffu, multi);
+        if (single) w->q1s[qsb + __popc(ms & ((1u << lane) - 1u))] = (int)(entry & 0xffffffu);
+        if (multi) w->q1[qb + __popc(mm & ((1u << lane) - 1u))] = (int)(entry & 0xffffffu);
+        qsb += __popc(ms); qb += __popc(mm);
         __syncwarp();
-        q2b = raster_round<WITH_ID>(c, w, 0, cnt, lane, q2b);
-        __syncwarp();
+        if (qsb >= 32) { qsb -= 32; q2b = raster_single<WITH_ID>(c, w, qsb, 32, lane, q2b); __syncwarp(); }
+        if (qb >= 32) { qb -= 32; q2b = raster_round<WITH_ID>(c, w, qb, 32, lane, q2b); __syncwarp(); }
       }
+      if (qsb) { q2b = raster_single<WITH_ID>(c, w, 0, qsb, lane, q2b); __syncwarp(); }
+      if (qb) { q2b = raster_round<WITH_ID>(c, w, 0, qb, lane, q2b); __syncwarp(); }
       if (q2b) raster_depth<WITH_ID>(c, w, 0, q2b, lane);
       __syncthreads();
     }
