@@ -80,6 +80,7 @@ struct rga_avatar {
   float4* part;                // [items_cap][256] per-pixel partial (C, T) of each segment
   unsigned* part_last;         // [items_cap][256] last contributing entry of the segment (1-based, 0 = none)
   long long items_cap;
+  float* env_pairs;            // [ceil(max_env / 2)][12] environment rows in list order, pairs side by side (fused kernel's table image)
   int* stop_seg;               // [pixels] segment in which the pixel's blend stops (-1: list exhausted)
   unsigned char* item_flag;    // [items_cap] work item has pixels to replay (cleared by the replay kernel)
   float* t_final; unsigned* n_contrib;

@@ -395,9 +395,11 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
       // the pre-scaled frame and the depth-test constants for the fused depth-test + shading kernel (vis_shade_kernels.cu,
       // a FAST file): written HERE, by the EXACT file's make_win / make_frame -- layout as light_frames_kernel below
       if (frames_out && band == 0 && t_begin == 0) {
-        frames_out[2 + 3 * k] = make_float4(F.us[0], F.us[1], F.us[2], F.w[0]);
-        frames_out[2 + 3 * k + 1] = make_float4(F.vs[0], F.vs[1], F.vs[2], F.w[1]);
-        frames_out[2 + 3 * k + 2] = make_float4(F.wn[0], F.wn[1], F.wn[2], F.w[2]);
+        // A = (us.xyz, vs.x)  B = (vs.yz, wn.xy)  C = (wn.z, w.xyz): the layout the fused kernel keeps in shared memory, so that
+        // its CTAs stage the table with one bulk copy
+        frames_out[2 + 3 * k] = make_float4(F.us[0], F.us[1], F.us[2], F.vs[0]);
+        frames_out[2 + 3 * k + 1] = make_float4(F.vs[1], F.vs[2], F.wn[0], F.wn[1]);
+        frames_out[2 + 3 * k + 2] = make_float4(F.wn[2], F.w[0], F.w[1], F.w[2]);
         if (k == 0) {
           frames_out[0] = make_float4(W.cx, W.cy, W.cz, W.hR);
           frames_out[1] = make_float4(bias_texels / (float)R, bias_world * W.inv2r, slope_max, (float)R);
@@ -715,7 +717,7 @@ int rga_vis_raster_needs_global_table(int max_res, int n_verts) {
 // Pre-scaled light frames and depth-test constants for the fused depth-test + shading kernel (vis_shade_kernels.cu, a FAST
 // file): computed HERE, in the EXACT file, by the same make_win / make_frame as every other visibility kernel.
 // out: float4[2 + 3K]: (cx, cy, cz, hR) (bias_texels / R, bias_world * inv2r, slope_max, R) then per direction
-// (us, w.x) (vs, w.y) (wn, w.z).
+// (us.xyz, vs.x) (vs.yz, wn.xy) (wn.z, w.xyz).
 __global__ void light_frames_kernel(int K, int R, const float* __restrict__ dirs, const float* __restrict__ window, float bias_texels,
                                     float bias_world, float slope_max, float4* __restrict__ out) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -726,9 +728,9 @@ __global__ void light_frames_kernel(int K, int R, const float* __restrict__ dirs
   }
   if (k >= K) return;
   const LightFrame f = make_frame(dirs + 3 * k, W);
-  out[2 + 3 * k] = make_float4(f.us[0], f.us[1], f.us[2], f.w[0]);
-  out[2 + 3 * k + 1] = make_float4(f.vs[0], f.vs[1], f.vs[2], f.w[1]);
-  out[2 + 3 * k + 2] = make_float4(f.wn[0], f.wn[1], f.wn[2], f.w[2]);
+  out[2 + 3 * k] = make_float4(f.us[0], f.us[1], f.us[2], f.vs[0]);
+  out[2 + 3 * k + 1] = make_float4(f.vs[1], f.vs[2], f.wn[0], f.wn[1]);
+  out[2 + 3 * k + 2] = make_float4(f.wn[2], f.w[0], f.w[1], f.w[2]);
 }
 
 cudaError_t rga_launch_light_frames(rga_avatar* av, const rga_vis_params* p, cudaStream_t s) {

@@ -63,7 +63,8 @@ __global__ void __launch_bounds__(256) front_compact_kernel(int ng, int words, f
 // texel index inside a direction) and eps[d] = largest chord |w_k - w_d| over its texels + 1e-3 (a direction without
 // texels gets eps = -4: never needed).  One CTA; ne <= 4096, K <= 2048.
 __global__ void __launch_bounds__(1024) texel_csr_kernel(int ne, int K, const int* __restrict__ t2d, const float* __restrict__ env_table,
-    const float* __restrict__ dirs, unsigned short* __restrict__ dir_start, unsigned short* __restrict__ tex_list, unsigned short* __restrict__ tex_dir, float* __restrict__ dir_eps) {
+    const float* __restrict__ dirs, unsigned short* __restrict__ dir_start, unsigned short* __restrict__ tex_list, unsigned short* __restrict__ tex_dir, float* __restrict__ dir_eps,
+    float* __restrict__ env_pairs) {
   __shared__ unsigned s_cnt[2048 + 1];
   __shared__ unsigned s_eps[2048];
   __shared__ unsigned short s_d[4096];
@@ -101,6 +102,18 @@ __global__ void __launch_bounds__(1024) texel_csr_kernel(int ne, int K, const in
     }
     for (int i = b; i < e; ++i) { tex_list[i] = s_list[i]; tex_dir[i] = (unsigned short)d; }
   }
+  // the environment rows in LIST order, two list positions side by side (12 floats per pair: wi.x0 wi.x1 wi.y0 wi.y1 wi.z0 wi.z1
+  // LA.r0 LA.r1 LA.g0 LA.g1 LA.b0 LA.b1): the image of the fused kernel's shared-memory table, staged there by one bulk copy
+  __syncthreads();
+  for (int t = threadIdx.x; t < ((ne + 1) & ~1); t += blockDim.x) {
+    float4 wi = make_float4(0.f, 0.f, 1.f, 0.f), LA = make_float4(0.f, 0.f, 0.f, 0.f);       // padding of an odd list: adds nothing
+    if (t < ne) {
+      const int k = (int)s_list[t];
+      wi = reinterpret_cast<const float4*>(env_table)[2 * k]; LA = reinterpret_cast<const float4*>(env_table)[2 * k + 1];
+    }
+    float* e = env_pairs + 12 * (size_t)(t >> 1) + (t & 1);
+    e[0] = wi.x; e[2] = wi.y; e[4] = wi.z; e[6] = LA.x; e[8] = LA.y; e[10] = LA.z;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -108,6 +121,7 @@ struct VsArgs {
   int K, R, ne, words;
   const float4* frames;              // [2 + 3K]: (cx,cy,cz,hR) (bt,bw,slope_max,R) then per direction (us,w.x) (vs,w.y) (wn,w.z)
   const float* env_table;            // [ne][8]
+  const float* env_pairs;            // [ceil(ne / 2)][12]: the rows in list order, pairs side by side (texel_csr_kernel)
   const unsigned short* dir_start; const unsigned short* tex_list; const unsigned short* tex_dir; const float* dir_eps;
   const unsigned* zmap;
   const int* front_list; const unsigned* n_front;
@@ -166,27 +180,35 @@ __global__ void __launch_bounds__(VS_TEAM_THREADS * TEAMS, VS_CTAS_PER_SM(TEAMS)
   unsigned short* sStart = reinterpret_cast<unsigned short*>(sEps + K);           // [K + 1]
   unsigned short* sTexD = sStart + ((K + 2) & ~1);                                // [ne + 2] direction of the texel at each list position
   __shared__ unsigned s_ticket[2][TEAMS];
-  for (int t = threadIdx.x; t < K; t += blockDim.x) {
-    const float4 u = a.frames[2 + 3 * t], v = a.frames[3 + 3 * t], w = a.frames[4 + 3 * t];
-    sF[3 * t] = make_float4(u.x, u.y, u.z, v.x); sF[3 * t + 1] = make_float4(v.y, v.z, w.x, w.y); sF[3 * t + 2] = make_float4(w.z, u.w, v.w, w.w);
-    sEps[t] = a.dir_eps[t];
+  // The two large tables arrive by bulk copies (cp.async.bulk, the TMA's linear form) that one thread issues and that signal an
+  // mbarrier with their byte count; both lie in global memory exactly as they lie here (light frames: written by the
+  // rasteriser; environment pairs: by texel_csr_kernel).  The small tables are staged by the threads meanwhile.
+  __shared__ __align__(8) unsigned long long s_bar;
+  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&s_bar);
+  const uint32_t bytesF = (uint32_t)K * 48u, bytesE = (uint32_t)((ne + 1) >> 1) * 48u;
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(1u) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytesF + bytesE) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"((uint32_t)__cvta_generic_to_shared(sF)), "l"(a.frames + 2), "r"(bytesF), "r"(bar) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"((uint32_t)__cvta_generic_to_shared(sE)), "l"(a.env_pairs), "r"(bytesE), "r"(bar) : "memory");
   }
-  for (int t = threadIdx.x; t < ((ne + 1) & ~1); t += blockDim.x) {
-    float4 wi = make_float4(0.f, 0.f, 1.f, 0.f), LA = make_float4(0.f, 0.f, 0.f, 0.f);       // padding of an odd list: adds nothing
-    if (t < ne) {
-      const int k = IDENT ? t : (int)a.tex_list[t];
-      wi = reinterpret_cast<const float4*>(a.env_table)[2 * k]; LA = reinterpret_cast<const float4*>(a.env_table)[2 * k + 1];
-    }
-    float* e = reinterpret_cast<float*>(sE + 3 * (t >> 1)) + (t & 1);
-    e[0] = wi.x; e[2] = wi.y; e[4] = wi.z; e[6] = LA.x; e[8] = LA.y; e[10] = LA.z;
-  }
+  for (int t = threadIdx.x; t < K; t += blockDim.x) sEps[t] = a.dir_eps[t];
   if (!IDENT) {
     for (int t = threadIdx.x; t <= K; t += blockDim.x) sStart[t] = a.dir_start[t];
     for (int t = threadIdx.x; t < ne + 2; t += blockDim.x) sTexD[t] = t < ne ? a.tex_dir[t] : (unsigned short)0;
   }
   const float4 h0 = a.frames[0], h1 = a.frames[1];
   if ((threadIdx.x & (VS_TEAM_THREADS - 1)) == 0) s_ticket[0][threadIdx.x / VS_TEAM_THREADS] = atomicAdd(a.counter, 1u);   // the team's first group
-  __syncthreads();
+  __syncthreads();                                                                // s_bar initialised, small tables staged
+  {
+    uint32_t done = 0;
+    while (!done)
+      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                   : "=r"(done) : "r"(bar), "r"(0u) : "memory");
+  }
   const float cx = h0.x, cy = h0.y, cz = h0.z, hR = h0.w, bt = h1.x, bw = h1.y, slope_max = h1.z;
   const int lane = threadIdx.x & 31, team = threadIdx.x / VS_TEAM_THREADS, tw = (threadIdx.x >> 5) & (VS_TEAM_WARPS - 1);
   const bool team_lead = (threadIdx.x & (VS_TEAM_THREADS - 1)) == 0;
@@ -392,7 +414,7 @@ cudaError_t rga_launch_front_compact(rga_avatar* av, int words, float3 cam, cuda
 // side stream: texels by direction (needs the environment table)
 cudaError_t rga_launch_texel_csr(rga_avatar* av, const rga_env* env, const rga_vis_params* vis, cudaStream_t s) {
   texel_csr_kernel<<<1, 1024, 0, s>>>(env->rows * env->cols, vis->n_dirs, env->texel_to_dir, av->env_table, vis->dirs, av->dir_start, av->tex_list,
-                                      av->tex_dir, av->dir_eps);
+                                      av->tex_dir, av->dir_eps, av->env_pairs);
   rga_prof_mark(av, "texel_csr", s);
   av->launches += 1;
   return cudaGetLastError();
@@ -403,7 +425,7 @@ cudaError_t rga_launch_vis_shade(rga_avatar* av, const rga_vis_params* vis, cons
   if (teams == 0) return cudaErrorInvalidConfiguration;
   VsArgs a;
   a.K = K; a.R = vis->res; a.ne = ne; a.words = (K + 31) / 32;
-  a.frames = reinterpret_cast<const float4*>(av->frames); a.env_table = av->env_table;
+  a.frames = reinterpret_cast<const float4*>(av->frames); a.env_table = av->env_table; a.env_pairs = av->env_pairs;
   a.dir_start = av->dir_start; a.tex_list = av->tex_list; a.tex_dir = av->tex_dir; a.dir_eps = av->dir_eps; a.zmap = av->zmap;
   a.front_list = av->front_list; a.n_front = av->n_front;
   a.g_posed = av->g_posed; a.g_nposed = av->g_nposed; a.g_static = av->g_static;
