@@ -99,6 +99,7 @@ struct RasterCtx {
   const float4* v_posed; const unsigned long long* faces_packed;
   unsigned* sz32; unsigned long long* sz64;
   const float* zf;             // shared memory: window centre (3) and the depth row of the light frame wn (3)
+  const float* sZ;             // shared memory: depth of every vertex for this direction (with the table in shared memory), or NULL
 };
 
 // pixel box of a triangle given its packed corners, clipped to the map and the band; returns the sample count
@@ -135,7 +136,6 @@ __device__ __forceinline__ void raster_depth(const RasterCtx& c, const RasterWar
   const unsigned t = q.x & 0xffffffu, mask = (q.x >> 24) & 0xfu;
   int i0, i1, i2;
   face_unpack(__ldg(c.faces_packed + t), i0, i1, i2);
-  const float4 a = __ldg(c.v_posed + i0), b = __ldg(c.v_posed + i1), e = __ldg(c.v_posed + i2);
   // a tall run (down a column) was sampled with x and y exchanged: exchange them here too (a 16-bit rotation of the packed
   // corner); edge functions and area both change sign under the exchange, so e1 / area and e2 / area are unchanged
   const bool tall = (q.x >> 28) & 1u;
@@ -145,10 +145,15 @@ __device__ __forceinline__ void raster_depth(const RasterCtx& c, const RasterWar
   const int x0 = P0 & 0xffff, y0 = P0 >> 16, x1 = P1 & 0xffff, y1 = P1 >> 16, x2 = P2 & 0xffff, y2 = P2 >> 16;
   // z = fma(wn.z, d.z, fma(wn.y, d.y, fma(wn.x, d.x, 0.5))): the frame is read from shared memory (kept in registers it
   // cost the sampling loop 20 registers it never uses)
-  const float cx = c.zf[0], cy = c.zf[1], cz = c.zf[2], wnx = c.zf[3], wny = c.zf[4], wnz = c.zf[5];
-  const float z0 = __fmaf_rn(wnz, a.z - cz, __fmaf_rn(wny, a.y - cy, __fmaf_rn(wnx, a.x - cx, 0.5f)));
-  const float z1 = __fmaf_rn(wnz, b.z - cz, __fmaf_rn(wny, b.y - cy, __fmaf_rn(wnx, b.x - cx, 0.5f)));
-  const float z2 = __fmaf_rn(wnz, e.z - cz, __fmaf_rn(wny, e.y - cy, __fmaf_rn(wnx, e.x - cx, 0.5f)));
+  float z0, z1, z2;
+  if (c.sZ) { z0 = c.sZ[i0]; z1 = c.sZ[i1]; z2 = c.sZ[i2]; }          // projected once per vertex in phase A (same chain)
+  else {
+    const float4 a = __ldg(c.v_posed + i0), b = __ldg(c.v_posed + i1), e = __ldg(c.v_posed + i2);
+    const float cx = c.zf[0], cy = c.zf[1], cz = c.zf[2], wnx = c.zf[3], wny = c.zf[4], wnz = c.zf[5];
+    z0 = __fmaf_rn(wnz, a.z - cz, __fmaf_rn(wny, a.y - cy, __fmaf_rn(wnx, a.x - cx, 0.5f)));
+    z1 = __fmaf_rn(wnz, b.z - cz, __fmaf_rn(wny, b.y - cy, __fmaf_rn(wnx, b.x - cx, 0.5f)));
+    z2 = __fmaf_rn(wnz, e.z - cz, __fmaf_rn(wny, e.y - cy, __fmaf_rn(wnx, e.x - cx, 0.5f)));
+  }
   const int pstep = tall ? c.R : 1;                                 // the run goes down a column (pixel stride R) or along a row
   if (!(q.x >> 31)) {
     const int area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0);
@@ -340,7 +345,7 @@ __device__ __forceinline__ int raster_single(const RasterCtx& c, RasterWarp* w, 
 }
 
 template <bool WITH_ID, bool BINNED, bool GTAB>
-__global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
+__global__ void __launch_bounds__(896, 1) vis_raster_kernel(int nf, int nv, int R, int band_rows, int n_bands, int n_units,
     int tail_first, int split,
     const float4* __restrict__ v_posed, const unsigned long long* __restrict__ faces_packed, const float* __restrict__ dirs,
     const float* __restrict__ window, unsigned* __restrict__ zmap, int* __restrict__ idmap,
@@ -350,7 +355,7 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
   __shared__ int s_next;
   __shared__ unsigned s_bin_cnt[RAST_MAX_BANDS];
   __shared__ float s_zf[8];
-  // layout: [RasterWarp x warps][map band_rows*R*(4|8)][sXY nv*4][svert (WITH_ID)]
+  // layout: [RasterWarp x warps][map band_rows*R*(4|8)][sXY nv*4][sZ nv*4][svert (WITH_ID)]
   const int nthreads = blockDim.x, nwarps = nthreads >> 5;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   RasterWarp* w = reinterpret_cast<RasterWarp*>(smem_raw) + warp;
@@ -361,7 +366,8 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
   // snapped vertex coordinates: shared memory, or (large meshes) this CTA's slice of an L2-resident scratch buffer
   // (a compile-time choice: with a run-time one every gather of the common shared-memory case becomes a generic load)
   unsigned* sXY = GTAB ? sxy_scratch + (size_t)blockIdx.x * nv : reinterpret_cast<unsigned*>(mp + map_bytes);
-  unsigned* svert = reinterpret_cast<unsigned*>(mp + map_bytes) + (GTAB ? 0 : nv);
+  float* sZ = GTAB ? nullptr : reinterpret_cast<float*>(mp + map_bytes) + nv;      // vertex depths, beside the table in shared memory
+  unsigned* svert = reinterpret_cast<unsigned*>(mp + map_bytes) + (GTAB ? 0 : 2 * nv);
   const int nv_words = (nv + 31) >> 5;
 
   // Work slots: units [0, tail_first) one CTA each; the units of the last, partial round of the persistent grid are cut
@@ -421,13 +427,14 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
       light_project_xy(a.x - W.cx, a.y - W.cy, a.z - W.cz, W, F, px, py);
       const int X = min(max(__float2int_rn(px * 256.0f), 0), 65535), Y = min(max(__float2int_rn(py * 256.0f), 0), 65535);
       sXY[v] = (unsigned)X | ((unsigned)Y << 16);
+      if (!GTAB) sZ[v] = __fmaf_rn(F.wn[2], a.z - W.cz, __fmaf_rn(F.wn[1], a.y - W.cy, __fmaf_rn(F.wn[0], a.x - W.cx, 0.5f)));
     }
     }
     __syncthreads();
 
     RasterCtx c;
     c.R = R; c.row0 = row0; c.rows = rows; c.sXY = sXY; c.v_posed = v_posed; c.faces_packed = faces_packed;
-    c.sz32 = sz32; c.sz64 = sz64; c.zf = s_zf;
+    c.sz32 = sz32; c.sz64 = sz64; c.zf = s_zf; c.sZ = sZ;
     // B1. triangles: one per lane, 32 per warp fetched dynamically; non-empty boxes queued
     int qn = 0, qsn = 0, q2n = 0;                           // warp-uniform queue fills
     // Binned maps (B1 only fills the band lists): the NEXT batch is drawn from the counter and its faces are requested before the
@@ -593,7 +600,10 @@ __global__ void __launch_bounds__(1024, 1) vis_raster_kernel(int nf, int nv, int
   }
 }
 
-// shared-memory plan: picks the CTA size (1024 / 512 / 256 threads) that minimises bands / warps; returns bytes.
+// shared-memory plan: picks the CTA size (896 / 448 / 224 threads) that minimises bands / warps; returns bytes.
+// 896 threads = 28 warps at 72 registers: the kernel needs 72 without spilling, and 1,024 threads cap it at 64 (measured at
+// config 1 / 2 / 4: 1,024 threads 133.4 / 603 / 1,141 us, 896: 131.7 / 597 / 1,132 us, 768 at 80 registers: 135 / 630 / 1,184 us,
+// 640 at 90: 145 / 652 / 1,221 us).
 // *sxy_global = 1: the 4-byte-per-vertex table of snapped coordinates does not fit beside a useful band of the map (meshes
 // beyond about 45k vertices) and lives in an L2-resident scratch buffer instead -- same kernel, slower gathers.
 static size_t raster_plan(int res, int with_id, int n_verts, bool table_in_smem, int* band_rows, int* threads) {
@@ -601,8 +611,8 @@ static size_t raster_plan(int res, int with_id, int n_verts, bool table_in_smem,
   const size_t per_row = (size_t)res * (with_id ? 8 : 4);
   size_t best = 0; double best_score = 1e30;
   *band_rows = 0; *threads = 0;
-  for (int th = 1024; th >= 256; th >>= 1) {
-    const size_t fixed = (size_t)(th / 32) * sizeof(RasterWarp) + (table_in_smem ? (size_t)n_verts * 4 : 0) +
+  for (int th = 896; th >= 224; th >>= 1) {
+    const size_t fixed = (size_t)(th / 32) * sizeof(RasterWarp) + (table_in_smem ? (size_t)n_verts * 8 : 0) +
                          (with_id ? (size_t)((n_verts + 31) / 32) * 4 : 0) + 32;
     if (fixed + per_row > budget) continue;
     int rows = (int)((budget - fixed) / per_row);
