@@ -35,11 +35,11 @@ def main():
         st = cb["single_thread"]
         print("| oracle, 1 thread | %.3f frames/s (%s) |" % (st["value"], ", ".join("%s %.3f s" % kv for kv in st["stage_s"].items())))
     print()
-    print("Per-kernel roofline of the headline frame (`roofline` list; CUDA-event time per kernel, one stream):")
+    print("Per-kernel roofline of the headline frame (`roofline_kernels`; `roofline` is its first row; CUDA-event time per kernel, one stream):")
     print()
     print("| kernel | stage | bound | time us | units | work per unit | achieved | peak (measured) | frac | DRAM MB (ncu) | issue slots busy |")
     print("|---|---|---|---|---|---|---|---|---|---|---|")
-    for r in d["roofline"]:
+    for r in (d.get("roofline_kernels") or d["roofline"]):
         unit = r.get("unit") or ""
         wpu = r.get("flop_eq_per_unit")
         if wpu is None and r.get("bytes_per_launch") and r.get("units_per_launch"):
