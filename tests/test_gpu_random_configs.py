@@ -15,7 +15,9 @@ pytestmark = pytest.mark.gpu
 FLAG_PER_PAIR = 2e-5
 
 
-@pytest.mark.parametrize("seed", list(range(24)))
+# seed 9489 (found by a 11,600-seed run): a light almost exactly opposite the viewer, |w_i + w_o| = 0.004 -- the stand-alone shading
+# kernel formed |w_i + w_o|^2 as 2 + 2 w_o.w_i there and lost the half vector to cancellation (6e-3 in the radiance)
+@pytest.mark.parametrize("seed", list(range(24)) + [9489])
 def test_random_configuration(seed):
     import torch
     from oracle import oracle as orc
