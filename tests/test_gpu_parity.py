@@ -634,6 +634,47 @@ def test_vertex_normals_from_the_geometry_when_none_are_passed():
     rga.avatar_free(h)
 
 
+def test_knn_ties_on_a_lattice_with_duplicate_vertices():
+    # Exact distance ties everywhere: vertices on an integer lattice, every eighth one duplicated (seam vertices of real meshes),
+    # Gaussians on lattice points, edge midpoints and cell centres.  The neighbour sets must be the oracle's (nearest first,
+    # equal distances by ascending vertex index: the stable-argsort rule pinned in test_oracle_pins.py), and so must the Eq.1
+    # weights -- both for the brute-force S_v kernel and for the uniform-grid S_g kernel, and again after gaussians_update.
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    g = np.arange(6, dtype=np.float32)
+    lat = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    v = np.concatenate([lat, lat[::8]]).astype(np.float32)                     # 216 + 27 duplicates
+    nv = len(v)
+    f = np.stack([np.arange(nv - 2), np.arange(1, nv - 1), np.arange(2, nv)], 1).astype(np.int32)   # any valid faces
+    rs = np.random.default_rng(4)
+    pts = [lat[rs.integers(0, len(lat), 300)],                                   # on a vertex: distance 0, then six ties at 1
+           lat[rs.integers(0, len(lat), 300)] + np.array([0.5, 0, 0], np.float32),   # edge midpoint: two ties at 0.25
+           np.clip(lat[rs.integers(0, len(lat), 300)], 0, 4) + 0.5]                  # cell centre: eight ties at 0.75
+    gp = np.concatenate(pts).astype(np.float32)
+    small = workloads.make(0)
+    inp = dict(small)
+    ng = len(gp)
+    inp.update(vert_pos=v, faces=f, vert_normal=np.tile(np.array([[0, 0, 1.0]], np.float32), (nv, 1)), vert_disp=None,
+               vert_skin_w=np.ascontiguousarray(np.tile(small["vert_skin_w"][:1], (nv, 1))),
+               vert_albedo=rs.uniform(0, 1, (nv, 3)).astype(np.float32), vert_rough=rs.uniform(0.1, 1, nv).astype(np.float32),
+               vert_spec=rs.uniform(0, 1, nv).astype(np.float32), gauss_pos=gp,
+               gauss_quat=np.tile(np.array([[1, 0, 0, 0]], np.float32), (ng, 1)), gauss_scale=np.full((ng, 3), 0.01, np.float32),
+               gauss_opacity=np.full(ng, 0.5, np.float32))
+    oav = orc.avatar_load(inp)
+    h = rga.avatar_load(inp, 64, 64, 16, 64, 128)
+    rd = lambda n: rga.rga_read_buffer(h, n)
+    assert np.array_equal(rd("KNN_V").reshape(nv, -1), oav["knn_v"]), "S_v with ties"
+    assert np.array_equal(rd("KNN_G").reshape(ng, -1), oav["knn_g"]), "S_g with ties"
+    assert np.array_equal(rd("UBAR_G").reshape(ng, -1), oav["ubar_g"]), "Eq.1 weights with ties and zero distances"
+    gp2 = np.ascontiguousarray(gp[::-1] + np.array([0, 0.5, 0], np.float32))
+    rga.gaussians_update(h, torch.as_tensor(gp2).cuda())
+    inp2 = dict(inp); inp2["gauss_pos"] = gp2
+    oav2 = orc.avatar_load(inp2)
+    assert np.array_equal(rd("KNN_G").reshape(ng, -1), oav2["knn_g"]) and np.array_equal(rd("UBAR_G").reshape(ng, -1), oav2["ubar_g"])
+    rga.avatar_free(h)
+
+
 def test_displacement_mlp_then_gaussians_update_then_static():
     # gaussians_update after displacement_mlp must keep the network's displacement (re-interpolated over the NEW
     # neighbour sets), and displacement_static must restore the load-time table -- each state equals a fresh oracle load
