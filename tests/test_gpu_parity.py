@@ -634,6 +634,34 @@ def test_vertex_normals_from_the_geometry_when_none_are_passed():
     rga.avatar_free(h)
 
 
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_degenerate_and_repeated_faces(vis_mode):
+    # faces that name a vertex twice or three times, faces of three collinear vertices (zero snapped area: skipped by the
+    # contract), and one face listed twice (equal depth everywhere: the lower triangle id wins in the id map) -- depth maps,
+    # id maps, visibility and the frame must equal the oracle's, and computed normals must survive the zero cross products
+    from oracle import oracle as orc
+    from parity_util import compare_all, run_gpu
+    inp = workloads.make(0)
+    f = inp["faces"]
+    v = inp["vert_pos"]
+    mid = (0.5 * (v[f[0, 0]] + v[f[0, 1]])).astype(np.float32)                 # a vertex on an edge: (a, mid, b) is collinear
+    nv = len(v)
+    extra_v = mid[None, :]
+    extra_f = np.array([[0, 0, 1], [2, 2, 2], [f[0, 0], nv, f[0, 1]], f[5], f[5], [3, 4, 3]], np.int32)
+    inp["vert_pos"] = np.concatenate([v, extra_v]).astype(np.float32)
+    for k in ("vert_skin_w", "vert_albedo", "vert_rough", "vert_spec", "vert_disp"):
+        if inp.get(k) is not None:
+            inp[k] = np.ascontiguousarray(np.concatenate([inp[k], inp[k][f[0, 0]][None]]))
+    inp["faces"] = np.ascontiguousarray(np.concatenate([f, extra_f]), np.int32)
+    inp["vert_normal"] = None                                                   # from the geometry, degenerate faces included
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=vis_mode)
+    av, img = run_gpu(inp, vis_mode=vis_mode)
+    assert np.array_equal(av.read("VERT_NORMAL").reshape(-1, 3), orc_av["vert_normal"])
+    print(compare_all(inp, av, img, orc_av, o, vis_mode))
+    av.close()
+
+
 def test_knn_ties_on_a_lattice_with_duplicate_vertices():
     # Exact distance ties everywhere: vertices on an integer lattice, every eighth one duplicated (seam vertices of real meshes),
     # Gaussians on lattice points, edge midpoints and cell centres.  The neighbour sets must be the oracle's (nearest first,
