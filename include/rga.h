@@ -175,7 +175,9 @@ RGA_API rga_status splat_backward(rga_avatar* av, const rga_camera* cam, const f
  * derivative 0 at and beyond the clamp limits (reading A33), so a Gaussian whose radiance is 0 (hidden,
  * facing away) or >= 1 in a channel gets no gradient from that channel.
  * Outputs are DEVICE buffers, each may be NULL: out_dalbedo [n_gauss][3], out_drough [n_gauss], out_dspec [n_gauss],
- * out_dnormal [n_gauss][3], out_dpos [n_gauss][3], out_denv [rows][cols][3].  Enqueue-only. */
+ * out_dnormal [n_gauss][3], out_dpos [n_gauss][3], out_denv [rows][cols][3].  Environment maps of more than 5,030 texels
+ * (46 bytes per texel of shared memory) are refused with RGA_ERR_INVALID_ARG; the forward calls take up to 6,595.
+ * Enqueue-only. */
 RGA_API rga_status shade_backward(rga_avatar* av, const rga_env* env, const float cam_pos[3], const float* dL_dcolor,
                                   float* out_dalbedo, float* out_drough, float* out_dspec, float* out_dnormal, float* out_dpos,
                                   float* out_denv, void* stream);
@@ -289,7 +291,11 @@ RGA_API rga_status splat_attribute(rga_avatar* av, const rga_camera* cam, const 
  * observes the whole frame in order; the call can be captured into a CUDA graph.
  * One difference in the intermediates: this call knows the camera when it tests visibility, so in mode 0 the depth test
  * is not run for Gaussians that face away from the camera (their opacity is 0 and shade_gaussians skips
- * them by the same test); their RGA_BUF_VISBITS words are 0.  Radiance, colour and image are unchanged.  To shade the
+ * them by the same test); their RGA_BUF_VISBITS words are 0.  Where the light-frame and environment tables fit shared memory
+ * (n_dirs <= 2,048, rows * cols <= 4,096 and 48 n_dirs + 24 rows * cols + 13 KB within 226 KB) depth test and shading run as one
+ * kernel that also leaves out the directions none of whose texels can light the Gaussian (n . w_i <= 0 for all of them); those
+ * bits are 0 as well.  Larger tables fall back to the two kernels of the separate calls, which test every direction of a
+ * camera-facing Gaussian.  Radiance, colour and image are unchanged.  To shade the
  * same pose from ANOTHER camera afterwards, call visibility_raster first (shade_gaussians returns RGA_ERR_STATE if not). */
 RGA_API rga_status rga_render_frame(rga_avatar* av, const float* bone_mats, const rga_vis_params* vis, const rga_env* env,
                                     const float cam_pos[3], const rga_camera* cam, const float bg[3], float* out_image,

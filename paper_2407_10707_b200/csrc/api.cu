@@ -16,6 +16,7 @@ struct NvtxRange {
 #include "rga_internal.h"
 
 int rga_shade_init_attributes(int max_env);
+int rga_shade_backward_max_texels();
 int rga_vis_init_attributes();
 int rga_composite_init_attributes();
 int rga_mlp_init_attributes();
@@ -23,6 +24,8 @@ int rga_mlp_init_attributes();
 static thread_local char g_err[512] = "";
 static rga_status fail(rga_status st, const char* fmt, ...) {
   va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof g_err, fmt, ap); va_end(ap);
+  // a CUDA error this call ran into has been reported: do not leave it for the next call's cudaGetLastError to trip over
+  if (st == RGA_ERR_CUDA || st == RGA_ERR_OOM) (void)cudaGetLastError();
   return st;
 }
 #define CU(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return fail(e_ == cudaErrorMemoryAllocation ? RGA_ERR_OOM : RGA_ERR_CUDA, \
@@ -345,6 +348,9 @@ extern "C" rga_status shade_backward(rga_avatar* av, const rga_env* env, const f
     return fail(RGA_ERR_STATE, "shade_backward: this pose's visibility was computed for another environment-map layout (rga_render_frame)");
   if (env->rows < 1 || env->cols < 1 || env->rows * env->cols > av->max_env || !(env->gamma > 0.f))
     return fail(RGA_ERR_INVALID_ARG, "shade_backward: env size/gamma out of range");
+  if (env->rows * env->cols > rga_shade_backward_max_texels())
+    return fail(RGA_ERR_INVALID_ARG, "shade_backward: %d environment texels are above the %d this kernel can stage in shared memory (46 bytes per "
+                "texel; the forward calls take up to %d)", env->rows * env->cols, rga_shade_backward_max_texels(), (int)((227 * 1024 - 8 * 1024) / 34));
   if (env->use_visibility && !env->texel_to_dir && env->rows * env->cols != av->vis_dirs)
     return fail(RGA_ERR_INVALID_ARG, "shade_backward: identity texel_to_dir needs rows*cols == n_dirs");
   cudaStream_t s = (cudaStream_t)stream;

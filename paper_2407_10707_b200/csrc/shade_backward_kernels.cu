@@ -220,7 +220,11 @@ cudaError_t rga_launch_shade_backward(rga_avatar* av, const rga_env* env, float3
   return cudaGetLastError();
 }
 
+// the backward kernels stage 46 bytes per environment texel: fewer texels fit than in the forward kernels (34 bytes)
+int rga_shade_backward_max_texels() { return (int)((227 * 1024 - 1024) / 46); }
+
 int rga_shade_backward_init_attributes(int max_env) {
+  if (max_env > rga_shade_backward_max_texels()) max_env = rga_shade_backward_max_texels();   // larger maps: forward only (shade_backward refuses them)
   const size_t smem = (size_t)max_env * 46;
   cudaError_t e = cudaSuccess;
   if (smem > 48 * 1024) {

@@ -39,7 +39,7 @@ def facing_split(inp, o, cam_pos=None):
     return f > 1e-3, f < -1e-3
 
 
-def check_frame_visbits(inp, o, vb, cam_pos=None):
+def check_frame_visbits(inp, o, vb, cam_pos=None, fused=True):
     """Visibility words written by rga_render_frame's fused depth-test + shading kernel (mode 0).  It tests a (Gaussian,
     direction) pair only when Eq.2 can read the result: the Gaussian faces the camera and the direction d
     has a texel k with w_i^k . n > 0 (v_g[k] max(0, w_i . n)), decided conservatively as
@@ -64,13 +64,14 @@ def check_frame_visbits(inp, o, vb, cam_pos=None):
         must = kept[a:b, None] & (cs > -eps[None, :] + 1e-5)
         never = cs < -eps[None, :] - 1e-5
         assert np.array_equal(got[a:b][must], ref[a:b][must]), "visibility bits of tested (Gaussian, direction) pairs"
-        assert not got[a:b][never].any(), "visibility bits of directions Eq.2 cannot read"
+        if fused:                                                         # the two-kernel fallback (tables beyond shared memory) tests every direction
+            assert not got[a:b][never].any(), "visibility bits of directions Eq.2 cannot read"
         n_checked += int(must.sum())
     assert n_checked > 0
     return n_checked
 
 
-def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=None, frame_call=False, flag_per_pair=None):
+def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=None, frame_call=False, flag_per_pair=None, fused=True):
     """Assert stage-by-stage parity.  `o` is oracle.render_frame's dict, `orc_av` oracle.avatar_load's.
     frame_call: the frame came from rga_render_frame, whose mode-0 depth test skips Gaussians that face away from the
     camera (their bits are never read): visibility bits are compared on the kept Gaussians and must be 0 on the culled."""
@@ -107,7 +108,7 @@ def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=N
         if vis_mode == 0:
             vb = rd("VISBITS").reshape(ng, words)
             if frame_call:
-                rep["visbits_checked"] = check_frame_visbits(inp, o, vb)
+                rep["visbits_checked"] = check_frame_visbits(inp, o, vb, fused=fused)
             else:
                 assert eq(vb, o["visbits"]), "visbits"
         else:

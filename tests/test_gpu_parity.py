@@ -662,6 +662,44 @@ def test_degenerate_and_repeated_faces(vis_mode):
     av.close()
 
 
+@pytest.mark.parametrize("dirs,env_rc,fused", [((32, 64), (32, 64), True), ((32, 64), (64, 64), False), ((33, 64), (66, 96), False)])
+def test_largest_direction_sets_and_environment_maps(dirs, env_rc, fused):
+    # the fused kernel's limits (2,048 directions with an identity map: tables fill shared memory), just beyond them (4,096
+    # texels on 2,048 directions: the two-kernel fallback, which tests every direction of a camera-facing Gaussian) and an
+    # environment map near the forward kernels' own limit (6,336 of 6,595 texels; more than shade_backward takes, which says so)
+    import torch
+    from oracle import oracle as orc
+    from paper_2407_10707_b200 import binding as rga
+    from parity_util import compare_all, run_gpu
+    inp = workloads.make(0, n_gauss=1500)
+    (Rd, Cd), (R, C) = dirs, env_rc
+    inp["vis_res"] = 32
+    inp["vis_dirs"] = workloads.latlong_dirs(Rd, Cd)
+    inp["texel_to_dir"] = workloads.texel_to_dir((R, C), (Rd, Cd))
+    inp["env"] = np.ascontiguousarray(np.random.default_rng(1).uniform(0, 2, (1, R, C, 3)), np.float32)
+    inp["env_rows"], inp["env_cols"] = R, C
+    orc_av = orc.avatar_load(inp)
+    o = orc.render_frame(orc_av, inp, vis_mode=0)
+    av, img = run_gpu(inp, vis_mode=0)
+    compare_all(inp, av, img, orc_av, o, 0)
+    if R * C > 5030:
+        env = torch.as_tensor(inp["env"][0]).cuda()
+        with pytest.raises(rga.RgaError) as e:
+            rga.shade_backward(av.h, env, inp["cam_pos"], torch.zeros((1500, 3), device="cuda"), texel_to_dir=torch.as_tensor(inp["texel_to_dir"]).cuda(),
+                               gamma=inp["gamma"], use_visibility=True, out_denv=torch.zeros_like(env))
+        assert "5030" in str(e.value)
+    av.close()
+    cam = inp["camera"]; W, H = cam["width"], cam["height"]
+    av = rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=Rd * Cd, max_vis_res=32, max_env_texels=R * C)
+    im = torch.empty((H, W, 3), dtype=torch.float32, device="cuda")
+    av.render(torch.as_tensor(inp["bone_mats"][0]).cuda(), torch.as_tensor(inp["vis_dirs"]).cuda(), 32, torch.as_tensor(inp["env"][0]).cuda(),
+              torch.as_tensor(inp["texel_to_dir"]).cuda(), inp["cam_pos"], cam, inp["bg"], im, vis_mode=0, gamma=inp["gamma"],
+              bias=(inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"]))
+    rga.rga_check(av.h)
+    print(compare_all(inp, av, im.cpu().numpy(), orc_av, o, 0, frame_call=True, fused=fused))
+    av.close()
+
+
 def test_knn_ties_on_a_lattice_with_duplicate_vertices():
     # Exact distance ties everywhere: vertices on an integer lattice, every eighth one duplicated (seam vertices of real meshes),
     # Gaussians on lattice points, edge midpoints and cell centres.  The neighbour sets must be the oracle's (nearest first,
