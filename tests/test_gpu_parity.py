@@ -700,6 +700,41 @@ def test_largest_direction_sets_and_environment_maps(dirs, env_rc, fused):
     av.close()
 
 
+def test_two_avatars_on_two_streams_do_not_disturb_each_other():
+    # frames of two handles issued concurrently on two streams (bench.py's frames_in_flight_fps does this for throughput) are
+    # bit-identical to the same frames rendered one after the other: no state is shared between handles
+    import torch
+    from paper_2407_10707_b200 import binding as rga
+    inp = workloads.make(3, n_gauss=20_000)
+    cam = inp["camera"]; W, H = cam["width"], cam["height"]
+    dirs = torch.as_tensor(inp["vis_dirs"]).cuda(); t2d = torch.as_tensor(inp["texel_to_dir"]).cuda()
+    bones = torch.as_tensor(inp["bone_mats"]).cuda(); envs = torch.as_tensor(inp["env"]).cuda()
+    avs = [rga.Avatar(inp, max_width=W, max_height=H, max_vis_dirs=len(inp["vis_dirs"]), max_vis_res=inp["vis_res"],
+                      max_env_texels=inp["env_rows"] * inp["env_cols"]) for _ in range(2)]
+    imgs = [torch.empty((H, W, 3), dtype=torch.float32, device="cuda") for _ in range(2)]
+
+    def frame(k, t):
+        avs[k].render(bones[t], dirs, inp["vis_res"], envs[int(inp["env_of_frame"][t])], t2d, inp["cam_pos"], cam, inp["bg"], imgs[k],
+                      vis_mode=0, gamma=inp["gamma"], bias=(inp["depth_bias_texels"], inp["depth_bias_world"], inp["slope_max"]))
+    poses = [(0, 31), (7, 40), (13, 63)]
+    ref = []
+    for ta, tb in poses:
+        frame(0, ta); frame(1, tb); torch.cuda.synchronize()
+        ref.append((imgs[0].clone(), imgs[1].clone()))
+    assert not torch.equal(ref[0][0], ref[0][1])
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for _ in range(5):
+        for i, (ta, tb) in enumerate(poses):
+            with torch.cuda.stream(streams[0]):
+                frame(0, ta)
+            with torch.cuda.stream(streams[1]):
+                frame(1, tb)
+            torch.cuda.synchronize()
+            assert torch.equal(imgs[0], ref[i][0]) and torch.equal(imgs[1], ref[i][1])
+    for a in avs:
+        rga.rga_check(a.h); a.close()
+
+
 def test_knn_ties_on_a_lattice_with_duplicate_vertices():
     # Exact distance ties everywhere: vertices on an integer lattice, every eighth one duplicated (seam vertices of real meshes),
     # Gaussians on lattice points, edge midpoints and cell centres.  The neighbour sets must be the oracle's (nearest first,
