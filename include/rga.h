@@ -32,6 +32,9 @@
  *    message.  Device-side capacity overflow (more (Gaussian,tile) duplicates than max_duplicates) sets a sticky
  *    device status word that rga_check() reads back; the frame's image is then undefined.
  *  - Calling a stage before its producer in the same pose returns RGA_ERR_STATE.
+ *  - Concurrency: an rga_avatar owns its scratch and its stage state, so calls on ONE handle must be ordered (one host thread
+ *    at a time, work enqueued on one stream at a time, or streams ordered by events).  Different handles share nothing and may
+ *    be used from different threads and streams at once (tests/test_gpu_parity.py renders two at once, bit-identical to serial).
  *  - Quaternions are (w,x,y,z).  World is z-up.  Camera looks down +z, x right, y down; image origin top-left;
  *    pixel (i,j) samples at (i+1/2, j+1/2).  Bone matrices are posed-global x inverse-bind, row-major 3x4.
  *  - There is no CPU fallback: without a CUDA device every entry point that computes returns RGA_ERR_CUDA.
