@@ -82,7 +82,9 @@ typedef struct {
   const float*   vert_skin_w;  /* dev [n_verts][n_bones] LBS weights w, rows sum to 1                */
   const float*   vert_disp;    /* dev [n_verts][3]  static average displacement or NULL = 0 */
   const float*   vert_albedo;  /* dev [n_verts][3]  a                                                */
-  const float*   vert_rough;   /* dev [n_verts]     gamma                                            */
+  const float*   vert_rough;   /* dev [n_verts]     gamma in (0, 1].  The radiance tolerance (2e-3 of max(1, L_o)) is met for
+                                  gamma >= 0.07; mirror-like values lose it to fp32 (gamma = 0.01: up to 4e-3 under a
+                                  strongly HDR map -- the half vector's tangential part is a difference of unit vectors) */
   const float*   vert_spec;    /* dev [n_verts]     specular tint p                                  */
   const float*   gauss_pos;    /* dev [n_gauss][3]  canonical x_g                                    */
   const float*   gauss_quat;   /* dev [n_gauss][4]  (w,x,y,z), any non-zero norm; NULL = interpolate vert_quat  */
