@@ -283,17 +283,40 @@ __device__ __forceinline__ float seg_alpha(const SegStage& st, int j, float fx, 
 __global__ void __launch_bounds__(CB, SEG_MINB) composite_segment_kernel(int W, int H, int TX, const unsigned* __restrict__ num_items,
     const unsigned* __restrict__ item_tab, const unsigned* __restrict__ seg_off, const uint2* __restrict__ ranges,
     const unsigned* __restrict__ vals, const float2* __restrict__ mu2d, const float4* __restrict__ conic_o,
-    const float4* __restrict__ color, float4* __restrict__ part, unsigned* __restrict__ part_last) {
+    const float4* __restrict__ color, float4* __restrict__ part, unsigned* __restrict__ part_last, unsigned* __restrict__ counter) {
   __shared__ SegStage st;
   __shared__ unsigned s_bm[CB / 32][RGA_SEG / 32];                  // per 8x4 pixel block (= warp): the entries whose box reaches it
+  __shared__ unsigned s_item;
   const unsigned n_items = *num_items;
-  for (unsigned item = blockIdx.x; item < n_items; item += gridDim.x) {
+  // Large frames (more than two items per CTA) draw their items from a counter: an item's cost differs several-fold with the
+  // number of entries that reach the tile's blocks, and with a fixed stride the slowest CTAs set the time (config 4: 344 ->
+  // 284 us, config 2: 107 -> 92 us).  The next ticket is drawn before the current item is worked on, so the atomic's round trip
+  // is hidden; every CTA draws one ticket beyond the items and the last one re-arms the counter.  With one or two items per
+  // CTA (config 1) the tickets only cost: 28.6 -> 33.5 us, so small frames keep the fixed stride.
+  const bool dynamic = n_items > 2u * gridDim.x;
+  unsigned next = blockIdx.x;
+  if (dynamic && threadIdx.x == 0) next = atomicAdd(counter, 1u);
+  for (;;) {
+    unsigned item = next;
+    if (dynamic) {
+      if (threadIdx.x == 0) s_item = next;
+      __syncthreads();                                                // also: the previous item's walk is done with `st`
+      item = s_item;
+      if (item >= n_items) {
+        if (threadIdx.x == 0 && item == n_items + gridDim.x - 1u) *counter = 0u;
+        break;
+      }
+      if (threadIdx.x == 0) next = atomicAdd(counter, 1u);
+    } else {
+      if (item >= n_items) break;
+      next = item + gridDim.x;
+      __syncthreads();
+    }
     const unsigned tile = item_tab[item];
     const unsigned seg = item - seg_off[tile];
     const uint2 rg = ranges[tile];
     const unsigned b0 = rg.x + seg * RGA_SEG;
     const int m = (int)min((unsigned)RGA_SEG, rg.y - b0);
-    __syncthreads();
     stage_segment(st, m, vals + b0, mu2d, conic_o, color);
     // Which entries can reach which of the tile's eight 8x4 pixel blocks: the staging thread of entry j tests its bounding box
     // against the eight block centres (pixel centres lie at +-3.5, +-1.5 around it) and the bits are transposed by ballots
@@ -552,7 +575,7 @@ cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStre
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, const float4* color, float* out, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
   composite_segment_kernel<<<av->num_sms * SEGMENT_GRID_MULT, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
-      av->ranges, av->vals[1], av->mu2d, av->conic_o, color, av->part, av->part_last);
+      av->ranges, av->vals[1], av->mu2d, av->conic_o, color, av->part, av->part_last, av->seg_counter);
   rga_prof_mark(av, "composite_segments", s);
   composite_resolve_kernel<<<dim3(TX, TY), CB, 0, s>>>(cam->width, cam->height, TX, (unsigned)av->max_dup, av->ranges, av->seg_off,
       av->part, av->part_last, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);

@@ -81,6 +81,7 @@ struct rga_avatar {
   unsigned* part_last;         // [items_cap][256] last contributing entry of the segment (1-based, 0 = none)
   long long items_cap;
   float* env_pairs;            // [ceil(max_env / 2)][12] environment rows in list order, pairs side by side (fused kernel's table image)
+  unsigned* seg_counter;       // [1] item tickets of composite_segment_kernel (zero between launches: the last CTA re-arms it)
   int* stop_seg;               // [pixels] segment in which the pixel's blend stops (-1: list exhausted)
   unsigned char* item_flag;    // [items_cap] work item has pixels to replay (cleared by the replay kernel)
   float* t_final; unsigned* n_contrib;
