@@ -74,7 +74,7 @@ extern "C" rga_status avatar_free(rga_avatar* av) {
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
                   av->radiance, av->color, av->attr_color, av->mu2d, av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->cursor, av->keys[0],
-                  av->keys[1], av->vals[0], av->num_dup, av->ranges, av->t_final, av->n_contrib, av->seg_off, av->num_items, av->item_tab, av->part, av->part_last, av->stop_seg, av->item_flag, av->seg_counter, av->env_pairs,
+                  av->keys[1], av->vals[0], av->num_dup, av->ranges, av->t_final, av->n_contrib, av->seg_off, av->num_items, av->item_tab, av->part, av->part_last, av->stop_seg, av->item_flag, av->item_desc, av->seg_counter, av->env_pairs,
                   av->status};
   for (void* p : ptrs) if (p) cudaFree(p);
   for (int i = 0; i < RGA_MAX_PROF; ++i) if (av->prof_ev[i]) cudaEventDestroy(av->prof_ev[i]);
@@ -150,7 +150,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->g_order, ng)); A(dalloc(&av->g_inv, ng)); A(dalloc(&av->gi_pos, 3 * ng)); A(dalloc(&av->bb_scratch, 8)); A(dalloc(&av->bb_dev, 8));
   A(dalloc(&av->num_dup, 1)); A(dalloc(&av->ranges, ntiles));
   av->items_cap = av->max_dup / RGA_SEG + (long long)ntiles + 1;
-  A(dalloc(&av->seg_off, ntiles + 1)); A(dalloc(&av->num_items, 1)); A(dalloc(&av->item_tab, (size_t)av->items_cap));
+  A(dalloc(&av->seg_off, ntiles + 1)); A(dalloc(&av->num_items, 1)); A(dalloc(&av->item_tab, (size_t)av->items_cap)); A(dalloc(&av->item_desc, (size_t)av->items_cap));
   A(dalloc(&av->part, (size_t)av->items_cap * 256)); A(dalloc(&av->part_last, (size_t)av->items_cap * 256));
   A(dalloc(&av->env_pairs, 12 * (((size_t)av->max_env + 1) / 2) + 4));
   A(dalloc(&av->seg_counter, 1)); A(cudaMemsetAsync(av->seg_counter, 0, sizeof(unsigned), s));

@@ -88,12 +88,16 @@ __device__ __forceinline__ void bitonic_sort(unsigned long long* buf, int n) {
 __device__ __forceinline__ void sort_tile(int tile, unsigned capacity, int scap, unsigned long long* s_keys,
     const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, unsigned long long* __restrict__ lkeys,
     unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ vals_int,
-    const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
+    const int* __restrict__ inv, unsigned* __restrict__ item_tab, uint2* __restrict__ item_desc) {
   uint2 rg = ranges[tile];
   rg.x = min(rg.x, capacity); rg.y = min(rg.y, capacity);
   const int n = (int)(rg.y - rg.x);
   const unsigned so = seg_off[tile];
-  for (int j = threadIdx.x; j < (n + RGA_SEG - 1) / RGA_SEG; j += SORT_THREADS) item_tab[so + j] = (unsigned)tile;
+  for (int j = threadIdx.x; j < (n + RGA_SEG - 1) / RGA_SEG; j += SORT_THREADS) {
+    item_tab[so + j] = (unsigned)tile;
+    // what the blend needs to know about the item, in one load: first list entry; tile | entries << 24
+    item_desc[so + j] = make_uint2(rg.x + (unsigned)j * RGA_SEG, (unsigned)tile | ((unsigned)min(RGA_SEG, n - j * RGA_SEG) << 24));
+  }
   unsigned long long* buf = lkeys + rg.x;
   if (n <= scap) {
     for (int i = threadIdx.x; i < n; i += SORT_THREADS) s_keys[i] = buf[i];
@@ -126,12 +130,16 @@ __device__ __forceinline__ void sort_tile(int tile, unsigned capacity, int scap,
 __device__ __forceinline__ void radix_sort_tile(int tile, unsigned capacity, int idx_bits, unsigned* s_hist /*[RADIX_WARPS][256]*/,
     unsigned* s_base /*[256]*/, int* s_flag, const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off,
     unsigned long long* __restrict__ lkeys, unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out,
-    unsigned* __restrict__ vals_int, const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
+    unsigned* __restrict__ vals_int, const int* __restrict__ inv, unsigned* __restrict__ item_tab, uint2* __restrict__ item_desc) {
   uint2 rg = ranges[tile];
   rg.x = min(rg.x, capacity); rg.y = min(rg.y, capacity);
   const int n = (int)(rg.y - rg.x);
   const unsigned so = seg_off[tile];
-  for (int j = threadIdx.x; j < (n + RGA_SEG - 1) / RGA_SEG; j += SORT_THREADS) item_tab[so + j] = (unsigned)tile;
+  for (int j = threadIdx.x; j < (n + RGA_SEG - 1) / RGA_SEG; j += SORT_THREADS) {
+    item_tab[so + j] = (unsigned)tile;
+    // what the blend needs to know about the item, in one load: first list entry; tile | entries << 24
+    item_desc[so + j] = make_uint2(rg.x + (unsigned)j * RGA_SEG, (unsigned)tile | ((unsigned)min(RGA_SEG, n - j * RGA_SEG) << 24));
+  }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   const int per = (((n + RADIX_WARPS - 1) / RADIX_WARPS) + 31) & ~31;          // whole batches per warp
@@ -225,7 +233,7 @@ __device__ __forceinline__ void radix_sort_tile(int tile, unsigned capacity, int
 __global__ void __launch_bounds__(SORT_THREADS) tile_sort_kernel(unsigned capacity, int scap, int idx_bits,
     const uint2* __restrict__ ranges, const unsigned* __restrict__ seg_off, unsigned long long* __restrict__ lkeys,
     unsigned long long* __restrict__ keys_out, unsigned* __restrict__ vals_out, unsigned* __restrict__ vals_int,
-    const int* __restrict__ inv, unsigned* __restrict__ item_tab) {
+    const int* __restrict__ inv, unsigned* __restrict__ item_tab, uint2* __restrict__ item_desc) {
   extern __shared__ __align__(16) unsigned long long s_keys[];                   // scap keys, or RADIX_WARPS x 256 counters
   __shared__ unsigned s_base[256];
   __shared__ int s_flag;
@@ -234,9 +242,9 @@ __global__ void __launch_bounds__(SORT_THREADS) tile_sort_kernel(unsigned capaci
   if (n == 0) return;
   if (n > (unsigned)scap)
     radix_sort_tile(blockIdx.x, capacity, idx_bits, reinterpret_cast<unsigned*>(s_keys), s_base, &s_flag, ranges, seg_off, lkeys, keys_out,
-                    vals_out, vals_int, inv, item_tab);
+                    vals_out, vals_int, inv, item_tab, item_desc);
   else
-    sort_tile(blockIdx.x, capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, vals_int, inv, item_tab);
+    sort_tile(blockIdx.x, capacity, scap, s_keys, ranges, seg_off, lkeys, keys_out, vals_out, vals_int, inv, item_tab, item_desc);
 }
 
 // Thread -> pixel of the 16x16 tile: a warp owns an 8x4 block of pixels (2 x 4 blocks per tile), so that a Gaussian
@@ -281,7 +289,7 @@ __device__ __forceinline__ float seg_alpha(const SegStage& st, int j, float fx, 
 #define SEG_MINB 8             // 8 CTAs per SM resident: caps the kernel at 32 registers (33.8 -> 32.9 us)
 #endif
 __global__ void __launch_bounds__(CB, SEG_MINB) composite_segment_kernel(int W, int H, int TX, const unsigned* __restrict__ num_items,
-    const unsigned* __restrict__ item_tab, const unsigned* __restrict__ seg_off, const uint2* __restrict__ ranges,
+    const uint2* __restrict__ item_desc,
     const unsigned* __restrict__ vals, const float2* __restrict__ mu2d, const float4* __restrict__ conic_o,
     const float4* __restrict__ color, float4* __restrict__ part, unsigned* __restrict__ part_last, unsigned* __restrict__ counter) {
   __shared__ SegStage st;
@@ -312,11 +320,9 @@ __global__ void __launch_bounds__(CB, SEG_MINB) composite_segment_kernel(int W, 
       next = item + gridDim.x;
       __syncthreads();
     }
-    const unsigned tile = item_tab[item];
-    const unsigned seg = item - seg_off[tile];
-    const uint2 rg = ranges[tile];
-    const unsigned b0 = rg.x + seg * RGA_SEG;
-    const int m = (int)min((unsigned)RGA_SEG, rg.y - b0);
+    const uint2 desc = item_desc[item];
+    const unsigned tile = desc.y & 0xffffffu, b0 = desc.x;
+    const int m = (int)(desc.y >> 24);
     stage_segment(st, m, vals + b0, mu2d, conic_o, color);
     // Which entries can reach which of the tile's eight 8x4 pixel blocks: the staging thread of entry j tests its bounding box
     // against the eight block centres (pixel centres lie at +-3.5, +-1.5 around it) and the bits are transposed by ballots
@@ -565,7 +571,7 @@ cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStre
   static_assert(SCAP_SMALL * 8 >= RADIX_WARPS * 256 * 4, "the radix histograms reuse the key buffer");
   int idx_bits = 1; while (idx_bits < 32 && (1ll << idx_bits) < (long long)av->n_gauss) ++idx_bits;
   tile_sort_kernel<<<ntiles, SORT_THREADS, SCAP_SMALL * 8, s>>>((unsigned)av->max_dup, SCAP_SMALL, idx_bits, av->ranges, av->seg_off, av->keys[0],
-                                                           av->keys[1], av->vals[0], av->vals[1], av->g_inv, av->item_tab);
+                                                           av->keys[1], av->vals[0], av->vals[1], av->g_inv, av->item_tab, av->item_desc);
   rga_prof_mark(av, "tile_sort", s);
   av->launches += 1;
   return cudaGetLastError();
@@ -574,8 +580,8 @@ cudaError_t rga_launch_tile_sort(rga_avatar* av, const rga_camera* cam, cudaStre
 // H10: blend (needs the sorted lists and the shaded colours)
 cudaError_t rga_launch_composite(rga_avatar* av, const rga_camera* cam, float3 bg, const float4* color, float* out, cudaStream_t s) {
   const int TX = (cam->width + RGA_TILE - 1) / RGA_TILE, TY = (cam->height + RGA_TILE - 1) / RGA_TILE;
-  composite_segment_kernel<<<av->num_sms * SEGMENT_GRID_MULT, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_tab, av->seg_off,
-      av->ranges, av->vals[1], av->mu2d, av->conic_o, color, av->part, av->part_last, av->seg_counter);
+  composite_segment_kernel<<<av->num_sms * SEGMENT_GRID_MULT, CB, 0, s>>>(cam->width, cam->height, TX, av->num_items, av->item_desc,
+      av->vals[1], av->mu2d, av->conic_o, color, av->part, av->part_last, av->seg_counter);
   rga_prof_mark(av, "composite_segments", s);
   composite_resolve_kernel<<<dim3(TX, TY), CB, 0, s>>>(cam->width, cam->height, TX, (unsigned)av->max_dup, av->ranges, av->seg_off,
       av->part, av->part_last, bg, out, av->t_final, av->n_contrib, av->stop_seg, av->item_flag);

@@ -77,6 +77,7 @@ struct rga_avatar {
   unsigned* seg_off;           // [tiles + 1] exclusive scan of ceil(n_t / RGA_SEG)
   unsigned* num_items;         // [1] number of (tile, segment) work items (device)
   unsigned* item_tab;          // [items_cap] tile of each work item
+  uint2* item_desc;            // [items_cap] (first list entry, tile | entries << 24) of each work item: all the blend needs, in one load
   float4* part;                // [items_cap][256] per-pixel partial (C, T) of each segment
   unsigned* part_last;         // [items_cap][256] last contributing entry of the segment (1-based, 0 = none)
   long long items_cap;
