@@ -17,7 +17,9 @@ FLAG_PER_PAIR = 2e-5
 
 # seed 9489 (found by a 11,600-seed run): a light almost exactly opposite the viewer, |w_i + w_o| = 0.004 -- the stand-alone shading
 # kernel formed |w_i + w_o|^2 as 2 + 2 w_o.w_i there and lost the half vector to cancellation (6e-3 in the radiance)
-@pytest.mark.parametrize("seed", list(range(24)) + [9489])
+# seeds 54952 and 56494 (an 18,256-seed run on the round's final build, no wrong output): ONE light direction that stands behind
+# every camera-facing Gaussian (nothing for the fused kernel to test: all its words must be 0), and a frame with 3 flagged pixels
+@pytest.mark.parametrize("seed", list(range(24)) + [9489, 54952, 56494])
 def test_random_configuration(seed):
     import torch
     from oracle import oracle as orc
