@@ -534,6 +534,9 @@ ORC void orc_tile_ranges(const uint64_t* keys, int64_t D, int ntiles, uint32_t* 
 //          its argument power * log2(e) is rounded twice) and the product:  rel(alpha) <= (16 + 4 M) U;
 //   T:     a product of n fp32 factors (1 - alpha_i) carries the relative error sum_i [U + delta(alpha_i) / (1 - alpha_i)]
 //          (an alpha clamped to 0.99 on both sides contributes no delta).
+// The flag says WHICH decision can flip, because the three move the pixel by different amounts (reading A38): bit 0 = alpha
+// against 1/255 (one contribution of alpha = 1/255), bit 1 = the stopping rule (the entry that takes T to 1e-4 contributes
+// alpha T with T (1 - alpha) = 1e-4: up to 0.99 / 0.01 * 1e-4 = 9.9e-3), bit 2 = the sign of power (a whole contribution).
 static void blend_pixel(double pxc, double pyc, const uint32_t* list, int64_t n, const float* mu, const float* conic_o,
                         const double* col, const float* bg, double* out3, double* Tout, uint32_t* ncontrib, uint8_t* flag) {
   const double U = 1.1920928955078125e-07;                 // 2^-23
@@ -544,15 +547,15 @@ static void blend_pixel(double pxc, double pyc, const uint32_t* list, int64_t n,
     const float* co = conic_o + 4 * (size_t)g;
     double power = -0.5 * ((double)co[0] * dx * dx + (double)co[2] * dy * dy) - (double)co[1] * dx * dy;
     double M = 0.5 * (std::fabs((double)co[0]) * dx * dx + std::fabs((double)co[2]) * dy * dy) + std::fabs((double)co[1] * dx * dy);
-    if (power != 0.0 && std::fabs(power) <= 8.0 * U * M) fl = 1;
+    if (power != 0.0 && std::fabs(power) <= 8.0 * U * M) fl |= 4;
     if (power > 0.0) continue;
     double raw = (double)co[3] * std::exp(power), rel = (16.0 + 4.0 * M) * U;
     double alpha = std::min(0.99, raw);
-    if (std::fabs(alpha - 1.0 / 255.0) <= rel * alpha) fl = 1;
+    if (std::fabs(alpha - 1.0 / 255.0) <= rel * alpha) fl |= 1;
     if (alpha < 1.0 / 255.0) continue;
     double dalpha = (raw > 0.99 * (1.0 + rel)) ? 0.0 : rel * alpha;       // clamped on both sides: exact
     double testT = T * (1.0 - alpha), eTest = eT + 2.0 * U + dalpha / (1.0 - alpha);
-    if (std::fabs(testT - 1e-4) <= eTest * testT) fl = 1;
+    if (std::fabs(testT - 1e-4) <= eTest * testT) fl |= 2;
     if (testT < 1e-4) break;
     for (int c = 0; c < 3; ++c) C[c] += col[3 * (size_t)g + c] * alpha * T;
     T = testT; eT = eTest; last = cnt;

@@ -3,7 +3,7 @@ inputs and compare every stage.  Integer / index / bit outputs must be identical
 north_star tolerances (max-abs 2e-3, mean-abs 2e-4 on [0,1] values)."""
 import numpy as np
 
-IMG_MAX, IMG_MEAN, FLAG_MAX = 2e-3, 2e-4, 1.0 / 255.0 + 2e-3
+IMG_MAX, IMG_MEAN = 2e-3, 2e-4
 
 
 def run_gpu(inp, vis_mode=0, frame=0, keep_maps=True, use_visibility=True, max_duplicates=0, camera=None):
@@ -156,8 +156,13 @@ def compare_all(inp, av, img, orc_av, o, vis_mode, use_visibility=True, report=N
     T = rd("T_FINAL").reshape(H, W).astype(np.float64)
     dT = np.abs(T - o["T_final"])
     if fl.any():
-        assert d[fl].max() <= FLAG_MAX, "flagged pixels max %g" % d[fl].max()
-        assert dT[fl].max() <= FLAG_MAX, "flagged pixels T_final %g" % dT[fl].max()
+        # what a flipped decision can move (A38): alpha against 1/255 -- one contribution of 1/255; the stopping rule -- the entry
+        # that takes T to 1e-4 weighs alpha T = 1e-4 alpha / (1 - alpha) <= 9.9e-3 (sweep seed 109469: 7.7e-3); the sign of power
+        # -- a whole contribution (not bounded)
+        kind = o["flags"].astype(np.int64)
+        bound = IMG_MAX + np.where(kind & 1, 1.0 / 255.0, 0.0) + np.where(kind & 2, 9.9e-3, 0.0) + np.where(kind & 4, 1.0, 0.0)
+        assert (d[fl] <= bound[fl]).all(), "flagged pixels: image off by %g" % (d[fl] - bound[fl]).max()
+        assert (dT[fl] <= bound[fl]).all(), "flagged pixels: T_final off by %g" % (dT[fl] - bound[fl]).max()
     assert dT[~fl].max() <= IMG_MAX, "T_final"
     nc = rd("N_CONTRIB").reshape(H, W)
     rep["n_contrib_mismatch"] = int((nc != o["n_contrib"])[~fl].sum())

@@ -19,7 +19,8 @@ FLAG_PER_PAIR = 2e-5
 # kernel formed |w_i + w_o|^2 as 2 + 2 w_o.w_i there and lost the half vector to cancellation (6e-3 in the radiance)
 # seeds 54952 and 56494 (an 18,256-seed run on the round's final build, no wrong output): ONE light direction that stands behind
 # every camera-facing Gaussian (nothing for the fused kernel to test: all its words must be 0), and a frame with 3 flagged pixels
-@pytest.mark.parametrize("seed", list(range(24)) + [9489, 54952, 56494])
+# seed 109469 (24,646 more seeds): a pixel whose STOPPING decision can flip (flag bit 1) and does: 7.7e-3, inside what that decision moves
+@pytest.mark.parametrize("seed", list(range(24)) + [9489, 54952, 56494, 109469])
 def test_random_configuration(seed):
     import torch
     from oracle import oracle as orc

@@ -180,14 +180,22 @@ def test_blend_flag_band_is_narrow_and_catches_knife_edges():
     # 4.8e-7 (relative) above the threshold -- inside what two fp32 alphas of 0.9 can move (2 * 16 ulp * 0.9 / 0.1 = 3.4e-5)
     vals, ranges, mu2, co = _stack([0.9, 0.9, 1.0])
     _, T, nc, fl = orc.composite(vals, ranges, mu2, co, np.ones((3, 3)), np.zeros(3, np.float32), 16, 16)
-    assert fl[8, 8] == 1 and nc[8, 8] == 3 and abs(T[8, 8] - 1.0000005e-4) < 1e-10
+    assert fl[8, 8] == 2 and nc[8, 8] == 3 and abs(T[8, 8] - 1.0000005e-4) < 1e-10          # bit 1: the stopping rule
     vals, ranges, mu2, co = _stack([0.9, 0.9, 0.985])                    # T = 1.5e-4: clearly above
     _, T, _, fl = orc.composite(vals, ranges, mu2, co, np.ones((3, 3)), np.zeros(3, np.float32), 16, 16)
     assert fl[8, 8] == 0
+    # the sign of power: a (degenerate) conic a = c = 1, b = -(1 - 2^-24) three pixels off the diagonal: the terms cancel to
+    # -2^-24 * 9 = 6e-8 * M / 2 -- inside 8 U M; with b = -0.99 the sum is decided
+    for b, want in ((-np.float32(1.0 - 2.0 ** -24), 4), (np.float32(-0.99), 0)):
+        vals, ranges, mu2, co = _stack([0.5])
+        mu2 = mu2.copy(); mu2[0] = (8.5 + 3.0, 8.5 + 3.0)
+        co = co.copy(); co[0, :3] = (1.0, b, 1.0)
+        _, _, _, fl = orc.composite(vals, ranges, mu2, co, col, np.zeros(3, np.float32), 16, 16)
+        assert (fl[8, 8] & 4) == want, (b, fl[8, 8])
     # on a real frame the band flags next to nothing (the round-1 band flagged 12 px at config 0 and 0.6 % at config 1)
     inp = workloads.make(0)
     o = orc.render_frame(orc.avatar_load(inp), inp, vis_mode=0)
-    assert o["flags"].mean() <= 1e-3
+    assert (o["flags"] != 0).mean() <= 1e-3
 
 
 # ------------------------------------------------------------------ window (reading A13)
