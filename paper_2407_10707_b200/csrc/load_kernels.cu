@@ -295,7 +295,7 @@ cudaError_t rga_build_knn_grid(rga_avatar* av, const float* aabb_host, cudaStrea
   if ((e = cudaMalloc((void**)&count, (size_t)ncell * 4)) != cudaSuccess) return e;
   if ((e = cudaMalloc((void**)&cursor, (size_t)ncell * 4)) != cudaSuccess) return e;
   if ((e = cudaMalloc((void**)&cell_of, (size_t)av->n_verts * 4)) != cudaSuccess) return e;
-  cudaMemsetAsync(count, 0, (size_t)ncell * 4, s);
+  if ((e = cudaMemsetAsync(count, 0, (size_t)ncell * 4, s)) != cudaSuccess) return e;
   KnnGrid g = {av->grid_o[0], av->grid_o[1], av->grid_o[2], av->grid_h, 1.0f / av->grid_h, G};
   grid_count_kernel<<<(av->n_verts + 255) / 256, 256, 0, s>>>(av->n_verts, g, av->vt_pos, count, cell_of);
   grid_scan_kernel<<<1, 1024, 0, s>>>(ncell, count, av->grid_start, cursor);

@@ -72,6 +72,7 @@ __global__ void __launch_bounds__(256) project_kernel(int ng, CamK cam, const fl
     for (int y = rc.y; y < rc.w; ++y)
       for (int x = rc.x; x < rc.z; ++x) {
         const int tile = y * cam.TX + x;
+        // (whatever subset of the warp happens to be converged here forms the peer sets: the histogram is the same for any grouping)
         const unsigned peers = __match_any_sync(__activemask(), tile);
         if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(tile_count + tile, (unsigned)__popc(peers));
       }
@@ -98,7 +99,8 @@ cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream
     k.C[r] = -abc;
   }
   int grid = (av->n_gauss + 255) / 256;
-  cudaMemsetAsync(av->tile_count, 0, (size_t)k.TX * k.TY * sizeof(unsigned), s);
+  const cudaError_t em = cudaMemsetAsync(av->tile_count, 0, (size_t)k.TX * k.TY * sizeof(unsigned), s);
+  if (em != cudaSuccess) return em;
   project_kernel<<<grid, 256, 0, s>>>(av->n_gauss, k, av->g_posed, av->g_nposed, av->g_cov, av->g_scale_op, av->mu2d,
                                       av->depth, av->conic_o, av->rect, av->touched, av->tile_count);
   av->launches += 1;

@@ -86,6 +86,8 @@ __global__ void __launch_bounds__(256) tile_scatter_kernel(int ng, int TX, long 
     for (int x = r.x; x < r.z; ++x) {
       // lanes of the warp that hit the same tile take consecutive slots from ONE atomic (spatially ordered Gaussians)
       const int tile = y * TX + x;
+      // (correct for ANY converged subset of the warp: each peer set takes its own consecutive slots, and the order inside a bucket
+      // is fixed by the per-tile sort, not here)
       const unsigned peers = __match_any_sync(__activemask(), tile);
       const int leader = __ffs(peers) - 1;
       unsigned base = 0;

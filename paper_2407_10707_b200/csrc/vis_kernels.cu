@@ -369,6 +369,7 @@ __global__ void __launch_bounds__(896, 1) vis_raster_kernel(int nf, int nv, int 
   float* sZ = GTAB ? nullptr : reinterpret_cast<float*>(mp + map_bytes) + nv;      // vertex depths, beside the table in shared memory
   unsigned* svert = reinterpret_cast<unsigned*>(mp + map_bytes) + (GTAB ? 0 : 2 * nv);
   const int nv_words = (nv + 31) >> 5;
+  constexpr bool FUSED_CLEAR = !WITH_ID && !BINNED;   // a depth-only whole map is cleared by the pass that writes it out
 
   // Work slots: units [0, tail_first) one CTA each; the units of the last, partial round of the persistent grid are cut
   // into `split` triangle ranges so that every SM works in that round too; their CTAs merge into the (pre-cleared)
@@ -412,9 +413,9 @@ __global__ void __launch_bounds__(896, 1) vis_raster_kernel(int nf, int nv, int 
         }
       }
     }
-    // clear the band
+    // clear the band (FUSED_CLEAR: only before the CTA's first unit -- the write-out below leaves the map cleared)
     if (WITH_ID) { for (int p = threadIdx.x; p < npix; p += nthreads) sz64[p] = ~0ull; }
-    else {
+    else if (!FUSED_CLEAR || slot == (int)blockIdx.x) {
       uint4* m4 = reinterpret_cast<uint4*>(sz32);
       const uint4 ones = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
       for (int p = threadIdx.x; p < (npix + 3) >> 2; p += nthreads) m4[p] = ones;
@@ -513,6 +514,9 @@ __global__ void __launch_bounds__(896, 1) vis_raster_kernel(int nf, int nv, int 
         }
       }
     }
+    // leftovers: when both queues fit one round, the single-run boxes go through the run dealing too (raster_round builds the
+    // same entry for them) -- one partial round instead of two (the leftovers are a tenth of a unit's time, profiles/r02_raster.md)
+    if (qsn && qn && qsn + qn <= 32) { if (lane < qsn) w->q1[qn + lane] = w->q1s[lane]; qn += qsn; qsn = 0; __syncwarp(); }
     if (qsn) { q2n = raster_single<WITH_ID>(c, w, 0, qsn, lane, q2n); __syncwarp(); }
     if (qn) { q2n = raster_round<WITH_ID>(c, w, 0, qn, lane, q2n); __syncwarp(); }
     if (q2n) raster_depth<WITH_ID>(c, w, 0, q2n, lane);
@@ -552,6 +556,7 @@ __global__ void __launch_bounds__(896, 1) vis_raster_kernel(int nf, int nv, int 
         if (qsb >= 32) { qsb -= 32; q2b = raster_single<WITH_ID>(c, w, qsb, 32, lane, q2b); __syncwarp(); }
         if (qb >= 32) { qb -= 32; q2b = raster_round<WITH_ID>(c, w, qb, 32, lane, q2b); __syncwarp(); }
       }
+      if (qsb && qb && qsb + qb <= 32) { if (lane < qsb) w->q1[qb + lane] = w->q1s[lane]; qb += qsb; qsb = 0; __syncwarp(); }
       if (qsb) { q2b = raster_single<WITH_ID>(c, w, 0, qsb, lane, q2b); __syncwarp(); }
       if (qb) { q2b = raster_round<WITH_ID>(c, w, 0, qb, lane, q2b); __syncwarp(); }
       if (q2b) raster_depth<WITH_ID>(c, w, 0, q2b, lane);
@@ -587,15 +592,22 @@ __global__ void __launch_bounds__(896, 1) vis_raster_kernel(int nf, int nv, int 
         }
       }
     } else if (shared_unit) {
-      for (int p = threadIdx.x; p < npix; p += nthreads) { const unsigned v = sz32[p]; if (v != 0xffffffffu) atomicMin(zmap + gbase + p, v); }
+      for (int p = threadIdx.x; p < npix; p += nthreads) {
+        const unsigned v = sz32[p];
+        if (v != 0xffffffffu) { atomicMin(zmap + gbase + p, v); if (FUSED_CLEAR) sz32[p] = 0xffffffffu; }
+      }
     } else if ((R & 3) == 0) {
-      const uint4* m4 = reinterpret_cast<const uint4*>(sz32);
+      uint4* m4 = reinterpret_cast<uint4*>(sz32);
       uint4* g4 = reinterpret_cast<uint4*>(zmap + gbase);
-      for (int p = threadIdx.x; p < npix >> 2; p += nthreads) g4[p] = m4[p];
+      const uint4 ones = make_uint4(0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu);
+      for (int p = threadIdx.x; p < npix >> 2; p += nthreads) { g4[p] = m4[p]; if (FUSED_CLEAR) m4[p] = ones; }
     } else {
-      for (int p = threadIdx.x; p < npix; p += nthreads) zmap[gbase + p] = sz32[p];
+      for (int p = threadIdx.x; p < npix; p += nthreads) { zmap[gbase + p] = sz32[p]; if (FUSED_CLEAR) sz32[p] = 0xffffffffu; }
     }
-    __syncthreads();                                      // the map and the vertex table are reused by the next band / unit
+    // The map and the vertex table are reused by the next band / unit.  FUSED_CLEAR: every thread has just cleared the texels it
+    // wrote out, and the next unit's head and phase A touch nothing this pass reads (every warp is past the barrier that ends
+    // phase B); the barrier after phase A orders the clearing before the next atomicMin -- one barrier and one pass fewer per unit
+    if (!FUSED_CLEAR) __syncthreads();
     }
   }
 }
@@ -664,7 +676,7 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
   // not faster -- 2,934 against 2,966 frames/s: the streams share the same SMs either way.)
   const int grid_sm = n_units < av->num_sms ? n_units : av->num_sms;
   unsigned* raw = (with_id && p->mode == 1) ? av->vbits_raw : nullptr;
-  if (raw) cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s);
+  if (raw) { const cudaError_t e = cudaMemsetAsync(raw, 0, (size_t)av->n_verts * words * 4, s); if (e != cudaSuccess) return e; }
   // last, partial round of the persistent grid: cut its units into triangle ranges (depth-only maps merge with atomicMin)
   int tail_first = n_units, split = 1;
   const int rem = n_units > grid_sm ? n_units % grid_sm : 0;
@@ -683,7 +695,8 @@ cudaError_t rga_launch_vis_raster(rga_avatar* av, const rga_vis_params* p, cudaS
     const size_t unit_px = (size_t)band_rows * p->res;       // bands are even; the last may be shorter (covered anyway)
     const size_t first_px = binned ? (size_t)tail_first * p->res * p->res      // a binned unit is a whole direction
                                    : (size_t)(tail_first / n_bands) * p->res * p->res + (size_t)(tail_first % n_bands) * unit_px;
-    cudaMemsetAsync(av->zmap + first_px, 0xff, ((size_t)p->n_dirs * p->res * p->res - first_px) * 4, s);
+    const cudaError_t e = cudaMemsetAsync(av->zmap + first_px, 0xff, ((size_t)p->n_dirs * p->res * p->res - first_px) * 4, s);
+    if (e != cudaSuccess) return e;
   }
   const int grid = grid_sm;
   const int band_magic = (65536 + band_rows - 1) / band_rows;   // (row * magic) >> 16 == row / band_rows for row < 256
