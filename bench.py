@@ -60,7 +60,6 @@ KERNELS = {
     "shade":              ("shade", "alu", "(camera-facing Gaussian, upper-hemisphere texel)", 70.0),
     "vis_shade":          ("shade", "alu", "(Gaussian, direction) test + (Gaussian, texel) BRDF", None),
     "project":            ("splat", "hbm", "Gaussian", 56.0 + 64.0),
-    "tile_scan":          ("splat", "hbm", "tile", None),
     "tile_scatter":       ("splat", "hbm", "duplicate", 8.0 + 8.0),
     "tile_sort":          ("splat", "smem", "list entry", None),
     "composite_T":        ("splat", "alu", "(pixel, list entry)", 50.0),

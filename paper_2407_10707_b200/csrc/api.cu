@@ -69,7 +69,7 @@ template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMallo
 
 extern "C" rga_status avatar_free(rga_avatar* av) {
   if (!av) return RGA_OK;
-  void* ptrs[] = {av->vt_quat, av->vt_scale, av->rast_sxy, av->rast_bins, av->frames, av->front_list, av->n_front, av->vs_counter, av->dir_start, av->tex_list, av->tex_dir, av->dir_eps, av->g_order, av->g_inv, av->gi_pos, av->bb_scratch, av->bb_dev, av->vals[1], av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
+  void* ptrs[] = {av->vt_quat, av->vt_scale, av->rast_sxy, av->rast_bins, av->frames, av->front_list, av->n_front, av->vs_counter, av->proj_counter, av->dir_start, av->tex_list, av->tex_dir, av->dir_eps, av->g_order, av->g_inv, av->gi_pos, av->bb_scratch, av->bb_dev, av->vals[1], av->reg_sums, av->loss_maps, av->loss_sums, av->work_counter, av->shade_counter, av->splat_grad, av->dens_dv, av->dens_pfix, av->dens_cdf, av->dens_ng, av->dens_block, av->dens_hdr, av->v_pos, av->v_disp, av->g_pos, av->mlp_bias1, av->vt_pos, av->vt_disp, av->vt_normal, av->vt_albedo, av->vt_rough,
                   av->vt_spec, av->knn_d2, av->grid_start, av->grid_verts, av->v_xbar, av->v_normal, av->v_skin_w, av->faces, av->faces_packed, av->knn_v, av->knn_g, av->ubar_g, av->g_static, av->g_skin_w,
                   av->g_quat, av->g_scale_op, av->v_posed, av->v_nposed, av->g_posed, av->g_nposed, av->g_cov, av->window, av->aabb,
                   av->zmap, av->idmap, av->visbits, av->vbits_a, av->vbits_b, av->vbits_raw, av->vcount, av->env_table,
@@ -145,7 +145,7 @@ extern "C" rga_status avatar_load(const rga_avatar_desc* d, void* stream, rga_av
   A(dalloc(&av->tile_count, ntiles)); A(dalloc(&av->cursor, ntiles));
   A(dalloc(&av->keys[0], (size_t)av->max_dup)); A(dalloc(&av->keys[1], (size_t)av->max_dup));
   A(dalloc(&av->vals[0], (size_t)av->max_dup)); A(dalloc(&av->vals[1], (size_t)av->max_dup));
-  A(dalloc(&av->frames, 4 * (2 + 3 * (size_t)av->max_dirs))); A(dalloc(&av->front_list, ng)); A(dalloc(&av->n_front, 1)); A(dalloc(&av->vs_counter, 1));
+  A(dalloc(&av->frames, 4 * (2 + 3 * (size_t)av->max_dirs))); A(dalloc(&av->front_list, ng)); A(dalloc(&av->n_front, 1)); A(dalloc(&av->vs_counter, 1)); A(dalloc(&av->proj_counter, 1)); A(cudaMemsetAsync(av->proj_counter, 0, sizeof(unsigned), s));
   A(cudaMemsetAsync(av->vs_counter, 0, sizeof(unsigned), s)); A(dalloc(&av->dir_start, (size_t)av->max_dirs + 2)); A(dalloc(&av->tex_list, (size_t)av->max_env + 1)); A(dalloc(&av->tex_dir, (size_t)av->max_env + 1)); A(dalloc(&av->dir_eps, (size_t)av->max_dirs));
   A(dalloc(&av->g_order, ng)); A(dalloc(&av->g_inv, ng)); A(dalloc(&av->gi_pos, 3 * ng)); A(dalloc(&av->bb_scratch, 8)); A(dalloc(&av->bb_dev, 8));
   A(dalloc(&av->num_dup, 1)); A(dalloc(&av->ranges, ntiles));

@@ -3,6 +3,7 @@
 // arithmetic, so the operation order is the one fixed in DESIGN.md "Arithmetic contract".
 // Also accumulates the per-tile histogram (the tile digit of the H8 sort).
 #include "rga_internal.h"
+#include "tile_scan.cuh"
 
 struct CamK {
   float R[9], t[3], fx, fy, cx, cy, znear, limx, limy, C[3];
@@ -12,7 +13,9 @@ struct CamK {
 __global__ void __launch_bounds__(256) project_kernel(int ng, CamK cam, const float4* __restrict__ g_posed,
     const float4* __restrict__ g_nposed, const float* __restrict__ g_cov, const float4* __restrict__ g_scale_op,
     float2* __restrict__ mu2d, float* __restrict__ depth, float4* __restrict__ conic_o, int4* __restrict__ rect,
-    unsigned* __restrict__ touched, unsigned* __restrict__ tile_count) {
+    unsigned* __restrict__ touched, unsigned* tile_count, unsigned* __restrict__ done_counter, int ntiles, long long capacity,
+    uint2* __restrict__ ranges, unsigned* __restrict__ cursor, unsigned* __restrict__ num_dup, unsigned* __restrict__ seg_off,
+    unsigned* __restrict__ num_items, int* __restrict__ status) {
   int g = blockIdx.x * blockDim.x + threadIdx.x;
   unsigned cnt = 0;
   if (g < ng) {
@@ -77,6 +80,19 @@ __global__ void __launch_bounds__(256) project_kernel(int ng, CamK cam, const fl
         if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(tile_count + tile, (unsigned)__popc(peers));
       }
   }
+  // The CTA that finishes the histogram LAST scans it (tile_scan.cuh): ranges, cursors, D, segment offsets.  Every thread's
+  // atomics precede its CTA's arrival (fence, barrier, one atomic on the arrival counter); the last arriver re-arms the counter.
+  __shared__ bool s_last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    s_last = atomicAdd(done_counter, 1u) == gridDim.x - 1u;
+    if (s_last) *done_counter = 0u;
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  rga_tile_scan<256>(ntiles, capacity, tile_count, ranges, cursor, num_dup, seg_off, num_items, status);
 }
 
 cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream_t s) {
@@ -102,7 +118,8 @@ cudaError_t rga_launch_project(rga_avatar* av, const rga_camera* cam, cudaStream
   const cudaError_t em = cudaMemsetAsync(av->tile_count, 0, (size_t)k.TX * k.TY * sizeof(unsigned), s);
   if (em != cudaSuccess) return em;
   project_kernel<<<grid, 256, 0, s>>>(av->n_gauss, k, av->g_posed, av->g_nposed, av->g_cov, av->g_scale_op, av->mu2d,
-                                      av->depth, av->conic_o, av->rect, av->touched, av->tile_count);
+                                      av->depth, av->conic_o, av->rect, av->touched, av->tile_count, av->proj_counter, k.TX * k.TY,
+                                      av->max_dup, av->ranges, av->cursor, av->num_dup, av->seg_off, av->num_items, av->status);
   av->launches += 1;
   rga_prof_mark(av, "project", s);
   return cudaGetLastError();

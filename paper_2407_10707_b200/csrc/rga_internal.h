@@ -90,7 +90,7 @@ struct rga_avatar {
   int disp_is_mlp;             // the current displacement is displacement_mlp's v_disp (else the static vt_disp table)
   float* loss_maps; double* loss_sums;   // image_loss: [max_h][max_w][9] SSIM derivative maps, {sum SSIM, sum |I - J|}
   // fused depth test + shading of rga_render_frame (vis_shade_kernels.cu)
-  float* frames; int* front_list; unsigned* n_front; unsigned* vs_counter; unsigned short* dir_start; unsigned short* tex_list; unsigned short* tex_dir; float* dir_eps;
+  float* frames; int* front_list; unsigned* n_front; unsigned* vs_counter; unsigned* proj_counter; unsigned short* dir_start; unsigned short* tex_list; unsigned short* tex_dir; float* dir_eps;
   int vis_partial; const int* vs_t2d; int vs_rows, vs_cols;   // the frame's visibility words hold only the directions its env map could read
   int* work_counter;           // [1] dynamic work distribution of persistent kernels (zeroed before the launch)
   unsigned* shade_counter;     // [1] group tickets of shade_kernel (zero between launches: the last CTA re-arms it)

@@ -10,66 +10,7 @@
 // Integer-only; D (the number of duplicates) never leaves the device.
 #include "rga_internal.h"
 
-// exclusive scans of the per-tile counts n_t and of the per-tile segment counts ceil(n_t / RGA_SEG) (one CTA, 1024
-// threads): ranges, scatter cursors, D, capacity check; segment offsets and the number of compositing work items
-__global__ void __launch_bounds__(1024) tile_scan_kernel(int ntiles, long long capacity, const unsigned* __restrict__ tile_count,
-    uint2* __restrict__ ranges, unsigned* __restrict__ cursor, unsigned* __restrict__ num_dup, unsigned* __restrict__ seg_off,
-    unsigned* __restrict__ num_items,
-    int* __restrict__ status) {
-  __shared__ unsigned wsum[32], wseg[32];
-  __shared__ unsigned carry, carry_seg;
-  __shared__ unsigned long long total64;                  // D in 64 bits: the 32-bit running sum may wrap before the capacity check
-  if (threadIdx.x == 0) { carry = 0; carry_seg = 0; total64 = 0ull; }
-  __syncthreads();
-  for (int base = 0; base < ntiles; base += 1024) {
-    int i = base + threadIdx.x;
-    unsigned v = (i < ntiles) ? tile_count[i] : 0u, incl = v;
-    unsigned g = (v + RGA_SEG - 1) / RGA_SEG, gincl = g;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      unsigned t = __shfl_up_sync(0xffffffffu, incl, o), tg = __shfl_up_sync(0xffffffffu, gincl, o);
-      if ((threadIdx.x & 31) >= o) { incl += t; gincl += tg; }
-    }
-    {
-      unsigned long long v64 = v;
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v64 += __shfl_xor_sync(0xffffffffu, v64, o);
-      if ((threadIdx.x & 31) == 0 && v64) atomicAdd(&total64, v64);
-    }
-    if ((threadIdx.x & 31) == 31) { wsum[threadIdx.x >> 5] = incl; wseg[threadIdx.x >> 5] = gincl; }
-    __syncthreads();
-    if (threadIdx.x < 32) {
-      unsigned w = wsum[threadIdx.x], wi = w, q = wseg[threadIdx.x], qi = q;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        unsigned t = __shfl_up_sync(0xffffffffu, wi, o), tq = __shfl_up_sync(0xffffffffu, qi, o);
-        if (threadIdx.x >= o) { wi += t; qi += tq; }
-      }
-      wsum[threadIdx.x] = wi - w; wseg[threadIdx.x] = qi - q;
-    }
-    __syncthreads();
-    unsigned excl = carry + wsum[threadIdx.x >> 5] + (incl - v);
-    unsigned gexcl = carry_seg + wseg[threadIdx.x >> 5] + (gincl - g);
-    if (i < ntiles) {
-      ranges[i] = v ? make_uint2(excl, excl + v) : make_uint2(0u, 0u);     // empty tiles report (0,0)
-      cursor[i] = excl;
-      seg_off[i] = gexcl;
-    }
-    __syncthreads();
-    if (threadIdx.x == 1023) { carry = excl + v; carry_seg = gexcl + g; }
-    __syncthreads();
-  }
-  __syncthreads();
-  const bool overflow = total64 > (unsigned long long)capacity;
-  if (overflow)                       // the key buffers cannot hold this frame: report it, render the background only
-    for (int i = threadIdx.x; i < ntiles; i += 1024) { ranges[i] = make_uint2(0u, 0u); seg_off[i] = 0u; }
-  if (threadIdx.x == 0) {
-    if (overflow) atomicExch(status, RGA_ERR_CAPACITY);
-    *num_dup = total64 > 0xffffffffull ? 0xffffffffu : carry;
-    seg_off[ntiles] = overflow ? 0u : carry_seg;
-    *num_items = overflow ? 0u : carry_seg;
-  }
-}
+// (the exclusive scans of the per-tile counts and segment counts: tile_scan.cuh, run by the last CTA of project_kernel)
 
 // scatter: every (Gaussian, tile) duplicate takes the next slot of its tile's bucket; the order inside a bucket is
 // arbitrary here and fixed by the per-tile sort.  local key = depth bits << 32 | Gaussian index (the caller's).
@@ -99,12 +40,9 @@ __global__ void __launch_bounds__(256) tile_scatter_kernel(int ng, int TX, long 
 }
 
 cudaError_t rga_launch_bin(rga_avatar* av, int TX, int ntiles, cudaStream_t s) {
-  tile_scan_kernel<<<1, 1024, 0, s>>>(ntiles, av->max_dup, av->tile_count, av->ranges, av->cursor, av->num_dup, av->seg_off,
-                                      av->num_items, av->status);
-  rga_prof_mark(av, "tile_scan", s);
   tile_scatter_kernel<<<(av->n_gauss + 255) / 256, 256, 0, s>>>(av->n_gauss, TX, av->max_dup, av->touched, av->rect, av->depth,
                                                                av->g_order, av->cursor, av->keys[0]);
   rga_prof_mark(av, "tile_scatter", s);
-  av->launches += 2;
+  av->launches += 1;
   return cudaGetLastError();
 }

@@ -22,7 +22,7 @@ from . import build as _build
 NAMES = [("vis_raster_kernel", "vis_raster"), ("vis_shade_kernel", "vis_shade"), ("vis_depth_test_kernel", "vis_depth_test"),
          ("vis_median_kernel", "vis_median"), ("vis_mean_kernel", "vis_mean"), ("shade_paper_kernel", "shade"), ("shade_kernel", "shade"),
          ("skin_kernel", "skin"), ("front_compact_kernel", "front_compact"), ("texel_csr_kernel", "texel_csr"),
-         ("env_table_kernel", "env_table"), ("project_kernel", "project"), ("tile_scan_kernel", "tile_scan"),
+         ("env_table_kernel", "env_table"), ("project_kernel", "project"),
          ("tile_scatter_kernel", "tile_scatter"), ("tile_sort_kernel", "tile_sort"),
          ("composite_segment_kernel", "composite_segments"), ("composite_resolve_kernel", "composite_resolve"),
          ("composite_replay_kernel", "composite_replay")]
